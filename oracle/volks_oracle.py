@@ -1,0 +1,164 @@
+"""ctypes front end of the float64 CPU oracle (oracle/volks_oracle.c).
+
+TEST INFRASTRUCTURE ONLY: imported by tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs.  It never imports the CUDA package and shares no code,
+table or constant with it.  The arithmetic lives in volks_oracle.c (each function cites the
+PAPER.md passage it follows); this file only marshals numpy arrays and applies the threshold /
+canonical ordering that DESIGN.md readings A3, A4, A9 fix:
+
+  candidate iff snr > snr_thresh (strict; PAPER.md:196 "exceeds the threshold", :208 "SNR > 6"),
+  candidates listed in canonical order (bl, ifq, q, j).
+
+Parity status: every function here is pinned by tests/test_oracle_pins.py (closed forms P1-P14 of
+DESIGN.md) except `window_match`, which is pinned only by hand-built constructions and a second
+brute-force statement of the same rule (the paper gives no worked example) - see DESIGN.md.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "volks_oracle.c")
+_LIB = os.path.join(_HERE, "libvolks_oracle.so")
+
+PEAK_DTYPE = np.dtype(
+    [("p1", "<f8"), ("p2", "<f8"), ("s1", "<f8"), ("snr", "<f8"), ("idx1", "<i8"), ("idx2", "<i8")]
+)
+CAND_DTYPE = np.dtype(
+    [("bl", "<i4"), ("ifq", "<i4"), ("wid", "<i4"), ("win", "<i4"), ("t0", "<i4"),
+     ("rate_idx", "<i4"), ("delay_idx", "<i4"), ("power", "<f8"), ("snr", "<f8")]
+)
+PULSE_DTYPE = np.dtype(
+    [("rep", "<i8"), ("nwidths_hit", "<i4"), ("t_begin", "<i4"), ("t_end", "<i4")]
+)
+
+MODES = {"direct": 0, "fft": 1, "cached": 2}
+
+
+def build(force=False):
+    """Compile the oracle with gcc (building the checker is not using it)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(
+            ["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"]
+        )
+    return _LIB
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        assert lib.vo_sizeof_peak() == PEAK_DTYPE.itemsize
+        lib.vo_window.restype = ctypes.c_int
+        lib.vo_search.restype = ctypes.c_int
+        lib.vo_window_match.restype = ctypes.c_int64
+        _lib = lib
+    return _lib
+
+
+def _as_f32_pairs(a):
+    a = np.ascontiguousarray(a, dtype=np.complex64)
+    return a, a.view(np.float32)
+
+
+def _i32(x):
+    return np.ascontiguousarray(np.asarray(x, dtype=np.int32))
+
+
+def nwin(nap, w, s):
+    return 0 if nap < w else (nap - w) // s + 1
+
+
+def window(win, nt, nf, mode="fft", want_plane=False):
+    """Fringe-search one window.  win: complex [w][nchan].  Returns (peak record, plane|None)."""
+    lib = _load()
+    win, wf = _as_f32_pairs(win)
+    w, nchan = win.shape
+    pk = np.zeros(1, dtype=PEAK_DTYPE)
+    plane = np.zeros((nt, nf), dtype=np.complex128) if want_plane else None
+    rc = lib.vo_window(
+        ctypes.c_int(MODES[mode]), wf.ctypes.data_as(ctypes.c_void_p), ctypes.c_int64(nchan),
+        ctypes.c_int(w), ctypes.c_int(nchan), ctypes.c_int(nt), ctypes.c_int(nf),
+        plane.ctypes.data_as(ctypes.c_void_p) if want_plane else None,
+        pk.ctypes.data_as(ctypes.c_void_p))
+    if rc != 0:
+        raise ValueError("vo_window: bad arguments")
+    return pk[0], plane
+
+
+def search(vis, widths, strides, nts, nf, mode="cached", select=None, nthreads=0):
+    """Peak record of every window (or of the canonical indices in `select`).
+
+    vis: complex64 [nbl][nif][nap][nchan].  Output order: canonical (bl, ifq, q, j).
+    Returns (peaks PEAK_DTYPE[n], threads_used)."""
+    lib = _load()
+    vis, vf = _as_f32_pairs(vis)
+    nbl, nif, nap, nchan = vis.shape
+    widths, strides, nts = _i32(widths), _i32(strides), _i32(nts)
+    per_pair = sum(nwin(nap, int(w), int(s)) for w, s in zip(widths, strides))
+    if select is None:
+        n, sel, selp = nbl * nif * per_pair, None, None
+        nsel = -1
+    else:
+        sel = np.ascontiguousarray(np.asarray(select, dtype=np.int64))
+        n, nsel, selp = sel.size, sel.size, sel.ctypes.data_as(ctypes.c_void_p)
+    out = np.zeros(n, dtype=PEAK_DTYPE)
+    used = lib.vo_search(
+        vf.ctypes.data_as(ctypes.c_void_p), ctypes.c_int(nbl), ctypes.c_int(nif),
+        ctypes.c_int(nap), ctypes.c_int(nchan), ctypes.c_int(len(widths)),
+        widths.ctypes.data_as(ctypes.c_void_p), strides.ctypes.data_as(ctypes.c_void_p),
+        nts.ctypes.data_as(ctypes.c_void_p), ctypes.c_int(nf), ctypes.c_int(MODES[mode]),
+        selp, ctypes.c_int64(nsel), out.ctypes.data_as(ctypes.c_void_p), ctypes.c_int(nthreads))
+    if used < 0:
+        raise ValueError("vo_search: bad arguments")
+    return out, used
+
+
+def canonical_table(nbl, nif, nap, widths, strides):
+    """(bl, ifq, wid, win, t0) int32 arrays for every window in canonical order."""
+    nws = [nwin(nap, int(w), int(s)) for w, s in zip(widths, strides)]
+    wid = np.concatenate([np.full(n, q, np.int32) for q, n in enumerate(nws)]) if nws else np.zeros(0, np.int32)
+    win = np.concatenate([np.arange(n, dtype=np.int32) for n in nws]) if nws else np.zeros(0, np.int32)
+    t0 = win * np.asarray(strides, np.int32)[wid] if wid.size else win
+    per = wid.size
+    pair = np.repeat(np.arange(nbl * nif, dtype=np.int32), per)
+    return (pair // nif, pair % nif, np.tile(wid, nbl * nif), np.tile(win, nbl * nif),
+            np.tile(t0, nbl * nif))
+
+
+def candidates(peaks, nbl, nif, nap, widths, strides, nf, snr_thresh):
+    """Threshold (strict >) the full canonical peak array into the canonical candidate list."""
+    bl, ifq, wid, win, t0 = canonical_table(nbl, nif, nap, widths, strides)
+    keep = np.nonzero(peaks["snr"] > snr_thresh)[0]
+    c = np.zeros(keep.size, dtype=CAND_DTYPE)
+    c["bl"], c["ifq"], c["wid"], c["win"], c["t0"] = bl[keep], ifq[keep], wid[keep], win[keep], t0[keep]
+    c["rate_idx"] = peaks["idx1"][keep] // nf
+    c["delay_idx"] = peaks["idx1"][keep] % nf
+    c["power"] = peaks["p1"][keep]
+    c["snr"] = peaks["snr"][keep]
+    return c, keep
+
+
+def window_match(cands, widths, min_widths=2):
+    """Per-(bl, ifq) multi-window match (A13)."""
+    lib = _load()
+    n = len(cands)
+    out = np.zeros(n, dtype=PULSE_DTYPE)
+    if n == 0:
+        return out
+    bl, ifq, wid, t0 = (_i32(cands[k]) for k in ("bl", "ifq", "wid", "t0"))
+    w = _i32(np.asarray(widths, np.int32)[wid])
+    snr = np.ascontiguousarray(cands["snr"], dtype=np.float64)
+    rep = np.zeros(n, np.int64)
+    nhit, tb, te = np.zeros(n, np.int32), np.zeros(n, np.int32), np.zeros(n, np.int32)
+    p = lambda a: a.ctypes.data_as(ctypes.c_void_p)
+    k = lib.vo_window_match(ctypes.c_int64(n), p(bl), p(ifq), p(wid), p(t0), p(w), p(snr),
+                            ctypes.c_int(min_widths), p(rep), p(nhit), p(tb), p(te))
+    out = out[:k]
+    out["rep"], out["nwidths_hit"], out["t_begin"], out["t_end"] = rep[:k], nhit[:k], tb[:k], te[:k]
+    return out

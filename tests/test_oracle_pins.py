@@ -1,0 +1,313 @@
+"""Pins of the float64 oracle against what the paper and the mathematics fix (P1-P14).
+
+None of these retype the oracle's formula: they are closed forms (Dirichlet kernel, Parseval),
+invariances, brute force in a second language (numpy einsum), a library special case
+(numpy.fft) and the statistics of the noise.  CPU only."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import workloads
+
+TWO_PI = 2 * math.pi
+
+
+def fringe(w, nchan, tau_c, rho_c, a=1.0, phi0=0.3):
+    t = np.arange(w)[:, None]
+    k = np.arange(nchan)[None, :]
+    return (a * np.exp(1j * (TWO_PI * (tau_c * k + rho_c * t) + phi0))).astype(np.complex64)
+
+
+def dirichlet(M, x):
+    x = np.asarray(x, dtype=np.float64)
+    num, den = np.sin(np.pi * M * x), np.sin(np.pi * x)
+    out = np.full(x.shape, float(M))
+    ok = np.abs(den) > 1e-12
+    out[ok] = num[ok] / den[ok]
+    return np.abs(out)
+
+
+@pytest.mark.parametrize("mode", ["direct", "fft"])
+@pytest.mark.parametrize("w,nchan,nt,nf,tau,rho", [(8, 32, 16, 64, 5, 2), (4, 16, 8, 64, 15, 3), (16, 8, 16, 8, 7, 15)])
+def test_p1_on_bin_fringe_closed_form(oracle, mode, w, nchan, nt, nf, tau, rho):
+    """P1: V = a e^{+i(2pi(tau k/nchan + rho t/w)+phi0)} peaks exactly at (rho Nt/w, tau Nf/nchan),
+    P1 = (a w nchan)^2, S1 = Nt Nf a^2 w nchan, snr = sqrt(w nchan).  Pins the e^{-i Phi} sign of
+    PAPER.md:74-79, the index mapping, the scaling and the SNR reading A3."""
+    a = 0.7
+    win = fringe(w, nchan, tau / nchan, rho / w, a=a)
+    pk, _ = oracle.window(win, nt, nf, mode=mode)
+    assert pk["idx1"] == (rho * nt // w) * nf + tau * nf // nchan
+    assert pk["p1"] == pytest.approx((a * w * nchan) ** 2, rel=1e-6)   # inputs are float32
+    assert pk["s1"] == pytest.approx(nt * nf * a * a * w * nchan, rel=1e-6)
+    assert pk["snr"] == pytest.approx(math.sqrt(w * nchan), rel=1e-6)
+
+
+def test_p1_negative_sign_would_fail(oracle):
+    """A conjugated kernel (wrong sign) would put the peak at the mirrored bin."""
+    win = fringe(8, 32, 5 / 32, 2 / 8)
+    pk, _ = oracle.window(win, 16, 64)
+    assert pk["idx1"] == 4 * 64 + 10 and pk["idx1"] != (16 - 4) * 64 + (64 - 10)
+
+
+@pytest.mark.parametrize("mode", ["direct", "fft"])
+def test_p2_parseval(oracle, mode):
+    rng = np.random.default_rng(5)
+    for (w, nchan, nt, nf) in [(3, 5, 8, 8), (8, 32, 16, 64), (7, 20, 32, 32)]:
+        win = (rng.normal(size=(w, nchan)) + 1j * rng.normal(size=(w, nchan))).astype(np.complex64)
+        pk, _ = oracle.window(win, nt, nf, mode=mode)
+        e = float(np.sum(np.abs(win.astype(np.complex128)) ** 2))
+        assert pk["s1"] == pytest.approx(nt * nf * e, rel=1e-9)
+
+
+def brute_plane(win, nt, nf):
+    """Second statement of the definition (numpy einsum over explicit DFT matrices)."""
+    w, nchan = win.shape
+    Et = np.exp(-1j * TWO_PI * np.outer(np.arange(nt), np.arange(w)) / nt)
+    Ef = np.exp(-1j * TWO_PI * np.outer(np.arange(nchan), np.arange(nf)) / nf)
+    return Et @ win.astype(np.complex128) @ Ef
+
+
+def test_p3_brute_force_random_planes(oracle):
+    rng = np.random.default_rng(11)
+    for (w, nchan, nt, nf) in [(2, 3, 4, 4), (4, 4, 4, 4), (5, 9, 8, 16), (8, 32, 16, 64), (16, 33, 16, 64)]:
+        win = (rng.normal(size=(w, nchan)) + 1j * rng.normal(size=(w, nchan))).astype(np.complex64)
+        ref = brute_plane(win, nt, nf)
+        for mode in ("direct", "fft"):
+            pk, plane = oracle.window(win, nt, nf, mode=mode, want_plane=True)
+            assert np.max(np.abs(plane - ref)) <= 1e-12 * np.max(np.abs(ref)) * nt * nf
+            P = np.abs(ref) ** 2
+            assert pk["idx1"] == int(np.argmax(P))
+            assert pk["p1"] == pytest.approx(P.max(), rel=1e-12)
+
+
+def test_p3_config0_all_windows_three_modes(oracle):
+    vis, c, _ = workloads.generate(0)
+    v = vis.numpy()
+    args = (v, c["widths"], c["strides"], c["nts"], c["nf"])
+    d, _ = oracle.search(*args, mode="direct")
+    f, _ = oracle.search(*args, mode="fft")
+    k, _ = oracle.search(*args, mode="cached")
+    assert len(d) == 505
+    for other in (f, k):
+        assert np.array_equal(d["idx1"], other["idx1"])
+        assert np.allclose(d["p1"], other["p1"], rtol=1e-12)
+        assert np.allclose(d["s1"], other["s1"], rtol=1e-12)
+        assert np.allclose(d["p2"], other["p2"], rtol=1e-12)
+
+
+def test_cached_equals_fft_config1_and_selection(oracle):
+    vis, c, _ = workloads.generate(1, nap=300)
+    v = vis.numpy()
+    args = (v, c["widths"], c["strides"], c["nts"], c["nf"])
+    f, _ = oracle.search(*args, mode="fft")
+    k, _ = oracle.search(*args, mode="cached")
+    assert np.array_equal(f["idx1"], k["idx1"]) and np.array_equal(f["idx2"], k["idx2"])
+    assert np.allclose(f["p1"], k["p1"], rtol=1e-12) and np.allclose(f["snr"], k["snr"], rtol=1e-12)
+    sel = np.array([0, 5, len(f) - 1, len(f) // 2, 17])
+    s, _ = oracle.search(*args, mode="fft", select=sel)
+    assert np.array_equal(s["idx1"], f["idx1"][sel]) and np.allclose(s["p1"], f["p1"][sel], rtol=1e-13)
+
+
+def test_p4_paper_1d_scheme_is_rate_zero_row(oracle):
+    """PAPER.md:133 + 143: FFT each AP along frequency, then sum the window's APs == row r=0."""
+    rng = np.random.default_rng(3)
+    w, nchan, nt, nf = 8, 32, 16, 128
+    win = (rng.normal(size=(w, nchan)) + 1j * rng.normal(size=(w, nchan))).astype(np.complex64)
+    _, plane = oracle.window(win, nt, nf, want_plane=True)
+    per_ap = np.fft.fft(win.astype(np.complex128), n=nf, axis=1)
+    assert np.allclose(plane[0], per_ap.sum(axis=0), rtol=0, atol=1e-10)
+    assert np.allclose(plane[0], np.fft.fft(win.astype(np.complex128).sum(axis=0), n=nf), atol=1e-10)
+
+
+def test_p5_off_bin_fringe_dirichlet(oracle):
+    w, nchan, nt, nf, a = 8, 32, 16, 64, 0.9
+    tau_c, rho_c = 0.1234, -0.3171
+    win64 = a * np.exp(1j * (TWO_PI * (tau_c * np.arange(nchan)[None, :] + rho_c * np.arange(w)[:, None]) + 0.4))
+    win = win64.astype(np.complex64)
+    _, plane = oracle.window(win, nt, nf, want_plane=True)
+    r = np.arange(nt)[:, None] / nt
+    d = np.arange(nf)[None, :] / nf
+    expect = a * dirichlet(w, r - rho_c) * dirichlet(nchan, d - tau_c)
+    assert np.max(np.abs(np.abs(plane) - expect)) < 2e-5 * a * w * nchan   # float32 input rounding
+
+
+def test_p6_delta_input(oracle):
+    win = np.zeros((8, 32), np.complex64)
+    win[3, 7] = 2 - 1j
+    for mode in ("direct", "fft"):
+        pk, _ = oracle.window(win, 16, 64, mode=mode)
+        assert pk["p1"] == pytest.approx(5.0, rel=1e-12) and pk["snr"] == pytest.approx(1.0, rel=1e-12)
+    pk, _ = oracle.window(np.array([[1 + 0j]], np.complex64), 4, 8)
+    assert pk["idx1"] == 0 and pk["idx2"] == 1 and pk["p1"] == pk["p2"] == 1.0
+
+
+def test_p6_all_zero_window(oracle):
+    pk, _ = oracle.window(np.zeros((4, 8), np.complex64), 8, 16)
+    assert pk["p1"] == 0.0 and pk["snr"] == 0.0 and pk["idx1"] == 0
+
+
+def test_p7_width_one(oracle):
+    rng = np.random.default_rng(9)
+    row = (rng.normal(size=(1, 32)) + 1j * rng.normal(size=(1, 32))).astype(np.complex64)
+    pk, plane = oracle.window(row, 2, 128, want_plane=True)
+    spec = np.abs(np.fft.fft(row[0].astype(np.complex128), n=128)) ** 2
+    assert np.allclose(np.abs(plane[0]) ** 2, spec) and np.allclose(np.abs(plane[1]) ** 2, spec)
+    assert pk["idx1"] == int(np.argmax(spec))          # r* = 0 (first of the tied rows)
+    assert pk["idx1"] < 128 and pk["idx2"] == pk["idx1"] + 128
+
+
+def test_p8_scaling_and_phase_invariance(oracle):
+    vis, c, _ = workloads.generate(0)
+    v = vis.numpy()[:, :, :64]
+    args = (c["widths"], c["strides"], c["nts"], c["nf"])
+    a, _ = oracle.search(v, *args, mode="fft")
+    b, _ = oracle.search((v * np.complex64(2j)).astype(np.complex64), *args, mode="fft")
+    assert np.array_equal(a["idx1"], b["idx1"])
+    assert np.allclose(b["p1"], 4 * a["p1"], rtol=1e-12) and np.allclose(a["snr"], b["snr"], rtol=1e-12)
+
+
+def test_p9_shift_invariance(oracle):
+    vis, c, _ = workloads.generate(1, nap=200)
+    v = vis.numpy()
+    q = 2
+    w, s, nt = c["widths"][q], c["strides"][q], c["nts"][q]
+    m = 3
+    a, _ = oracle.search(v, [w], [s], [nt], c["nf"], mode="fft")
+    b, _ = oracle.search(np.ascontiguousarray(v[:, :, m * s:]), [w], [s], [nt], c["nf"], mode="fft")
+    na, nb = workloads.gen.nwin(200, w, s), workloads.gen.nwin(200 - m * s, w, s)
+    A, Bv = a.reshape(8, na), b.reshape(8, nb)
+    assert np.array_equal(A["idx1"][:, m:], Bv["idx1"]) and np.array_equal(A["p1"][:, m:], Bv["p1"])
+
+
+def test_p10_padding_consistency(oracle):
+    rng = np.random.default_rng(21)
+    w, nchan = 8, 16
+    win = (rng.normal(size=(w, nchan)) + 1j * rng.normal(size=(w, nchan))).astype(np.complex64)
+    _, small = oracle.window(win, 8, 16, want_plane=True)
+    _, big = oracle.window(win, 32, 64, want_plane=True)
+    assert np.allclose(big[::4, ::4], small, atol=1e-11)
+
+
+def test_p11_width_doubling_identity(oracle):
+    rng = np.random.default_rng(22)
+    w, nchan, nf = 4, 16, 32
+    x = (rng.normal(size=(2 * w, nchan)) + 1j * rng.normal(size=(2 * w, nchan))).astype(np.complex64)
+    _, f1 = oracle.window(x[:w], 2 * w, nf, want_plane=True)
+    _, f2 = oracle.window(x[w:], 2 * w, nf, want_plane=True)
+    _, fb = oracle.window(x, 4 * w, nf, want_plane=True)
+    sign = ((-1.0) ** np.arange(2 * w))[:, None]
+    assert np.allclose(fb[::2], f1 + sign * f2, atol=1e-11)
+
+
+def test_p12_numpy_fft2_special_case(oracle):
+    rng = np.random.default_rng(23)
+    for (w, nchan, nt, nf) in [(8, 32, 16, 64), (32, 64, 64, 128), (64, 128, 128, 256)]:
+        win = (rng.normal(size=(w, nchan)) + 1j * rng.normal(size=(w, nchan))).astype(np.complex64)
+        pk, plane = oracle.window(win, nt, nf, want_plane=True)
+        ref = np.fft.fft2(win.astype(np.complex128), s=(nt, nf))
+        assert np.max(np.abs(plane - ref)) < 1e-10 * np.max(np.abs(ref))
+        assert pk["idx1"] == int(np.argmax(np.abs(ref) ** 2))
+
+
+def test_p13_noise_statistics(oracle):
+    vis, c, _ = workloads.generate(0, npulses=0)
+    pk, _ = oracle.search(vis.numpy(), [8], [8], [8], 32, mode="fft")     # unpadded, disjoint
+    noise = pk["s1"] / (8 * 32)
+    assert np.mean(noise) == pytest.approx(8 * 32, rel=0.05)
+    emax = np.mean(pk["p1"] / noise)
+    assert emax == pytest.approx(math.log(8 * 32) + 0.5772, rel=0.2)
+
+
+def test_p14_config0_expectation(oracle):
+    exp = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "config0_expectation.txt")) as f:
+        for line in f:
+            if not line.startswith("#"):
+                k, v = line.split()
+                exp[k] = float(v)
+    vis, c, _ = workloads.generate(0)
+    pk, _ = oracle.search(vis.numpy(), c["widths"], c["strides"], c["nts"], c["nf"], mode="cached")
+    j = int(exp["t0"])
+    assert pk["idx1"][j] == int(exp["rate_idx"]) * c["nf"] + int(exp["delay_idx"])
+    assert pk["p1"][j] == pytest.approx(exp["signal_power"] + exp["noise_mean"], rel=0.35)
+    assert pk["snr"][j] > exp["snr_thresh"]
+    cands, keep = oracle.candidates(pk, 1, 1, c["nap"], c["widths"], c["strides"], c["nf"], exp["snr_thresh"])
+    assert len(cands) >= 1 and np.all(np.abs(cands["t0"] - 200) <= 3)     # no noise-only candidate
+    assert np.all(cands["rate_idx"] == 4) and np.all(cands["delay_idx"] == 10)
+    assert list(cands["win"]) == sorted(cands["win"])
+
+
+def test_candidates_canonical_order_and_strict_threshold(oracle):
+    vis, c, _ = workloads.generate(1, nap=400)
+    pk, _ = oracle.search(vis.numpy(), c["widths"], c["strides"], c["nts"], c["nf"], mode="cached")
+    thr = float(np.sort(pk["snr"])[-20])
+    cands, keep = oracle.candidates(pk, 1, 8, 400, c["widths"], c["strides"], c["nf"], thr)
+    assert len(cands) == 19                                   # strict >: the 20th is excluded
+    key = list(zip(cands["bl"], cands["ifq"], cands["wid"], cands["win"]))
+    assert key == sorted(key)
+    assert np.all(cands["t0"] == cands["win"] * np.asarray(c["strides"])[cands["wid"]])
+
+
+# ---- a8 window match: constructions + a second brute-force statement of the rule ----
+
+def _cands(oracle, rows):
+    c = np.zeros(len(rows), dtype=oracle.CAND_DTYPE)
+    for i, (bl, ifq, wid, win, t0, snr) in enumerate(rows):
+        c[i]["bl"], c[i]["ifq"], c[i]["wid"], c[i]["win"], c[i]["t0"], c[i]["snr"] = bl, ifq, wid, win, t0, snr
+    return c
+
+
+def test_window_match_constructions(oracle):
+    widths = [4, 8, 16]
+    # two widths overlapping -> kept, representative = max snr
+    p = oracle.window_match(_cands(oracle, [(0, 0, 0, 10, 10, 7.0), (0, 0, 1, 1, 8, 9.0)]), widths)
+    assert len(p) == 1 and p[0]["rep"] == 1 and p[0]["nwidths_hit"] == 2 and (p[0]["t_begin"], p[0]["t_end"]) == (8, 16)
+    # one width twice -> dropped
+    assert len(oracle.window_match(_cands(oracle, [(0, 0, 0, 10, 10, 7.0), (0, 0, 0, 11, 11, 9.0)]), widths)) == 0
+    # chain A-B-C: A and C do not overlap but both overlap B -> one cluster
+    p = oracle.window_match(_cands(oracle, [(0, 0, 0, 0, 0, 7.0), (0, 0, 1, 0, 3, 6.5), (0, 0, 0, 2, 10, 8.0)]), widths)
+    assert len(p) == 1 and p[0]["rep"] == 2 and (p[0]["t_begin"], p[0]["t_end"]) == (0, 14)
+    # touching intervals [0,4) and [4,12) do not overlap
+    assert len(oracle.window_match(_cands(oracle, [(0, 0, 0, 0, 0, 7.0), (0, 0, 1, 0, 4, 7.0)]), widths)) == 0
+    # different IF or baseline never match
+    assert len(oracle.window_match(_cands(oracle, [(0, 0, 0, 0, 0, 7.0), (0, 1, 1, 0, 0, 7.0)]), widths)) == 0
+    assert len(oracle.window_match(_cands(oracle, [(0, 0, 0, 0, 0, 7.0), (1, 0, 1, 0, 0, 7.0)]), widths)) == 0
+    # snr tie -> lowest canonical position
+    p = oracle.window_match(_cands(oracle, [(0, 0, 0, 0, 0, 7.0), (0, 0, 1, 0, 0, 7.0)]), widths)
+    assert p[0]["rep"] == 0
+
+
+def test_window_match_vs_python_graph_search(oracle):
+    rng = np.random.default_rng(4)
+    widths = [2, 4, 8, 16]
+    rows = []
+    for _ in range(120):
+        wid = int(rng.integers(0, 4))
+        rows.append((int(rng.integers(0, 2)), int(rng.integers(0, 2)), wid, 0, int(rng.integers(0, 300)), float(rng.uniform(6, 20))))
+    rows.sort(key=lambda r: (r[0], r[1], r[2], r[4]))
+    c = _cands(oracle, rows)
+    got = oracle.window_match(c, widths, 2)
+    # flood fill on the explicit overlap graph
+    n = len(rows)
+    iv = [(r[4], r[4] + widths[r[2]]) for r in rows]
+    adj = [[k for k in range(n) if k != i and rows[i][:2] == rows[k][:2] and iv[i][0] < iv[k][1] and iv[k][0] < iv[i][1]] for i in range(n)]
+    seen, expect = set(), []
+    for i in range(n):
+        if i in seen:
+            continue
+        comp, stack = [], [i]
+        seen.add(i)
+        while stack:
+            x = stack.pop()
+            comp.append(x)
+            for y in adj[x]:
+                if y not in seen:
+                    seen.add(y)
+                    stack.append(y)
+        if len({rows[x][2] for x in comp}) >= 2:
+            best = max(sorted(comp), key=lambda x: (rows[x][5], -x))
+            expect.append((best, len({rows[x][2] for x in comp}), min(iv[x][0] for x in comp), max(iv[x][1] for x in comp)))
+    expect.sort()
+    assert [(int(p["rep"]), int(p["nwidths_hit"]), int(p["t_begin"]), int(p["t_end"])) for p in got] == expect
