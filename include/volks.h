@@ -1,0 +1,136 @@
+/*
+ * volks.h - C-ABI of the B200-native cross-spectrum fringe search (libvolks_b200.so).
+ *
+ * The hot path of the VOLKS2 single-pulse search (arXiv 2108.05602; PAPER.md = the paper text):
+ * for every baseline, IF, window width and sliding window position, the window of complex
+ * visibilities [w x nchan] is zero-padded to [Nt x Nf] and 2-D DFT'd (frequency -> delay, time ->
+ * fringe rate), |.|^2 is taken, the peak and a noise statistic are found, an SNR is formed, and
+ * the windows above threshold are compacted into an ordered candidate list.
+ *
+ *   - transform and its sign:  G = sum S e^{-i Phi}, Phi = 2 pi f dtau        PAPER.md:74-79 (Eq. 1)
+ *   - FFT search with zero padding; the 2-D (delay x rate) geodetic scheme
+ *   - step 5 "for each AP, FFT along the frequency axis"
+ *   - step 6 "combine the FFTed APs along the time axis ... find the maximum" PAPER.md:143
+ *   - windows of several sizes per baseline
+ *   - "selected if its normalized power exceeds the threshold"; "SNR > 6"
+ *   - "a single pulse is selected if it appears in at least 2 windows"
+ *
+ * Definition (DESIGN.md section "Path"): for window (bl, ifq, q, j), t0 = j*stride[q],
+ *   F[r][d] = sum_{t<w_q} sum_{k<nchan} vis[bl][ifq][t0+t][k] exp(-2 pi i (r t/Nt_q + d k/Nf))
+ *   P = |F|^2, P1 = max P, (r*, d*) = first argmax in row-major order (r major, d minor),
+ *   noise = mean of P over the whole padded plane, snr = sqrt(P1/noise) (0 if noise == 0),
+ *   candidate iff snr > snr_thresh (strict).
+ *
+ * All compute runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.  Plain pointers
+ * and sizes only: every pointer below is marked HOST or DEVICE.  The caller owns every buffer;
+ * volks_fringe_search never allocates.  The plan owns small device tables (twiddles, the width
+ * schedule) allocated in volks_plan_create and freed in volks_plan_destroy.
+ *
+ * Errors: every int-returning call gives 0 (VOLKS_OK) or a negative code; nothing throws, exits or
+ * prints.  Non-finite visibilities are a precondition violation (results unspecified, no crash).
+ * Determinism: identical inputs give bit-identical outputs run to run (the peak reduction is an
+ * order-independent max over a total order; the compaction is an ordered scan).
+ */
+#ifndef VOLKS_H
+#define VOLKS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define VOLKS_OK 0
+#define VOLKS_EINVAL (-1)    /* bad dims, non-power-of-two pad, nt<w, nf<nchan, null pointer      */
+#define VOLKS_ECUDA (-2)     /* CUDA allocation / launch failure (sticky error text: strerror)   */
+#define VOLKS_ENOMEM (-3)    /* host allocation failure                                           */
+#define VOLKS_EOVERFLOW (-4) /* returned by volks_window_match when capacity < number of pulses   */
+
+#define VOLKS_MAX_WIDTHS 16
+
+/* Search parameters.  HOST memory, copied by volks_plan_create (arrays need not outlive it). */
+typedef struct {
+  int32_t nbl, nif, nap, nchan; /* vis is cf32[nbl][nif][nap][nchan], channel fastest, DEVICE      */
+  int32_t nwidths;              /* 1..VOLKS_MAX_WIDTHS                                             */
+  const int32_t *width;         /* HOST [nwidths] w_q >= 1 APs                  */
+  const int32_t *stride;        /* HOST [nwidths] s_q >= 1 APs; partial windows are dropped        */
+  const int32_t *nt;            /* HOST [nwidths] padded time size: power of two, >= w_q           */
+  int32_t nf;                   /* padded frequency size: power of two, >= nchan     */
+  float snr_thresh;             /* candidate iff snr > snr_thresh              */
+} volks_params;
+
+/* One candidate = one window above threshold.  36 bytes, no padding. */
+typedef struct {
+  int32_t bl, ifq, wid, win, t0; /* wid = width index q; win = ordinal j; t0 = j*stride[q]         */
+  int32_t rate_idx, delay_idx;   /* raw FFT bins r* in [0,Nt_q), d* in [0,Nf); upper half negative */
+  float power, snr;              /* P1 and sqrt(P1/noise)                                          */
+} volks_cand;
+
+/* Dense per-window peak (optional output).  16 bytes. */
+typedef struct {
+  float power, snr;
+  int32_t rate_idx, delay_idx;
+} volks_peak;
+
+/* One matched pulse of volks_window_match. */
+typedef struct {
+  volks_cand best;     /* max-snr member of the cluster (ties: first in canonical order)          */
+  int32_t nwidths_hit; /* distinct width indices in the cluster                                    */
+  int32_t t_begin, t_end; /* union AP extent [t_begin, t_end) of the cluster                       */
+} volks_pulse;
+
+typedef struct volks_plan volks_plan; /* opaque */
+
+/* Validate `p` (HOST), build the window schedule (per width: window count, kernel variant, grid
+ * shape, canonical offsets) and upload the twiddle tables.  Uses the current CUDA device.
+ * nap < w_q gives zero windows for that width, not an error.  *out receives the plan. */
+int volks_plan_create(const volks_params *p, volks_plan **out);
+int volks_plan_destroy(volks_plan *plan);
+
+/* Sizes the caller needs.  All outputs HOST, each nullable.  nwin_per_width[q] counts windows of
+ * ONE (bl, ifq) pair: floor((nap-w_q)/s_q)+1; nwin_total = nbl*nif*sum_q nwin_per_width[q]. */
+int volks_plan_query(const volks_plan *plan, size_t *workspace_bytes, int64_t *nwin_per_width,
+                     int64_t *nwin_total);
+
+/* The hot path.  Asynchronous: every kernel is enqueued on `cuda_stream` (a cudaStream_t; NULL =
+ * legacy default stream); results are valid after the stream is synchronised.
+ *   d_vis        DEVICE cf32[nbl][nif][nap][nchan], read-only, 8-byte aligned
+ *   d_workspace  DEVICE scratch of >= workspace_bytes (256-byte aligned); contents undefined after
+ *   d_peaks      DEVICE volks_peak[nwin_total] or NULL.  Dense layout:
+ *                d_peaks[off_q + (bl*nif + ifq)*nwin_q + j], off_q = nbl*nif*sum_{q'<q} nwin_q'
+ *   d_cands      DEVICE volks_cand[cand_capacity]; candidates in canonical order (bl, ifq, q, j)
+ *   d_ncand      DEVICE uint32: the TRUE total number of candidates; if it exceeds cand_capacity
+ *                only the first cand_capacity candidates (canonical order) were written
+ * Returns VOLKS_OK, VOLKS_EINVAL (null plan/vis/workspace/ncand, or null d_cands with capacity>0)
+ * or VOLKS_ECUDA (a launch failed). */
+int volks_fringe_search(const volks_plan *plan, const void *d_vis, void *d_workspace,
+                        volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity,
+                        uint32_t *d_ncand, void *cuda_stream);
+
+/* Per-baseline multi-window match (reading A13).  HOST call on HOST
+ * arrays (integer work on a list of at most a few thousand records).  Within one (bl, ifq),
+ * candidates whose AP intervals [t0, t0+width[wid]) overlap are linked; connected components are
+ * clusters; a cluster with >= min_widths distinct width indices gives one volks_pulse.  Output is
+ * ordered by the canonical position of `best`.  `cands` must be in canonical order; `width` is
+ * the HOST [nwidths] width table the candidates' `wid` fields index (needs no plan and no GPU).
+ * *nout receives the number of pulses found; returns VOLKS_EOVERFLOW if it exceeds `capacity`
+ * (the first `capacity` are written). */
+int volks_window_match(const volks_cand *cands, uint32_t ncand, const int32_t *width, int32_t nwidths,
+                       int32_t min_widths, volks_pulse *out, uint32_t capacity, uint32_t *nout);
+
+/* HOST helper: signed physical units from raw bins (upper half of each axis is negative):
+ * rate_hz = r_signed/(nt*ap_seconds), delay_s = d_signed/(nf*chan_hz); nt = Nt_q of the width. */
+int volks_bin_to_physical(int32_t nt, int32_t nf, int32_t rate_idx, int32_t delay_idx,
+                          double ap_seconds, double chan_hz, double *rate_hz, double *delay_s);
+
+/* Number of kernels one volks_fringe_search enqueues (for launch accounting). */
+int volks_plan_launch_count(const volks_plan *plan);
+
+const char *volks_strerror(int code);
+int volks_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VOLKS_H */

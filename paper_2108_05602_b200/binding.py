@@ -1,0 +1,173 @@
+"""Thin ctypes binding of libvolks_b200.so (include/volks.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels.  torch is used for device memory and
+streams.  There is no CPU fallback: if the shared library is missing this module raises."""
+import ctypes
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libvolks_b200.so")
+
+VOLKS_OK, VOLKS_EINVAL, VOLKS_ECUDA, VOLKS_ENOMEM, VOLKS_EOVERFLOW = 0, -1, -2, -3, -4
+
+EXPORTS = (
+    "volks_plan_create", "volks_plan_destroy", "volks_plan_query", "volks_fringe_search",
+    "volks_window_match", "volks_bin_to_physical", "volks_plan_launch_count", "volks_strerror",
+    "volks_version",
+)
+
+
+class volks_params(ctypes.Structure):
+    _fields_ = [("nbl", ctypes.c_int32), ("nif", ctypes.c_int32), ("nap", ctypes.c_int32),
+                ("nchan", ctypes.c_int32), ("nwidths", ctypes.c_int32),
+                ("width", ctypes.POINTER(ctypes.c_int32)), ("stride", ctypes.POINTER(ctypes.c_int32)),
+                ("nt", ctypes.POINTER(ctypes.c_int32)), ("nf", ctypes.c_int32),
+                ("snr_thresh", ctypes.c_float)]
+
+
+CAND_DTYPE = np.dtype([("bl", "<i4"), ("ifq", "<i4"), ("wid", "<i4"), ("win", "<i4"), ("t0", "<i4"),
+                       ("rate_idx", "<i4"), ("delay_idx", "<i4"), ("power", "<f4"), ("snr", "<f4")])
+PEAK_DTYPE = np.dtype([("power", "<f4"), ("snr", "<f4"), ("rate_idx", "<i4"), ("delay_idx", "<i4")])
+PULSE_DTYPE = np.dtype([("best", CAND_DTYPE), ("nwidths_hit", "<i4"), ("t_begin", "<i4"), ("t_end", "<i4")])
+assert CAND_DTYPE.itemsize == 36 and PEAK_DTYPE.itemsize == 16 and PULSE_DTYPE.itemsize == 48
+
+_lib = None
+
+
+def lib():
+    """Load the C-ABI library; fails loudly if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(
+                "libvolks_b200.so is missing: run `python -m paper_2108_05602_b200.build` "
+                "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        L.volks_strerror.restype = ctypes.c_char_p
+        L.volks_strerror.argtypes = [ctypes.c_int]
+        L.volks_plan_create.argtypes = [ctypes.POINTER(volks_params), ctypes.POINTER(ctypes.c_void_p)]
+        L.volks_plan_destroy.argtypes = [ctypes.c_void_p]
+        L.volks_plan_query.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_size_t),
+                                       ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
+        L.volks_fringe_search.argtypes = [ctypes.c_void_p] * 5 + [ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
+        L.volks_window_match.argtypes = [ctypes.c_void_p, ctypes.c_uint32, ctypes.c_void_p, ctypes.c_int32,
+                                         ctypes.c_int32, ctypes.c_void_p, ctypes.c_uint32,
+                                         ctypes.POINTER(ctypes.c_uint32)]
+        L.volks_bin_to_physical.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
+                                            ctypes.c_double, ctypes.c_double,
+                                            ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+        L.volks_plan_launch_count.argtypes = [ctypes.c_void_p]
+        _lib = L
+    return _lib
+
+
+class VolksError(RuntimeError):
+    def __init__(self, code):
+        self.code = code
+        super().__init__("volks error %d: %s" % (code, lib().volks_strerror(code).decode()))
+
+
+def _check(rc):
+    if rc != VOLKS_OK:
+        raise VolksError(rc)
+
+
+def plan_create_raw(nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh):
+    """volks_plan_create; returns (rc, handle) without raising (for error-path tests)."""
+    n = len(widths)
+    arr = lambda v: (ctypes.c_int32 * max(len(v), 1))(*[int(x) for x in v])
+    w, s, t = arr(widths), arr(strides), arr(nts)
+    p = volks_params(nbl, nif, nap, nchan, n, w, s, t, nf, float(snr_thresh))
+    h = ctypes.c_void_p()
+    rc = lib().volks_plan_create(ctypes.byref(p), ctypes.byref(h))
+    return rc, h
+
+
+class Plan:
+    """volks_plan_* : validated parameters + window schedule + device tables."""
+
+    def __init__(self, nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh):
+        self.shape = (nbl, nif, nap, nchan)
+        self.widths, self.strides, self.nts, self.nf = list(widths), list(strides), list(nts), nf
+        self.snr_thresh = float(snr_thresh)
+        rc, self._h = plan_create_raw(nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh)
+        _check(rc)
+        ws, tot = ctypes.c_size_t(), ctypes.c_int64()
+        per = (ctypes.c_int64 * len(widths))()
+        _check(lib().volks_plan_query(self._h, ctypes.byref(ws), per, ctypes.byref(tot)))
+        self.workspace_bytes, self.nwin_total, self.nwin_per_width = ws.value, tot.value, list(per)
+        self.launches = lib().volks_plan_launch_count(self._h)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().volks_plan_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def fringe_search(self, vis, workspace, cands, ncand, peaks=None, stream=None):
+        """volks_fringe_search on torch CUDA tensors (asynchronous on `stream`).
+        vis complex64 [nbl][nif][nap][nchan]; workspace uint8 >= workspace_bytes;
+        cands uint8 [capacity*36]; ncand int32/uint32 [1]; peaks uint8 [nwin_total*16] or None."""
+        assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous()
+        assert tuple(vis.shape) == self.shape
+        assert workspace.is_cuda and workspace.numel() * workspace.element_size() >= self.workspace_bytes
+        cap = cands.numel() * cands.element_size() // CAND_DTYPE.itemsize
+        if peaks is not None:
+            assert peaks.numel() * peaks.element_size() >= self.nwin_total * PEAK_DTYPE.itemsize
+        st = (stream or torch.cuda.current_stream(vis.device)).cuda_stream
+        _check(lib().volks_fringe_search(
+            self._h, vis.data_ptr(), workspace.data_ptr(), peaks.data_ptr() if peaks is not None else None,
+            cands.data_ptr() if cap else None, cap, ncand.data_ptr(), st))
+
+    def window_match(self, cands, min_widths=2):
+        return window_match(cands, self.widths, min_widths)
+
+    def bin_to_physical(self, wid, rate_idx, delay_idx, ap_seconds, chan_hz):
+        return bin_to_physical(self.nts[wid], self.nf, rate_idx, delay_idx, ap_seconds, chan_hz)
+
+
+def window_match(cands, widths, min_widths=2):
+    """volks_window_match on a host numpy CAND_DTYPE array (canonical order)."""
+    cands = np.ascontiguousarray(cands, dtype=CAND_DTYPE)
+    w = np.ascontiguousarray(widths, dtype=np.int32)
+    out = np.zeros(max(len(cands), 1), dtype=PULSE_DTYPE)
+    n = ctypes.c_uint32()
+    _check(lib().volks_window_match(cands.ctypes.data, len(cands), w.ctypes.data, len(w), min_widths,
+                                    out.ctypes.data, len(out), ctypes.byref(n)))
+    return out[:n.value]
+
+
+def bin_to_physical(nt, nf, rate_idx, delay_idx, ap_seconds, chan_hz):
+    r, d = ctypes.c_double(), ctypes.c_double()
+    _check(lib().volks_bin_to_physical(nt, nf, rate_idx, delay_idx, ap_seconds, chan_hz,
+                                       ctypes.byref(r), ctypes.byref(d)))
+    return r.value, d.value
+
+
+def fringe_search(vis, widths=None, strides=None, nts=None, nf=None, snr_thresh=None, want_peaks=False,
+                  cand_capacity=1 << 20, plan=None):
+    """Convenience one-shot call: allocates workspace/outputs with torch, runs the search on the
+    current stream, synchronises and returns (cands CAND_DTYPE[n], ncand_true, peaks|None)."""
+    if not vis.is_cuda:
+        raise RuntimeError("volks fringe_search needs a CUDA tensor (there is no CPU fallback)")
+    own = plan is None
+    if own:
+        nbl, nif, nap, nchan = vis.shape
+        plan = Plan(nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh)
+    dev = vis.device
+    ws = torch.empty(plan.workspace_bytes, dtype=torch.uint8, device=dev)
+    cands = torch.empty(cand_capacity * CAND_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    ncand = torch.zeros(1, dtype=torch.int32, device=dev)
+    peaks = torch.empty(max(plan.nwin_total, 1) * PEAK_DTYPE.itemsize, dtype=torch.uint8, device=dev) if want_peaks else None
+    plan.fringe_search(vis, ws, cands, ncand, peaks)
+    torch.cuda.synchronize(dev)
+    n = int(ncand.item()) & 0xFFFFFFFF
+    c = cands[: min(n, cand_capacity) * CAND_DTYPE.itemsize].cpu().numpy().view(CAND_DTYPE)
+    p = peaks[: plan.nwin_total * PEAK_DTYPE.itemsize].cpu().numpy().view(PEAK_DTYPE) if want_peaks else None
+    if own:
+        plan.close()
+    return c, n, p

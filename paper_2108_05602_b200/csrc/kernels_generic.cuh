@@ -1,0 +1,315 @@
+// kernels_generic.cuh - the general (any width / stride / padding) multi-pass fringe-search kernels.
+//
+//   k_row_fft   a2+a3: slab load, zero-pad, delay FFT of every AP row (PAPER.md:133 step 5), and
+//               the per-AP energy sum_k |V|^2 used for the noise statistic (Parseval, A3)
+//   k_col<L>    a4+a5+a6: per (window, delay column): zero-padded rate DFT,
+//               |.|^2, argmax; per-window max over a total order through 64-bit atomicMax keys
+//
+// The rate transform of one delay column d of window (t0, w) on the padded grid Nt = L*M is split
+// by residue rho = r mod M (Cooley-Tukey, decimation in frequency):
+//   F[rho + M s] = sum_{t2<L} e^{-2 pi i s t2/L} a_rho[t2],
+//   a_rho[t2]    = sum_{t1: t2+L t1 < w} y[t0 + t2 + L t1] e^{-2 pi i rho (t2 + L t1)/Nt}
+// so one thread folds the w samples of its column into L registers and runs an L-point FFT there.
+#pragma once
+#include "common.cuh"
+
+namespace volks {
+
+// ------------------------------------------------------------------------------------------------
+// Row (delay) FFT: radix-4 Stockham autosort passes in shared memory (+ one radix-2 pass when
+// log2(nf) is odd).  One group of `tpr` threads per AP row, several rows per CTA.
+// vis rows and Y rows are indexed by the flattened (pair, AP) row number.
+// ------------------------------------------------------------------------------------------------
+struct RowArgs {
+  const float2 *vis;   // [rows_total][nchan]
+  float2 *Y;           // [nrows][nf] for rows row0 .. row0+nrows-1
+  float *E;            // [rows_total] per-AP energy
+  const float2 *twf;   // [nf] exp(-2 pi i k/nf)
+  long long row0, nrows;
+  int nchan, nf, tpr, rows_per_cta;
+};
+
+__global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
+  extern __shared__ float2 sm[];
+  const int nf = a.nf, tpr = a.tpr;
+  const int rl = threadIdx.x / tpr, lane = threadIdx.x % tpr;
+  const long long rrel = (long long)blockIdx.x * a.rows_per_cta + rl;
+  const bool live = rrel < a.nrows;
+  float2 *buf0 = sm + (size_t)rl * nf;
+  float2 *buf1 = sm + (size_t)(a.rows_per_cta + rl) * nf;
+  float *esm = (float *)(sm + (size_t)2 * a.rows_per_cta * nf);   // [rows_per_cta][16] warp partials
+
+  float e = 0.f;
+  if (live) {
+    const float2 *src = a.vis + (a.row0 + rrel) * (long long)a.nchan;
+    for (int k = lane; k < nf; k += tpr) {
+      float2 v = make_float2(0.f, 0.f);
+      if (k < a.nchan) { v = __ldg(src + k); e += cnorm(v); }
+      buf0[k] = v;
+    }
+  }
+  // energy: fixed tree (shuffle inside the row's lanes of a warp, then warp partials in order)
+  {
+    const int seg = tpr < 32 ? tpr : 32;
+    for (int o = seg >> 1; o >= 1; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+    if (tpr <= 32) {
+      if (live && lane == 0) a.E[a.row0 + rrel] = e;
+    } else {
+      if ((lane & 31) == 0) esm[rl * 16 + (lane >> 5)] = e;
+    }
+  }
+  __syncthreads();
+  if (tpr > 32 && live && lane == 0) {
+    float s = 0.f;
+    for (int i = 0; i < tpr / 32; ++i) s += esm[rl * 16 + i];
+    a.E[a.row0 + rrel] = s;
+  }
+
+  float2 *in = buf0, *out = buf1;
+  int Ns = 1;
+  // radix-4 passes
+  while (Ns * 4 <= nf) {
+    const int nb = nf >> 2;
+    if (live)
+      for (int j = lane; j < nb; j += tpr) {
+        const int k = j & (Ns - 1);
+        const int tstep = nf / (Ns * 4);            // table stride for angle unit 1/(4 Ns)
+        float2 v0 = in[j], v1 = in[j + nb], v2 = in[j + 2 * nb], v3 = in[j + 3 * nb];
+        if (k) {
+          v1 = cmul(v1, __ldg(a.twf + k * tstep));
+          v2 = cmul(v2, __ldg(a.twf + 2 * k * tstep));
+          v3 = cmul(v3, __ldg(a.twf + 3 * k * tstep));
+        }
+        float2 s02 = cadd(v0, v2), d02 = csub(v0, v2), s13 = cadd(v1, v3), d13 = csub(v1, v3);
+        float2 md13 = make_float2(d13.y, -d13.x);   // -i * d13
+        const int j0 = ((j - k) << 2) + k;
+        out[j0] = cadd(s02, s13);
+        out[j0 + Ns] = cadd(d02, md13);
+        out[j0 + 2 * Ns] = csub(s02, s13);
+        out[j0 + 3 * Ns] = csub(d02, md13);
+      }
+    __syncthreads();
+    float2 *t = in; in = out; out = t;
+    Ns <<= 2;
+  }
+  if (Ns < nf) {   // one radix-2 pass
+    const int nb = nf >> 1;
+    if (live)
+      for (int j = lane; j < nb; j += tpr) {
+        const int k = j & (Ns - 1);
+        float2 v0 = in[j], v1 = in[j + nb];
+        if (k) v1 = cmul(v1, __ldg(a.twf + k * (nf / (Ns * 2))));
+        const int j0 = ((j - k) << 1) + k;
+        out[j0] = cadd(v0, v1);
+        out[j0 + Ns] = csub(v0, v1);
+      }
+    __syncthreads();
+    float2 *t = in; in = out; out = t;
+  }
+  if (live) {
+    float2 *dst = a.Y + rrel * (long long)nf;
+    for (int k = lane; k < nf; k += tpr) dst[k] = in[k];
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Column (rate) transform + power + argmax, generic.
+// Thread task id (d fastest): ((pair_local * nwin + j) * M + rho) * nf + d.
+// ------------------------------------------------------------------------------------------------
+struct ColArgs {
+  const float2 *Y;      // [npairs_chunk][nap][nf]
+  u64 *keys;            // canonical window keys
+  const float2 *twt;    // [nt] exp(-2 pi i k/nt)
+  long long total;      // number of thread tasks
+  long long per_pair;   // windows per (bl, ifq) pair over all widths
+  long long offc;       // canonical offset of this width inside a pair
+  long long pair0;      // first pair of the chunk
+  int nap, nf, log2nf, w, stride, nt, log2m, nwin;
+};
+
+template <int L>
+__global__ void __launch_bounds__(256) k_col(ColArgs a) {
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool live = gid < a.total;
+  const int M = 1 << a.log2m;
+  u64 key = 0;
+  long long c = 0;
+  if (live) {
+    const int d = (int)(gid & (a.nf - 1));
+    long long rest = gid >> a.log2nf;
+    const int rho = (int)(rest & (M - 1));
+    rest >>= a.log2m;
+    const int j = (int)(rest % a.nwin);
+    const long long pl = rest / a.nwin;
+    c = (a.pair0 + pl) * a.per_pair + a.offc + j;
+    const int t0 = j * a.stride;
+    const float2 *col = a.Y + ((pl * a.nap + t0) * (long long)a.nf + d);
+    float2 acc[L];
+#pragma unroll
+    for (int i = 0; i < L; ++i) acc[i] = make_float2(0.f, 0.f);
+    const int ntm = a.nt - 1;
+    for (int tb = 0; tb < a.w; tb += L) {
+#pragma unroll
+      for (int t2 = 0; t2 < L; ++t2) {
+        const int t = tb + t2;
+        if (t < a.w) {
+          const float2 y = __ldg(col + (long long)t * a.nf);
+          const float2 tw = __ldg(a.twt + ((rho * t) & ntm));
+          cmac(acc[t2], y, tw);
+        }
+      }
+    }
+    FftDif<L, 0, L>::run(acc);
+    float best = -1.f;
+    int bs = 0;
+#pragma unroll
+    for (int s = 0; s < L; ++s) {
+      const float p = cnorm(acc[brev<L>(s)]);
+      if (p > best) { best = p; bs = s; }
+    }
+    const uint32_t r = (uint32_t)(rho + (bs << a.log2m));
+    key = make_key(best, r * (uint32_t)a.nf + (uint32_t)d);
+  }
+  if ((long long)a.nf << a.log2m >= 32) {
+    // all 32 lanes belong to one window (tasks per window is a multiple of 32)
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) {
+      const u64 other = __shfl_xor_sync(0xffffffffu, key, o);
+      key = other > key ? other : key;
+    }
+    if (live && (threadIdx.x & 31) == 0) atomicMax(a.keys + c, key);
+  } else if (live) {
+    atomicMax(a.keys + c, key);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Finalize: SNR, threshold, dense peaks, ordered compaction (count -> scan -> scatter).
+// ------------------------------------------------------------------------------------------------
+struct Sched {   // the window schedule (device copy lives in the plan)
+  int nwidths, nbl, nif, nap, nf, log2nf;
+  float snr_thresh;
+  long long per_pair, nwin_total;
+  int width[16], stride[16], nt[16];
+  long long nwin[16];     // windows per pair
+  long long offc[16];     // canonical offset inside a pair
+  long long offd[16];     // dense-layout offset: npair * sum_{q'<q} nwin
+};
+
+struct WinStat { float power, snr; int rate_idx, delay_idx, q, j, t0; long long pair; };
+
+__device__ __forceinline__ WinStat window_stat(const Sched &s, const u64 *keys, const float *E, long long c) {
+  WinStat o;
+  o.pair = c / s.per_pair;
+  long long rem = c - o.pair * s.per_pair;
+  int q = 0;
+  while (q + 1 < s.nwidths && rem >= s.nwin[q]) { rem -= s.nwin[q]; ++q; }
+  o.q = q; o.j = (int)rem; o.t0 = o.j * s.stride[q];
+  const u64 k = keys[c];
+  o.power = key_power(k);
+  const uint32_t idx = key_index(k);
+  o.rate_idx = (int)(idx >> s.log2nf);
+  o.delay_idx = (int)(idx & (uint32_t)(s.nf - 1));
+  // noise = mean |F|^2 over the padded plane = sum over the window of |V|^2 (Parseval)
+  const float *e = E + o.pair * s.nap + o.t0;
+  float es = 0.f;
+  for (int t = 0; t < s.width[q]; ++t) es += e[t];
+  o.snr = es > 0.f ? sqrtf(o.power / es) : 0.f;
+  return o;
+}
+
+constexpr int FIN_THREADS = 256, FIN_TILES = 8;   // 2048 windows per CTA
+
+__global__ void __launch_bounds__(FIN_THREADS) k_finalize(const Sched *sp, const u64 *keys, const float *E,
+                                                          float4 *peaks, uint32_t *blockcount) {
+  __shared__ Sched s;
+  __shared__ uint32_t wsum[FIN_THREADS / 32];
+  if (threadIdx.x == 0) s = *sp;
+  __syncthreads();
+  uint32_t mine = 0;
+  const long long base = (long long)blockIdx.x * (FIN_THREADS * FIN_TILES);
+  for (int tile = 0; tile < FIN_TILES; ++tile) {
+    const long long c = base + tile * FIN_THREADS + threadIdx.x;
+    if (c < s.nwin_total) {
+      const WinStat o = window_stat(s, keys, E, c);
+      if (peaks) {
+        const long long di = s.offd[o.q] + o.pair * s.nwin[o.q] + o.j;
+        peaks[di] = make_float4(o.power, o.snr, __int_as_float(o.rate_idx), __int_as_float(o.delay_idx));
+      }
+      mine += o.snr > s.snr_thresh ? 1u : 0u;
+    }
+  }
+  for (int o = 16; o >= 1; o >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, o);
+  if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = mine;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t t = 0;
+    for (int i = 0; i < FIN_THREADS / 32; ++i) t += wsum[i];
+    blockcount[blockIdx.x] = t;
+  }
+}
+
+// single CTA: exclusive scan of blockcount[n] in place, total -> *ncand
+__global__ void __launch_bounds__(1024) k_scan(uint32_t *blockcount, long long n, uint32_t *ncand) {
+  __shared__ uint32_t part[1024];
+  const long long per = (n + 1023) / 1024;
+  const long long lo = threadIdx.x * per, hi = lo + per < n ? lo + per : n;
+  uint32_t s = 0;
+  for (long long i = lo; i < hi; ++i) s += blockcount[i];
+  part[threadIdx.x] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t run = 0;
+    for (int i = 0; i < 1024; ++i) { const uint32_t v = part[i]; part[i] = run; run += v; }
+    *ncand = run;
+  }
+  __syncthreads();
+  uint32_t run = part[threadIdx.x];
+  for (long long i = lo; i < hi; ++i) { const uint32_t v = blockcount[i]; blockcount[i] = run; run += v; }
+}
+
+struct CandOut { int bl, ifq, wid, win, t0, rate_idx, delay_idx; float power, snr; };
+
+__global__ void __launch_bounds__(FIN_THREADS) k_scatter(const Sched *sp, const u64 *keys, const float *E,
+                                                         const uint32_t *blockoff, CandOut *cands,
+                                                         uint32_t capacity) {
+  __shared__ Sched s;
+  __shared__ uint32_t wsum[FIN_THREADS / 32];
+  __shared__ uint32_t running;
+  if (threadIdx.x == 0) { s = *sp; running = blockoff[blockIdx.x]; }
+  __syncthreads();
+  const long long base = (long long)blockIdx.x * (FIN_THREADS * FIN_TILES);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int tile = 0; tile < FIN_TILES; ++tile) {
+    const long long c = base + tile * FIN_THREADS + threadIdx.x;
+    WinStat o;
+    bool flag = false;
+    if (c < s.nwin_total) {
+      o = window_stat(s, keys, E, c);
+      flag = o.snr > s.snr_thresh;
+    }
+    const uint32_t bal = __ballot_sync(0xffffffffu, flag);
+    if (lane == 0) wsum[wid] = __popc(bal);
+    __syncthreads();
+    uint32_t before = running;
+    for (int i = 0; i < wid; ++i) before += wsum[i];
+    if (flag) {
+      const uint32_t pos = before + __popc(bal & ((1u << lane) - 1u));
+      if (pos < capacity) {
+        CandOut r;
+        r.bl = (int)(o.pair / s.nif); r.ifq = (int)(o.pair % s.nif); r.wid = o.q; r.win = o.j; r.t0 = o.t0;
+        r.rate_idx = o.rate_idx; r.delay_idx = o.delay_idx; r.power = o.power; r.snr = o.snr;
+        cands[pos] = r;
+      }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      uint32_t t = 0;
+      for (int i = 0; i < FIN_THREADS / 32; ++i) t += wsum[i];
+      running += t;
+    }
+    __syncthreads();
+  }
+}
+
+}  // namespace volks

@@ -1,0 +1,292 @@
+// volks_api.cu - C-ABI entry points (include/volks.h): plan / window scheduler, launches, host helpers.
+#include "../../include/volks.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "kernels_generic.cuh"
+
+using namespace volks;
+
+namespace {
+
+thread_local char g_cuda_msg[256] = "";
+
+inline bool is_pow2(long long n) { return n >= 1 && (n & (n - 1)) == 0; }
+inline int ilog2(long long n) { int l = 0; while ((1LL << l) < n) ++l; return l; }
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+bool cuda_ok(cudaError_t e) {
+  if (e == cudaSuccess) return true;
+  snprintf(g_cuda_msg, sizeof g_cuda_msg, "%s", cudaGetErrorString(e));
+  return false;
+}
+
+// one width's entry of the window schedule (a1)
+struct WidthPlan {
+  int w, s, nt, L, log2m;
+  long long nwin;       // per pair
+  size_t tw_off;        // offset (float2) of its rate twiddle table in d_tables
+};
+
+template <int L>
+static void launch_col(const ColArgs &a, cudaStream_t st) {
+  const long long blocks = (a.total + 255) / 256;
+  k_col<L><<<(unsigned)blocks, 256, 0, st>>>(a);
+}
+
+}  // namespace
+
+struct volks_plan {
+  Sched sched;                 // host copy
+  Sched *d_sched = nullptr;    // device copy
+  std::vector<WidthPlan> wp;
+  float2 *d_tables = nullptr;  // [nf] delay twiddles, then per width [nt] rate twiddles
+  int nchan = 0;
+  long long npair = 0;
+  // workspace layout (byte offsets)
+  size_t off_keys = 0, off_E = 0, off_cnt = 0, off_Y = 0, ws_bytes = 0;
+  long long nfin_blocks = 0;
+  long long pairs_per_chunk = 0, nchunks = 0;
+  // row kernel shape
+  int row_tpr = 1, row_rows_per_cta = 1;
+  size_t row_smem = 0;
+  int launches = 0;
+};
+
+extern "C" {
+
+int volks_version(void) { return 100; }
+
+const char *volks_strerror(int code) {
+  switch (code) {
+    case VOLKS_OK: return "ok";
+    case VOLKS_EINVAL: return "invalid argument";
+    case VOLKS_ECUDA: return g_cuda_msg[0] ? g_cuda_msg : "CUDA error";
+    case VOLKS_ENOMEM: return "out of host memory";
+    case VOLKS_EOVERFLOW: return "output capacity exceeded";
+    default: return "unknown error";
+  }
+}
+
+int volks_plan_create(const volks_params *p, volks_plan **out) {
+  if (!p || !out) return VOLKS_EINVAL;
+  *out = nullptr;
+  if (p->nbl < 1 || p->nif < 1 || p->nap < 0 || p->nchan < 1) return VOLKS_EINVAL;
+  if (p->nwidths < 1 || p->nwidths > VOLKS_MAX_WIDTHS || !p->width || !p->stride || !p->nt) return VOLKS_EINVAL;
+  if (!is_pow2(p->nf) || p->nf < p->nchan || p->nf > (1 << 14)) return VOLKS_EINVAL;
+  if (!(p->snr_thresh == p->snr_thresh)) return VOLKS_EINVAL;
+  for (int q = 0; q < p->nwidths; ++q) {
+    if (p->width[q] < 1 || p->stride[q] < 1 || !is_pow2(p->nt[q]) || p->nt[q] < p->width[q]) return VOLKS_EINVAL;
+    if ((long long)p->nt[q] * p->nf > (1LL << 31)) return VOLKS_EINVAL;   // plane index must fit 32 bits
+  }
+  volks_plan *pl = new (std::nothrow) volks_plan();
+  if (!pl) return VOLKS_ENOMEM;
+  Sched &s = pl->sched;
+  memset(&s, 0, sizeof s);
+  s.nwidths = p->nwidths; s.nbl = p->nbl; s.nif = p->nif; s.nap = p->nap; s.nf = p->nf;
+  s.log2nf = ilog2(p->nf); s.snr_thresh = p->snr_thresh;
+  pl->nchan = p->nchan;
+  pl->npair = (long long)p->nbl * p->nif;
+  long long per_pair = 0;
+  size_t tw_total = (size_t)p->nf;
+  for (int q = 0; q < p->nwidths; ++q) {
+    WidthPlan w;
+    w.w = p->width[q]; w.s = p->stride[q]; w.nt = p->nt[q];
+    w.nwin = p->nap < w.w ? 0 : (long long)(p->nap - w.w) / w.s + 1;
+    w.L = std::min(16, w.nt);
+    w.log2m = ilog2(w.nt / w.L);
+    w.tw_off = tw_total;
+    tw_total += (size_t)w.nt;
+    s.width[q] = w.w; s.stride[q] = w.s; s.nt[q] = w.nt; s.nwin[q] = w.nwin; s.offc[q] = per_pair;
+    per_pair += w.nwin;
+    pl->wp.push_back(w);
+  }
+  s.per_pair = per_pair;
+  s.nwin_total = per_pair * pl->npair;
+  long long acc = 0;
+  for (int q = 0; q < p->nwidths; ++q) { s.offd[q] = acc; acc += pl->npair * s.nwin[q]; }
+  if (s.nwin_total >= (1LL << 40)) { delete pl; return VOLKS_EINVAL; }
+
+  // row kernel shape: nf/4 threads per row (at least 1, at most 512), ~256 threads per CTA
+  pl->row_tpr = std::max(1, std::min(512, p->nf / 4));
+  pl->row_rows_per_cta = std::max(1, 256 / pl->row_tpr);
+  pl->row_smem = (size_t)2 * pl->row_rows_per_cta * p->nf * sizeof(float2) + (size_t)pl->row_rows_per_cta * 16 * sizeof(float);
+  if (pl->row_smem > 200 * 1024) { delete pl; return VOLKS_EINVAL; }
+
+  // chunking of the delay-spectrum intermediate Y over (bl, ifq) pairs: <= 4 GiB per chunk
+  const size_t y_pair = (size_t)p->nap * p->nf * sizeof(float2);
+  const size_t budget = (size_t)4 << 30;
+  long long ppc = y_pair ? (long long)std::max<size_t>(1, budget / std::max<size_t>(y_pair, 1)) : pl->npair;
+  ppc = std::min(ppc, pl->npair);
+  pl->nchunks = (pl->npair + ppc - 1) / ppc;
+  pl->pairs_per_chunk = (pl->npair + pl->nchunks - 1) / pl->nchunks;
+  pl->nchunks = (pl->npair + pl->pairs_per_chunk - 1) / pl->pairs_per_chunk;
+
+  pl->nfin_blocks = (s.nwin_total + FIN_THREADS * FIN_TILES - 1) / (FIN_THREADS * FIN_TILES);
+  size_t off = 0;
+  pl->off_keys = off; off = align_up(off + (size_t)std::max<long long>(s.nwin_total, 1) * sizeof(u64), 256);
+  pl->off_E = off;    off = align_up(off + (size_t)std::max<long long>(pl->npair * p->nap, 1) * sizeof(float), 256);
+  pl->off_cnt = off;  off = align_up(off + (size_t)std::max<long long>(pl->nfin_blocks, 1) * sizeof(uint32_t), 256);
+  pl->off_Y = off;    off = align_up(off + (size_t)pl->pairs_per_chunk * std::max<size_t>(y_pair, 8), 256);
+  pl->ws_bytes = off;
+
+  int active = 0;
+  for (auto &w : pl->wp) active += w.nwin > 0 ? 1 : 0;
+  pl->launches = s.nwin_total > 0 ? (int)(1 + pl->nchunks * (1 + active) + 3) : 1;
+
+  // tables, computed in double precision on the host
+  std::vector<float2> tab(tw_total);
+  const double PI = 3.14159265358979323846264338327950288;
+  for (int k = 0; k < p->nf; ++k) {
+    const double a = -2.0 * PI * k / p->nf;
+    tab[k] = make_float2((float)cos(a), (float)sin(a));
+  }
+  for (auto &w : pl->wp)
+    for (int k = 0; k < w.nt; ++k) {
+      const double a = -2.0 * PI * k / w.nt;
+      tab[w.tw_off + k] = make_float2((float)cos(a), (float)sin(a));
+    }
+  bool ok = cuda_ok(cudaMalloc(&pl->d_tables, tw_total * sizeof(float2))) &&
+            cuda_ok(cudaMalloc(&pl->d_sched, sizeof(Sched))) &&
+            cuda_ok(cudaMemcpy(pl->d_tables, tab.data(), tw_total * sizeof(float2), cudaMemcpyHostToDevice)) &&
+            cuda_ok(cudaMemcpy(pl->d_sched, &s, sizeof(Sched), cudaMemcpyHostToDevice)) &&
+            cuda_ok(cudaFuncSetAttribute(k_row_fft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->row_smem));
+  if (!ok) { volks_plan_destroy(pl); return VOLKS_ECUDA; }
+  *out = pl;
+  return VOLKS_OK;
+}
+
+int volks_plan_destroy(volks_plan *pl) {
+  if (!pl) return VOLKS_EINVAL;
+  if (pl->d_tables) cudaFree(pl->d_tables);
+  if (pl->d_sched) cudaFree(pl->d_sched);
+  delete pl;
+  return VOLKS_OK;
+}
+
+int volks_plan_query(const volks_plan *pl, size_t *workspace_bytes, int64_t *nwin_per_width, int64_t *nwin_total) {
+  if (!pl) return VOLKS_EINVAL;
+  if (workspace_bytes) *workspace_bytes = pl->ws_bytes;
+  if (nwin_per_width) for (int q = 0; q < pl->sched.nwidths; ++q) nwin_per_width[q] = pl->sched.nwin[q];
+  if (nwin_total) *nwin_total = pl->sched.nwin_total;
+  return VOLKS_OK;
+}
+
+int volks_plan_launch_count(const volks_plan *pl) { return pl ? pl->launches : VOLKS_EINVAL; }
+
+int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspace, volks_peak *d_peaks,
+                        volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand, void *cuda_stream) {
+  if (!pl || !d_vis || !d_workspace || !d_ncand || (!d_cands && cand_capacity > 0)) return VOLKS_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const Sched &s = pl->sched;
+  char *ws = (char *)d_workspace;
+  u64 *keys = (u64 *)(ws + pl->off_keys);
+  float *E = (float *)(ws + pl->off_E);
+  uint32_t *cnt = (uint32_t *)(ws + pl->off_cnt);
+  float2 *Y = (float2 *)(ws + pl->off_Y);
+  if (s.nwin_total == 0) {
+    return cuda_ok(cudaMemsetAsync(d_ncand, 0, sizeof(uint32_t), st)) ? VOLKS_OK : VOLKS_ECUDA;
+  }
+  if (!cuda_ok(cudaMemsetAsync(keys, 0, (size_t)s.nwin_total * sizeof(u64), st))) return VOLKS_ECUDA;
+  for (long long ch = 0; ch < pl->nchunks; ++ch) {
+    const long long pair0 = ch * pl->pairs_per_chunk;
+    const long long np = std::min(pl->pairs_per_chunk, pl->npair - pair0);
+    RowArgs ra;
+    ra.vis = (const float2 *)d_vis; ra.Y = Y; ra.E = E; ra.twf = pl->d_tables;
+    ra.row0 = pair0 * s.nap; ra.nrows = np * s.nap;
+    ra.nchan = pl->nchan; ra.nf = s.nf; ra.tpr = pl->row_tpr; ra.rows_per_cta = pl->row_rows_per_cta;
+    const long long rblocks = (ra.nrows + ra.rows_per_cta - 1) / ra.rows_per_cta;
+    k_row_fft<<<(unsigned)rblocks, ra.tpr * ra.rows_per_cta, pl->row_smem, st>>>(ra);
+    for (int q = 0; q < s.nwidths; ++q) {
+      const WidthPlan &w = pl->wp[q];
+      if (w.nwin == 0) continue;
+      ColArgs ca;
+      ca.Y = Y; ca.keys = keys; ca.twt = pl->d_tables + w.tw_off;
+      ca.per_pair = s.per_pair; ca.offc = s.offc[q]; ca.pair0 = pair0;
+      ca.nap = s.nap; ca.nf = s.nf; ca.log2nf = s.log2nf; ca.w = w.w; ca.stride = w.s; ca.nt = w.nt;
+      ca.log2m = w.log2m; ca.nwin = (int)w.nwin;
+      ca.total = ((np * w.nwin) << w.log2m) * s.nf;
+      switch (w.L) {
+        case 1: launch_col<1>(ca, st); break;
+        case 2: launch_col<2>(ca, st); break;
+        case 4: launch_col<4>(ca, st); break;
+        case 8: launch_col<8>(ca, st); break;
+        default: launch_col<16>(ca, st); break;
+      }
+    }
+  }
+  k_finalize<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, (float4 *)d_peaks, cnt);
+  k_scan<<<1, 1024, 0, st>>>(cnt, pl->nfin_blocks, d_ncand);
+  k_scatter<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity);
+  return cuda_ok(cudaGetLastError()) ? VOLKS_OK : VOLKS_ECUDA;
+}
+
+// Host: sweep over candidates sorted by start AP inside each (bl, ifq) group.  Interval-overlap
+// connected components are exactly the maximal runs whose start lies before the running end.
+int volks_window_match(const volks_cand *cands, uint32_t ncand, const int32_t *width, int32_t nwidths,
+                       int32_t min_widths, volks_pulse *out, uint32_t capacity, uint32_t *nout) {
+  if (!width || nwidths < 1 || nwidths > VOLKS_MAX_WIDTHS || !nout || (!cands && ncand) || (!out && capacity))
+    return VOLKS_EINVAL;
+  struct { const int32_t *width; int nwidths; } s = {width, nwidths};
+  std::vector<uint32_t> ord(ncand);
+  for (uint32_t i = 0; i < ncand; ++i) {
+    if (cands[i].wid < 0 || cands[i].wid >= s.nwidths) return VOLKS_EINVAL;
+    ord[i] = i;
+  }
+  std::stable_sort(ord.begin(), ord.end(), [&](uint32_t a, uint32_t b) {
+    const volks_cand &x = cands[a], &y = cands[b];
+    if (x.bl != y.bl) return x.bl < y.bl;
+    if (x.ifq != y.ifq) return x.ifq < y.ifq;
+    return x.t0 < y.t0;
+  });
+  struct Rec { uint32_t best; int nhit, tb, te; };
+  std::vector<Rec> found;
+  uint32_t i = 0;
+  while (i < ncand) {
+    const volks_cand &f = cands[ord[i]];
+    int end = f.t0 + s.width[f.wid];
+    uint32_t best = ord[i];
+    uint32_t mask = 1u << f.wid;
+    uint32_t k = i + 1;
+    while (k < ncand) {
+      const volks_cand &c = cands[ord[k]];
+      if (c.bl != f.bl || c.ifq != f.ifq || c.t0 >= end) break;
+      end = std::max(end, c.t0 + s.width[c.wid]);
+      mask |= 1u << c.wid;
+      const volks_cand &b = cands[best];
+      if (c.snr > b.snr || (c.snr == b.snr && ord[k] < best)) best = ord[k];
+      ++k;
+    }
+    int nhit = 0;
+    for (uint32_t m = mask; m; m &= m - 1) ++nhit;
+    if (nhit >= min_widths) found.push_back({best, nhit, f.t0, end});
+    i = k;
+  }
+  std::sort(found.begin(), found.end(), [](const Rec &a, const Rec &b) { return a.best < b.best; });
+  *nout = (uint32_t)found.size();
+  for (uint32_t n = 0; n < found.size() && n < capacity; ++n) {
+    out[n].best = cands[found[n].best];
+    out[n].nwidths_hit = found[n].nhit; out[n].t_begin = found[n].tb; out[n].t_end = found[n].te;
+  }
+  return found.size() > capacity ? VOLKS_EOVERFLOW : VOLKS_OK;
+}
+
+int volks_bin_to_physical(int32_t nt, int32_t nf, int32_t rate_idx, int32_t delay_idx, double ap_seconds,
+                          double chan_hz, double *rate_hz, double *delay_s) {
+  if (nt < 1 || nf < 1) return VOLKS_EINVAL;
+  if (rate_idx < 0 || rate_idx >= nt || delay_idx < 0 || delay_idx >= nf) return VOLKS_EINVAL;
+  if (!(ap_seconds > 0) || !(chan_hz > 0)) return VOLKS_EINVAL;
+  const int rs = rate_idx >= (nt + 1) / 2 && nt > 1 ? rate_idx - nt : rate_idx;
+  const int ds = delay_idx >= (nf + 1) / 2 && nf > 1 ? delay_idx - nf : delay_idx;
+  if (rate_hz) *rate_hz = rs / (nt * ap_seconds);
+  if (delay_s) *delay_s = ds / (nf * chan_hz);
+  return VOLKS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,75 @@
+"""Comparison rules CUDA path vs oracle (north_star).
+
+ * per window: (r*, d*) must equal the oracle's first argmax idx1, except where the oracle's top two
+   powers differ by < 1e-5 relative, where idx2 is accepted too;
+ * |P1_gpu - P1| <= 1e-4 P1 and |snr_gpu - snr| <= 1e-4 snr;
+ * candidate lists identical and in canonical order, except that a window whose oracle snr lies
+   within 1e-4 relative of the threshold may be present or absent.
+"""
+import numpy as np
+
+RTOL = 1e-4
+TIE = 1e-5
+
+
+def dense_index(nbl, nif, nwin_per_width):
+    """dense-layout index (include/volks.h) of every window in canonical order."""
+    npair = nbl * nif
+    per = int(sum(nwin_per_width))
+    out = np.empty(npair * per, dtype=np.int64)
+    offd, offc = 0, 0
+    for n in nwin_per_width:
+        j = np.arange(n, dtype=np.int64)
+        for pair in range(npair):
+            out[pair * per + offc: pair * per + offc + n] = offd + pair * n + j
+        offd += npair * n
+        offc += n
+    return out
+
+
+def check_peaks(gpu_peaks, ora, nf):
+    """gpu_peaks: PEAK records aligned with `ora` (oracle PEAK records).  Returns #ties used."""
+    gidx = gpu_peaks["rate_idx"].astype(np.int64) * nf + gpu_peaks["delay_idx"].astype(np.int64)
+    p1 = ora["p1"]
+    safe = np.where(p1 > 0, p1, 1.0)
+    near_tie = (p1 - ora["p2"]) / safe < TIE
+    ok_idx = (gidx == ora["idx1"]) | (near_tie & (gidx == ora["idx2"]))
+    bad = np.nonzero(~ok_idx)[0]
+    assert bad.size == 0, "argmax mismatch at %s: gpu %s oracle %s/%s gap %s" % (
+        bad[:5], gidx[bad[:5]], ora["idx1"][bad[:5]], ora["idx2"][bad[:5]], ((p1 - ora["p2"]) / safe)[bad[:5]])
+    perr = np.abs(gpu_peaks["power"].astype(np.float64) - p1) / safe
+    assert perr.max(initial=0.0) <= RTOL, "power error %g" % perr.max()
+    ssafe = np.where(ora["snr"] > 0, ora["snr"], 1.0)
+    serr = np.abs(gpu_peaks["snr"].astype(np.float64) - ora["snr"]) / ssafe
+    assert serr.max(initial=0.0) <= RTOL, "snr error %g" % serr.max()
+    return int(np.count_nonzero(gidx != ora["idx1"])), float(perr.max(initial=0.0)), float(serr.max(initial=0.0))
+
+
+def check_candidates(gpu_cands, ora_cands, ora_peaks, keep, thresh, nf):
+    """Ordered candidate list equality, with the near-threshold exemption: a window whose oracle
+    snr lies within RTOL of the threshold may be present or absent.  `keep` = canonical window index
+    of every oracle candidate.  Returns (#candidates compared, #marginal windows)."""
+    key = lambda c: (int(c["bl"]), int(c["ifq"]), int(c["wid"]), int(c["win"]))
+    gk = [key(c) for c in gpu_cands]
+    assert gk == sorted(gk), "GPU candidates not in canonical order"
+    assert len(set(gk)) == len(gk), "duplicate GPU candidates"
+    marg = np.abs(ora_peaks["snr"][keep] - thresh) <= RTOL * thresh        # marginal oracle candidates
+    nmarg_all = int(np.count_nonzero(np.abs(ora_peaks["snr"] - thresh) <= RTOL * thresh))
+    omap = {key(c): i for i, c in enumerate(ora_cands)}
+    gset = set(gk)
+    for k_, i in omap.items():                      # every firm oracle candidate must be present
+        assert k_ in gset or marg[i], "missing candidate %s (oracle snr %r)" % (k_, ora_cands[i]["snr"])
+    extra = [k_ for k_ in gk if k_ not in omap]     # extras are allowed only if marginal
+    assert len(extra) <= nmarg_all - int(marg.sum()), "unexpected candidates %s" % extra[:5]
+    n = 0
+    for g in gpu_cands:
+        i = omap.get(key(g))
+        if i is None:
+            assert abs(float(g["snr"]) - thresh) <= 2 * RTOL * thresh
+            continue
+        o = ora_cands[i]
+        assert g["t0"] == o["t0"]
+        assert abs(float(g["power"]) - o["power"]) <= RTOL * o["power"]
+        assert abs(float(g["snr"]) - o["snr"]) <= RTOL * o["snr"]
+        n += 1
+    return n, nmarg_all

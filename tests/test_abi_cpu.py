@@ -1,0 +1,123 @@
+"""CPU-side checks of the boundary: the library loads, exports every symbol include/volks.h
+declares, validates parameters before touching CUDA, and the host-side calls work without a GPU."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def vb():
+    from paper_2108_05602_b200 import build
+    build.build()
+    import paper_2108_05602_b200 as v
+    return v
+
+
+def test_exports_every_declared_symbol(vb):
+    hdr = open(os.path.join(ROOT, "include", "volks.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(volks_[a-z_]+)\s*\(", hdr))
+    assert {"volks_plan_create", "volks_fringe_search", "volks_window_match"} <= declared
+    L = vb.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+    from paper_2108_05602_b200 import binding
+    assert declared == set(binding.EXPORTS)
+
+
+def test_struct_sizes_match_header(vb):
+    assert vb.CAND_DTYPE.itemsize == 36 and vb.PEAK_DTYPE.itemsize == 16 and vb.PULSE_DTYPE.itemsize == 48
+
+
+@pytest.mark.parametrize("kw", [
+    dict(nts=[12]), dict(nts=[4]), dict(nf=48), dict(nf=16), dict(widths=[0]), dict(strides=[0]),
+    dict(nbl=0), dict(nchan=0), dict(nap=-1), dict(widths=[], strides=[], nts=[]),
+])
+def test_plan_create_rejects_bad_params_before_cuda(vb, kw):
+    a = dict(nbl=1, nif=1, nap=512, nchan=32, widths=[8], strides=[1], nts=[16], nf=64, snr_thresh=6.0)
+    a.update(kw)
+    rc, h = vb.plan_create_raw(**a)
+    assert rc == -1 and not h
+
+
+def test_strerror_and_version(vb):
+    L = vb.lib()
+    assert L.volks_version() >= 100
+    assert L.volks_strerror(0) == b"ok" and b"invalid" in L.volks_strerror(-1)
+
+
+def test_null_arguments(vb):
+    L = vb.lib()
+    assert L.volks_plan_create(None, None) == -1
+    assert L.volks_plan_destroy(None) == -1
+    assert L.volks_plan_query(None, None, None, None) == -1
+    assert L.volks_fringe_search(None, None, None, None, None, 0, None, None) == -1
+
+
+def test_no_oracle_or_fallback_in_product():
+    """The product path must not import or link anything under oracle/ (nor any CPU fallback)."""
+    pkg = os.path.join(ROOT, "paper_2108_05602_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in src.replace("no CPU fallback", ""), f
+                assert "cufft" not in src.lower(), f
+
+
+def _mk(vb, rows):
+    c = np.zeros(len(rows), dtype=vb.CAND_DTYPE)
+    for i, (bl, ifq, wid, win, t0, snr) in enumerate(rows):
+        c[i]["bl"], c[i]["ifq"], c[i]["wid"], c[i]["win"], c[i]["t0"], c[i]["snr"] = bl, ifq, wid, win, t0, snr
+    return c
+
+
+def test_window_match_host_vs_oracle(vb, oracle):
+    """a8 runs on the host (integer work): product sweep vs the oracle's O(n^2) union-find."""
+    rng = np.random.default_rng(8)
+    widths = [2, 4, 8, 16, 32]
+    for trial in range(20):
+        rows = []
+        for _ in range(int(rng.integers(0, 150))):
+            rows.append((int(rng.integers(0, 3)), int(rng.integers(0, 2)), int(rng.integers(0, 5)), 0,
+                         int(rng.integers(0, 400)), float(rng.integers(60, 90)) / 10))
+        rows.sort(key=lambda r: (r[0], r[1], r[2], r[4]))
+        got = vb.window_match(_mk(vb, rows), widths, 2)
+        oc = np.zeros(len(rows), dtype=oracle.CAND_DTYPE)
+        for i, r in enumerate(rows):
+            oc[i]["bl"], oc[i]["ifq"], oc[i]["wid"], oc[i]["win"], oc[i]["t0"], oc[i]["snr"] = r
+        exp = oracle.window_match(oc, widths, 2)
+        assert len(got) == len(exp)
+        for g, e in zip(got, exp):
+            r = rows[int(e["rep"])]
+            assert (g["best"]["bl"], g["best"]["ifq"], g["best"]["wid"], g["best"]["t0"]) == (r[0], r[1], r[2], r[4])
+            assert g["best"]["snr"] == np.float32(r[5])
+            assert (g["nwidths_hit"], g["t_begin"], g["t_end"]) == (e["nwidths_hit"], e["t_begin"], e["t_end"])
+
+
+def test_window_match_capacity_and_errors(vb):
+    L = vb.lib()
+    c = _mk(vb, [(0, 0, 0, 0, 0, 7.0), (0, 0, 1, 0, 1, 8.0), (0, 0, 0, 50, 50, 7.0), (0, 0, 1, 25, 50, 7.5)])
+    w = np.array([4, 8], np.int32)
+    out = np.zeros(1, dtype=vb.PULSE_DTYPE)
+    n = ctypes.c_uint32()
+    rc = L.volks_window_match(c.ctypes.data, 4, w.ctypes.data, 2, 2, out.ctypes.data, 1, ctypes.byref(n))
+    assert rc == -4 and n.value == 2 and out[0]["best"]["t0"] == 1
+    bad = c.copy(); bad[0]["wid"] = 5
+    assert L.volks_window_match(bad.ctypes.data, 4, w.ctypes.data, 2, 2, out.ctypes.data, 1, ctypes.byref(n)) == -1
+
+
+def test_bin_to_physical(vb):
+    r, d = vb.bin_to_physical(16, 64, 4, 10, 1e-3, 5e5)
+    assert r == pytest.approx(4 / (16 * 1e-3)) and d == pytest.approx(10 / (64 * 5e5))
+    r, d = vb.bin_to_physical(16, 64, 12, 54, 1e-3, 5e5)
+    assert r == pytest.approx(-4 / (16 * 1e-3)) and d == pytest.approx(-10 / (64 * 5e5))
+    r, d = vb.bin_to_physical(16, 64, 8, 32, 1e-3, 5e5)          # Nyquist bins are negative
+    assert r < 0 and d < 0
+    with pytest.raises(vb.VolksError):
+        vb.bin_to_physical(16, 64, 16, 0, 1e-3, 5e5)

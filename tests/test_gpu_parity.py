@@ -1,0 +1,152 @@
+"""Parity of the CUDA path (through the C-ABI binding) against the float64 oracle on the same
+seeded inputs.  Needs a GPU (B200)."""
+import numpy as np
+import pytest
+import torch
+
+import workloads
+from _parity import check_candidates, check_peaks, dense_index
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def vb():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2108_05602_b200 as v
+    v.lib()          # must load: no fallback
+    return v
+
+
+def run_both(vb, oracle, vis, c, thresh=None, mode="cached"):
+    thresh = c["snr_thresh"] if thresh is None else thresh
+    nbl, nif, nap, nchan = vis.shape
+    cands, n, peaks = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], thresh,
+                                       want_peaks=True)
+    ora, _ = oracle.search(vis.cpu().numpy(), c["widths"], c["strides"], c["nts"], c["nf"], mode=mode)
+    nw = [workloads.gen.nwin(nap, w, s) for w, s in zip(c["widths"], c["strides"])]
+    di = dense_index(nbl, nif, nw)
+    assert len(ora) == len(peaks) == len(di)
+    stats = check_peaks(peaks[di], ora, c["nf"])
+    oc, keep = oracle.candidates(ora, nbl, nif, nap, c["widths"], c["strides"], c["nf"], thresh)
+    assert n == len(cands)
+    ncand, nmarg = check_candidates(cands, oc, ora, keep, thresh, c["nf"])
+    return stats, ncand, cands, ora
+
+
+def test_config0_full(vb, oracle):
+    vis, c, _ = workloads.generate(0)
+    stats, ncand, cands, ora = run_both(vb, oracle, vis, c)
+    assert ncand >= 1 and all(cands["rate_idx"] == 4) and all(cands["delay_idx"] == 10)
+
+
+def test_config1_full(vb, oracle):
+    vis, c, _ = workloads.generate(1)
+    stats, ncand, cands, ora = run_both(vb, oracle, vis, c)
+    assert ncand >= 1
+
+
+@pytest.mark.parametrize("cfg,over", [
+    (2, dict(nbl=2, nif=1, nap=400, npulses=3)),
+    (3, dict(nbl=3, nif=2, nap=1000, npulses=4)),
+    (4, dict(nbl=1, nif=1, nap=600, npulses=1)),
+])
+def test_reduced_configs(vb, oracle, cfg, over):
+    """configs 2-4 at reduced extent (same nchan / widths / strides / padding): several tiles and a
+    ragged tail, every window compared."""
+    vis, c, _ = workloads.generate(cfg, **over)
+    run_both(vb, oracle, vis, c)
+    run_both(vb, oracle, vis, c, thresh=3.0)      # PAPER.md:196 stress threshold
+
+
+@pytest.mark.parametrize("shape", [
+    # nbl nif nap nchan widths strides nts nf
+    (1, 1, 40, 20, [1, 3, 5], [1, 2, 7], [2, 4, 8], 32),       # ragged: non-pow2 nchan / widths, stride > w
+    (2, 1, 33, 5, [2, 4], [1, 3], [2, 4], 8),                  # tiny planes (M*nf < 32 path), nt == w
+    (1, 2, 10, 8, [4, 16], [1, 1], [8, 16], 8),                # nap < w for one width -> zero windows
+    (1, 1, 70, 64, [8], [4], [64], 64),                        # pad x8 in time
+    (1, 1, 50, 3, [2], [1], [4], 4),                           # nf = 4
+    (1, 1, 17, 1, [4], [1], [8], 1),                           # single channel, nf = 1
+    (1, 1, 300, 100, [32, 64], [5, 9], [64, 128], 512),        # big nf, odd strides
+])
+def test_edge_shapes(vb, oracle, shape):
+    nbl, nif, nap, nchan, widths, strides, nts, nf = shape
+    g = torch.Generator().manual_seed(nap * 7 + nchan)
+    vis = torch.view_as_complex(torch.randn((nbl, nif, nap, nchan, 2), generator=g) * 0.7071)
+    c = dict(widths=widths, strides=strides, nts=nts, nf=nf, snr_thresh=2.5)
+    run_both(vb, oracle, vis, c, mode="fft")
+
+
+def test_zero_windows_and_empty(vb):
+    vis = torch.zeros((1, 1, 3, 8), dtype=torch.complex64)
+    cands, n, peaks = vb.fringe_search(vis.cuda(), [4], [1], [8], 8, 6.0, want_peaks=True)
+    assert n == 0 and len(cands) == 0 and len(peaks) == 0
+
+
+def test_degenerate_inputs_tie_break(vb, oracle):
+    """A8: all-zero windows (snr 0, argmax (0,0)); a delta input (constant plane -> (0,0), snr 1);
+    w = 1 (identical rate rows -> r* = 0)."""
+    vis = torch.zeros((1, 1, 64, 32), dtype=torch.complex64)
+    vis[0, 0, 20, 7] = 2 - 1j
+    c = dict(widths=[1, 8], strides=[1, 1], nts=[2, 16], nf=64, snr_thresh=0.5)
+    cands, n, peaks = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], 0.5, want_peaks=True)
+    assert np.all(peaks["rate_idx"] == 0) and np.all(peaks["delay_idx"] == 0)
+    hit = peaks["power"] > 0
+    assert np.allclose(peaks["power"][hit], 5.0, rtol=1e-6) and np.allclose(peaks["snr"][hit], 1.0, rtol=1e-6)
+    assert np.all(peaks["snr"][~hit] == 0) and hit.sum() == 1 + 8 and n == 9
+    g = torch.Generator().manual_seed(3)
+    v1 = torch.view_as_complex(torch.randn((1, 1, 50, 32, 2), generator=g))
+    cands, n, peaks = vb.fringe_search(v1.cuda(), [1], [1], [2], 128, 6.0, want_peaks=True)
+    assert np.all(peaks["rate_idx"] == 0)
+    ora, _ = oracle.search(v1.numpy(), [1], [1], [2], 128, mode="fft")
+    assert np.array_equal(peaks["delay_idx"], ora["idx1"] % 128)
+
+
+def test_capacity_overflow_and_determinism(vb):
+    vis, c, _ = workloads.generate(1, nap=500)
+    v = vis.cuda()
+    a, na, pa = vb.fringe_search(v, c["widths"], c["strides"], c["nts"], c["nf"], 3.0, want_peaks=True)
+    b, nb, pb = vb.fringe_search(v, c["widths"], c["strides"], c["nts"], c["nf"], 3.0, want_peaks=True)
+    assert na == nb and a.tobytes() == b.tobytes() and pa.tobytes() == pb.tobytes()   # bit-identical
+    assert na > 10
+    s, ns, _ = vb.fringe_search(v, c["widths"], c["strides"], c["nts"], c["nf"], 3.0, cand_capacity=7)
+    assert ns == na and len(s) == 7 and s.tobytes() == a[:7].tobytes()                # true count, first 7
+    z, nz, _ = vb.fringe_search(v, c["widths"], c["strides"], c["nts"], c["nf"], 3.0, cand_capacity=0)
+    assert nz == na and len(z) == 0
+
+
+def test_peaks_optional_same_candidates(vb):
+    vis, c, _ = workloads.generate(0)
+    a, na, _ = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], 6.0, want_peaks=False)
+    b, nb, _ = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], 6.0, want_peaks=True)
+    assert na == nb and a.tobytes() == b.tobytes()
+
+
+def test_non_default_stream(vb):
+    vis, c, _ = workloads.generate(0)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        a, na, _ = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], 6.0)
+    b, nb, _ = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], 6.0)
+    assert na == nb and a.tobytes() == b.tobytes()
+
+
+def test_cpu_tensor_is_rejected_loudly(vb):
+    vis, c, _ = workloads.generate(0)
+    with pytest.raises(RuntimeError):
+        vb.fringe_search(vis, c["widths"], c["strides"], c["nts"], c["nf"], 6.0)
+
+
+def test_window_match_on_gpu_candidates(vb, oracle):
+    vis, c, _ = workloads.generate(1)
+    cands, n, _ = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], 4.0)
+    got = vb.window_match(cands, c["widths"], 2)
+    oc = np.zeros(len(cands), dtype=oracle.CAND_DTYPE)
+    for k in ("bl", "ifq", "wid", "win", "t0", "snr"):
+        oc[k] = cands[k]
+    exp = oracle.window_match(oc, c["widths"], 2)
+    assert len(got) == len(exp) and len(got) >= 1
+    for g, e in zip(got, exp):
+        assert g["best"].tobytes() == cands[int(e["rep"])].tobytes()
+        assert (g["nwidths_hit"], g["t_begin"], g["t_end"]) == (e["nwidths_hit"], e["t_begin"], e["t_end"])
