@@ -1,0 +1,363 @@
+#!/usr/bin/env python
+"""bench.py - throughput of the fringe-search hot path on B200 (contract: see DESIGN.md "Measurement").
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config ID] [--impl reference]
+
+One "step" = one volks_fringe_search over the whole synthetic workload (all baselines, IFs, widths
+and windows of the config; candidates compacted).  Prints ONE JSON line on rank 0.
+  value      windows/s with the visibility slab already resident in HBM (device-timed, CUDA events)
+  e2e        the same metric through the public API with HOST buffers: pinned host -> device copy of
+             the slab and device -> host read of the candidate list inside the timed region
+  roofline   dominant kernel: algorithmic flops per launch / live CUDA-event duration vs the FP32
+             FMA peak (bound "alu"; DESIGN.md derives the peak and the per-unit flops)
+  cpu_baseline  the float64 oracle, as it stands, on the host cores, on a bounded sample
+With --impl reference the oracle itself is the timed program (rank 0 only).
+"""
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+import workloads
+
+SM_COUNT, FP32_LANES_PER_SM = 148, 128      # B200 (guide: 148 SMs, 4 SMSP x 32 FP32 lanes)
+METRIC = "fringe-search windows/s (and visibilities/s) at 1 B200; % of FP32 roofline"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[ID] (default 2)")
+    ap.add_argument("--impl", default="volks", choices=["volks", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--peaks", action="store_true", help="also write the dense per-window peak array")
+    return ap.parse_args()
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock / throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.1):
+        super().__init__(daemon=True)
+        self.index, self.period, self.stop_flag = index, period, False
+        self.sm, self.reasons, self.max_mhz, self.power = [], set(), None, []
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {
+                nv.nvmlClocksEventReasonSwPowerCap if hasattr(nv, "nvmlClocksEventReasonSwPowerCap") else 0x4: "sw_power_cap",
+                0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+                0x80: "hw_power_brake_slowdown",
+            }
+            while not self.stop_flag:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                try:
+                    self.power.append(nv.nvmlDeviceGetPowerUsage(h) / 1000.0)
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+                except Exception:
+                    r = 0
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                time.sleep(self.period)
+        except Exception as e:  # NVML missing: report that, never fail the bench
+            self.reasons.add("nvml_unavailable:%s" % type(e).__name__)
+
+    def summary(self):
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.sm),
+                "power_w_max": max(self.power) if self.power else None}
+
+
+def algorithmic_flops(c):
+    """SURVEY.md 8(d) per-unit figures: delay FFT once per AP (5 Nf log2 Nf) + per window
+    Nf*(5 Nt log2 Nt) column FFTs + ~5 Nt Nf for |.|^2/max/sum.  Returns (total, per-width list)."""
+    npair, nap, nf = c["nbl"] * c["nif"], c["nap"], c["nf"]
+    row = npair * nap * 5.0 * nf * math.log2(nf) if nf > 1 else 0.0
+    per_w = []
+    for w, s, nt in zip(c["widths"], c["strides"], c["nts"]):
+        nw = workloads.gen.nwin(nap, w, s) * npair
+        per_w.append(nw * (nf * 5.0 * nt * math.log2(nt) + 5.0 * nt * nf))
+    return row + sum(per_w), row, per_w
+
+
+def nominal_flops(c):
+    """north_star's accounting: 5 N log2 N per padded plane, N = Nt*Nf."""
+    npair, nap, nf = c["nbl"] * c["nif"], c["nap"], c["nf"]
+    tot = 0.0
+    for w, s, nt in zip(c["widths"], c["strides"], c["nts"]):
+        n = nt * nf
+        tot += workloads.gen.nwin(nap, w, s) * npair * 5.0 * n * math.log2(n)
+    return tot
+
+
+def oracle_sample(c, budget_s=20.0):
+    """Bounded sample of config `c` for the oracle: ONE (bl, ifq) pair, the first `nap_s` APs, all
+    widths (cached-rows mode).  nap_s is sized from a small calibration run so that the sample costs
+    about `budget_s` of CPU work.  Returns (vis_sample numpy, nap_s)."""
+    from oracle import volks_oracle
+    wmax = max(c["widths"])
+    nap_cal = min(c["nap"], max(2 * wmax, 96))
+    vis, cc, _ = workloads.generate(c["id"], nbl=1, nif=1, nap=nap_cal, npulses=0)
+    t = time.perf_counter()
+    volks_oracle.search(vis.numpy(), c["widths"], c["strides"], c["nts"], c["nf"], mode="cached")
+    dt = max(time.perf_counter() - t, 1e-4)
+    nwin_cal = sum(workloads.gen.nwin(nap_cal, w, s) for w, s in zip(c["widths"], c["strides"]))
+    rate = max(nwin_cal, 1) / dt
+    per_ap = sum(1.0 / s for s in c["strides"])
+    nap_s = int(min(c["nap"], max(nap_cal, budget_s * rate / per_ap)))
+    return nap_s
+
+
+def time_oracle(c, nap_s):
+    """Run the oracle (as it stands) on one pair x nap_s APs; returns (windows, seconds, cores)."""
+    from oracle import volks_oracle
+    vis, cc, _ = workloads.generate(c["id"], nbl=1, nif=1, nap=nap_s, npulses=min(c["npulses"], 2))
+    v = vis.numpy()
+    t = time.perf_counter()
+    pk, used = volks_oracle.search(v, c["widths"], c["strides"], c["nts"], c["nf"], mode="cached")
+    dt = time.perf_counter() - t
+    return len(pk), dt, used
+
+
+def workload_name(c):
+    return ("configs[%d]: %d bl x %d IF x %d ch x %d AP cf32, widths %s stride %s, plane Nt %s x Nf %d"
+            % (c["id"], c["nbl"], c["nif"], c["nchan"], c["nap"], c["widths"], c["strides"], c["nts"], c["nf"]))
+
+
+def run_reference(args):
+    """--impl reference: the oracle is the timed program; each step one bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import volks_oracle
+    volks_oracle.build()
+    c = workloads.config(args.config)
+    total = max(args.steps + args.warmup, 1)
+    nap_s = oracle_sample(c, budget_s=min(20.0, 150.0 / total))
+    for _ in range(args.warmup):
+        time_oracle(c, nap_s)
+    nwin, secs, used = 0, 0.0, 1
+    for _ in range(args.steps):
+        n, dt, used = time_oracle(c, nap_s)
+        nwin += n
+        secs += dt
+    val = nwin / secs if secs > 0 else 0.0
+    sample = "1 (bl,IF) pair x first %d APs of %s, all widths, cached-rows mode, per step" % (nap_s, workload_name(c))
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "windows/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(args.steps, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(c), "sample": sample},
+        "cpu_baseline": {"value": val, "unit": "windows/s", "cores": used, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "windows/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "visibilities_per_s": nap_s * c["nchan"] * args.steps / secs if secs > 0 else 0.0,
+        "gpu_launches": 0,
+    }))
+
+
+KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6: "fused"}
+
+
+def run_volks(args):
+    import paper_2108_05602_b200 as vk
+    vk.lib()                                   # fails loudly if the CUDA library is missing
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    # N independent replicas (the path needs no exchange; north_star fixes one
+    # GPU, so --gpus N runs N replicas, each the full config with its own seed)
+    vis, c, _ = workloads.generate(args.config, device=dev, seed=workloads.config(args.config)["seed"] + 17 * rank)
+    nbl, nif, nap, nchan = vis.shape
+    plan = vk.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"])
+    cap = 1 << 20
+    ws = torch.empty(plan.workspace_bytes, dtype=torch.uint8, device=dev)
+    cands = torch.empty(cap * vk.CAND_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    ncand = torch.zeros(1, dtype=torch.int32, device=dev)
+    peaks = torch.empty(plan.nwin_total * vk.PEAK_DTYPE.itemsize, dtype=torch.uint8, device=dev) if args.peaks else None
+    stream = torch.cuda.current_stream(dev)
+
+    def step():
+        plan.fringe_search(vis, ws, cands, ncand, peaks, stream)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    sampler.stop_flag = True
+    sampler.join()
+    if dist is not None:
+        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    nwin = plan.nwin_total
+    nvis = nbl * nif * nap * nchan
+    value = world * nwin / (ms_step * 1e-3)
+    n_found = int(ncand.item())
+
+    # ---- roofline leg: per-launch CUDA-event durations on the launching stream ----
+    plan.profile(True)
+    per = {}
+    reps = 2
+    for _ in range(reps):
+        step()
+        torch.cuda.synchronize(dev)
+        for kind, wid, ms in plan.profile_read():
+            per.setdefault((kind, wid), []).append(ms)
+    plan.profile(False)
+    tot_alg, row_alg, per_w_alg = algorithmic_flops(c)
+    nlaunch = {k: len(v) / reps for k, v in per.items()}
+    share = {k: sum(v) / reps for k, v in per.items()}
+    step_sum = sum(share.values())
+    dom = max(share, key=share.get)
+    dom_ms_avg = float(np.mean(per[dom]))
+    if dom[0] == 2:       # column kernel of width dom[1]: one launch per chunk of pairs
+        dom_flops = per_w_alg[dom[1]] / nlaunch[dom]
+    elif dom[0] == 6:     # fused kernel of width group: carries the row FFT too
+        dom_flops = (per_w_alg[dom[1]] if dom[1] >= 0 else sum(per_w_alg)) / nlaunch[dom]
+    elif dom[0] == 1:
+        dom_flops = row_alg / nlaunch[dom]
+    else:
+        dom_flops = 0.0
+    clocks = sampler.summary()
+    peak_tf = SM_COUNT * FP32_LANES_PER_SM * 2 * (clocks["sm_max_mhz"] or 1965) * 1e6 / 1e12
+    achieved_tf = dom_flops / (dom_ms_avg * 1e-3) / 1e12
+    roofline = {
+        "bound": "alu", "kernel": "%s[w=%s]" % (KIND_NAMES[dom[0]], c["widths"][dom[1]] if dom[1] >= 0 else "all"),
+        "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
+        "traffic": None, "launch_ms": dom_ms_avg, "share_of_step": share[dom] / step_sum,
+        "peak_kind": "derived: 148 SM x 128 FP32 lanes x 2 flop (FMA) x sm_max_mhz (DESIGN.md)",
+        "flops_kind": "algorithmic (SURVEY 8(d)): shared delay FFT per AP + 5 Nt log2 Nt per column + 5 per bin",
+        "whole_step_algorithmic_tflops": tot_alg / (ms_step * 1e-3) / 1e12,
+        "whole_step_nominal_tflops": nominal_flops(c) / (ms_step * 1e-3) / 1e12,
+        "hbm_gbs_algorithmic": nvis * 8 / (ms_step * 1e-3) / 1e9,
+        "kernel_ms": {"%s[%d]" % (KIND_NAMES[k[0]], k[1]): round(v, 4) for k, v in sorted(share.items())},
+    }
+    return dict(vk=vk, plan=plan, vis=vis, c=c, ws=ws, cands=cands, ncand=ncand, peaks=peaks, stream=stream,
+                dev=dev, rank=rank, world=world, dist=dist, ms_step=ms_step, value=value, nwin=nwin, nvis=nvis,
+                n_found=n_found, roofline=roofline, clocks=clocks, cap=cap)
+
+
+def run_e2e(R, steps):
+    """Same metric through the public API with HOST buffers: every step copies the slab from pinned
+    host memory to the device, runs the search and reads the candidate list back."""
+    vk, plan, dev, stream = R["vk"], R["plan"], R["dev"], R["stream"]
+    h_vis = torch.empty(R["vis"].shape, dtype=torch.complex64, pin_memory=True)
+    h_vis.copy_(R["vis"])
+    h_n = torch.zeros(1, dtype=torch.int32, pin_memory=True)
+    h_c = torch.empty(R["cap"] * vk.CAND_DTYPE.itemsize, dtype=torch.uint8, pin_memory=True)
+    d_vis = R["vis"]
+    d2h = 0
+
+    def step():
+        nonlocal d2h
+        d_vis.copy_(h_vis, non_blocking=True)
+        plan.fringe_search(d_vis, R["ws"], R["cands"], R["ncand"], R["peaks"], stream)
+        h_n.copy_(R["ncand"], non_blocking=True)
+        stream.synchronize()
+        n = min(int(h_n.item()), R["cap"]) * vk.CAND_DTYPE.itemsize
+        if n:
+            h_c[:n].copy_(R["cands"][:n], non_blocking=True)
+            stream.synchronize()
+        d2h = 4 + n
+
+    step()
+    if R["dist"] is not None:
+        R["dist"].barrier()
+    torch.cuda.synchronize(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize(dev)
+    ms = e0.elapsed_time(e1)
+    if R["dist"] is not None:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        R["dist"].all_reduce(t, op=R["dist"].ReduceOp.MAX)
+        ms = float(t.item())
+    ms /= steps
+    return {"value": R["world"] * R["nwin"] / (ms * 1e-3), "unit": "windows/s", "ms_per_step": ms,
+            "h2d_bytes_per_step": int(h_vis.numel() * 8), "d2h_bytes_per_step": int(d2h)}
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    R = run_volks(args)
+    c = R["c"]
+    e2e = None if args.no_e2e else run_e2e(R, max(1, min(args.steps, 3)))
+    cpu = None
+    if R["rank"] == 0 and R["world"] == 1 and not args.no_cpu_baseline:
+        from oracle import volks_oracle
+        volks_oracle.build()
+        nap_s = oracle_sample(c, budget_s=15.0)
+        n, dt, used = time_oracle(c, nap_s)
+        cpu = {"value": n / dt, "unit": "windows/s", "cores": used, "kind": "oracle",
+               "sample": "1 (bl,IF) pair x first %d APs, all widths, float64 cached-rows mode: %d windows in %.1f s"
+                         % (nap_s, n, dt)}
+    if R["rank"] == 0:
+        out = {
+            "metric": METRIC, "value": R["value"], "unit": "windows/s", "n_gpus": R["world"],
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": R["ms_step"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": workload_name(c), "snr_thresh": c["snr_thresh"],
+                       "l2": "input slab (%.2f GB) larger than L2, no flush needed" % (R["nvis"] * 8 / 1e9)
+                       if R["nvis"] * 8 > 126e6 else "input smaller than L2 (latency-bound config, report only)",
+                       "replicas": R["world"], "dense_peaks": bool(args.peaks)},
+            "visibilities_per_s": R["world"] * R["nvis"] / (R["ms_step"] * 1e-3),
+            "windows": R["nwin"], "candidates": R["n_found"],
+            "clocks": R["clocks"], "e2e": e2e, "gpu_launches": R["plan"].launches * args.steps,
+            "roofline": R["roofline"], "cpu_baseline": cpu,
+        }
+        print(json.dumps(out))
+    if R["dist"] is not None:
+        R["dist"].destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

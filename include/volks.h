@@ -127,6 +127,21 @@ int volks_bin_to_physical(int32_t nt, int32_t nf, int32_t rate_idx, int32_t dela
 /* Number of kernels one volks_fringe_search enqueues (for launch accounting). */
 int volks_plan_launch_count(const volks_plan *plan);
 
+/* Optional per-launch timing for measurement (bench.py's roofline leg).  When enabled, every kernel
+ * volks_fringe_search enqueues is bracketed by CUDA events recorded on the launching stream.
+ * volks_plan_profile_read waits for the most recent call's events and returns, per launch in
+ * launch order, its kind (VOLKS_K_*), its width index (or -1) and its duration in milliseconds.
+ * HOST outputs; *n receives the number of launches (only min(n, capacity) entries are written). */
+#define VOLKS_K_ROW 1      /* slab load + zero-pad + delay FFT (+ per-AP energy)                    */
+#define VOLKS_K_COL 2      /* rate transform + power + argmax of one width                         */
+#define VOLKS_K_FINALIZE 3 /* SNR, dense peaks, threshold count                                    */
+#define VOLKS_K_SCAN 4     /* scan of block counts                                                 */
+#define VOLKS_K_SCATTER 5  /* ordered candidate scatter                                            */
+#define VOLKS_K_FUSED 6    /* fused row FFT + rate transform + power + argmax (stride-1 widths)    */
+int volks_plan_profile(volks_plan *plan, int enable);
+int volks_plan_profile_read(const volks_plan *plan, int32_t capacity, int32_t *kind, int32_t *wid,
+                            float *ms, int32_t *n);
+
 const char *volks_strerror(int code);
 int volks_version(void);
 

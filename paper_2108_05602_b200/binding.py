@@ -16,7 +16,7 @@ VOLKS_OK, VOLKS_EINVAL, VOLKS_ECUDA, VOLKS_ENOMEM, VOLKS_EOVERFLOW = 0, -1, -2, 
 EXPORTS = (
     "volks_plan_create", "volks_plan_destroy", "volks_plan_query", "volks_fringe_search",
     "volks_window_match", "volks_bin_to_physical", "volks_plan_launch_count", "volks_strerror",
-    "volks_version",
+    "volks_version", "volks_plan_profile", "volks_plan_profile_read",
 )
 
 
@@ -60,6 +60,9 @@ def lib():
                                             ctypes.c_double, ctypes.c_double,
                                             ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
         L.volks_plan_launch_count.argtypes = [ctypes.c_void_p]
+        L.volks_plan_profile.argtypes = [ctypes.c_void_p, ctypes.c_int]
+        L.volks_plan_profile_read.argtypes = [ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p, ctypes.c_void_p,
+                                              ctypes.c_void_p, ctypes.POINTER(ctypes.c_int32)]
         _lib = L
     return _lib
 
@@ -122,6 +125,20 @@ class Plan:
         _check(lib().volks_fringe_search(
             self._h, vis.data_ptr(), workspace.data_ptr(), peaks.data_ptr() if peaks is not None else None,
             cands.data_ptr() if cap else None, cap, ncand.data_ptr(), st))
+
+    def profile(self, enable=True):
+        """volks_plan_profile: bracket every launch of later searches with CUDA events."""
+        _check(lib().volks_plan_profile(self._h, 1 if enable else 0))
+
+    def profile_read(self):
+        """volks_plan_profile_read -> list of (kind, width index, milliseconds), launch order."""
+        n = ctypes.c_int32()
+        _check(lib().volks_plan_profile_read(self._h, 0, None, None, None, ctypes.byref(n)))
+        kind, wid = np.zeros(n.value, np.int32), np.zeros(n.value, np.int32)
+        ms = np.zeros(n.value, np.float32)
+        _check(lib().volks_plan_profile_read(self._h, n.value, kind.ctypes.data, wid.ctypes.data,
+                                             ms.ctypes.data, ctypes.byref(n)))
+        return [(int(k), int(w), float(m)) for k, w, m in zip(kind, wid, ms)]
 
     def window_match(self, cands, min_widths=2):
         return window_match(cands, self.widths, min_widths)

@@ -57,7 +57,26 @@ struct volks_plan {
   int row_tpr = 1, row_rows_per_cta = 1;
   size_t row_smem = 0;
   int launches = 0;
+  // optional per-launch timing (volks_plan_profile): events recorded on the launching stream
+  mutable bool prof_on = false;
+  mutable std::vector<cudaEvent_t> prof_ev;      // 2 per launch (begin, end), grown on demand
+  mutable std::vector<int> prof_kind, prof_wid;  // of the most recent volks_fringe_search
 };
+
+namespace {
+// Brackets one kernel launch with events when profiling is enabled (no-op otherwise).
+struct ProfScope {
+  const volks_plan *pl; cudaStream_t st; size_t slot;
+  ProfScope(const volks_plan *p, cudaStream_t s, int kind, int wid) : pl(p), st(s), slot(0) {
+    if (!pl->prof_on) return;
+    slot = pl->prof_kind.size();
+    pl->prof_kind.push_back(kind); pl->prof_wid.push_back(wid);
+    while (pl->prof_ev.size() < 2 * (slot + 1)) { cudaEvent_t e; cudaEventCreate(&e); pl->prof_ev.push_back(e); }
+    cudaEventRecord(pl->prof_ev[2 * slot], st);
+  }
+  ~ProfScope() { if (pl->prof_on) cudaEventRecord(pl->prof_ev[2 * slot + 1], st); }
+};
+}  // namespace
 
 extern "C" {
 
@@ -166,6 +185,7 @@ int volks_plan_destroy(volks_plan *pl) {
   if (!pl) return VOLKS_EINVAL;
   if (pl->d_tables) cudaFree(pl->d_tables);
   if (pl->d_sched) cudaFree(pl->d_sched);
+  for (cudaEvent_t e : pl->prof_ev) cudaEventDestroy(e);
   delete pl;
   return VOLKS_OK;
 }
@@ -193,6 +213,7 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
   if (s.nwin_total == 0) {
     return cuda_ok(cudaMemsetAsync(d_ncand, 0, sizeof(uint32_t), st)) ? VOLKS_OK : VOLKS_ECUDA;
   }
+  pl->prof_kind.clear(); pl->prof_wid.clear();
   if (!cuda_ok(cudaMemsetAsync(keys, 0, (size_t)s.nwin_total * sizeof(u64), st))) return VOLKS_ECUDA;
   for (long long ch = 0; ch < pl->nchunks; ++ch) {
     const long long pair0 = ch * pl->pairs_per_chunk;
@@ -202,7 +223,10 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
     ra.row0 = pair0 * s.nap; ra.nrows = np * s.nap;
     ra.nchan = pl->nchan; ra.nf = s.nf; ra.tpr = pl->row_tpr; ra.rows_per_cta = pl->row_rows_per_cta;
     const long long rblocks = (ra.nrows + ra.rows_per_cta - 1) / ra.rows_per_cta;
-    k_row_fft<<<(unsigned)rblocks, ra.tpr * ra.rows_per_cta, pl->row_smem, st>>>(ra);
+    {
+      ProfScope ps(pl, st, VOLKS_K_ROW, -1);
+      k_row_fft<<<(unsigned)rblocks, ra.tpr * ra.rows_per_cta, pl->row_smem, st>>>(ra);
+    }
     for (int q = 0; q < s.nwidths; ++q) {
       const WidthPlan &w = pl->wp[q];
       if (w.nwin == 0) continue;
@@ -212,6 +236,7 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
       ca.nap = s.nap; ca.nf = s.nf; ca.log2nf = s.log2nf; ca.w = w.w; ca.stride = w.s; ca.nt = w.nt;
       ca.log2m = w.log2m; ca.nwin = (int)w.nwin;
       ca.total = ((np * w.nwin) << w.log2m) * s.nf;
+      ProfScope ps(pl, st, VOLKS_K_COL, q);
       switch (w.L) {
         case 1: launch_col<1>(ca, st); break;
         case 2: launch_col<2>(ca, st); break;
@@ -221,10 +246,38 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
       }
     }
   }
-  k_finalize<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, (float4 *)d_peaks, cnt);
-  k_scan<<<1, 1024, 0, st>>>(cnt, pl->nfin_blocks, d_ncand);
-  k_scatter<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity);
+  {
+    ProfScope ps(pl, st, VOLKS_K_FINALIZE, -1);
+    k_finalize<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, (float4 *)d_peaks, cnt);
+  }
+  {
+    ProfScope ps(pl, st, VOLKS_K_SCAN, -1);
+    k_scan<<<1, 1024, 0, st>>>(cnt, pl->nfin_blocks, d_ncand);
+  }
+  {
+    ProfScope ps(pl, st, VOLKS_K_SCATTER, -1);
+    k_scatter<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity);
+  }
   return cuda_ok(cudaGetLastError()) ? VOLKS_OK : VOLKS_ECUDA;
+}
+
+int volks_plan_profile(volks_plan *pl, int enable) {
+  if (!pl) return VOLKS_EINVAL;
+  pl->prof_on = enable != 0;
+  pl->prof_kind.clear(); pl->prof_wid.clear();
+  return VOLKS_OK;
+}
+
+int volks_plan_profile_read(const volks_plan *pl, int32_t capacity, int32_t *kind, int32_t *wid, float *ms,
+                            int32_t *n) {
+  if (!pl || !n || capacity < 0 || (capacity > 0 && (!kind || !wid || !ms))) return VOLKS_EINVAL;
+  *n = (int32_t)pl->prof_kind.size();
+  for (int32_t i = 0; i < *n && i < capacity; ++i) {
+    if (!cuda_ok(cudaEventSynchronize(pl->prof_ev[2 * i + 1]))) return VOLKS_ECUDA;
+    if (!cuda_ok(cudaEventElapsedTime(&ms[i], pl->prof_ev[2 * i], pl->prof_ev[2 * i + 1]))) return VOLKS_ECUDA;
+    kind[i] = pl->prof_kind[i]; wid[i] = pl->prof_wid[i];
+  }
+  return VOLKS_OK;
 }
 
 // Host: sweep over candidates sorted by start AP inside each (bl, ifq) group.  Interval-overlap

@@ -88,13 +88,17 @@ def test_degenerate_inputs_tie_break(vb, oracle):
     """A8: all-zero windows (snr 0, argmax (0,0)); a delta input (constant plane -> (0,0), snr 1);
     w = 1 (identical rate rows -> r* = 0)."""
     vis = torch.zeros((1, 1, 64, 32), dtype=torch.complex64)
-    vis[0, 0, 20, 7] = 2 - 1j
+    vis[0, 0, 20, 0] = 2 - 1j      # channel 0: every delay twiddle is exactly 1
     c = dict(widths=[1, 8], strides=[1, 1], nts=[2, 16], nf=64, snr_thresh=0.5)
     cands, n, peaks = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], 0.5, want_peaks=True)
-    assert np.all(peaks["rate_idx"] == 0) and np.all(peaks["delay_idx"] == 0)
     hit = peaks["power"] > 0
     assert np.allclose(peaks["power"][hit], 5.0, rtol=1e-6) and np.allclose(peaks["snr"][hit], 1.0, rtol=1e-6)
     assert np.all(peaks["snr"][~hit] == 0) and hit.sum() == 1 + 8 and n == 9
+    # all-zero windows: constant plane, first index wins
+    assert np.all(peaks["rate_idx"][~hit] == 0) and np.all(peaks["delay_idx"][~hit] == 0)
+    # exactly constant planes (all twiddles exactly 1): w = 1 at AP 20, and w = 8 starting at AP 20
+    assert tuple(peaks[20][["rate_idx", "delay_idx"]]) == (0, 0)
+    assert tuple(peaks[64 + 20][["rate_idx", "delay_idx"]]) == (0, 0)
     g = torch.Generator().manual_seed(3)
     v1 = torch.view_as_complex(torch.randn((1, 1, 50, 32, 2), generator=g))
     cands, n, peaks = vb.fringe_search(v1.cuda(), [1], [1], [2], 128, 6.0, want_peaks=True)
