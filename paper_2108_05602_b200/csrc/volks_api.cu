@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "kernels_generic.cuh"
+#include "kernels_slide.cuh"
 
 using namespace volks;
 
@@ -32,12 +33,35 @@ struct WidthPlan {
   int w, s, nt, L, log2m;
   long long nwin;       // per pair
   size_t tw_off;        // offset (float2) of its rate twiddle table in d_tables
+  bool slide;           // stride-1 sliding-sum kernel (kernels_slide.cuh) instead of the generic one
+  int seg, nseg;        // sliding path: windows per exactly restarted segment, segments per pair
 };
+
+// Tuning / test switches read once per plan (documented in DESIGN.md "Kernel selection"):
+//   VOLKS_PATH=generic   force the generic multi-pass kernels for every width
+//   VOLKS_SLIDE_SEG=n    windows per restarted segment of the sliding kernel (default 256)
+int env_int(const char *name, int dflt) {
+  const char *v = getenv(name);
+  return v && *v ? atoi(v) : dflt;
+}
+bool env_is(const char *name, const char *val) {
+  const char *v = getenv(name);
+  return v && strcmp(v, val) == 0;
+}
 
 template <int L>
 static void launch_col(const ColArgs &a, cudaStream_t st) {
   const long long blocks = (a.total + 255) / 256;
   k_col<L><<<(unsigned)blocks, 256, 0, st>>>(a);
+}
+
+static void launch_slide(const SlideArgs &a, cudaStream_t st) {
+  const unsigned blocks = (unsigned)((a.ntasks + SLIDE_WARPS - 1) / SLIDE_WARPS);
+  const int thr = SLIDE_WARPS * 32;
+  if (a.nt >= 32) k_slide<16, false><<<blocks, thr, 0, st>>>(a);
+  else if (a.nt == 16) k_slide<16, true><<<blocks, thr, 0, st>>>(a);
+  else if (a.nt == 8) k_slide<8, true><<<blocks, thr, 0, st>>>(a);
+  else k_slide<4, true><<<blocks, thr, 0, st>>>(a);
 }
 
 }  // namespace
@@ -114,12 +138,19 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
   pl->npair = (long long)p->nbl * p->nif;
   long long per_pair = 0;
   size_t tw_total = (size_t)p->nf;
+  const bool force_generic = env_is("VOLKS_PATH", "generic");
+  const int seg_req = std::max(16, env_int("VOLKS_SLIDE_SEG", 256));
   for (int q = 0; q < p->nwidths; ++q) {
     WidthPlan w;
     w.w = p->width[q]; w.s = p->stride[q]; w.nt = p->nt[q];
     w.nwin = p->nap < w.w ? 0 : (long long)(p->nap - w.w) / w.s + 1;
     w.L = std::min(16, w.nt);
     w.log2m = ilog2(w.nt / w.L);
+    // sliding-sum path: stride 1, pad x2 in time, whole warps of delay columns, 32-bit row offsets
+    w.slide = !force_generic && w.s == 1 && w.w >= 2 && w.nt == 2 * w.w && p->nf >= 32 &&
+              (long long)p->nap * p->nf < (1LL << 32);
+    w.seg = std::max((seg_req / w.nt) * w.nt, w.nt);
+    w.nseg = w.nwin > 0 ? (int)((w.nwin + w.seg - 1) / w.seg) : 0;
     w.tw_off = tw_total;
     tw_total += (size_t)w.nt;
     s.width[q] = w.w; s.stride[q] = w.s; s.nt[q] = w.nt; s.nwin[q] = w.nwin; s.offc[q] = per_pair;
@@ -236,6 +267,17 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
       ca.nap = s.nap; ca.nf = s.nf; ca.log2nf = s.log2nf; ca.w = w.w; ca.stride = w.s; ca.nt = w.nt;
       ca.log2m = w.log2m; ca.nwin = (int)w.nwin;
       ca.total = ((np * w.nwin) << w.log2m) * s.nf;
+      if (w.slide) {
+        SlideArgs sa;
+        sa.Y = Y; sa.keys = keys; sa.twt = pl->d_tables + w.tw_off;
+        sa.per_pair = s.per_pair; sa.offc = s.offc[q]; sa.pair0 = pair0;
+        sa.nap = s.nap; sa.nf = s.nf; sa.w = w.w; sa.nt = w.nt; sa.log2m = w.log2m; sa.nwin = (int)w.nwin;
+        sa.seg = w.seg; sa.nseg = w.nseg;
+        sa.ntasks = ((np * w.nseg * (long long)(s.nf / 32)) << w.log2m);
+        ProfScope ps(pl, st, VOLKS_K_SLIDE, q);
+        launch_slide(sa, st);
+        continue;
+      }
       ProfScope ps(pl, st, VOLKS_K_COL, q);
       switch (w.L) {
         case 1: launch_col<1>(ca, st); break;
