@@ -26,6 +26,9 @@
 namespace volks {
 
 constexpr int SLIDE_WARPS = 8;   // warps per CTA
+#ifndef SLIDE_MIN_CTAS
+#define SLIDE_MIN_CTAS 2        // register cap 128 (no spills); measured: 2 and 4 within 3 %, 3 slower
+#endif
 
 struct SlideArgs {
   const float2 *Y;      // [npairs_chunk][nap][nf] delay spectra
@@ -36,6 +39,7 @@ struct SlideArgs {
   long long offc;       // canonical offset of this width inside a pair
   long long pair0;      // first pair of the chunk
   int nap, nf, w, nt, log2m, nwin, seg, nseg;
+  uint32_t keymask;     // 0xFFFFFFF0, passed as data so that (p & mask) | id is ONE LOP3 (register mask)
 };
 
 // acc += exp(-2 pi i K16/16) * g, K16 a compile-time constant.  exp(-i th) g = (c gx + s gy, c gy - s gx).
@@ -61,35 +65,38 @@ __device__ __forceinline__ void cmac_w16(float2 &a, const float2 g) {
   }
 }
 
+// One warp's state while it walks a segment of consecutive windows.
+template <int L>
+struct SlideState {
+  float2 A[L];           // bins r = rho + M s of this lane's column, absolute-phase form
+  float2 yin, yout, tw;  // prefetched operands of the NEXT update (loaded one step ahead)
+  const char *pout;      // this lane's column of the pair's delay spectra, row 0
+  const char *pin;       // the same column, row w
+  const char *twt;
+  u64 *keyp;             // canonical key of window t0 = keyp[t0]
+  uint32_t rowb;         // bytes per Y row
+  uint32_t nf, ntmask, rho, log2m, d, keymask;
+  float sgn;             // (-1)^rho (used when M is even: every bin of the thread has rho's parity)
+};
+
 // Per-thread peak key of the L bins: power with its 4 low mantissa bits replaced by (15 - s), so one
 // unsigned max orders by (power descending, s ascending).  Relative power error <= 2^-19.
 template <int L>
-__device__ __forceinline__ uint32_t slide_local_key(const float2 (&A)[L]) {
+__device__ __forceinline__ uint32_t slide_local_key(const SlideState<L> &S) {
   uint32_t best = 0;
 #pragma unroll
   for (int s = 0; s < L; ++s) {
-    const float p = cnorm(A[s]);
-    const uint32_t k = (__float_as_uint(p) & 0xFFFFFFF0u) | (uint32_t)(15 - s);
+    const float p = cnorm(S.A[s]);
+    const uint32_t k = (__float_as_uint(p) & S.keymask) | (uint32_t)(15 - s);
     best = k > best ? k : best;
   }
   return best;
 }
 
-// One warp's state while it walks a segment of consecutive windows.
-template <int L>
-struct SlideState {
-  float2 A[L];           // bins r = rho + M s of this lane's column, absolute-phase form
-  const float2 *ybase;   // Y of this pair, at this lane's column
-  const float2 *twt;
-  u64 *keyp;             // canonical key of window t0 = keyp[t0]
-  uint32_t nf, w, ntmask, rho, log2m, d;
-  float sgn;             // (-1)^rho (used when M is even: every bin of the thread has rho's parity)
-};
-
 // emit the window's contribution: warp max of the local keys, winner lane(s) update the 64-bit key
 template <int L>
 __device__ __forceinline__ void slide_emit(const SlideState<L> &S, uint32_t t0) {
-  const uint32_t best = slide_local_key<L>(S.A);
+  const uint32_t best = slide_local_key<L>(S);
   const uint32_t km = __reduce_max_sync(0xffffffffu, best);
   if (best == km) {
     const uint32_t s = 15u - (km & 15u);
@@ -98,7 +105,7 @@ __device__ __forceinline__ void slide_emit(const SlideState<L> &S, uint32_t t0) 
   }
 }
 
-// acc[s] += W_L^{(s B) mod L} * g for every bin s of the thread (s, B compile time).  GE/GO: the
+// acc[s] += W_L^{(s B) mod L} * g for every bin s of the thread (s, B compile time).  ge / go: the
 // delta of even / odd rate bins (the same value when every bin of the thread has one parity).
 template <int L, int B, int S_>
 struct SlideBins {
@@ -111,11 +118,21 @@ struct SlideBins {
   }
 };
 
-// advance window t0 -> t0+1;  B = t0 mod L (compile time)
+// load the operands of the update t -> t+1 (rows t and t+w, warp-uniform twiddle W_Nt^{rho t})
+template <int L, bool MODD>
+__device__ __forceinline__ void slide_prefetch(SlideState<L> &S, uint32_t t) {
+  const uint32_t off = t * S.rowb;
+  S.yin = __ldg((const float2 *)(S.pin + off));
+  S.yout = __ldg((const float2 *)(S.pout + off));
+  if constexpr (!MODD) S.tw = __ldg((const float2 *)(S.twt + (((S.rho * t) & S.ntmask) << 3)));
+}
+
+// advance window t0 -> t0+1;  B = t0 mod L (compile time).  Uses the operands prefetched one step
+// ago and prefetches those of t0+1 (row t0+1+w <= nap: the Y buffer carries one padding row).
 template <int L, int B, bool MODD>
 __device__ __forceinline__ void slide_update(SlideState<L> &S, uint32_t t0) {
-  const float2 yin = __ldg(S.ybase + (size_t)((t0 + S.w) * S.nf));
-  const float2 yout = __ldg(S.ybase + (size_t)(t0 * S.nf));
+  const float2 yin = S.yin, yout = S.yout, tw = S.tw;
+  slide_prefetch<L, MODD>(S, t0 + 1);
   if constexpr (MODD) {
     // M == 1, rho == 0: the thread holds every rate bin, both parities; W_Nt = W_L
     const float2 ge = make_float2(yin.x - yout.x, yin.y - yout.y);
@@ -124,7 +141,6 @@ __device__ __forceinline__ void slide_update(SlideState<L> &S, uint32_t t0) {
   } else {
     // M even: every bin has rho's parity; g = W_Nt^{rho t0} ((-1)^rho y_in - y_out)
     const float2 dl = make_float2(fmaf(S.sgn, yin.x, -yout.x), fmaf(S.sgn, yin.y, -yout.y));
-    const float2 tw = __ldg(S.twt + ((S.rho * t0) & S.ntmask));
     const float2 g = cmul(dl, tw);
     SlideBins<L, B, 0>::run(S.A, g, g);
   }
@@ -146,7 +162,7 @@ struct SlideSteps {
 
 // L = min(16, Nt) bins per thread;  MODD <=> M == 1 (Nt <= 16).
 template <int L, bool MODD>
-__global__ void __launch_bounds__(SLIDE_WARPS * 32) k_slide(SlideArgs a) {
+__global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(SlideArgs a) {
   long long wt = (long long)blockIdx.x * SLIDE_WARPS + (threadIdx.x >> 5);
   if (wt >= a.ntasks) return;                     // whole warps only: no divergence inside a warp
   const uint32_t lane = threadIdx.x & 31u;
@@ -157,29 +173,33 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32) k_slide(SlideArgs a) {
   const int dt = (int)(wt % ndt); wt /= ndt;
   const int sg = (int)(wt % a.nseg);
   const long long pl = wt / a.nseg;
-  S.nf = (uint32_t)a.nf; S.w = (uint32_t)a.w; S.ntmask = (uint32_t)(a.nt - 1); S.log2m = (uint32_t)a.log2m;
+  S.nf = (uint32_t)a.nf; S.ntmask = (uint32_t)(a.nt - 1); S.log2m = (uint32_t)a.log2m;
   S.d = (uint32_t)(dt * 32) + lane;
   S.sgn = (S.rho & 1u) ? -1.f : 1.f;
-  S.ybase = a.Y + (size_t)pl * a.nap * a.nf + S.d;
-  S.twt = a.twt;
+  S.keymask = a.keymask;
+  S.rowb = (uint32_t)a.nf * 8u;
+  S.pout = (const char *)(a.Y + (size_t)pl * a.nap * a.nf + S.d);
+  S.pin = S.pout + (size_t)a.w * S.rowb;
+  S.twt = (const char *)a.twt;
   S.keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
   const uint32_t T0 = (uint32_t)sg * (uint32_t)a.seg;                 // multiple of Nt and of L
   const uint32_t tend = min((uint32_t)a.nwin, T0 + (uint32_t)a.seg);  // windows [T0, tend)
+  slide_prefetch<L, MODD>(S, T0);
 
-  // exact start: A[rho + M s] = sum_{t2<L} W_L^{s t2} a[t2],  a[t2] = sum_{t1} y[T0+t2+L t1] W_Nt^{rho (t2+L t1)}
+  // exact start: A[rho + M s] = sum_{t2<L} W_L^{s t2} f[t2],  f[t2] = sum_{t1} y[T0+t2+L t1] W_Nt^{rho (t2+L t1)}
   // (T0 = 0 mod Nt, so absolute and window-relative phases coincide here)
   {
     float2 f[L];
 #pragma unroll
     for (int i = 0; i < L; ++i) f[i] = make_float2(0.f, 0.f);
-    for (uint32_t tb = 0; tb < S.w; tb += L) {
+    for (uint32_t tb = 0; tb < (uint32_t)a.w; tb += L) {
 #pragma unroll
       for (int t2 = 0; t2 < L; ++t2) {
         const uint32_t t = tb + t2;
-        if (t < S.w) {
-          const float2 y = __ldg(S.ybase + (size_t)((T0 + t) * S.nf));
+        if (t < (uint32_t)a.w) {
+          const float2 y = __ldg((const float2 *)(S.pout + (T0 + t) * S.rowb));
           if constexpr (MODD) { f[t2].x += y.x; f[t2].y += y.y; }
-          else cmac(f[t2], y, __ldg(S.twt + ((S.rho * t) & S.ntmask)));
+          else cmac(f[t2], y, __ldg((const float2 *)(S.twt + (((S.rho * t) & S.ntmask) << 3))));
         }
       }
     }
