@@ -20,12 +20,23 @@
 // unrolled - most are trivial (+-1, +-i, (+-1 +- i)/sqrt 2).
 // Warps never synchronise with each other; the per-window maximum is combined across warps with a
 // 64-bit atomicMax on the same total-order key the generic kernel uses.
+//
+// Arithmetic layout (sm_100a packed FP32): bins s and s + L/2 of a thread share one 64-bit register
+// pair per component, X[j] = (Re A[j], Re A[j+L/2]), Y[j] = (Im A[j], Im A[j+L/2]).  Their twiddles
+// are equal (even step) or opposite (odd step), so one FFMA2 / FADD2 (fma.rn.f32x2, add.rn.f32x2)
+// with a broadcast immediate updates both, and |A|^2 of both costs one FMUL2 + one FFMA2.  Measured
+// on B200: FFMA2 runs at half the warp-instruction rate of FFMA (same
+// flops) but leaves the issue port free for the half-rate ALU-pipe instructions (LOP3 key tags),
+// which overlap with it almost perfectly; scalar FFMA + LOP3 do not.
 #pragma once
 #include "common.cuh"
 
 namespace volks {
 
 constexpr int SLIDE_WARPS = 8;   // warps per CTA
+#ifndef SLIDE_PF
+#define SLIDE_PF 8              // L1 prefetch distance in steps (rows)
+#endif
 #ifndef SLIDE_MIN_CTAS
 #define SLIDE_MIN_CTAS 2        // register cap 128 (no spills); measured: 2 and 4 within 3 %, 3 slower
 #endif
@@ -42,41 +53,64 @@ struct SlideArgs {
   uint32_t keymask;     // 0xFFFFFFF0, passed as data so that (p & mask) | id is ONE LOP3 (register mask)
 };
 
-// acc += exp(-2 pi i K16/16) * g, K16 a compile-time constant.  exp(-i th) g = (c gx + s gy, c gy - s gx).
+typedef unsigned long long f32x2;   // two packed floats (lo, hi) in one 64-bit register pair
+
+__device__ __forceinline__ f32x2 pk(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ float lo32(f32x2 v) { float a, b; asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return a; }
+__device__ __forceinline__ float hi32(f32x2 v) { float a, b; asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return b; }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+
+// The per-step operand of one parity class: g = (gx, gy) replicated into both halves with the hi
+// half carrying the pair sign sigma = (-1)^B, plus the (1 -+ i)/sqrt 2 products of the even twiddles.
+struct SlideG { f32x2 GX, GY, PP, QQ; };
+
+template <int B>
+__device__ __forceinline__ SlideG slide_make_g(float gx, float gy) {
+  constexpr float H = 0.70710678118654752f;
+  SlideG G;
+  G.GX = (B & 1) ? pk(gx, -gx) : pk(gx, gx);
+  G.GY = (B & 1) ? pk(gy, -gy) : pk(gy, gy);
+  G.PP = mul2(add2(G.GX, G.GY), pk(H, H));   // H (gx + gy)   (dead code when the step has no such bin)
+  G.QQ = mul2(sub2(G.GY, G.GX), pk(H, H));   // H (gy - gx)
+  return G;
+}
+
+// (X, Y) += exp(-2 pi i K16/16) * g for the bin pair;  exp(-i th) g = (c gx + s gy, c gy - s gx).
 template <int K16>
-__device__ __forceinline__ void cmac_w16(float2 &a, const float2 g) {
-  constexpr float C1 = 0.92387953251128674f, S1 = 0.38268343236508977f, H = 0.70710678118654752f;
+__device__ __forceinline__ void cmac2_w16(f32x2 &X, f32x2 &Y, const SlideG &G) {
+  constexpr float C1 = 0.92387953251128674f, S1 = 0.38268343236508977f;
   constexpr int k = K16 & 15;
-  if constexpr (k == 0) { a.x += g.x; a.y += g.y; }
-  else if constexpr (k == 8) { a.x -= g.x; a.y -= g.y; }
-  else if constexpr (k == 4) { a.x += g.y; a.y -= g.x; }
-  else if constexpr (k == 12) { a.x -= g.y; a.y += g.x; }
-  else if constexpr ((k & 1) == 0) {
-    const float P = H * (g.x + g.y), Q = H * (g.y - g.x);   // shared by every such bin of the step (CSE)
-    if constexpr (k == 2) { a.x += P; a.y += Q; }
-    else if constexpr (k == 6) { a.x += Q; a.y -= P; }
-    else if constexpr (k == 10) { a.x -= P; a.y -= Q; }
-    else { a.x -= Q; a.y += P; }   // 14
-  } else {
+  if constexpr (k == 0) { X = add2(X, G.GX); Y = add2(Y, G.GY); }
+  else if constexpr (k == 8) { X = sub2(X, G.GX); Y = sub2(Y, G.GY); }
+  else if constexpr (k == 4) { X = add2(X, G.GY); Y = sub2(Y, G.GX); }
+  else if constexpr (k == 12) { X = sub2(X, G.GY); Y = add2(Y, G.GX); }
+  else if constexpr (k == 2) { X = add2(X, G.PP); Y = add2(Y, G.QQ); }
+  else if constexpr (k == 6) { X = add2(X, G.QQ); Y = sub2(Y, G.PP); }
+  else if constexpr (k == 10) { X = sub2(X, G.PP); Y = sub2(Y, G.QQ); }
+  else if constexpr (k == 14) { X = sub2(X, G.QQ); Y = add2(Y, G.PP); }
+  else {
     constexpr float c = (k == 1 || k == 15) ? C1 : (k == 3 || k == 13) ? S1 : (k == 5 || k == 11) ? -S1 : -C1;
     constexpr float s = (k == 1 || k == 7) ? S1 : (k == 3 || k == 5) ? C1 : (k == 9 || k == 15) ? -S1 : -C1;
-    a.x = fmaf(c, g.x, fmaf(s, g.y, a.x));
-    a.y = fmaf(c, g.y, fmaf(-s, g.x, a.y));
+    X = fma2(G.GX, pk(c, c), fma2(G.GY, pk(s, s), X));
+    Y = fma2(G.GY, pk(c, c), fma2(G.GX, pk(-s, -s), Y));
   }
 }
 
 // One warp's state while it walks a segment of consecutive windows.
 template <int L>
 struct SlideState {
-  float2 A[L];           // bins r = rho + M s of this lane's column, absolute-phase form
-  float2 yin, yout, tw;  // prefetched operands of the NEXT update (loaded one step ahead)
-  const char *pout;      // this lane's column of the pair's delay spectra, row 0
-  const char *pin;       // the same column, row w
+  f32x2 X[L / 2], Y[L / 2];   // X[j] = (Re A[j], Re A[j+L/2]), Y[j] = (Im ...), absolute-phase form
+  float2 yin, yout, tw;       // prefetched operands of the NEXT update (loaded one step ahead)
+  const char *pout;           // this lane's column of the pair's delay spectra, row 0
+  const char *pin;            // the same column, row w
   const char *twt;
-  u64 *keyp;             // canonical key of window t0 = keyp[t0]
-  uint32_t rowb;         // bytes per Y row
-  uint32_t nf, ntmask, rho, log2m, d, keymask;
-  float sgn;             // (-1)^rho (used when M is even: every bin of the thread has rho's parity)
+  u64 *keyp;                  // canonical key of window t0 = keyp[t0]
+  uint32_t rowb;              // bytes per Y row
+  uint32_t ntmask, rho, idx0, idxs, keymask;   // plane index of bin s: idx0 + s * idxs
+  float sgn;                  // (-1)^rho (M even: every bin of the thread has rho's parity)
 };
 
 // Per-thread peak key of the L bins: power with its 4 low mantissa bits replaced by (15 - s), so one
@@ -85,10 +119,11 @@ template <int L>
 __device__ __forceinline__ uint32_t slide_local_key(const SlideState<L> &S) {
   uint32_t best = 0;
 #pragma unroll
-  for (int s = 0; s < L; ++s) {
-    const float p = cnorm(S.A[s]);
-    const uint32_t k = (__float_as_uint(p) & S.keymask) | (uint32_t)(15 - s);
-    best = k > best ? k : best;
+  for (int j = 0; j < L / 2; ++j) {
+    const f32x2 pw = fma2(S.Y[j], S.Y[j], mul2(S.X[j], S.X[j]));
+    const uint32_t k0 = (__float_as_uint(lo32(pw)) & S.keymask) | (uint32_t)(15 - j);
+    const uint32_t k1 = (__float_as_uint(hi32(pw)) & S.keymask) | (uint32_t)(15 - j - L / 2);
+    best = max(best, max(k0, k1));
   }
   return best;
 }
@@ -100,20 +135,19 @@ __device__ __forceinline__ void slide_emit(const SlideState<L> &S, uint32_t t0) 
   const uint32_t km = __reduce_max_sync(0xffffffffu, best);
   if (best == km) {
     const uint32_t s = 15u - (km & 15u);
-    const uint32_t r = S.rho + (s << S.log2m);
-    atomicMax(S.keyp + t0, make_key(__uint_as_float(km & 0xFFFFFFF0u), r * S.nf + S.d));
+    atomicMax(S.keyp + t0, make_key(__uint_as_float(km & 0xFFFFFFF0u), S.idx0 + s * S.idxs));
   }
 }
 
-// acc[s] += W_L^{(s B) mod L} * g for every bin s of the thread (s, B compile time).  ge / go: the
-// delta of even / odd rate bins (the same value when every bin of the thread has one parity).
-template <int L, int B, int S_>
+// pairs j = J .. L/2-1:  (X[j], Y[j]) += W_L^{(j B) mod L} * g   (bin j + L/2: the same times (-1)^B).
+// Ge / Go: operand of the even / odd rate bins (identical when every bin of the thread has one parity).
+template <int L, int B, int J>
 struct SlideBins {
-  static __device__ __forceinline__ void run(float2 (&A)[L], const float2 ge, const float2 go) {
-    if constexpr (S_ < L) {
-      constexpr int K16 = ((S_ * B) % L) * (16 / L);
-      cmac_w16<K16>(A[S_], (S_ & 1) ? go : ge);
-      SlideBins<L, B, S_ + 1>::run(A, ge, go);
+  static __device__ __forceinline__ void run(SlideState<L> &S, const SlideG &Ge, const SlideG &Go) {
+    if constexpr (J < L / 2) {
+      constexpr int K16 = ((J * B) % L) * (16 / L);
+      cmac2_w16<K16>(S.X[J], S.Y[J], (J & 1) ? Go : Ge);
+      SlideBins<L, B, J + 1>::run(S, Ge, Go);
     }
   }
 };
@@ -122,6 +156,9 @@ struct SlideBins {
 template <int L, bool MODD>
 __device__ __forceinline__ void slide_prefetch(SlideState<L> &S, uint32_t t) {
   const uint32_t off = t * S.rowb;
+  // row t+w is new to this SM: pull the row SLIDE_PF steps ahead into L1 now, so that the register
+  // load one step ahead is an L1 hit (the Y buffer carries SLIDE_PF + 1 padding rows)
+  asm volatile("prefetch.global.L1 [%0];" ::"l"(S.pin + off + SLIDE_PF * S.rowb));
   S.yin = __ldg((const float2 *)(S.pin + off));
   S.yout = __ldg((const float2 *)(S.pout + off));
   if constexpr (!MODD) S.tw = __ldg((const float2 *)(S.twt + (((S.rho * t) & S.ntmask) << 3)));
@@ -135,14 +172,15 @@ __device__ __forceinline__ void slide_update(SlideState<L> &S, uint32_t t0) {
   slide_prefetch<L, MODD>(S, t0 + 1);
   if constexpr (MODD) {
     // M == 1, rho == 0: the thread holds every rate bin, both parities; W_Nt = W_L
-    const float2 ge = make_float2(yin.x - yout.x, yin.y - yout.y);
-    const float2 go = make_float2(-yin.x - yout.x, -yin.y - yout.y);
-    SlideBins<L, B, 0>::run(S.A, ge, go);
+    const SlideG Ge = slide_make_g<B>(yin.x - yout.x, yin.y - yout.y);
+    const SlideG Go = slide_make_g<B>(-yin.x - yout.x, -yin.y - yout.y);
+    SlideBins<L, B, 0>::run(S, Ge, Go);
   } else {
     // M even: every bin has rho's parity; g = W_Nt^{rho t0} ((-1)^rho y_in - y_out)
     const float2 dl = make_float2(fmaf(S.sgn, yin.x, -yout.x), fmaf(S.sgn, yin.y, -yout.y));
     const float2 g = cmul(dl, tw);
-    SlideBins<L, B, 0>::run(S.A, g, g);
+    const SlideG G = slide_make_g<B>(g.x, g.y);
+    SlideBins<L, B, 0>::run(S, G, G);
   }
 }
 
@@ -173,12 +211,14 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   const int dt = (int)(wt % ndt); wt /= ndt;
   const int sg = (int)(wt % a.nseg);
   const long long pl = wt / a.nseg;
-  S.nf = (uint32_t)a.nf; S.ntmask = (uint32_t)(a.nt - 1); S.log2m = (uint32_t)a.log2m;
-  S.d = (uint32_t)(dt * 32) + lane;
+  const uint32_t d = (uint32_t)(dt * 32) + lane;
+  S.ntmask = (uint32_t)(a.nt - 1);
+  S.idx0 = S.rho * (uint32_t)a.nf + d;            // plane index r * nf + d of bin s: r = rho + M s
+  S.idxs = (uint32_t)a.nf << a.log2m;
   S.sgn = (S.rho & 1u) ? -1.f : 1.f;
   S.keymask = a.keymask;
   S.rowb = (uint32_t)a.nf * 8u;
-  S.pout = (const char *)(a.Y + (size_t)pl * a.nap * a.nf + S.d);
+  S.pout = (const char *)(a.Y + (size_t)pl * a.nap * a.nf + d);
   S.pin = S.pout + (size_t)a.w * S.rowb;
   S.twt = (const char *)a.twt;
   S.keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
@@ -205,7 +245,10 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
     }
     FftDif<L, 0, L>::run(f);
 #pragma unroll
-    for (int s = 0; s < L; ++s) S.A[s] = f[brev<L>(s)];
+    for (int j = 0; j < L / 2; ++j) {
+      S.X[j] = pk(f[brev<L>(j)].x, f[brev<L>(j + L / 2)].x);
+      S.Y[j] = pk(f[brev<L>(j)].y, f[brev<L>(j + L / 2)].y);
+    }
   }
 
   uint32_t t0 = T0;

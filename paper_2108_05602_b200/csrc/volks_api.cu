@@ -148,7 +148,7 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
     w.log2m = ilog2(w.nt / w.L);
     // sliding-sum path: stride 1, pad x2 in time, whole warps of delay columns, 32-bit row offsets
     w.slide = !force_generic && w.s == 1 && w.w >= 2 && w.nt == 2 * w.w && p->nf >= 32 &&
-              ((long long)p->nap + 1) * p->nf * 8 < (1LL << 32);
+              ((long long)p->nap + SLIDE_PF + 2) * p->nf * 8 < (1LL << 32);
     w.seg = std::max((seg_req / w.nt) * w.nt, w.nt);
     w.nseg = w.nwin > 0 ? (int)((w.nwin + w.seg - 1) / w.seg) : 0;
     w.tw_off = tw_total;
@@ -183,8 +183,8 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
   pl->off_keys = off; off = align_up(off + (size_t)std::max<long long>(s.nwin_total, 1) * sizeof(u64), 256);
   pl->off_E = off;    off = align_up(off + (size_t)std::max<long long>(pl->npair * p->nap, 1) * sizeof(float), 256);
   pl->off_cnt = off;  off = align_up(off + (size_t)std::max<long long>(pl->nfin_blocks, 1) * sizeof(uint32_t), 256);
-  // + one padding row: the sliding kernel prefetches one row past the last window's last sample
-  pl->off_Y = off;    off = align_up(off + (size_t)pl->pairs_per_chunk * std::max<size_t>(y_pair, 8) + (size_t)p->nf * sizeof(float2), 256);
+  // + padding rows: the sliding kernel loads one row, and prefetches SLIDE_PF + 1 rows, past the last sample
+  pl->off_Y = off;    off = align_up(off + (size_t)pl->pairs_per_chunk * std::max<size_t>(y_pair, 8) + (size_t)(SLIDE_PF + 2) * p->nf * sizeof(float2), 256);
   pl->ws_bytes = off;
 
   int active = 0;
