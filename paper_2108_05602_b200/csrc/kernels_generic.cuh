@@ -22,11 +22,11 @@ namespace volks {
 // ------------------------------------------------------------------------------------------------
 struct RowArgs {
   const float2 *vis;   // [rows_total][nchan]
-  float2 *Y;           // [nrows][nf] for rows row0 .. row0+nrows-1
+  float2 *Y;           // [nrows][pitch] for rows row0 .. row0+nrows-1 (first nf of each row used)
   float *E;            // [rows_total] per-AP energy
   const float2 *twf;   // [nf] exp(-2 pi i k/nf)
   long long row0, nrows;
-  int nchan, nf, tpr, rows_per_cta;
+  int nchan, nf, tpr, rows_per_cta, pitch;
 };
 
 __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
     float2 *t = in; in = out; out = t;
   }
   if (live) {
-    float2 *dst = a.Y + rrel * (long long)nf;
+    float2 *dst = a.Y + rrel * (long long)a.pitch;
     for (int k = lane; k < nf; k += tpr) dst[k] = in[k];
   }
 }
@@ -117,14 +117,14 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
 // Thread task id (d fastest): ((pair_local * nwin + j) * M + rho) * nf + d.
 // ------------------------------------------------------------------------------------------------
 struct ColArgs {
-  const float2 *Y;      // [npairs_chunk][nap][nf]
+  const float2 *Y;      // [npairs_chunk][nap][pitch]
   u64 *keys;            // canonical window keys
   const float2 *twt;    // [nt] exp(-2 pi i k/nt)
   long long total;      // number of thread tasks
   long long per_pair;   // windows per (bl, ifq) pair over all widths
   long long offc;       // canonical offset of this width inside a pair
   long long pair0;      // first pair of the chunk
-  int nap, nf, log2nf, w, stride, nt, log2m, nwin;
+  int nap, nf, log2nf, w, stride, nt, log2m, nwin, pitch;
 };
 
 template <int L>
@@ -143,7 +143,7 @@ __global__ void __launch_bounds__(256) k_col(ColArgs a) {
     const long long pl = rest / a.nwin;
     c = (a.pair0 + pl) * a.per_pair + a.offc + j;
     const int t0 = j * a.stride;
-    const float2 *col = a.Y + ((pl * a.nap + t0) * (long long)a.nf + d);
+    const float2 *col = a.Y + ((pl * a.nap + t0) * (long long)a.pitch + d);
     float2 acc[L];
 #pragma unroll
     for (int i = 0; i < L; ++i) acc[i] = make_float2(0.f, 0.f);
@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(256) k_col(ColArgs a) {
       for (int t2 = 0; t2 < L; ++t2) {
         const int t = tb + t2;
         if (t < a.w) {
-          const float2 y = __ldg(col + (long long)t * a.nf);
+          const float2 y = __ldg(col + (long long)t * a.pitch);
           const float2 tw = __ldg(a.twt + ((rho * t) & ntm));
           cmac(acc[t2], y, tw);
         }

@@ -42,14 +42,14 @@ constexpr int SLIDE_WARPS = 8;   // warps per CTA
 #endif
 
 struct SlideArgs {
-  const float2 *Y;      // [npairs_chunk][nap][nf] delay spectra
+  const float2 *Y;      // [npairs_chunk][nap][pitch] delay spectra
   u64 *keys;            // canonical window keys
   const float2 *twt;    // [nt] exp(-2 pi i k/nt)
   long long ntasks;     // warp tasks = npairs * nseg * (nf/32) * M
   long long per_pair;   // windows per (bl, ifq) pair over all widths
   long long offc;       // canonical offset of this width inside a pair
   long long pair0;      // first pair of the chunk
-  int nap, nf, w, nt, log2m, nwin, seg, nseg;
+  int nap, nf, w, nt, log2m, nwin, seg, nseg, pitch;
   uint32_t keymask;     // 0xFFFFFFF0, passed as data so that (p & mask) | id is ONE LOP3 (register mask)
 };
 
@@ -109,7 +109,7 @@ struct SlideState {
   const char *twt;
   u64 *keyp;                  // canonical key of window t0 = keyp[t0]
   uint32_t rowb;              // bytes per Y row
-  uint32_t ntmask, rho, idx0, idxs, keymask;   // plane index of bin s: idx0 + s * idxs
+  uint32_t ntmask, rho, idx0, idxs, keymask, lane;   // plane index of bin s: idx0 + s * idxs
   float sgn;                  // (-1)^rho (M even: every bin of the thread has rho's parity)
 };
 
@@ -128,14 +128,30 @@ __device__ __forceinline__ uint32_t slide_local_key(const SlideState<L> &S) {
   return best;
 }
 
-// emit the window's contribution: warp max of the local keys, winner lane(s) update the 64-bit key
+// emit the window's contribution: warp max of the local keys; the winning lane (lowest column among
+// equal keys) parks the 64-bit key in the CTA's shared slot [step in block][warp].  slide_flush
+// combines the warps of the CTA and issues ONE global atomicMax per window and CTA.
 template <int L>
-__device__ __forceinline__ void slide_emit(const SlideState<L> &S, uint32_t t0) {
+__device__ __forceinline__ void slide_emit(const SlideState<L> &S, u64 *slot) {
   const uint32_t best = slide_local_key<L>(S);
   const uint32_t km = __reduce_max_sync(0xffffffffu, best);
-  if (best == km) {
+  const uint32_t tied = __ballot_sync(0xffffffffu, best == km);
+  if (S.lane == (uint32_t)__ffs(tied) - 1u) {
     const uint32_t s = 15u - (km & 15u);
-    atomicMax(S.keyp + t0, make_key(__uint_as_float(km & 0xFFFFFFF0u), S.idx0 + s * S.idxs));
+    *slot = make_key(__uint_as_float(km & 0xFFFFFFF0u), S.idx0 + s * S.idxs);
+  }
+}
+
+// after a block of nsteps (<= 16) windows starting at t0: lanes 0..nsteps-1 of warp 0 reduce the
+// warps' slots of their window and update the canonical key.  Slots are double-buffered, so one
+// __syncthreads per block orders both the reads here and the next writes.
+__device__ __forceinline__ void slide_flush(u64 *keyp, const u64 *slots, uint32_t t0, uint32_t nsteps, int nwarps) {
+  __syncthreads();
+  if (threadIdx.x < nsteps) {
+    const u64 *p = slots + threadIdx.x * SLIDE_WARPS;
+    u64 k = p[0];
+    for (int i = 1; i < nwarps; ++i) k = p[i] > k ? p[i] : k;
+    atomicMax(keyp + t0 + threadIdx.x, k);
   }
 }
 
@@ -187,13 +203,13 @@ __device__ __forceinline__ void slide_update(SlideState<L> &S, uint32_t t0) {
 // L consecutive steps starting at t0 (t0 mod L == 0).  GUARD: only windows < tend exist.
 template <int L, int B, bool MODD, bool GUARD>
 struct SlideSteps {
-  static __device__ __forceinline__ void run(SlideState<L> &S, uint32_t t0, uint32_t tend) {
+  static __device__ __forceinline__ void run(SlideState<L> &S, uint32_t t0, uint32_t tend, u64 *slot) {
     if constexpr (B < L) {
       if (!GUARD || t0 + B < tend) {
-        slide_emit<L>(S, t0 + B);
+        slide_emit<L>(S, slot + B * SLIDE_WARPS);
         if (!GUARD || t0 + B + 1 < tend) slide_update<L, B, MODD>(S, t0 + B);
       }
-      SlideSteps<L, B + 1, MODD, GUARD>::run(S, t0, tend);
+      SlideSteps<L, B + 1, MODD, GUARD>::run(S, t0, tend, slot);
     }
   }
 };
@@ -201,12 +217,15 @@ struct SlideSteps {
 // L = min(16, Nt) bins per thread;  MODD <=> M == 1 (Nt <= 16).
 template <int L, bool MODD>
 __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(SlideArgs a) {
-  long long wt = (long long)blockIdx.x * SLIDE_WARPS + (threadIdx.x >> 5);
-  if (wt >= a.ntasks) return;                     // whole warps only: no divergence inside a warp
+  // blockDim.x = 32 * min(SLIDE_WARPS, ndt * M): every warp of a CTA works on the same (pair, segment)
+  __shared__ u64 slots[2][16 * SLIDE_WARPS];
+  const int nwarps = blockDim.x >> 5, warp = threadIdx.x >> 5;
+  long long wt = (long long)blockIdx.x * nwarps + warp;
   const uint32_t lane = threadIdx.x & 31u;
   const int M = 1 << a.log2m;
   const int ndt = a.nf >> 5;
   SlideState<L> S;
+  S.lane = lane;
   S.rho = (uint32_t)(wt & (M - 1)); wt >>= a.log2m;
   const int dt = (int)(wt % ndt); wt /= ndt;
   const int sg = (int)(wt % a.nseg);
@@ -217,8 +236,8 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   S.idxs = (uint32_t)a.nf << a.log2m;
   S.sgn = (S.rho & 1u) ? -1.f : 1.f;
   S.keymask = a.keymask;
-  S.rowb = (uint32_t)a.nf * 8u;
-  S.pout = (const char *)(a.Y + (size_t)pl * a.nap * a.nf + d);
+  S.rowb = (uint32_t)a.pitch * 8u;
+  S.pout = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch + d);
   S.pin = S.pout + (size_t)a.w * S.rowb;
   S.twt = (const char *)a.twt;
   S.keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
@@ -251,9 +270,13 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
     }
   }
 
-  uint32_t t0 = T0;
-  for (; t0 + L < tend; t0 += L) SlideSteps<L, 0, MODD, false>::run(S, t0, tend);
-  SlideSteps<L, 0, MODD, true>::run(S, t0, tend);
+  uint32_t t0 = T0, buf = 0;
+  for (; t0 + L < tend; t0 += L, buf ^= 1u) {
+    SlideSteps<L, 0, MODD, false>::run(S, t0, tend, &slots[buf][warp]);
+    slide_flush(S.keyp, slots[buf], t0, L, nwarps);
+  }
+  SlideSteps<L, 0, MODD, true>::run(S, t0, tend, &slots[buf][warp]);
+  slide_flush(S.keyp, slots[buf], t0, tend - t0, nwarps);
 }
 
 }  // namespace volks

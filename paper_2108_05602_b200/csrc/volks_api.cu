@@ -56,8 +56,11 @@ static void launch_col(const ColArgs &a, cudaStream_t st) {
 }
 
 static void launch_slide(const SlideArgs &a, cudaStream_t st) {
-  const unsigned blocks = (unsigned)((a.ntasks + SLIDE_WARPS - 1) / SLIDE_WARPS);
-  const int thr = SLIDE_WARPS * 32;
+  // every warp of a CTA must share its (pair, segment): warps per CTA = min(SLIDE_WARPS, ndt * M)
+  const long long per_seg = (long long)(a.nf / 32) << a.log2m;
+  const int wpb = (int)std::min<long long>(SLIDE_WARPS, per_seg);
+  const unsigned blocks = (unsigned)(a.ntasks / wpb);
+  const int thr = wpb * 32;
   if (a.nt >= 32) k_slide<16, false><<<blocks, thr, 0, st>>>(a);
   else if (a.nt == 16) k_slide<16, true><<<blocks, thr, 0, st>>>(a);
   else if (a.nt == 8) k_slide<8, true><<<blocks, thr, 0, st>>>(a);
@@ -71,7 +74,7 @@ struct volks_plan {
   Sched *d_sched = nullptr;    // device copy
   std::vector<WidthPlan> wp;
   float2 *d_tables = nullptr;  // [nf] delay twiddles, then per width [nt] rate twiddles
-  int nchan = 0;
+  int nchan = 0, pitch = 0;
   long long npair = 0;
   // workspace layout (byte offsets)
   size_t off_keys = 0, off_E = 0, off_cnt = 0, off_Y = 0, ws_bytes = 0;
@@ -148,7 +151,7 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
     w.log2m = ilog2(w.nt / w.L);
     // sliding-sum path: stride 1, pad x2 in time, whole warps of delay columns, 32-bit row offsets
     w.slide = !force_generic && w.s == 1 && w.w >= 2 && w.nt == 2 * w.w && p->nf >= 32 &&
-              ((long long)p->nap + SLIDE_PF + 2) * p->nf * 8 < (1LL << 32);
+              ((long long)p->nap + SLIDE_PF + 2) * (p->nf + 64) * 8 < (1LL << 32);
     w.seg = std::max((seg_req / w.nt) * w.nt, w.nt);
     w.nseg = w.nwin > 0 ? (int)((w.nwin + w.seg - 1) / w.seg) : 0;
     w.tw_off = tw_total;
@@ -170,7 +173,10 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
   if (pl->row_smem > 200 * 1024) { delete pl; return VOLKS_EINVAL; }
 
   // chunking of the delay-spectrum intermediate Y over (bl, ifq) pairs: <= 4 GiB per chunk
-  const size_t y_pair = (size_t)p->nap * p->nf * sizeof(float2);
+  // Y row pitch: nf + 16 elements (one 128-byte line) when rows would otherwise sit a power of two
+  // apart and fall into the same few L1 sets (kernels_slide.cuh reads w+1 rows of a column tile)
+  pl->pitch = p->nf >= 32 ? p->nf + env_int("VOLKS_Y_PAD", 16) : p->nf;
+  const size_t y_pair = (size_t)p->nap * pl->pitch * sizeof(float2);
   const size_t budget = (size_t)4 << 30;
   long long ppc = y_pair ? (long long)std::max<size_t>(1, budget / std::max<size_t>(y_pair, 1)) : pl->npair;
   ppc = std::min(ppc, pl->npair);
@@ -184,7 +190,7 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
   pl->off_E = off;    off = align_up(off + (size_t)std::max<long long>(pl->npair * p->nap, 1) * sizeof(float), 256);
   pl->off_cnt = off;  off = align_up(off + (size_t)std::max<long long>(pl->nfin_blocks, 1) * sizeof(uint32_t), 256);
   // + padding rows: the sliding kernel loads one row, and prefetches SLIDE_PF + 1 rows, past the last sample
-  pl->off_Y = off;    off = align_up(off + (size_t)pl->pairs_per_chunk * std::max<size_t>(y_pair, 8) + (size_t)(SLIDE_PF + 2) * p->nf * sizeof(float2), 256);
+  pl->off_Y = off;    off = align_up(off + (size_t)pl->pairs_per_chunk * std::max<size_t>(y_pair, 8) + (size_t)(SLIDE_PF + 2) * pl->pitch * sizeof(float2), 256);
   pl->ws_bytes = off;
 
   int active = 0;
@@ -253,7 +259,7 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
     RowArgs ra;
     ra.vis = (const float2 *)d_vis; ra.Y = Y; ra.E = E; ra.twf = pl->d_tables;
     ra.row0 = pair0 * s.nap; ra.nrows = np * s.nap;
-    ra.nchan = pl->nchan; ra.nf = s.nf; ra.tpr = pl->row_tpr; ra.rows_per_cta = pl->row_rows_per_cta;
+    ra.nchan = pl->nchan; ra.nf = s.nf; ra.tpr = pl->row_tpr; ra.rows_per_cta = pl->row_rows_per_cta; ra.pitch = pl->pitch;
     const long long rblocks = (ra.nrows + ra.rows_per_cta - 1) / ra.rows_per_cta;
     {
       ProfScope ps(pl, st, VOLKS_K_ROW, -1);
@@ -266,14 +272,14 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
       ca.Y = Y; ca.keys = keys; ca.twt = pl->d_tables + w.tw_off;
       ca.per_pair = s.per_pair; ca.offc = s.offc[q]; ca.pair0 = pair0;
       ca.nap = s.nap; ca.nf = s.nf; ca.log2nf = s.log2nf; ca.w = w.w; ca.stride = w.s; ca.nt = w.nt;
-      ca.log2m = w.log2m; ca.nwin = (int)w.nwin;
+      ca.log2m = w.log2m; ca.nwin = (int)w.nwin; ca.pitch = pl->pitch;
       ca.total = ((np * w.nwin) << w.log2m) * s.nf;
       if (w.slide) {
         SlideArgs sa;
         sa.Y = Y; sa.keys = keys; sa.twt = pl->d_tables + w.tw_off;
         sa.per_pair = s.per_pair; sa.offc = s.offc[q]; sa.pair0 = pair0;
         sa.nap = s.nap; sa.nf = s.nf; sa.w = w.w; sa.nt = w.nt; sa.log2m = w.log2m; sa.nwin = (int)w.nwin;
-        sa.seg = w.seg; sa.nseg = w.nseg; sa.keymask = 0xFFFFFFF0u;
+        sa.seg = w.seg; sa.nseg = w.nseg; sa.keymask = 0xFFFFFFF0u; sa.pitch = pl->pitch;
         sa.ntasks = ((np * w.nseg * (long long)(s.nf / 32)) << w.log2m);
         ProfScope ps(pl, st, VOLKS_K_SLIDE, q);
         launch_slide(sa, st);
