@@ -27,6 +27,11 @@ struct RowArgs {
   const float2 *twf;   // [nf] exp(-2 pi i k/nf)
   long long row0, nrows;
   int nchan, nf, tpr, rows_per_cta, pitch;
+  // width w == 1 (if the search has one): its plane is the row's delay spectrum repeated over every
+  // rate bin, so the peak is max_d |Y[t][d]|^2 at r* = 0 (tie-break A8) and is emitted right here
+  u64 *keys1;           // canonical key base of that width (keys + offc), or nullptr
+  long long per_pair;   // windows per pair over all widths
+  int nap, stride1, nwin1;
 };
 
 __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
@@ -106,9 +111,36 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
     __syncthreads();
     float2 *t = in; in = out; out = t;
   }
+  u64 key = 0;
   if (live) {
     float2 *dst = a.Y + rrel * (long long)a.pitch;
-    for (int k = lane; k < nf; k += tpr) dst[k] = in[k];
+    for (int k = lane; k < nf; k += tpr) {
+      const float2 v = in[k];
+      dst[k] = v;
+      const u64 kk = make_key(cnorm(v), (uint32_t)k);
+      key = kk > key ? kk : key;
+    }
+  }
+  if (a.keys1) {   // uniform branch
+    const int seg = tpr < 32 ? tpr : 32;
+    for (int o = seg >> 1; o >= 1; o >>= 1) {
+      const u64 other = __shfl_xor_sync(0xffffffffu, key, o);
+      key = other > key ? other : key;
+    }
+    u64 *ksm = (u64 *)esm;                      // [rows_per_cta][16] warp partials (reuses the energy area)
+    if (tpr > 32) {
+      __syncthreads();
+      if ((lane & 31) == 0) ksm[rl * 16 + (lane >> 5)] = key;
+      __syncthreads();
+      if (lane == 0) for (int i = 0; i < tpr / 32; ++i) key = ksm[rl * 16 + i] > key ? ksm[rl * 16 + i] : key;
+    }
+    if (live && lane == 0) {
+      const long long row = a.row0 + rrel;
+      const long long pair = row / a.nap;
+      const int t = (int)(row - pair * a.nap);
+      const int j = t / a.stride1;
+      if (j * a.stride1 == t && j < a.nwin1) a.keys1[pair * a.per_pair + j] = key;
+    }
   }
 }
 

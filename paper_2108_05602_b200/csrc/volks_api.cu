@@ -75,6 +75,7 @@ struct volks_plan {
   std::vector<WidthPlan> wp;
   float2 *d_tables = nullptr;  // [nf] delay twiddles, then per width [nt] rate twiddles
   int nchan = 0, pitch = 0;
+  int wid1 = -1;                // a width with w == 1 whose peaks the row kernel emits itself (or -1)
   long long npair = 0;
   // workspace layout (byte offsets)
   size_t off_keys = 0, off_E = 0, off_cnt = 0, off_Y = 0, ws_bytes = 0;
@@ -169,7 +170,7 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
   // row kernel shape: nf/4 threads per row (at least 1, at most 512), ~256 threads per CTA
   pl->row_tpr = std::max(1, std::min(512, p->nf / 4));
   pl->row_rows_per_cta = std::max(1, 256 / pl->row_tpr);
-  pl->row_smem = (size_t)2 * pl->row_rows_per_cta * p->nf * sizeof(float2) + (size_t)pl->row_rows_per_cta * 16 * sizeof(float);
+  pl->row_smem = (size_t)2 * pl->row_rows_per_cta * p->nf * sizeof(float2) + (size_t)pl->row_rows_per_cta * 16 * sizeof(u64);
   if (pl->row_smem > 200 * 1024) { delete pl; return VOLKS_EINVAL; }
 
   // chunking of the delay-spectrum intermediate Y over (bl, ifq) pairs: <= 4 GiB per chunk
@@ -194,7 +195,10 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
   pl->ws_bytes = off;
 
   int active = 0;
-  for (auto &w : pl->wp) active += w.nwin > 0 ? 1 : 0;
+  if (!force_generic)
+    for (int q = 0; q < p->nwidths && pl->wid1 < 0; ++q)
+      if (pl->wp[q].w == 1 && pl->wp[q].nwin > 0) pl->wid1 = q;
+  for (int q = 0; q < p->nwidths; ++q) active += (pl->wp[q].nwin > 0 && q != pl->wid1) ? 1 : 0;
   pl->launches = s.nwin_total > 0 ? (int)(1 + pl->nchunks * (1 + active) + 3) : 1;
 
   // tables, computed in double precision on the host
@@ -260,6 +264,8 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
     ra.vis = (const float2 *)d_vis; ra.Y = Y; ra.E = E; ra.twf = pl->d_tables;
     ra.row0 = pair0 * s.nap; ra.nrows = np * s.nap;
     ra.nchan = pl->nchan; ra.nf = s.nf; ra.tpr = pl->row_tpr; ra.rows_per_cta = pl->row_rows_per_cta; ra.pitch = pl->pitch;
+    ra.keys1 = nullptr; ra.per_pair = s.per_pair; ra.nap = s.nap; ra.stride1 = 1; ra.nwin1 = 0;
+    if (pl->wid1 >= 0) { ra.keys1 = keys + s.offc[pl->wid1]; ra.stride1 = s.stride[pl->wid1]; ra.nwin1 = (int)s.nwin[pl->wid1]; }
     const long long rblocks = (ra.nrows + ra.rows_per_cta - 1) / ra.rows_per_cta;
     {
       ProfScope ps(pl, st, VOLKS_K_ROW, -1);
@@ -267,7 +273,7 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
     }
     for (int q = 0; q < s.nwidths; ++q) {
       const WidthPlan &w = pl->wp[q];
-      if (w.nwin == 0) continue;
+      if (w.nwin == 0 || q == pl->wid1) continue;
       ColArgs ca;
       ca.Y = Y; ca.keys = keys; ca.twt = pl->d_tables + w.tw_off;
       ca.per_pair = s.per_pair; ca.offc = s.offc[q]; ca.pair0 = pair0;
