@@ -173,7 +173,7 @@ def run_reference(args):
     }))
 
 
-KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6: "slide"}
+KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6: "slide", 7: "colfft"}
 
 
 def run_volks(args):
@@ -254,7 +254,7 @@ def run_volks(args):
     dom_ms_avg = float(np.mean(per[dom]))
     if dom[0] == 2:       # column kernel of width dom[1]: one launch per chunk of pairs
         dom_flops = per_w_alg[dom[1]] / nlaunch[dom]
-    elif dom[0] == 6:     # sliding-sum kernel of width dom[1]
+    elif dom[0] in (6, 7):     # sliding-sum / column-FFT kernel of width dom[1]
         dom_flops = (per_w_alg[dom[1]] if dom[1] >= 0 else sum(per_w_alg)) / nlaunch[dom]
     elif dom[0] == 1:
         dom_flops = row_alg / nlaunch[dom]

@@ -138,6 +138,7 @@ int volks_plan_launch_count(const volks_plan *plan);
 #define VOLKS_K_SCAN 4     /* scan of block counts                                                 */
 #define VOLKS_K_SCATTER 5  /* ordered candidate scatter                                            */
 #define VOLKS_K_SLIDE 6    /* stride-1 widths: sliding-sum rate transform + power + argmax          */
+#define VOLKS_K_COLFFT 7   /* any stride, Nt 32..512: two-pass shared-memory column FFT + argmax    */
 int volks_plan_profile(volks_plan *plan, int enable);
 int volks_plan_profile_read(const volks_plan *plan, int32_t capacity, int32_t *kind, int32_t *wid,
                             float *ms, int32_t *n);

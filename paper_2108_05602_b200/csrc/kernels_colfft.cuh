@@ -1,0 +1,154 @@
+// kernels_colfft.cuh - rate transform of windows with any stride, Nt = 16 * L1 (L1 = 2..32), as a
+// two-pass Cooley-Tukey FFT through shared memory (the "multi-pass path" of configs[4]: the padded
+// plane 512 x 2048 exceeds shared memory, so a CTA owns a 32-column strip of it).
+//
+//   k_colfft<L1>   a4+a5+a6 for every window of one width.
+//
+// Column d of window (t0, w) on the padded grid Nt = 16 * L1, with t = t2 + 16 t1 and r = rho + L1 s:
+//   F[rho + L1 s] = sum_{t2<16} W_16^{s t2} [ W_Nt^{rho t2} Z_{t2}[rho] ],
+//   Z_{t2}[rho]   = sum_{t1<L1} y[t0 + t2 + 16 t1] W_{L1}^{rho t1}          (zero for t2 + 16 t1 >= w)
+// pass 1: warp t2 (16 warps), lane = column: L1-point DIF FFT over t1 in registers, pruned at compile
+//         time to the NZ = ceil(w/16) (rounded up to a power of two) leading non-zero inputs; the L1
+//         outputs go to shared memory S[rho][t2][column].
+// pass 2: warp <-> residues rho (L1/16 each... one or two per warp), lane = column: 16 shared loads,
+//         the twiddle W_Nt^{rho t2} from a shared table, a 16-point DIF FFT in registers, |.|^2, the
+//         tagged 32-bit peak key of kernels_slide.cuh (R1), warp redux, one slot per warp;
+//         after the pass one thread combines the slots and issues the window's global atomicMax.
+// Consecutive windows of a CTA overlap by w - stride samples: their rows stay in L1.
+#pragma once
+#include "common.cuh"
+
+namespace volks {
+
+constexpr int CF_WARPS = 16;
+
+struct ColFftArgs {
+  const float2 *Y;      // [npairs_chunk][nap][pitch]
+  u64 *keys;            // canonical window keys
+  const float2 *twt;    // [nt] exp(-2 pi i k/nt)
+  long long per_pair, offc, pair0;
+  int nap, nf, w, stride, nt, nwin, pitch;
+  int wpc;              // windows per CTA (consecutive)
+  int nrange;           // ceil(nwin / wpc)
+  uint32_t keymask;     // 0xFFFFFFF0 (register operand of the single-LOP3 key tag)
+};
+
+// z * exp(-2 pi i K/32), 0 <= K < 16, compile time
+template <int K>
+__device__ __forceinline__ float2 mul_w32(float2 z) {
+  static_assert(K >= 0 && K < 16, "first-half twiddles only");
+  if constexpr ((K & 1) == 0) return mul_w<K / 2, 16>(z);
+  else {
+    constexpr float C[8] = {0.98078528040323043f, 0.83146961230254524f, 0.55557023301960218f, 0.19509032201612825f,
+                            -0.19509032201612825f, -0.55557023301960218f, -0.83146961230254524f, -0.98078528040323043f};
+    constexpr float S[8] = {0.19509032201612825f, 0.55557023301960218f, 0.83146961230254524f, 0.98078528040323043f,
+                            0.98078528040323043f, 0.83146961230254524f, 0.55557023301960218f, 0.19509032201612825f};
+    constexpr float c = C[K / 2], s = S[K / 2];   // cos, sin of 2 pi K/32
+    return make_float2(fmaf(z.x, c, z.y * s), fmaf(z.y, c, -z.x * s));
+  }
+}
+
+// z * exp(-2 pi i K/N) for N in {2,4,8,16,32}
+template <int K, int N>
+__device__ __forceinline__ float2 mul_wn(float2 z) {
+  if constexpr (N == 32) return mul_w32<K>(z);
+  else return mul_w<K, N>(z);
+}
+
+// In-register radix-2 DIF FFT of N points a[OFF .. OFF+N), forward, output BIT-REVERSED, where only
+// the first NZ inputs are non-zero (the rest are never read): a stage whose upper half is all zero
+// degenerates to  a[k + N/2] = W_N^k a[k].
+template <int N, int NZ, int OFF, int TOTAL>
+struct FftDifPruned {
+  template <int K>
+  static __device__ __forceinline__ void stage(float2 (&a)[TOTAL]) {
+    if constexpr (K < N / 2) {
+      if constexpr (NZ <= N / 2) {
+        if constexpr (K < NZ) a[OFF + K + N / 2] = mul_wn<K, N>(a[OFF + K]);
+      } else {
+        const float2 u = a[OFF + K], v = a[OFF + K + N / 2];
+        a[OFF + K] = cadd(u, v);
+        a[OFF + K + N / 2] = mul_wn<K, N>(csub(u, v));
+      }
+      stage<K + 1>(a);
+    }
+  }
+  static __device__ __forceinline__ void run(float2 (&a)[TOTAL]) {
+    if constexpr (N >= 2) {
+      stage<0>(a);
+      constexpr int NZ2 = NZ < N / 2 ? NZ : N / 2;
+      FftDifPruned<N / 2, NZ2, OFF, TOTAL>::run(a);
+      FftDifPruned<N / 2, NZ2, OFF + N / 2, TOTAL>::run(a);
+    }
+  }
+};
+
+// L1 = Nt/16 (2..32), NZ = leading non-zero inputs of the L1-point transform (power of two <= L1).
+template <int L1, int NZ>
+__global__ void __launch_bounds__(CF_WARPS * 32) k_colfft(ColFftArgs a) {
+  extern __shared__ float2 cf_sm[];
+  float2 *S = cf_sm;                                   // [L1][16][32]
+  float2 *tws = cf_sm + (size_t)L1 * 16 * 32;          // [nt] rate twiddles
+  u64 *slots = (u64 *)(tws + a.nt);                    // [L1] per-residue window keys
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int ntile = a.nf >> 5;
+  long long u = blockIdx.x;
+  const int rg = (int)(u % a.nrange); u /= a.nrange;
+  const int tile = (int)(u % ntile);
+  const long long pl = u / ntile;
+  const int d = tile * 32 + lane;
+  const float2 *ycol = a.Y + (size_t)pl * a.nap * a.pitch + d;
+  u64 *keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
+  for (int i = threadIdx.x; i < a.nt; i += CF_WARPS * 32) tws[i] = a.twt[i];
+  const int j0 = rg * a.wpc, j1 = min(a.nwin, j0 + a.wpc);
+  const int ntm = a.nt - 1;
+
+  for (int j = j0; j < j1; ++j) {
+    const int t0 = j * a.stride;
+    // ---- pass 1: warp = t2, L1-point pruned FFT over t1 ----
+    {
+      const int t2 = warp;
+      float2 z[L1];
+#pragma unroll
+      for (int t1 = 0; t1 < NZ; ++t1) {
+        const int t = t2 + 16 * t1;
+        z[t1] = t < a.w ? __ldg(ycol + (size_t)(t0 + t) * a.pitch) : make_float2(0.f, 0.f);
+      }
+      FftDifPruned<L1, NZ, 0, L1>::run(z);
+#pragma unroll
+      for (int i = 0; i < L1; ++i) S[(brev<L1>(i) * 16 + t2) * 32 + lane] = z[i];
+    }
+    __syncthreads();
+    // ---- pass 2: warp = residue rho, 16-point FFT over t2, power, tagged key ----
+    for (int rho = warp; rho < L1; rho += CF_WARPS) {
+      float2 f[16];
+#pragma unroll
+      for (int t2 = 0; t2 < 16; ++t2) f[t2] = cmul(S[(rho * 16 + t2) * 32 + lane], tws[(rho * t2) & ntm]);
+      FftDif<16, 0, 16>::run(f);
+      uint32_t best = 0;
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        const uint32_t k = (__float_as_uint(cnorm(f[i])) & a.keymask) | (uint32_t)(15 - brev<16>(i));
+        best = max(best, k);
+      }
+      const uint32_t km = __reduce_max_sync(0xffffffffu, best);
+      const uint32_t tied = __ballot_sync(0xffffffffu, best == km);
+      if (lane == __ffs(tied) - 1) {
+        const uint32_t s = 15u - (km & 15u);
+        slots[rho] = make_key(__uint_as_float(km & 0xFFFFFFF0u), (uint32_t)(rho + L1 * s) * (uint32_t)a.nf + (uint32_t)d);
+      }
+    }
+    __syncthreads();
+    if (warp == 0) {
+      u64 k = lane < L1 ? slots[lane] : 0ull;
+#pragma unroll
+      for (int o = 16; o >= 1; o >>= 1) {
+        const u64 other = __shfl_xor_sync(0xffffffffu, k, o);
+        k = other > k ? other : k;
+      }
+      if (lane == 0) atomicMax(keyp + j, k);
+    }
+  }
+}
+
+}  // namespace volks

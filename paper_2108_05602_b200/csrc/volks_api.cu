@@ -11,6 +11,7 @@
 
 #include "kernels_generic.cuh"
 #include "kernels_slide.cuh"
+#include "kernels_colfft.cuh"
 
 using namespace volks;
 
@@ -34,6 +35,8 @@ struct WidthPlan {
   long long nwin;       // per pair
   size_t tw_off;        // offset (float2) of its rate twiddle table in d_tables
   bool slide;           // stride-1 sliding-sum kernel (kernels_slide.cuh) instead of the generic one
+  bool colfft;          // two-pass shared-memory column FFT (kernels_colfft.cuh): Nt = 32..512, nf % 32 == 0
+  int cf_l1, cf_nz, cf_wpc, cf_nrange;
   int seg, nseg;        // sliding path: windows per exactly restarted segment, segments per pair
 };
 
@@ -53,6 +56,42 @@ template <int L>
 static void launch_col(const ColArgs &a, cudaStream_t st) {
   const long long blocks = (a.total + 255) / 256;
   k_col<L><<<(unsigned)blocks, 256, 0, st>>>(a);
+}
+
+inline size_t colfft_smem(int l1, int nt) { return (size_t)l1 * 16 * 32 * sizeof(float2) + (size_t)nt * sizeof(float2) + (size_t)l1 * sizeof(u64); }
+
+template <int L1, int NZ>
+static cudaError_t colfft_one(const ColFftArgs &a, unsigned blocks, cudaStream_t st, bool attr_only) {
+  const size_t smem = colfft_smem(L1, a.nt);
+  if (attr_only) return cudaFuncSetAttribute(k_colfft<L1, NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  k_colfft<L1, NZ><<<blocks, CF_WARPS * 32, smem, st>>>(a);
+  return cudaSuccess;
+}
+
+template <int L1>
+static cudaError_t colfft_l1(const ColFftArgs &a, int nz, unsigned blocks, cudaStream_t st, bool attr_only) {
+  switch (nz) {
+    case 1: return colfft_one<L1, 1>(a, blocks, st, attr_only);
+    case 2: return colfft_one<L1, 2>(a, blocks, st, attr_only);
+    case 4: if constexpr (L1 >= 4) return colfft_one<L1, 4>(a, blocks, st, attr_only); break;
+    case 8: if constexpr (L1 >= 8) return colfft_one<L1, 8>(a, blocks, st, attr_only); break;
+    case 16: if constexpr (L1 >= 16) return colfft_one<L1, 16>(a, blocks, st, attr_only); break;
+    case 32: if constexpr (L1 >= 32) return colfft_one<L1, 32>(a, blocks, st, attr_only); break;
+  }
+  return cudaErrorInvalidValue;
+}
+
+// attr_only: raise the kernel's dynamic shared memory limit (plan creation) instead of launching
+static cudaError_t launch_colfft(const ColFftArgs &a, int l1, int nz, long long units, cudaStream_t st, bool attr_only) {
+  const unsigned blocks = (unsigned)units;
+  switch (l1) {
+    case 2: return colfft_l1<2>(a, nz, blocks, st, attr_only);
+    case 4: return colfft_l1<4>(a, nz, blocks, st, attr_only);
+    case 8: return colfft_l1<8>(a, nz, blocks, st, attr_only);
+    case 16: return colfft_l1<16>(a, nz, blocks, st, attr_only);
+    case 32: return colfft_l1<32>(a, nz, blocks, st, attr_only);
+  }
+  return cudaErrorInvalidValue;
 }
 
 static void launch_slide(const SlideArgs &a, cudaStream_t st) {
@@ -153,6 +192,14 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
     // sliding-sum path: stride 1, pad x2 in time, whole warps of delay columns, 32-bit row offsets
     w.slide = !force_generic && w.s == 1 && w.w >= 2 && w.nt == 2 * w.w && p->nf >= 32 &&
               ((long long)p->nap + SLIDE_PF + 2) * (p->nf + 64) * 8 < (1LL << 32);
+    w.colfft = !force_generic && !w.slide && w.nt >= 32 && w.nt <= 512 && p->nf >= 32 && w.nwin > 0;
+    w.cf_l1 = w.nt / 16;
+    w.cf_nz = 1;
+    while (w.cf_nz * 16 < w.w) w.cf_nz *= 2;
+    // windows per CTA: up to 128 (L1 reuse of overlapping windows), fewer when the grid would not fill 148 SMs x 4
+    w.cf_wpc = (int)std::min<long long>(env_int("VOLKS_CF_WPC", 128),
+                                        std::max<long long>(8, (long long)p->nbl * p->nif * (p->nf / 32) * w.nwin / 592));
+    w.cf_nrange = (int)((w.nwin + w.cf_wpc - 1) / w.cf_wpc);
     w.seg = std::max((seg_req / w.nt) * w.nt, w.nt);
     w.nseg = w.nwin > 0 ? (int)((w.nwin + w.seg - 1) / w.seg) : 0;
     w.tw_off = tw_total;
@@ -218,6 +265,11 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
             cuda_ok(cudaMemcpy(pl->d_tables, tab.data(), tw_total * sizeof(float2), cudaMemcpyHostToDevice)) &&
             cuda_ok(cudaMemcpy(pl->d_sched, &s, sizeof(Sched), cudaMemcpyHostToDevice)) &&
             cuda_ok(cudaFuncSetAttribute(k_row_fft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->row_smem));
+  for (auto &w : pl->wp)
+    if (ok && w.colfft) {
+      ColFftArgs ca; memset(&ca, 0, sizeof ca); ca.nt = w.nt;
+      ok = cuda_ok(launch_colfft(ca, w.cf_l1, w.cf_nz, 0, nullptr, true));
+    }
   if (!ok) { volks_plan_destroy(pl); return VOLKS_ECUDA; }
   *out = pl;
   return VOLKS_OK;
@@ -289,6 +341,16 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
         sa.ntasks = ((np * w.nseg * (long long)(s.nf / 32)) << w.log2m);
         ProfScope ps(pl, st, VOLKS_K_SLIDE, q);
         launch_slide(sa, st);
+        continue;
+      }
+      if (w.colfft) {
+        ColFftArgs fa;
+        fa.Y = Y; fa.keys = keys; fa.twt = pl->d_tables + w.tw_off;
+        fa.per_pair = s.per_pair; fa.offc = s.offc[q]; fa.pair0 = pair0;
+        fa.nap = s.nap; fa.nf = s.nf; fa.w = w.w; fa.stride = w.s; fa.nt = w.nt; fa.nwin = (int)w.nwin;
+        fa.pitch = pl->pitch; fa.wpc = w.cf_wpc; fa.nrange = w.cf_nrange; fa.keymask = 0xFFFFFFF0u;
+        ProfScope ps(pl, st, VOLKS_K_COLFFT, q);
+        if (!cuda_ok(launch_colfft(fa, w.cf_l1, w.cf_nz, np * (s.nf / 32) * w.cf_nrange, st, false))) return VOLKS_ECUDA;
         continue;
       }
       ProfScope ps(pl, st, VOLKS_K_COL, q);

@@ -60,6 +60,23 @@ def test_reduced_configs(vb, oracle, cfg, over):
     run_both(vb, oracle, vis, c, thresh=3.0)      # PAPER.md:196 stress threshold
 
 
+@pytest.mark.parametrize("cfg,over", [
+    (2, dict(nbl=1, nif=2, nap=700, npulses=3)),
+    (3, dict(nbl=2, nif=2, nap=900, npulses=4)),
+])
+def test_generic_and_sliding_paths_agree_with_oracle(vb, oracle, cfg, over, monkeypatch):
+    """The same stride-1 inputs through the generic kernels (VOLKS_PATH=generic) and through the
+    sliding-sum kernels with a short restart interval (several segments + a ragged tail)."""
+    vis, c, _ = workloads.generate(cfg, **over)
+    monkeypatch.setenv("VOLKS_PATH", "generic")
+    run_both(vb, oracle, vis, c)
+    monkeypatch.delenv("VOLKS_PATH")
+    monkeypatch.setenv("VOLKS_SLIDE_SEG", "128")
+    run_both(vb, oracle, vis, c, thresh=3.0)
+    monkeypatch.setenv("VOLKS_SLIDE_SEG", "1024")
+    run_both(vb, oracle, vis, c)
+
+
 @pytest.mark.parametrize("shape", [
     # nbl nif nap nchan widths strides nts nf
     (1, 1, 40, 20, [1, 3, 5], [1, 2, 7], [2, 4, 8], 32),       # ragged: non-pow2 nchan / widths, stride > w
