@@ -36,6 +36,8 @@ struct RowArgs {
 
 __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
   extern __shared__ float2 sm[];
+  // a row never spans warps when tpr <= 32: a warp barrier is enough (rows of a CTA are independent)
+#define ROW_SYNC() do { if (a.tpr <= 32) __syncwarp(); else __syncthreads(); } while (0)
   const int nf = a.nf, tpr = a.tpr;
   const int rl = threadIdx.x / tpr, lane = threadIdx.x % tpr;
   const long long rrel = (long long)blockIdx.x * a.rows_per_cta + rl;
@@ -63,7 +65,7 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
       if ((lane & 31) == 0) esm[rl * 16 + (lane >> 5)] = e;
     }
   }
-  __syncthreads();
+  ROW_SYNC();
   if (tpr > 32 && live && lane == 0) {
     float s = 0.f;
     for (int i = 0; i < tpr / 32; ++i) s += esm[rl * 16 + i];
@@ -93,7 +95,7 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
         out[j0 + 2 * Ns] = csub(s02, s13);
         out[j0 + 3 * Ns] = csub(d02, md13);
       }
-    __syncthreads();
+    ROW_SYNC();
     float2 *t = in; in = out; out = t;
     Ns <<= 2;
   }
@@ -108,7 +110,7 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
         out[j0] = cadd(v0, v1);
         out[j0 + Ns] = csub(v0, v1);
       }
-    __syncthreads();
+    ROW_SYNC();
     float2 *t = in; in = out; out = t;
   }
   u64 key = 0;
@@ -129,9 +131,9 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
     }
     u64 *ksm = (u64 *)esm;                      // [rows_per_cta][16] warp partials (reuses the energy area)
     if (tpr > 32) {
-      __syncthreads();
+      ROW_SYNC();
       if ((lane & 31) == 0) ksm[rl * 16 + (lane >> 5)] = key;
-      __syncthreads();
+      ROW_SYNC();
       if (lane == 0) for (int i = 0; i < tpr / 32; ++i) key = ksm[rl * 16 + i] > key ? ksm[rl * 16 + i] : key;
     }
     if (live && lane == 0) {
@@ -143,6 +145,7 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
     }
   }
 }
+#undef ROW_SYNC
 
 // ------------------------------------------------------------------------------------------------
 // Column (rate) transform + power + argmax, generic.

@@ -215,7 +215,8 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
   if (s.nwin_total >= (1LL << 40)) { delete pl; return VOLKS_EINVAL; }
 
   // row kernel shape: nf/4 threads per row (at least 1, at most 512), ~256 threads per CTA
-  pl->row_tpr = std::max(1, std::min(512, p->nf / 4));
+  // one warp per row up to nf = 512 (warp barriers only); wider rows take nf/4 threads and a whole CTA
+  pl->row_tpr = p->nf <= 512 ? std::max(1, std::min(32, p->nf / 4)) : std::min(512, p->nf / 4);
   pl->row_rows_per_cta = std::max(1, 256 / pl->row_tpr);
   pl->row_smem = (size_t)2 * pl->row_rows_per_cta * p->nf * sizeof(float2) + (size_t)pl->row_rows_per_cta * 16 * sizeof(u64);
   if (pl->row_smem > 200 * 1024) { delete pl; return VOLKS_EINVAL; }
