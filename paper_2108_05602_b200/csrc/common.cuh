@@ -67,6 +67,17 @@ __host__ __device__ constexpr int brev(int i) {
   return r;
 }
 
+// Delay-spectrum intermediate Y.  Rows of `pitch` complex elements.  When `paired` the two columns
+// 2c, 2c+1 of a row share one float4 (re[2c], re[2c+1], im[2c], im[2c+1]) - the layout the packed
+// sliding kernel loads straight into (column a, column b) register pairs; otherwise plain float2.
+__device__ __forceinline__ float2 ld_y(const float2 *Y, size_t row_elem_off, int d, int paired) {
+  if (paired) {
+    const float *p = (const float *)(Y + row_elem_off) + ((d >> 1) << 2) + (d & 1);
+    return make_float2(__ldg(p), __ldg(p + 2));
+  }
+  return __ldg(Y + row_elem_off + d);
+}
+
 // Peak key: total order (power descending, plane index ascending) as one unsigned 64-bit max.
 // power >= 0 so its IEEE bit pattern is monotone.
 __device__ __forceinline__ u64 make_key(float p, uint32_t idx) {

@@ -27,7 +27,7 @@ struct ColFftArgs {
   u64 *keys;            // canonical window keys
   const float2 *twt;    // [nt] exp(-2 pi i k/nt)
   long long per_pair, offc, pair0;
-  int nap, nf, w, stride, nt, nwin, pitch;
+  int nap, nf, w, stride, nt, nwin, pitch, paired;
   int wpc;              // windows per CTA (consecutive)
   int nrange;           // ceil(nwin / wpc)
   uint32_t keymask;     // 0xFFFFFFF0 (register operand of the single-LOP3 key tag)
@@ -97,7 +97,7 @@ __global__ void __launch_bounds__(CF_WARPS * 32) k_colfft(ColFftArgs a) {
   const int tile = (int)(u % ntile);
   const long long pl = u / ntile;
   const int d = tile * 32 + lane;
-  const float2 *ycol = a.Y + (size_t)pl * a.nap * a.pitch + d;
+  const size_t prow = (size_t)pl * a.nap;
   u64 *keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
   for (int i = threadIdx.x; i < a.nt; i += CF_WARPS * 32) tws[i] = a.twt[i];
   const int j0 = rg * a.wpc, j1 = min(a.nwin, j0 + a.wpc);
@@ -112,7 +112,7 @@ __global__ void __launch_bounds__(CF_WARPS * 32) k_colfft(ColFftArgs a) {
 #pragma unroll
       for (int t1 = 0; t1 < NZ; ++t1) {
         const int t = t2 + 16 * t1;
-        z[t1] = t < a.w ? __ldg(ycol + (size_t)(t0 + t) * a.pitch) : make_float2(0.f, 0.f);
+        z[t1] = t < a.w ? ld_y(a.Y, (prow + t0 + t) * a.pitch, d, a.paired) : make_float2(0.f, 0.f);
       }
       FftDifPruned<L1, NZ, 0, L1>::run(z);
 #pragma unroll

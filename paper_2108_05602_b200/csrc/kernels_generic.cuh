@@ -26,7 +26,7 @@ struct RowArgs {
   float *E;            // [rows_total] per-AP energy
   const float2 *twf;   // [nf] exp(-2 pi i k/nf)
   long long row0, nrows;
-  int nchan, nf, tpr, rows_per_cta, pitch;
+  int nchan, nf, tpr, rows_per_cta, pitch, paired;
   // width w == 1 (if the search has one): its plane is the row's delay spectrum repeated over every
   // rate bin, so the peak is max_d |Y[t][d]|^2 at r* = 0 (tie-break A8) and is emitted right here
   u64 *keys1;           // canonical key base of that width (keys + offc), or nullptr
@@ -116,11 +116,21 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
   u64 key = 0;
   if (live) {
     float2 *dst = a.Y + rrel * (long long)a.pitch;
-    for (int k = lane; k < nf; k += tpr) {
-      const float2 v = in[k];
-      dst[k] = v;
-      const u64 kk = make_key(cnorm(v), (uint32_t)k);
-      key = kk > key ? kk : key;
+    if (a.paired) {
+      for (int c = lane; c < (nf >> 1); c += tpr) {
+        const float2 v0 = in[2 * c], v1 = in[2 * c + 1];
+        ((float4 *)dst)[c] = make_float4(v0.x, v1.x, v0.y, v1.y);
+        const u64 k0 = make_key(cnorm(v0), (uint32_t)(2 * c)), k1 = make_key(cnorm(v1), (uint32_t)(2 * c + 1));
+        key = k0 > key ? k0 : key;
+        key = k1 > key ? k1 : key;
+      }
+    } else {
+      for (int k = lane; k < nf; k += tpr) {
+        const float2 v = in[k];
+        dst[k] = v;
+        const u64 kk = make_key(cnorm(v), (uint32_t)k);
+        key = kk > key ? kk : key;
+      }
     }
   }
   if (a.keys1) {   // uniform branch
@@ -159,7 +169,7 @@ struct ColArgs {
   long long per_pair;   // windows per (bl, ifq) pair over all widths
   long long offc;       // canonical offset of this width inside a pair
   long long pair0;      // first pair of the chunk
-  int nap, nf, log2nf, w, stride, nt, log2m, nwin, pitch;
+  int nap, nf, log2nf, w, stride, nt, log2m, nwin, pitch, paired;
 };
 
 template <int L>
@@ -178,7 +188,7 @@ __global__ void __launch_bounds__(256) k_col(ColArgs a) {
     const long long pl = rest / a.nwin;
     c = (a.pair0 + pl) * a.per_pair + a.offc + j;
     const int t0 = j * a.stride;
-    const float2 *col = a.Y + ((pl * a.nap + t0) * (long long)a.pitch + d);
+    const size_t row0 = (size_t)(pl * a.nap + t0) * a.pitch;
     float2 acc[L];
 #pragma unroll
     for (int i = 0; i < L; ++i) acc[i] = make_float2(0.f, 0.f);
@@ -188,7 +198,7 @@ __global__ void __launch_bounds__(256) k_col(ColArgs a) {
       for (int t2 = 0; t2 < L; ++t2) {
         const int t = tb + t2;
         if (t < a.w) {
-          const float2 y = __ldg(col + (long long)t * a.pitch);
+          const float2 y = ld_y(a.Y, row0 + (size_t)t * a.pitch, d, a.paired);
           const float2 tw = __ldg(a.twt + ((rho * t) & ntm));
           cmac(acc[t2], y, tw);
         }

@@ -21,31 +21,34 @@
 // Warps never synchronise with each other; the per-window maximum is combined across warps with a
 // 64-bit atomicMax on the same total-order key the generic kernel uses.
 //
-// Arithmetic layout (sm_100a packed FP32): bins s and s + L/2 of a thread share one 64-bit register
-// pair per component, X[j] = (Re A[j], Re A[j+L/2]), Y[j] = (Im A[j], Im A[j+L/2]).  Their twiddles
-// are equal (even step) or opposite (odd step), so one FFMA2 / FADD2 (fma.rn.f32x2, add.rn.f32x2)
-// with a broadcast immediate updates both, and |A|^2 of both costs one FMUL2 + one FFMA2.  Measured
-// on B200: FFMA2 runs at half the warp-instruction rate of FFMA (same
-// flops) but leaves the issue port free for the half-rate ALU-pipe instructions (LOP3 key tags),
-// which overlap with it almost perfectly; scalar FFMA + LOP3 do not.
+// Arithmetic layout (sm_100a packed FP32): a thread works on TWO adjacent delay columns (2c, 2c+1)
+// and keeps every quantity as a 64-bit register pair (column a, column b): X[s] = (Re A_a[s], Re A_b[s]),
+// Y[s] = (Im ...).  The delay spectra are stored pair-interleaved (common.cuh ld_y), so one 128-bit
+// load yields the (re_a, re_b), (im_a, im_b) pairs directly; the warp-uniform twiddle comes from a
+// pre-broadcast table (c, c, s, s); the compile-time W_L twiddles are broadcast immediates.  Every
+// arithmetic instruction is then an FFMA2 / FADD2 / FMUL2 (fma.rn.f32x2 ...) with no register moves.
+// Measured on B200: FFMA2 runs at half the warp-instruction rate of FFMA
+// (same flops) but leaves the issue port free for the half-rate ALU-pipe instructions (LOP3 key
+// tags), which overlap with it almost perfectly; scalar FFMA + LOP3 do not.
 #pragma once
 #include "common.cuh"
 
 namespace volks {
 
-constexpr int SLIDE_WARPS = 8;   // warps per CTA
+constexpr int SLIDE_WARPS = 8;   // warps per CTA (at most)
 #ifndef SLIDE_PF
 #define SLIDE_PF 8              // L1 prefetch distance in steps (rows)
 #endif
 #ifndef SLIDE_MIN_CTAS
-#define SLIDE_MIN_CTAS 2        // register cap 128 (no spills); measured: 2 and 4 within 3 %, 3 slower
+#define SLIDE_MIN_CTAS 2        // register cap 128
 #endif
 
 struct SlideArgs {
-  const float2 *Y;      // [npairs_chunk][nap][pitch] delay spectra
+  const float2 *Y;      // [npairs_chunk][nap][pitch] delay spectra, pair-interleaved rows
   u64 *keys;            // canonical window keys
   const float2 *twt;    // [nt] exp(-2 pi i k/nt)
-  long long ntasks;     // warp tasks = npairs * nseg * (nf/32) * M
+  const float4 *tw4;    // [nt] the same, pre-broadcast: (re, re, im, im)
+  long long ntasks;     // warp tasks = npairs * nseg * (nf/64) * M
   long long per_pair;   // windows per (bl, ifq) pair over all widths
   long long offc;       // canonical offset of this width inside a pair
   long long pair0;      // first pair of the chunk
@@ -56,29 +59,32 @@ struct SlideArgs {
 typedef unsigned long long f32x2;   // two packed floats (lo, hi) in one 64-bit register pair
 
 __device__ __forceinline__ f32x2 pk(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
-__device__ __forceinline__ float lo32(f32x2 v) { float a, b; asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return a; }
-__device__ __forceinline__ float hi32(f32x2 v) { float a, b; asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return b; }
+__device__ __forceinline__ float lo32(f32x2 v) { float a, b; asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); (void)b; return a; }
+__device__ __forceinline__ float hi32(f32x2 v) { float a, b; asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); (void)a; return b; }
+__device__ __forceinline__ f32x2 neg2(f32x2 v) { return pk(-lo32(v), -hi32(v)); }   // folds into an operand modifier
 __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
 __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+// 128-bit read-only load as two register pairs
+__device__ __forceinline__ void ldg2(const void *p, f32x2 &a, f32x2 &b) {
+  asm volatile("ld.global.nc.v2.b64 {%0,%1}, [%2];" : "=l"(a), "=l"(b) : "l"(p));
+}
 
-// The per-step operand of one parity class: g = (gx, gy) replicated into both halves with the hi
-// half carrying the pair sign sigma = (-1)^B, plus the (1 -+ i)/sqrt 2 products of the even twiddles.
+// The per-step operand of one parity class, both columns: g = (GX, GY) and the (1 -+ i)/sqrt 2
+// products of the even twiddles (dead code in steps that have no such bin).
 struct SlideG { f32x2 GX, GY, PP, QQ; };
 
-template <int B>
-__device__ __forceinline__ SlideG slide_make_g(float gx, float gy) {
+__device__ __forceinline__ SlideG slide_make_g(f32x2 gx, f32x2 gy) {
   constexpr float H = 0.70710678118654752f;
   SlideG G;
-  G.GX = (B & 1) ? pk(gx, -gx) : pk(gx, gx);
-  G.GY = (B & 1) ? pk(gy, -gy) : pk(gy, gy);
-  G.PP = mul2(add2(G.GX, G.GY), pk(H, H));   // H (gx + gy)   (dead code when the step has no such bin)
-  G.QQ = mul2(sub2(G.GY, G.GX), pk(H, H));   // H (gy - gx)
+  G.GX = gx; G.GY = gy;
+  G.PP = mul2(add2(gx, gy), pk(H, H));   // H (gx + gy)
+  G.QQ = mul2(sub2(gy, gx), pk(H, H));   // H (gy - gx)
   return G;
 }
 
-// (X, Y) += exp(-2 pi i K16/16) * g for the bin pair;  exp(-i th) g = (c gx + s gy, c gy - s gx).
+// (X, Y) += exp(-2 pi i K16/16) * g, both columns;  exp(-i th) g = (c gx + s gy, c gy - s gx).
 template <int K16>
 __device__ __forceinline__ void cmac2_w16(f32x2 &X, f32x2 &Y, const SlideG &G) {
   constexpr float C1 = 0.92387953251128674f, S1 = 0.38268343236508977f;
@@ -102,48 +108,43 @@ __device__ __forceinline__ void cmac2_w16(f32x2 &X, f32x2 &Y, const SlideG &G) {
 // One warp's state while it walks a segment of consecutive windows.
 template <int L>
 struct SlideState {
-  f32x2 X[L / 2], Y[L / 2];   // X[j] = (Re A[j], Re A[j+L/2]), Y[j] = (Im ...), absolute-phase form
-  float2 yin, yout, tw;       // prefetched operands of the NEXT update (loaded one step ahead)
-  const char *pout;           // this lane's column of the pair's delay spectra, row 0
-  const char *pin;            // the same column, row w
-  const char *twt;
-  u64 *keyp;                  // canonical key of window t0 = keyp[t0]
-  uint32_t rowb;              // bytes per Y row
-  uint32_t ntmask, rho, idx0, idxs, keymask, lane;   // plane index of bin s: idx0 + s * idxs
-  float sgn;                  // (-1)^rho (M even: every bin of the thread has rho's parity)
+  f32x2 X[L], Y[L];             // bins r = rho + M s of columns (a, b), absolute-phase form
+  f32x2 xin, yin, xout, yout;   // prefetched operands of the NEXT update (loaded one step ahead)
+  f32x2 twx, twy;               // ... and its warp-uniform twiddle, pre-broadcast
+  f32x2 sgn2;                   // ((-1)^rho, (-1)^rho)  (M even: every bin of the thread has rho's parity)
+  const char *pout;             // this lane's column pair, row 0 of the pair's delay spectra
+  const char *pin;              // the same columns, row w
+  const char *tw4;
+  u64 *keyp;                    // canonical key of window t0 = keyp[t0]
+  uint32_t rowb;                // bytes per Y row
+  uint32_t ntmask, rho, idx0, idxs, keymask, lane;   // plane index of bin s, column a: idx0 + s * idxs
 };
 
-// Per-thread peak key of the L bins: power with its 4 low mantissa bits replaced by (15 - s), so one
-// unsigned max orders by (power descending, s ascending).  Relative power error <= 2^-19.
-template <int L>
-__device__ __forceinline__ uint32_t slide_local_key(const SlideState<L> &S) {
-  uint32_t best = 0;
-#pragma unroll
-  for (int j = 0; j < L / 2; ++j) {
-    const f32x2 pw = fma2(S.Y[j], S.Y[j], mul2(S.X[j], S.X[j]));
-    const uint32_t k0 = (__float_as_uint(lo32(pw)) & S.keymask) | (uint32_t)(15 - j);
-    const uint32_t k1 = (__float_as_uint(hi32(pw)) & S.keymask) | (uint32_t)(15 - j - L / 2);
-    best = max(best, max(k0, k1));
-  }
-  return best;
-}
-
-// emit the window's contribution: warp max of the local keys; the winning lane (lowest column among
-// equal keys) parks the 64-bit key in the CTA's shared slot [step in block][warp].  slide_flush
-// combines the warps of the CTA and issues ONE global atomicMax per window and CTA.
+// emit the window's contribution: per column the max of (power with its 4 low mantissa bits replaced
+// by 15 - s): one unsigned max orders by (power descending, s ascending), relative power error
+// <= 2^-19 (R1).  Then the better column (ties: the lower one), the warp max, and the
+// winning lane (lowest among equal keys) parks the 64-bit key in the CTA's slot [step][warp].
 template <int L>
 __device__ __forceinline__ void slide_emit(const SlideState<L> &S, u64 *slot) {
-  const uint32_t best = slide_local_key<L>(S);
+  uint32_t ba = 0, bb = 0;
+#pragma unroll
+  for (int s = 0; s < L; ++s) {
+    const f32x2 pw = fma2(S.Y[s], S.Y[s], mul2(S.X[s], S.X[s]));
+    ba = max(ba, (__float_as_uint(lo32(pw)) & S.keymask) | (uint32_t)(15 - s));
+    bb = max(bb, (__float_as_uint(hi32(pw)) & S.keymask) | (uint32_t)(15 - s));
+  }
+  const bool colb = bb > ba;
+  const uint32_t best = colb ? bb : ba;
   const uint32_t km = __reduce_max_sync(0xffffffffu, best);
   const uint32_t tied = __ballot_sync(0xffffffffu, best == km);
   if (S.lane == (uint32_t)__ffs(tied) - 1u) {
     const uint32_t s = 15u - (km & 15u);
-    *slot = make_key(__uint_as_float(km & 0xFFFFFFF0u), S.idx0 + s * S.idxs);
+    *slot = make_key(__uint_as_float(km & 0xFFFFFFF0u), S.idx0 + s * S.idxs + (colb ? 1u : 0u));
   }
 }
 
-// after a block of nsteps (<= 16) windows starting at t0: lanes 0..nsteps-1 of warp 0 reduce the
-// warps' slots of their window and update the canonical key.  Slots are double-buffered, so one
+// after a block of nsteps (<= 16) windows starting at t0: threads 0..nsteps-1 reduce the warps'
+// slots of their window and update the canonical key.  Slots are double-buffered, so one
 // __syncthreads per block orders both the reads here and the next writes.
 __device__ __forceinline__ void slide_flush(u64 *keyp, const u64 *slots, uint32_t t0, uint32_t nsteps, int nwarps) {
   __syncthreads();
@@ -155,47 +156,48 @@ __device__ __forceinline__ void slide_flush(u64 *keyp, const u64 *slots, uint32_
   }
 }
 
-// pairs j = J .. L/2-1:  (X[j], Y[j]) += W_L^{(j B) mod L} * g   (bin j + L/2: the same times (-1)^B).
-// Ge / Go: operand of the even / odd rate bins (identical when every bin of the thread has one parity).
-template <int L, int B, int J>
+// bins s = S_ .. L-1:  (X[s], Y[s]) += W_L^{(s B) mod L} * g.   Ge / Go: operand of the even / odd
+// rate bins (identical when every bin of the thread has one parity).
+template <int L, int B, int S_>
 struct SlideBins {
   static __device__ __forceinline__ void run(SlideState<L> &S, const SlideG &Ge, const SlideG &Go) {
-    if constexpr (J < L / 2) {
-      constexpr int K16 = ((J * B) % L) * (16 / L);
-      cmac2_w16<K16>(S.X[J], S.Y[J], (J & 1) ? Go : Ge);
-      SlideBins<L, B, J + 1>::run(S, Ge, Go);
+    if constexpr (S_ < L) {
+      constexpr int K16 = ((S_ * B) % L) * (16 / L);
+      cmac2_w16<K16>(S.X[S_], S.Y[S_], (S_ & 1) ? Go : Ge);
+      SlideBins<L, B, S_ + 1>::run(S, Ge, Go);
     }
   }
 };
 
-// load the operands of the update t -> t+1 (rows t and t+w, warp-uniform twiddle W_Nt^{rho t})
+// load the operands of the update t -> t+1 (rows t and t+w of both columns, warp-uniform twiddle)
 template <int L, bool MODD>
 __device__ __forceinline__ void slide_prefetch(SlideState<L> &S, uint32_t t) {
   const uint32_t off = t * S.rowb;
   // row t+w is new to this SM: pull the row SLIDE_PF steps ahead into L1 now, so that the register
-  // load one step ahead is an L1 hit (the Y buffer carries SLIDE_PF + 1 padding rows)
+  // load one step ahead is an L1 hit (the Y buffer carries SLIDE_PF + 2 padding rows)
   asm volatile("prefetch.global.L1 [%0];" ::"l"(S.pin + off + SLIDE_PF * S.rowb));
-  S.yin = __ldg((const float2 *)(S.pin + off));
-  S.yout = __ldg((const float2 *)(S.pout + off));
-  if constexpr (!MODD) S.tw = __ldg((const float2 *)(S.twt + (((S.rho * t) & S.ntmask) << 3)));
+  ldg2(S.pin + off, S.xin, S.yin);
+  ldg2(S.pout + off, S.xout, S.yout);
+  if constexpr (!MODD) ldg2(S.tw4 + (((S.rho * t) & S.ntmask) << 4), S.twx, S.twy);
 }
 
 // advance window t0 -> t0+1;  B = t0 mod L (compile time).  Uses the operands prefetched one step
-// ago and prefetches those of t0+1 (row t0+1+w <= nap: the Y buffer carries one padding row).
+// ago and prefetches those of t0+1.
 template <int L, int B, bool MODD>
 __device__ __forceinline__ void slide_update(SlideState<L> &S, uint32_t t0) {
-  const float2 yin = S.yin, yout = S.yout, tw = S.tw;
+  const f32x2 xin = S.xin, yin = S.yin, xout = S.xout, yout = S.yout, twx = S.twx, twy = S.twy;
   slide_prefetch<L, MODD>(S, t0 + 1);
   if constexpr (MODD) {
     // M == 1, rho == 0: the thread holds every rate bin, both parities; W_Nt = W_L
-    const SlideG Ge = slide_make_g<B>(yin.x - yout.x, yin.y - yout.y);
-    const SlideG Go = slide_make_g<B>(-yin.x - yout.x, -yin.y - yout.y);
+    const SlideG Ge = slide_make_g(sub2(xin, xout), sub2(yin, yout));
+    const SlideG Go = slide_make_g(sub2(neg2(xin), xout), sub2(neg2(yin), yout));
     SlideBins<L, B, 0>::run(S, Ge, Go);
   } else {
     // M even: every bin has rho's parity; g = W_Nt^{rho t0} ((-1)^rho y_in - y_out)
-    const float2 dl = make_float2(fmaf(S.sgn, yin.x, -yout.x), fmaf(S.sgn, yin.y, -yout.y));
-    const float2 g = cmul(dl, tw);
-    const SlideG G = slide_make_g<B>(g.x, g.y);
+    const f32x2 dx = fma2(xin, S.sgn2, neg2(xout)), dy = fma2(yin, S.sgn2, neg2(yout));
+    const f32x2 gx = fma2(dx, twx, mul2(dy, neg2(twy)));
+    const f32x2 gy = fma2(dx, twy, mul2(dy, twx));
+    const SlideG G = slide_make_g(gx, gy);
     SlideBins<L, B, 0>::run(S, G, G);
   }
 }
@@ -214,6 +216,32 @@ struct SlideSteps {
   }
 };
 
+// exact transform of window T0 for ONE column (col = 0/1 of the pair):
+//   A[rho + M s] = sum_{t2<L} W_L^{s t2} f[t2],  f[t2] = sum_{t1} y[T0+t2+L t1] W_Nt^{rho (t2+L t1)}
+// (T0 = 0 mod Nt, so absolute and window-relative phases coincide).  Result in natural s order.
+template <int L, bool MODD>
+__device__ __forceinline__ void slide_start_column(float2 (&A)[L], const char *pout, uint32_t rowb, uint32_t T0,
+                                                   uint32_t w, const float2 *twt, uint32_t rho, uint32_t ntmask, int col) {
+  float2 f[L];
+#pragma unroll
+  for (int i = 0; i < L; ++i) f[i] = make_float2(0.f, 0.f);
+  for (uint32_t tb = 0; tb < w; tb += L) {
+#pragma unroll
+    for (int t2 = 0; t2 < L; ++t2) {
+      const uint32_t t = tb + t2;
+      if (t < w) {
+        const float *p = (const float *)(pout + (T0 + t) * rowb) + col;
+        const float2 y = make_float2(__ldg(p), __ldg(p + 2));
+        if constexpr (MODD) { f[t2].x += y.x; f[t2].y += y.y; }
+        else cmac(f[t2], y, __ldg(twt + ((rho * t) & ntmask)));
+      }
+    }
+  }
+  FftDif<L, 0, L>::run(f);
+#pragma unroll
+  for (int s = 0; s < L; ++s) A[s] = f[brev<L>(s)];
+}
+
 // L = min(16, Nt) bins per thread;  MODD <=> M == 1 (Nt <= 16).
 template <int L, bool MODD>
 __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(SlideArgs a) {
@@ -223,51 +251,34 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   long long wt = (long long)blockIdx.x * nwarps + warp;
   const uint32_t lane = threadIdx.x & 31u;
   const int M = 1 << a.log2m;
-  const int ndt = a.nf >> 5;
+  const int ndt = a.nf >> 6;                      // 64 columns per warp
   SlideState<L> S;
   S.lane = lane;
   S.rho = (uint32_t)(wt & (M - 1)); wt >>= a.log2m;
   const int dt = (int)(wt % ndt); wt /= ndt;
   const int sg = (int)(wt % a.nseg);
   const long long pl = wt / a.nseg;
-  const uint32_t d = (uint32_t)(dt * 32) + lane;
+  const uint32_t c = (uint32_t)(dt * 32) + lane;  // column pair (2c, 2c+1)
   S.ntmask = (uint32_t)(a.nt - 1);
-  S.idx0 = S.rho * (uint32_t)a.nf + d;            // plane index r * nf + d of bin s: r = rho + M s
+  S.idx0 = S.rho * (uint32_t)a.nf + 2u * c;       // plane index r * nf + d of bin s: r = rho + M s
   S.idxs = (uint32_t)a.nf << a.log2m;
-  S.sgn = (S.rho & 1u) ? -1.f : 1.f;
+  const float sg1 = (S.rho & 1u) ? -1.f : 1.f;
+  S.sgn2 = pk(sg1, sg1);
   S.keymask = a.keymask;
   S.rowb = (uint32_t)a.pitch * 8u;
-  S.pout = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch + d);
+  S.pout = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch) + (size_t)c * 16u;
   S.pin = S.pout + (size_t)a.w * S.rowb;
-  S.twt = (const char *)a.twt;
+  S.tw4 = (const char *)a.tw4;
   S.keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
   const uint32_t T0 = (uint32_t)sg * (uint32_t)a.seg;                 // multiple of Nt and of L
   const uint32_t tend = min((uint32_t)a.nwin, T0 + (uint32_t)a.seg);  // windows [T0, tend)
   slide_prefetch<L, MODD>(S, T0);
-
-  // exact start: A[rho + M s] = sum_{t2<L} W_L^{s t2} f[t2],  f[t2] = sum_{t1} y[T0+t2+L t1] W_Nt^{rho (t2+L t1)}
-  // (T0 = 0 mod Nt, so absolute and window-relative phases coincide here)
   {
-    float2 f[L];
+    float2 Aa[L], Ab[L];
+    slide_start_column<L, MODD>(Aa, S.pout, S.rowb, T0, (uint32_t)a.w, a.twt, S.rho, S.ntmask, 0);
+    slide_start_column<L, MODD>(Ab, S.pout, S.rowb, T0, (uint32_t)a.w, a.twt, S.rho, S.ntmask, 1);
 #pragma unroll
-    for (int i = 0; i < L; ++i) f[i] = make_float2(0.f, 0.f);
-    for (uint32_t tb = 0; tb < (uint32_t)a.w; tb += L) {
-#pragma unroll
-      for (int t2 = 0; t2 < L; ++t2) {
-        const uint32_t t = tb + t2;
-        if (t < (uint32_t)a.w) {
-          const float2 y = __ldg((const float2 *)(S.pout + (T0 + t) * S.rowb));
-          if constexpr (MODD) { f[t2].x += y.x; f[t2].y += y.y; }
-          else cmac(f[t2], y, __ldg((const float2 *)(S.twt + (((S.rho * t) & S.ntmask) << 3))));
-        }
-      }
-    }
-    FftDif<L, 0, L>::run(f);
-#pragma unroll
-    for (int j = 0; j < L / 2; ++j) {
-      S.X[j] = pk(f[brev<L>(j)].x, f[brev<L>(j + L / 2)].x);
-      S.Y[j] = pk(f[brev<L>(j)].y, f[brev<L>(j + L / 2)].y);
-    }
+    for (int s = 0; s < L; ++s) { S.X[s] = pk(Aa[s].x, Ab[s].x); S.Y[s] = pk(Aa[s].y, Ab[s].y); }
   }
 
   uint32_t t0 = T0, buf = 0;

@@ -34,6 +34,7 @@ struct WidthPlan {
   int w, s, nt, L, log2m;
   long long nwin;       // per pair
   size_t tw_off;        // offset (float2) of its rate twiddle table in d_tables
+  size_t tw4_off;       // offset (float2, even) of the pre-broadcast copy (re, re, im, im) used by k_slide
   bool slide;           // stride-1 sliding-sum kernel (kernels_slide.cuh) instead of the generic one
   bool colfft;          // two-pass shared-memory column FFT (kernels_colfft.cuh): Nt = 32..512, nf % 32 == 0
   int cf_l1, cf_nz, cf_wpc, cf_nrange;
@@ -96,7 +97,7 @@ static cudaError_t launch_colfft(const ColFftArgs &a, int l1, int nz, long long 
 
 static void launch_slide(const SlideArgs &a, cudaStream_t st) {
   // every warp of a CTA must share its (pair, segment): warps per CTA = min(SLIDE_WARPS, ndt * M)
-  const long long per_seg = (long long)(a.nf / 32) << a.log2m;
+  const long long per_seg = (long long)(a.nf / 64) << a.log2m;
   const int wpb = (int)std::min<long long>(SLIDE_WARPS, per_seg);
   const unsigned blocks = (unsigned)(a.ntasks / wpb);
   const int thr = wpb * 32;
@@ -114,6 +115,7 @@ struct volks_plan {
   std::vector<WidthPlan> wp;
   float2 *d_tables = nullptr;  // [nf] delay twiddles, then per width [nt] rate twiddles
   int nchan = 0, pitch = 0;
+  int paired = 0;               // Y rows pair-interleaved (common.cuh ld_y)
   int wid1 = -1;                // a width with w == 1 whose peaks the row kernel emits itself (or -1)
   long long npair = 0;
   // workspace layout (byte offsets)
@@ -190,7 +192,7 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
     w.L = std::min(16, w.nt);
     w.log2m = ilog2(w.nt / w.L);
     // sliding-sum path: stride 1, pad x2 in time, whole warps of delay columns, 32-bit row offsets
-    w.slide = !force_generic && w.s == 1 && w.w >= 2 && w.nt == 2 * w.w && p->nf >= 32 &&
+    w.slide = !force_generic && w.s == 1 && w.w >= 2 && w.nt == 2 * w.w && p->nf >= 64 &&
               ((long long)p->nap + SLIDE_PF + 2) * (p->nf + 64) * 8 < (1LL << 32);
     w.colfft = !force_generic && !w.slide && w.nt >= 32 && w.nt <= 512 && p->nf >= 32 && w.nwin > 0;
     w.cf_l1 = w.nt / 16;
@@ -204,6 +206,9 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
     w.nseg = w.nwin > 0 ? (int)((w.nwin + w.seg - 1) / w.seg) : 0;
     w.tw_off = tw_total;
     tw_total += (size_t)w.nt;
+    tw_total += tw_total & 1;          // 16-byte alignment of the float4 copy
+    w.tw4_off = tw_total;
+    tw_total += (size_t)2 * w.nt;
     s.width[q] = w.w; s.stride[q] = w.s; s.nt[q] = w.nt; s.nwin[q] = w.nwin; s.offc[q] = per_pair;
     per_pair += w.nwin;
     pl->wp.push_back(w);
@@ -225,6 +230,7 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
   // Y row pitch: nf + 16 elements (one 128-byte line) when rows would otherwise sit a power of two
   // apart and fall into the same few L1 sets (kernels_slide.cuh reads w+1 rows of a column tile)
   pl->pitch = p->nf >= 32 ? p->nf + env_int("VOLKS_Y_PAD", 16) : p->nf;
+  pl->paired = p->nf >= 2 ? 1 : 0;
   const size_t y_pair = (size_t)p->nap * pl->pitch * sizeof(float2);
   const size_t budget = (size_t)4 << 30;
   long long ppc = y_pair ? (long long)std::max<size_t>(1, budget / std::max<size_t>(y_pair, 1)) : pl->npair;
@@ -260,6 +266,8 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
     for (int k = 0; k < w.nt; ++k) {
       const double a = -2.0 * PI * k / w.nt;
       tab[w.tw_off + k] = make_float2((float)cos(a), (float)sin(a));
+      tab[w.tw4_off + 2 * k] = make_float2((float)cos(a), (float)cos(a));
+      tab[w.tw4_off + 2 * k + 1] = make_float2((float)sin(a), (float)sin(a));
     }
   bool ok = cuda_ok(cudaMalloc(&pl->d_tables, tw_total * sizeof(float2))) &&
             cuda_ok(cudaMalloc(&pl->d_sched, sizeof(Sched))) &&
@@ -316,7 +324,7 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
     RowArgs ra;
     ra.vis = (const float2 *)d_vis; ra.Y = Y; ra.E = E; ra.twf = pl->d_tables;
     ra.row0 = pair0 * s.nap; ra.nrows = np * s.nap;
-    ra.nchan = pl->nchan; ra.nf = s.nf; ra.tpr = pl->row_tpr; ra.rows_per_cta = pl->row_rows_per_cta; ra.pitch = pl->pitch;
+    ra.nchan = pl->nchan; ra.nf = s.nf; ra.tpr = pl->row_tpr; ra.rows_per_cta = pl->row_rows_per_cta; ra.pitch = pl->pitch; ra.paired = pl->paired;
     ra.keys1 = nullptr; ra.per_pair = s.per_pair; ra.nap = s.nap; ra.stride1 = 1; ra.nwin1 = 0;
     if (pl->wid1 >= 0) { ra.keys1 = keys + s.offc[pl->wid1]; ra.stride1 = s.stride[pl->wid1]; ra.nwin1 = (int)s.nwin[pl->wid1]; }
     const long long rblocks = (ra.nrows + ra.rows_per_cta - 1) / ra.rows_per_cta;
@@ -331,15 +339,15 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
       ca.Y = Y; ca.keys = keys; ca.twt = pl->d_tables + w.tw_off;
       ca.per_pair = s.per_pair; ca.offc = s.offc[q]; ca.pair0 = pair0;
       ca.nap = s.nap; ca.nf = s.nf; ca.log2nf = s.log2nf; ca.w = w.w; ca.stride = w.s; ca.nt = w.nt;
-      ca.log2m = w.log2m; ca.nwin = (int)w.nwin; ca.pitch = pl->pitch;
+      ca.log2m = w.log2m; ca.nwin = (int)w.nwin; ca.pitch = pl->pitch; ca.paired = pl->paired;
       ca.total = ((np * w.nwin) << w.log2m) * s.nf;
       if (w.slide) {
         SlideArgs sa;
-        sa.Y = Y; sa.keys = keys; sa.twt = pl->d_tables + w.tw_off;
+        sa.Y = Y; sa.keys = keys; sa.twt = pl->d_tables + w.tw_off; sa.tw4 = (const float4 *)(pl->d_tables + w.tw4_off);
         sa.per_pair = s.per_pair; sa.offc = s.offc[q]; sa.pair0 = pair0;
         sa.nap = s.nap; sa.nf = s.nf; sa.w = w.w; sa.nt = w.nt; sa.log2m = w.log2m; sa.nwin = (int)w.nwin;
         sa.seg = w.seg; sa.nseg = w.nseg; sa.keymask = 0xFFFFFFF0u; sa.pitch = pl->pitch;
-        sa.ntasks = ((np * w.nseg * (long long)(s.nf / 32)) << w.log2m);
+        sa.ntasks = ((np * w.nseg * (long long)(s.nf / 64)) << w.log2m);
         ProfScope ps(pl, st, VOLKS_K_SLIDE, q);
         launch_slide(sa, st);
         continue;
@@ -349,7 +357,7 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
         fa.Y = Y; fa.keys = keys; fa.twt = pl->d_tables + w.tw_off;
         fa.per_pair = s.per_pair; fa.offc = s.offc[q]; fa.pair0 = pair0;
         fa.nap = s.nap; fa.nf = s.nf; fa.w = w.w; fa.stride = w.s; fa.nt = w.nt; fa.nwin = (int)w.nwin;
-        fa.pitch = pl->pitch; fa.wpc = w.cf_wpc; fa.nrange = w.cf_nrange; fa.keymask = 0xFFFFFFF0u;
+        fa.pitch = pl->pitch; fa.paired = pl->paired; fa.wpc = w.cf_wpc; fa.nrange = w.cf_nrange; fa.keymask = 0xFFFFFFF0u;
         ProfScope ps(pl, st, VOLKS_K_COLFFT, q);
         if (!cuda_ok(launch_colfft(fa, w.cf_l1, w.cf_nz, np * (s.nf / 32) * w.cf_nrange, st, false))) return VOLKS_ECUDA;
         continue;
