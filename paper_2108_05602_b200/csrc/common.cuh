@@ -67,6 +67,75 @@ __host__ __device__ constexpr int brev(int i) {
   return r;
 }
 
+// ---- packed FP32 (sm_100a fma.rn.f32x2 / add / sub / mul .f32x2 -> SASS FFMA2 / FADD2 / FMUL2) ----
+typedef unsigned long long f32x2;   // two packed floats (lo, hi) in one 64-bit register pair
+
+__device__ __forceinline__ f32x2 pk(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ float lo32(f32x2 v) { float a, b; asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); (void)b; return a; }
+__device__ __forceinline__ float hi32(f32x2 v) { float a, b; asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); (void)a; return b; }
+__device__ __forceinline__ f32x2 neg2(f32x2 v) { return pk(-lo32(v), -hi32(v)); }   // folds into an operand modifier
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+// 128-bit read-only load as two register pairs
+__device__ __forceinline__ void ldg2(const void *p, f32x2 &a, f32x2 &b) {
+  asm volatile("ld.global.nc.v2.b64 {%0,%1}, [%2];" : "=l"(a), "=l"(b) : "l"(p));
+}
+
+// complex numbers as packed pairs (lo = re, hi = im)
+__device__ __forceinline__ f32x2 c2_from(float2 z) { return pk(z.x, z.y); }
+// (y, -x) = -i z : a swap + sign operand modifier for the consuming instruction
+__device__ __forceinline__ f32x2 c2_mulnegi(f32x2 z) { return pk(hi32(z), -lo32(z)); }
+// z * (c - i s) for real constants c, s:  (x c + y s, y c - x s)
+__device__ __forceinline__ f32x2 c2_mulcs(f32x2 z, float c, float s) { return fma2(c2_mulnegi(z), pk(s, s), mul2(z, pk(c, c))); }
+
+// z * exp(-2 pi i K/N), N in {2,4,8,16,32}, 0 <= K < N/2, compile time
+template <int K, int N>
+__device__ __forceinline__ f32x2 c2_mul_w(f32x2 z) {
+  constexpr int k32 = K * (32 / N);
+  static_assert(k32 >= 0 && k32 < 16, "first-half twiddles only");
+  constexpr float H = 0.70710678118654752f;
+  constexpr float C[16] = {1.f, 0.98078528040323043f, 0.92387953251128674f, 0.83146961230254524f, H, 0.55557023301960218f,
+                           0.38268343236508977f, 0.19509032201612825f, 0.f, -0.19509032201612825f, -0.38268343236508977f,
+                           -0.55557023301960218f, -H, -0.83146961230254524f, -0.92387953251128674f, -0.98078528040323043f};
+  constexpr float S[16] = {0.f, 0.19509032201612825f, 0.38268343236508977f, 0.55557023301960218f, H, 0.83146961230254524f,
+                           0.92387953251128674f, 0.98078528040323043f, 1.f, 0.98078528040323043f, 0.92387953251128674f,
+                           0.83146961230254524f, H, 0.55557023301960218f, 0.38268343236508977f, 0.19509032201612825f};
+  if constexpr (k32 == 0) return z;
+  else if constexpr (k32 == 8) return c2_mulnegi(z);
+  else if constexpr (k32 == 4) return mul2(add2(z, c2_mulnegi(z)), pk(H, H));    // H (x + y, y - x)
+  else if constexpr (k32 == 12) return mul2(sub2(c2_mulnegi(z), z), pk(H, H));   // H (y - x, -x - y)
+  else return c2_mulcs(z, C[k32], S[k32]);
+}
+
+// Packed in-register radix-2 DIF FFT of N (<= 32) points a[OFF .. OFF+N), forward, output
+// BIT-REVERSED, only the first NZ inputs non-zero (NZ = N: the plain transform).
+template <int N, int NZ, int OFF, int TOTAL>
+struct FftDif2 {
+  template <int K>
+  static __device__ __forceinline__ void stage(f32x2 (&a)[TOTAL]) {
+    if constexpr (K < N / 2) {
+      if constexpr (NZ <= N / 2) {
+        if constexpr (K < NZ) a[OFF + K + N / 2] = c2_mul_w<K, N>(a[OFF + K]);
+      } else {
+        const f32x2 u = a[OFF + K], v = a[OFF + K + N / 2];
+        a[OFF + K] = add2(u, v);
+        a[OFF + K + N / 2] = c2_mul_w<K, N>(sub2(u, v));
+      }
+      stage<K + 1>(a);
+    }
+  }
+  static __device__ __forceinline__ void run(f32x2 (&a)[TOTAL]) {
+    if constexpr (N >= 2) {
+      stage<0>(a);
+      constexpr int NZ2 = NZ < N / 2 ? NZ : N / 2;
+      FftDif2<N / 2, NZ2, OFF, TOTAL>::run(a);
+      FftDif2<N / 2, NZ2, OFF + N / 2, TOTAL>::run(a);
+    }
+  }
+};
+
 // Delay-spectrum intermediate Y.  Rows of `pitch` complex elements.  When `paired` the two columns
 // 2c, 2c+1 of a row share one float4 (re[2c], re[2c+1], im[2c], im[2c+1]) - the layout the packed
 // sliding kernel loads straight into (column a, column b) register pairs; otherwise plain float2.

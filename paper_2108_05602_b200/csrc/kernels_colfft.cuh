@@ -25,7 +25,7 @@ constexpr int CF_WARPS = 16;
 struct ColFftArgs {
   const float2 *Y;      // [npairs_chunk][nap][pitch]
   u64 *keys;            // canonical window keys
-  const float2 *twt;    // [nt] exp(-2 pi i k/nt)
+  const float4 *tw4;    // [nt] exp(-2 pi i k/nt), pre-broadcast (re, re, im, im)
   long long per_pair, offc, pair0;
   int nap, nf, w, stride, nt, nwin, pitch, paired;
   int wpc;              // windows per CTA (consecutive)
@@ -84,12 +84,13 @@ struct FftDifPruned {
 };
 
 // L1 = Nt/16 (2..32), NZ = leading non-zero inputs of the L1-point transform (power of two <= L1).
+// Complex values travel as packed pairs (re, im): butterflies are FADD2, twiddles two FFMA2/FMUL2.
 template <int L1, int NZ>
 __global__ void __launch_bounds__(CF_WARPS * 32) k_colfft(ColFftArgs a) {
-  extern __shared__ float2 cf_sm[];
-  float2 *S = cf_sm;                                   // [L1][16][32]
-  float2 *tws = cf_sm + (size_t)L1 * 16 * 32;          // [nt] rate twiddles
-  u64 *slots = (u64 *)(tws + a.nt);                    // [L1] per-residue window keys
+  extern __shared__ float4 cf_sm4[];
+  float4 *tw4s = cf_sm4;                                // [nt] rate twiddles (re, re, im, im)
+  f32x2 *S = (f32x2 *)(cf_sm4 + a.nt);                  // [L1][16][32]
+  u64 *slots = (u64 *)(S + (size_t)L1 * 16 * 32);       // [L1] per-residue window keys
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int ntile = a.nf >> 5;
   long long u = blockIdx.x;
@@ -99,36 +100,51 @@ __global__ void __launch_bounds__(CF_WARPS * 32) k_colfft(ColFftArgs a) {
   const int d = tile * 32 + lane;
   const size_t prow = (size_t)pl * a.nap;
   u64 *keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
-  for (int i = threadIdx.x; i < a.nt; i += CF_WARPS * 32) tws[i] = a.twt[i];
+  for (int i = threadIdx.x; i < a.nt; i += CF_WARPS * 32) tw4s[i] = a.tw4[i];
   const int j0 = rg * a.wpc, j1 = min(a.nwin, j0 + a.wpc);
   const int ntm = a.nt - 1;
 
-  for (int j = j0; j < j1; ++j) {
+  // pass-1 inputs of a window: rows t0 + warp + 16 t1 of this lane's column (zero beyond the window)
+  f32x2 zin[NZ];
+  auto load_window = [&](int j) {
     const int t0 = j * a.stride;
+#pragma unroll
+    for (int t1 = 0; t1 < NZ; ++t1) {
+      const int t = warp + 16 * t1;
+      zin[t1] = (j < j1 && t < a.w) ? c2_from(ld_y(a.Y, (prow + t0 + t) * a.pitch, d, a.paired)) : pk(0.f, 0.f);
+    }
+  };
+  load_window(j0);
+
+  for (int j = j0; j < j1; ++j) {
     // ---- pass 1: warp = t2, L1-point pruned FFT over t1 ----
     {
       const int t2 = warp;
-      float2 z[L1];
+      f32x2 z[L1];
 #pragma unroll
-      for (int t1 = 0; t1 < NZ; ++t1) {
-        const int t = t2 + 16 * t1;
-        z[t1] = t < a.w ? ld_y(a.Y, (prow + t0 + t) * a.pitch, d, a.paired) : make_float2(0.f, 0.f);
-      }
-      FftDifPruned<L1, NZ, 0, L1>::run(z);
+      for (int t1 = 0; t1 < NZ; ++t1) z[t1] = zin[t1];
+      FftDif2<L1, NZ, 0, L1>::run(z);
 #pragma unroll
       for (int i = 0; i < L1; ++i) S[(brev<L1>(i) * 16 + t2) * 32 + lane] = z[i];
     }
+    load_window(j + 1);   // in flight during pass 2
     __syncthreads();
     // ---- pass 2: warp = residue rho, 16-point FFT over t2, power, tagged key ----
     for (int rho = warp; rho < L1; rho += CF_WARPS) {
-      float2 f[16];
+      f32x2 f[16];
 #pragma unroll
-      for (int t2 = 0; t2 < 16; ++t2) f[t2] = cmul(S[(rho * 16 + t2) * 32 + lane], tws[(rho * t2) & ntm]);
-      FftDif<16, 0, 16>::run(f);
+      for (int t2 = 0; t2 < 16; ++t2) {
+        const f32x2 z = S[(rho * 16 + t2) * 32 + lane];
+        const float4 w4 = tw4s[(rho * t2) & ntm];
+        // z * w = (zx wx - zy wy, zx wy + zy wx)
+        f[t2] = fma2(pk(-hi32(z), lo32(z)), pk(w4.z, w4.w), mul2(z, pk(w4.x, w4.y)));
+      }
+      FftDif2<16, 16, 0, 16>::run(f);
       uint32_t best = 0;
 #pragma unroll
       for (int i = 0; i < 16; ++i) {
-        const uint32_t k = (__float_as_uint(cnorm(f[i])) & a.keymask) | (uint32_t)(15 - brev<16>(i));
+        const f32x2 q = mul2(f[i], f[i]);
+        const uint32_t k = (__float_as_uint(lo32(q) + hi32(q)) & a.keymask) | (uint32_t)(15 - brev<16>(i));
         best = max(best, k);
       }
       const uint32_t km = __reduce_max_sync(0xffffffffu, best);

@@ -56,21 +56,6 @@ struct SlideArgs {
   uint32_t keymask;     // 0xFFFFFFF0, passed as data so that (p & mask) | id is ONE LOP3 (register mask)
 };
 
-typedef unsigned long long f32x2;   // two packed floats (lo, hi) in one 64-bit register pair
-
-__device__ __forceinline__ f32x2 pk(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
-__device__ __forceinline__ float lo32(f32x2 v) { float a, b; asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); (void)b; return a; }
-__device__ __forceinline__ float hi32(f32x2 v) { float a, b; asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); (void)a; return b; }
-__device__ __forceinline__ f32x2 neg2(f32x2 v) { return pk(-lo32(v), -hi32(v)); }   // folds into an operand modifier
-__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
-__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
-__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
-__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
-// 128-bit read-only load as two register pairs
-__device__ __forceinline__ void ldg2(const void *p, f32x2 &a, f32x2 &b) {
-  asm volatile("ld.global.nc.v2.b64 {%0,%1}, [%2];" : "=l"(a), "=l"(b) : "l"(p));
-}
-
 // The per-step operand of one parity class, both columns: g = (GX, GY) and the (1 -+ i)/sqrt 2
 // products of the even twiddles (dead code in steps that have no such bin).
 struct SlideG { f32x2 GX, GY, PP, QQ; };

@@ -59,7 +59,7 @@ static void launch_col(const ColArgs &a, cudaStream_t st) {
   k_col<L><<<(unsigned)blocks, 256, 0, st>>>(a);
 }
 
-inline size_t colfft_smem(int l1, int nt) { return (size_t)l1 * 16 * 32 * sizeof(float2) + (size_t)nt * sizeof(float2) + (size_t)l1 * sizeof(u64); }
+inline size_t colfft_smem(int l1, int nt) { return (size_t)l1 * 16 * 32 * sizeof(float2) + (size_t)nt * sizeof(float4) + (size_t)l1 * sizeof(u64); }
 
 template <int L1, int NZ>
 static cudaError_t colfft_one(const ColFftArgs &a, unsigned blocks, cudaStream_t st, bool attr_only) {
@@ -354,7 +354,7 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
       }
       if (w.colfft) {
         ColFftArgs fa;
-        fa.Y = Y; fa.keys = keys; fa.twt = pl->d_tables + w.tw_off;
+        fa.Y = Y; fa.keys = keys; fa.tw4 = (const float4 *)(pl->d_tables + w.tw4_off);
         fa.per_pair = s.per_pair; fa.offc = s.offc[q]; fa.pair0 = pair0;
         fa.nap = s.nap; fa.nf = s.nf; fa.w = w.w; fa.stride = w.s; fa.nt = w.nt; fa.nwin = (int)w.nwin;
         fa.pitch = pl->pitch; fa.paired = pl->paired; fa.wpc = w.cf_wpc; fa.nrange = w.cf_nrange; fa.keymask = 0xFFFFFFF0u;

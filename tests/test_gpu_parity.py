@@ -95,6 +95,22 @@ def test_edge_shapes(vb, oracle, shape):
     run_both(vb, oracle, vis, c, mode="fft")
 
 
+@pytest.mark.parametrize("shape", [
+    # stride-1, pad x2 widths on nf >= 64: the sliding-sum kernels (every L / M variant), ragged tails
+    (1, 1, 20, 33, [2, 4, 8], [1, 1, 1], [4, 8, 16], 64),        # fewer windows than one unrolled block
+    (2, 1, 47, 64, [16, 32], [1, 1], [32, 64], 64),              # M = 2, 4; nwin = 32, 16
+    (1, 2, 300, 40, [2, 64, 128], [1, 1, 1], [4, 128, 256], 128),  # M = 8, 16; segment seam at 256
+    (1, 1, 530, 17, [8, 16], [1, 1], [16, 32], 256),             # several column groups per CTA
+])
+def test_sliding_kernel_shapes(vb, oracle, shape):
+    nbl, nif, nap, nchan, widths, strides, nts, nf = shape
+    g = torch.Generator().manual_seed(nap * 11 + nchan)
+    vis = torch.view_as_complex(torch.randn((nbl, nif, nap, nchan, 2), generator=g) * 0.7071)
+    vis[0, 0, nap // 2: nap // 2 + 5] += 1.5 + 0.5j              # a coherent burst (a clear peak)
+    c = dict(widths=widths, strides=strides, nts=nts, nf=nf, snr_thresh=2.5)
+    run_both(vb, oracle, vis, c, mode="fft")
+
+
 def test_zero_windows_and_empty(vb):
     vis = torch.zeros((1, 1, 3, 8), dtype=torch.complex64)
     cands, n, peaks = vb.fringe_search(vis.cuda(), [4], [1], [8], 8, 6.0, want_peaks=True)
