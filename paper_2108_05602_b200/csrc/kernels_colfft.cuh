@@ -130,28 +130,40 @@ __global__ void __launch_bounds__(CF_WARPS * 32) k_colfft(ColFftArgs a) {
     load_window(j + 1);   // in flight during pass 2
     __syncthreads();
     // ---- pass 2: warp = residue rho, 16-point FFT over t2, power, tagged key ----
-    for (int rho = warp; rho < L1; rho += CF_WARPS) {
-      f32x2 f[16];
+    // (for L1 = 32 a warp owns two residues and works on both at once: twice the independent work
+    //  under each shared-memory load and each dependent FFT stage)
+    constexpr int RH = L1 > CF_WARPS ? L1 / CF_WARPS : 1;
+    if (warp < L1) {
+      f32x2 f[RH][16];
 #pragma unroll
-      for (int t2 = 0; t2 < 16; ++t2) {
-        const f32x2 z = S[(rho * 16 + t2) * 32 + lane];
-        const float4 w4 = tw4s[(rho * t2) & ntm];
-        // z * w = (zx wx - zy wy, zx wy + zy wx)
-        f[t2] = fma2(pk(-hi32(z), lo32(z)), pk(w4.z, w4.w), mul2(z, pk(w4.x, w4.y)));
-      }
-      FftDif2<16, 16, 0, 16>::run(f);
-      uint32_t best = 0;
+      for (int h = 0; h < RH; ++h) {
+        const int rho = warp + h * CF_WARPS;
 #pragma unroll
-      for (int i = 0; i < 16; ++i) {
-        const f32x2 q = mul2(f[i], f[i]);
-        const uint32_t k = (__float_as_uint(lo32(q) + hi32(q)) & a.keymask) | (uint32_t)(15 - brev<16>(i));
-        best = max(best, k);
+        for (int t2 = 0; t2 < 16; ++t2) {
+          const f32x2 z = S[(rho * 16 + t2) * 32 + lane];
+          const float4 w4 = tw4s[(rho * t2) & ntm];
+          // z * w = (zx wx - zy wy, zx wy + zy wx)
+          f[h][t2] = fma2(pk(-hi32(z), lo32(z)), pk(w4.z, w4.w), mul2(z, pk(w4.x, w4.y)));
+        }
       }
-      const uint32_t km = __reduce_max_sync(0xffffffffu, best);
-      const uint32_t tied = __ballot_sync(0xffffffffu, best == km);
-      if (lane == __ffs(tied) - 1) {
-        const uint32_t s = 15u - (km & 15u);
-        slots[rho] = make_key(__uint_as_float(km & 0xFFFFFFF0u), (uint32_t)(rho + L1 * s) * (uint32_t)a.nf + (uint32_t)d);
+#pragma unroll
+      for (int h = 0; h < RH; ++h) FftDif2<16, 16, 0, 16>::run(f[h]);
+#pragma unroll
+      for (int h = 0; h < RH; ++h) {
+        const int rho = warp + h * CF_WARPS;
+        uint32_t best = 0;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          const f32x2 q = mul2(f[h][i], f[h][i]);
+          const uint32_t k = (__float_as_uint(lo32(q) + hi32(q)) & a.keymask) | (uint32_t)(15 - brev<16>(i));
+          best = max(best, k);
+        }
+        const uint32_t km = __reduce_max_sync(0xffffffffu, best);
+        const uint32_t tied = __ballot_sync(0xffffffffu, best == km);
+        if (lane == __ffs(tied) - 1) {
+          const uint32_t s = 15u - (km & 15u);
+          slots[rho] = make_key(__uint_as_float(km & 0xFFFFFFF0u), (uint32_t)(rho + L1 * s) * (uint32_t)a.nf + (uint32_t)d);
+        }
       }
     }
     __syncthreads();
