@@ -158,6 +158,81 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
 #undef ROW_SYNC
 
 // ------------------------------------------------------------------------------------------------
+// Row (delay) FFT, register form, for nf = N1 * N2 in {64, 128, 256}: n = n1 + N1 n2, k = N2 k1 + k2,
+//   X[N2 k1 + k2] = sum_{n1} W_N1^{n1 k1} [ W_nf^{n1 k2} sum_{n2} x[n1 + N1 n2] W_N2^{n2 k2} ].
+// A row is a group of N2 lanes (never spanning warps): step A, lane n1 < N1: N2-point packed DIF FFT
+// over n2 in registers, pruned to the NZA leading non-zero inputs (only nchan of nf are non-zero),
+// times W_nf^{n1 k2}, into shared memory; step C, lane k2: N1-point FFT over n1, paired store, the
+// w = 1 peak.  One warp barrier per row instead of log4(nf) block barriers.
+// ------------------------------------------------------------------------------------------------
+template <int N1, int N2, int NZA>
+__global__ void __launch_bounds__(256) k_row2(RowArgs a) {
+  static_assert(N1 <= N2 && N2 <= 16, "row group = N2 lanes");
+  constexpr int G = N2, RPC = 256 / G, EP = N2 + 1;
+  __shared__ f32x2 ex[RPC * N1 * EP];
+  const int g = threadIdx.x / G, l = threadIdx.x % G;
+  const long long rrel = (long long)blockIdx.x * RPC + g;
+  const bool live = rrel < a.nrows;
+  f32x2 *E = ex + g * (N1 * EP);
+  float e = 0.f;
+  if (l < N1) {
+    f32x2 z[N2];
+    const float2 *src = a.vis + (a.row0 + rrel) * (long long)a.nchan;
+#pragma unroll
+    for (int n2 = 0; n2 < NZA; ++n2) {
+      const int n = l + N1 * n2;
+      float2 v = make_float2(0.f, 0.f);
+      if (live && n < a.nchan) { v = __ldg(src + n); e += cnorm(v); }
+      z[n2] = c2_from(v);
+    }
+    FftDif2<N2, NZA, 0, N2>::run(z);
+#pragma unroll
+    for (int i = 0; i < N2; ++i) {
+      constexpr int dummy = 0; (void)dummy;
+      const int k2 = brev<N2>(i);
+      const float2 tw = __ldg(a.twf + l * k2);          // W_nf^{n1 k2}, n1 k2 < nf
+      E[l * EP + k2] = fma2(pk(-hi32(z[i]), lo32(z[i])), pk(tw.y, tw.y), mul2(z[i], pk(tw.x, tw.x)));
+    }
+  }
+#pragma unroll
+  for (int o = G >> 1; o >= 1; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+  if (live && l == 0) a.E[a.row0 + rrel] = e;
+  __syncwarp();
+  f32x2 v[N1];
+#pragma unroll
+  for (int n1 = 0; n1 < N1; ++n1) v[n1] = E[n1 * EP + l];
+  FftDif2<N1, N1, 0, N1>::run(v);
+  u64 key = 0;
+  float *dst = (float *)(a.Y + rrel * (long long)a.pitch);
+#pragma unroll
+  for (int i = 0; i < N1; ++i) {
+    const int col = N2 * brev<N1>(i) + l;
+    const float re = lo32(v[i]), im = hi32(v[i]);
+    const float got = __shfl_xor_sync(0xffffffffu, (l & 1) ? re : im, 1);
+    if (live) {
+      float *p = dst + ((col >> 1) << 2) + ((l & 1) << 1);
+      *(float2 *)p = (l & 1) ? make_float2(got, im) : make_float2(re, got);
+    }
+    const u64 kk = make_key(fmaf(re, re, im * im), (uint32_t)col);
+    key = kk > key ? kk : key;
+  }
+  if (a.keys1) {   // uniform branch
+#pragma unroll
+    for (int o = G >> 1; o >= 1; o >>= 1) {
+      const u64 other = __shfl_xor_sync(0xffffffffu, key, o);
+      key = other > key ? other : key;
+    }
+    if (live && l == 0) {
+      const long long row = a.row0 + rrel;
+      const long long pair = row / a.nap;
+      const int t = (int)(row - pair * a.nap);
+      const int j = t / a.stride1;
+      if (j * a.stride1 == t && j < a.nwin1) a.keys1[pair * a.per_pair + j] = key;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Column (rate) transform + power + argmax, generic.
 // Thread task id (d fastest): ((pair_local * nwin + j) * M + rho) * nf + d.
 // ------------------------------------------------------------------------------------------------

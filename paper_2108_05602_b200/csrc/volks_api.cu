@@ -95,6 +95,31 @@ static cudaError_t launch_colfft(const ColFftArgs &a, int l1, int nz, long long 
   return cudaErrorInvalidValue;
 }
 
+template <int N1, int N2>
+static bool row2_nz(const RowArgs &a, int nza, unsigned blocks, cudaStream_t st) {
+  switch (nza) {
+    case 1: k_row2<N1, N2, 1><<<blocks, 256, 0, st>>>(a); return true;
+    case 2: k_row2<N1, N2, 2><<<blocks, 256, 0, st>>>(a); return true;
+    case 4: k_row2<N1, N2, 4><<<blocks, 256, 0, st>>>(a); return true;
+    case 8: k_row2<N1, N2, 8><<<blocks, 256, 0, st>>>(a); return true;
+    case 16: if constexpr (N2 >= 16) { k_row2<N1, N2, 16><<<blocks, 256, 0, st>>>(a); return true; } break;
+  }
+  return false;
+}
+
+// register-form row FFT for nf in {64, 128, 256} with the paired Y layout; false = not applicable
+static bool launch_row2(const RowArgs &a, cudaStream_t st) {
+  if (!a.paired) return false;
+  int n1, n2;
+  if (a.nf == 256) { n1 = 16; n2 = 16; } else if (a.nf == 128) { n1 = 8; n2 = 16; } else if (a.nf == 64) { n1 = 8; n2 = 8; } else return false;
+  int nza = 1;
+  while (nza * n1 < a.nchan) nza *= 2;                       // leading non-zero inputs of the N2-point transform
+  const unsigned blocks = (unsigned)((a.nrows + 256 / n2 - 1) / (256 / n2));
+  if (a.nf == 256) return row2_nz<16, 16>(a, nza, blocks, st);
+  if (a.nf == 128) return row2_nz<8, 16>(a, nza, blocks, st);
+  return row2_nz<8, 8>(a, nza, blocks, st);
+}
+
 static void launch_slide(const SlideArgs &a, cudaStream_t st) {
   // every warp of a CTA must share its (pair, segment): warps per CTA = min(SLIDE_WARPS, ndt * M)
   const long long per_seg = (long long)(a.nf / 64) << a.log2m;
@@ -116,6 +141,7 @@ struct volks_plan {
   float2 *d_tables = nullptr;  // [nf] delay twiddles, then per width [nt] rate twiddles
   int nchan = 0, pitch = 0;
   int paired = 0;               // Y rows pair-interleaved (common.cuh ld_y)
+  bool row_generic = false;     // VOLKS_PATH=generic: the shared-memory Stockham row kernel only
   int wid1 = -1;                // a width with w == 1 whose peaks the row kernel emits itself (or -1)
   long long npair = 0;
   // workspace layout (byte offsets)
@@ -231,6 +257,7 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
   // apart and fall into the same few L1 sets (kernels_slide.cuh reads w+1 rows of a column tile)
   pl->pitch = p->nf >= 32 ? p->nf + env_int("VOLKS_Y_PAD", 16) : p->nf;
   pl->paired = p->nf >= 2 ? 1 : 0;
+  pl->row_generic = force_generic;
   const size_t y_pair = (size_t)p->nap * pl->pitch * sizeof(float2);
   const size_t budget = (size_t)4 << 30;
   long long ppc = y_pair ? (long long)std::max<size_t>(1, budget / std::max<size_t>(y_pair, 1)) : pl->npair;
@@ -330,7 +357,8 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
     const long long rblocks = (ra.nrows + ra.rows_per_cta - 1) / ra.rows_per_cta;
     {
       ProfScope ps(pl, st, VOLKS_K_ROW, -1);
-      k_row_fft<<<(unsigned)rblocks, ra.tpr * ra.rows_per_cta, pl->row_smem, st>>>(ra);
+      if (pl->row_generic || !launch_row2(ra, st))
+        k_row_fft<<<(unsigned)rblocks, ra.tpr * ra.rows_per_cta, pl->row_smem, st>>>(ra);
     }
     for (int q = 0; q < s.nwidths; ++q) {
       const WidthPlan &w = pl->wp[q];
