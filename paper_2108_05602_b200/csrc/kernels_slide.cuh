@@ -103,6 +103,9 @@ struct SlideState {
   u64 *keyp;                    // canonical key of window t0 = keyp[t0]
   uint32_t rowb;                // bytes per Y row
   uint32_t ntmask, rho, idx0, idxs, keymask, lane;   // plane index of bin s, column a: idx0 + s * idxs
+  // RING variant: shared-memory addresses of this lane's entry in the ring rows of the current block's
+  // first leaving row (sm_out) and first entering row (sm_in); ring geometry in bytes
+  uint32_t sm_out, sm_in, ring_lo, ring_hi, rrowb;
 };
 
 // emit the window's contribution: per column the max of (power with its 4 low mantissa bits replaced
@@ -154,24 +157,40 @@ struct SlideBins {
   }
 };
 
-// load the operands of the update t -> t+1 (rows t and t+w of both columns, warp-uniform twiddle)
-template <int L, bool MODD>
+// 128-bit shared-memory load as two register pairs
+__device__ __forceinline__ void lds2(uint32_t addr, f32x2 &a, f32x2 &b) {
+  asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(a), "=l"(b) : "r"(addr));
+}
+
+// load the operands of the update t -> t+1 (rows t and t+w of both columns, warp-uniform twiddle).
+// BN = t - (first window of the current 16-step block), 0..16 (compile time; RING only).
+template <int L, bool MODD, bool RING, int BN>
 __device__ __forceinline__ void slide_prefetch(SlideState<L> &S, uint32_t t) {
-  const uint32_t off = t * S.rowb;
-  // row t+w is new to this SM: pull the row SLIDE_PF steps ahead into L1 now, so that the register
-  // load one step ahead is an L1 hit (the Y buffer carries SLIDE_PF + 2 padding rows)
-  asm volatile("prefetch.global.L1 [%0];" ::"l"(S.pin + off + SLIDE_PF * S.rowb));
-  ldg2(S.pin + off, S.xin, S.yin);
-  ldg2(S.pout + off, S.xout, S.yout);
+  if constexpr (RING) {
+    uint32_t ao = S.sm_out + BN * S.rrowb, ai = S.sm_in + BN * S.rrowb;
+    if constexpr (BN == 16) {   // first row of the next block: the ring may wrap here (and only here)
+      ao = ao >= S.ring_hi ? ao - (S.ring_hi - S.ring_lo) : ao;
+      ai = ai >= S.ring_hi ? ai - (S.ring_hi - S.ring_lo) : ai;
+    }
+    lds2(ai, S.xin, S.yin);
+    lds2(ao, S.xout, S.yout);
+  } else {
+    const uint32_t off = t * S.rowb;
+    // row t+w is new to this SM: pull the row SLIDE_PF steps ahead into L1 now, so that the register
+    // load one step ahead is an L1 hit (the Y buffer carries SLIDE_PF + 2 padding rows)
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(S.pin + off + SLIDE_PF * S.rowb));
+    ldg2(S.pin + off, S.xin, S.yin);
+    ldg2(S.pout + off, S.xout, S.yout);
+  }
   if constexpr (!MODD) ldg2(S.tw4 + (((S.rho * t) & S.ntmask) << 4), S.twx, S.twy);
 }
 
 // advance window t0 -> t0+1;  B = t0 mod L (compile time).  Uses the operands prefetched one step
 // ago and prefetches those of t0+1.
-template <int L, int B, bool MODD>
+template <int L, int B, bool MODD, bool RING>
 __device__ __forceinline__ void slide_update(SlideState<L> &S, uint32_t t0) {
   const f32x2 xin = S.xin, yin = S.yin, xout = S.xout, yout = S.yout, twx = S.twx, twy = S.twy;
-  slide_prefetch<L, MODD>(S, t0 + 1);
+  slide_prefetch<L, MODD, RING, B + 1>(S, t0 + 1);
   if constexpr (MODD) {
     // M == 1, rho == 0: the thread holds every rate bin, both parities; W_Nt = W_L
     const SlideG Ge = slide_make_g(sub2(xin, xout), sub2(yin, yout));
@@ -188,15 +207,15 @@ __device__ __forceinline__ void slide_update(SlideState<L> &S, uint32_t t0) {
 }
 
 // L consecutive steps starting at t0 (t0 mod L == 0).  GUARD: only windows < tend exist.
-template <int L, int B, bool MODD, bool GUARD>
+template <int L, int B, bool MODD, bool GUARD, bool RING>
 struct SlideSteps {
   static __device__ __forceinline__ void run(SlideState<L> &S, uint32_t t0, uint32_t tend, u64 *slot) {
     if constexpr (B < L) {
       if (!GUARD || t0 + B < tend) {
         slide_emit<L>(S, slot + B * SLIDE_WARPS);
-        if (!GUARD || t0 + B + 1 < tend) slide_update<L, B, MODD>(S, t0 + B);
+        if (!GUARD || t0 + B + 1 < tend) slide_update<L, B, MODD, RING>(S, t0 + B);
       }
-      SlideSteps<L, B + 1, MODD, GUARD>::run(S, t0, tend, slot);
+      SlideSteps<L, B + 1, MODD, GUARD, RING>::run(S, t0, tend, slot);
     }
   }
 };
@@ -227,11 +246,37 @@ __device__ __forceinline__ void slide_start_column(float2 (&A)[L], const char *p
   for (int s = 0; s < L; ++s) A[s] = f[brev<L>(s)];
 }
 
-// L = min(16, Nt) bins per thread;  MODD <=> M == 1 (Nt <= 16).
-template <int L, bool MODD>
+// RING variant: the CTA's rows of delay spectra travel through a shared-memory ring of R = w + 48 rows
+// (its 64 * DT columns), filled 16 rows per block with cp.async one block ahead.  rel = row index
+// relative to the segment start T0; ring slot = rel mod R; R is a multiple of 16 and block starts are
+// multiples of 16, so the 16 rows of a block never wrap.
+struct SlideRing {
+  uint32_t base;      // shared address of the ring
+  uint32_t rrowb;     // bytes per ring row = 512 * DT
+  uint32_t R;         // rows
+  const char *gsrc;   // global address of (pair row 0, first column of the CTA)
+  uint32_t rowb;      // bytes per Y row
+  uint32_t T0, nap;
+};
+
+// all threads of the CTA: copy rows rel in [r0, r0 + n) into the ring (source row clamped to the padding row)
+__device__ __forceinline__ void slide_ring_fill(const SlideRing &G, uint32_t r0, uint32_t n) {
+  const uint32_t cpr = G.rrowb >> 4;                       // 16-byte chunks per ring row
+  for (uint32_t i = threadIdx.x; i < n * cpr; i += blockDim.x) {
+    const uint32_t r = i / cpr, c = i - r * cpr, rel = r0 + r;
+    const uint32_t grow = min(G.T0 + rel, G.nap);
+    const uint32_t dst = G.base + (rel % G.R) * G.rrowb + (c << 4);
+    const char *src = G.gsrc + (size_t)grow * G.rowb + (c << 4);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src));
+  }
+}
+
+// L = min(16, Nt) bins per thread;  MODD <=> M == 1 (Nt <= 16);  RING (M >= 4 only): rows through shared memory.
+template <int L, bool MODD, bool RING>
 __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(SlideArgs a) {
   // blockDim.x = 32 * min(SLIDE_WARPS, ndt * M): every warp of a CTA works on the same (pair, segment)
   __shared__ u64 slots[2][16 * SLIDE_WARPS];
+  extern __shared__ float4 slide_ring[];
   const int nwarps = blockDim.x >> 5, warp = threadIdx.x >> 5;
   long long wt = (long long)blockIdx.x * nwarps + warp;
   const uint32_t lane = threadIdx.x & 31u;
@@ -257,7 +302,28 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   S.keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
   const uint32_t T0 = (uint32_t)sg * (uint32_t)a.seg;                 // multiple of Nt and of L
   const uint32_t tend = min((uint32_t)a.nwin, T0 + (uint32_t)a.seg);  // windows [T0, tend)
-  slide_prefetch<L, MODD>(S, T0);
+  SlideRing G;
+  if constexpr (RING) {
+    // the CTA's warps are (rho fastest, then dt): its first warp's dt is the first column group
+    const long long wt0 = ((long long)blockIdx.x * nwarps) >> a.log2m;
+    const int dt0 = (int)(wt0 % ndt);
+    const int dtc = nwarps >> a.log2m > 0 ? nwarps >> a.log2m : 1;    // column groups per CTA
+    G.base = (uint32_t)__cvta_generic_to_shared(slide_ring);
+    G.rrowb = 512u * (uint32_t)dtc;
+    G.R = (uint32_t)a.w + 48u;
+    G.rowb = S.rowb;
+    G.gsrc = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch) + (size_t)dt0 * 512u;
+    G.T0 = T0; G.nap = (uint32_t)a.nap;
+    S.rrowb = G.rrowb;
+    S.ring_lo = G.base + (uint32_t)(dt - dt0) * 512u + lane * 16u;    // this lane's entry of ring row 0
+    S.ring_hi = S.ring_lo + G.R * G.rrowb;
+    S.sm_out = S.ring_lo;                                             // rel 0
+    S.sm_in = S.ring_lo + (uint32_t)a.w * G.rrowb;                    // rel w
+    slide_ring_fill(G, 0u, (uint32_t)a.w + 17u);                      // rows of block 0 (and the start window)
+    asm volatile("cp.async.wait_all;" ::: "memory");
+    __syncthreads();
+  }
+  slide_prefetch<L, MODD, RING, 0>(S, T0);
   {
     float2 Aa[L], Ab[L];
     slide_start_column<L, MODD>(Aa, S.pout, S.rowb, T0, (uint32_t)a.w, a.twt, S.rho, S.ntmask, 0);
@@ -267,12 +333,19 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   }
 
   uint32_t t0 = T0, buf = 0;
-  for (; t0 + L < tend; t0 += L, buf ^= 1u) {
-    SlideSteps<L, 0, MODD, false>::run(S, t0, tend, &slots[buf][warp]);
-    slide_flush(S.keyp, slots[buf], t0, L, nwarps);
+  for (;; t0 += L, buf ^= 1u) {
+    const bool full = t0 + L < tend;
+    if constexpr (RING) slide_ring_fill(G, t0 - T0 + (uint32_t)a.w + 17u, 16u);   // the next block's new rows
+    if (full) SlideSteps<L, 0, MODD, false, RING>::run(S, t0, tend, &slots[buf][warp]);
+    else SlideSteps<L, 0, MODD, true, RING>::run(S, t0, tend, &slots[buf][warp]);
+    if constexpr (RING) asm volatile("cp.async.wait_all;" ::: "memory");
+    slide_flush(S.keyp, slots[buf], t0, full ? (uint32_t)L : tend - t0, nwarps);
+    if (!full) break;
+    if constexpr (RING) {   // advance the block base by 16 rows (wraps only at a block boundary)
+      S.sm_out += 16u * S.rrowb; S.sm_out = S.sm_out >= S.ring_hi ? S.sm_out - (S.ring_hi - S.ring_lo) : S.sm_out;
+      S.sm_in += 16u * S.rrowb;  S.sm_in = S.sm_in >= S.ring_hi ? S.sm_in - (S.ring_hi - S.ring_lo) : S.sm_in;
+    }
   }
-  SlideSteps<L, 0, MODD, true>::run(S, t0, tend, &slots[buf][warp]);
-  slide_flush(S.keyp, slots[buf], t0, tend - t0, nwarps);
 }
 
 }  // namespace volks

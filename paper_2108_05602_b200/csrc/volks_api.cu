@@ -126,10 +126,16 @@ static void launch_slide(const SlideArgs &a, cudaStream_t st) {
   const int wpb = (int)std::min<long long>(SLIDE_WARPS, per_seg);
   const unsigned blocks = (unsigned)(a.ntasks / wpb);
   const int thr = wpb * 32;
-  if (a.nt >= 32) k_slide<16, false><<<blocks, thr, 0, st>>>(a);
-  else if (a.nt == 16) k_slide<16, true><<<blocks, thr, 0, st>>>(a);
-  else if (a.nt == 8) k_slide<8, true><<<blocks, thr, 0, st>>>(a);
-  else k_slide<4, true><<<blocks, thr, 0, st>>>(a);
+  if (a.nt >= 32) {
+    // M >= 4: rows travel through a shared-memory ring of (w + 48) x 512 * (column groups) bytes
+    const int dtc = std::max(1, wpb >> a.log2m);
+    const size_t ring = (size_t)(a.w + 48) * 512 * dtc;
+    if (a.log2m >= 2 && ring <= 100 * 1024) k_slide<16, false, true><<<blocks, thr, ring, st>>>(a);
+    else k_slide<16, false, false><<<blocks, thr, 0, st>>>(a);
+  }
+  else if (a.nt == 16) k_slide<16, true, false><<<blocks, thr, 0, st>>>(a);
+  else if (a.nt == 8) k_slide<8, true, false><<<blocks, thr, 0, st>>>(a);
+  else k_slide<4, true, false><<<blocks, thr, 0, st>>>(a);
 }
 
 }  // namespace
@@ -306,6 +312,7 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
       ColFftArgs ca; memset(&ca, 0, sizeof ca); ca.nt = w.nt;
       ok = cuda_ok(launch_colfft(ca, w.cf_l1, w.cf_nz, 0, nullptr, true));
     }
+  ok = ok && cuda_ok(cudaFuncSetAttribute(k_slide<16, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
   if (!ok) { volks_plan_destroy(pl); return VOLKS_ECUDA; }
   *out = pl;
   return VOLKS_OK;
