@@ -173,6 +173,10 @@ def run_reference(args):
     }))
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` captures (profiles/r01_ncu_rate_kernels.md); keyed by (config, kernel, width)
+NCU_TRAFFIC = {(2, "slide", 64): 3.97e9, (4, "colfft", 64): 3.97e9}
+
 KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6: "slide", 7: "colfft"}
 
 
@@ -260,13 +264,23 @@ def run_volks(args):
         dom_flops = row_alg / nlaunch[dom]
     else:
         dom_flops = 0.0
+    # flops the dominant kernel actually executes per launch: the sliding kernel does
+    # one complex multiply-add (4 FMA = 8 flops) + |.|^2 (3 flops) per bin per window instead of an FFT
+    if dom[0] == 6:
+        w_, nt_ = c["widths"][dom[1]], c["nts"][dom[1]]
+        exec_flops = workloads.gen.nwin(nap, w_, 1) * nbl * nif * nt_ * c["nf"] * 11.0 / nlaunch[dom]
+    else:
+        exec_flops = dom_flops
     clocks = sampler.summary()
     peak_tf = SM_COUNT * FP32_LANES_PER_SM * 2 * (clocks["sm_max_mhz"] or 1965) * 1e6 / 1e12
     achieved_tf = dom_flops / (dom_ms_avg * 1e-3) / 1e12
     roofline = {
         "bound": "alu", "kernel": "%s[w=%s]" % (KIND_NAMES[dom[0]], c["widths"][dom[1]] if dom[1] >= 0 else "all"),
         "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
-        "traffic": None, "launch_ms": dom_ms_avg, "share_of_step": share[dom] / step_sum,
+        "traffic": NCU_TRAFFIC.get((c["id"], KIND_NAMES[dom[0]], c["widths"][dom[1]] if dom[1] >= 0 else -1)),
+        "launch_ms": dom_ms_avg,
+        "executed_tflops": exec_flops / (dom_ms_avg * 1e-3) / 1e12,
+        "executed_frac": exec_flops / (dom_ms_avg * 1e-3) / 1e12 / peak_tf, "share_of_step": share[dom] / step_sum,
         "peak_kind": "derived: 148 SM x 128 FP32 lanes x 2 flop (FMA) x sm_max_mhz (DESIGN.md)",
         "flops_kind": "algorithmic (SURVEY 8(d)): shared delay FFT per AP + 5 Nt log2 Nt per column + 5 per bin",
         "whole_step_algorithmic_tflops": tot_alg / (ms_step * 1e-3) / 1e12,

@@ -286,7 +286,8 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
     for (int q = 0; q < p->nwidths && pl->wid1 < 0; ++q)
       if (pl->wp[q].w == 1 && pl->wp[q].nwin > 0) pl->wid1 = q;
   for (int q = 0; q < p->nwidths; ++q) active += (pl->wp[q].nwin > 0 && q != pl->wid1) ? 1 : 0;
-  pl->launches = s.nwin_total > 0 ? (int)(1 + pl->nchunks * (1 + active) + 3) : 1;
+  // kernels of this library per search (the key memset is a driver memset, not counted)
+  pl->launches = s.nwin_total > 0 ? (int)(pl->nchunks * (1 + active) + 3) : 0;
 
   // tables, computed in double precision on the host
   std::vector<float2> tab(tw_total);
