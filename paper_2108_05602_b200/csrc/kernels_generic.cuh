@@ -233,6 +233,115 @@ __global__ void __launch_bounds__(256) k_row2(RowArgs a) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// Row (delay) FFT, register form, for nf = 256 * N3 (N3 = 2, 4, 8: nf = 512, 1024, 2048 = config 4).
+// One row per CTA of 256 threads.  n = n' + 256 n3 (n' < 256), k = N3 k' + k3:
+//   X[N3 k' + k3] = sum_{n'} W_256^{n' k'} [ W_nf^{n' k3} sum_{n3} x[n' + 256 n3] W_N3^{n3 k3} ]
+// step 1, thread n': N3-point packed DIF FFT over n3 (pruned to the NZA non-zero inputs), twiddle,
+//         V[k3][n'] to shared memory;
+// step 2, 16-lane group k3: the 256-point transform over n' as in k_row2 (n' = n1 + 16 n2,
+//         k' = 16 k1 + k2): lane n1: 16-point FFT over n2, W_256^{n1 k2}, exchange; lane k2: 16-point
+//         FFT over n1; results to a shared row image in the pair-interleaved layout;
+// step 3: coalesced 128-bit stores of the row, the w = 1 peak.
+// ------------------------------------------------------------------------------------------------
+template <int N3, int NZA>
+__global__ void __launch_bounds__(256) k_row3(RowArgs a) {
+  constexpr int NF = 256 * N3, EP = 17;
+  __shared__ f32x2 V[NF];               // [k3][n']   (reused as the row image [NF] in step 2b)
+  __shared__ f32x2 Ex[N3 * 16 * EP];    // [k3][n1][k2] padded
+  __shared__ u64 kred[8];
+  __shared__ float ered[8];
+  const int tid = threadIdx.x;
+  const long long rrel = blockIdx.x;     // one row per CTA; the grid is exactly nrows
+  // ---- step 1 ----
+  float e = 0.f;
+  {
+    f32x2 z[N3];
+    const float2 *src = a.vis + (a.row0 + rrel) * (long long)a.nchan;
+#pragma unroll
+    for (int n3 = 0; n3 < NZA; ++n3) {
+      const int n = tid + 256 * n3;
+      float2 v = make_float2(0.f, 0.f);
+      if (n < a.nchan) { v = __ldg(src + n); e += cnorm(v); }
+      z[n3] = c2_from(v);
+    }
+    FftDif2<N3, NZA, 0, N3>::run(z);
+#pragma unroll
+    for (int i = 0; i < N3; ++i) {
+      const int k3 = brev<N3>(i);
+      const float2 tw = __ldg(a.twf + tid * k3);        // W_nf^{n' k3}, n' k3 < nf
+      V[k3 * 256 + tid] = fma2(pk(-hi32(z[i]), lo32(z[i])), pk(tw.y, tw.y), mul2(z[i], pk(tw.x, tw.x)));
+    }
+  }
+#pragma unroll
+  for (int o = 16; o >= 1; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+  if ((tid & 31) == 0) ered[tid >> 5] = e;
+  __syncthreads();
+  if (tid == 0) {
+    float s = 0.f;
+    for (int i = 0; i < 8; ++i) s += ered[i];
+    a.E[a.row0 + rrel] = s;
+  }
+  // ---- step 2: groups of 16 lanes, group g <-> k3 (N3 <= 16 groups of the 16 available) ----
+  const int g = tid >> 4, l = tid & 15;
+  if (g < N3) {
+    f32x2 z[16];
+#pragma unroll
+    for (int n2 = 0; n2 < 16; ++n2) z[n2] = V[g * 256 + l + 16 * n2];
+    FftDif2<16, 16, 0, 16>::run(z);
+    f32x2 *E = Ex + g * (16 * EP);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+      const int k2 = brev<16>(i);
+      const float2 tw = __ldg(a.twf + (l * k2) * N3);   // W_256^{n1 k2}
+      E[l * EP + k2] = fma2(pk(-hi32(z[i]), lo32(z[i])), pk(tw.y, tw.y), mul2(z[i], pk(tw.x, tw.x)));
+    }
+  }
+  __syncthreads();                                       // every group is done with V; E complete
+  float *img = (float *)V;                               // row image, pair-interleaved floats
+  if (g < N3) {
+    const f32x2 *E = Ex + g * (16 * EP);
+    f32x2 v[16];
+#pragma unroll
+    for (int n1 = 0; n1 < 16; ++n1) v[n1] = E[n1 * EP + l];
+    FftDif2<16, 16, 0, 16>::run(v);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+      const int col = N3 * (16 * brev<16>(i) + l) + g;
+      float *p = img + ((col >> 1) << 2) + (col & 1);
+      p[0] = lo32(v[i]); p[2] = hi32(v[i]);
+    }
+  }
+  __syncthreads();
+  // ---- step 3 ----
+  u64 key = 0;
+  float4 *dst = (float4 *)(a.Y + rrel * (long long)a.pitch);
+  for (int c = tid; c < NF / 2; c += 256) {
+    const float4 q = ((const float4 *)img)[c];
+    dst[c] = q;
+    const u64 k0 = make_key(fmaf(q.x, q.x, q.z * q.z), (uint32_t)(2 * c)), k1 = make_key(fmaf(q.y, q.y, q.w * q.w), (uint32_t)(2 * c + 1));
+    key = k0 > key ? k0 : key;
+    key = k1 > key ? k1 : key;
+  }
+  if (a.keys1) {   // uniform branch
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) {
+      const u64 other = __shfl_xor_sync(0xffffffffu, key, o);
+      key = other > key ? other : key;
+    }
+    if ((tid & 31) == 0) kred[tid >> 5] = key;
+    __syncthreads();
+    if (tid == 0) {
+      for (int i = 0; i < 8; ++i) key = kred[i] > key ? kred[i] : key;
+      const long long row = a.row0 + rrel;
+      const long long pair = row / a.nap;
+      const int t = (int)(row - pair * a.nap);
+      const int j = t / a.stride1;
+      if (j * a.stride1 == t && j < a.nwin1) a.keys1[pair * a.per_pair + j] = key;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Column (rate) transform + power + argmax, generic.
 // Thread task id (d fastest): ((pair_local * nwin + j) * M + rho) * nf + d.
 // ------------------------------------------------------------------------------------------------

@@ -107,9 +107,32 @@ static bool row2_nz(const RowArgs &a, int nza, unsigned blocks, cudaStream_t st)
   return false;
 }
 
-// register-form row FFT for nf in {64, 128, 256} with the paired Y layout; false = not applicable
+template <int N3>
+static bool row3_nz(const RowArgs &a, int nza, cudaStream_t st) {
+  const unsigned blocks = (unsigned)a.nrows;
+  switch (nza) {
+    case 1: k_row3<N3, 1><<<blocks, 256, 0, st>>>(a); return true;
+    case 2: k_row3<N3, 2><<<blocks, 256, 0, st>>>(a); return true;
+    case 4: if constexpr (N3 >= 4) { k_row3<N3, 4><<<blocks, 256, 0, st>>>(a); return true; } break;
+    case 8: if constexpr (N3 >= 8) { k_row3<N3, 8><<<blocks, 256, 0, st>>>(a); return true; } break;
+  }
+  return false;
+}
+
+// register-form row FFT for nf in {64, 128, 256} (k_row2) and {512 .. 2048} (k_row3) with the paired Y
+// layout; false = not applicable
 static bool launch_row2(const RowArgs &a, cudaStream_t st) {
   if (!a.paired) return false;
+  if (a.nf >= 512 && a.nf <= 2048 && a.nrows < (1LL << 31)) {
+    int nza = 1;
+    while (nza * 256 < a.nchan) nza *= 2;
+    switch (a.nf / 256) {
+      case 2: return row3_nz<2>(a, nza, st);
+      case 4: return row3_nz<4>(a, nza, st);
+      case 8: return row3_nz<8>(a, nza, st);
+    }
+    return false;
+  }
   int n1, n2;
   if (a.nf == 256) { n1 = 16; n2 = 16; } else if (a.nf == 128) { n1 = 8; n2 = 16; } else if (a.nf == 64) { n1 = 8; n2 = 8; } else return false;
   int nza = 1;

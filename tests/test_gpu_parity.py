@@ -86,6 +86,8 @@ def test_generic_and_sliding_paths_agree_with_oracle(vb, oracle, cfg, over, monk
     (1, 1, 50, 3, [2], [1], [4], 4),                           # nf = 4
     (1, 1, 17, 1, [4], [1], [8], 1),                           # single channel, nf = 1
     (1, 1, 300, 100, [32, 64], [5, 9], [64, 128], 512),        # big nf, odd strides
+    (1, 1, 90, 300, [16, 40], [8, 10], [32, 64], 1024),        # nf = 1024 row kernel, pruned inputs
+    (1, 1, 70, 2048, [8], [1], [16], 2048),                    # nf = 2048, nchan = nf (no pruning)
 ])
 def test_edge_shapes(vb, oracle, shape):
     nbl, nif, nap, nchan, widths, strides, nts, nf = shape
