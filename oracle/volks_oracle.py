@@ -119,6 +119,39 @@ def search(vis, widths, strides, nts, nf, mode="cached", select=None, nthreads=0
     return out, used
 
 
+K_DM_MS = 4.148808  # cold-plasma dispersion constant [ms GHz^2 cm^3 / pc] (textbook; the paper gives none)
+
+
+def dm_shifts(dm, f_chan_mhz, f_ref_mhz, t_ap_s):
+    """Integer AP shift of every frequency point for a dispersion measure `dm` [pc cm^-3]:
+    round(delay / T_ap), delay = 4.148808 ms * DM * (f^-2 - f_ref^-2) with f in GHz.  Step 4 of the
+    paper applies "a specific time shift" per frequency point without stating
+    the formula; this is the textbook one (reading R3).  f_chan_mhz: array [nif][nchan]."""
+    f = np.asarray(f_chan_mhz, dtype=np.float64) * 1e-3
+    delay_s = K_DM_MS * 1e-3 * float(dm) * (f ** -2 - (float(f_ref_mhz) * 1e-3) ** -2)
+    return np.rint(delay_s / float(t_ap_s)).astype(np.int32)
+
+
+def dedisperse(vis, shifts):
+    """Step 4: for each frequency point a time shift.  out[bl][ifq][t][k] =
+    vis[bl][ifq][t + shifts[ifq][k]][k], zero where t + shift falls outside [0, nap).  Written as the
+    plain loop over (ifq, k) it is in the paper."""
+    vis = np.asarray(vis)
+    nbl, nif, nap, nchan = vis.shape
+    sh = np.asarray(shifts, dtype=np.int64).reshape(nif, nchan)
+    out = np.zeros_like(vis)
+    for n in range(nif):
+        for k in range(nchan):
+            d = int(sh[n, k])
+            if d >= nap or d <= -nap:
+                continue
+            if d >= 0:
+                out[:, n, :nap - d, k] = vis[:, n, d:, k]
+            else:
+                out[:, n, -d:, k] = vis[:, n, :nap + d, k]
+    return out
+
+
 def canonical_table(nbl, nif, nap, widths, strides):
     """(bl, ifq, wid, win, t0) int32 arrays for every window in canonical order."""
     nws = [nwin(nap, int(w), int(s)) for w, s in zip(widths, strides)]

@@ -311,3 +311,51 @@ def test_window_match_vs_python_graph_search(oracle):
             expect.append((best, len({rows[x][2] for x in comp}), min(iv[x][0] for x in comp), max(iv[x][1] for x in comp)))
     expect.sort()
     assert [(int(p["rep"]), int(p["nwidths_hit"]), int(p["t_begin"]), int(p["t_end"])) for p in got] == expect
+
+
+def test_dedispersion_pins(oracle):
+    """f1: per frequency point a time shift.  Pins: zero shift is the identity; a
+    pulse dispersed by known shifts is restored sample for sample; samples shifted in from beyond the
+    end are zero; the textbook delay 4.148808 ms DM (f^-2 - f_ref^-2) at a hand-computed point."""
+    rng = np.random.default_rng(5)
+    nbl, nif, nap, nchan = 2, 3, 40, 8
+    clean = (rng.normal(size=(nbl, nif, nap, nchan)) + 1j * rng.normal(size=(nbl, nif, nap, nchan))).astype(np.complex64)
+    assert np.array_equal(oracle.dedisperse(clean, np.zeros((nif, nchan), np.int32)), clean)
+    sh = rng.integers(0, 7, size=(nif, nchan)).astype(np.int32)
+    disp = np.zeros_like(clean)                      # channel k arrives sh[k] APs late
+    for n in range(nif):
+        for k in range(nchan):
+            d = int(sh[n, k])
+            disp[:, n, d:, k] = clean[:, n, :nap - d, k]
+    back = oracle.dedisperse(disp, sh)
+    for n in range(nif):
+        for k in range(nchan):
+            d = int(sh[n, k])
+            assert np.array_equal(back[:, n, :nap - d, k], clean[:, n, :nap - d, k])
+            assert np.all(back[:, n, nap - d:, k] == 0)
+    # DM 100 pc cm^-3, 1400 MHz against 1500 MHz: 4.148808e-3 s * 100 * (1/1.4^2 - 1/1.5^2) = 27.2821 ms
+    d = oracle.dm_shifts(100.0, np.array([[1400.0, 1500.0]]), 1500.0, 1e-3)
+    assert d.tolist() == [[27, 0]]
+    assert abs(4.148808e-3 * 100 * (1 / 1.4 ** 2 - 1 / 1.5 ** 2) - 0.0272821) < 1e-6
+
+
+def test_dedispersed_pulse_closed_form(oracle):
+    """A noiseless on-bin fringe, dispersed channel by channel, then dedispersed with the matching
+    shifts, peaks where the undispersed one does with P1 = (a w nchan)^2 (pin P1 through step 4)."""
+    w, nchan, nt, nf, a, tau, rho = 8, 16, 16, 32, 0.7, 3, 2
+    nap, tp = 64, 20
+    t = np.arange(w)[:, None]
+    k = np.arange(nchan)[None, :]
+    pulse = (a * np.exp(2j * np.pi * (tau * k / nchan + rho * t / w))).astype(np.complex64)
+    sh = (np.arange(nchan)[::-1] // 2).astype(np.int32).reshape(1, nchan)     # low channels later
+    vis = np.zeros((1, 1, nap, nchan), np.complex64)
+    for kk in range(nchan):
+        d = int(sh[0, kk])
+        vis[0, 0, tp + d: tp + d + w, kk] = pulse[:, kk]
+    ded = oracle.dedisperse(vis, sh)
+    pk, _ = oracle.search(ded, [w], [1], [nt], nf, mode="fft")
+    o = pk[tp]
+    assert o["idx1"] == (rho * nt // w) * nf + tau * nf // nchan
+    assert abs(o["p1"] - (a * w * nchan) ** 2) < 1e-6 * o["p1"]
+    raw, _ = oracle.search(vis, [w], [1], [nt], nf, mode="fft")
+    assert raw["p1"].max() < 0.5 * o["p1"]            # without step 4 the pulse is smeared
