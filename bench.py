@@ -44,6 +44,8 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--peaks", action="store_true", help="also write the dense per-window peak array")
+    ap.add_argument("--dm", type=float, default=0.0,
+                    help="dedisperse (f1, fused into the slab load) with this DM [pc cm^-3]; 0 = plain search")
     return ap.parse_args()
 
 
@@ -207,8 +209,14 @@ def run_volks(args):
     peaks = torch.empty(plan.nwin_total * vk.PEAK_DTYPE.itemsize, dtype=torch.uint8, device=dev) if args.peaks else None
     stream = torch.cuda.current_stream(dev)
 
+    shift = None
+    if args.dm:
+        # IFs of 16 MHz above 1400 MHz (L band, like EL060: PAPER.md:172-173), referenced to the top frequency
+        f = 1400.0 + 16.0 * np.arange(nif)[:, None] + (16.0 / nchan) * np.arange(nchan)[None, :]
+        shift = torch.as_tensor(vk.dm_shifts(args.dm, f, f.max(), c["t_ap"]), device=dev)
+
     def step():
-        plan.fringe_search(vis, ws, cands, ncand, peaks, stream)
+        plan.fringe_search(vis, ws, cands, ncand, peaks, stream, shift=shift)
 
     def barrier():
         if dist is not None:
@@ -290,7 +298,7 @@ def run_volks(args):
     }
     return dict(vk=vk, plan=plan, vis=vis, c=c, ws=ws, cands=cands, ncand=ncand, peaks=peaks, stream=stream,
                 dev=dev, rank=rank, world=world, dist=dist, ms_step=ms_step, value=value, nwin=nwin, nvis=nvis,
-                n_found=n_found, roofline=roofline, clocks=clocks, cap=cap)
+                n_found=n_found, roofline=roofline, clocks=clocks, cap=cap, shift=shift)
 
 
 def run_e2e(R, steps):
@@ -307,7 +315,7 @@ def run_e2e(R, steps):
     def step():
         nonlocal d2h
         d_vis.copy_(h_vis, non_blocking=True)
-        plan.fringe_search(d_vis, R["ws"], R["cands"], R["ncand"], R["peaks"], stream)
+        plan.fringe_search(d_vis, R["ws"], R["cands"], R["ncand"], R["peaks"], stream, shift=R["shift"])
         h_n.copy_(R["ncand"], non_blocking=True)
         stream.synchronize()
         n = min(int(h_n.item()), R["cap"]) * vk.CAND_DTYPE.itemsize
@@ -362,7 +370,7 @@ def main():
             "config": {"workload": workload_name(c), "snr_thresh": c["snr_thresh"],
                        "l2": "input slab (%.2f GB) larger than L2, no flush needed" % (R["nvis"] * 8 / 1e9)
                        if R["nvis"] * 8 > 126e6 else "input smaller than L2 (latency-bound config, report only)",
-                       "replicas": R["world"], "dense_peaks": bool(args.peaks)},
+                       "replicas": R["world"], "dense_peaks": bool(args.peaks), "dm": args.dm},
             "visibilities_per_s": R["world"] * R["nvis"] / (R["ms_step"] * 1e-3),
             "windows": R["nwin"], "candidates": R["n_found"],
             "clocks": R["clocks"], "e2e": e2e, "gpu_launches": R["plan"].launches * args.steps,

@@ -108,6 +108,22 @@ int volks_fringe_search(const volks_plan *plan, const void *d_vis, void *d_works
                         volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity,
                         uint32_t *d_ncand, void *cuda_stream);
 
+/* The same search on DEDISPERSED data (step 4 of the paper: "for each frequency
+ * point ... a specific time shift"), fused into the slab load: element (t, k) of pair (bl, ifq) is
+ * taken from AP t + d_shift[ifq*nchan + k], and is zero where that falls outside [0, nap).
+ *   d_shift  DEVICE int32[nif][nchan] AP offsets for one DM (volks_dm_shifts fills a HOST table to
+ *            upload), or NULL = volks_fringe_search.  One call per DM value; d_vis is never modified.
+ * Everything else as volks_fringe_search. */
+int volks_fringe_search_dd(const volks_plan *plan, const void *d_vis, const int32_t *d_shift,
+                           void *d_workspace, volks_peak *d_peaks, volks_cand *d_cands,
+                           uint32_t cand_capacity, uint32_t *d_ncand, void *cuda_stream);
+
+/* HOST helper: integer AP shift of every frequency point for dispersion measure `dm` [pc cm^-3]:
+ * shift = round(4.148808e-3 s * dm * (f_GHz^-2 - fref_GHz^-2) / ap_seconds) (the textbook cold-plasma
+ * delay; the paper states no formula - DESIGN.md R3).  f_chan_mhz, shift: HOST [n]. */
+int volks_dm_shifts(double dm, const double *f_chan_mhz, int32_t n, double f_ref_mhz, double ap_seconds,
+                    int32_t *shift);
+
 /* Per-baseline multi-window match (reading A13).  HOST call on HOST
  * arrays (integer work on a list of at most a few thousand records).  Within one (bl, ifq),
  * candidates whose AP intervals [t0, t0+width[wid]) overlap are linked; connected components are

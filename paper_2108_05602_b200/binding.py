@@ -16,7 +16,7 @@ VOLKS_OK, VOLKS_EINVAL, VOLKS_ECUDA, VOLKS_ENOMEM, VOLKS_EOVERFLOW = 0, -1, -2, 
 EXPORTS = (
     "volks_plan_create", "volks_plan_destroy", "volks_plan_query", "volks_fringe_search",
     "volks_window_match", "volks_bin_to_physical", "volks_plan_launch_count", "volks_strerror",
-    "volks_version", "volks_plan_profile", "volks_plan_profile_read",
+    "volks_version", "volks_plan_profile", "volks_plan_profile_read", "volks_fringe_search_dd", "volks_dm_shifts",
 )
 
 
@@ -53,6 +53,9 @@ def lib():
         L.volks_plan_query.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_size_t),
                                        ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
         L.volks_fringe_search.argtypes = [ctypes.c_void_p] * 5 + [ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
+        L.volks_fringe_search_dd.argtypes = [ctypes.c_void_p] * 6 + [ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
+        L.volks_dm_shifts.argtypes = [ctypes.c_double, ctypes.c_void_p, ctypes.c_int32, ctypes.c_double,
+                                      ctypes.c_double, ctypes.c_void_p]
         L.volks_window_match.argtypes = [ctypes.c_void_p, ctypes.c_uint32, ctypes.c_void_p, ctypes.c_int32,
                                          ctypes.c_int32, ctypes.c_void_p, ctypes.c_uint32,
                                          ctypes.POINTER(ctypes.c_uint32)]
@@ -111,10 +114,11 @@ class Plan:
 
     __del__ = close
 
-    def fringe_search(self, vis, workspace, cands, ncand, peaks=None, stream=None):
-        """volks_fringe_search on torch CUDA tensors (asynchronous on `stream`).
+    def fringe_search(self, vis, workspace, cands, ncand, peaks=None, stream=None, shift=None):
+        """volks_fringe_search[_dd] on torch CUDA tensors (asynchronous on `stream`).
         vis complex64 [nbl][nif][nap][nchan]; workspace uint8 >= workspace_bytes;
-        cands uint8 [capacity*36]; ncand int32/uint32 [1]; peaks uint8 [nwin_total*16] or None."""
+        cands uint8 [capacity*36]; ncand int32/uint32 [1]; peaks uint8 [nwin_total*16] or None;
+        shift int32 CUDA [nif][nchan] dedispersion AP offsets or None."""
         assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous()
         assert tuple(vis.shape) == self.shape
         assert workspace.is_cuda and workspace.numel() * workspace.element_size() >= self.workspace_bytes
@@ -122,9 +126,13 @@ class Plan:
         if peaks is not None:
             assert peaks.numel() * peaks.element_size() >= self.nwin_total * PEAK_DTYPE.itemsize
         st = (stream or torch.cuda.current_stream(vis.device)).cuda_stream
-        _check(lib().volks_fringe_search(
-            self._h, vis.data_ptr(), workspace.data_ptr(), peaks.data_ptr() if peaks is not None else None,
-            cands.data_ptr() if cap else None, cap, ncand.data_ptr(), st))
+        if shift is not None:
+            assert shift.is_cuda and shift.dtype == torch.int32 and shift.is_contiguous()
+            assert tuple(shift.shape) == (self.shape[1], self.shape[3])
+        _check(lib().volks_fringe_search_dd(
+            self._h, vis.data_ptr(), shift.data_ptr() if shift is not None else None, workspace.data_ptr(),
+            peaks.data_ptr() if peaks is not None else None, cands.data_ptr() if cap else None, cap,
+            ncand.data_ptr(), st))
 
     def profile(self, enable=True):
         """volks_plan_profile: bracket every launch of later searches with CUDA events."""
@@ -165,8 +173,16 @@ def bin_to_physical(nt, nf, rate_idx, delay_idx, ap_seconds, chan_hz):
     return r.value, d.value
 
 
+def dm_shifts(dm, f_chan_mhz, f_ref_mhz, ap_seconds):
+    """volks_dm_shifts: int32 AP shifts (same shape as f_chan_mhz) for one dispersion measure."""
+    f = np.ascontiguousarray(f_chan_mhz, dtype=np.float64)
+    out = np.zeros(f.shape, dtype=np.int32)
+    _check(lib().volks_dm_shifts(float(dm), f.ctypes.data, f.size, float(f_ref_mhz), float(ap_seconds), out.ctypes.data))
+    return out
+
+
 def fringe_search(vis, widths=None, strides=None, nts=None, nf=None, snr_thresh=None, want_peaks=False,
-                  cand_capacity=1 << 20, plan=None):
+                  cand_capacity=1 << 20, plan=None, shifts=None):
     """Convenience one-shot call: allocates workspace/outputs with torch, runs the search on the
     current stream, synchronises and returns (cands CAND_DTYPE[n], ncand_true, peaks|None)."""
     if not vis.is_cuda:
@@ -180,7 +196,8 @@ def fringe_search(vis, widths=None, strides=None, nts=None, nf=None, snr_thresh=
     cands = torch.empty(cand_capacity * CAND_DTYPE.itemsize, dtype=torch.uint8, device=dev)
     ncand = torch.zeros(1, dtype=torch.int32, device=dev)
     peaks = torch.empty(max(plan.nwin_total, 1) * PEAK_DTYPE.itemsize, dtype=torch.uint8, device=dev) if want_peaks else None
-    plan.fringe_search(vis, ws, cands, ncand, peaks)
+    shift = None if shifts is None else torch.as_tensor(np.ascontiguousarray(shifts, dtype=np.int32), device=dev)
+    plan.fringe_search(vis, ws, cands, ncand, peaks, shift=shift)
     torch.cuda.synchronize(dev)
     n = int(ncand.item()) & 0xFFFFFFFF
     c = cands[: min(n, cand_capacity) * CAND_DTYPE.itemsize].cpu().numpy().view(CAND_DTYPE)

@@ -32,6 +32,30 @@ struct RowArgs {
   u64 *keys1;           // canonical key base of that width (keys + offc), or nullptr
   long long per_pair;   // windows per pair over all widths
   int nap, stride1, nwin1;
+  // f1 dedispersion fused into the slab load: element (t, k) of pair (bl, ifq) is
+  // read from AP t + shift[ifq][k] (zero beyond the slab); nullptr = no shift
+  const int *shift;     // DEVICE [nif][nchan] or nullptr
+  int nif;
+};
+
+// Source of one AP row: plain (base pointer) or dedispersed (per-channel row offsets).
+struct RowSrc {
+  const float2 *base;   // vis + row * nchan (plain) or vis + pair * nap * nchan (dedispersed)
+  const int *sh;        // shift row of this IF, or nullptr
+  int t, nap, nchan;
+  __device__ __forceinline__ RowSrc(const RowArgs &a, long long row) : nap(a.nap), nchan(a.nchan) {
+    if (a.shift) {
+      const long long pair = row / a.nap;
+      t = (int)(row - pair * a.nap);
+      base = a.vis + pair * a.nap * (long long)a.nchan;
+      sh = a.shift + (pair % a.nif) * a.nchan;
+    } else { base = a.vis + row * (long long)a.nchan; sh = nullptr; t = 0; }
+  }
+  __device__ __forceinline__ float2 operator()(int k) const {
+    if (!sh) return __ldg(base + k);
+    const int ts = t + __ldg(sh + k);
+    return (ts >= 0 && ts < nap) ? __ldg(base + (long long)ts * nchan + k) : make_float2(0.f, 0.f);
+  }
 };
 
 __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
@@ -48,10 +72,10 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
 
   float e = 0.f;
   if (live) {
-    const float2 *src = a.vis + (a.row0 + rrel) * (long long)a.nchan;
+    const RowSrc src(a, a.row0 + rrel);
     for (int k = lane; k < nf; k += tpr) {
       float2 v = make_float2(0.f, 0.f);
-      if (k < a.nchan) { v = __ldg(src + k); e += cnorm(v); }
+      if (k < a.nchan) { v = src(k); e += cnorm(v); }
       buf0[k] = v;
     }
   }
@@ -177,12 +201,12 @@ __global__ void __launch_bounds__(256) k_row2(RowArgs a) {
   float e = 0.f;
   if (l < N1) {
     f32x2 z[N2];
-    const float2 *src = a.vis + (a.row0 + rrel) * (long long)a.nchan;
+    const RowSrc src(a, live ? a.row0 + rrel : a.row0);
 #pragma unroll
     for (int n2 = 0; n2 < NZA; ++n2) {
       const int n = l + N1 * n2;
       float2 v = make_float2(0.f, 0.f);
-      if (live && n < a.nchan) { v = __ldg(src + n); e += cnorm(v); }
+      if (live && n < a.nchan) { v = src(n); e += cnorm(v); }
       z[n2] = c2_from(v);
     }
     FftDif2<N2, NZA, 0, N2>::run(z);
@@ -256,12 +280,12 @@ __global__ void __launch_bounds__(256) k_row3(RowArgs a) {
   float e = 0.f;
   {
     f32x2 z[N3];
-    const float2 *src = a.vis + (a.row0 + rrel) * (long long)a.nchan;
+    const RowSrc src(a, a.row0 + rrel);
 #pragma unroll
     for (int n3 = 0; n3 < NZA; ++n3) {
       const int n = tid + 256 * n3;
       float2 v = make_float2(0.f, 0.f);
-      if (n < a.nchan) { v = __ldg(src + n); e += cnorm(v); }
+      if (n < a.nchan) { v = src(n); e += cnorm(v); }
       z[n3] = c2_from(v);
     }
     FftDif2<N3, NZA, 0, N3>::run(z);
@@ -444,6 +468,10 @@ __device__ __forceinline__ WinStat window_stat(const Sched &s, const u64 *keys, 
   float es = 0.f;
   for (int t = 0; t < s.width[q]; ++t) es += e[t];
   o.snr = es > 0.f ? sqrtf(o.power / es) : 0.f;
+  // an all-zero window (flagged data, the zero fill of dedispersion) has an identically zero plane:
+  // P1 = 0 at (0, 0) by the tie rule.  The sliding sum would leave rounding residue of earlier samples
+  // here, so the exact statement is made from the energy (es == 0 iff every sample is zero).
+  if (es == 0.f) { o.power = 0.f; o.rate_idx = 0; o.delay_idx = 0; }
   return o;
 }
 

@@ -363,6 +363,12 @@ int volks_plan_launch_count(const volks_plan *pl) { return pl ? pl->launches : V
 
 int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspace, volks_peak *d_peaks,
                         volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand, void *cuda_stream) {
+  return volks_fringe_search_dd(pl, d_vis, nullptr, d_workspace, d_peaks, d_cands, cand_capacity, d_ncand, cuda_stream);
+}
+
+int volks_fringe_search_dd(const volks_plan *pl, const void *d_vis, const int32_t *d_shift, void *d_workspace,
+                           volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand,
+                           void *cuda_stream) {
   if (!pl || !d_vis || !d_workspace || !d_ncand || (!d_cands && cand_capacity > 0)) return VOLKS_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const Sched &s = pl->sched;
@@ -383,6 +389,7 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
     ra.vis = (const float2 *)d_vis; ra.Y = Y; ra.E = E; ra.twf = pl->d_tables;
     ra.row0 = pair0 * s.nap; ra.nrows = np * s.nap;
     ra.nchan = pl->nchan; ra.nf = s.nf; ra.tpr = pl->row_tpr; ra.rows_per_cta = pl->row_rows_per_cta; ra.pitch = pl->pitch; ra.paired = pl->paired;
+    ra.shift = d_shift; ra.nif = s.nif;
     ra.keys1 = nullptr; ra.per_pair = s.per_pair; ra.nap = s.nap; ra.stride1 = 1; ra.nwin1 = 0;
     if (pl->wid1 >= 0) { ra.keys1 = keys + s.offc[pl->wid1]; ra.stride1 = s.stride[pl->wid1]; ra.nwin1 = (int)s.nwin[pl->wid1]; }
     const long long rblocks = (ra.nrows + ra.rows_per_cta - 1) / ra.rows_per_cta;
@@ -513,6 +520,18 @@ int volks_window_match(const volks_cand *cands, uint32_t ncand, const int32_t *w
     out[n].nwidths_hit = found[n].nhit; out[n].t_begin = found[n].tb; out[n].t_end = found[n].te;
   }
   return found.size() > capacity ? VOLKS_EOVERFLOW : VOLKS_OK;
+}
+
+int volks_dm_shifts(double dm, const double *f_chan_mhz, int32_t n, double f_ref_mhz, double ap_seconds,
+                    int32_t *shift) {
+  if (!f_chan_mhz || !shift || n < 0 || !(f_ref_mhz > 0) || !(ap_seconds > 0) || !(dm == dm)) return VOLKS_EINVAL;
+  const double fr = f_ref_mhz * 1e-3;
+  for (int32_t i = 0; i < n; ++i) {
+    if (!(f_chan_mhz[i] > 0)) return VOLKS_EINVAL;
+    const double f = f_chan_mhz[i] * 1e-3;
+    shift[i] = (int32_t)llrint(4.148808e-3 * dm * (1.0 / (f * f) - 1.0 / (fr * fr)) / ap_seconds);
+  }
+  return VOLKS_OK;
 }
 
 int volks_bin_to_physical(int32_t nt, int32_t nf, int32_t rate_idx, int32_t delay_idx, double ap_seconds,

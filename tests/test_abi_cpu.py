@@ -121,3 +121,11 @@ def test_bin_to_physical(vb):
     assert r < 0 and d < 0
     with pytest.raises(vb.VolksError):
         vb.bin_to_physical(16, 64, 16, 0, 1e-3, 5e5)
+
+
+def test_dm_shifts_host_vs_oracle(vb, oracle):
+    f = 1400.0 + 16.0 * np.arange(8)[:, None] + 0.25 * np.arange(64)[None, :]
+    for dm in (0.0, 26.8, 557.0):
+        got = vb.dm_shifts(dm, f, f.max(), 1.024e-3)
+        assert np.array_equal(got, oracle.dm_shifts(dm, f, f.max(), 1.024e-3))
+    assert vb.dm_shifts(100.0, np.array([1400.0, 1500.0]), 1500.0, 1e-3).tolist() == [27, 0]

@@ -19,6 +19,20 @@ def vb():
     return v
 
 
+def make_plane_power(oracle, vis_np, c):
+    """Oracle power of one bin of one canonical window (recomputes that window's plane)."""
+    nbl, nif, nap, nchan = vis_np.shape
+    bl, ifq, wid, win, t0 = oracle.canonical_table(nbl, nif, nap, c["widths"], c["strides"])
+
+    def plane_power(i, idx):
+        q = int(wid[i])
+        slab = vis_np[bl[i], ifq[i], t0[i]: t0[i] + c["widths"][q]]
+        _, plane = oracle.window(slab, c["nts"][q], c["nf"], mode="fft", want_plane=True)
+        z = plane.reshape(-1)[idx]
+        return float(z.real * z.real + z.imag * z.imag)
+    return plane_power
+
+
 def run_both(vb, oracle, vis, c, thresh=None, mode="cached"):
     thresh = c["snr_thresh"] if thresh is None else thresh
     nbl, nif, nap, nchan = vis.shape
@@ -28,7 +42,7 @@ def run_both(vb, oracle, vis, c, thresh=None, mode="cached"):
     nw = [workloads.gen.nwin(nap, w, s) for w, s in zip(c["widths"], c["strides"])]
     di = dense_index(nbl, nif, nw)
     assert len(ora) == len(peaks) == len(di)
-    stats = check_peaks(peaks[di], ora, c["nf"])
+    stats = check_peaks(peaks[di], ora, c["nf"], make_plane_power(oracle, vis.cpu().numpy(), c))
     oc, keep = oracle.candidates(ora, nbl, nif, nap, c["widths"], c["strides"], c["nf"], thresh)
     assert n == len(cands)
     ncand, nmarg = check_candidates(cands, oc, ora, keep, thresh, c["nf"])
@@ -189,3 +203,39 @@ def test_window_match_on_gpu_candidates(vb, oracle):
     for g, e in zip(got, exp):
         assert g["best"].tobytes() == cands[int(e["rep"])].tobytes()
         assert (g["nwidths_hit"], g["t_begin"], g["t_end"]) == (e["nwidths_hit"], e["t_begin"], e["t_end"])
+
+
+@pytest.mark.parametrize("cfg,over", [
+    (2, dict(nbl=1, nif=2, nap=500, npulses=2)),      # k_row2 + sliding kernels
+    (4, dict(nbl=1, nif=1, nap=700, npulses=1)),      # k_row3 + column FFT
+    (1, dict(nap=600)),                               # k_row2 (nf = 128) + generic / column FFT
+])
+def test_dedispersed_search_matches_oracle(vb, oracle, cfg, over):
+    """f1: dedispersion fused into the slab load == oracle.dedisperse followed by the plain search."""
+    vis, c, _ = workloads.generate(cfg, **over)
+    nbl, nif, nap, nchan = vis.shape
+    f = 1400.0 + 16.0 * np.arange(nif)[:, None] + (16.0 / nchan) * np.arange(nchan)[None, :]
+    sh = vb.dm_shifts(300.0, f, f.max(), c["t_ap"])
+    assert sh.max() > 3 and sh.min() == 0
+    cands, n, peaks = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"],
+                                       want_peaks=True, shifts=sh)
+    ded = oracle.dedisperse(vis.numpy(), sh)
+    ora, _ = oracle.search(ded, c["widths"], c["strides"], c["nts"], c["nf"], mode="cached")
+    nw = [workloads.gen.nwin(nap, w, s) for w, s in zip(c["widths"], c["strides"])]
+    check_peaks(peaks[dense_index(nbl, nif, nw)], ora, c["nf"], make_plane_power(oracle, ded, c))
+    oc, keep = oracle.candidates(ora, nbl, nif, nap, c["widths"], c["strides"], c["nf"], c["snr_thresh"])
+    check_candidates(cands, oc, ora, keep, c["snr_thresh"], c["nf"])
+    # negative shifts and shifts past the end are legal: zero fill
+    sh2 = sh.copy(); sh2[0, 0] = -5; sh2[-1, -1] = nap + 3
+    _, _, p2 = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"], want_peaks=True, shifts=sh2)
+    ora2, _ = oracle.search(oracle.dedisperse(vis.numpy(), sh2), c["widths"], c["strides"], c["nts"], c["nf"], mode="cached")
+    check_peaks(p2[dense_index(nbl, nif, nw)], ora2, c["nf"], make_plane_power(oracle, oracle.dedisperse(vis.numpy(), sh2), c))
+
+
+def test_flagged_zero_span_inside_data(vb, oracle):
+    """Exact zeros (flagged APs) after ordinary data: windows inside the span have an identically
+    zero plane (P1 = 0 at (0,0), snr 0) - the sliding sum must not leak rounding residue there."""
+    vis, c, _ = workloads.generate(2, nbl=1, nif=1, nap=700, npulses=2)
+    vis[0, 0, 300:420] = 0
+    stats, ncand, cands, ora = run_both(vb, oracle, vis, c)
+    assert np.count_nonzero(ora["p1"] == 0) > 100
