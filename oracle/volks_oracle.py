@@ -12,6 +12,8 @@ canonical ordering that DESIGN.md readings A3, A4, A9 fix:
 Parity status: every function here is pinned by tests/test_oracle_pins.py (closed forms P1-P14 of
 DESIGN.md) except `window_match`, which is pinned only by hand-built constructions and a second
 brute-force statement of the same rule (the paper gives no worked example) - see DESIGN.md.
+`dedisperse` / `dm_shifts` (step 4) are pinned by test_dedispersion_pins and
+test_dedispersed_pulse_closed_form.
 """
 import ctypes
 import os
