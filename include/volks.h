@@ -135,6 +135,22 @@ int volks_dm_shifts(double dm, const double *f_chan_mhz, int32_t n, double f_ref
 int volks_window_match(const volks_cand *cands, uint32_t ncand, const int32_t *width, int32_t nwidths,
                        int32_t min_widths, volks_pulse *out, uint32_t capacity, uint32_t *nout);
 
+/* One cross-baseline detection of volks_baseline_match. */
+typedef struct {
+  volks_pulse best;       /* max-snr pulse of the cluster (ties: first in input order)             */
+  int32_t nbaselines;     /* distinct `bl` values in the cluster                                     */
+  int32_t t_begin, t_end; /* union AP extent [t_begin, t_end) of the cluster                         */
+} volks_detection;
+
+/* Multi-baseline cross-match ("A single pulse is identified if it is
+ * detected with at least 5 baselines"; reading A19).  HOST call on HOST arrays: the pulses
+ * of volks_window_match for ALL (bl, ifq) are clustered by overlap of their AP extents
+ * [t_begin, t_end) (connected components); a cluster seen on >= min_baselines distinct baselines
+ * gives one volks_detection.  Output ordered by t_begin (ties: position of `best` in the input).
+ * *nout = number found; VOLKS_EOVERFLOW if it exceeds `capacity` (the first `capacity` are written). */
+int volks_baseline_match(const volks_pulse *pulses, uint32_t npulse, int32_t min_baselines,
+                         volks_detection *out, uint32_t capacity, uint32_t *nout);
+
 /* HOST helper: signed physical units from raw bins (upper half of each axis is negative):
  * rate_hz = r_signed/(nt*ap_seconds), delay_s = d_signed/(nf*chan_hz); nt = Nt_q of the width. */
 int volks_bin_to_physical(int32_t nt, int32_t nf, int32_t rate_idx, int32_t delay_idx,

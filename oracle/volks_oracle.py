@@ -197,3 +197,37 @@ def window_match(cands, widths, min_widths=2):
     out = out[:k]
     out["rep"], out["nwidths_hit"], out["t_begin"], out["t_end"] = rep[:k], nhit[:k], tb[:k], te[:k]
     return out
+
+
+def baseline_match(bl, snr, t_begin, t_end, min_baselines=5):
+    """Multi-baseline cross-match ("identified if it is detected with at least 5
+    baselines"; A19), written as the definition: pulses i, j are linked when their AP
+    extents [t_begin, t_end) overlap; connected components (union-find over all O(n^2) pairs) are
+    clusters; a cluster with >= min_baselines distinct baselines is a detection.  Returns a list of
+    dicts {rep, nbaselines, t_begin, t_end} ordered by (t_begin, rep); rep = max-snr member (ties:
+    lowest index).  Pinned by hand constructions only (the paper prints no example)."""
+    n = len(bl)
+    parent = list(range(n))
+
+    def find(x):
+        while parent[x] != x:
+            parent[x] = parent[parent[x]]
+            x = parent[x]
+        return x
+    for i in range(n):
+        for j in range(i + 1, n):
+            if t_begin[i] < t_end[j] and t_begin[j] < t_end[i]:
+                parent[find(i)] = find(j)
+    groups = {}
+    for i in range(n):
+        groups.setdefault(find(i), []).append(i)
+    out = []
+    for members in groups.values():
+        nb = len({int(bl[i]) for i in members})
+        if nb < min_baselines:
+            continue
+        rep = max(members, key=lambda i: (float(snr[i]), -i))
+        out.append(dict(rep=rep, nbaselines=nb, t_begin=int(min(t_begin[i] for i in members)),
+                        t_end=int(max(t_end[i] for i in members))))
+    out.sort(key=lambda d: (d["t_begin"], d["rep"]))
+    return out

@@ -17,6 +17,7 @@ EXPORTS = (
     "volks_plan_create", "volks_plan_destroy", "volks_plan_query", "volks_fringe_search",
     "volks_window_match", "volks_bin_to_physical", "volks_plan_launch_count", "volks_strerror",
     "volks_version", "volks_plan_profile", "volks_plan_profile_read", "volks_fringe_search_dd", "volks_dm_shifts",
+    "volks_baseline_match",
 )
 
 
@@ -32,7 +33,9 @@ CAND_DTYPE = np.dtype([("bl", "<i4"), ("ifq", "<i4"), ("wid", "<i4"), ("win", "<
                        ("rate_idx", "<i4"), ("delay_idx", "<i4"), ("power", "<f4"), ("snr", "<f4")])
 PEAK_DTYPE = np.dtype([("power", "<f4"), ("snr", "<f4"), ("rate_idx", "<i4"), ("delay_idx", "<i4")])
 PULSE_DTYPE = np.dtype([("best", CAND_DTYPE), ("nwidths_hit", "<i4"), ("t_begin", "<i4"), ("t_end", "<i4")])
+DETECTION_DTYPE = np.dtype([("best", PULSE_DTYPE), ("nbaselines", "<i4"), ("t_begin", "<i4"), ("t_end", "<i4")])
 assert CAND_DTYPE.itemsize == 36 and PEAK_DTYPE.itemsize == 16 and PULSE_DTYPE.itemsize == 48
+assert DETECTION_DTYPE.itemsize == 60
 
 _lib = None
 
@@ -56,6 +59,8 @@ def lib():
         L.volks_fringe_search_dd.argtypes = [ctypes.c_void_p] * 6 + [ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
         L.volks_dm_shifts.argtypes = [ctypes.c_double, ctypes.c_void_p, ctypes.c_int32, ctypes.c_double,
                                       ctypes.c_double, ctypes.c_void_p]
+        L.volks_baseline_match.argtypes = [ctypes.c_void_p, ctypes.c_uint32, ctypes.c_int32, ctypes.c_void_p,
+                                           ctypes.c_uint32, ctypes.POINTER(ctypes.c_uint32)]
         L.volks_window_match.argtypes = [ctypes.c_void_p, ctypes.c_uint32, ctypes.c_void_p, ctypes.c_int32,
                                          ctypes.c_int32, ctypes.c_void_p, ctypes.c_uint32,
                                          ctypes.POINTER(ctypes.c_uint32)]
@@ -163,6 +168,16 @@ def window_match(cands, widths, min_widths=2):
     n = ctypes.c_uint32()
     _check(lib().volks_window_match(cands.ctypes.data, len(cands), w.ctypes.data, len(w), min_widths,
                                     out.ctypes.data, len(out), ctypes.byref(n)))
+    return out[:n.value]
+
+
+def baseline_match(pulses, min_baselines=5):
+    """volks_baseline_match on a host numpy PULSE_DTYPE array (the output of window_match)."""
+    pulses = np.ascontiguousarray(pulses, dtype=PULSE_DTYPE)
+    out = np.zeros(max(len(pulses), 1), dtype=DETECTION_DTYPE)
+    n = ctypes.c_uint32()
+    _check(lib().volks_baseline_match(pulses.ctypes.data, len(pulses), min_baselines, out.ctypes.data, len(out),
+                                      ctypes.byref(n)))
     return out[:n.value]
 
 

@@ -1,6 +1,6 @@
 // kernels_slide.cuh - stride-1 rate transform by a sliding sum (widths with stride == 1, Nt == 2w).
 //
-//   k_slide<L>   a4+a5+a6 for every window of one width: per (window, delay column) the zero-padded
+//   k_slide<L, MODD, RING>   a4+a5+a6 for every window of one width: per (window, delay column) the zero-padded
 //                rate DFT, |.|^2 and the per-window argmax, WITHOUT recomputing
 //                the transform of each window from scratch.
 //
@@ -13,13 +13,13 @@
 // segment of SEG windows restarts from an exactly computed transform (fold + L-point FFT), which
 // bounds the growth.
 //
-// Work split: a warp owns 32 adjacent delay columns (lane = column) and one residue rho of the rate
-// index: its thread keeps the L bins r = rho + M s (s < L, M = Nt/L) of its column in registers.
+// Work split: a warp owns 64 adjacent delay columns (lane = column pair) and one residue rho of the
+// rate index: its thread keeps the L bins r = rho + M s (s < L, M = Nt/L) of its two columns in registers.
 //   W_Nt^{r t} = W_Nt^{rho t} * W_L^{s t}:  the first factor is one warp-uniform table value per
 // step, the second depends only on (s, t mod L) and is a compile-time constant once L steps are
 // unrolled - most are trivial (+-1, +-i, (+-1 +- i)/sqrt 2).
-// Warps never synchronise with each other; the per-window maximum is combined across warps with a
-// 64-bit atomicMax on the same total-order key the generic kernel uses.
+// The per-window maximum is combined across the warps of a CTA through shared slots (one barrier per
+// 16 windows) and across CTAs with a 64-bit atomicMax on the total-order key the generic kernel uses.
 //
 // Arithmetic layout (sm_100a packed FP32): a thread works on TWO adjacent delay columns (2c, 2c+1)
 // and keeps every quantity as a 64-bit register pair (column a, column b): X[s] = (Re A_a[s], Re A_b[s]),

@@ -522,6 +522,44 @@ int volks_window_match(const volks_cand *cands, uint32_t ncand, const int32_t *w
   return found.size() > capacity ? VOLKS_EOVERFLOW : VOLKS_OK;
 }
 
+// Host: interval-overlap components over ALL pulses = maximal runs, in t_begin order, whose start lies
+// before the running end.
+int volks_baseline_match(const volks_pulse *pulses, uint32_t npulse, int32_t min_baselines, volks_detection *out,
+                         uint32_t capacity, uint32_t *nout) {
+  if (!nout || (!pulses && npulse) || (!out && capacity)) return VOLKS_EINVAL;
+  std::vector<uint32_t> ord(npulse);
+  for (uint32_t i = 0; i < npulse; ++i) ord[i] = i;
+  std::stable_sort(ord.begin(), ord.end(), [&](uint32_t x, uint32_t y) { return pulses[x].t_begin < pulses[y].t_begin; });
+  uint32_t found = 0, i = 0;
+  std::vector<int32_t> bls;
+  while (i < npulse) {
+    const volks_pulse &f = pulses[ord[i]];
+    int end = f.t_end;
+    uint32_t best = ord[i], k = i + 1;
+    bls.assign(1, f.best.bl);
+    while (k < npulse && pulses[ord[k]].t_begin < end) {
+      const volks_pulse &c = pulses[ord[k]];
+      end = std::max(end, c.t_end);
+      bls.push_back(c.best.bl);
+      const volks_pulse &b = pulses[best];
+      if (c.best.snr > b.best.snr || (c.best.snr == b.best.snr && ord[k] < best)) best = ord[k];
+      ++k;
+    }
+    std::sort(bls.begin(), bls.end());
+    const int nb = (int)(std::unique(bls.begin(), bls.end()) - bls.begin());
+    if (nb >= min_baselines) {
+      if (found < capacity) {
+        out[found].best = pulses[best]; out[found].nbaselines = nb;
+        out[found].t_begin = f.t_begin; out[found].t_end = end;
+      }
+      ++found;
+    }
+    i = k;
+  }
+  *nout = found;
+  return found > capacity ? VOLKS_EOVERFLOW : VOLKS_OK;
+}
+
 int volks_dm_shifts(double dm, const double *f_chan_mhz, int32_t n, double f_ref_mhz, double ap_seconds,
                     int32_t *shift) {
   if (!f_chan_mhz || !shift || n < 0 || !(f_ref_mhz > 0) || !(ap_seconds > 0) || !(dm == dm)) return VOLKS_EINVAL;

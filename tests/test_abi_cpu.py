@@ -129,3 +129,39 @@ def test_dm_shifts_host_vs_oracle(vb, oracle):
         got = vb.dm_shifts(dm, f, f.max(), 1.024e-3)
         assert np.array_equal(got, oracle.dm_shifts(dm, f, f.max(), 1.024e-3))
     assert vb.dm_shifts(100.0, np.array([1400.0, 1500.0]), 1500.0, 1e-3).tolist() == [27, 0]
+
+
+def test_baseline_match_host_vs_oracle(vb, oracle):
+    """f3: constructions (5 baselines overlapping -> kept; 4 -> dropped; same baseline repeated does
+    not count twice; chain overlap A-B-C is one cluster) and random lists against the O(n^2) oracle."""
+    def mk(rows):
+        p = np.zeros(len(rows), dtype=vb.PULSE_DTYPE)
+        for i, (bl, tb, te, snr) in enumerate(rows):
+            p[i]["best"]["bl"], p[i]["best"]["snr"], p[i]["t_begin"], p[i]["t_end"] = bl, snr, tb, te
+        return p
+    five = mk([(b, 100 + b, 110 + b, 7.0 + b) for b in range(5)])
+    d = vb.baseline_match(five, 5)
+    assert len(d) == 1 and d[0]["nbaselines"] == 5 and (d[0]["t_begin"], d[0]["t_end"]) == (100, 114)
+    assert d[0]["best"]["best"]["bl"] == 4
+    assert len(vb.baseline_match(five[:4], 5)) == 0
+    rep = mk([(0, 10, 20, 8.0), (0, 12, 22, 9.0), (1, 15, 25, 7.0)])
+    assert len(vb.baseline_match(rep, 3)) == 0 and vb.baseline_match(rep, 2)[0]["nbaselines"] == 2
+    chain = mk([(0, 0, 10, 6.5), (1, 9, 20, 6.6), (2, 19, 30, 6.4), (3, 40, 50, 9.0)])
+    d = vb.baseline_match(chain, 3)
+    assert len(d) == 1 and (d[0]["t_begin"], d[0]["t_end"], d[0]["nbaselines"]) == (0, 30, 3)
+    rng = np.random.default_rng(9)
+    for trial in range(20):
+        n = int(rng.integers(0, 60))
+        rows = [(int(rng.integers(0, 10)), int(t), int(t + rng.integers(1, 30)), float(rng.integers(60, 90)) / 10)
+                for t in rng.integers(0, 600, n)]
+        p = mk(rows)
+        got = vb.baseline_match(p, 3)
+        exp = oracle.baseline_match(p["best"]["bl"], p["best"]["snr"], p["t_begin"], p["t_end"], 3)
+        assert len(got) == len(exp)
+        for g, e in zip(got, exp):
+            assert g["best"].tobytes() == p[e["rep"]].tobytes()
+            assert (g["nbaselines"], g["t_begin"], g["t_end"]) == (e["nbaselines"], e["t_begin"], e["t_end"])
+    cap = (ctypes.c_uint32(), np.zeros(1, dtype=vb.DETECTION_DTYPE))
+    two = mk([(b, 100, 110, 7.0) for b in range(5)] + [(b, 300, 310, 7.0) for b in range(5)])
+    rc = vb.lib().volks_baseline_match(two.ctypes.data, len(two), 5, cap[1].ctypes.data, 1, ctypes.byref(cap[0]))
+    assert rc == -4 and cap[0].value == 2

@@ -239,3 +239,27 @@ def test_flagged_zero_span_inside_data(vb, oracle):
     vis[0, 0, 300:420] = 0
     stats, ncand, cands, ora = run_both(vb, oracle, vis, c)
     assert np.count_nonzero(ora["p1"] == 0) > 100
+
+
+def test_detection_chain_on_gpu_candidates(vb, oracle):
+    """a7 -> a8 -> f3 on config 2 at reduced extent (10 baselines): candidates -> per-baseline
+    multi-window match -> multi-baseline cross-match (>= 5 baselines).  The host chain
+    must equal the oracle chain on the same candidates, find the station-consistent injected pulses
+    and drop the single-baseline RFI."""
+    vis, c, truth = workloads.generate(2, nbl=10, nif=1, nap=3000, npulses=4)
+    cands, n, _ = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"])
+    pulses = vb.window_match(cands, c["widths"], 2)
+    dets = vb.baseline_match(pulses, 5)
+    exp = oracle.baseline_match(pulses["best"]["bl"], pulses["best"]["snr"], pulses["t_begin"], pulses["t_end"], 5)
+    assert len(dets) == len(exp)
+    for d, e in zip(dets, exp):
+        assert d["best"].tobytes() == pulses[e["rep"]].tobytes()
+        assert (d["nbaselines"], d["t_begin"], d["t_end"]) == (e["nbaselines"], e["t_begin"], e["t_end"])
+    strong = [p for p in truth["pulses"] if p["amp"] * np.sqrt(p["width"] * c["nchan"]) >= 1.5 * c["snr_thresh"] and p["width"] >= 4]
+    assert strong, "the reduced workload must contain a detectable pulse"
+    for p in strong:
+        assert any(d["t_begin"] < p["t0"] + p["width"] and p["t0"] < d["t_end"] for d in dets), p
+    assert all(d["nbaselines"] >= 5 for d in dets)
+    # only the injected pulses are common to >= 5 baselines: every detection must sit on one of them
+    for d in dets:
+        assert any(d["t_begin"] < p["t0"] + p["width"] + 64 and p["t0"] - 64 < d["t_end"] for p in truth["pulses"]), d
