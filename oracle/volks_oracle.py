@@ -231,3 +231,30 @@ def baseline_match(bl, snr, t_begin, t_end, min_baselines=5):
                         t_end=int(max(t_end[i] for i in members))))
     out.sort(key=lambda d: (d["t_begin"], d["rep"]))
     return out
+
+
+def zscore_candidates(peaks, nbl, nif, nap, widths, strides, nf, z_thresh):
+    """f4 - the other reading of PAPER.md:196 ("for the time segments series of given window size, a
+    single pulse is selected if its normalized power exceeds the threshold, which is set to 3"):
+    per (bl, ifq, width) the series of window peak powers P1_j is normalised across windows,
+    z_j = (P1_j - mean_j P1) / std_j P1 (population std; z = 0 when std = 0), candidate iff z > z_thresh.
+    Returns (candidates in canonical order with `snr` = z, z of every window in canonical order)."""
+    bl, ifq, wid, win, t0 = canonical_table(nbl, nif, nap, widths, strides)
+    p1 = np.asarray(peaks["p1"], dtype=np.float64)
+    z = np.zeros(len(p1))
+    per = len(p1) // max(nbl * nif, 1)
+    nws = [nwin(nap, int(w), int(s)) for w, s in zip(widths, strides)]
+    for pair in range(nbl * nif):
+        off = pair * per
+        for n in nws:
+            x = p1[off: off + n]
+            if n:
+                sd = x.std()
+                z[off: off + n] = (x - x.mean()) / sd if sd > 0 else 0.0
+            off += n
+    keep = np.nonzero(z > z_thresh)[0]
+    out = np.zeros(len(keep), dtype=CAND_DTYPE)
+    out["bl"], out["ifq"], out["wid"], out["win"], out["t0"] = bl[keep], ifq[keep], wid[keep], win[keep], t0[keep]
+    out["rate_idx"], out["delay_idx"] = peaks["idx1"][keep] // nf, peaks["idx1"][keep] % nf
+    out["power"], out["snr"] = p1[keep], z[keep]
+    return out, z

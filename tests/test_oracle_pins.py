@@ -359,3 +359,25 @@ def test_dedispersed_pulse_closed_form(oracle):
     assert abs(o["p1"] - (a * w * nchan) ** 2) < 1e-6 * o["p1"]
     raw, _ = oracle.search(vis, [w], [1], [nt], nf, mode="fft")
     assert raw["p1"].max() < 0.5 * o["p1"]            # without step 4 the pulse is smeared
+
+
+def test_zscore_selection_pins(oracle):
+    """f4: hand-computed series.  P1 = [1, 1, 1, 1, 9]: mean 2.6, population std 3.2 -> z = [-0.5]*4 + [2.0];
+    strict threshold; a constant series (std 0) selects nothing; series of different (pair, width) are
+    normalised separately."""
+    def peaks_of(p):
+        pk = np.zeros(len(p), dtype=oracle.PEAK_DTYPE)
+        pk["p1"] = p
+        pk["idx1"] = 7
+        return pk
+    c, z = oracle.zscore_candidates(peaks_of([1, 1, 1, 1, 9]), 1, 1, 5, [1], [1], 4, 1.9)
+    assert np.allclose(z, [-0.5, -0.5, -0.5, -0.5, 2.0]) and len(c) == 1 and c[0]["win"] == 4 and c[0]["snr"] == 2.0
+    assert (c[0]["rate_idx"], c[0]["delay_idx"]) == (1, 3)
+    assert len(oracle.zscore_candidates(peaks_of([1, 1, 1, 1, 9]), 1, 1, 5, [1], [1], 4, 2.0)[0]) == 0   # strict >
+    assert len(oracle.zscore_candidates(peaks_of([3, 3, 3, 3, 3]), 1, 1, 5, [1], [1], 4, 0.0)[0]) == 0
+    # two pairs x two widths (nap = 4: widths 1 and 2 -> 4 + 3 windows per pair)
+    p = [1, 1, 1, 9,   2, 2, 8,    5, 5, 5, 5,   0, 10, 0]
+    c, z = oracle.zscore_candidates(peaks_of(p), 2, 1, 4, [1, 2], [1, 1], 4, 1.0)
+    assert np.allclose(z[:4], (np.array([1, 1, 1, 9]) - 3) / np.std([1, 1, 1, 9]))
+    assert np.allclose(z[7:11], 0) and np.allclose(z[11:], (np.array([0, 10, 0]) - 10 / 3) / np.std([0, 10, 0]))
+    assert [(int(r["bl"]), int(r["wid"]), int(r["win"])) for r in c] == [(0, 0, 3), (0, 1, 2), (1, 1, 1)]
