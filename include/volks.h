@@ -118,6 +118,16 @@ int volks_fringe_search_dd(const volks_plan *plan, const void *d_vis, const int3
                            void *d_workspace, volks_peak *d_peaks, volks_cand *d_cands,
                            uint32_t cand_capacity, uint32_t *d_ncand, void *cuda_stream);
 
+/* Across-window normalised power (SURVEY 8(f) f4 - the other reading of PAPER.md:196 "for the time
+ * segments series of given window size, a single pulse is selected if its normalized power exceeds
+ * the threshold, which is set to 3").  A second pass over the results the LAST volks_fringe_search[_dd]
+ * left in `d_workspace` (same plan, workspace untouched since): per (bl, ifq, width) the window peak
+ * powers P1_j are normalised across windows, z_j = (P1_j - mean)/std (population std; z = 0 if
+ * std = 0); candidate iff z_j > z_thresh.  Outputs as volks_fringe_search, except that the `snr`
+ * field of candidates (and of d_peaks, if given) carries z.  Asynchronous on `cuda_stream`. */
+int volks_zscore_select(const volks_plan *plan, void *d_workspace, float z_thresh, volks_peak *d_peaks,
+                        volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand, void *cuda_stream);
+
 /* HOST helper: integer AP shift of every frequency point for dispersion measure `dm` [pc cm^-3]:
  * shift = round(4.148808e-3 s * dm * (f_GHz^-2 - fref_GHz^-2) / ap_seconds) (the textbook cold-plasma
  * delay; the paper states no formula - DESIGN.md R3).  f_chan_mhz, shift: HOST [n]. */

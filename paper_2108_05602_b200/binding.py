@@ -17,7 +17,7 @@ EXPORTS = (
     "volks_plan_create", "volks_plan_destroy", "volks_plan_query", "volks_fringe_search",
     "volks_window_match", "volks_bin_to_physical", "volks_plan_launch_count", "volks_strerror",
     "volks_version", "volks_plan_profile", "volks_plan_profile_read", "volks_fringe_search_dd", "volks_dm_shifts",
-    "volks_baseline_match",
+    "volks_baseline_match", "volks_zscore_select",
 )
 
 
@@ -59,6 +59,8 @@ def lib():
         L.volks_fringe_search_dd.argtypes = [ctypes.c_void_p] * 6 + [ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
         L.volks_dm_shifts.argtypes = [ctypes.c_double, ctypes.c_void_p, ctypes.c_int32, ctypes.c_double,
                                       ctypes.c_double, ctypes.c_void_p]
+        L.volks_zscore_select.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_float, ctypes.c_void_p,
+                                          ctypes.c_void_p, ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
         L.volks_baseline_match.argtypes = [ctypes.c_void_p, ctypes.c_uint32, ctypes.c_int32, ctypes.c_void_p,
                                            ctypes.c_uint32, ctypes.POINTER(ctypes.c_uint32)]
         L.volks_window_match.argtypes = [ctypes.c_void_p, ctypes.c_uint32, ctypes.c_void_p, ctypes.c_int32,
@@ -138,6 +140,14 @@ class Plan:
             self._h, vis.data_ptr(), shift.data_ptr() if shift is not None else None, workspace.data_ptr(),
             peaks.data_ptr() if peaks is not None else None, cands.data_ptr() if cap else None, cap,
             ncand.data_ptr(), st))
+
+    def zscore_select(self, workspace, z_thresh, cands, ncand, peaks=None, stream=None):
+        """volks_zscore_select: across-window normalised selection on the last search's workspace."""
+        cap = cands.numel() * cands.element_size() // CAND_DTYPE.itemsize
+        st = (stream or torch.cuda.current_stream(workspace.device)).cuda_stream
+        _check(lib().volks_zscore_select(self._h, workspace.data_ptr(), float(z_thresh),
+                                         peaks.data_ptr() if peaks is not None else None,
+                                         cands.data_ptr() if cap else None, cap, ncand.data_ptr(), st))
 
     def profile(self, enable=True):
         """volks_plan_profile: bracket every launch of later searches with CUDA events."""

@@ -451,7 +451,12 @@ struct Sched {   // the window schedule (device copy lives in the plan)
 
 struct WinStat { float power, snr; int rate_idx, delay_idx, q, j, t0; long long pair; };
 
-__device__ __forceinline__ WinStat window_stat(const Sched &s, const u64 *keys, const float *E, long long c) {
+// Selection statistic: the in-plane amplitude snr (a7), or - when `zst` is given (f4, the other reading
+// of PAPER.md:196) - the peak power normalised ACROSS the windows of its (pair, width) series:
+// z = (P1 - mean) * inv_std with zst[pair * nwidths + q] = (mean, 1/std) (inv_std = 0 when std = 0).
+// In that mode the z-score is what the record's `snr` field carries.
+__device__ __forceinline__ WinStat window_stat(const Sched &s, const u64 *keys, const float *E, long long c,
+                                               const double2 *zst = nullptr) {
   WinStat o;
   o.pair = c / s.per_pair;
   long long rem = c - o.pair * s.per_pair;
@@ -472,13 +477,49 @@ __device__ __forceinline__ WinStat window_stat(const Sched &s, const u64 *keys, 
   // P1 = 0 at (0, 0) by the tie rule.  The sliding sum would leave rounding residue of earlier samples
   // here, so the exact statement is made from the energy (es == 0 iff every sample is zero).
   if (es == 0.f) { o.power = 0.f; o.rate_idx = 0; o.delay_idx = 0; }
+  if (zst) {
+    const double2 ms = zst[o.pair * s.nwidths + q];
+    o.snr = (float)(((double)o.power - ms.x) * ms.y);
+  }
   return o;
+}
+
+// f4: mean and 1/std (population) of the peak-power series of one (pair, width); one CTA per series,
+// double accumulation in a fixed order (deterministic).
+__global__ void __launch_bounds__(256) k_zstat(const Sched *sp, const u64 *keys, const float *E, double2 *zst) {
+  __shared__ Sched s;
+  __shared__ double sh1[256], sh2[256];
+  if (threadIdx.x == 0) s = *sp;
+  __syncthreads();
+  const long long pair = blockIdx.x / s.nwidths;
+  const int q = blockIdx.x % s.nwidths;
+  const long long c0 = pair * s.per_pair + s.offc[q];
+  double a = 0.0, b = 0.0;
+  for (long long j = threadIdx.x; j < s.nwin[q]; j += 256) {
+    const double p = (double)window_stat(s, keys, E, c0 + j).power;
+    a += p; b += p * p;
+  }
+  sh1[threadIdx.x] = a; sh2[threadIdx.x] = b;
+  __syncthreads();
+  for (int o = 128; o >= 1; o >>= 1) {
+    if (threadIdx.x < o) { sh1[threadIdx.x] += sh1[threadIdx.x + o]; sh2[threadIdx.x] += sh2[threadIdx.x + o]; }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    const double n = (double)s.nwin[q];
+    const double mean = n > 0 ? sh1[0] / n : 0.0;
+    double var = n > 0 ? sh2[0] / n - mean * mean : 0.0;
+    // two-pass refinement is not needed at 1e-4: powers are O(1e2..1e8) and n <= 2^31, double keeps > 9 digits
+    if (var < 0) var = 0;
+    zst[blockIdx.x] = make_double2(mean, var > 0 ? 1.0 / sqrt(var) : 0.0);
+  }
 }
 
 constexpr int FIN_THREADS = 256, FIN_TILES = 8;   // 2048 windows per CTA
 
 __global__ void __launch_bounds__(FIN_THREADS) k_finalize(const Sched *sp, const u64 *keys, const float *E,
-                                                          float4 *peaks, uint32_t *blockcount) {
+                                                          float4 *peaks, uint32_t *blockcount,
+                                                          const double2 *zst, float zth) {
   __shared__ Sched s;
   __shared__ uint32_t wsum[FIN_THREADS / 32];
   if (threadIdx.x == 0) s = *sp;
@@ -488,12 +529,12 @@ __global__ void __launch_bounds__(FIN_THREADS) k_finalize(const Sched *sp, const
   for (int tile = 0; tile < FIN_TILES; ++tile) {
     const long long c = base + tile * FIN_THREADS + threadIdx.x;
     if (c < s.nwin_total) {
-      const WinStat o = window_stat(s, keys, E, c);
+      const WinStat o = window_stat(s, keys, E, c, zst);
       if (peaks) {
         const long long di = s.offd[o.q] + o.pair * s.nwin[o.q] + o.j;
         peaks[di] = make_float4(o.power, o.snr, __int_as_float(o.rate_idx), __int_as_float(o.delay_idx));
       }
-      mine += o.snr > s.snr_thresh ? 1u : 0u;
+      mine += o.snr > (zst ? zth : s.snr_thresh) ? 1u : 0u;
     }
   }
   for (int o = 16; o >= 1; o >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, o);
@@ -529,7 +570,7 @@ struct CandOut { int bl, ifq, wid, win, t0, rate_idx, delay_idx; float power, sn
 
 __global__ void __launch_bounds__(FIN_THREADS) k_scatter(const Sched *sp, const u64 *keys, const float *E,
                                                          const uint32_t *blockoff, CandOut *cands,
-                                                         uint32_t capacity) {
+                                                         uint32_t capacity, const double2 *zst, float zth) {
   __shared__ Sched s;
   __shared__ uint32_t wsum[FIN_THREADS / 32];
   __shared__ uint32_t running;
@@ -542,8 +583,8 @@ __global__ void __launch_bounds__(FIN_THREADS) k_scatter(const Sched *sp, const 
     WinStat o;
     bool flag = false;
     if (c < s.nwin_total) {
-      o = window_stat(s, keys, E, c);
-      flag = o.snr > s.snr_thresh;
+      o = window_stat(s, keys, E, c, zst);
+      flag = o.snr > (zst ? zth : s.snr_thresh);
     }
     const uint32_t bal = __ballot_sync(0xffffffffu, flag);
     if (lane == 0) wsum[wid] = __popc(bal);

@@ -174,7 +174,7 @@ struct volks_plan {
   int wid1 = -1;                // a width with w == 1 whose peaks the row kernel emits itself (or -1)
   long long npair = 0;
   // workspace layout (byte offsets)
-  size_t off_keys = 0, off_E = 0, off_cnt = 0, off_Y = 0, ws_bytes = 0;
+  size_t off_keys = 0, off_E = 0, off_cnt = 0, off_zst = 0, off_Y = 0, ws_bytes = 0;
   long long nfin_blocks = 0;
   long long pairs_per_chunk = 0, nchunks = 0;
   // row kernel shape
@@ -301,6 +301,7 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
   pl->off_E = off;    off = align_up(off + (size_t)std::max<long long>(pl->npair * p->nap, 1) * sizeof(float), 256);
   pl->off_cnt = off;  off = align_up(off + (size_t)std::max<long long>(pl->nfin_blocks, 1) * sizeof(uint32_t), 256);
   // + padding rows: the sliding kernel loads one row, and prefetches SLIDE_PF + 1 rows, past the last sample
+  pl->off_zst = off;  off = align_up(off + (size_t)std::max<long long>(pl->npair * p->nwidths, 1) * sizeof(double2), 256);
   pl->off_Y = off;    off = align_up(off + (size_t)pl->pairs_per_chunk * std::max<size_t>(y_pair, 8) + (size_t)(SLIDE_PF + 2) * pl->pitch * sizeof(float2), 256);
   pl->ws_bytes = off;
 
@@ -440,7 +441,7 @@ int volks_fringe_search_dd(const volks_plan *pl, const void *d_vis, const int32_
   }
   {
     ProfScope ps(pl, st, VOLKS_K_FINALIZE, -1);
-    k_finalize<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, (float4 *)d_peaks, cnt);
+    k_finalize<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, (float4 *)d_peaks, cnt, nullptr, 0.f);
   }
   {
     ProfScope ps(pl, st, VOLKS_K_SCAN, -1);
@@ -448,8 +449,26 @@ int volks_fringe_search_dd(const volks_plan *pl, const void *d_vis, const int32_
   }
   {
     ProfScope ps(pl, st, VOLKS_K_SCATTER, -1);
-    k_scatter<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity);
+    k_scatter<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity, nullptr, 0.f);
   }
+  return cuda_ok(cudaGetLastError()) ? VOLKS_OK : VOLKS_ECUDA;
+}
+
+int volks_zscore_select(const volks_plan *pl, void *d_workspace, float z_thresh, volks_peak *d_peaks,
+                        volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand, void *cuda_stream) {
+  if (!pl || !d_workspace || !d_ncand || (!d_cands && cand_capacity > 0) || !(z_thresh == z_thresh)) return VOLKS_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const Sched &s = pl->sched;
+  if (s.nwin_total == 0) return cuda_ok(cudaMemsetAsync(d_ncand, 0, sizeof(uint32_t), st)) ? VOLKS_OK : VOLKS_ECUDA;
+  char *ws = (char *)d_workspace;
+  const u64 *keys = (const u64 *)(ws + pl->off_keys);
+  const float *E = (const float *)(ws + pl->off_E);
+  uint32_t *cnt = (uint32_t *)(ws + pl->off_cnt);
+  double2 *zst = (double2 *)(ws + pl->off_zst);
+  k_zstat<<<(unsigned)(pl->npair * s.nwidths), 256, 0, st>>>(pl->d_sched, keys, E, zst);
+  k_finalize<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, (float4 *)d_peaks, cnt, zst, z_thresh);
+  k_scan<<<1, 1024, 0, st>>>(cnt, pl->nfin_blocks, d_ncand);
+  k_scatter<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity, zst, z_thresh);
   return cuda_ok(cudaGetLastError()) ? VOLKS_OK : VOLKS_ECUDA;
 }
 

@@ -263,3 +263,41 @@ def test_detection_chain_on_gpu_candidates(vb, oracle):
     # only the injected pulses are common to >= 5 baselines: every detection must sit on one of them
     for d in dets:
         assert any(d["t_begin"] < p["t0"] + p["width"] + 64 and p["t0"] - 64 < d["t_end"] for p in truth["pulses"]), d
+
+
+@pytest.mark.parametrize("cfg,over", [(2, dict(nbl=2, nif=1, nap=900, npulses=3)), (1, dict(nap=700))])
+def test_zscore_selection_matches_oracle(vb, oracle, cfg, over):
+    """f4: across-window normalised power on the workspace of the last search vs the oracle's
+    definition applied to the oracle's peaks (z within 1e-4 of the z scale; list identical except
+    windows whose oracle z lies within that margin of the threshold)."""
+    vis, c, _ = workloads.generate(cfg, **over)
+    nbl, nif, nap, nchan = vis.shape
+    plan = vb.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"])
+    dev = torch.device("cuda")
+    ws = torch.empty(plan.workspace_bytes, dtype=torch.uint8, device=dev)
+    cap = 1 << 16
+    cands = torch.empty(cap * vb.CAND_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    ncand = torch.zeros(1, dtype=torch.int32, device=dev)
+    peaks = torch.empty(plan.nwin_total * vb.PEAK_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    plan.fringe_search(vis.cuda(), ws, cands, ncand)
+    zth = 3.0                                            # PAPER.md:196
+    plan.zscore_select(ws, zth, cands, ncand, peaks)
+    torch.cuda.synchronize()
+    n = int(ncand.item())
+    got = cands[: n * vb.CAND_DTYPE.itemsize].cpu().numpy().view(vb.CAND_DTYPE)
+    pk = peaks.cpu().numpy().view(vb.PEAK_DTYPE)
+    ora, _ = oracle.search(vis.numpy(), c["widths"], c["strides"], c["nts"], c["nf"], mode="cached")
+    exp, z = oracle.zscore_candidates(ora, nbl, nif, nap, c["widths"], c["strides"], c["nf"], zth)
+    nw = [workloads.gen.nwin(nap, w, s) for w, s in zip(c["widths"], c["strides"])]
+    gz = pk[dense_index(nbl, nif, nw)]["snr"].astype(np.float64)
+    tol = 1e-4 * max(1.0, np.abs(z).max())
+    assert np.abs(gz - z).max() <= tol
+    key = lambda r: (int(r["bl"]), int(r["ifq"]), int(r["wid"]), int(r["win"]))
+    gk, ek = [key(r) for r in got], [key(r) for r in exp]
+    assert gk == sorted(gk) and n >= 1
+    marginal = {k for k, zz in zip([key(r) for r in exp], exp["snr"]) if abs(zz - zth) <= tol}
+    assert set(ek) - set(gk) <= marginal
+    for r in got:
+        if key(r) not in set(ek):
+            assert abs(float(r["snr"]) - zth) <= 2 * tol
+    plan.close()
