@@ -179,6 +179,21 @@ def run_reference(args):
 # `ncu --set full` captures (profiles/r01_ncu_rate_kernels.md); keyed by (config, kernel, width)
 NCU_TRAFFIC = {(2, "slide", 64): 3.97e9, (4, "colfft", 64): 3.97e9}
 
+def max_over_ranks(dist, ms, device):
+    """Replicas only: the one cross-rank step is the MAX of the device-timed
+    milliseconds; `dist` is torch.distributed or None (single process)."""
+    if dist is None:
+        return float(ms)
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(world, units_per_rank, ms_step):
+    """Whole-job throughput of `world` independent replicas, each doing `units_per_rank` per step."""
+    return world * units_per_rank / (ms_step * 1e-3)
+
+
 KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6: "slide", 7: "colfft"}
 
 
@@ -238,14 +253,11 @@ def run_volks(args):
     ms_total = e0.elapsed_time(e1)
     sampler.stop_flag = True
     sampler.join()
-    if dist is not None:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(dist, ms_total, dev)
     ms_step = ms_total / args.steps
     nwin = plan.nwin_total
     nvis = nbl * nif * nap * nchan
-    value = world * nwin / (ms_step * 1e-3)
+    value = aggregate_value(world, nwin, ms_step)
     n_found = int(ncand.item())
 
     # ---- roofline leg: per-launch CUDA-event durations on the launching stream ----
@@ -335,11 +347,7 @@ def run_e2e(R, steps):
     e1.record(stream)
     torch.cuda.synchronize(dev)
     ms = e0.elapsed_time(e1)
-    if R["dist"] is not None:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        R["dist"].all_reduce(t, op=R["dist"].ReduceOp.MAX)
-        ms = float(t.item())
-    ms /= steps
+    ms = max_over_ranks(R["dist"], ms, dev) / steps
     return {"value": R["world"] * R["nwin"] / (ms * 1e-3), "unit": "windows/s", "ms_per_step": ms,
             "h2d_bytes_per_step": int(h_vis.numel() * 8), "d2h_bytes_per_step": int(d2h)}
 
