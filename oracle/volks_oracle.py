@@ -258,3 +258,43 @@ def zscore_candidates(peaks, nbl, nif, nap, widths, strides, nf, z_thresh):
     out["rate_idx"], out["delay_idx"] = peaks["idx1"][keep] // nf, peaks["idx1"][keep] % nf
     out["power"], out["snr"] = p1[keep], z[keep]
     return out, z
+
+
+def allif_band(vis):
+    """[nbl][nif][nap][nchan] -> [nbl][nap][nif*nchan]: the frequency points of all IFs of one AP in
+    sky-frequency order, IFs contiguous (f = f0 + (n*nchan + j)*df; reading A21)."""
+    vis = np.asarray(vis)
+    nbl, nif, nap, nchan = vis.shape
+    return np.ascontiguousarray(vis.transpose(0, 2, 1, 3)).reshape(nbl, nap, nif * nchan)
+
+
+def allif_search(vis, widths, strides, nfa):
+    """f2 - VOLKS2's own fringe search, Eq. 1: ONE delay across all IFs,
+        G(dtau) = sum_n sum_j S(n, j) e^{-i Phi},  Phi = 2 pi f_j^n dtau,
+    evaluated with one zero-padded FFT over the whole band per AP ("32768 sized FFT"),
+    the APs of a window summed coherently (step 6), then the maximum along the delay axis.
+    Per (bl, width, window): A[d] = sum_{t<w} sum_m band[t0+t][m] e^{-2 pi i m d/nfa}; P = |A|^2;
+    (P1, idx1) first argmax, (P2, idx2) runner-up, S1 = sum_d P, snr = sqrt(P1/(S1/nfa)) (A3's statistic
+    on the delay axis).  Evaluated as the rate-0 row of this oracle's own 2-D plane of the band window
+    (pin P4 / PAPER.md:133, 143: summing per-AP spectra == spectrum of the sum).
+    Output order: canonical (bl, q, j); PEAK_DTYPE records."""
+    band = allif_band(vis)
+    nbl, nap, nm = band.shape
+    out = []
+    for b in range(nbl):
+        for w, s in zip(widths, strides):
+            nt = 1
+            while nt < w:
+                nt *= 2
+            for j in range(nwin(nap, int(w), int(s))):
+                _, plane = window(band[b, j * s: j * s + w], nt, nfa, mode="fft", want_plane=True)
+                a = plane[0]
+                p = a.real * a.real + a.imag * a.imag
+                i1 = int(np.argmax(p))
+                q = p.copy()
+                q[i1] = -1.0
+                i2 = int(np.argmax(q)) if nfa > 1 else i1
+                s1 = float(p.sum())
+                noise = s1 / nfa
+                out.append((p[i1], q[i2] if nfa > 1 else 0.0, s1, np.sqrt(p[i1] / noise) if noise > 0 else 0.0, i1, i2))
+    return np.array(out, dtype=PEAK_DTYPE) if out else np.zeros(0, dtype=PEAK_DTYPE)

@@ -381,3 +381,39 @@ def test_zscore_selection_pins(oracle):
     assert np.allclose(z[:4], (np.array([1, 1, 1, 9]) - 3) / np.std([1, 1, 1, 9]))
     assert np.allclose(z[7:11], 0) and np.allclose(z[11:], (np.array([0, 10, 0]) - 10 / 3) / np.std([0, 10, 0]))
     assert [(int(r["bl"]), int(r["wid"]), int(r["win"])) for r in c] == [(0, 0, 3), (0, 1, 2), (1, 1, 1)]
+
+
+def test_allif_search_pins(oracle):
+    """f2 (Eq. 1).  Closed form: a noiseless fringe with one delay across all IFs,
+    S = a e^{+2 pi i tau m / (nif nchan)} on every AP of the window, peaks at d = tau nfa/(nif nchan) with
+    P1 = (a w nif nchan)^2 and snr = sqrt(nif nchan); the sign-flipped fringe must land at -tau.  Library
+    special case: numpy.fft.fft of the time-summed band.  Parseval: S1 = nfa sum_m |sum_t S|^2.  A delay
+    that is NOT common to the IFs (a per-IF fringe restarting its phase in every IF) must not reach that peak."""
+    nbl, nif, nap, nchan, w, nfa, a, tau = 2, 4, 12, 8, 4, 128, 0.5, 5
+    m = np.arange(nif * nchan)
+    fr = (a * np.exp(2j * np.pi * tau * m / (nif * nchan))).astype(np.complex64).reshape(nif, 1, nchan)
+    vis = np.zeros((nbl, nif, nap, nchan), np.complex64)
+    vis[0, :, 3:3 + w, :] = fr
+    vis[1, :, 3:3 + w, :] = np.conj(fr)
+    pk = oracle.allif_search(vis, [w], [1], nfa)
+    nwin = nap - w + 1
+    o = pk[3]
+    assert o["idx1"] == tau * nfa // (nif * nchan) and abs(o["p1"] - (a * w * nif * nchan) ** 2) < 1e-6 * o["p1"]   # complex64 inputs
+    assert abs(o["snr"] - np.sqrt(nif * nchan)) < 1e-6
+    assert pk[nwin + 3]["idx1"] == nfa - tau * nfa // (nif * nchan)
+    rng = np.random.default_rng(11)
+    noise = (rng.normal(size=vis.shape) + 1j * rng.normal(size=vis.shape)).astype(np.complex64)
+    pk = oracle.allif_search(noise, [w, 2], [3, 1], nfa)
+    band = oracle.allif_band(noise).astype(np.complex128)
+    k = 0
+    for b in range(nbl):
+        for ww, s in ((w, 3), (2, 1)):
+            for j in range((nap - ww) // s + 1):
+                ref = np.abs(np.fft.fft(band[b, j * s: j * s + ww].sum(axis=0), nfa)) ** 2
+                assert pk[k]["idx1"] == int(np.argmax(ref)) and abs(pk[k]["p1"] - ref.max()) < 1e-9 * ref.max()
+                assert abs(pk[k]["s1"] - nfa * (np.abs(band[b, j * s: j * s + ww].sum(axis=0)) ** 2).sum()) < 1e-9 * pk[k]["s1"]
+                k += 1
+    assert k == len(pk)
+    per_if = np.zeros((1, nif, nap, nchan), np.complex64)
+    per_if[0, :, 3:3 + w, :] = (a * np.exp(2j * np.pi * tau * np.arange(nchan) / nchan)).astype(np.complex64)
+    assert oracle.allif_search(per_if, [w], [1], nfa)[3]["p1"] < 0.9 * (a * w * nif * nchan) ** 2 or tau % nif == 0
