@@ -415,5 +415,6 @@ def test_allif_search_pins(oracle):
                 k += 1
     assert k == len(pk)
     per_if = np.zeros((1, nif, nap, nchan), np.complex64)
-    per_if[0, :, 3:3 + w, :] = (a * np.exp(2j * np.pi * tau * np.arange(nchan) / nchan)).astype(np.complex64)
-    assert oracle.allif_search(per_if, [w], [1], nfa)[3]["p1"] < 0.9 * (a * w * nif * nchan) ** 2 or tau % nif == 0
+    # phase restarting in every IF with a half-integer per-IF delay: adjacent IFs are pi apart
+    per_if[0, :, 3:3 + w, :] = (a * np.exp(2j * np.pi * 2.5 * np.arange(nchan) / nchan)).astype(np.complex64)
+    assert oracle.allif_search(per_if, [w], [1], nfa)[3]["p1"] < 0.9 * (a * w * nif * nchan) ** 2
