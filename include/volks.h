@@ -118,6 +118,24 @@ int volks_fringe_search_dd(const volks_plan *plan, const void *d_vis, const int3
                            void *d_workspace, volks_peak *d_peaks, volks_cand *d_cands,
                            uint32_t cand_capacity, uint32_t *d_ncand, void *cuda_stream);
 
+/* f2 - VOLKS2's own search: ONE delay across all IFs (Eq. 1), rate 0 only.  For every
+ * baseline, width and window the per-AP all-IF delay spectra (one zero-padded FFT over the whole band
+ * of nif*nchan frequency points per AP; IFs contiguous in frequency, A21) are summed
+ * coherently over the window's APs (step 6) and the maximum along the delay axis is found:
+ *   A[d] = sum_{t<w} sum_{m<nif*nchan} band[t0+t][m] exp(-2 pi i m d/nfa),  m = n*nchan + j,
+ *   P = |A|^2, (P1, d*) first argmax, noise = mean_d P, snr = sqrt(P1/noise), candidate iff snr > snr_thresh.
+ * volks_plan_create_allif reads nbl, nif, nap, nchan, nwidths, width[], stride[], snr_thresh and
+ * nf = nfa (power of two, nif*nchan <= nfa, 64 <= nfa <= 8192); nt[] is ignored (may be NULL).
+ * volks_allif_search takes the same buffers as volks_fringe_search_dd (d_shift: dedispersion, or NULL);
+ * sizes from volks_plan_query (nwin_total = nbl * sum_q nwin_q).  Records: ifq = -1, rate_idx = 0,
+ * delay_idx in [0, nfa); canonical order (bl, q, j); dense peaks d_peaks[off_q + bl*nwin_q + j].
+ * volks_zscore_select, volks_window_match (ifq = -1 groups a baseline) and volks_baseline_match apply
+ * to its results unchanged. */
+int volks_plan_create_allif(const volks_params *p, volks_plan **out);
+int volks_allif_search(const volks_plan *plan, const void *d_vis, const int32_t *d_shift, void *d_workspace,
+                       volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity,
+                       uint32_t *d_ncand, void *cuda_stream);
+
 /* Across-window normalised power (SURVEY 8(f) f4 - the other reading of PAPER.md:196 "for the time
  * segments series of given window size, a single pulse is selected if its normalized power exceeds
  * the threshold, which is set to 3").  A second pass over the results the LAST volks_fringe_search[_dd]
@@ -181,6 +199,7 @@ int volks_plan_launch_count(const volks_plan *plan);
 #define VOLKS_K_SCATTER 5  /* ordered candidate scatter                                            */
 #define VOLKS_K_SLIDE 6    /* stride-1 widths: sliding-sum rate transform + power + argmax          */
 #define VOLKS_K_COLFFT 7   /* any stride, Nt 32..512: two-pass shared-memory column FFT + argmax    */
+#define VOLKS_K_ALLIF 8    /* f2: all-IF rate-0 window sums + argmax + noise                          */
 int volks_plan_profile(volks_plan *plan, int enable);
 int volks_plan_profile_read(const volks_plan *plan, int32_t capacity, int32_t *kind, int32_t *wid,
                             float *ms, int32_t *n);

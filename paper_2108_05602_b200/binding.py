@@ -17,7 +17,7 @@ EXPORTS = (
     "volks_plan_create", "volks_plan_destroy", "volks_plan_query", "volks_fringe_search",
     "volks_window_match", "volks_bin_to_physical", "volks_plan_launch_count", "volks_strerror",
     "volks_version", "volks_plan_profile", "volks_plan_profile_read", "volks_fringe_search_dd", "volks_dm_shifts",
-    "volks_baseline_match", "volks_zscore_select",
+    "volks_baseline_match", "volks_zscore_select", "volks_plan_create_allif", "volks_allif_search",
 )
 
 
@@ -52,6 +52,8 @@ def lib():
         L.volks_strerror.restype = ctypes.c_char_p
         L.volks_strerror.argtypes = [ctypes.c_int]
         L.volks_plan_create.argtypes = [ctypes.POINTER(volks_params), ctypes.POINTER(ctypes.c_void_p)]
+        L.volks_plan_create_allif.argtypes = [ctypes.POINTER(volks_params), ctypes.POINTER(ctypes.c_void_p)]
+        L.volks_allif_search.argtypes = [ctypes.c_void_p] * 6 + [ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
         L.volks_plan_destroy.argtypes = [ctypes.c_void_p]
         L.volks_plan_query.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_size_t),
                                        ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
@@ -88,25 +90,28 @@ def _check(rc):
         raise VolksError(rc)
 
 
-def plan_create_raw(nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh):
-    """volks_plan_create; returns (rc, handle) without raising (for error-path tests)."""
+def plan_create_raw(nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh, allif=False):
+    """volks_plan_create[_allif]; returns (rc, handle) without raising (for error-path tests)."""
     n = len(widths)
     arr = lambda v: (ctypes.c_int32 * max(len(v), 1))(*[int(x) for x in v])
     w, s, t = arr(widths), arr(strides), arr(nts)
     p = volks_params(nbl, nif, nap, nchan, n, w, s, t, nf, float(snr_thresh))
     h = ctypes.c_void_p()
-    rc = lib().volks_plan_create(ctypes.byref(p), ctypes.byref(h))
+    rc = (lib().volks_plan_create_allif if allif else lib().volks_plan_create)(ctypes.byref(p), ctypes.byref(h))
     return rc, h
 
 
 class Plan:
     """volks_plan_* : validated parameters + window schedule + device tables."""
 
-    def __init__(self, nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh):
+    def __init__(self, nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh, allif=False):
+        """allif=True: the f2 plan (volks_plan_create_allif; `nts` ignored, nf = nfa)."""
+        self.allif = bool(allif)
+        nts = [1] * len(widths) if allif else nts
         self.shape = (nbl, nif, nap, nchan)
         self.widths, self.strides, self.nts, self.nf = list(widths), list(strides), list(nts), nf
         self.snr_thresh = float(snr_thresh)
-        rc, self._h = plan_create_raw(nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh)
+        rc, self._h = plan_create_raw(nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh, allif)
         _check(rc)
         ws, tot = ctypes.c_size_t(), ctypes.c_int64()
         per = (ctypes.c_int64 * len(widths))()
@@ -136,7 +141,7 @@ class Plan:
         if shift is not None:
             assert shift.is_cuda and shift.dtype == torch.int32 and shift.is_contiguous()
             assert tuple(shift.shape) == (self.shape[1], self.shape[3])
-        _check(lib().volks_fringe_search_dd(
+        _check((lib().volks_allif_search if self.allif else lib().volks_fringe_search_dd)(
             self._h, vis.data_ptr(), shift.data_ptr() if shift is not None else None, workspace.data_ptr(),
             peaks.data_ptr() if peaks is not None else None, cands.data_ptr() if cap else None, cap,
             ncand.data_ptr(), st))
@@ -204,6 +209,16 @@ def dm_shifts(dm, f_chan_mhz, f_ref_mhz, ap_seconds):
     out = np.zeros(f.shape, dtype=np.int32)
     _check(lib().volks_dm_shifts(float(dm), f.ctypes.data, f.size, float(f_ref_mhz), float(ap_seconds), out.ctypes.data))
     return out
+
+
+def allif_search(vis, widths, strides, nfa, snr_thresh, want_peaks=False, cand_capacity=1 << 20, shifts=None):
+    """One-shot f2 search (volks_plan_create_allif + volks_allif_search); returns like fringe_search."""
+    nbl, nif, nap, nchan = vis.shape
+    plan = Plan(nbl, nif, nap, nchan, widths, strides, None, nfa, snr_thresh, allif=True)
+    try:
+        return fringe_search(vis, want_peaks=want_peaks, cand_capacity=cand_capacity, plan=plan, shifts=shifts)
+    finally:
+        plan.close()
 
 
 def fringe_search(vis, widths=None, strides=None, nts=None, nf=None, snr_thresh=None, want_peaks=False,

@@ -1,0 +1,106 @@
+// kernels_allif.cuh - f2: VOLKS2's own fringe search, one delay across all IFs (Eq. 1).
+//
+//   k_allif   per (baseline, width, window): A[d] = sum_{t<w} Y[t0+t][d] (the coherent sum of the
+//             per-AP all-IF delay spectra, step 6 of the paper), P = |A|^2, the first
+//             argmax over the delay axis, and S1 = sum_d P (noise statistic, A3 on the
+//             delay axis).  Y[t][d] is the zero-padded FFT of the AP's whole band (all IFs in
+//             frequency order) written by the row kernels in their all-IF gather mode.
+//
+// Stride-1 windows slide: A_{t0+1} = A_t0 + Y[t0+w] - Y[t0] (no twiddle: rate 0 only), restarted from
+// a direct sum every `seg` windows like kernels_slide.cuh; any other stride sums the window directly.
+// One CTA owns ALL delay columns of its windows (thread = CP column pairs, packed FP32), so the
+// argmax and the sum need no atomics: per 16 windows one barrier, fixed-order reductions, plain stores.
+#pragma once
+#include "common.cuh"
+
+namespace volks {
+
+constexpr int AI_MAXWARPS = 32;
+
+struct AllifArgs {
+  const float2 *Y;      // [nbl_chunk][nap][pitch] all-IF delay spectra, pair-interleaved rows
+  u64 *keys;            // canonical window keys
+  float *noise;         // canonical per-window noise = S1 / nfa
+  long long per_pair, offc, pair0;
+  int nap, nf, w, stride, nwin, seg, nseg, pitch;
+};
+
+// CP = column pairs per thread (nf / 2 / blockDim.x)
+template <int CP>
+__global__ void __launch_bounds__(1024) k_allif(AllifArgs a) {
+  __shared__ u64 kslot[16][AI_MAXWARPS];
+  __shared__ float sslot[16][AI_MAXWARPS];
+  const int nwarps = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int sg = blockIdx.x % a.nseg;
+  const long long pl = blockIdx.x / a.nseg;
+  const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch);
+  const size_t rowb = (size_t)a.pitch * 8u;
+  const long long c0 = (a.pair0 + pl) * a.per_pair + a.offc;
+  const int j0 = sg * a.seg, j1 = min(a.nwin, j0 + a.seg);
+  const bool slide = a.stride == 1;
+
+  f32x2 AX[CP], AY[CP];
+  auto direct = [&](int t0) {
+#pragma unroll
+    for (int i = 0; i < CP; ++i) { AX[i] = pk(0.f, 0.f); AY[i] = pk(0.f, 0.f); }
+    for (int t = 0; t < a.w; ++t) {
+#pragma unroll
+      for (int i = 0; i < CP; ++i) {
+        f32x2 x, y;
+        ldg2(ybase + (size_t)(t0 + t) * rowb + (size_t)(threadIdx.x + i * blockDim.x) * 16u, x, y);
+        AX[i] = add2(AX[i], x); AY[i] = add2(AY[i], y);
+      }
+    }
+  };
+  if (slide) direct(j0);
+
+  for (int jb = j0; jb < j1; jb += 16) {
+    const int nst = min(16, j1 - jb);
+    for (int b = 0; b < nst; ++b) {
+      const int j = jb + b;
+      if (!slide) direct(j * a.stride);
+      // power, thread-local best (power bits, then lowest column) and power sum
+      uint32_t pb = 0, db = 0xFFFFFFFFu;
+      float ps = 0.f;
+#pragma unroll
+      for (int i = 0; i < CP; ++i) {
+        const f32x2 pw = fma2(AY[i], AY[i], mul2(AX[i], AX[i]));
+        const uint32_t d0 = 2u * (uint32_t)(threadIdx.x + i * blockDim.x);
+        const uint32_t p0 = __float_as_uint(lo32(pw)), p1 = __float_as_uint(hi32(pw));
+        if (p0 > pb || (p0 == pb && d0 < db)) { pb = p0; db = d0; }
+        if (p1 > pb || (p1 == pb && d0 + 1 < db)) { pb = p1; db = d0 + 1; }
+        ps += lo32(pw) + hi32(pw);
+      }
+      const uint32_t km = __reduce_max_sync(0xffffffffu, pb);
+      const uint32_t dm = __reduce_min_sync(0xffffffffu, pb == km ? db : 0xFFFFFFFFu);
+#pragma unroll
+      for (int o = 16; o >= 1; o >>= 1) ps += __shfl_xor_sync(0xffffffffu, ps, o);
+      if (lane == 0) { kslot[b][warp] = make_key(__uint_as_float(km), dm); sslot[b][warp] = ps; }
+      // next window
+      if (slide && j + 1 < j1) {
+#pragma unroll
+        for (int i = 0; i < CP; ++i) {
+          f32x2 xi, yi, xo, yo;
+          const size_t co = (size_t)(threadIdx.x + i * blockDim.x) * 16u;
+          ldg2(ybase + (size_t)(j + a.w) * rowb + co, xi, yi);
+          ldg2(ybase + (size_t)j * rowb + co, xo, yo);
+          AX[i] = add2(AX[i], sub2(xi, xo)); AY[i] = add2(AY[i], sub2(yi, yo));
+        }
+      }
+    }
+    __syncthreads();
+    if (threadIdx.x < nst) {
+      u64 k = kslot[threadIdx.x][0];
+      float s = sslot[threadIdx.x][0];
+      for (int i = 1; i < nwarps; ++i) {
+        k = kslot[threadIdx.x][i] > k ? kslot[threadIdx.x][i] : k;
+        s += sslot[threadIdx.x][i];
+      }
+      a.keys[c0 + jb + threadIdx.x] = k;
+      a.noise[c0 + jb + threadIdx.x] = s / (float)a.nf;
+    }
+    __syncthreads();
+  }
+}
+
+}  // namespace volks

@@ -36,25 +36,40 @@ struct RowArgs {
   // read from AP t + shift[ifq][k] (zero beyond the slab); nullptr = no shift
   const int *shift;     // DEVICE [nif][nchan] or nullptr
   int nif;
+  // f2 all-IF mode (kernels_allif.cuh): a row is the whole band of one (bl, AP): nchan = nif_src * nchan_src
+  // frequency points gathered from vis[bl][n][t][j], m = n * nchan_src + j.  0 = off.
+  int allif_nif, allif_nchan;
 };
 
-// Source of one AP row: plain (base pointer) or dedispersed (per-channel row offsets).
+// Source of one AP row: plain (base pointer), dedispersed (per-channel row offsets), or the all-IF
+// band of one (bl, AP) gathered across IFs (with or without dedispersion).
 struct RowSrc {
-  const float2 *base;   // vis + row * nchan (plain) or vis + pair * nap * nchan (dedispersed)
-  const int *sh;        // shift row of this IF, or nullptr
-  int t, nap, nchan;
-  __device__ __forceinline__ RowSrc(const RowArgs &a, long long row) : nap(a.nap), nchan(a.nchan) {
-    if (a.shift) {
+  const float2 *base;   // vis + row * nchan (plain) or vis + pair * nap * nchan (dedispersed / all-IF: pair = bl * nif_src)
+  const int *sh;        // shift row of this IF (all-IF: the whole [nif][nchan] table), or nullptr
+  int t, nap, nchan, ai_nchan;
+  bool gather;
+  __device__ __forceinline__ RowSrc(const RowArgs &a, long long row) : nap(a.nap), nchan(a.nchan), ai_nchan(a.allif_nchan) {
+    if (a.allif_nif) {
+      const long long bl = row / a.nap;
+      t = (int)(row - bl * a.nap);
+      base = a.vis + bl * a.allif_nif * a.nap * (long long)a.allif_nchan;
+      sh = a.shift; gather = true;
+    } else if (a.shift) {
       const long long pair = row / a.nap;
       t = (int)(row - pair * a.nap);
       base = a.vis + pair * a.nap * (long long)a.nchan;
-      sh = a.shift + (pair % a.nif) * a.nchan;
-    } else { base = a.vis + row * (long long)a.nchan; sh = nullptr; t = 0; }
+      sh = a.shift + (pair % a.nif) * a.nchan; gather = true;
+    } else { base = a.vis + row * (long long)a.nchan; sh = nullptr; t = 0; gather = false; }
   }
   __device__ __forceinline__ float2 operator()(int k) const {
-    if (!sh) return __ldg(base + k);
-    const int ts = t + __ldg(sh + k);
-    return (ts >= 0 && ts < nap) ? __ldg(base + (long long)ts * nchan + k) : make_float2(0.f, 0.f);
+    if (!gather) return __ldg(base + k);
+    const int ts = t + (sh ? __ldg(sh + k) : 0);
+    if (ts < 0 || ts >= nap) return make_float2(0.f, 0.f);
+    if (ai_nchan) {
+      const int n = k / ai_nchan, j = k - n * ai_nchan;
+      return __ldg(base + ((long long)n * nap + ts) * ai_nchan + j);
+    }
+    return __ldg(base + (long long)ts * nchan + k);
   }
 };
 
@@ -441,6 +456,7 @@ __global__ void __launch_bounds__(256) k_col(ColArgs a) {
 // ------------------------------------------------------------------------------------------------
 struct Sched {   // the window schedule (device copy lives in the plan)
   int nwidths, nbl, nif, nap, nf, log2nf;
+  int allif;              // f2: one delay across all IFs (pairs = baselines; records carry ifq = -1)
   float snr_thresh;
   long long per_pair, nwin_total;
   int width[16], stride[16], nt[16];
@@ -455,8 +471,10 @@ struct WinStat { float power, snr; int rate_idx, delay_idx, q, j, t0; long long 
 // of PAPER.md:196) - the peak power normalised ACROSS the windows of its (pair, width) series:
 // z = (P1 - mean) * inv_std with zst[pair * nwidths + q] = (mean, 1/std) (inv_std = 0 when std = 0).
 // In that mode the z-score is what the record's `snr` field carries.
+// `noise` (f2): the per-window noise written by k_allif (mean of P over the delay axis) replaces the
+// Parseval sum of per-AP energies, which still decides whether the window is identically zero.
 __device__ __forceinline__ WinStat window_stat(const Sched &s, const u64 *keys, const float *E, long long c,
-                                               const double2 *zst = nullptr) {
+                                               const double2 *zst = nullptr, const float *noise = nullptr) {
   WinStat o;
   o.pair = c / s.per_pair;
   long long rem = c - o.pair * s.per_pair;
@@ -472,7 +490,8 @@ __device__ __forceinline__ WinStat window_stat(const Sched &s, const u64 *keys, 
   const float *e = E + o.pair * s.nap + o.t0;
   float es = 0.f;
   for (int t = 0; t < s.width[q]; ++t) es += e[t];
-  o.snr = es > 0.f ? sqrtf(o.power / es) : 0.f;
+  const float nz = noise ? noise[c] : es;
+  o.snr = (es > 0.f && nz > 0.f) ? sqrtf(o.power / nz) : 0.f;
   // an all-zero window (flagged data, the zero fill of dedispersion) has an identically zero plane:
   // P1 = 0 at (0, 0) by the tie rule.  The sliding sum would leave rounding residue of earlier samples
   // here, so the exact statement is made from the energy (es == 0 iff every sample is zero).
@@ -486,7 +505,8 @@ __device__ __forceinline__ WinStat window_stat(const Sched &s, const u64 *keys, 
 
 // f4: mean and 1/std (population) of the peak-power series of one (pair, width); one CTA per series,
 // double accumulation in a fixed order (deterministic).
-__global__ void __launch_bounds__(256) k_zstat(const Sched *sp, const u64 *keys, const float *E, double2 *zst) {
+__global__ void __launch_bounds__(256) k_zstat(const Sched *sp, const u64 *keys, const float *E, double2 *zst,
+                                               const float *noise) {
   __shared__ Sched s;
   __shared__ double sh1[256], sh2[256];
   if (threadIdx.x == 0) s = *sp;
@@ -496,7 +516,7 @@ __global__ void __launch_bounds__(256) k_zstat(const Sched *sp, const u64 *keys,
   const long long c0 = pair * s.per_pair + s.offc[q];
   double a = 0.0, b = 0.0;
   for (long long j = threadIdx.x; j < s.nwin[q]; j += 256) {
-    const double p = (double)window_stat(s, keys, E, c0 + j).power;
+    const double p = (double)window_stat(s, keys, E, c0 + j, nullptr, noise).power;
     a += p; b += p * p;
   }
   sh1[threadIdx.x] = a; sh2[threadIdx.x] = b;
@@ -519,7 +539,7 @@ constexpr int FIN_THREADS = 256, FIN_TILES = 8;   // 2048 windows per CTA
 
 __global__ void __launch_bounds__(FIN_THREADS) k_finalize(const Sched *sp, const u64 *keys, const float *E,
                                                           float4 *peaks, uint32_t *blockcount,
-                                                          const double2 *zst, float zth) {
+                                                          const double2 *zst, float zth, const float *noise) {
   __shared__ Sched s;
   __shared__ uint32_t wsum[FIN_THREADS / 32];
   if (threadIdx.x == 0) s = *sp;
@@ -529,7 +549,7 @@ __global__ void __launch_bounds__(FIN_THREADS) k_finalize(const Sched *sp, const
   for (int tile = 0; tile < FIN_TILES; ++tile) {
     const long long c = base + tile * FIN_THREADS + threadIdx.x;
     if (c < s.nwin_total) {
-      const WinStat o = window_stat(s, keys, E, c, zst);
+      const WinStat o = window_stat(s, keys, E, c, zst, noise);
       if (peaks) {
         const long long di = s.offd[o.q] + o.pair * s.nwin[o.q] + o.j;
         peaks[di] = make_float4(o.power, o.snr, __int_as_float(o.rate_idx), __int_as_float(o.delay_idx));
@@ -570,7 +590,7 @@ struct CandOut { int bl, ifq, wid, win, t0, rate_idx, delay_idx; float power, sn
 
 __global__ void __launch_bounds__(FIN_THREADS) k_scatter(const Sched *sp, const u64 *keys, const float *E,
                                                          const uint32_t *blockoff, CandOut *cands,
-                                                         uint32_t capacity, const double2 *zst, float zth) {
+                                                         uint32_t capacity, const double2 *zst, float zth, const float *noise) {
   __shared__ Sched s;
   __shared__ uint32_t wsum[FIN_THREADS / 32];
   __shared__ uint32_t running;
@@ -583,7 +603,7 @@ __global__ void __launch_bounds__(FIN_THREADS) k_scatter(const Sched *sp, const 
     WinStat o;
     bool flag = false;
     if (c < s.nwin_total) {
-      o = window_stat(s, keys, E, c, zst);
+      o = window_stat(s, keys, E, c, zst, noise);
       flag = o.snr > (zst ? zth : s.snr_thresh);
     }
     const uint32_t bal = __ballot_sync(0xffffffffu, flag);
@@ -595,7 +615,7 @@ __global__ void __launch_bounds__(FIN_THREADS) k_scatter(const Sched *sp, const 
       const uint32_t pos = before + __popc(bal & ((1u << lane) - 1u));
       if (pos < capacity) {
         CandOut r;
-        r.bl = (int)(o.pair / s.nif); r.ifq = (int)(o.pair % s.nif); r.wid = o.q; r.win = o.j; r.t0 = o.t0;
+        r.bl = (int)(o.pair / s.nif); r.ifq = s.allif ? -1 : (int)(o.pair % s.nif); r.wid = o.q; r.win = o.j; r.t0 = o.t0;
         r.rate_idx = o.rate_idx; r.delay_idx = o.delay_idx; r.power = o.power; r.snr = o.snr;
         cands[pos] = r;
       }

@@ -12,6 +12,7 @@
 #include "kernels_generic.cuh"
 #include "kernels_slide.cuh"
 #include "kernels_colfft.cuh"
+#include "kernels_allif.cuh"
 
 using namespace volks;
 
@@ -170,6 +171,8 @@ struct volks_plan {
   float2 *d_tables = nullptr;  // [nf] delay twiddles, then per width [nt] rate twiddles
   int nchan = 0, pitch = 0;
   int paired = 0;               // Y rows pair-interleaved (common.cuh ld_y)
+  int ai_nif = 0, ai_nchan = 0; // f2 all-IF plan: source nif / nchan (0 = ordinary per-IF plan)
+  size_t off_noise = 0;         // f2: per-window noise written by k_allif
   bool row_generic = false;     // VOLKS_PATH=generic: the shared-memory Stockham row kernel only
   int wid1 = -1;                // a width with w == 1 whose peaks the row kernel emits itself (or -1)
   long long npair = 0;
@@ -217,15 +220,32 @@ const char *volks_strerror(int code) {
   }
 }
 
-int volks_plan_create(const volks_params *p, volks_plan **out) {
+static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif, int ai_nchan);
+
+int volks_plan_create(const volks_params *p, volks_plan **out) { return plan_create_impl(p, out, 0, 0); }
+
+int volks_plan_create_allif(const volks_params *p, volks_plan **out) {
   if (!p || !out) return VOLKS_EINVAL;
   *out = nullptr;
+  if (p->nbl < 1 || p->nif < 1 || p->nchan < 1 || p->nwidths < 1 || p->nwidths > VOLKS_MAX_WIDTHS) return VOLKS_EINVAL;
+  if ((long long)p->nif * p->nchan > p->nf || p->nf < 64 || p->nf > 8192) return VOLKS_EINVAL;
+  int32_t ones[VOLKS_MAX_WIDTHS];
+  for (int q = 0; q < VOLKS_MAX_WIDTHS; ++q) ones[q] = 1;
+  volks_params b = *p;          // the band of one (bl, AP) as a single "IF" of nif * nchan points; no rate axis
+  b.nif = 1; b.nchan = p->nif * p->nchan; b.nt = ones;
+  return plan_create_impl(&b, out, p->nif, p->nchan);
+}
+
+static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif, int ai_nchan) {
+  if (!p || !out) return VOLKS_EINVAL;
+  *out = nullptr;
+  const bool allif = ai_nif > 0;
   if (p->nbl < 1 || p->nif < 1 || p->nap < 0 || p->nchan < 1) return VOLKS_EINVAL;
   if (p->nwidths < 1 || p->nwidths > VOLKS_MAX_WIDTHS || !p->width || !p->stride || !p->nt) return VOLKS_EINVAL;
   if (!is_pow2(p->nf) || p->nf < p->nchan || p->nf > (1 << 14)) return VOLKS_EINVAL;
   if (!(p->snr_thresh == p->snr_thresh)) return VOLKS_EINVAL;
   for (int q = 0; q < p->nwidths; ++q) {
-    if (p->width[q] < 1 || p->stride[q] < 1 || !is_pow2(p->nt[q]) || p->nt[q] < p->width[q]) return VOLKS_EINVAL;
+    if (p->width[q] < 1 || p->stride[q] < 1 || !is_pow2(p->nt[q]) || (!allif && p->nt[q] < p->width[q])) return VOLKS_EINVAL;
     if ((long long)p->nt[q] * p->nf > (1LL << 31)) return VOLKS_EINVAL;   // plane index must fit 32 bits
   }
   volks_plan *pl = new (std::nothrow) volks_plan();
@@ -236,6 +256,7 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
   s.log2nf = ilog2(p->nf); s.snr_thresh = p->snr_thresh;
   pl->nchan = p->nchan;
   pl->npair = (long long)p->nbl * p->nif;
+  pl->ai_nif = ai_nif; pl->ai_nchan = ai_nchan; s.allif = allif ? 1 : 0;
   long long per_pair = 0;
   size_t tw_total = (size_t)p->nf;
   const bool force_generic = env_is("VOLKS_PATH", "generic");
@@ -249,7 +270,8 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
     // sliding-sum path: stride 1, pad x2 in time, whole warps of delay columns, 32-bit row offsets
     w.slide = !force_generic && w.s == 1 && w.w >= 2 && w.nt == 2 * w.w && p->nf >= 64 &&
               ((long long)p->nap + SLIDE_PF + 2) * (p->nf + 64) * 8 < (1LL << 32);
-    w.colfft = !force_generic && !w.slide && w.nt >= 32 && w.nt <= 512 && p->nf >= 32 && w.nwin > 0;
+    if (allif) w.slide = false;
+    w.colfft = !allif && !force_generic && !w.slide && w.nt >= 32 && w.nt <= 512 && p->nf >= 32 && w.nwin > 0;
     w.cf_l1 = w.nt / 16;
     w.cf_nz = 1;
     while (w.cf_nz * 16 < w.w) w.cf_nz *= 2;
@@ -258,6 +280,7 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
                                         std::max<long long>(8, (long long)p->nbl * p->nif * (p->nf / 32) * w.nwin / 592));
     w.cf_nrange = (int)((w.nwin + w.cf_wpc - 1) / w.cf_wpc);
     w.seg = std::max((seg_req / w.nt) * w.nt, w.nt);
+    if (allif) w.seg = std::max(16, (seg_req / 16) * 16);
     w.nseg = w.nwin > 0 ? (int)((w.nwin + w.seg - 1) / w.seg) : 0;
     w.tw_off = tw_total;
     tw_total += (size_t)w.nt;
@@ -301,12 +324,13 @@ int volks_plan_create(const volks_params *p, volks_plan **out) {
   pl->off_E = off;    off = align_up(off + (size_t)std::max<long long>(pl->npair * p->nap, 1) * sizeof(float), 256);
   pl->off_cnt = off;  off = align_up(off + (size_t)std::max<long long>(pl->nfin_blocks, 1) * sizeof(uint32_t), 256);
   // + padding rows: the sliding kernel loads one row, and prefetches SLIDE_PF + 1 rows, past the last sample
+  pl->off_noise = off; off = align_up(off + (allif ? (size_t)std::max<long long>(s.nwin_total, 1) * sizeof(float) : 0), 256);
   pl->off_zst = off;  off = align_up(off + (size_t)std::max<long long>(pl->npair * p->nwidths, 1) * sizeof(double2), 256);
   pl->off_Y = off;    off = align_up(off + (size_t)pl->pairs_per_chunk * std::max<size_t>(y_pair, 8) + (size_t)(SLIDE_PF + 2) * pl->pitch * sizeof(float2), 256);
   pl->ws_bytes = off;
 
   int active = 0;
-  if (!force_generic)
+  if (!force_generic && !allif)
     for (int q = 0; q < p->nwidths && pl->wid1 < 0; ++q)
       if (pl->wp[q].w == 1 && pl->wp[q].nwin > 0) pl->wid1 = q;
   for (int q = 0; q < p->nwidths; ++q) active += (pl->wp[q].nwin > 0 && q != pl->wid1) ? 1 : 0;
@@ -367,9 +391,27 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
   return volks_fringe_search_dd(pl, d_vis, nullptr, d_workspace, d_peaks, d_cands, cand_capacity, d_ncand, cuda_stream);
 }
 
+static int run_search(const volks_plan *pl, const void *d_vis, const int32_t *d_shift, void *d_workspace,
+                      volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand,
+                      void *cuda_stream);
+
 int volks_fringe_search_dd(const volks_plan *pl, const void *d_vis, const int32_t *d_shift, void *d_workspace,
                            volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand,
                            void *cuda_stream) {
+  if (pl && pl->ai_nif) return VOLKS_EINVAL;     // an all-IF plan: use volks_allif_search
+  return run_search(pl, d_vis, d_shift, d_workspace, d_peaks, d_cands, cand_capacity, d_ncand, cuda_stream);
+}
+
+int volks_allif_search(const volks_plan *pl, const void *d_vis, const int32_t *d_shift, void *d_workspace,
+                       volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand,
+                       void *cuda_stream) {
+  if (!pl || !pl->ai_nif) return VOLKS_EINVAL;   // needs a plan from volks_plan_create_allif
+  return run_search(pl, d_vis, d_shift, d_workspace, d_peaks, d_cands, cand_capacity, d_ncand, cuda_stream);
+}
+
+static int run_search(const volks_plan *pl, const void *d_vis, const int32_t *d_shift, void *d_workspace,
+                      volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand,
+                      void *cuda_stream) {
   if (!pl || !d_vis || !d_workspace || !d_ncand || (!d_cands && cand_capacity > 0)) return VOLKS_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const Sched &s = pl->sched;
@@ -378,6 +420,7 @@ int volks_fringe_search_dd(const volks_plan *pl, const void *d_vis, const int32_
   float *E = (float *)(ws + pl->off_E);
   uint32_t *cnt = (uint32_t *)(ws + pl->off_cnt);
   float2 *Y = (float2 *)(ws + pl->off_Y);
+  const float *noise = pl->ai_nif ? (const float *)(ws + pl->off_noise) : nullptr;
   if (s.nwin_total == 0) {
     return cuda_ok(cudaMemsetAsync(d_ncand, 0, sizeof(uint32_t), st)) ? VOLKS_OK : VOLKS_ECUDA;
   }
@@ -390,7 +433,7 @@ int volks_fringe_search_dd(const volks_plan *pl, const void *d_vis, const int32_
     ra.vis = (const float2 *)d_vis; ra.Y = Y; ra.E = E; ra.twf = pl->d_tables;
     ra.row0 = pair0 * s.nap; ra.nrows = np * s.nap;
     ra.nchan = pl->nchan; ra.nf = s.nf; ra.tpr = pl->row_tpr; ra.rows_per_cta = pl->row_rows_per_cta; ra.pitch = pl->pitch; ra.paired = pl->paired;
-    ra.shift = d_shift; ra.nif = s.nif;
+    ra.shift = d_shift; ra.nif = s.nif; ra.allif_nif = pl->ai_nif; ra.allif_nchan = pl->ai_nchan;
     ra.keys1 = nullptr; ra.per_pair = s.per_pair; ra.nap = s.nap; ra.stride1 = 1; ra.nwin1 = 0;
     if (pl->wid1 >= 0) { ra.keys1 = keys + s.offc[pl->wid1]; ra.stride1 = s.stride[pl->wid1]; ra.nwin1 = (int)s.nwin[pl->wid1]; }
     const long long rblocks = (ra.nrows + ra.rows_per_cta - 1) / ra.rows_per_cta;
@@ -408,6 +451,20 @@ int volks_fringe_search_dd(const volks_plan *pl, const void *d_vis, const int32_
       ca.nap = s.nap; ca.nf = s.nf; ca.log2nf = s.log2nf; ca.w = w.w; ca.stride = w.s; ca.nt = w.nt;
       ca.log2m = w.log2m; ca.nwin = (int)w.nwin; ca.pitch = pl->pitch; ca.paired = pl->paired;
       ca.total = ((np * w.nwin) << w.log2m) * s.nf;
+      if (pl->ai_nif) {
+        AllifArgs aa;
+        aa.Y = Y; aa.keys = keys; aa.noise = (float *)(ws + pl->off_noise);
+        aa.per_pair = s.per_pair; aa.offc = s.offc[q]; aa.pair0 = pair0;
+        aa.nap = s.nap; aa.nf = s.nf; aa.w = w.w; aa.stride = w.s; aa.nwin = (int)w.nwin; aa.seg = w.seg;
+        aa.nseg = w.nseg; aa.pitch = pl->pitch;
+        const int thr = std::min(1024, s.nf / 2), cp = s.nf / 2 / thr;
+        const unsigned blocks = (unsigned)(np * w.nseg);
+        ProfScope ps(pl, st, VOLKS_K_ALLIF, q);
+        if (cp == 1) k_allif<1><<<blocks, thr, 0, st>>>(aa);
+        else if (cp == 2) k_allif<2><<<blocks, thr, 0, st>>>(aa);
+        else k_allif<4><<<blocks, thr, 0, st>>>(aa);
+        continue;
+      }
       if (w.slide) {
         SlideArgs sa;
         sa.Y = Y; sa.keys = keys; sa.twt = pl->d_tables + w.tw_off; sa.tw4 = (const float4 *)(pl->d_tables + w.tw4_off);
@@ -441,7 +498,7 @@ int volks_fringe_search_dd(const volks_plan *pl, const void *d_vis, const int32_
   }
   {
     ProfScope ps(pl, st, VOLKS_K_FINALIZE, -1);
-    k_finalize<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, (float4 *)d_peaks, cnt, nullptr, 0.f);
+    k_finalize<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, (float4 *)d_peaks, cnt, nullptr, 0.f, noise);
   }
   {
     ProfScope ps(pl, st, VOLKS_K_SCAN, -1);
@@ -449,7 +506,7 @@ int volks_fringe_search_dd(const volks_plan *pl, const void *d_vis, const int32_
   }
   {
     ProfScope ps(pl, st, VOLKS_K_SCATTER, -1);
-    k_scatter<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity, nullptr, 0.f);
+    k_scatter<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity, nullptr, 0.f, noise);
   }
   return cuda_ok(cudaGetLastError()) ? VOLKS_OK : VOLKS_ECUDA;
 }
@@ -465,10 +522,11 @@ int volks_zscore_select(const volks_plan *pl, void *d_workspace, float z_thresh,
   const float *E = (const float *)(ws + pl->off_E);
   uint32_t *cnt = (uint32_t *)(ws + pl->off_cnt);
   double2 *zst = (double2 *)(ws + pl->off_zst);
-  k_zstat<<<(unsigned)(pl->npair * s.nwidths), 256, 0, st>>>(pl->d_sched, keys, E, zst);
-  k_finalize<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, (float4 *)d_peaks, cnt, zst, z_thresh);
+  const float *noise = pl->ai_nif ? (const float *)(ws + pl->off_noise) : nullptr;
+  k_zstat<<<(unsigned)(pl->npair * s.nwidths), 256, 0, st>>>(pl->d_sched, keys, E, zst, noise);
+  k_finalize<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, (float4 *)d_peaks, cnt, zst, z_thresh, noise);
   k_scan<<<1, 1024, 0, st>>>(cnt, pl->nfin_blocks, d_ncand);
-  k_scatter<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity, zst, z_thresh);
+  k_scatter<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity, zst, z_thresh, noise);
   return cuda_ok(cudaGetLastError()) ? VOLKS_OK : VOLKS_ECUDA;
 }
 

@@ -301,3 +301,53 @@ def test_zscore_selection_matches_oracle(vb, oracle, cfg, over):
         if key(r) not in set(ek):
             assert abs(float(r["snr"]) - zth) <= 2 * tol
     plan.close()
+
+
+@pytest.mark.parametrize("shape", [
+    # nbl nif nap nchan widths strides nfa dm
+    (2, 4, 300, 32, [2, 8, 16], [1, 1, 1], 256, 0.0),      # k_row2, sliding windows, several segments? (seg 256)
+    (1, 8, 700, 64, [4, 32], [1, 1], 2048, 0.0),           # pad x4 like the paper (8 IF x 64 ch x 4), k_row3
+    (2, 2, 200, 100, [3, 10], [2, 5], 512, 0.0),           # ragged band (200 of 512), strides > 1: direct sums
+    (1, 4, 400, 32, [4, 16], [1, 1], 256, 300.0),          # dedispersed all-IF search
+    (1, 2, 120, 1024, [8], [1], 4096, 0.0),                # nfa = 4096: generic row kernel, 2 column pairs per thread
+])
+def test_allif_search_matches_oracle(vb, oracle, shape):
+    """f2: one delay across all IFs (Eq. 1) vs oracle.allif_search on the same inputs."""
+    nbl, nif, nap, nchan, widths, strides, nfa, dm = shape
+    g = torch.Generator().manual_seed(nap + nchan)
+    vis = torch.view_as_complex(torch.randn((nbl, nif, nap, nchan, 2), generator=g) * 0.7071)
+    m = torch.arange(nif * nchan, dtype=torch.float64).reshape(nif, 1, nchan)
+    vis[0, :, nap // 3: nap // 3 + 12] += torch.polar(torch.full((nif, 1, nchan), 0.4, dtype=torch.float64),
+                                                      2 * np.pi * 0.0137 * m).to(torch.complex64)   # one delay, all IFs
+    vis[-1, :, nap // 2: nap // 2 + 20] = 0                                                           # flagged span
+    sh = None
+    src = vis.numpy()
+    if dm:
+        f = 1400.0 + 16.0 * np.arange(nif)[:, None] + (16.0 / nchan) * np.arange(nchan)[None, :]
+        sh = vb.dm_shifts(dm, f, f.max(), 1e-3)
+        src = oracle.dedisperse(src, sh)
+    thresh = 4.0
+    cands, n, peaks = vb.allif_search(vis.cuda(), widths, strides, nfa, thresh, want_peaks=True, shifts=sh)
+    ora = oracle.allif_search(src, widths, strides, nfa)
+    nw = [workloads.gen.nwin(nap, w, s) for w, s in zip(widths, strides)]
+    pk = peaks[dense_index(nbl, 1, nw)]
+    assert np.all(pk["rate_idx"] == 0)
+    band = oracle.allif_band(src)
+
+    def plane_power(i, idx):       # oracle power of one delay bin of canonical window i
+        per = sum(nw)
+        b, r = divmod(i, per)
+        q = 0
+        while r >= nw[q]:
+            r -= nw[q]; q += 1
+        a = np.fft.fft(band[b, r * strides[q]: r * strides[q] + widths[q]].astype(np.complex128).sum(axis=0), nfa)[idx]
+        return float(abs(a) ** 2)
+    check_peaks(pk, ora, nfa, plane_power)
+    exp = np.nonzero(ora["snr"] > thresh)[0]
+    marg = np.abs(ora["snr"] - thresh) <= 1e-4 * thresh
+    assert abs(n - len(exp)) <= int(marg.sum()) and n >= 1
+    assert np.all(cands["ifq"] == -1) and np.all(cands["rate_idx"] == 0)
+    key = [(int(c["bl"]), int(c["wid"]), int(c["win"])) for c in cands]
+    assert key == sorted(key)
+    hit = [c for c in cands if c["bl"] == 0 and nap // 3 - 16 <= c["t0"] <= nap // 3 + 12]
+    assert hit and all(abs(int(c["delay_idx"]) - round(0.0137 * nfa)) <= 1 for c in hit if c["snr"] > 8)
