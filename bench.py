@@ -44,6 +44,8 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--peaks", action="store_true", help="also write the dense per-window peak array")
+    ap.add_argument("--allif", action="store_true",
+                    help="time f2 instead: VOLKS2's all-IF one-delay search (Eq. 1) on the config's slab, band padded x2")
     ap.add_argument("--dm", type=float, default=0.0,
                     help="dedisperse (f1, fused into the slab load) with this DM [pc cm^-3]; 0 = plain search")
     return ap.parse_args()
@@ -194,7 +196,7 @@ def aggregate_value(world, units_per_rank, ms_step):
     return world * units_per_rank / (ms_step * 1e-3)
 
 
-KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6: "slide", 7: "colfft"}
+KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6: "slide", 7: "colfft", 8: "allif"}
 
 
 def run_volks(args):
@@ -216,7 +218,11 @@ def run_volks(args):
     # GPU, so --gpus N runs N replicas, each the full config with its own seed)
     vis, c, _ = workloads.generate(args.config, device=dev, seed=workloads.config(args.config)["seed"] + 17 * rank)
     nbl, nif, nap, nchan = vis.shape
-    plan = vk.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"])
+    if args.allif:
+        nfa = workloads.gen.next_pow2(2 * nif * nchan)
+        plan = vk.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], None, nfa, c["snr_thresh"], allif=True)
+    else:
+        plan = vk.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"])
     cap = 1 << 20
     ws = torch.empty(plan.workspace_bytes, dtype=torch.uint8, device=dev)
     cands = torch.empty(cap * vk.CAND_DTYPE.itemsize, dtype=torch.uint8, device=dev)
@@ -292,6 +298,23 @@ def run_volks(args):
     else:
         exec_flops = dom_flops
     clocks = sampler.summary()
+    if args.allif:
+        # f2 is bandwidth work: the row pass reads the slab once and writes the all-IF delay spectra, every
+        # width's k_allif reads them once.  Roofline of the dominant kernel against measured HBM bandwidth.
+        peaks_json = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        hbm = json.load(open(peaks_json))["hbm_gbs"] if os.path.exists(peaks_json) else 6650.0
+        ybytes = nbl * nap * (plan.nf + 16) * 8.0
+        dom_bytes = (ybytes + nvis * 8.0 if dom[0] == 1 else ybytes) / nlaunch[dom]
+        gbs = dom_bytes / (dom_ms_avg * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": "%s[w=%s]" % (KIND_NAMES[dom[0]], c["widths"][dom[1]] if dom[1] >= 0 else "all"),
+                    "achieved": gbs, "peak": hbm, "unit": "GB/s", "frac": gbs / hbm, "traffic": None,
+                    "launch_ms": dom_ms_avg, "share_of_step": share[dom] / step_sum,
+                    "peak_kind": "measured (MEASURED_PEAKS.json hbm_gbs)" if os.path.exists(peaks_json) else "fallback 6650 GB/s",
+                    "bytes_kind": "algorithmic: the chunk's all-IF delay spectra read once (row pass: + the slab read once)",
+                    "kernel_ms": {"%s[%d]" % (KIND_NAMES[k[0]], k[1]): round(v, 4) for k, v in sorted(share.items())}}
+        return dict(vk=vk, plan=plan, vis=vis, c=c, ws=ws, cands=cands, ncand=ncand, peaks=peaks, stream=stream,
+                    dev=dev, rank=rank, world=world, dist=dist, ms_step=ms_step, value=value, nwin=nwin, nvis=nvis,
+                    n_found=n_found, roofline=roofline, clocks=clocks, cap=cap, shift=shift)
     peak_tf = SM_COUNT * FP32_LANES_PER_SM * 2 * (clocks["sm_max_mhz"] or 1965) * 1e6 / 1e12
     achieved_tf = dom_flops / (dom_ms_avg * 1e-3) / 1e12
     roofline = {
@@ -378,7 +401,8 @@ def main():
             "config": {"workload": workload_name(c), "snr_thresh": c["snr_thresh"],
                        "l2": "input slab (%.2f GB) larger than L2, no flush needed" % (R["nvis"] * 8 / 1e9)
                        if R["nvis"] * 8 > 126e6 else "input smaller than L2 (latency-bound config, report only)",
-                       "replicas": R["world"], "dense_peaks": bool(args.peaks), "dm": args.dm},
+                       "replicas": R["world"], "dense_peaks": bool(args.peaks), "dm": args.dm,
+                       "search": "f2 all-IF one-delay search (Eq. 1), nfa %d" % R["plan"].nf if args.allif else "2-D per-IF fringe search"},
             "visibilities_per_s": R["world"] * R["nvis"] / (R["ms_step"] * 1e-3),
             "windows": R["nwin"], "candidates": R["n_found"],
             "clocks": R["clocks"], "e2e": e2e, "gpu_launches": R["plan"].launches * args.steps,

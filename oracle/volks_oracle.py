@@ -13,7 +13,8 @@ Parity status: every function here is pinned by tests/test_oracle_pins.py (close
 DESIGN.md) except `window_match`, which is pinned only by hand-built constructions and a second
 brute-force statement of the same rule (the paper gives no worked example) - see DESIGN.md.
 `dedisperse` / `dm_shifts` (step 4) are pinned by test_dedispersion_pins and
-test_dedispersed_pulse_closed_form.
+test_dedispersed_pulse_closed_form; `allif_search` (Eq. 1) by test_allif_search_pins; `zscore_candidates`
+by test_zscore_selection_pins; `baseline_match` by constructions only (parity unpinned beyond those).
 """
 import ctypes
 import os

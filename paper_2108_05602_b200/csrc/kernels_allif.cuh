@@ -6,8 +6,9 @@
 //             delay axis).  Y[t][d] is the zero-padded FFT of the AP's whole band (all IFs in
 //             frequency order) written by the row kernels in their all-IF gather mode.
 //
-// Stride-1 windows slide: A_{t0+1} = A_t0 + Y[t0+w] - Y[t0] (no twiddle: rate 0 only), restarted from
-// a direct sum every `seg` windows like kernels_slide.cuh; any other stride sums the window directly.
+// Overlapping windows slide: A_{j+1} = A_j + sum_{t<s} (Y[t0+w+t] - Y[t0+t]) (no twiddle: rate 0 only;
+// 2 s row reads per window instead of w), restarted from a direct sum every `seg` windows like
+// kernels_slide.cuh; windows with 2 s > w are summed directly.
 // One CTA owns ALL delay columns of its windows (thread = CP column pairs, packed FP32), so the
 // argmax and the sum need no atomics: per 16 windows one barrier, fixed-order reductions, plain stores.
 #pragma once
@@ -37,7 +38,7 @@ __global__ void __launch_bounds__(1024) k_allif(AllifArgs a) {
   const size_t rowb = (size_t)a.pitch * 8u;
   const long long c0 = (a.pair0 + pl) * a.per_pair + a.offc;
   const int j0 = sg * a.seg, j1 = min(a.nwin, j0 + a.seg);
-  const bool slide = a.stride == 1;
+  const bool slide = 2 * a.stride <= a.w;
 
   f32x2 AX[CP], AY[CP];
   auto direct = [&](int t0) {
@@ -52,7 +53,7 @@ __global__ void __launch_bounds__(1024) k_allif(AllifArgs a) {
       }
     }
   };
-  if (slide) direct(j0);
+  if (slide) direct(j0 * a.stride);
 
   for (int jb = j0; jb < j1; jb += 16) {
     const int nst = min(16, j1 - jb);
@@ -78,13 +79,16 @@ __global__ void __launch_bounds__(1024) k_allif(AllifArgs a) {
       if (lane == 0) { kslot[b][warp] = make_key(__uint_as_float(km), dm); sslot[b][warp] = ps; }
       // next window
       if (slide && j + 1 < j1) {
+        const int t0 = j * a.stride;
+        for (int t = 0; t < a.stride; ++t) {
 #pragma unroll
-        for (int i = 0; i < CP; ++i) {
-          f32x2 xi, yi, xo, yo;
-          const size_t co = (size_t)(threadIdx.x + i * blockDim.x) * 16u;
-          ldg2(ybase + (size_t)(j + a.w) * rowb + co, xi, yi);
-          ldg2(ybase + (size_t)j * rowb + co, xo, yo);
-          AX[i] = add2(AX[i], sub2(xi, xo)); AY[i] = add2(AY[i], sub2(yi, yo));
+          for (int i = 0; i < CP; ++i) {
+            f32x2 xi, yi, xo, yo;
+            const size_t co = (size_t)(threadIdx.x + i * blockDim.x) * 16u;
+            ldg2(ybase + (size_t)(t0 + t + a.w) * rowb + co, xi, yi);
+            ldg2(ybase + (size_t)(t0 + t) * rowb + co, xo, yo);
+            AX[i] = add2(AX[i], sub2(xi, xo)); AY[i] = add2(AY[i], sub2(yi, yo));
+          }
         }
       }
     }

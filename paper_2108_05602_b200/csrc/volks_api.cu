@@ -280,7 +280,8 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
                                         std::max<long long>(8, (long long)p->nbl * p->nif * (p->nf / 32) * w.nwin / 592));
     w.cf_nrange = (int)((w.nwin + w.cf_wpc - 1) / w.cf_wpc);
     w.seg = std::max((seg_req / w.nt) * w.nt, w.nt);
-    if (allif) w.seg = std::max(16, (seg_req / 16) * 16);
+    // f2: one CTA per (baseline, segment): segments short enough to fill 148 SMs x 2, at most seg_req windows
+    if (allif) w.seg = (int)std::max<long long>(16, std::min<long long>((seg_req / 16) * 16, (w.nwin * p->nbl / 296 + 15) / 16 * 16));
     w.nseg = w.nwin > 0 ? (int)((w.nwin + w.seg - 1) / w.seg) : 0;
     w.tw_off = tw_total;
     tw_total += (size_t)w.nt;

@@ -307,7 +307,8 @@ def test_zscore_selection_matches_oracle(vb, oracle, cfg, over):
     # nbl nif nap nchan widths strides nfa dm
     (2, 4, 300, 32, [2, 8, 16], [1, 1, 1], 256, 0.0),      # k_row2, sliding windows, several segments? (seg 256)
     (1, 8, 700, 64, [4, 32], [1, 1], 2048, 0.0),           # pad x4 like the paper (8 IF x 64 ch x 4), k_row3
-    (2, 2, 200, 100, [3, 10], [2, 5], 512, 0.0),           # ragged band (200 of 512), strides > 1: direct sums
+    (2, 2, 200, 100, [3, 10], [2, 5], 512, 0.0),           # ragged band (200 of 512): direct sums (2s > w) and stride-5 sliding
+    (1, 2, 900, 32, [64, 16], [16, 4], 128, 0.0),          # config-4-like strides w/4: sliding by blocks over several segments
     (1, 4, 400, 32, [4, 16], [1, 1], 256, 300.0),          # dedispersed all-IF search
     (1, 2, 120, 1024, [8], [1], 4096, 0.0),                # nfa = 4096: generic row kernel, 2 column pairs per thread
 ])
