@@ -347,10 +347,12 @@ def run_e2e(R, steps):
     d_vis = R["vis"]
     d2h = 0
 
+    stage = torch.empty(2 * plan.stage_bytes, dtype=torch.uint8, device=dev)
+
     def step():
         nonlocal d2h
-        d_vis.copy_(h_vis, non_blocking=True)
-        plan.fringe_search(d_vis, R["ws"], R["cands"], R["ncand"], R["peaks"], stream, shift=R["shift"])
+        # the public host-slab call: chunked pinned-host -> device copies overlapped with the kernels
+        plan.search_host(h_vis, stage, R["ws"], R["cands"], R["ncand"], R["peaks"], stream, shift=R["shift"])
         h_n.copy_(R["ncand"], non_blocking=True)
         stream.synchronize()
         n = min(int(h_n.item()), R["cap"]) * vk.CAND_DTYPE.itemsize

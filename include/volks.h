@@ -136,6 +136,19 @@ int volks_allif_search(const volks_plan *plan, const void *d_vis, const int32_t 
                        volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity,
                        uint32_t *d_ncand, void *cuda_stream);
 
+/* The same searches on a HOST slab (pinned memory recommended), for slabs that are produced on the host
+ * or do not fit the device: the slab is copied chunk by chunk (the (bl, ifq) pairs - baselines for an
+ * all-IF plan - of one internal chunk at a time) into the two halves of `d_stage` on an internal copy
+ * stream, each copy overlapped with the kernels of the previous chunk; the result is identical to the
+ * device-slab calls.  Works with both plan kinds (volks_plan_create / volks_plan_create_allif).
+ *   h_vis    HOST cf32[nbl][nif][nap][nchan]; must stay valid until `cuda_stream` has run the call
+ *   d_stage  DEVICE scratch of 2 * stage_bytes (volks_plan_query_host), 256-byte aligned
+ * Other arguments as volks_fringe_search_dd. */
+int volks_plan_query_host(const volks_plan *plan, size_t *stage_bytes);
+int volks_search_host(const volks_plan *plan, const void *h_vis, void *d_stage, const int32_t *d_shift,
+                      void *d_workspace, volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity,
+                      uint32_t *d_ncand, void *cuda_stream);
+
 /* Across-window normalised power (SURVEY 8(f) f4 - the other reading of PAPER.md:196 "for the time
  * segments series of given window size, a single pulse is selected if its normalized power exceeds
  * the threshold, which is set to 3").  A second pass over the results the LAST volks_fringe_search[_dd]

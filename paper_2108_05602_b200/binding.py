@@ -18,6 +18,7 @@ EXPORTS = (
     "volks_window_match", "volks_bin_to_physical", "volks_plan_launch_count", "volks_strerror",
     "volks_version", "volks_plan_profile", "volks_plan_profile_read", "volks_fringe_search_dd", "volks_dm_shifts",
     "volks_baseline_match", "volks_zscore_select", "volks_plan_create_allif", "volks_allif_search",
+    "volks_plan_query_host", "volks_search_host",
 )
 
 
@@ -54,6 +55,8 @@ def lib():
         L.volks_plan_create.argtypes = [ctypes.POINTER(volks_params), ctypes.POINTER(ctypes.c_void_p)]
         L.volks_plan_create_allif.argtypes = [ctypes.POINTER(volks_params), ctypes.POINTER(ctypes.c_void_p)]
         L.volks_allif_search.argtypes = [ctypes.c_void_p] * 6 + [ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
+        L.volks_plan_query_host.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_size_t)]
+        L.volks_search_host.argtypes = [ctypes.c_void_p] * 7 + [ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
         L.volks_plan_destroy.argtypes = [ctypes.c_void_p]
         L.volks_plan_query.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_size_t),
                                        ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
@@ -145,6 +148,26 @@ class Plan:
             self._h, vis.data_ptr(), shift.data_ptr() if shift is not None else None, workspace.data_ptr(),
             peaks.data_ptr() if peaks is not None else None, cands.data_ptr() if cap else None, cap,
             ncand.data_ptr(), st))
+
+    @property
+    def stage_bytes(self):
+        """volks_plan_query_host: bytes of ONE half of the staging buffer of search_host."""
+        n = ctypes.c_size_t()
+        _check(lib().volks_plan_query_host(self._h, ctypes.byref(n)))
+        return n.value
+
+    def search_host(self, h_vis, stage, workspace, cands, ncand, peaks=None, stream=None, shift=None):
+        """volks_search_host: h_vis is a HOST complex64 tensor (pinned recommended), `stage` a CUDA uint8
+        tensor of >= 2 * stage_bytes; copies overlap the kernels chunk by chunk.  Asynchronous."""
+        assert (not h_vis.is_cuda) and h_vis.dtype == torch.complex64 and h_vis.is_contiguous()
+        assert tuple(h_vis.shape) == self.shape
+        assert stage.is_cuda and stage.numel() * stage.element_size() >= 2 * self.stage_bytes
+        cap = cands.numel() * cands.element_size() // CAND_DTYPE.itemsize
+        st = (stream or torch.cuda.current_stream(stage.device)).cuda_stream
+        _check(lib().volks_search_host(
+            self._h, h_vis.data_ptr(), stage.data_ptr(), shift.data_ptr() if shift is not None else None,
+            workspace.data_ptr(), peaks.data_ptr() if peaks is not None else None,
+            cands.data_ptr() if cap else None, cap, ncand.data_ptr(), st))
 
     def zscore_select(self, workspace, z_thresh, cands, ncand, peaks=None, stream=None):
         """volks_zscore_select: across-window normalised selection on the last search's workspace."""

@@ -171,6 +171,8 @@ struct volks_plan {
   float2 *d_tables = nullptr;  // [nf] delay twiddles, then per width [nt] rate twiddles
   int nchan = 0, pitch = 0;
   int paired = 0;               // Y rows pair-interleaved (common.cuh ld_y)
+  mutable cudaStream_t copy_stream = nullptr;      // volks_search_host: H2D copies of the slab chunks
+  mutable cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
   int ai_nif = 0, ai_nchan = 0; // f2 all-IF plan: source nif / nchan (0 = ordinary per-IF plan)
   size_t off_noise = 0;         // f2: per-window noise written by k_allif
   bool row_generic = false;     // VOLKS_PATH=generic: the shared-memory Stockham row kernel only
@@ -312,7 +314,8 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   pl->paired = p->nf >= 2 ? 1 : 0;
   pl->row_generic = force_generic;
   const size_t y_pair = (size_t)p->nap * pl->pitch * sizeof(float2);
-  const size_t budget = (size_t)4 << 30;
+  // VOLKS_CHUNK_MB: bytes of delay spectra per chunk of pairs (default 4 GiB; tests use small chunks)
+  const size_t budget = (size_t)std::max(1, env_int("VOLKS_CHUNK_MB", 4096)) << 20;
   long long ppc = y_pair ? (long long)std::max<size_t>(1, budget / std::max<size_t>(y_pair, 1)) : pl->npair;
   ppc = std::min(ppc, pl->npair);
   pl->nchunks = (pl->npair + ppc - 1) / ppc;
@@ -373,6 +376,8 @@ int volks_plan_destroy(volks_plan *pl) {
   if (pl->d_tables) cudaFree(pl->d_tables);
   if (pl->d_sched) cudaFree(pl->d_sched);
   for (cudaEvent_t e : pl->prof_ev) cudaEventDestroy(e);
+  for (int k = 0; k < 2; ++k) { if (pl->ev_copied[k]) cudaEventDestroy(pl->ev_copied[k]); if (pl->ev_free[k]) cudaEventDestroy(pl->ev_free[k]); }
+  if (pl->copy_stream) cudaStreamDestroy(pl->copy_stream);
   delete pl;
   return VOLKS_OK;
 }
@@ -392,7 +397,7 @@ int volks_fringe_search(const volks_plan *pl, const void *d_vis, void *d_workspa
   return volks_fringe_search_dd(pl, d_vis, nullptr, d_workspace, d_peaks, d_cands, cand_capacity, d_ncand, cuda_stream);
 }
 
-static int run_search(const volks_plan *pl, const void *d_vis, const int32_t *d_shift, void *d_workspace,
+static int run_search(const volks_plan *pl, const void *vis, void *d_stage, const int32_t *d_shift, void *d_workspace,
                       volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand,
                       void *cuda_stream);
 
@@ -400,20 +405,47 @@ int volks_fringe_search_dd(const volks_plan *pl, const void *d_vis, const int32_
                            volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand,
                            void *cuda_stream) {
   if (pl && pl->ai_nif) return VOLKS_EINVAL;     // an all-IF plan: use volks_allif_search
-  return run_search(pl, d_vis, d_shift, d_workspace, d_peaks, d_cands, cand_capacity, d_ncand, cuda_stream);
+  return run_search(pl, d_vis, nullptr, d_shift, d_workspace, d_peaks, d_cands, cand_capacity, d_ncand, cuda_stream);
 }
 
 int volks_allif_search(const volks_plan *pl, const void *d_vis, const int32_t *d_shift, void *d_workspace,
                        volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand,
                        void *cuda_stream) {
   if (!pl || !pl->ai_nif) return VOLKS_EINVAL;   // needs a plan from volks_plan_create_allif
-  return run_search(pl, d_vis, d_shift, d_workspace, d_peaks, d_cands, cand_capacity, d_ncand, cuda_stream);
+  return run_search(pl, d_vis, nullptr, d_shift, d_workspace, d_peaks, d_cands, cand_capacity, d_ncand, cuda_stream);
 }
 
-static int run_search(const volks_plan *pl, const void *d_vis, const int32_t *d_shift, void *d_workspace,
+int volks_plan_query_host(const volks_plan *pl, size_t *stage_bytes) {
+  if (!pl || !stage_bytes) return VOLKS_EINVAL;
+  *stage_bytes = align_up((size_t)pl->pairs_per_chunk * pl->sched.nap * pl->nchan * sizeof(float2), 256);
+  return VOLKS_OK;
+}
+
+int volks_search_host(const volks_plan *pl, const void *h_vis, void *d_stage, const int32_t *d_shift,
+                      void *d_workspace, volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity,
+                      uint32_t *d_ncand, void *cuda_stream) {
+  if (!pl || !h_vis || !d_stage) return VOLKS_EINVAL;
+  return run_search(pl, h_vis, d_stage, d_shift, d_workspace, d_peaks, d_cands, cand_capacity, d_ncand, cuda_stream);
+}
+
+// vis: DEVICE slab (d_stage == nullptr) or HOST slab copied chunk by chunk through the two halves of
+// d_stage on the plan's copy stream, overlapped with the kernels of the previous chunk.
+static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, const int32_t *d_shift, void *d_workspace,
                       volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand,
                       void *cuda_stream) {
   if (!pl || !d_vis || !d_workspace || !d_ncand || (!d_cands && cand_capacity > 0)) return VOLKS_EINVAL;
+  const size_t pair_elems = (size_t)pl->sched.nap * pl->nchan;   // visibilities of one pair (all-IF: one baseline)
+  size_t stage_bytes = 0;
+  if (d_stage) {
+    volks_plan_query_host(pl, &stage_bytes);
+    if (!pl->copy_stream) {
+      if (!cuda_ok(cudaStreamCreateWithFlags(&pl->copy_stream, cudaStreamNonBlocking))) return VOLKS_ECUDA;
+      for (int k = 0; k < 2; ++k) {
+        if (!cuda_ok(cudaEventCreateWithFlags(&pl->ev_copied[k], cudaEventDisableTiming)) ||
+            !cuda_ok(cudaEventCreateWithFlags(&pl->ev_free[k], cudaEventDisableTiming))) return VOLKS_ECUDA;
+      }
+    }
+  }
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const Sched &s = pl->sched;
   char *ws = (char *)d_workspace;
@@ -431,7 +463,20 @@ static int run_search(const volks_plan *pl, const void *d_vis, const int32_t *d_
     const long long pair0 = ch * pl->pairs_per_chunk;
     const long long np = std::min(pl->pairs_per_chunk, pl->npair - pair0);
     RowArgs ra;
-    ra.vis = (const float2 *)d_vis; ra.Y = Y; ra.E = E; ra.twf = pl->d_tables;
+    ra.vis = (const float2 *)d_vis;
+    if (d_stage) {
+      const int k = (int)(ch & 1);
+      char *dst = (char *)d_stage + (size_t)k * stage_bytes;
+      // the stage half is free once the row kernel that last read it (chunk ch-2, or the previous call's)
+      // is done: ev_free[k] is recorded right after that kernel; a never-recorded event does not block
+      if (!cuda_ok(cudaStreamWaitEvent(pl->copy_stream, pl->ev_free[k], 0))) return VOLKS_ECUDA;
+      if (!cuda_ok(cudaMemcpyAsync(dst, (const char *)d_vis + (size_t)pair0 * pair_elems * sizeof(float2),
+                                   (size_t)np * pair_elems * sizeof(float2), cudaMemcpyHostToDevice, pl->copy_stream)) ||
+          !cuda_ok(cudaEventRecord(pl->ev_copied[k], pl->copy_stream)) ||
+          !cuda_ok(cudaStreamWaitEvent(st, pl->ev_copied[k], 0))) return VOLKS_ECUDA;
+      ra.vis = (const float2 *)dst - (size_t)pair0 * pair_elems;   // kernels index by absolute pair
+    }
+    ra.Y = Y; ra.E = E; ra.twf = pl->d_tables;
     ra.row0 = pair0 * s.nap; ra.nrows = np * s.nap;
     ra.nchan = pl->nchan; ra.nf = s.nf; ra.tpr = pl->row_tpr; ra.rows_per_cta = pl->row_rows_per_cta; ra.pitch = pl->pitch; ra.paired = pl->paired;
     ra.shift = d_shift; ra.nif = s.nif; ra.allif_nif = pl->ai_nif; ra.allif_nchan = pl->ai_nchan;
@@ -442,6 +487,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, const int32_t *d_
       ProfScope ps(pl, st, VOLKS_K_ROW, -1);
       if (pl->row_generic || !launch_row2(ra, st))
         k_row_fft<<<(unsigned)rblocks, ra.tpr * ra.rows_per_cta, pl->row_smem, st>>>(ra);
+      if (d_stage && !cuda_ok(cudaEventRecord(pl->ev_free[ch & 1], st))) return VOLKS_ECUDA;
     }
     for (int q = 0; q < s.nwidths; ++q) {
       const WidthPlan &w = pl->wp[q];

@@ -352,3 +352,38 @@ def test_allif_search_matches_oracle(vb, oracle, shape):
     assert key == sorted(key)
     hit = [c for c in cands if c["bl"] == 0 and nap // 3 - 16 <= c["t0"] <= nap // 3 + 12]
     assert hit and all(abs(int(c["delay_idx"]) - round(0.0137 * nfa)) <= 1 for c in hit if c["snr"] > 8)
+
+
+@pytest.mark.parametrize("allif", [False, True])
+def test_host_slab_search_is_identical(vb, allif, monkeypatch):
+    """volks_search_host (slab in pinned host memory, chunked copies overlapped with the kernels) must
+    give bit-identical candidates and peaks to the device-slab call; small chunks force several
+    copy/compute rounds through both stage halves, twice in a row (stage reuse across calls)."""
+    monkeypatch.setenv("VOLKS_CHUNK_MB", "1")
+    vis, c, _ = workloads.generate(2, nbl=3, nif=3, nap=600, npulses=3)
+    nbl, nif, nap, nchan = vis.shape
+    if allif:
+        plan = vb.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], None, 1024, 4.0, allif=True)
+    else:
+        plan = vb.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], c["nts"], c["nf"], 4.0)
+    dev = torch.device("cuda")
+    ws = torch.empty(plan.workspace_bytes, dtype=torch.uint8, device=dev)
+    cap = 1 << 16
+    mk = lambda: (torch.empty(cap * vb.CAND_DTYPE.itemsize, dtype=torch.uint8, device=dev),
+                  torch.zeros(1, dtype=torch.int32, device=dev),
+                  torch.empty(plan.nwin_total * vb.PEAK_DTYPE.itemsize, dtype=torch.uint8, device=dev))
+    c0, n0, p0 = mk()
+    plan.fringe_search(vis.cuda(), ws, c0, n0, p0)
+    torch.cuda.synchronize()
+    ref = (int(n0.item()), c0.cpu().numpy()[: int(n0.item()) * 36].tobytes(), p0.cpu().numpy().tobytes())
+    assert ref[0] >= 1
+    h = vis.pin_memory()
+    stage = torch.empty(2 * plan.stage_bytes, dtype=torch.uint8, device=dev)
+    assert plan.stage_bytes < h.numel() * 8 / 2          # several chunks
+    for _ in range(2):
+        c1, n1, p1 = mk()
+        plan.search_host(h, stage, ws, c1, n1, p1)
+        torch.cuda.synchronize()
+        assert int(n1.item()) == ref[0]
+        assert c1.cpu().numpy()[: ref[0] * 36].tobytes() == ref[1] and p1.cpu().numpy().tobytes() == ref[2]
+    plan.close()
