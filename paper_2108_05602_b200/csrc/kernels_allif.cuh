@@ -24,6 +24,7 @@ struct AllifArgs {
   float *noise;         // canonical per-window noise = S1 / nfa
   long long per_pair, offc, pair0;
   int nap, nf, w, stride, nwin, seg, nseg, pitch;
+  int psub, nfb;        // nf = psub * nfb: column c of a row is sub-row rho = c / nfb, d' = c % nfb, delay d = psub d' + rho
 };
 
 // CP = column pairs per thread (nf / 2 / blockDim.x)
@@ -66,10 +67,12 @@ __global__ void __launch_bounds__(1024) k_allif(AllifArgs a) {
 #pragma unroll
       for (int i = 0; i < CP; ++i) {
         const f32x2 pw = fma2(AY[i], AY[i], mul2(AX[i], AX[i]));
-        const uint32_t d0 = 2u * (uint32_t)(threadIdx.x + i * blockDim.x);
+        const uint32_t c0l = 2u * (uint32_t)(threadIdx.x + i * blockDim.x);       // linear column of the pair
+        const uint32_t rho = c0l / (uint32_t)a.nfb, dp = c0l - rho * (uint32_t)a.nfb;
+        const uint32_t d0 = dp * (uint32_t)a.psub + rho, d1 = d0 + (uint32_t)a.psub;  // true delay bins (d' and d'+1)
         const uint32_t p0 = __float_as_uint(lo32(pw)), p1 = __float_as_uint(hi32(pw));
         if (p0 > pb || (p0 == pb && d0 < db)) { pb = p0; db = d0; }
-        if (p1 > pb || (p1 == pb && d0 + 1 < db)) { pb = p1; db = d0 + 1; }
+        if (p1 > pb || (p1 == pb && d1 < db)) { pb = p1; db = d1; }
         ps += lo32(pw) + hi32(pw);
       }
       const uint32_t km = __reduce_max_sync(0xffffffffu, pb);

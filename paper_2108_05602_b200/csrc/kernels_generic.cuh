@@ -39,6 +39,10 @@ struct RowArgs {
   // f2 all-IF mode (kernels_allif.cuh): a row is the whole band of one (bl, AP): nchan = nif_src * nchan_src
   // frequency points gathered from vis[bl][n][t][j], m = n * nchan_src + j.  0 = off.
   int allif_nif, allif_nchan;
+  // all-IF with nfa = psub * nf (nfa > 8192): AP row t is transformed as psub virtual rows rho = 0..psub-1,
+  // delay d = psub d' + rho:  A[rho + psub d'] = sum_m (x[m] W_nfa^{m rho}) W_nf^{m d'};  premod = W_nfa table
+  int psub;             // 1 = off
+  const float2 *premod; // [psub * nf] exp(-2 pi i k/(psub nf))
 };
 
 // Source of one AP row: plain (base pointer), dedispersed (per-channel row offsets), or the all-IF
@@ -46,9 +50,12 @@ struct RowArgs {
 struct RowSrc {
   const float2 *base;   // vis + row * nchan (plain) or vis + pair * nap * nchan (dedispersed / all-IF: pair = bl * nif_src)
   const int *sh;        // shift row of this IF (all-IF: the whole [nif][nchan] table), or nullptr
-  int t, nap, nchan, ai_nchan;
+  int t, nap, nchan, ai_nchan, rho;
+  const float2 *premod;
   bool gather;
   __device__ __forceinline__ RowSrc(const RowArgs &a, long long row) : nap(a.nap), nchan(a.nchan), ai_nchan(a.allif_nchan) {
+    rho = 0; premod = nullptr;
+    if (a.psub > 1) { rho = (int)(row % a.psub); row /= a.psub; premod = a.premod; }
     if (a.allif_nif) {
       const long long bl = row / a.nap;
       t = (int)(row - bl * a.nap);
@@ -67,7 +74,8 @@ struct RowSrc {
     if (ts < 0 || ts >= nap) return make_float2(0.f, 0.f);
     if (ai_nchan) {
       const int n = k / ai_nchan, j = k - n * ai_nchan;
-      return __ldg(base + ((long long)n * nap + ts) * ai_nchan + j);
+      const float2 v = __ldg(base + ((long long)n * nap + ts) * ai_nchan + j);
+      return rho ? cmul(v, __ldg(premod + (long long)k * rho)) : v;
     }
     return __ldg(base + (long long)ts * nchan + k);
   }
@@ -99,7 +107,7 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
     const int seg = tpr < 32 ? tpr : 32;
     for (int o = seg >> 1; o >= 1; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
     if (tpr <= 32) {
-      if (live && lane == 0) a.E[a.row0 + rrel] = e;
+      if (live && lane == 0 && (a.row0 + rrel) % a.psub == 0) a.E[(a.row0 + rrel) / a.psub] = e;
     } else {
       if ((lane & 31) == 0) esm[rl * 16 + (lane >> 5)] = e;
     }
@@ -108,7 +116,7 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
   if (tpr > 32 && live && lane == 0) {
     float s = 0.f;
     for (int i = 0; i < tpr / 32; ++i) s += esm[rl * 16 + i];
-    a.E[a.row0 + rrel] = s;
+    if ((a.row0 + rrel) % a.psub == 0) a.E[(a.row0 + rrel) / a.psub] = s;
   }
 
   float2 *in = buf0, *out = buf1;
@@ -235,7 +243,7 @@ __global__ void __launch_bounds__(256) k_row2(RowArgs a) {
   }
 #pragma unroll
   for (int o = G >> 1; o >= 1; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
-  if (live && l == 0) a.E[a.row0 + rrel] = e;
+  if (live && l == 0 && (a.row0 + rrel) % a.psub == 0) a.E[(a.row0 + rrel) / a.psub] = e;
   __syncwarp();
   f32x2 v[N1];
 #pragma unroll
@@ -318,7 +326,7 @@ __global__ void __launch_bounds__(256) k_row3(RowArgs a) {
   if (tid == 0) {
     float s = 0.f;
     for (int i = 0; i < 8; ++i) s += ered[i];
-    a.E[a.row0 + rrel] = s;
+    if ((a.row0 + rrel) % a.psub == 0) a.E[(a.row0 + rrel) / a.psub] = s;
   }
   // ---- step 2: groups of 16 lanes, group g <-> k3 (N3 <= 16 groups of the 16 available) ----
   const int g = tid >> 4, l = tid & 15;

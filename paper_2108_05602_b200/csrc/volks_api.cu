@@ -173,6 +173,9 @@ struct volks_plan {
   int paired = 0;               // Y rows pair-interleaved (common.cuh ld_y)
   mutable cudaStream_t copy_stream = nullptr;      // volks_search_host: H2D copies of the slab chunks
   mutable cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
+  int ai_psub = 1;               // f2 with nfa > 8192: nfa = ai_psub * row_nf (virtual sub-rows, kernels_generic.cuh)
+  int row_nf = 0;                // size of the row transform (= sched.nf unless ai_psub > 1)
+  size_t premod_off = 0;         // offset (float2) of the W_nfa table in d_tables
   int ai_nif = 0, ai_nchan = 0; // f2 all-IF plan: source nif / nchan (0 = ordinary per-IF plan)
   size_t off_noise = 0;         // f2: per-window noise written by k_allif
   bool row_generic = false;     // VOLKS_PATH=generic: the shared-memory Stockham row kernel only
@@ -222,7 +225,7 @@ const char *volks_strerror(int code) {
   }
 }
 
-static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif, int ai_nchan);
+static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif, int ai_nchan, int psub = 1);
 
 int volks_plan_create(const volks_params *p, volks_plan **out) { return plan_create_impl(p, out, 0, 0); }
 
@@ -230,15 +233,19 @@ int volks_plan_create_allif(const volks_params *p, volks_plan **out) {
   if (!p || !out) return VOLKS_EINVAL;
   *out = nullptr;
   if (p->nbl < 1 || p->nif < 1 || p->nchan < 1 || p->nwidths < 1 || p->nwidths > VOLKS_MAX_WIDTHS) return VOLKS_EINVAL;
-  if ((long long)p->nif * p->nchan > p->nf || p->nf < 64 || p->nf > 8192) return VOLKS_EINVAL;
+  if ((long long)p->nif * p->nchan > p->nf || p->nf < 64 || p->nf > 32768 || !is_pow2(p->nf)) return VOLKS_EINVAL;
+  if ((long long)p->nif * p->nchan > 8192) return VOLKS_EINVAL;      // the band must fit one 8192-point row transform
   int32_t ones[VOLKS_MAX_WIDTHS];
   for (int q = 0; q < VOLKS_MAX_WIDTHS; ++q) ones[q] = 1;
   volks_params b = *p;          // the band of one (bl, AP) as a single "IF" of nif * nchan points; no rate axis
   b.nif = 1; b.nchan = p->nif * p->nchan; b.nt = ones;
-  return plan_create_impl(&b, out, p->nif, p->nchan);
+  // nfa > 8192 (EL060: 8 IF x 1024 x pad 4 = 32768): psub interleaved 8192-point transforms per AP
+  const int psub = p->nf > 8192 ? p->nf / 8192 : 1;
+  b.nf = p->nf / psub;
+  return plan_create_impl(&b, out, p->nif, p->nchan, psub);
 }
 
-static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif, int ai_nchan) {
+static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif, int ai_nchan, int psub) {
   if (!p || !out) return VOLKS_EINVAL;
   *out = nullptr;
   const bool allif = ai_nif > 0;
@@ -254,8 +261,9 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   if (!pl) return VOLKS_ENOMEM;
   Sched &s = pl->sched;
   memset(&s, 0, sizeof s);
-  s.nwidths = p->nwidths; s.nbl = p->nbl; s.nif = p->nif; s.nap = p->nap; s.nf = p->nf;
-  s.log2nf = ilog2(p->nf); s.snr_thresh = p->snr_thresh;
+  s.nwidths = p->nwidths; s.nbl = p->nbl; s.nif = p->nif; s.nap = p->nap; s.nf = p->nf * psub;
+  s.log2nf = ilog2(s.nf); s.snr_thresh = p->snr_thresh;
+  pl->ai_psub = psub; pl->row_nf = p->nf;
   pl->nchan = p->nchan;
   pl->npair = (long long)p->nbl * p->nif;
   pl->ai_nif = ai_nif; pl->ai_nchan = ai_nchan; s.allif = allif ? 1 : 0;
@@ -310,10 +318,10 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   // chunking of the delay-spectrum intermediate Y over (bl, ifq) pairs: <= 4 GiB per chunk
   // Y row pitch: nf + 16 elements (one 128-byte line) when rows would otherwise sit a power of two
   // apart and fall into the same few L1 sets (kernels_slide.cuh reads w+1 rows of a column tile)
-  pl->pitch = p->nf >= 32 ? p->nf + env_int("VOLKS_Y_PAD", 16) : p->nf;
+  pl->pitch = (p->nf >= 32 && psub == 1) ? p->nf + env_int("VOLKS_Y_PAD", 16) : p->nf;   // sub-rows are contiguous
   pl->paired = p->nf >= 2 ? 1 : 0;
   pl->row_generic = force_generic;
-  const size_t y_pair = (size_t)p->nap * pl->pitch * sizeof(float2);
+  const size_t y_pair = (size_t)p->nap * psub * pl->pitch * sizeof(float2);
   // VOLKS_CHUNK_MB: bytes of delay spectra per chunk of pairs (default 4 GiB; tests use small chunks)
   const size_t budget = (size_t)std::max(1, env_int("VOLKS_CHUNK_MB", 4096)) << 20;
   long long ppc = y_pair ? (long long)std::max<size_t>(1, budget / std::max<size_t>(y_pair, 1)) : pl->npair;
@@ -342,7 +350,12 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   pl->launches = s.nwin_total > 0 ? (int)(pl->nchunks * (1 + active) + 3) : 0;
 
   // tables, computed in double precision on the host
+  if (psub > 1) { pl->premod_off = tw_total; tw_total += (size_t)s.nf; }
   std::vector<float2> tab(tw_total);
+  for (int k = 0; psub > 1 && k < s.nf; ++k) {
+    const double a = -2.0 * 3.14159265358979323846264338327950288 * k / s.nf;
+    tab[pl->premod_off + k] = make_float2((float)cos(a), (float)sin(a));
+  }
   const double PI = 3.14159265358979323846264338327950288;
   for (int k = 0; k < p->nf; ++k) {
     const double a = -2.0 * PI * k / p->nf;
@@ -477,8 +490,9 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
       ra.vis = (const float2 *)dst - (size_t)pair0 * pair_elems;   // kernels index by absolute pair
     }
     ra.Y = Y; ra.E = E; ra.twf = pl->d_tables;
-    ra.row0 = pair0 * s.nap; ra.nrows = np * s.nap;
-    ra.nchan = pl->nchan; ra.nf = s.nf; ra.tpr = pl->row_tpr; ra.rows_per_cta = pl->row_rows_per_cta; ra.pitch = pl->pitch; ra.paired = pl->paired;
+    ra.row0 = pair0 * s.nap * pl->ai_psub; ra.nrows = np * s.nap * pl->ai_psub;
+    ra.psub = pl->ai_psub; ra.premod = pl->ai_psub > 1 ? pl->d_tables + pl->premod_off : nullptr;
+    ra.nchan = pl->nchan; ra.nf = pl->row_nf; ra.tpr = pl->row_tpr; ra.rows_per_cta = pl->row_rows_per_cta; ra.pitch = pl->pitch; ra.paired = pl->paired;
     ra.shift = d_shift; ra.nif = s.nif; ra.allif_nif = pl->ai_nif; ra.allif_nchan = pl->ai_nchan;
     ra.keys1 = nullptr; ra.per_pair = s.per_pair; ra.nap = s.nap; ra.stride1 = 1; ra.nwin1 = 0;
     if (pl->wid1 >= 0) { ra.keys1 = keys + s.offc[pl->wid1]; ra.stride1 = s.stride[pl->wid1]; ra.nwin1 = (int)s.nwin[pl->wid1]; }
@@ -503,13 +517,15 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         aa.Y = Y; aa.keys = keys; aa.noise = (float *)(ws + pl->off_noise);
         aa.per_pair = s.per_pair; aa.offc = s.offc[q]; aa.pair0 = pair0;
         aa.nap = s.nap; aa.nf = s.nf; aa.w = w.w; aa.stride = w.s; aa.nwin = (int)w.nwin; aa.seg = w.seg;
-        aa.nseg = w.nseg; aa.pitch = pl->pitch;
+        aa.nseg = w.nseg; aa.pitch = pl->pitch * pl->ai_psub; aa.psub = pl->ai_psub; aa.nfb = pl->row_nf;
         const int thr = std::min(1024, s.nf / 2), cp = s.nf / 2 / thr;
         const unsigned blocks = (unsigned)(np * w.nseg);
         ProfScope ps(pl, st, VOLKS_K_ALLIF, q);
         if (cp == 1) k_allif<1><<<blocks, thr, 0, st>>>(aa);
         else if (cp == 2) k_allif<2><<<blocks, thr, 0, st>>>(aa);
-        else k_allif<4><<<blocks, thr, 0, st>>>(aa);
+        else if (cp == 4) k_allif<4><<<blocks, thr, 0, st>>>(aa);
+        else if (cp == 8) k_allif<8><<<blocks, thr, 0, st>>>(aa);
+        else k_allif<16><<<blocks, thr, 0, st>>>(aa);
         continue;
       }
       if (w.slide) {

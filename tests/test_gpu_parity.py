@@ -311,6 +311,9 @@ def test_zscore_selection_matches_oracle(vb, oracle, cfg, over):
     (1, 2, 900, 32, [64, 16], [16, 4], 128, 0.0),          # config-4-like strides w/4: sliding by blocks over several segments
     (1, 4, 400, 32, [4, 16], [1, 1], 256, 300.0),          # dedispersed all-IF search
     (1, 2, 120, 1024, [8], [1], 4096, 0.0),                # nfa = 4096: generic row kernel, 2 column pairs per thread
+    (1, 2, 40, 1024, [4], [1], 16384, 0.0),                # nfa = 16384 = 2 interleaved 8192-point transforms
+    (2, 8, 26, 1024, [2, 4], [1, 1], 32768, 0.0),          # the paper's shape: 8 IF x 1024 x pad 4
+    (1, 8, 30, 512, [4], [2], 32768, 300.0),               # pad x8, dedispersed, stride 2
 ])
 def test_allif_search_matches_oracle(vb, oracle, shape):
     """f2: one delay across all IFs (Eq. 1) vs oracle.allif_search on the same inputs."""
@@ -351,7 +354,8 @@ def test_allif_search_matches_oracle(vb, oracle, shape):
     key = [(int(c["bl"]), int(c["wid"]), int(c["win"])) for c in cands]
     assert key == sorted(key)
     hit = [c for c in cands if c["bl"] == 0 and nap // 3 - 16 <= c["t0"] <= nap // 3 + 12]
-    assert hit and all(abs(int(c["delay_idx"]) - round(0.0137 * nfa)) <= 1 for c in hit if c["snr"] > 8)
+    res = max(1, nfa // (nif * nchan))            # one unpadded resolution element of the delay axis
+    assert hit and all(abs(int(c["delay_idx"]) - round(0.0137 * nfa)) <= res for c in hit if c["snr"] > 8)
 
 
 @pytest.mark.parametrize("allif", [False, True])
