@@ -45,6 +45,12 @@ struct RowArgs {
   const float2 *premod; // [psub * nf] exp(-2 pi i k/(psub nf))
 };
 
+// index of a row's per-AP energy: every row when psub == 1, else only the rho == 0 sub-row (-1 = none)
+__device__ __forceinline__ long long e_index(const RowArgs &a, long long row) {
+  if (a.psub == 1) return row;
+  return row % a.psub == 0 ? row / a.psub : -1;
+}
+
 // Source of one AP row: plain (base pointer), dedispersed (per-channel row offsets), or the all-IF
 // band of one (bl, AP) gathered across IFs (with or without dedispersion).
 struct RowSrc {
@@ -55,7 +61,7 @@ struct RowSrc {
   bool gather;
   __device__ __forceinline__ RowSrc(const RowArgs &a, long long row) : nap(a.nap), nchan(a.nchan), ai_nchan(a.allif_nchan) {
     rho = 0; premod = nullptr;
-    if (a.psub > 1) { rho = (int)(row % a.psub); row /= a.psub; premod = a.premod; }
+    if (a.psub > 1) { rho = (int)(row % a.psub); row /= a.psub; premod = a.premod; }   // uniform branch, rare
     if (a.allif_nif) {
       const long long bl = row / a.nap;
       t = (int)(row - bl * a.nap);
@@ -107,7 +113,7 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
     const int seg = tpr < 32 ? tpr : 32;
     for (int o = seg >> 1; o >= 1; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
     if (tpr <= 32) {
-      if (live && lane == 0 && (a.row0 + rrel) % a.psub == 0) a.E[(a.row0 + rrel) / a.psub] = e;
+      if (live && lane == 0) { const long long ei = e_index(a, a.row0 + rrel); if (ei >= 0) a.E[ei] = e; }
     } else {
       if ((lane & 31) == 0) esm[rl * 16 + (lane >> 5)] = e;
     }
@@ -116,7 +122,8 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
   if (tpr > 32 && live && lane == 0) {
     float s = 0.f;
     for (int i = 0; i < tpr / 32; ++i) s += esm[rl * 16 + i];
-    if ((a.row0 + rrel) % a.psub == 0) a.E[(a.row0 + rrel) / a.psub] = s;
+    const long long ei = e_index(a, a.row0 + rrel);
+    if (ei >= 0) a.E[ei] = s;
   }
 
   float2 *in = buf0, *out = buf1;
@@ -225,13 +232,22 @@ __global__ void __launch_bounds__(256) k_row2(RowArgs a) {
   if (l < N1) {
     f32x2 z[N2];
     const RowSrc src(a, live ? a.row0 + rrel : a.row0);
+    float2 v[NZA];
+    if (!src.gather) {          // unswitched: the plain path keeps its independent, hoistable loads
 #pragma unroll
-    for (int n2 = 0; n2 < NZA; ++n2) {
-      const int n = l + N1 * n2;
-      float2 v = make_float2(0.f, 0.f);
-      if (live && n < a.nchan) { v = src(n); e += cnorm(v); }
-      z[n2] = c2_from(v);
+      for (int n2 = 0; n2 < NZA; ++n2) {
+        const int n = l + N1 * n2;
+        v[n2] = (live && n < a.nchan) ? __ldg(src.base + n) : make_float2(0.f, 0.f);
+      }
+    } else {
+#pragma unroll
+      for (int n2 = 0; n2 < NZA; ++n2) {
+        const int n = l + N1 * n2;
+        v[n2] = (live && n < a.nchan) ? src(n) : make_float2(0.f, 0.f);
+      }
     }
+#pragma unroll
+    for (int n2 = 0; n2 < NZA; ++n2) { e += cnorm(v[n2]); z[n2] = c2_from(v[n2]); }
     FftDif2<N2, NZA, 0, N2>::run(z);
 #pragma unroll
     for (int i = 0; i < N2; ++i) {
@@ -243,7 +259,7 @@ __global__ void __launch_bounds__(256) k_row2(RowArgs a) {
   }
 #pragma unroll
   for (int o = G >> 1; o >= 1; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
-  if (live && l == 0 && (a.row0 + rrel) % a.psub == 0) a.E[(a.row0 + rrel) / a.psub] = e;
+  if (live && l == 0) { const long long ei = e_index(a, a.row0 + rrel); if (ei >= 0) a.E[ei] = e; }
   __syncwarp();
   f32x2 v[N1];
 #pragma unroll
@@ -304,13 +320,22 @@ __global__ void __launch_bounds__(256) k_row3(RowArgs a) {
   {
     f32x2 z[N3];
     const RowSrc src(a, a.row0 + rrel);
+    float2 v[NZA];
+    if (!src.gather) {
 #pragma unroll
-    for (int n3 = 0; n3 < NZA; ++n3) {
-      const int n = tid + 256 * n3;
-      float2 v = make_float2(0.f, 0.f);
-      if (n < a.nchan) { v = src(n); e += cnorm(v); }
-      z[n3] = c2_from(v);
+      for (int n3 = 0; n3 < NZA; ++n3) {
+        const int n = tid + 256 * n3;
+        v[n3] = n < a.nchan ? __ldg(src.base + n) : make_float2(0.f, 0.f);
+      }
+    } else {
+#pragma unroll
+      for (int n3 = 0; n3 < NZA; ++n3) {
+        const int n = tid + 256 * n3;
+        v[n3] = n < a.nchan ? src(n) : make_float2(0.f, 0.f);
+      }
     }
+#pragma unroll
+    for (int n3 = 0; n3 < NZA; ++n3) { e += cnorm(v[n3]); z[n3] = c2_from(v[n3]); }
     FftDif2<N3, NZA, 0, N3>::run(z);
 #pragma unroll
     for (int i = 0; i < N3; ++i) {
@@ -326,7 +351,8 @@ __global__ void __launch_bounds__(256) k_row3(RowArgs a) {
   if (tid == 0) {
     float s = 0.f;
     for (int i = 0; i < 8; ++i) s += ered[i];
-    if ((a.row0 + rrel) % a.psub == 0) a.E[(a.row0 + rrel) / a.psub] = s;
+    const long long ei = e_index(a, a.row0 + rrel);
+    if (ei >= 0) a.E[ei] = s;
   }
   // ---- step 2: groups of 16 lanes, group g <-> k3 (N3 <= 16 groups of the 16 available) ----
   const int g = tid >> 4, l = tid & 15;
