@@ -391,3 +391,31 @@ def test_host_slab_search_is_identical(vb, allif, monkeypatch):
         assert int(n1.item()) == ref[0]
         assert c1.cpu().numpy()[: ref[0] * 36].tobytes() == ref[1] and p1.cpu().numpy().tobytes() == ref[2]
     plan.close()
+
+
+def test_search_is_cuda_graph_capturable(vb):
+    """The search is stream-asynchronous with no host synchronisation or allocation inside, so a
+    launch-bound small search (config 1) can be captured once in a CUDA graph and replayed."""
+    vis, c, _ = workloads.generate(1)
+    nbl, nif, nap, nchan = vis.shape
+    plan = vb.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"])
+    dev = torch.device("cuda")
+    d_vis = vis.cuda()
+    ws = torch.empty(plan.workspace_bytes, dtype=torch.uint8, device=dev)
+    cap = 1 << 14
+    cands = torch.zeros(cap * vb.CAND_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    ncand = torch.zeros(1, dtype=torch.int32, device=dev)
+    plan.fringe_search(d_vis, ws, cands, ncand)
+    torch.cuda.synchronize()
+    ref = (int(ncand.item()), cands.cpu().numpy().tobytes())
+    graph = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            plan.fringe_search(d_vis, ws, cands, ncand, stream=side)
+    for _ in range(3):
+        cands.zero_(); ncand.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert (int(ncand.item()), cands.cpu().numpy().tobytes()) == ref
+    plan.close()
