@@ -7,9 +7,9 @@
 // Column d of window (t0, w) on the padded grid Nt = 16 * L1, with t = t2 + 16 t1 and r = rho + L1 s:
 //   F[rho + L1 s] = sum_{t2<16} W_16^{s t2} [ W_Nt^{rho t2} Z_{t2}[rho] ],
 //   Z_{t2}[rho]   = sum_{t1<L1} y[t0 + t2 + 16 t1] W_{L1}^{rho t1}          (zero for t2 + 16 t1 >= w)
-// pass 1: warp t2 (16 warps), lane = column: L1-point DIF FFT over t1 in registers, pruned at compile
-//         time to the NZ = ceil(w/16) (rounded up to a power of two) leading non-zero inputs; the L1
-//         outputs go to shared memory S[rho][t2][column].
+// pass 1: warp t2 (16 warps), lane = column: L1-point packed DIF FFT (common.cuh FftDif2) over t1 in
+//         registers, pruned at compile time to the NZ = ceil(w/16) (rounded up to a power of two) leading
+//         non-zero inputs; the L1 outputs go to shared memory S[rho][t2][column].
 // pass 2: warp <-> residues rho (L1/16 each... one or two per warp), lane = column: 16 shared loads,
 //         the twiddle W_Nt^{rho t2} from a shared table, a 16-point DIF FFT in registers, |.|^2, the
 //         tagged 32-bit peak key of kernels_slide.cuh (R1), warp redux, one slot per warp;
@@ -31,56 +31,6 @@ struct ColFftArgs {
   int wpc;              // windows per CTA (consecutive)
   int nrange;           // ceil(nwin / wpc)
   uint32_t keymask;     // 0xFFFFFFF0 (register operand of the single-LOP3 key tag)
-};
-
-// z * exp(-2 pi i K/32), 0 <= K < 16, compile time
-template <int K>
-__device__ __forceinline__ float2 mul_w32(float2 z) {
-  static_assert(K >= 0 && K < 16, "first-half twiddles only");
-  if constexpr ((K & 1) == 0) return mul_w<K / 2, 16>(z);
-  else {
-    constexpr float C[8] = {0.98078528040323043f, 0.83146961230254524f, 0.55557023301960218f, 0.19509032201612825f,
-                            -0.19509032201612825f, -0.55557023301960218f, -0.83146961230254524f, -0.98078528040323043f};
-    constexpr float S[8] = {0.19509032201612825f, 0.55557023301960218f, 0.83146961230254524f, 0.98078528040323043f,
-                            0.98078528040323043f, 0.83146961230254524f, 0.55557023301960218f, 0.19509032201612825f};
-    constexpr float c = C[K / 2], s = S[K / 2];   // cos, sin of 2 pi K/32
-    return make_float2(fmaf(z.x, c, z.y * s), fmaf(z.y, c, -z.x * s));
-  }
-}
-
-// z * exp(-2 pi i K/N) for N in {2,4,8,16,32}
-template <int K, int N>
-__device__ __forceinline__ float2 mul_wn(float2 z) {
-  if constexpr (N == 32) return mul_w32<K>(z);
-  else return mul_w<K, N>(z);
-}
-
-// In-register radix-2 DIF FFT of N points a[OFF .. OFF+N), forward, output BIT-REVERSED, where only
-// the first NZ inputs are non-zero (the rest are never read): a stage whose upper half is all zero
-// degenerates to  a[k + N/2] = W_N^k a[k].
-template <int N, int NZ, int OFF, int TOTAL>
-struct FftDifPruned {
-  template <int K>
-  static __device__ __forceinline__ void stage(float2 (&a)[TOTAL]) {
-    if constexpr (K < N / 2) {
-      if constexpr (NZ <= N / 2) {
-        if constexpr (K < NZ) a[OFF + K + N / 2] = mul_wn<K, N>(a[OFF + K]);
-      } else {
-        const float2 u = a[OFF + K], v = a[OFF + K + N / 2];
-        a[OFF + K] = cadd(u, v);
-        a[OFF + K + N / 2] = mul_wn<K, N>(csub(u, v));
-      }
-      stage<K + 1>(a);
-    }
-  }
-  static __device__ __forceinline__ void run(float2 (&a)[TOTAL]) {
-    if constexpr (N >= 2) {
-      stage<0>(a);
-      constexpr int NZ2 = NZ < N / 2 ? NZ : N / 2;
-      FftDifPruned<N / 2, NZ2, OFF, TOTAL>::run(a);
-      FftDifPruned<N / 2, NZ2, OFF + N / 2, TOTAL>::run(a);
-    }
-  }
 };
 
 // L1 = Nt/16 (2..32), NZ = leading non-zero inputs of the L1-point transform (power of two <= L1).

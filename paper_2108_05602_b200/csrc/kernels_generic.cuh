@@ -380,7 +380,10 @@ __global__ void __launch_bounds__(256) k_row3(RowArgs a) {
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
       const int col = N3 * (16 * brev<16>(i) + l) + g;
-      float *p = img + ((col >> 1) << 2) + (col & 1);
+      // float4 slot of the column pair, XOR-swizzled by bits 3..5 so that the 16 lanes (column stride N3)
+      // spread over the banks instead of hitting two of them
+      const int q = col >> 1, qs = q ^ ((q >> 3) & 7);
+      float *p = img + (qs << 2) + (col & 1);
       p[0] = lo32(v[i]); p[2] = hi32(v[i]);
     }
   }
@@ -389,7 +392,7 @@ __global__ void __launch_bounds__(256) k_row3(RowArgs a) {
   u64 key = 0;
   float4 *dst = (float4 *)(a.Y + rrel * (long long)a.pitch);
   for (int c = tid; c < NF / 2; c += 256) {
-    const float4 q = ((const float4 *)img)[c];
+    const float4 q = ((const float4 *)img)[c ^ ((c >> 3) & 7)];
     dst[c] = q;
     const u64 k0 = make_key(fmaf(q.x, q.x, q.z * q.z), (uint32_t)(2 * c)), k1 = make_key(fmaf(q.y, q.y, q.w * q.w), (uint32_t)(2 * c + 1));
     key = k0 > key ? k0 : key;
