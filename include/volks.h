@@ -28,6 +28,8 @@
  *
  * Errors: every int-returning call gives 0 (VOLKS_OK) or a negative code; nothing throws, exits or
  * prints.  Non-finite visibilities are a precondition violation (results unspecified, no crash).
+ * Threads: a plan holds per-call state (profiling events, the copy stream of volks_search_host); use a
+ * plan from one host thread at a time (several plans may run concurrently on different streams).
  * Determinism: identical inputs give bit-identical outputs run to run (the peak reduction is an
  * order-independent max over a total order; the compaction is an ordered scan).
  */
