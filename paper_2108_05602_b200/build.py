@@ -8,7 +8,8 @@ LIB = os.path.join(HERE, "libvolks_b200.so")
 SOURCES = ["volks_api.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-shared", 
+    "-Xcompiler", "-fPIC", "-shared", "-diag-suppress", "550",   # 550: the unused half of a mov.b64 unpack
+    
 ]
 
 
