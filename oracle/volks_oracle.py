@@ -299,3 +299,20 @@ def allif_search(vis, widths, strides, nfa):
                 noise = s1 / nfa
                 out.append((p[i1], q[i2] if nfa > 1 else 0.0, s1, np.sqrt(p[i1] / noise) if noise > 0 else 0.0, i1, i2))
     return np.array(out, dtype=PEAK_DTYPE) if out else np.zeros(0, dtype=PEAK_DTYPE)
+
+
+def cal_phasors(delay_s, phase_rad, nchan, chan_hz):
+    """Initial-calibration phasors of Eq. 1: the last two terms of
+    Phi(n, j) = ... + 2 pi f_j dtau0^n + dphi0^n, with f_j = j * chan_hz the j-th frequency point inside
+    the IF, enter G as S(n, j) e^{-i(2 pi f_j dtau0^n + dphi0^n)}.  delay_s, phase_rad: [nbl][nif]
+    (per baseline and IF).  Returns complex64 [nbl][nif][nchan]."""
+    d = np.asarray(delay_s, dtype=np.float64)[..., None]
+    p = np.asarray(phase_rad, dtype=np.float64)[..., None]
+    f = np.arange(nchan, dtype=np.float64) * float(chan_hz)
+    return np.exp(-1j * (2.0 * np.pi * f * d + p)).astype(np.complex64)
+
+
+def calibrate(vis, cal):
+    """Step 3: vis[bl][ifq][t][k] * cal[bl][ifq][k], formed in double, stored as complex64."""
+    v = np.asarray(vis).astype(np.complex128) * np.asarray(cal).astype(np.complex128)[:, :, None, :]
+    return v.astype(np.complex64)

@@ -418,3 +418,31 @@ def test_allif_search_pins(oracle):
     # phase restarting in every IF with a half-integer per-IF delay: adjacent IFs are pi apart
     per_if[0, :, 3:3 + w, :] = (a * np.exp(2j * np.pi * 2.5 * np.arange(nchan) / nchan)).astype(np.complex64)
     assert oracle.allif_search(per_if, [w], [1], nfa)[3]["p1"] < 0.9 * (a * w * nif * nchan) ** 2
+
+
+def test_initial_calibration_pins(oracle):
+    """Eq. 1's calibration terms.  A band-coherent fringe corrupted by per-IF
+    delays and phases ("the large IF delay ... discrepancies of initial delay and phase between IFs")
+    loses coherence across IFs; multiplying by cal_phasors of the same values restores the closed-form
+    all-IF peak P1 = (a w nif nchan)^2 at the injected delay ("after calibration, fringe phase become
+    flat and aligned across IFs").  Zero delay and phase give unit phasors; a pure phase is a constant."""
+    nbl, nif, nap, nchan, w, nfa, a, tau = 1, 4, 10, 16, 4, 256, 0.8, 3
+    chan_hz = 16e6 / nchan
+    rng = np.random.default_rng(3)
+    d0 = rng.uniform(-40e-9, 40e-9, (nbl, nif))
+    p0 = rng.uniform(-np.pi, np.pi, (nbl, nif))
+    assert np.allclose(oracle.cal_phasors(np.zeros((1, 2)), np.zeros((1, 2)), 8, 1e6), 1.0)
+    c = oracle.cal_phasors(np.zeros((1, 1)), np.full((1, 1), 0.5), 8, 1e6)
+    assert np.allclose(c, np.exp(-0.5j), atol=1e-7)
+    m = np.arange(nif * nchan).reshape(nif, 1, nchan)
+    clean = a * np.exp(2j * np.pi * tau * m / (nif * nchan))
+    j = np.arange(nchan)[None, None, :]
+    corrupt = clean * np.exp(1j * (2 * np.pi * (j * chan_hz) * d0[0][:, None, None] + p0[0][:, None, None]))
+    vis = np.zeros((nbl, nif, nap, nchan), np.complex64)
+    vis[0, :, 2:2 + w, :] = corrupt.astype(np.complex64)
+    before = oracle.allif_search(vis, [w], [1], nfa)[2]
+    cal = oracle.cal_phasors(d0, p0, nchan, chan_hz)
+    after = oracle.allif_search(oracle.calibrate(vis, cal), [w], [1], nfa)[2]
+    full = (a * w * nif * nchan) ** 2
+    assert abs(after["p1"] - full) < 1e-5 * full and after["idx1"] == tau * nfa // (nif * nchan)
+    assert before["p1"] < 0.8 * full
