@@ -197,7 +197,7 @@ def aggregate_value(world, units_per_rank, ms_step):
     return world * units_per_rank / (ms_step * 1e-3)
 
 
-KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6: "slide", 7: "colfft", 8: "allif"}
+KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6: "slide", 7: "colfft", 8: "allif", 9: "fixup"}
 
 
 def run_volks(args):

@@ -161,6 +161,18 @@ int volks_search_host(const volks_plan *plan, const void *h_vis, void *d_stage, 
 int volks_zscore_select(const volks_plan *plan, void *d_workspace, float z_thresh, volks_peak *d_peaks,
                         volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand, void *cuda_stream);
 
+/* Initial calibration (step 3 of the paper; the last two terms of Eq. 1, PAPER.md:74-79:
+ * Phi = ... + 2 pi f_j dtau0^n + dphi0^n with f_j the j-th frequency point inside IF n, values per IF
+ * and baseline), fused into the slab load: every later search with this plan multiplies
+ * vis[bl][ifq][t][k] by d_cal[bl][ifq][k] as it is read.
+ *   d_cal  DEVICE cf32[nbl][nif][nchan] (the SOURCE shape, also for an all-IF plan), or NULL to switch
+ *          it off.  The plan keeps the pointer, not a copy: the table must outlive the searches.
+ * volks_cal_phasors (HOST) fills a table with e^{-i (2 pi j chan_hz delay_s[p] + phase_rad[p])},
+ * p = bl*nif + ifq, j < nchan: cal is HOST float[2*npair*nchan] (re, im). */
+int volks_plan_set_cal(volks_plan *plan, const void *d_cal);
+int volks_cal_phasors(const double *delay_s, const double *phase_rad, int32_t npair, int32_t nchan,
+                      double chan_hz, float *cal);
+
 /* HOST helper: integer AP shift of every frequency point for dispersion measure `dm` [pc cm^-3]:
  * shift = round(4.148808e-3 s * dm * (f_GHz^-2 - fref_GHz^-2) / ap_seconds) (the textbook cold-plasma
  * delay; the paper states no formula - DESIGN.md R3).  f_chan_mhz, shift: HOST [n]. */
@@ -215,6 +227,7 @@ int volks_plan_launch_count(const volks_plan *plan);
 #define VOLKS_K_SLIDE 6    /* stride-1 widths: sliding-sum rate transform + power + argmax          */
 #define VOLKS_K_COLFFT 7   /* any stride, Nt 32..512: two-pass shared-memory column FFT + argmax    */
 #define VOLKS_K_ALLIF 8    /* f2: all-IF rate-0 window sums + argmax + noise                          */
+#define VOLKS_K_FIXUP 9    /* exact re-evaluation of the sliding widths' outlier windows               */
 int volks_plan_profile(volks_plan *plan, int enable);
 int volks_plan_profile_read(const volks_plan *plan, int32_t capacity, int32_t *kind, int32_t *wid,
                             float *ms, int32_t *n);

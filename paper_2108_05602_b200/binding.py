@@ -18,7 +18,7 @@ EXPORTS = (
     "volks_window_match", "volks_bin_to_physical", "volks_plan_launch_count", "volks_strerror",
     "volks_version", "volks_plan_profile", "volks_plan_profile_read", "volks_fringe_search_dd", "volks_dm_shifts",
     "volks_baseline_match", "volks_zscore_select", "volks_plan_create_allif", "volks_allif_search",
-    "volks_plan_query_host", "volks_search_host",
+    "volks_plan_query_host", "volks_search_host", "volks_plan_set_cal", "volks_cal_phasors",
 )
 
 
@@ -57,6 +57,9 @@ def lib():
         L.volks_allif_search.argtypes = [ctypes.c_void_p] * 6 + [ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
         L.volks_plan_query_host.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_size_t)]
         L.volks_search_host.argtypes = [ctypes.c_void_p] * 7 + [ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
+        L.volks_plan_set_cal.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+        L.volks_cal_phasors.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32,
+                                        ctypes.c_double, ctypes.c_void_p]
         L.volks_plan_destroy.argtypes = [ctypes.c_void_p]
         L.volks_plan_query.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_size_t),
                                        ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
@@ -149,6 +152,14 @@ class Plan:
             peaks.data_ptr() if peaks is not None else None, cands.data_ptr() if cap else None, cap,
             ncand.data_ptr(), st))
 
+    def set_cal(self, cal):
+        """volks_plan_set_cal: cal = CUDA complex64 [nbl][nif][nchan] (kept alive by this object) or None."""
+        if cal is not None:
+            assert cal.is_cuda and cal.dtype == torch.complex64 and cal.is_contiguous()
+            assert tuple(cal.shape) == (self.shape[0], self.shape[1], self.shape[3])
+        self._cal = cal
+        _check(lib().volks_plan_set_cal(self._h, cal.data_ptr() if cal is not None else None))
+
     @property
     def stage_bytes(self):
         """volks_plan_query_host: bytes of ONE half of the staging buffer of search_host."""
@@ -207,6 +218,16 @@ def window_match(cands, widths, min_widths=2):
     _check(lib().volks_window_match(cands.ctypes.data, len(cands), w.ctypes.data, len(w), min_widths,
                                     out.ctypes.data, len(out), ctypes.byref(n)))
     return out[:n.value]
+
+
+def cal_phasors(delay_s, phase_rad, nchan, chan_hz):
+    """volks_cal_phasors: complex64 [..., nchan] calibration phasors for delay_s / phase_rad of shape [...]."""
+    d = np.ascontiguousarray(delay_s, dtype=np.float64)
+    p = np.ascontiguousarray(phase_rad, dtype=np.float64)
+    assert d.shape == p.shape
+    out = np.zeros(d.shape + (nchan, 2), dtype=np.float32)
+    _check(lib().volks_cal_phasors(d.ctypes.data, p.ctypes.data, d.size, nchan, float(chan_hz), out.ctypes.data))
+    return out.view(np.complex64)[..., 0]
 
 
 def baseline_match(pulses, min_baselines=5):

@@ -8,7 +8,10 @@
 //
 // Overlapping windows slide: A_{j+1} = A_j + sum_{t<s} (Y[t0+w+t] - Y[t0+t]) (no twiddle: rate 0 only;
 // 2 s row reads per window instead of w), restarted from a direct sum every `seg` windows like
-// kernels_slide.cuh; windows with 2 s > w are summed directly.
+// kernels_slide.cuh; windows with 2 s > w are summed directly.  A sample leaves a rounding residue of
+// about 6e-8 of its size in the running sum; when the window energy (from the per-AP energies, tracked
+// in double) falls below 1e-3 of the largest since the last exact sum, the window is summed directly
+// again (a uniform decision: every thread evaluates the same scalars).
 // One CTA owns ALL delay columns of its windows (thread = CP column pairs, packed FP32), so the
 // argmax and the sum need no atomics: per 16 windows one barrier, fixed-order reductions, plain stores.
 #pragma once
@@ -22,6 +25,7 @@ struct AllifArgs {
   const float2 *Y;      // [nbl_chunk][nap][pitch] all-IF delay spectra, pair-interleaved rows
   u64 *keys;            // canonical window keys
   float *noise;         // canonical per-window noise = S1 / nfa
+  const float *E;       // per-AP band energies [npairs_total][nap] (row kernel): detects energy collapse
   long long per_pair, offc, pair0;
   int nap, nf, w, stride, nwin, seg, nseg, pitch;
   int psub, nfb;        // nf = psub * nfb: column c of a row is sub-row rho = c / nfb, d' = c % nfb, delay d = psub d' + rho
@@ -54,7 +58,13 @@ __global__ void __launch_bounds__(1024) k_allif(AllifArgs a) {
       }
     }
   };
-  if (slide) direct(j0 * a.stride);
+  const float *Ep = a.E + (a.pair0 + pl) * (long long)a.nap;
+  double es = 0.0, esmax = 0.0;
+  if (slide) {
+    direct(j0 * a.stride);
+    for (int t = 0; t < a.w; ++t) es += (double)__ldg(Ep + j0 * a.stride + t);
+    esmax = es;
+  }
 
   for (int jb = j0; jb < j1; jb += 16) {
     const int nst = min(16, j1 - jb);
@@ -83,6 +93,13 @@ __global__ void __launch_bounds__(1024) k_allif(AllifArgs a) {
       // next window
       if (slide && j + 1 < j1) {
         const int t0 = j * a.stride;
+        for (int t = 0; t < a.stride; ++t) es += (double)__ldg(Ep + t0 + t + a.w) - (double)__ldg(Ep + t0 + t);
+        if (es < 1e-3 * esmax) {          // energy collapse: the residue of what left would dominate - sum exactly
+          direct(t0 + a.stride);
+          esmax = es;
+          continue;
+        }
+        esmax = es > esmax ? es : esmax;
         for (int t = 0; t < a.stride; ++t) {
 #pragma unroll
           for (int i = 0; i < CP; ++i) {

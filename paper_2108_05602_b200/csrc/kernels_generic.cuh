@@ -43,6 +43,10 @@ struct RowArgs {
   // delay d = psub d' + rho:  A[rho + psub d'] = sum_m (x[m] W_nfa^{m rho}) W_nf^{m d'};  premod = W_nfa table
   int psub;             // 1 = off
   const float2 *premod; // [psub * nf] exp(-2 pi i k/(psub nf))
+  // initial calibration (Eq. 1's last two terms): element (pair, k) is multiplied by
+  // cal[pair * nchan + k] (all-IF mode: pair = bl, k = n * nchan_src + j - the same memory layout
+  // cf32[nbl][nif][nchan]); nullptr = none
+  const float2 *cal;
 };
 
 // index of a row's per-AP energy: every row when psub == 1, else only the rho == 0 sub-row (-1 = none)
@@ -58,10 +62,12 @@ struct RowSrc {
   const int *sh;        // shift row of this IF (all-IF: the whole [nif][nchan] table), or nullptr
   int t, nap, nchan, ai_nchan, rho;
   const float2 *premod;
+  const float2 *calrow;   // calibration phasors of this row's pair, or nullptr
   bool gather;
   __device__ __forceinline__ RowSrc(const RowArgs &a, long long row) : nap(a.nap), nchan(a.nchan), ai_nchan(a.allif_nchan) {
-    rho = 0; premod = nullptr;
+    rho = 0; premod = nullptr; calrow = nullptr;
     if (a.psub > 1) { rho = (int)(row % a.psub); row /= a.psub; premod = a.premod; }   // uniform branch, rare
+    if (a.cal) calrow = a.cal + (row / a.nap) * (long long)a.nchan;
     if (a.allif_nif) {
       const long long bl = row / a.nap;
       t = (int)(row - bl * a.nap);
@@ -72,10 +78,10 @@ struct RowSrc {
       t = (int)(row - pair * a.nap);
       base = a.vis + pair * a.nap * (long long)a.nchan;
       sh = a.shift + (pair % a.nif) * a.nchan; gather = true;
-    } else { base = a.vis + row * (long long)a.nchan; sh = nullptr; t = 0; gather = false; }
+    } else { base = a.vis + row * (long long)a.nchan; sh = nullptr; t = 0; gather = calrow != nullptr; }
   }
-  __device__ __forceinline__ float2 operator()(int k) const {
-    if (!gather) return __ldg(base + k);
+  __device__ __forceinline__ float2 fetch(int k) const {
+    if (!sh && !ai_nchan) return __ldg(base + k);   // plain row (only the calibration is applied)
     const int ts = t + (sh ? __ldg(sh + k) : 0);
     if (ts < 0 || ts >= nap) return make_float2(0.f, 0.f);
     if (ai_nchan) {
@@ -84,6 +90,11 @@ struct RowSrc {
       return rho ? cmul(v, __ldg(premod + (long long)k * rho)) : v;
     }
     return __ldg(base + (long long)ts * nchan + k);
+  }
+  __device__ __forceinline__ float2 operator()(int k) const {
+    if (!gather) return __ldg(base + k);
+    const float2 v = fetch(k);
+    return calrow ? cmul(v, __ldg(calrow + k)) : v;
   }
 };
 

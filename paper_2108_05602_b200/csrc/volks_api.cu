@@ -13,6 +13,7 @@
 #include "kernels_slide.cuh"
 #include "kernels_colfft.cuh"
 #include "kernels_allif.cuh"
+#include "kernels_fixup.cuh"
 
 using namespace volks;
 
@@ -173,6 +174,8 @@ struct volks_plan {
   int paired = 0;               // Y rows pair-interleaved (common.cuh ld_y)
   mutable cudaStream_t copy_stream = nullptr;      // volks_search_host: H2D copies of the slab chunks
   mutable cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
+  mutable const float2 *d_cal = nullptr;   // volks_plan_set_cal: DEVICE cf32[nbl][nif][nchan] applied in the slab load
+  int nslide = 0;                // widths on the sliding-sum path (k_fixup re-evaluates their outlier windows)
   int ai_psub = 1;               // f2 with nfa > 8192: nfa = ai_psub * row_nf (virtual sub-rows, kernels_generic.cuh)
   int row_nf = 0;                // size of the row transform (= sched.nf unless ai_psub > 1)
   size_t premod_off = 0;         // offset (float2) of the W_nfa table in d_tables
@@ -342,12 +345,13 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   pl->ws_bytes = off;
 
   int active = 0;
+  for (auto &w : pl->wp) pl->nslide += (w.slide && w.nwin > 0) ? 1 : 0;
   if (!force_generic && !allif)
     for (int q = 0; q < p->nwidths && pl->wid1 < 0; ++q)
       if (pl->wp[q].w == 1 && pl->wp[q].nwin > 0) pl->wid1 = q;
   for (int q = 0; q < p->nwidths; ++q) active += (pl->wp[q].nwin > 0 && q != pl->wid1) ? 1 : 0;
   // kernels of this library per search (the key memset is a driver memset, not counted)
-  pl->launches = s.nwin_total > 0 ? (int)(pl->nchunks * (1 + active) + 3) : 0;
+  pl->launches = s.nwin_total > 0 ? (int)(pl->nchunks * (1 + active + (pl->nslide > 0 ? 1 : 0)) + 3) : 0;
 
   // tables, computed in double precision on the host
   if (psub > 1) { pl->premod_off = tw_total; tw_total += (size_t)s.nf; }
@@ -428,6 +432,25 @@ int volks_allif_search(const volks_plan *pl, const void *d_vis, const int32_t *d
   return run_search(pl, d_vis, nullptr, d_shift, d_workspace, d_peaks, d_cands, cand_capacity, d_ncand, cuda_stream);
 }
 
+int volks_plan_set_cal(volks_plan *pl, const void *d_cal) {
+  if (!pl) return VOLKS_EINVAL;
+  pl->d_cal = (const float2 *)d_cal;
+  return VOLKS_OK;
+}
+
+int volks_cal_phasors(const double *delay_s, const double *phase_rad, int32_t npair, int32_t nchan, double chan_hz,
+                      float *cal) {
+  if (!delay_s || !phase_rad || !cal || npair < 0 || nchan < 1 || !(chan_hz > 0)) return VOLKS_EINVAL;
+  const double TWO_PI = 6.28318530717958647692528676655900577;
+  for (int32_t p = 0; p < npair; ++p)
+    for (int32_t j = 0; j < nchan; ++j) {
+      const double ph = -(TWO_PI * (j * chan_hz) * delay_s[p] + phase_rad[p]);
+      cal[2 * ((size_t)p * nchan + j)] = (float)cos(ph);
+      cal[2 * ((size_t)p * nchan + j) + 1] = (float)sin(ph);
+    }
+  return VOLKS_OK;
+}
+
 int volks_plan_query_host(const volks_plan *pl, size_t *stage_bytes) {
   if (!pl || !stage_bytes) return VOLKS_EINVAL;
   *stage_bytes = align_up((size_t)pl->pairs_per_chunk * pl->sched.nap * pl->nchan * sizeof(float2), 256);
@@ -493,6 +516,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
     ra.row0 = pair0 * s.nap * pl->ai_psub; ra.nrows = np * s.nap * pl->ai_psub;
     ra.psub = pl->ai_psub; ra.premod = pl->ai_psub > 1 ? pl->d_tables + pl->premod_off : nullptr;
     ra.nchan = pl->nchan; ra.nf = pl->row_nf; ra.tpr = pl->row_tpr; ra.rows_per_cta = pl->row_rows_per_cta; ra.pitch = pl->pitch; ra.paired = pl->paired;
+    ra.cal = pl->d_cal;
     ra.shift = d_shift; ra.nif = s.nif; ra.allif_nif = pl->ai_nif; ra.allif_nchan = pl->ai_nchan;
     ra.keys1 = nullptr; ra.per_pair = s.per_pair; ra.nap = s.nap; ra.stride1 = 1; ra.nwin1 = 0;
     if (pl->wid1 >= 0) { ra.keys1 = keys + s.offc[pl->wid1]; ra.stride1 = s.stride[pl->wid1]; ra.nwin1 = (int)s.nwin[pl->wid1]; }
@@ -514,7 +538,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
       ca.total = ((np * w.nwin) << w.log2m) * s.nf;
       if (pl->ai_nif) {
         AllifArgs aa;
-        aa.Y = Y; aa.keys = keys; aa.noise = (float *)(ws + pl->off_noise);
+        aa.Y = Y; aa.keys = keys; aa.noise = (float *)(ws + pl->off_noise); aa.E = E;
         aa.per_pair = s.per_pair; aa.offc = s.offc[q]; aa.pair0 = pair0;
         aa.nap = s.nap; aa.nf = s.nf; aa.w = w.w; aa.stride = w.s; aa.nwin = (int)w.nwin; aa.seg = w.seg;
         aa.nseg = w.nseg; aa.pitch = pl->pitch * pl->ai_psub; aa.psub = pl->ai_psub; aa.nfb = pl->row_nf;
@@ -557,6 +581,23 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         case 8: launch_col<8>(ca, st); break;
         default: launch_col<16>(ca, st); break;
       }
+    }
+    // exact re-evaluation of the sliding widths' windows that sit far below an earlier window of their segment
+    if (pl->nslide > 0) {
+      FixArgs fa;
+      fa.Y = Y; fa.keys = keys; fa.tables = pl->d_tables; fa.per_pair = s.per_pair; fa.pair0 = pair0;
+      fa.nap = s.nap; fa.nf = s.nf; fa.log2nf = s.log2nf; fa.pitch = pl->pitch; fa.paired = pl->paired;
+      fa.nq = 0; fa.unit0[0] = 0;
+      for (int q = 0; q < s.nwidths; ++q) {
+        const WidthPlan &w = pl->wp[q];
+        if (!w.slide || w.nwin == 0) continue;
+        const int i = fa.nq++;
+        fa.q[i] = q; fa.w[i] = w.w; fa.nt[i] = w.nt; fa.seg[i] = w.seg; fa.nseg[i] = w.nseg; fa.nwin[i] = (int)w.nwin;
+        fa.offc[i] = s.offc[q]; fa.tw_off[i] = (long long)w.tw_off;
+        fa.unit0[i + 1] = fa.unit0[i] + w.nseg;
+      }
+      ProfScope ps(pl, st, VOLKS_K_FIXUP, -1);
+      k_fixup<<<(unsigned)(np * fa.unit0[fa.nq]), 256, 0, st>>>(fa);
     }
   }
   {

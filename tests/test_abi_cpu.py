@@ -165,3 +165,12 @@ def test_baseline_match_host_vs_oracle(vb, oracle):
     two = mk([(b, 100, 110, 7.0) for b in range(5)] + [(b, 300, 310, 7.0) for b in range(5)])
     rc = vb.lib().volks_baseline_match(two.ctypes.data, len(two), 5, cap[1].ctypes.data, 1, ctypes.byref(cap[0]))
     assert rc == -4 and cap[0].value == 2
+
+
+def test_cal_phasors_host_vs_oracle(vb, oracle):
+    rng = np.random.default_rng(2)
+    d, p = rng.uniform(-50e-9, 50e-9, (3, 4)), rng.uniform(-3, 3, (3, 4))
+    got = vb.cal_phasors(d, p, 64, 250e3)
+    exp = oracle.cal_phasors(d, p, 64, 250e3)
+    assert got.shape == exp.shape == (3, 4, 64) and np.abs(got - exp).max() < 3e-7
+    assert np.allclose(np.abs(got), 1.0, atol=1e-6)

@@ -419,3 +419,67 @@ def test_search_is_cuda_graph_capturable(vb):
         torch.cuda.synchronize()
         assert (int(ncand.item()), cands.cpu().numpy().tobytes()) == ref
     plan.close()
+
+
+def test_calibration_fused_into_slab_load(vb, oracle):
+    """Eq. 1's calibration terms applied while the slab is read == oracle.calibrate followed by the
+    plain search; per-IF 2-D search (with and without dedispersion) and the all-IF search, where the
+    calibration is what makes the IFs coherent."""
+    vis, c, _ = workloads.generate(2, nbl=2, nif=4, nap=400, npulses=2)
+    nbl, nif, nap, nchan = vis.shape
+    rng = np.random.default_rng(8)
+    d0, p0 = rng.uniform(-40e-9, 40e-9, (nbl, nif)), rng.uniform(-np.pi, np.pi, (nbl, nif))
+    chan_hz = 16e6 / nchan
+    cal = vb.cal_phasors(d0, p0, nchan, chan_hz)
+    # corrupt the data with the inverse phasors, so that calibration restores the injected pulses
+    raw = (vis.numpy().astype(np.complex128) * np.conj(cal.astype(np.complex128))[:, :, None, :]).astype(np.complex64)
+    d_raw, d_cal = torch.from_numpy(raw).cuda(), torch.from_numpy(cal).cuda()
+    nw = [workloads.gen.nwin(nap, w, s) for w, s in zip(c["widths"], c["strides"])]
+    f = 1400.0 + 16.0 * np.arange(nif)[:, None] + (16.0 / nchan) * np.arange(nchan)[None, :]
+    sh = vb.dm_shifts(200.0, f, f.max(), c["t_ap"])
+    for shifts in (None, sh):
+        plan = vb.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"])
+        plan.set_cal(d_cal)
+        cands, n, peaks = vb.fringe_search(d_raw, want_peaks=True, plan=plan, shifts=shifts)
+        src = oracle.calibrate(raw, cal)
+        if shifts is not None:
+            src = oracle.dedisperse(src, shifts)
+        ora, _ = oracle.search(src, c["widths"], c["strides"], c["nts"], c["nf"], mode="cached")
+        check_peaks(peaks[dense_index(nbl, nif, nw)], ora, c["nf"], make_plane_power(oracle, src, c))
+        plan.set_cal(None)
+        _, _, p_off = vb.fringe_search(d_raw, want_peaks=True, plan=plan, shifts=shifts)
+        assert not np.array_equal(p_off["delay_idx"], peaks["delay_idx"])      # switching it off changes the result
+        plan.close()
+    # all-IF: coherent only after calibration
+    nfa = 1024
+    plan = vb.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], None, nfa, 5.0, allif=True)
+    plan.set_cal(d_cal)
+    cands, n, peaks = vb.fringe_search(d_raw, want_peaks=True, plan=plan)
+    ora = oracle.allif_search(oracle.calibrate(raw, cal), c["widths"], c["strides"], nfa)
+    pk = peaks[dense_index(nbl, 1, nw)]
+    perr = np.abs(pk["power"] - ora["p1"]) / ora["p1"]
+    gap = (ora["p1"] - ora["p2"]) / ora["p1"]
+    ok = (pk["delay_idx"] == ora["idx1"]) | ((gap < 1e-5) & (pk["delay_idx"] == ora["idx2"]))
+    assert perr.max() <= 1e-4 and ok.all()
+    plan.set_cal(None)
+    _, n_off, _ = vb.fringe_search(d_raw, want_peaks=True, plan=plan)
+    assert n > n_off                                  # uncalibrated IFs do not add up
+    plan.close()
+
+
+def test_dynamic_range_after_strong_samples(vb, oracle):
+    """A 3000x burst followed by ordinary noise, then a nearly empty stretch (one surviving sample per
+    window): the running sums would carry the burst's rounding residue; the exact re-evaluation
+    (k_fixup / k_allif's direct re-sum) keeps every window within the 1e-4 bound."""
+    vis, c, _ = workloads.generate(2, nbl=1, nif=2, nap=700, npulses=2)
+    vis[0, :, 100:104] *= 3000.0
+    vis[0, 0, 300:500] = 0
+    vis[0, 0, 400, 7] = 0.3 + 0.1j
+    run_both(vb, oracle, vis, c)
+    cands, n, peaks = vb.allif_search(vis.cuda(), c["widths"], c["strides"], 512, 4.0, want_peaks=True)
+    ora = oracle.allif_search(vis.numpy(), c["widths"], c["strides"], 512)
+    nw = [workloads.gen.nwin(vis.shape[2], w, s) for w, s in zip(c["widths"], c["strides"])]
+    pk = peaks[dense_index(1, 1, nw)]
+    ok = ora["p1"] > 0
+    assert (np.abs(pk["power"][ok] - ora["p1"][ok]) / ora["p1"][ok]).max() <= 1e-4
+    assert np.all(pk["power"][~ok] == 0)
