@@ -483,3 +483,30 @@ def test_dynamic_range_after_strong_samples(vb, oracle):
     ok = ora["p1"] > 0
     assert (np.abs(pk["power"][ok] - ora["p1"][ok]) / ora["p1"][ok]).max() <= 1e-4
     assert np.all(pk["power"][~ok] == 0)
+
+
+@pytest.mark.parametrize("seed", list(range(10)))
+def test_random_shapes(vb, oracle, seed):
+    """Seeded random small problems across every kernel-selection branch (row kernels by nf, sliding /
+    column-FFT / generic rate kernels by width, stride and padding), every window compared."""
+    rng = np.random.default_rng(1000 + seed)
+    nf = int(2 ** rng.integers(3, 10))                      # 8 .. 512
+    nchan = int(rng.integers(max(1, nf // 4), nf + 1))
+    nbl, nif = int(rng.integers(1, 3)), int(rng.integers(1, 3))
+    nwid = int(rng.integers(1, 5))
+    widths, strides, nts = [], [], []
+    for _ in range(nwid):
+        w = int(rng.choice([1, 2, 3, 4, 6, 8, 16, 20, 32]))
+        pad = int(rng.choice([1, 2, 2, 2, 4]))
+        nt = 1
+        while nt < w * pad:
+            nt *= 2
+        widths.append(w); nts.append(nt)
+        strides.append(1 if rng.random() < 0.6 else int(rng.integers(1, w + 3)))
+    nap = int(rng.integers(max(widths), max(widths) + 400))
+    g = torch.Generator().manual_seed(seed)
+    vis = torch.view_as_complex(torch.randn((nbl, nif, nap, nchan, 2), generator=g) * 0.7071)
+    t0 = int(rng.integers(0, max(1, nap - 8)))
+    vis[0, 0, t0:t0 + 8] += 1.0 + 1.0j
+    c = dict(widths=widths, strides=strides, nts=nts, nf=nf, snr_thresh=3.0)
+    run_both(vb, oracle, vis, c, mode="fft")
