@@ -10,8 +10,9 @@
 // 2 s row reads per window instead of w), restarted from a direct sum every `seg` windows like
 // kernels_slide.cuh; windows with 2 s > w are summed directly.  A sample leaves a rounding residue of
 // about 6e-8 of its size in the running sum; when the window energy (from the per-AP energies, tracked
-// in double) falls below 1e-3 of the largest since the last exact sum, the window is summed directly
-// again (a uniform decision: every thread evaluates the same scalars).
+// as a float sliding sum, re-summed exactly at every restart: FP64 adds would cost more than the whole
+// step on this part) falls below 1e-3 of the largest since the last exact sum, the window is summed
+// directly again (a uniform decision: every thread evaluates the same scalars).
 // One CTA owns ALL delay columns of its windows (thread = CP column pairs, packed FP32), so the
 // argmax and the sum need no atomics: per 16 windows one barrier, fixed-order reductions, plain stores.
 #pragma once
@@ -59,11 +60,11 @@ __global__ void __launch_bounds__(1024) k_allif(AllifArgs a) {
     }
   };
   const float *Ep = a.E + (a.pair0 + pl) * (long long)a.nap;
-  double es = 0.0, esmax = 0.0;
+  float es = 0.f, esmax = 0.f;
+  auto energy = [&](int t0) { float s = 0.f; for (int t = 0; t < a.w; ++t) s += __ldg(Ep + t0 + t); return s; };
   if (slide) {
     direct(j0 * a.stride);
-    for (int t = 0; t < a.w; ++t) es += (double)__ldg(Ep + j0 * a.stride + t);
-    esmax = es;
+    es = esmax = energy(j0 * a.stride);
   }
 
   for (int jb = j0; jb < j1; jb += 16) {
@@ -71,6 +72,11 @@ __global__ void __launch_bounds__(1024) k_allif(AllifArgs a) {
     for (int b = 0; b < nst; ++b) {
       const int j = jb + b;
       if (!slide) direct(j * a.stride);
+      // energy of the NEXT window, loaded now so that the decision below does not wait on memory
+      float es_next = es;
+      if (slide && j + 1 < j1)
+        for (int t = 0; t < a.stride; ++t)
+          es_next += __ldg(Ep + j * a.stride + t + a.w) - __ldg(Ep + j * a.stride + t);
       // power, thread-local best (power bits, then lowest column) and power sum
       uint32_t pb = 0, db = 0xFFFFFFFFu;
       float ps = 0.f;
@@ -93,10 +99,10 @@ __global__ void __launch_bounds__(1024) k_allif(AllifArgs a) {
       // next window
       if (slide && j + 1 < j1) {
         const int t0 = j * a.stride;
-        for (int t = 0; t < a.stride; ++t) es += (double)__ldg(Ep + t0 + t + a.w) - (double)__ldg(Ep + t0 + t);
-        if (es < 1e-3 * esmax) {          // energy collapse: the residue of what left would dominate - sum exactly
+        es = es_next;
+        if (es < 1e-3f * esmax) {         // energy collapse: the residue of what left would dominate - sum exactly
           direct(t0 + a.stride);
-          esmax = es;
+          es = esmax = energy(t0 + a.stride);
           continue;
         }
         esmax = es > esmax ? es : esmax;

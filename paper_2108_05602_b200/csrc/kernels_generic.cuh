@@ -429,6 +429,120 @@ __global__ void __launch_bounds__(256) k_row3(RowArgs a) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// Row (delay) FFT for large nf = 4096, 8192 (the band transforms of the all-IF search): radix-16 Stockham
+// passes with the 16-point butterflies in registers (packed FFT), ONE shared buffer of nf complex used in
+// place (every thread reads its 16 inputs, barrier, writes its 16 outputs, barrier), a final radix-2 /
+// radix-1 pass... nf = 16^a * R with R in {1, 2, 4, 8}:  4096 = 16^3, 8192 = 16^3 * 2.
+// One row per CTA of nf/16 threads.  Pass with Ns = product of the earlier radices, radix R, butterfly j
+// (k = j mod Ns):  v[m] = in[j + m nf/R] W_{Ns R}^{k m};  out[(j - k) R + k + m' Ns] = DFT_R(v)[m'].
+// ------------------------------------------------------------------------------------------------
+template <int R, int NZ>
+__device__ __forceinline__ void rowbig_pass(f32x2 (&v)[16], const RowArgs &a, int j, int Ns, int nf) {
+  // twiddle W_{Ns R}^{k m} = W_nf^{k m nf/(Ns R)}, then the R-point transform; output bit-reversed
+  const int k = j & (Ns - 1);
+  if (k) {
+    const int tstep = nf / (Ns * R);
+#pragma unroll
+    for (int m = 1; m < (NZ < R ? NZ : R); ++m) {
+      const float2 tw = __ldg(a.twf + k * m * tstep);
+      v[m] = fma2(pk(-hi32(v[m]), lo32(v[m])), pk(tw.y, tw.y), mul2(v[m], pk(tw.x, tw.x)));
+    }
+  }
+  FftDif2<R, (NZ < R ? NZ : R), 0, 16>::run(v);
+}
+
+template <int NF, int NZ>
+__global__ void __launch_bounds__(NF / 16) k_rowbig(RowArgs a) {
+  constexpr int T = NF / 16;                     // threads = radix-16 butterflies per pass
+  constexpr int RL = NF == 8192 ? 2 : 1;         // last radix (8192 = 16^3 * 2)
+  extern __shared__ f32x2 rb[];                  // [NF]
+  __shared__ u64 kred[16];
+  __shared__ float ered[16];
+  const int tid = threadIdx.x;
+  const long long rrel = blockIdx.x;
+  const RowSrc src(a, a.row0 + rrel);
+  f32x2 v[16];
+  float e = 0.f;
+  // ---- pass 1 (Ns = 1): inputs straight from the slab, element tid + m T; only the first NZ of the 16 are non-zero
+#pragma unroll
+  for (int m = 0; m < NZ; ++m) {
+    const int n = tid + m * T;
+    const float2 x = n < a.nchan ? src(n) : make_float2(0.f, 0.f);
+    e += cnorm(x);
+    v[m] = c2_from(x);
+  }
+  rowbig_pass<16, NZ>(v, a, tid, 1, NF);
+#pragma unroll
+  for (int i = 0; i < 16; ++i) rb[tid * 16 + brev<16>(i)] = v[i];     // (j - k) R + k + m' Ns with Ns = 1, k = 0
+#pragma unroll
+  for (int o = 16; o >= 1; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+  if ((tid & 31) == 0) ered[tid >> 5] = e;
+  __syncthreads();
+  if (tid == 0) {
+    float s = 0.f;
+    for (int i = 0; i < T / 32; ++i) s += ered[i];
+    const long long ei = e_index(a, a.row0 + rrel);
+    if (ei >= 0) a.E[ei] = s;
+  }
+  // ---- passes 2, 3 (Ns = 16, 256): radix 16 in place
+#pragma unroll
+  for (int Ns = 16; Ns <= 256; Ns *= 16) {
+#pragma unroll
+    for (int m = 0; m < 16; ++m) v[m] = rb[tid + m * T];
+    __syncthreads();
+    rowbig_pass<16, 16>(v, a, tid, Ns, NF);
+    const int k = tid & (Ns - 1), j0 = (tid - k) * 16 + k;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) rb[j0 + brev<16>(i) * Ns] = v[i];
+    __syncthreads();
+  }
+  // ---- last pass (Ns = 4096, radix 2) for nf = 8192: 4096 butterflies, 8 per thread
+  if constexpr (RL == 2) {
+    f32x2 lo[8], hi[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { lo[q] = rb[tid + q * T]; hi[q] = rb[tid + q * T + NF / 2]; }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      const int j = tid + q * T;                 // k = j (Ns = 4096 > j), twiddle W_8192^j
+      const float2 tw = __ldg(a.twf + j);
+      const f32x2 h = fma2(pk(-hi32(hi[q]), lo32(hi[q])), pk(tw.y, tw.y), mul2(hi[q], pk(tw.x, tw.x)));
+      rb[j] = add2(lo[q], h);
+      rb[j + NF / 2] = sub2(lo[q], h);
+    }
+    __syncthreads();
+  }
+  // ---- store: pair-interleaved float4 rows, the w = 1 peak
+  u64 key = 0;
+  float4 *dst = (float4 *)(a.Y + rrel * (long long)a.pitch);
+  for (int c = tid; c < NF / 2; c += T) {
+    const f32x2 z0 = rb[2 * c], z1 = rb[2 * c + 1];
+    const float4 q = make_float4(lo32(z0), lo32(z1), hi32(z0), hi32(z1));
+    dst[c] = q;
+    const u64 k0 = make_key(fmaf(q.x, q.x, q.z * q.z), (uint32_t)(2 * c)), k1 = make_key(fmaf(q.y, q.y, q.w * q.w), (uint32_t)(2 * c + 1));
+    key = k0 > key ? k0 : key;
+    key = k1 > key ? k1 : key;
+  }
+  if (a.keys1) {   // uniform branch
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) {
+      const u64 other = __shfl_xor_sync(0xffffffffu, key, o);
+      key = other > key ? other : key;
+    }
+    if ((tid & 31) == 0) kred[tid >> 5] = key;
+    __syncthreads();
+    if (tid == 0) {
+      for (int i = 0; i < T / 32; ++i) key = kred[i] > key ? kred[i] : key;
+      const long long row = a.row0 + rrel;
+      const long long pair = row / a.nap;
+      const int t = (int)(row - pair * a.nap);
+      const int jw = t / a.stride1;
+      if (jw * a.stride1 == t && jw < a.nwin1) a.keys1[pair * a.per_pair + jw] = key;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Column (rate) transform + power + argmax, generic.
 // Thread task id (d fastest): ((pair_local * nwin + j) * M + rho) * nf + d.
 // ------------------------------------------------------------------------------------------------

@@ -121,6 +121,29 @@ static bool row3_nz(const RowArgs &a, int nza, cudaStream_t st) {
   return false;
 }
 
+template <int NF>
+static bool rowbig_nz(const RowArgs &a, int nz, cudaStream_t st, bool attr_only) {
+  const unsigned blocks = (unsigned)a.nrows;
+  const size_t smem = (size_t)NF * sizeof(float2);
+#define VOLKS_ROWBIG(NZ_)                                                                                        \
+  case NZ_:                                                                                                      \
+    if (attr_only) return cudaFuncSetAttribute(k_rowbig<NF, NZ_>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
+                                               (int)smem) == cudaSuccess;                                        \
+    k_rowbig<NF, NZ_><<<blocks, NF / 16, smem, st>>>(a);                                                         \
+    return true;
+  switch (nz) { VOLKS_ROWBIG(1) VOLKS_ROWBIG(2) VOLKS_ROWBIG(4) VOLKS_ROWBIG(8) VOLKS_ROWBIG(16) }
+#undef VOLKS_ROWBIG
+  return false;
+}
+
+// radix-16 row FFT for nf = 4096 / 8192 (k_rowbig); attr_only: raise its dynamic shared memory limit
+static bool launch_rowbig(const RowArgs &a, cudaStream_t st, bool attr_only) {
+  if (!a.paired || (a.nf != 4096 && a.nf != 8192) || a.nrows >= (1LL << 31)) return false;
+  int nz = 1;
+  while (nz * (a.nf / 16) < a.nchan) nz *= 2;
+  return a.nf == 4096 ? rowbig_nz<4096>(a, nz, st, attr_only) : rowbig_nz<8192>(a, nz, st, attr_only);
+}
+
 // register-form row FFT for nf in {64, 128, 256} (k_row2) and {512 .. 2048} (k_row3) with the paired Y
 // layout; false = not applicable
 static bool launch_row2(const RowArgs &a, cudaStream_t st) {
@@ -383,6 +406,11 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
       ok = cuda_ok(launch_colfft(ca, w.cf_l1, w.cf_nz, 0, nullptr, true));
     }
   ok = ok && cuda_ok(cudaFuncSetAttribute(k_slide<16, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+  if (ok && (p->nf == 4096 || p->nf == 8192)) {
+    RowArgs ra; memset(&ra, 0, sizeof ra);
+    ra.paired = pl->paired; ra.nf = p->nf; ra.nchan = p->nchan; ra.nrows = 1;
+    launch_rowbig(ra, nullptr, true);
+  }
   if (!ok) { volks_plan_destroy(pl); return VOLKS_ECUDA; }
   *out = pl;
   return VOLKS_OK;
@@ -523,7 +551,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
     const long long rblocks = (ra.nrows + ra.rows_per_cta - 1) / ra.rows_per_cta;
     {
       ProfScope ps(pl, st, VOLKS_K_ROW, -1);
-      if (pl->row_generic || !launch_row2(ra, st))
+      if (pl->row_generic || !(launch_row2(ra, st) || launch_rowbig(ra, st, false)))
         k_row_fft<<<(unsigned)rblocks, ra.tpr * ra.rows_per_cta, pl->row_smem, st>>>(ra);
       if (d_stage && !cuda_ok(cudaEventRecord(pl->ev_free[ch & 1], st))) return VOLKS_ECUDA;
     }
