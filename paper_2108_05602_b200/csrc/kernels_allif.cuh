@@ -13,8 +13,10 @@
 // as a float sliding sum, re-summed exactly at every restart: FP64 adds would cost more than the whole
 // step on this part) falls below 1e-3 of the largest since the last exact sum, the window is summed
 // directly again (a uniform decision: every thread evaluates the same scalars).
-// One CTA owns ALL delay columns of its windows (thread = CP column pairs, packed FP32), so the
-// argmax and the sum need no atomics: per 16 windows one barrier, fixed-order reductions, plain stores.
+// A CTA owns all delay columns of its windows (thread = CP column pairs, packed FP32) - or, beyond 8192
+// columns, one of the `gsplit` interleaved sub-rows of 8192: per 16 windows one barrier and fixed-order reductions;
+// the parts' keys meet in an atomicMax (exact, order-free), their power sums in `gsplit` slots per
+// window that the finalize adds in order (deterministic).
 #pragma once
 #include "common.cuh"
 
@@ -29,18 +31,24 @@ struct AllifArgs {
   const float *E;       // per-AP band energies [npairs_total][nap] (row kernel): detects energy collapse
   long long per_pair, offc, pair0;
   int nap, nf, w, stride, nwin, seg, nseg, pitch;
-  int psub, nfb;        // nf = psub * nfb: column c of a row is sub-row rho = c / nfb, d' = c % nfb, delay d = psub d' + rho
+  int gsplit;           // nfa > 8192: nf = gsplit * 8192, column c of a row is sub-row rho = c / 8192, d' = c % 8192,
+                        // delay d = gsplit d' + rho; one CTA per (baseline, segment, sub-row) (CP = 4);
+                        // keys combine by atomicMax, the noise as gsplit partial sums added in order by the finalize
 };
 
-// CP = column pairs per thread (nf / 2 / blockDim.x)
-template <int CP>
+// CP = column pairs per thread (nf / gsplit / 2 / blockDim.x); SPLIT = (gsplit > 1), a compile-time switch
+// so that the one-CTA form keeps its shorter address arithmetic
+template <int CP, bool SPLIT>
 __global__ void __launch_bounds__(1024) k_allif(AllifArgs a) {
   __shared__ u64 kslot[16][AI_MAXWARPS];
   __shared__ float sslot[16][AI_MAXWARPS];
   const int nwarps = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int sg = blockIdx.x % a.nseg;
-  const long long pl = blockIdx.x / a.nseg;
-  const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch);
+  const int gs = SPLIT ? a.gsplit : 1;
+  const int gpart = SPLIT ? blockIdx.x % gs : 0;
+  const int sg = (blockIdx.x / gs) % a.nseg;
+  const long long pl = blockIdx.x / (gs * a.nseg);
+  const uint32_t pair_base = SPLIT ? (uint32_t)gpart * (uint32_t)(a.nf / 2 / gs) : 0u;   // first column pair of this part
+  const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch) + (size_t)pair_base * 16u;
   const size_t rowb = (size_t)a.pitch * 8u;
   const long long c0 = (a.pair0 + pl) * a.per_pair + a.offc;
   const int j0 = sg * a.seg, j1 = min(a.nwin, j0 + a.seg);
@@ -83,9 +91,9 @@ __global__ void __launch_bounds__(1024) k_allif(AllifArgs a) {
 #pragma unroll
       for (int i = 0; i < CP; ++i) {
         const f32x2 pw = fma2(AY[i], AY[i], mul2(AX[i], AX[i]));
-        const uint32_t c0l = 2u * (uint32_t)(threadIdx.x + i * blockDim.x);       // linear column of the pair
-        const uint32_t rho = c0l / (uint32_t)a.nfb, dp = c0l - rho * (uint32_t)a.nfb;
-        const uint32_t d0 = dp * (uint32_t)a.psub + rho, d1 = d0 + (uint32_t)a.psub;  // true delay bins (d' and d'+1)
+        // true delay bins of the pair (d' and d' + 1 of sub-row rho = gpart: d = psub d' + rho)
+        const uint32_t dp = 2u * (uint32_t)(threadIdx.x + i * blockDim.x);
+        const uint32_t d0 = SPLIT ? dp * (uint32_t)gs + (uint32_t)gpart : dp, d1 = d0 + (uint32_t)gs;
         const uint32_t p0 = __float_as_uint(lo32(pw)), p1 = __float_as_uint(hi32(pw));
         if (p0 > pb || (p0 == pb && d0 < db)) { pb = p0; db = d0; }
         if (p1 > pb || (p1 == pb && d1 < db)) { pb = p1; db = d1; }
@@ -119,15 +127,16 @@ __global__ void __launch_bounds__(1024) k_allif(AllifArgs a) {
       }
     }
     __syncthreads();
-    if (threadIdx.x < nst) {
+    if (threadIdx.x < nst) {      // (a warp-per-window shuffle tree here measured slower: 6.6 -> 7.1 ms per width)
       u64 k = kslot[threadIdx.x][0];
       float s = sslot[threadIdx.x][0];
       for (int i = 1; i < nwarps; ++i) {
         k = kslot[threadIdx.x][i] > k ? kslot[threadIdx.x][i] : k;
         s += sslot[threadIdx.x][i];
       }
-      a.keys[c0 + jb + threadIdx.x] = k;
-      a.noise[c0 + jb + threadIdx.x] = s / (float)a.nf;
+      if (!SPLIT) a.keys[c0 + jb + threadIdx.x] = k;
+      else atomicMax(a.keys + c0 + jb + threadIdx.x, k);
+      a.noise[(c0 + jb + threadIdx.x) * gs + gpart] = s / (float)a.nf;
     }
     __syncthreads();
   }

@@ -619,6 +619,7 @@ __global__ void __launch_bounds__(256) k_col(ColArgs a) {
 struct Sched {   // the window schedule (device copy lives in the plan)
   int nwidths, nbl, nif, nap, nf, log2nf;
   int allif;              // f2: one delay across all IFs (pairs = baselines; records carry ifq = -1)
+  int ngs;                // f2: partial noise sums per window (k_allif's gsplit), 1 otherwise
   float snr_thresh;
   long long per_pair, nwin_total;
   int width[16], stride[16], nt[16];
@@ -652,7 +653,8 @@ __device__ __forceinline__ WinStat window_stat(const Sched &s, const u64 *keys, 
   const float *e = E + o.pair * s.nap + o.t0;
   float es = 0.f;
   for (int t = 0; t < s.width[q]; ++t) es += e[t];
-  const float nz = noise ? noise[c] : es;
+  float nz = es;
+  if (noise) { nz = 0.f; for (int g = 0; g < s.ngs; ++g) nz += noise[c * s.ngs + g]; }
   o.snr = (es > 0.f && nz > 0.f) ? sqrtf(o.power / nz) : 0.f;
   // an all-zero window (flagged data, the zero fill of dedispersion) has an identically zero plane:
   // P1 = 0 at (0, 0) by the tie rule.  The sliding sum would leave rounding residue of earlier samples

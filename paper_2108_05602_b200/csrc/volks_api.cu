@@ -293,6 +293,9 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   pl->nchan = p->nchan;
   pl->npair = (long long)p->nbl * p->nif;
   pl->ai_nif = ai_nif; pl->ai_nchan = ai_nchan; s.allif = allif ? 1 : 0;
+  // k_allif: one CTA per sub-row of 8192 delay columns (CP = 4 pairs per thread, no spills); measured on config 5
+  // (nfa 32768): 4096 -> 8.1 ms per width, 8192 -> 7.0, 16384 -> 7.0-7.7, one CTA (CP = 16, spills) 15-16
+  s.ngs = allif ? psub : 1;
   long long per_pair = 0;
   size_t tw_total = (size_t)p->nf;
   const bool force_generic = env_is("VOLKS_PATH", "generic");
@@ -362,7 +365,7 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   pl->off_E = off;    off = align_up(off + (size_t)std::max<long long>(pl->npair * p->nap, 1) * sizeof(float), 256);
   pl->off_cnt = off;  off = align_up(off + (size_t)std::max<long long>(pl->nfin_blocks, 1) * sizeof(uint32_t), 256);
   // + padding rows: the sliding kernel loads one row, and prefetches SLIDE_PF + 1 rows, past the last sample
-  pl->off_noise = off; off = align_up(off + (allif ? (size_t)std::max<long long>(s.nwin_total, 1) * sizeof(float) : 0), 256);
+  pl->off_noise = off; off = align_up(off + (allif ? (size_t)std::max<long long>(s.nwin_total, 1) * s.ngs * sizeof(float) : 0), 256);
   pl->off_zst = off;  off = align_up(off + (size_t)std::max<long long>(pl->npair * p->nwidths, 1) * sizeof(double2), 256);
   pl->off_Y = off;    off = align_up(off + (size_t)pl->pairs_per_chunk * std::max<size_t>(y_pair, 8) + (size_t)(SLIDE_PF + 2) * pl->pitch * sizeof(float2), 256);
   pl->ws_bytes = off;
@@ -569,15 +572,16 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         aa.Y = Y; aa.keys = keys; aa.noise = (float *)(ws + pl->off_noise); aa.E = E;
         aa.per_pair = s.per_pair; aa.offc = s.offc[q]; aa.pair0 = pair0;
         aa.nap = s.nap; aa.nf = s.nf; aa.w = w.w; aa.stride = w.s; aa.nwin = (int)w.nwin; aa.seg = w.seg;
-        aa.nseg = w.nseg; aa.pitch = pl->pitch * pl->ai_psub; aa.psub = pl->ai_psub; aa.nfb = pl->row_nf;
-        const int thr = std::min(1024, s.nf / 2), cp = s.nf / 2 / thr;
-        const unsigned blocks = (unsigned)(np * w.nseg);
+        aa.nseg = w.nseg; aa.pitch = pl->pitch * pl->ai_psub;
+        aa.gsplit = s.ngs;
+        const int cols = s.nf / s.ngs;                               // columns per CTA
+        const int thr = std::min(1024, cols / 2), cp = cols / 2 / thr;
+        const unsigned blocks = (unsigned)(np * w.nseg * s.ngs);
         ProfScope ps(pl, st, VOLKS_K_ALLIF, q);
-        if (cp == 1) k_allif<1><<<blocks, thr, 0, st>>>(aa);
-        else if (cp == 2) k_allif<2><<<blocks, thr, 0, st>>>(aa);
-        else if (cp == 4) k_allif<4><<<blocks, thr, 0, st>>>(aa);
-        else if (cp == 8) k_allif<8><<<blocks, thr, 0, st>>>(aa);
-        else k_allif<16><<<blocks, thr, 0, st>>>(aa);
+        if (s.ngs > 1) k_allif<4, true><<<blocks, thr, 0, st>>>(aa);   // cols = 8192
+        else if (cp == 1) k_allif<1, false><<<blocks, thr, 0, st>>>(aa);
+        else if (cp == 2) k_allif<2, false><<<blocks, thr, 0, st>>>(aa);
+        else k_allif<4, false><<<blocks, thr, 0, st>>>(aa);
         continue;
       }
       if (w.slide) {
