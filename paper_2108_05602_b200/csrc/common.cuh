@@ -90,6 +90,11 @@ __device__ __forceinline__ f32x2 c2_mulnegi(f32x2 z) { return pk(hi32(z), -lo32(
 // z * (c - i s) for real constants c, s:  (x c + y s, y c - x s)
 __device__ __forceinline__ f32x2 c2_mulcs(f32x2 z, float c, float s) { return fma2(c2_mulnegi(z), pk(s, s), mul2(z, pk(c, c))); }
 
+// z * w, both packed (re, im):  z wx + (-zy, zx) wy
+__device__ __forceinline__ f32x2 c2_mul(f32x2 z, f32x2 w) {
+  return fma2(pk(-hi32(z), lo32(z)), pk(hi32(w), hi32(w)), mul2(z, pk(lo32(w), lo32(w))));
+}
+
 // z * exp(-2 pi i K/N), N in {2,4,8,16,32}, 0 <= K < N/2, compile time
 template <int K, int N>
 __device__ __forceinline__ f32x2 c2_mul_w(f32x2 z) {

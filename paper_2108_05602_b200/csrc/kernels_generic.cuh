@@ -96,6 +96,68 @@ struct RowSrc {
     const float2 v = fetch(k);
     return calrow ? cmul(v, __ldg(calrow + k)) : v;
   }
+  // The NZ elements k = k0 + m step (m < NZ) of the row, zero from `kmax` on (k_rowbig).  Same values as
+  // operator(), but branch-free and without a division per element (the IF index and channel of k advance
+  // by step / ai_nchan and step % ai_nchan), so that the NZ shift loads, then the NZ data loads, are all in
+  // flight together instead of one dependent chain after another.
+  template <int NZ>
+  __device__ __forceinline__ void load_strided(int k0, int step, int kmax, float2 (&x)[NZ]) const {
+    if (!gather) {
+#pragma unroll
+      for (int m = 0; m < NZ; ++m) {
+        const int k = k0 + m * step;
+        x[m] = k < kmax ? __ldg(base + k) : make_float2(0.f, 0.f);
+      }
+      return;
+    }
+    // (the mode tests below are uniform branches around whole loops, not per-element predicates)
+    int ts[NZ];
+    if (sh) {
+#pragma unroll
+      for (int m = 0; m < NZ; ++m) {
+        const int k = k0 + m * step;
+        ts[m] = t + __ldg(sh + (k < kmax ? k : 0));
+      }
+    } else {
+#pragma unroll
+      for (int m = 0; m < NZ; ++m) ts[m] = t;
+    }
+    const float2 *p[NZ];      // nullptr = zero
+    if (ai_nchan) {
+      int n = k0 / ai_nchan, j = k0 - n * ai_nchan;
+      const int dq = step / ai_nchan, dr = step - dq * ai_nchan;
+#pragma unroll
+      for (int m = 0; m < NZ; ++m) {
+        const bool ok = k0 + m * step < kmax && (unsigned)ts[m] < (unsigned)nap;
+        p[m] = ok ? base + (long long)(n * nap + ts[m]) * ai_nchan + j : nullptr;
+        n += dq; j += dr;
+        if (j >= ai_nchan) { j -= ai_nchan; ++n; }
+      }
+    } else {
+#pragma unroll
+      for (int m = 0; m < NZ; ++m) {
+        const int k = k0 + m * step;
+        const bool ok = k < kmax && (unsigned)ts[m] < (unsigned)nap;
+        p[m] = ok ? base + (long long)ts[m] * nchan + k : nullptr;
+      }
+    }
+#pragma unroll
+    for (int m = 0; m < NZ; ++m) x[m] = p[m] ? __ldg(p[m]) : make_float2(0.f, 0.f);
+    if (rho) {
+      // premodulation W^{k rho} = W^{k0 rho} W^{m step rho}: one strided table read per thread, the other
+      // factor is the same address in every thread (a broadcast)
+      const float2 pm0 = __ldg(premod + k0 * rho);
+#pragma unroll
+      for (int m = 0; m < NZ; ++m) x[m] = cmul(x[m], cmul(pm0, __ldg(premod + m * step * rho)));
+    }
+    if (calrow) {
+#pragma unroll
+      for (int m = 0; m < NZ; ++m) {
+        const int k = k0 + m * step;
+        x[m] = cmul(x[m], __ldg(calrow + (k < kmax ? k : 0)));
+      }
+    }
+  }
 };
 
 __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
@@ -433,29 +495,38 @@ __global__ void __launch_bounds__(256) k_row3(RowArgs a) {
 // passes with the 16-point butterflies in registers (packed FFT), ONE shared buffer of nf complex used in
 // place (every thread reads its 16 inputs, barrier, writes its 16 outputs, barrier), a final radix-2 /
 // radix-1 pass... nf = 16^a * R with R in {1, 2, 4, 8}:  4096 = 16^3, 8192 = 16^3 * 2.
+// The buffer is padded by one element per 16 (index p -> p + p/16, RBI): the first pass stores 16
+// consecutive elements per thread, which would otherwise be a 16-way bank conflict.
 // One row per CTA of nf/16 threads.  Pass with Ns = product of the earlier radices, radix R, butterfly j
 // (k = j mod Ns):  v[m] = in[j + m nf/R] W_{Ns R}^{k m};  out[(j - k) R + k + m' Ns] = DFT_R(v)[m'].
 // ------------------------------------------------------------------------------------------------
-template <int R, int NZ>
+#define RBI(p) ((p) + ((p) >> 4))
+template <int NZ, bool TW>
 __device__ __forceinline__ void rowbig_pass(f32x2 (&v)[16], const RowArgs &a, int j, int Ns, int nf) {
-  // twiddle W_{Ns R}^{k m} = W_nf^{k m nf/(Ns R)}, then the R-point transform; output bit-reversed
-  const int k = j & (Ns - 1);
-  if (k) {
-    const int tstep = nf / (Ns * R);
-#pragma unroll
-    for (int m = 1; m < (NZ < R ? NZ : R); ++m) {
-      const float2 tw = __ldg(a.twf + k * m * tstep);
-      v[m] = fma2(pk(-hi32(v[m]), lo32(v[m])), pk(tw.y, tw.y), mul2(v[m], pk(tw.x, tw.x)));
-    }
+  // twiddles W_{16 Ns}^{k m} = W_nf^{k m nf/(16 Ns)} (m < 16; none in the first pass, k = 0), then the
+  // 16-point transform; output bit-reversed.  Only m = 1, 2, 4, 8 come from the table (lanes read it with a
+  // stride of m entries: 15 loads per thread were 60 % of this kernel's L1 traffic); the others are products
+  // of at most three of them.
+  if constexpr (TW) {
+    static_assert(NZ == 16, "later passes are dense");
+    const int ts = (j & (Ns - 1)) * (nf / (Ns * 16));
+    const f32x2 w1 = c2_from(__ldg(a.twf + ts)), w2 = c2_from(__ldg(a.twf + 2 * ts));
+    const f32x2 w4 = c2_from(__ldg(a.twf + 4 * ts)), w8 = c2_from(__ldg(a.twf + 8 * ts));
+    const f32x2 w3 = c2_mul(w2, w1), w5 = c2_mul(w4, w1), w6 = c2_mul(w4, w2), w7 = c2_mul(w4, w3);
+    v[1] = c2_mul(v[1], w1); v[2] = c2_mul(v[2], w2); v[3] = c2_mul(v[3], w3); v[4] = c2_mul(v[4], w4);
+    v[5] = c2_mul(v[5], w5); v[6] = c2_mul(v[6], w6); v[7] = c2_mul(v[7], w7); v[8] = c2_mul(v[8], w8);
+    v[9] = c2_mul(v[9], c2_mul(w8, w1)); v[10] = c2_mul(v[10], c2_mul(w8, w2)); v[11] = c2_mul(v[11], c2_mul(w8, w3));
+    v[12] = c2_mul(v[12], c2_mul(w8, w4)); v[13] = c2_mul(v[13], c2_mul(w8, w5)); v[14] = c2_mul(v[14], c2_mul(w8, w6));
+    v[15] = c2_mul(v[15], c2_mul(w8, w7));
   }
-  FftDif2<R, (NZ < R ? NZ : R), 0, 16>::run(v);
+  FftDif2<16, NZ, 0, 16>::run(v);
 }
 
 template <int NF, int NZ>
-__global__ void __launch_bounds__(NF / 16) k_rowbig(RowArgs a) {
+__global__ void __launch_bounds__(NF / 16, 2) k_rowbig(RowArgs a) {
   constexpr int T = NF / 16;                     // threads = radix-16 butterflies per pass
   constexpr int RL = NF == 8192 ? 2 : 1;         // last radix (8192 = 16^3 * 2)
-  extern __shared__ f32x2 rb[];                  // [NF]
+  extern __shared__ f32x2 rb[];                  // [NF + NF/16]
   __shared__ u64 kred[16];
   __shared__ float ered[16];
   const int tid = threadIdx.x;
@@ -464,16 +535,15 @@ __global__ void __launch_bounds__(NF / 16) k_rowbig(RowArgs a) {
   f32x2 v[16];
   float e = 0.f;
   // ---- pass 1 (Ns = 1): inputs straight from the slab, element tid + m T; only the first NZ of the 16 are non-zero
+  {
+    float2 x[NZ];
+    src.template load_strided<NZ>(tid, T, a.nchan, x);
 #pragma unroll
-  for (int m = 0; m < NZ; ++m) {
-    const int n = tid + m * T;
-    const float2 x = n < a.nchan ? src(n) : make_float2(0.f, 0.f);
-    e += cnorm(x);
-    v[m] = c2_from(x);
+    for (int m = 0; m < NZ; ++m) { e += cnorm(x[m]); v[m] = c2_from(x[m]); }
   }
-  rowbig_pass<16, NZ>(v, a, tid, 1, NF);
+  rowbig_pass<NZ, false>(v, a, tid, 1, NF);
 #pragma unroll
-  for (int i = 0; i < 16; ++i) rb[tid * 16 + brev<16>(i)] = v[i];     // (j - k) R + k + m' Ns with Ns = 1, k = 0
+  for (int i = 0; i < 16; ++i) rb[RBI(tid * 16 + brev<16>(i))] = v[i];     // (j - k) R + k + m' Ns with Ns = 1, k = 0
 #pragma unroll
   for (int o = 16; o >= 1; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
   if ((tid & 31) == 0) ered[tid >> 5] = e;
@@ -488,27 +558,27 @@ __global__ void __launch_bounds__(NF / 16) k_rowbig(RowArgs a) {
 #pragma unroll
   for (int Ns = 16; Ns <= 256; Ns *= 16) {
 #pragma unroll
-    for (int m = 0; m < 16; ++m) v[m] = rb[tid + m * T];
+    for (int m = 0; m < 16; ++m) v[m] = rb[RBI(tid + m * T)];
     __syncthreads();
-    rowbig_pass<16, 16>(v, a, tid, Ns, NF);
+    rowbig_pass<16, true>(v, a, tid, Ns, NF);
     const int k = tid & (Ns - 1), j0 = (tid - k) * 16 + k;
 #pragma unroll
-    for (int i = 0; i < 16; ++i) rb[j0 + brev<16>(i) * Ns] = v[i];
+    for (int i = 0; i < 16; ++i) rb[RBI(j0 + brev<16>(i) * Ns)] = v[i];
     __syncthreads();
   }
   // ---- last pass (Ns = 4096, radix 2) for nf = 8192: 4096 butterflies, 8 per thread
   if constexpr (RL == 2) {
     f32x2 lo[8], hi[8];
 #pragma unroll
-    for (int q = 0; q < 8; ++q) { lo[q] = rb[tid + q * T]; hi[q] = rb[tid + q * T + NF / 2]; }
+    for (int q = 0; q < 8; ++q) { lo[q] = rb[RBI(tid + q * T)]; hi[q] = rb[RBI(tid + q * T + NF / 2)]; }
     __syncthreads();
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
       const int j = tid + q * T;                 // k = j (Ns = 4096 > j), twiddle W_8192^j
       const float2 tw = __ldg(a.twf + j);
       const f32x2 h = fma2(pk(-hi32(hi[q]), lo32(hi[q])), pk(tw.y, tw.y), mul2(hi[q], pk(tw.x, tw.x)));
-      rb[j] = add2(lo[q], h);
-      rb[j + NF / 2] = sub2(lo[q], h);
+      rb[RBI(j)] = add2(lo[q], h);
+      rb[RBI(j + NF / 2)] = sub2(lo[q], h);
     }
     __syncthreads();
   }
@@ -516,12 +586,14 @@ __global__ void __launch_bounds__(NF / 16) k_rowbig(RowArgs a) {
   u64 key = 0;
   float4 *dst = (float4 *)(a.Y + rrel * (long long)a.pitch);
   for (int c = tid; c < NF / 2; c += T) {
-    const f32x2 z0 = rb[2 * c], z1 = rb[2 * c + 1];
+    const f32x2 z0 = rb[RBI(2 * c)], z1 = rb[RBI(2 * c + 1)];
     const float4 q = make_float4(lo32(z0), lo32(z1), hi32(z0), hi32(z1));
     dst[c] = q;
-    const u64 k0 = make_key(fmaf(q.x, q.x, q.z * q.z), (uint32_t)(2 * c)), k1 = make_key(fmaf(q.y, q.y, q.w * q.w), (uint32_t)(2 * c + 1));
-    key = k0 > key ? k0 : key;
-    key = k1 > key ? k1 : key;
+    if (a.keys1) {   // uniform
+      const u64 k0 = make_key(fmaf(q.x, q.x, q.z * q.z), (uint32_t)(2 * c)), k1 = make_key(fmaf(q.y, q.y, q.w * q.w), (uint32_t)(2 * c + 1));
+      key = k0 > key ? k0 : key;
+      key = k1 > key ? k1 : key;
+    }
   }
   if (a.keys1) {   // uniform branch
 #pragma unroll

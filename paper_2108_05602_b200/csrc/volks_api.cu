@@ -124,7 +124,7 @@ static bool row3_nz(const RowArgs &a, int nza, cudaStream_t st) {
 template <int NF>
 static bool rowbig_nz(const RowArgs &a, int nz, cudaStream_t st, bool attr_only) {
   const unsigned blocks = (unsigned)a.nrows;
-  const size_t smem = (size_t)NF * sizeof(float2);
+  const size_t smem = (size_t)(NF + NF / 16) * sizeof(float2);   // padded, RBI in kernels_generic.cuh
 #define VOLKS_ROWBIG(NZ_)                                                                                        \
   case NZ_:                                                                                                      \
     if (attr_only) return cudaFuncSetAttribute(k_rowbig<NF, NZ_>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
