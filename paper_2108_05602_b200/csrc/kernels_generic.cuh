@@ -11,6 +11,7 @@
 //   a_rho[t2]    = sum_{t1: t2+L t1 < w} y[t0 + t2 + L t1] e^{-2 pi i rho (t2 + L t1)/Nt}
 // so one thread folds the w samples of its column into L registers and runs an L-point FFT there.
 #pragma once
+#include <type_traits>
 #include "common.cuh"
 
 namespace volks {
@@ -313,11 +314,7 @@ __global__ void __launch_bounds__(256) k_row2(RowArgs a) {
         v[n2] = (live && n < a.nchan) ? __ldg(src.base + n) : make_float2(0.f, 0.f);
       }
     } else {
-#pragma unroll
-      for (int n2 = 0; n2 < NZA; ++n2) {
-        const int n = l + N1 * n2;
-        v[n2] = (live && n < a.nchan) ? src(n) : make_float2(0.f, 0.f);
-      }
+      src.template load_strided<NZA>(l, N1, live ? a.nchan : 0, v);
     }
 #pragma unroll
     for (int n2 = 0; n2 < NZA; ++n2) { e += cnorm(v[n2]); z[n2] = c2_from(v[n2]); }
@@ -401,11 +398,7 @@ __global__ void __launch_bounds__(256) k_row3(RowArgs a) {
         v[n3] = n < a.nchan ? __ldg(src.base + n) : make_float2(0.f, 0.f);
       }
     } else {
-#pragma unroll
-      for (int n3 = 0; n3 < NZA; ++n3) {
-        const int n = tid + 256 * n3;
-        v[n3] = n < a.nchan ? src(n) : make_float2(0.f, 0.f);
-      }
+      src.template load_strided<NZA>(tid, 256, a.nchan, v);
     }
 #pragma unroll
     for (int n3 = 0; n3 < NZA; ++n3) { e += cnorm(v[n3]); z[n3] = c2_from(v[n3]); }
@@ -504,14 +497,14 @@ __global__ void __launch_bounds__(256) k_row3(RowArgs a) {
 template <int NZ, bool TW>
 __device__ __forceinline__ void rowbig_pass(f32x2 (&v)[16], const RowArgs &a, int j, int Ns, int nf) {
   // twiddles W_{16 Ns}^{k m} = W_nf^{k m nf/(16 Ns)} (m < 16; none in the first pass, k = 0), then the
-  // 16-point transform; output bit-reversed.  Only m = 1, 2, 4, 8 come from the table (lanes read it with a
+  // 16-point transform; output bit-reversed.  Only m = 1 and 4 come from the table (lanes read it with a
   // stride of m entries: 15 loads per thread were 60 % of this kernel's L1 traffic); the others are products
-  // of at most three of them.
+  // of at most four of them.
   if constexpr (TW) {
     static_assert(NZ == 16, "later passes are dense");
     const int ts = (j & (Ns - 1)) * (nf / (Ns * 16));
-    const f32x2 w1 = c2_from(__ldg(a.twf + ts)), w2 = c2_from(__ldg(a.twf + 2 * ts));
-    const f32x2 w4 = c2_from(__ldg(a.twf + 4 * ts)), w8 = c2_from(__ldg(a.twf + 8 * ts));
+    const f32x2 w1 = c2_from(__ldg(a.twf + ts)), w4 = c2_from(__ldg(a.twf + 4 * ts));
+    const f32x2 w2 = c2_mul(w1, w1), w8 = c2_mul(w4, w4);
     const f32x2 w3 = c2_mul(w2, w1), w5 = c2_mul(w4, w1), w6 = c2_mul(w4, w2), w7 = c2_mul(w4, w3);
     v[1] = c2_mul(v[1], w1); v[2] = c2_mul(v[2], w2); v[3] = c2_mul(v[3], w3); v[4] = c2_mul(v[4], w4);
     v[5] = c2_mul(v[5], w5); v[6] = c2_mul(v[6], w6); v[7] = c2_mul(v[7], w7); v[8] = c2_mul(v[8], w8);
@@ -566,27 +559,10 @@ __global__ void __launch_bounds__(NF / 16, 2) k_rowbig(RowArgs a) {
     for (int i = 0; i < 16; ++i) rb[RBI(j0 + brev<16>(i) * Ns)] = v[i];
     __syncthreads();
   }
-  // ---- last pass (Ns = 4096, radix 2) for nf = 8192: 4096 butterflies, 8 per thread
-  if constexpr (RL == 2) {
-    f32x2 lo[8], hi[8];
-#pragma unroll
-    for (int q = 0; q < 8; ++q) { lo[q] = rb[RBI(tid + q * T)]; hi[q] = rb[RBI(tid + q * T + NF / 2)]; }
-    __syncthreads();
-#pragma unroll
-    for (int q = 0; q < 8; ++q) {
-      const int j = tid + q * T;                 // k = j (Ns = 4096 > j), twiddle W_8192^j
-      const float2 tw = __ldg(a.twf + j);
-      const f32x2 h = fma2(pk(-hi32(hi[q]), lo32(hi[q])), pk(tw.y, tw.y), mul2(hi[q], pk(tw.x, tw.x)));
-      rb[RBI(j)] = add2(lo[q], h);
-      rb[RBI(j + NF / 2)] = sub2(lo[q], h);
-    }
-    __syncthreads();
-  }
   // ---- store: pair-interleaved float4 rows, the w = 1 peak
   u64 key = 0;
   float4 *dst = (float4 *)(a.Y + rrel * (long long)a.pitch);
-  for (int c = tid; c < NF / 2; c += T) {
-    const f32x2 z0 = rb[RBI(2 * c)], z1 = rb[RBI(2 * c + 1)];
+  auto emit = [&](int c, f32x2 z0, f32x2 z1) {   // columns 2c, 2c + 1
     const float4 q = make_float4(lo32(z0), lo32(z1), hi32(z0), hi32(z1));
     dst[c] = q;
     if (a.keys1) {   // uniform
@@ -594,6 +570,25 @@ __global__ void __launch_bounds__(NF / 16, 2) k_rowbig(RowArgs a) {
       key = k0 > key ? k0 : key;
       key = k1 > key ? k1 : key;
     }
+  };
+  if constexpr (RL == 2) {
+    // last pass (Ns = 4096, radix 2) for nf = 8192, fused with the store: out[j] = lo[j] + W_8192^j hi[j],
+    // out[j + 4096] = lo[j] - W_8192^j hi[j].  Thread: column pairs c = tid + 512 q (q < 4), j = 2c, 2c + 1;
+    // W^{2c} = W^{2 tid} W_8^q: two table reads per thread, the W_8^q are compile-time constants.
+    const f32x2 wa = c2_from(__ldg(a.twf + 2 * tid)), wb = c2_from(__ldg(a.twf + 2 * tid + 1));
+    auto last = [&](auto qc) {
+      constexpr int q = decltype(qc)::value;
+      const int c = tid + q * T;
+      const f32x2 lo0 = rb[RBI(2 * c)], lo1 = rb[RBI(2 * c + 1)];
+      const f32x2 h0 = c2_mul(rb[RBI(2 * c + NF / 2)], c2_mul_w<q, 8>(wa));
+      const f32x2 h1 = c2_mul(rb[RBI(2 * c + 1 + NF / 2)], c2_mul_w<q, 8>(wb));
+      emit(c, add2(lo0, h0), add2(lo1, h1));
+      emit(c + NF / 4, sub2(lo0, h0), sub2(lo1, h1));
+    };
+    last(std::integral_constant<int, 0>{}); last(std::integral_constant<int, 1>{});
+    last(std::integral_constant<int, 2>{}); last(std::integral_constant<int, 3>{});
+  } else {
+    for (int c = tid; c < NF / 2; c += T) emit(c, rb[RBI(2 * c)], rb[RBI(2 * c + 1)]);
   }
   if (a.keys1) {   // uniform branch
 #pragma unroll
