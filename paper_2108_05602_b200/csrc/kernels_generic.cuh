@@ -721,7 +721,8 @@ __device__ __forceinline__ WinStat window_stat(const Sched &s, const u64 *keys, 
   float es = 0.f;
   for (int t = 0; t < s.width[q]; ++t) es += e[t];
   float nz = es;
-  if (noise) { nz = 0.f; for (int g = 0; g < s.ngs; ++g) nz += noise[c * s.ngs + g]; }
+  // (a w = 1 window's peak comes from the row kernel; its mean of P over the delay axis IS the AP's energy)
+  if (noise && s.width[q] > 1) { nz = 0.f; for (int g = 0; g < s.ngs; ++g) nz += noise[c * s.ngs + g]; }
   o.snr = (es > 0.f && nz > 0.f) ? sqrtf(o.power / nz) : 0.f;
   // an all-zero window (flagged data, the zero fill of dedispersion) has an identically zero plane:
   // P1 = 0 at (0, 0) by the tie rule.  The sliding sum would leave rounding residue of earlier samples

@@ -314,6 +314,7 @@ def test_zscore_selection_matches_oracle(vb, oracle, cfg, over):
     (1, 2, 40, 1024, [4], [1], 16384, 0.0),                # nfa = 16384 = 2 interleaved 8192-point transforms
     (2, 8, 26, 1024, [2, 4], [1, 1], 32768, 0.0),          # the paper's shape: 8 IF x 1024 x pad 4
     (1, 8, 30, 512, [4], [2], 32768, 300.0),               # pad x8, dedispersed, stride 2
+    (2, 4, 150, 64, [1, 4], [1, 2], 1024, 0.0),            # w = 1: peaks from the row kernel, noise = the AP's energy
 ])
 def test_allif_search_matches_oracle(vb, oracle, shape):
     """f2: one delay across all IFs (Eq. 1) vs oracle.allif_search on the same inputs."""
