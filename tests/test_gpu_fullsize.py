@@ -67,3 +67,43 @@ def test_fullsize_sampled(vb, oracle, cfg, nrandom):
         assert abs(float(g["snr"]) - o["snr"]) <= RTOL * o["snr"]
         assert (o["snr"] > c["snr_thresh"]) == (float(g["snr"]) > c["snr_thresh"]) or abs(o["snr"] - c["snr_thresh"]) < RTOL * c["snr_thresh"]
     plan.close()
+
+
+def test_fullsize_allif_sampled(vb, oracle):
+    """f2 at the paper's size in the launch configuration `bench.py --config 5 --allif --dm 26.8` times
+    (21 baselines x 3906 APs x 8 IF x 1024 points, nfa 32768 = 4 interleaved 8192-point transforms, dedispersed):
+    sampled windows against oracle.dedisperse + oracle.allif_search on the window's own APs."""
+    cfg = 5
+    vis, c, _ = workloads.generate(cfg, device="cuda")
+    nbl, nif, nap, nchan = vis.shape
+    nfa = workloads.gen.next_pow2(4 * nif * nchan)
+    assert nfa == 32768
+    f = 1400.0 + 16.0 * np.arange(nif)[:, None] + (16.0 / nchan) * np.arange(nchan)[None, :]
+    sh = vb.dm_shifts(26.8, f, f.max(), c["t_ap"])
+    plan = vb.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], None, nfa, c["snr_thresh"], allif=True)
+    cands, n, peaks = vb.fringe_search(vis, None, None, None, None, None, want_peaks=True, cand_capacity=1 << 20,
+                                       plan=plan, shifts=sh)
+    nw = plan.nwin_per_width
+    per = sum(nw)
+    assert len(peaks) == nbl * per == plan.nwin_total
+    assert np.all(peaks["rate_idx"] == 0) and peaks["delay_idx"].min() >= 0 and peaks["delay_idx"].max() < nfa
+    assert np.all(np.isfinite(peaks["snr"])) and np.all(peaks["power"] >= 0)
+    assert n == np.count_nonzero(peaks["snr"] > c["snr_thresh"])
+    keys = list(zip(cands["bl"], cands["wid"], cands["win"]))
+    assert keys == sorted(keys) and np.all(cands["ifq"] == -1)
+    rng = np.random.default_rng(505)
+    for bl in (0, int(rng.integers(1, nbl - 1)), nbl - 1):
+        src = oracle.dedisperse(vis[bl:bl + 1].cpu().numpy(), sh)
+        sample = {(q, int(rng.integers(0, nw[q]))) for q in range(len(nw)) for _ in range(4)}
+        sample |= {(q, 0) for q in range(len(nw))} | {(q, nw[q] - 1) for q in range(len(nw))}   # zero-filled head / tail
+        sample |= {(int(cd["wid"]), int(cd["win"])) for cd in cands[cands["bl"] == bl][:6]}
+        for (q, j) in sorted(sample):
+            w, s = c["widths"][q], c["strides"][q]
+            o = oracle.allif_search(src[:, :, j * s: j * s + w], [w], [1], nfa)[0]
+            g = peaks[nbl * sum(nw[:q]) + bl * nw[q] + j]      # dense peaks are laid out [width][baseline][window]
+            gi = int(g["delay_idx"])
+            tie = o["p1"] > 0 and (o["p1"] - o["p2"]) / o["p1"] < TIE
+            assert gi == o["idx1"] or (tie and gi == o["idx2"]), (bl, q, j, gi, o)
+            assert abs(float(g["power"]) - o["p1"]) <= RTOL * o["p1"]
+            assert abs(float(g["snr"]) - o["snr"]) <= RTOL * max(o["snr"], 1e-30)
+    plan.close()
