@@ -358,6 +358,20 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   pl->nchunks = (pl->npair + ppc - 1) / ppc;
   pl->pairs_per_chunk = (pl->npair + pl->nchunks - 1) / pl->nchunks;
   pl->nchunks = (pl->npair + pl->pairs_per_chunk - 1) / pl->pairs_per_chunk;
+  if (allif) {
+    // k_allif launches pairs_per_chunk x psub x nseg CTAs of up to 1024 threads (two per SM): size the
+    // segments of windows for about VOLKS_AI_WAVES (default 2) waves of 296 CTAs (restart cost per segment: w rows;
+    // measured at the paper's size: 1 wave 41.5 ms per trial, 2 waves 38.1, 4 waves 38.7, 8 waves 39.7)
+    const long long waves = std::max(1, env_int("VOLKS_AI_WAVES", 2));
+    for (auto &w : pl->wp) {
+      if (w.nwin <= 0) continue;
+      const long long want = std::max<long long>(1, (296 * waves + pl->pairs_per_chunk * psub - 1) / (pl->pairs_per_chunk * psub));
+      long long seg = ((w.nwin + want - 1) / want + 15) / 16 * 16;
+      seg = std::max<long long>(seg, 16);
+      w.seg = (int)seg;
+      w.nseg = (int)((w.nwin + seg - 1) / seg);
+    }
+  }
 
   pl->nfin_blocks = (s.nwin_total + FIN_THREADS * FIN_TILES - 1) / (FIN_THREADS * FIN_TILES);
   size_t off = 0;
