@@ -140,7 +140,7 @@ int volks_allif_search(const volks_plan *plan, const void *d_vis, const int32_t 
 
 /* The same searches on a HOST slab (pinned memory recommended), for slabs that are produced on the host
  * or do not fit the device: the slab is copied chunk by chunk (the (bl, ifq) pairs - baselines for an
- * all-IF plan - of one internal chunk at a time) into the two halves of `d_stage` on an internal copy
+ * all-IF plan - of a quarter of an internal chunk at a time) into the two halves of `d_stage` on an internal copy
  * stream, each copy overlapped with the kernels of the previous chunk; the result is identical to the
  * device-slab calls.  Works with both plan kinds (volks_plan_create / volks_plan_create_allif).
  *   h_vis    HOST cf32[nbl][nif][nap][nchan]; must stay valid until `cuda_stream` has run the call

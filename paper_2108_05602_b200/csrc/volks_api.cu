@@ -211,6 +211,7 @@ struct volks_plan {
   size_t off_keys = 0, off_E = 0, off_cnt = 0, off_zst = 0, off_Y = 0, ws_bytes = 0;
   long long nfin_blocks = 0;
   long long pairs_per_chunk = 0, nchunks = 0;
+  int host_split = 4;            // volks_search_host: copies (and kernel chunks) of pairs_per_chunk / host_split pairs
   // row kernel shape
   int row_tpr = 1, row_rows_per_cta = 1;
   size_t row_smem = 0;
@@ -358,6 +359,7 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   pl->nchunks = (pl->npair + ppc - 1) / ppc;
   pl->pairs_per_chunk = (pl->npair + pl->nchunks - 1) / pl->nchunks;
   pl->nchunks = (pl->npair + pl->pairs_per_chunk - 1) / pl->pairs_per_chunk;
+  pl->host_split = std::max(1, env_int("VOLKS_HOST_SPLIT", 4));
   if (allif) {
     // k_allif launches pairs_per_chunk x psub x nseg CTAs of up to 1024 threads (two per SM): size the
     // segments of windows for about VOLKS_AI_WAVES (default 2) waves of 296 CTAs (restart cost per segment: w rows;
@@ -498,7 +500,8 @@ int volks_cal_phasors(const double *delay_s, const double *phase_rad, int32_t np
 
 int volks_plan_query_host(const volks_plan *pl, size_t *stage_bytes) {
   if (!pl || !stage_bytes) return VOLKS_EINVAL;
-  *stage_bytes = align_up((size_t)pl->pairs_per_chunk * pl->sched.nap * pl->nchan * sizeof(float2), 256);
+  const long long ppc = std::max<long long>(1, (pl->pairs_per_chunk + pl->host_split - 1) / pl->host_split);   // run_search's host chunk
+  *stage_bytes = align_up((size_t)ppc * pl->sched.nap * pl->nchan * sizeof(float2), 256);
   return VOLKS_OK;
 }
 
@@ -540,9 +543,16 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
   }
   pl->prof_kind.clear(); pl->prof_wid.clear();
   if (!cuda_ok(cudaMemsetAsync(keys, 0, (size_t)s.nwin_total * sizeof(u64), st))) return VOLKS_ECUDA;
-  for (long long ch = 0; ch < pl->nchunks; ++ch) {
-    const long long pair0 = ch * pl->pairs_per_chunk;
-    const long long np = std::min(pl->pairs_per_chunk, pl->npair - pair0);
+  // host slab: a quarter of the plan's chunk per copy (VOLKS_HOST_SPLIT, default 4), so that the first copy
+  // and the last chunk's kernels - the two parts of the pipeline nothing overlaps - are short (config 2:
+  // 211 -> 187 ms per step from pinned memory; the device-resident search keeps the large chunks, which its
+  // kernels prefer: 163 against 168 ms)
+  const long long ppc = d_stage ? std::max<long long>(1, (pl->pairs_per_chunk + pl->host_split - 1) / pl->host_split)
+                                : pl->pairs_per_chunk;
+  const long long nchunks = (pl->npair + ppc - 1) / ppc;
+  for (long long ch = 0; ch < nchunks; ++ch) {
+    const long long pair0 = ch * ppc;
+    const long long np = std::min(ppc, pl->npair - pair0);
     RowArgs ra;
     ra.vis = (const float2 *)d_vis;
     if (d_stage) {
