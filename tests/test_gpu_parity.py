@@ -359,12 +359,13 @@ def test_allif_search_matches_oracle(vb, oracle, shape):
     assert hit and all(abs(int(c["delay_idx"]) - round(0.0137 * nfa)) <= res for c in hit if c["snr"] > 8)
 
 
+@pytest.mark.parametrize("chunk_mb", ["1", "8"])   # 8 MB: several pairs per plan chunk, the host path takes a quarter at a time
 @pytest.mark.parametrize("allif", [False, True])
-def test_host_slab_search_is_identical(vb, allif, monkeypatch):
+def test_host_slab_search_is_identical(vb, allif, chunk_mb, monkeypatch):
     """volks_search_host (slab in pinned host memory, chunked copies overlapped with the kernels) must
     give bit-identical candidates and peaks to the device-slab call; small chunks force several
     copy/compute rounds through both stage halves, twice in a row (stage reuse across calls)."""
-    monkeypatch.setenv("VOLKS_CHUNK_MB", "1")
+    monkeypatch.setenv("VOLKS_CHUNK_MB", chunk_mb)
     vis, c, _ = workloads.generate(2, nbl=3, nif=3, nap=600, npulses=3)
     nbl, nif, nap, nchan = vis.shape
     if allif:
