@@ -95,6 +95,18 @@ __device__ __forceinline__ f32x2 c2_mul(f32x2 z, f32x2 w) {
   return fma2(pk(-hi32(z), lo32(z)), pk(hi32(w), hi32(w)), mul2(z, pk(lo32(w), lo32(w))));
 }
 
+// w[m] = tab[m ts] for m = 1..15 (tab[k] = exp(-2 pi i k/n): powers of one root).  Only m = 1 and 4 are read
+// - lanes read the table with a stride of m entries, and 15 such reads per thread saturate L1 (ncu: 60 % of
+// k_rowbig's and 90 % of k_row3's L1 sectors) - the others are products, at most four deep.
+__device__ __forceinline__ void c2_powers16(const float2 *tab, int ts, f32x2 (&w)[16]) {
+  w[0] = pk(1.f, 0.f);
+  w[1] = c2_from(__ldg(tab + ts)); w[4] = c2_from(__ldg(tab + 4 * ts));
+  w[2] = c2_mul(w[1], w[1]); w[8] = c2_mul(w[4], w[4]);
+  w[3] = c2_mul(w[2], w[1]); w[5] = c2_mul(w[4], w[1]); w[6] = c2_mul(w[4], w[2]); w[7] = c2_mul(w[4], w[3]);
+#pragma unroll
+  for (int m = 1; m < 8; ++m) w[8 + m] = c2_mul(w[8], w[m]);
+}
+
 // z * exp(-2 pi i K/N), N in {2,4,8,16,32}, 0 <= K < N/2, compile time
 template <int K, int N>
 __device__ __forceinline__ f32x2 c2_mul_w(f32x2 z) {

@@ -403,11 +403,16 @@ __global__ void __launch_bounds__(256) k_row3(RowArgs a) {
 #pragma unroll
     for (int n3 = 0; n3 < NZA; ++n3) { e += cnorm(v[n3]); z[n3] = c2_from(v[n3]); }
     FftDif2<N3, NZA, 0, N3>::run(z);
+    // W_nf^{n' k3}: one coalesced table read (k3 = 1), the other powers as products (strided reads of the
+    // table were 90 % of this kernel's L1 traffic, and L1 its limit)
+    f32x2 w3[8];
+    w3[0] = pk(1.f, 0.f); w3[1] = c2_from(__ldg(a.twf + tid));
+    w3[2] = c2_mul(w3[1], w3[1]); w3[3] = c2_mul(w3[2], w3[1]); w3[4] = c2_mul(w3[2], w3[2]);
+    w3[5] = c2_mul(w3[4], w3[1]); w3[6] = c2_mul(w3[4], w3[2]); w3[7] = c2_mul(w3[4], w3[3]);
 #pragma unroll
     for (int i = 0; i < N3; ++i) {
       const int k3 = brev<N3>(i);
-      const float2 tw = __ldg(a.twf + tid * k3);        // W_nf^{n' k3}, n' k3 < nf
-      V[k3 * 256 + tid] = fma2(pk(-hi32(z[i]), lo32(z[i])), pk(tw.y, tw.y), mul2(z[i], pk(tw.x, tw.x)));
+      V[k3 * 256 + tid] = k3 ? c2_mul(z[i], w3[k3]) : z[i];
     }
   }
 #pragma unroll
@@ -428,11 +433,12 @@ __global__ void __launch_bounds__(256) k_row3(RowArgs a) {
     for (int n2 = 0; n2 < 16; ++n2) z[n2] = V[g * 256 + l + 16 * n2];
     FftDif2<16, 16, 0, 16>::run(z);
     f32x2 *E = Ex + g * (16 * EP);
+    f32x2 w2[16];
+    c2_powers16(a.twf, l * N3, w2);                        // W_256^{n1 m} = twf[n1 m N3]
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
       const int k2 = brev<16>(i);
-      const float2 tw = __ldg(a.twf + (l * k2) * N3);   // W_256^{n1 k2}
-      E[l * EP + k2] = fma2(pk(-hi32(z[i]), lo32(z[i])), pk(tw.y, tw.y), mul2(z[i], pk(tw.x, tw.x)));
+      E[l * EP + k2] = k2 ? c2_mul(z[i], w2[k2]) : z[i];   // W_256^{n1 k2}
     }
   }
   __syncthreads();                                       // every group is done with V; E complete
@@ -502,15 +508,10 @@ __device__ __forceinline__ void rowbig_pass(f32x2 (&v)[16], const RowArgs &a, in
   // of at most four of them.
   if constexpr (TW) {
     static_assert(NZ == 16, "later passes are dense");
-    const int ts = (j & (Ns - 1)) * (nf / (Ns * 16));
-    const f32x2 w1 = c2_from(__ldg(a.twf + ts)), w4 = c2_from(__ldg(a.twf + 4 * ts));
-    const f32x2 w2 = c2_mul(w1, w1), w8 = c2_mul(w4, w4);
-    const f32x2 w3 = c2_mul(w2, w1), w5 = c2_mul(w4, w1), w6 = c2_mul(w4, w2), w7 = c2_mul(w4, w3);
-    v[1] = c2_mul(v[1], w1); v[2] = c2_mul(v[2], w2); v[3] = c2_mul(v[3], w3); v[4] = c2_mul(v[4], w4);
-    v[5] = c2_mul(v[5], w5); v[6] = c2_mul(v[6], w6); v[7] = c2_mul(v[7], w7); v[8] = c2_mul(v[8], w8);
-    v[9] = c2_mul(v[9], c2_mul(w8, w1)); v[10] = c2_mul(v[10], c2_mul(w8, w2)); v[11] = c2_mul(v[11], c2_mul(w8, w3));
-    v[12] = c2_mul(v[12], c2_mul(w8, w4)); v[13] = c2_mul(v[13], c2_mul(w8, w5)); v[14] = c2_mul(v[14], c2_mul(w8, w6));
-    v[15] = c2_mul(v[15], c2_mul(w8, w7));
+    f32x2 w[16];
+    c2_powers16(a.twf, (j & (Ns - 1)) * (nf / (Ns * 16)), w);
+#pragma unroll
+    for (int m = 1; m < 16; ++m) v[m] = c2_mul(v[m], w[m]);
   }
   FftDif2<16, NZ, 0, 16>::run(v);
 }
