@@ -319,12 +319,12 @@ __global__ void __launch_bounds__(256) k_row2(RowArgs a) {
 #pragma unroll
     for (int n2 = 0; n2 < NZA; ++n2) { e += cnorm(v[n2]); z[n2] = c2_from(v[n2]); }
     FftDif2<N2, NZA, 0, N2>::run(z);
+    f32x2 w2[16];
+    c2_powers16(a.twf, l, w2);                            // W_nf^{n1 m}: two coalesced reads, products (k_row3)
 #pragma unroll
     for (int i = 0; i < N2; ++i) {
-      constexpr int dummy = 0; (void)dummy;
       const int k2 = brev<N2>(i);
-      const float2 tw = __ldg(a.twf + l * k2);          // W_nf^{n1 k2}, n1 k2 < nf
-      E[l * EP + k2] = fma2(pk(-hi32(z[i]), lo32(z[i])), pk(tw.y, tw.y), mul2(z[i], pk(tw.x, tw.x)));
+      E[l * EP + k2] = k2 ? c2_mul(z[i], w2[k2]) : z[i];   // W_nf^{n1 k2}, n1 k2 < nf
     }
   }
 #pragma unroll
