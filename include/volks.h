@@ -127,7 +127,9 @@ int volks_fringe_search_dd(const volks_plan *plan, const void *d_vis, const int3
  *   A[d] = sum_{t<w} sum_{m<nif*nchan} band[t0+t][m] exp(-2 pi i m d/nfa),  m = n*nchan + j,
  *   P = |A|^2, (P1, d*) first argmax, noise = mean_d P, snr = sqrt(P1/noise), candidate iff snr > snr_thresh.
  * volks_plan_create_allif reads nbl, nif, nap, nchan, nwidths, width[], stride[], snr_thresh and
- * nf = nfa (power of two, nif*nchan <= nfa, 64 <= nfa <= 8192); nt[] is ignored (may be NULL).
+ * nf = nfa (power of two, 64 <= nfa <= 32768, nif*nchan <= min(nfa, 8192): beyond 8192 the transform is
+ * computed as nfa/8192 interleaved 8192-point transforms of the pre-modulated band, which must fit one of
+ * them; VOLKS_EINVAL otherwise); nt[] is ignored (may be NULL).
  * volks_allif_search takes the same buffers as volks_fringe_search_dd (d_shift: dedispersion, or NULL);
  * sizes from volks_plan_query (nwin_total = nbl * sum_q nwin_q).  Records: ifq = -1, rate_idx = 0,
  * delay_idx in [0, nfa); canonical order (bl, q, j); dense peaks d_peaks[off_q + bl*nwin_q + j].

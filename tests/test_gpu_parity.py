@@ -512,3 +512,84 @@ def test_random_shapes(vb, oracle, seed):
     vis[0, 0, t0:t0 + 8] += 1.0 + 1.0j
     c = dict(widths=widths, strides=strides, nts=nts, nf=nf, snr_thresh=3.0)
     run_both(vb, oracle, vis, c, mode="fft")
+
+
+@pytest.mark.parametrize("seed", list(range(8)))
+def test_random_gather_shapes(vb, oracle, seed):
+    """Seeded random problems through the gather modes of every row kernel (k_row2: nf 64..256, k_row3:
+    512..2048, k_rowbig: 4096 / 8192, generic: the rest): random per-channel shifts (negative and past the
+    end included), a ragged band (nchan < nf), optional calibration phasors; per-IF search vs
+    oracle.calibrate + oracle.dedisperse + oracle.search, every window compared."""
+    rng = np.random.default_rng(7000 + seed)
+    nf = int([64, 128, 256, 512, 1024, 2048, 4096, 8192][seed])
+    nchan = int(rng.integers(nf // 8 + 1, nf + 1))
+    nbl, nif = int(rng.integers(1, 3)), int(rng.integers(1, 4))
+    widths, strides, nts = [], [], []
+    for w in rng.choice([1, 2, 4, 8, 16], size=2, replace=False):
+        w = int(w)
+        widths.append(w); strides.append(1 if rng.random() < 0.5 else int(rng.integers(1, w + 2)))
+        nts.append(int(workloads.gen.next_pow2(w * int(rng.choice([1, 2])))))
+    nap = int(rng.integers(40, 90)) if nf >= 1024 else int(rng.integers(60, 300))
+    g = torch.Generator().manual_seed(900 + seed)
+    vis = torch.view_as_complex(torch.randn((nbl, nif, nap, nchan, 2), generator=g) * 0.7071)
+    vis[0, 0, nap // 2: nap // 2 + 6] += 1.0 + 0.5j
+    sh = rng.integers(-3, 13, size=(nif, nchan)).astype(np.int32)
+    sh[0, 0] = nap + 2
+    raw = vis.numpy()
+    cal = None
+    if seed % 2:
+        cal = vb.cal_phasors(rng.uniform(-30e-9, 30e-9, (nbl, nif)), rng.uniform(-np.pi, np.pi, (nbl, nif)), nchan, 16e6 / nchan)
+    plan = vb.Plan(nbl, nif, nap, nchan, widths, strides, nts, nf, 3.0)
+    if cal is not None:
+        plan.set_cal(torch.from_numpy(cal).cuda())
+    cands, n, peaks = vb.fringe_search(vis.cuda(), want_peaks=True, plan=plan, shifts=sh)
+    plan.close()
+    src = oracle.dedisperse(oracle.calibrate(raw, cal) if cal is not None else raw, sh)
+    c = dict(widths=widths, strides=strides, nts=nts, nf=nf)
+    ora, _ = oracle.search(src, widths, strides, nts, nf, mode="cached")
+    nw = [workloads.gen.nwin(nap, w, s) for w, s in zip(widths, strides)]
+    check_peaks(peaks[dense_index(nbl, nif, nw)], ora, nf, make_plane_power(oracle, src, c))
+    oc, keep = oracle.candidates(ora, nbl, nif, nap, widths, strides, nf, 3.0)
+    check_candidates(cands, oc, ora, keep, 3.0, nf)
+
+
+@pytest.mark.parametrize("seed", list(range(6)))
+def test_random_allif_shapes(vb, oracle, seed):
+    """Seeded random all-IF searches (f2): nfa 256..16384 (k_row2, k_row3, generic, k_rowbig, interleaved
+    sub-rows), random per-channel shifts, a band that does not fill nfa, optional calibration; every window
+    against oracle.allif_search."""
+    rng = np.random.default_rng(8100 + seed)
+    nfa = int([256, 1024, 2048, 4096, 8192, 16384][seed])
+    nif = int(rng.integers(1, 5))
+    nchan = int(rng.integers(max(1, nfa // (8 * nif)), min(nfa, 8192) // nif + 1))     # the band fits one 8192-point row
+    nbl = int(rng.integers(1, 3))
+    widths = [int(w) for w in rng.choice([1, 2, 3, 4, 8, 16, 24], size=2, replace=False)]
+    strides = [1 if rng.random() < 0.5 else int(rng.integers(1, w + 2)) for w in widths]
+    nap = int(rng.integers(40, 80)) if nfa >= 4096 else int(rng.integers(80, 400))
+    g = torch.Generator().manual_seed(300 + seed)
+    vis = torch.view_as_complex(torch.randn((nbl, nif, nap, nchan, 2), generator=g) * 0.7071)
+    sh = rng.integers(-2, 9, size=(nif, nchan)).astype(np.int32)
+    raw = vis.numpy()
+    cal = None
+    if seed % 2 == 0:
+        cal = vb.cal_phasors(rng.uniform(-30e-9, 30e-9, (nbl, nif)), rng.uniform(-np.pi, np.pi, (nbl, nif)), nchan, 16e6 / nchan)
+    plan = vb.Plan(nbl, nif, nap, nchan, widths, strides, None, nfa, 3.0, allif=True)
+    if cal is not None:
+        plan.set_cal(torch.from_numpy(cal).cuda())
+    cands, n, peaks = vb.fringe_search(vis.cuda(), want_peaks=True, plan=plan, shifts=sh)
+    plan.close()
+    src = oracle.dedisperse(oracle.calibrate(raw, cal) if cal is not None else raw, sh)
+    ora = oracle.allif_search(src, widths, strides, nfa)
+    nw = [workloads.gen.nwin(nap, w, s) for w, s in zip(widths, strides)]
+    band = oracle.allif_band(src)
+
+    def plane_power(i, idx):
+        b, r = divmod(i, sum(nw))
+        q = 0
+        while r >= nw[q]:
+            r -= nw[q]; q += 1
+        a = np.fft.fft(band[b, r * strides[q]: r * strides[q] + widths[q]].astype(np.complex128).sum(axis=0), nfa)[idx]
+        return float(abs(a) ** 2)
+    check_peaks(peaks[dense_index(nbl, 1, nw)], ora, nfa, plane_power)
+    marg = np.abs(ora["snr"] - 3.0) <= 1e-4 * 3.0
+    assert abs(n - np.count_nonzero(ora["snr"] > 3.0)) <= int(marg.sum())
