@@ -28,6 +28,7 @@ struct ColFftArgs {
   const float4 *tw4;    // [nt] exp(-2 pi i k/nt), pre-broadcast (re, re, im, im)
   long long per_pair, offc, pair0;
   int nap, nf, w, stride, nt, nwin, pitch, paired;
+  int split2;           // host side only: launch k_colfft2 (kernels_colfft2.cuh) where it exists
   int wpc;              // windows per CTA (consecutive)
   int nrange;           // ceil(nwin / wpc)
   uint32_t keymask;     // 0xFFFFFFF0 (register operand of the single-LOP3 key tag)

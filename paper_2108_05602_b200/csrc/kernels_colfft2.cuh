@@ -1,0 +1,213 @@
+// kernels_colfft2.cuh - k_colfft (kernels_colfft.cuh) for Nt = 256 / 512 (L1 = 16 / 32) with TWO delay columns
+// per thread in the split format of kernels_slide.cuh: X = (Re z_a, Re z_b), Y = (Im z_a, Im z_b).
+//
+//   k_colfft2<L1, NZ>   a4+a5+a6 for every window of one width; the decomposition
+//                       t = t2 + 16 t1, r = rho + L1 s is the one of k_colfft.
+//
+// Why: with one complex number per register pair every non-trivial twiddle (and the power) needs the
+// (im, re) swap of the pair - register moves and ALU work next to each FMUL2/FFMA2 - and the pair-interleaved
+// delay spectra (common.cuh ld_y) are gathered with two 32-bit loads per element.  In the split format a row
+// of the pair is ONE 128-bit load, z * w is four FFMA2/FMUL2 for two columns with no moves, -i z is a
+// renaming, and |z|^2 of both columns is FMUL2 + FFMA2.
+//
+// CTA = 512 threads = a 32-column strip (16 column pairs) x a range of consecutive windows.
+// pass 1: thread = (t2, column pair, parity hb of rho); warp = (hb, t2 in {w/2, w/2 + 8}).  The first DIF
+//         stage of the L1-point transform over t1 separates even and odd rho, so each parity is an
+//         (L1/2)-point pruned FFT of its own: e[k] = z[k] + z[k + L1/2],  o[k] = (z[k] - z[k + L1/2]) W_L1^k.
+//         Outputs go to shared memory S[rho][t2][pair] as (X, Y) = one float4.
+// pass 2: thread = (rho, column pair); warp = two residues.  16 float4 loads, the twiddle W_Nt^{rho t2}
+//         (shared table, pre-broadcast), a 16-point DIF FFT, powers, tagged keys (R1), warp max.
+#pragma once
+#include "common.cuh"
+#include "kernels_colfft.cuh"
+
+namespace volks {
+
+// (X + i Y) * exp(-2 pi i K/N) for both columns; N in {2,..,32}, 0 <= K < N/2, compile time
+template <int K, int N>
+__device__ __forceinline__ void s2_mul_w(f32x2 &X, f32x2 &Y) {
+  constexpr int k32 = K * (32 / N);
+  static_assert(k32 >= 0 && k32 < 16, "first-half twiddles only");
+  constexpr float H = 0.70710678118654752f;
+  constexpr float C[16] = {1.f, 0.98078528040323043f, 0.92387953251128674f, 0.83146961230254524f, H, 0.55557023301960218f,
+                           0.38268343236508977f, 0.19509032201612825f, 0.f, -0.19509032201612825f, -0.38268343236508977f,
+                           -0.55557023301960218f, -H, -0.83146961230254524f, -0.92387953251128674f, -0.98078528040323043f};
+  constexpr float S[16] = {0.f, 0.19509032201612825f, 0.38268343236508977f, 0.55557023301960218f, H, 0.83146961230254524f,
+                           0.92387953251128674f, 0.98078528040323043f, 1.f, 0.98078528040323043f, 0.92387953251128674f,
+                           0.83146961230254524f, H, 0.55557023301960218f, 0.38268343236508977f, 0.19509032201612825f};
+  // (x + i y)(c - i s) = (x c + y s) + i (y c - x s)
+  if constexpr (k32 == 0) return;
+  else if constexpr (k32 == 8) { const f32x2 t = X; X = Y; Y = neg2(t); }
+  else if constexpr (k32 == 4) { const f32x2 t = add2(X, Y); Y = mul2(sub2(Y, X), pk(H, H)); X = mul2(t, pk(H, H)); }
+  else if constexpr (k32 == 12) { const f32x2 t = sub2(Y, X); Y = mul2(add2(X, Y), pk(-H, -H)); X = mul2(t, pk(H, H)); }
+  else {
+    constexpr float c = C[k32], s = S[k32];
+    const f32x2 t = fma2(X, pk(c, c), mul2(Y, pk(s, s)));
+    Y = fma2(Y, pk(c, c), mul2(X, pk(-s, -s)));
+    X = t;
+  }
+}
+
+// Split-format in-register radix-2 DIF FFT of N (<= 16) points (X, Y)[OFF .. OFF+N), forward, output
+// BIT-REVERSED, only the first NZ inputs non-zero (NZ = N: the plain transform).
+template <int N, int NZ, int OFF, int TOTAL>
+struct FftDifS {
+  template <int K>
+  static __device__ __forceinline__ void stage(f32x2 (&X)[TOTAL], f32x2 (&Y)[TOTAL]) {
+    if constexpr (K < N / 2) {
+      if constexpr (NZ <= N / 2) {
+        if constexpr (K < NZ) {
+          X[OFF + K + N / 2] = X[OFF + K]; Y[OFF + K + N / 2] = Y[OFF + K];
+          s2_mul_w<K, N>(X[OFF + K + N / 2], Y[OFF + K + N / 2]);
+        }
+      } else {
+        const f32x2 ux = X[OFF + K], uy = Y[OFF + K], vx = X[OFF + K + N / 2], vy = Y[OFF + K + N / 2];
+        X[OFF + K] = add2(ux, vx); Y[OFF + K] = add2(uy, vy);
+        X[OFF + K + N / 2] = sub2(ux, vx); Y[OFF + K + N / 2] = sub2(uy, vy);
+        s2_mul_w<K, N>(X[OFF + K + N / 2], Y[OFF + K + N / 2]);
+      }
+      stage<K + 1>(X, Y);
+    }
+  }
+  static __device__ __forceinline__ void run(f32x2 (&X)[TOTAL], f32x2 (&Y)[TOTAL]) {
+    if constexpr (N >= 2) {
+      stage<0>(X, Y);
+      constexpr int NZ2 = NZ < N / 2 ? NZ : N / 2;
+      FftDifS<N / 2, NZ2, OFF, TOTAL>::run(X, Y);
+      FftDifS<N / 2, NZ2, OFF + N / 2, TOTAL>::run(X, Y);
+    }
+  }
+};
+
+// (X, Y)[k] *= W_N^k for k < KN
+template <int K, int KN, int N, int TOTAL>
+struct S2Twiddle {
+  static __device__ __forceinline__ void run(f32x2 (&X)[TOTAL], f32x2 (&Y)[TOTAL]) {
+    if constexpr (K < KN) {
+      s2_mul_w<K, N>(X[K], Y[K]);
+      S2Twiddle<K + 1, KN, N, TOTAL>::run(X, Y);
+    }
+  }
+};
+
+__device__ __forceinline__ void cf2_lds(uint32_t addr, f32x2 &a, f32x2 &b) {
+  asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(a), "=l"(b) : "r"(addr));
+}
+__device__ __forceinline__ void cf2_sts(uint32_t addr, f32x2 a, f32x2 b) {
+  asm volatile("st.shared.v2.b64 [%0], {%1,%2};" ::"r"(addr), "l"(a), "l"(b) : "memory");
+}
+
+// pass 1 of one thread: parity HB of rho.  zx/zy: the NZ leading rows t2 + 16 t1 of the column pair.
+template <int L1, int NZ, int HB>
+__device__ __forceinline__ void cf2_pass1(const f32x2 (&zx)[NZ], const f32x2 (&zy)[NZ], uint32_t sdst) {
+  constexpr int H = L1 / 2;
+  constexpr int NZH = NZ < H ? NZ : H;          // non-zero inputs of the half-size transform
+  f32x2 X[H], Y[H];
+  if constexpr (NZ <= H) {
+#pragma unroll
+    for (int k = 0; k < NZ; ++k) { X[k] = zx[k]; Y[k] = zy[k]; }
+  } else {
+#pragma unroll
+    for (int k = 0; k < H; ++k) {
+      X[k] = HB ? sub2(zx[k], zx[k + H]) : add2(zx[k], zx[k + H]);
+      Y[k] = HB ? sub2(zy[k], zy[k + H]) : add2(zy[k], zy[k + H]);
+    }
+  }
+  if constexpr (HB == 1) S2Twiddle<0, NZH, L1, H>::run(X, Y);
+  FftDifS<H, NZH, 0, H>::run(X, Y);
+  // output i of the half transform is m = brev(i); rho = 2 m + HB; S[rho][t2][pair]: 4096 bytes per rho
+#pragma unroll
+  for (int i = 0; i < H; ++i) cf2_sts(sdst + (uint32_t)(2 * brev<H>(i) + HB) * 4096u, X[i], Y[i]);
+}
+
+template <int L1, int NZ>
+__global__ void __launch_bounds__(CF_WARPS * 32) k_colfft2(ColFftArgs a) {
+  static_assert(L1 == 16 || L1 == 32, "Nt = 256 or 512");
+  extern __shared__ float4 cf_sm4[];
+  float4 *tw4s = cf_sm4;                                // [nt] rate twiddles (re, re, im, im)
+  float4 *S4 = cf_sm4 + a.nt;                           // [L1][16][16] (X, Y) of a column pair
+  u64 *slots = (u64 *)(S4 + (size_t)L1 * 16 * 16);      // [CF_WARPS] per-warp window keys
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int cp = lane & 15, hi = lane >> 4;
+  const int ntile = a.nf >> 5;
+  long long u = blockIdx.x;
+  const int rg = (int)(u % a.nrange); u /= a.nrange;
+  const int tile = (int)(u % ntile);
+  const long long pl = u / ntile;
+  const uint32_t rowb = (uint32_t)a.pitch * 8u;
+  const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch) + (size_t)(tile * 16 + cp) * 16u;
+  u64 *keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
+  for (int i = threadIdx.x; i < a.nt; i += CF_WARPS * 32) tw4s[i] = a.tw4[i];
+  const int j0 = rg * a.wpc, j1 = min(a.nwin, j0 + a.wpc);
+  const uint32_t ntm = (uint32_t)a.nt - 1u;
+  const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(S4);
+  const uint32_t twbase = (uint32_t)__cvta_generic_to_shared(tw4s);
+  // pass-1 role
+  const int hb = warp & 1, t2 = (warp >> 1) + 8 * hi;
+  const uint32_t sdst = sbase + (uint32_t)(t2 * 16 + cp) * 16u;
+  // pass-2 role
+  const uint32_t rho = 2u * (uint32_t)warp + (uint32_t)hi;
+  const uint32_t ssrc = sbase + rho * 4096u + (uint32_t)cp * 16u;
+  constexpr bool PREFETCH = NZ <= 8;                    // NZ = 16 (+ pass 2's 64 registers) would spill
+
+  f32x2 zx[NZ], zy[NZ];
+  auto load_window = [&](int j) {
+    const size_t t0 = (size_t)j * a.stride;
+#pragma unroll
+    for (int t1 = 0; t1 < NZ; ++t1) {
+      const int t = t2 + 16 * t1;
+      if (j < j1 && t < a.w) ldg2(ybase + (t0 + t) * rowb, zx[t1], zy[t1]);
+      else { zx[t1] = pk(0.f, 0.f); zy[t1] = pk(0.f, 0.f); }
+    }
+  };
+  if constexpr (PREFETCH) load_window(j0);
+
+  for (int j = j0; j < j1; ++j) {
+    if constexpr (!PREFETCH) load_window(j);
+    if (hb) cf2_pass1<L1, NZ, 1>(zx, zy, sdst);
+    else cf2_pass1<L1, NZ, 0>(zx, zy, sdst);
+    if constexpr (PREFETCH) load_window(j + 1);   // in flight during pass 2
+    __syncthreads();
+    if (warp < L1 / 2) {
+      f32x2 X[16], Y[16];
+#pragma unroll
+      for (int k = 0; k < 16; ++k) {
+        f32x2 zx2, zy2, wx, wy;
+        cf2_lds(ssrc + (uint32_t)k * 256u, zx2, zy2);
+        cf2_lds(twbase + (((rho * (uint32_t)k) & ntm) << 4), wx, wy);
+        // z * w = (zx wx - zy wy) + i (zx wy + zy wx)
+        X[k] = fma2(zx2, wx, mul2(zy2, neg2(wy)));
+        Y[k] = fma2(zx2, wy, mul2(zy2, wx));
+      }
+      FftDifS<16, 16, 0, 16>::run(X, Y);
+      uint32_t ba = 0, bb = 0;
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        const f32x2 pw = fma2(Y[i], Y[i], mul2(X[i], X[i]));
+        ba = max(ba, (__float_as_uint(lo32(pw)) & a.keymask) | (uint32_t)(15 - brev<16>(i)));
+        bb = max(bb, (__float_as_uint(hi32(pw)) & a.keymask) | (uint32_t)(15 - brev<16>(i)));
+      }
+      const bool colb = bb > ba;
+      const uint32_t best = colb ? bb : ba;
+      const uint32_t km = __reduce_max_sync(0xffffffffu, best);
+      const uint32_t tied = __ballot_sync(0xffffffffu, best == km);
+      if (lane == __ffs(tied) - 1) {
+        const uint32_t s = 15u - (km & 15u);
+        slots[warp] = make_key(__uint_as_float(km & 0xFFFFFFF0u),
+                               (rho + (uint32_t)L1 * s) * (uint32_t)a.nf + (uint32_t)(tile * 32 + 2 * cp) + (colb ? 1u : 0u));
+      }
+    }
+    __syncthreads();
+    if (warp == 0) {
+      u64 k = lane < L1 / 2 ? slots[lane] : 0ull;
+#pragma unroll
+      for (int o = 8; o >= 1; o >>= 1) {
+        const u64 other = __shfl_xor_sync(0xffffffffu, k, o);
+        k = other > k ? other : k;
+      }
+      if (lane == 0) atomicMax(keyp + j, k);
+    }
+  }
+}
+
+}  // namespace volks

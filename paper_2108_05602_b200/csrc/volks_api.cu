@@ -11,6 +11,7 @@
 
 #include "kernels_generic.cuh"
 #include "kernels_slide.cuh"
+#include "kernels_colfft2.cuh"
 #include "kernels_colfft.cuh"
 #include "kernels_allif.cuh"
 #include "kernels_fixup.cuh"
@@ -66,6 +67,17 @@ inline size_t colfft_smem(int l1, int nt) { return (size_t)l1 * 16 * 32 * sizeof
 template <int L1, int NZ>
 static cudaError_t colfft_one(const ColFftArgs &a, unsigned blocks, cudaStream_t st, bool attr_only) {
   const size_t smem = colfft_smem(L1, a.nt);
+  if constexpr (L1 >= 16) {
+    // Nt = 256 / 512: two columns per thread in split format (kernels_colfft2.cuh) unless VOLKS_CF2=0
+    const bool cf2 = a.split2 != 0;
+    if (attr_only) {
+      const cudaError_t e = cudaFuncSetAttribute(k_colfft2<L1, NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      if (e != cudaSuccess) return e;
+    } else if (cf2) {
+      k_colfft2<L1, NZ><<<blocks, CF_WARPS * 32, smem, st>>>(a);
+      return cudaSuccess;
+    }
+  }
   if (attr_only) return cudaFuncSetAttribute(k_colfft<L1, NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   k_colfft<L1, NZ><<<blocks, CF_WARPS * 32, smem, st>>>(a);
   return cudaSuccess;
@@ -199,6 +211,7 @@ struct volks_plan {
   mutable cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
   mutable const float2 *d_cal = nullptr;   // volks_plan_set_cal: DEVICE cf32[nbl][nif][nchan] applied in the slab load
   int nslide = 0;                // widths on the sliding-sum path (k_fixup re-evaluates their outlier windows)
+  int cf_split2 = 1;             // VOLKS_CF2: k_colfft2 (two columns per thread, split format) for Nt = 256 / 512
   int ai_psub = 1;               // f2 with nfa > 8192: nfa = ai_psub * row_nf (virtual sub-rows, kernels_generic.cuh)
   int row_nf = 0;                // size of the row transform (= sched.nf unless ai_psub > 1)
   size_t premod_off = 0;         // offset (float2) of the W_nfa table in d_tables
@@ -301,6 +314,7 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   size_t tw_total = (size_t)p->nf;
   const bool force_generic = env_is("VOLKS_PATH", "generic");
   const int seg_req = std::max(16, env_int("VOLKS_SLIDE_SEG", 256));
+  pl->cf_split2 = env_int("VOLKS_CF2", 1) != 0 ? 1 : 0;   // (k_colfft needs nf >= 32: Y rows are always pair-interleaved there)
   for (int q = 0; q < p->nwidths; ++q) {
     WidthPlan w;
     w.w = p->width[q]; w.s = p->stride[q]; w.nt = p->nt[q];
@@ -624,7 +638,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         fa.Y = Y; fa.keys = keys; fa.tw4 = (const float4 *)(pl->d_tables + w.tw4_off);
         fa.per_pair = s.per_pair; fa.offc = s.offc[q]; fa.pair0 = pair0;
         fa.nap = s.nap; fa.nf = s.nf; fa.w = w.w; fa.stride = w.s; fa.nt = w.nt; fa.nwin = (int)w.nwin;
-        fa.pitch = pl->pitch; fa.paired = pl->paired; fa.wpc = w.cf_wpc; fa.nrange = w.cf_nrange; fa.keymask = 0xFFFFFFF0u;
+        fa.pitch = pl->pitch; fa.paired = pl->paired; fa.split2 = pl->cf_split2; fa.wpc = w.cf_wpc; fa.nrange = w.cf_nrange; fa.keymask = 0xFFFFFFF0u;
         ProfScope ps(pl, st, VOLKS_K_COLFFT, q);
         if (!cuda_ok(launch_colfft(fa, w.cf_l1, w.cf_nz, np * (s.nf / 32) * w.cf_nrange, st, false))) return VOLKS_ECUDA;
         continue;
