@@ -98,7 +98,7 @@ __device__ __forceinline__ void cf2_sts(uint32_t addr, f32x2 a, f32x2 b) {
 }
 
 // pass 1 of one thread: parity HB of rho.  zx/zy: the NZ leading rows t2 + 16 t1 of the column pair.
-template <int L1, int NZ, int HB>
+template <int L1, int NZ, int HB, int CP>
 __device__ __forceinline__ void cf2_pass1(const f32x2 (&zx)[NZ], const f32x2 (&zy)[NZ], uint32_t sdst) {
   constexpr int H = L1 / 2;
   constexpr int NZH = NZ < H ? NZ : H;          // non-zero inputs of the half-size transform
@@ -115,39 +115,46 @@ __device__ __forceinline__ void cf2_pass1(const f32x2 (&zx)[NZ], const f32x2 (&z
   }
   if constexpr (HB == 1) S2Twiddle<0, NZH, L1, H>::run(X, Y);
   FftDifS<H, NZH, 0, H>::run(X, Y);
-  // output i of the half transform is m = brev(i); rho = 2 m + HB; S[rho][t2][pair]: 4096 bytes per rho
+  // output i of the half transform is m = brev(i); rho = 2 m + HB; S[rho][t2][pair]: 256 CP bytes per rho
 #pragma unroll
-  for (int i = 0; i < H; ++i) cf2_sts(sdst + (uint32_t)(2 * brev<H>(i) + HB) * 4096u, X[i], Y[i]);
+  for (int i = 0; i < H; ++i) cf2_sts(sdst + (uint32_t)(2 * brev<H>(i) + HB) * (256u * CP), X[i], Y[i]);
 }
 
-template <int L1, int NZ>
-__global__ void __launch_bounds__(CF_WARPS * 32) k_colfft2(ColFftArgs a) {
+#ifndef CF2_MIN_CTAS8
+#define CF2_MIN_CTAS8 2   // CTAs per SM the CP = 8 variant is compiled for (register cap 128)
+#endif
+// CP = column pairs per CTA (16: a 32-column strip, 512 threads; 8: a 16-column strip, 256 threads, several CTAs per SM)
+template <int L1, int NZ, int CP>
+__global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : 1) k_colfft2(ColFftArgs a) {
   static_assert(L1 == 16 || L1 == 32, "Nt = 256 or 512");
+  static_assert(CP == 16 || CP == 8, "strip of 32 or 16 columns");
+  constexpr int G = 32 / CP;                            // (t2 | rho) groups per warp
+  constexpr int NW = CP;                                // warps per CTA
   extern __shared__ float4 cf_sm4[];
   float4 *tw4s = cf_sm4;                                // [nt] rate twiddles (re, re, im, im)
-  float4 *S4 = cf_sm4 + a.nt;                           // [L1][16][16] (X, Y) of a column pair
-  u64 *slots = (u64 *)(S4 + (size_t)L1 * 16 * 16);      // [CF_WARPS] per-warp window keys
+  float4 *S4 = cf_sm4 + a.nt;                           // [L1][16][CP] (X, Y) of a column pair
+  u64 *slots = (u64 *)(S4 + (size_t)L1 * 16 * CP);      // [NW] per-warp window keys
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int cp = lane & 15, hi = lane >> 4;
-  const int ntile = a.nf >> 5;
+  const int cp = lane & (CP - 1), hi = lane / CP;
+  const int ntile = a.nf / (2 * CP);
   long long u = blockIdx.x;
   const int rg = (int)(u % a.nrange); u /= a.nrange;
   const int tile = (int)(u % ntile);
   const long long pl = u / ntile;
   const uint32_t rowb = (uint32_t)a.pitch * 8u;
-  const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch) + (size_t)(tile * 16 + cp) * 16u;
+  const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch) + (size_t)(tile * CP + cp) * 16u;
   u64 *keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
-  for (int i = threadIdx.x; i < a.nt; i += CF_WARPS * 32) tw4s[i] = a.tw4[i];
+  for (int i = threadIdx.x; i < a.nt; i += NW * 32) tw4s[i] = a.tw4[i];
   const int j0 = rg * a.wpc, j1 = min(a.nwin, j0 + a.wpc);
   const uint32_t ntm = (uint32_t)a.nt - 1u;
   const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(S4);
   const uint32_t twbase = (uint32_t)__cvta_generic_to_shared(tw4s);
   // pass-1 role
-  const int hb = warp & 1, t2 = (warp >> 1) + 8 * hi;
-  const uint32_t sdst = sbase + (uint32_t)(t2 * 16 + cp) * 16u;
+  const int hb = warp & 1, t2 = (warp >> 1) + (16 / G) * hi;
+  const uint32_t sdst = sbase + (uint32_t)(t2 * CP + cp) * 16u;
   // pass-2 role
-  const uint32_t rho = 2u * (uint32_t)warp + (uint32_t)hi;
-  const uint32_t ssrc = sbase + rho * 4096u + (uint32_t)cp * 16u;
+  const uint32_t rho = (uint32_t)(G * warp + hi);
+  const uint32_t ssrc = sbase + rho * (256u * CP) + (uint32_t)cp * 16u;
   constexpr bool PREFETCH = NZ <= 8;                    // NZ = 16 (+ pass 2's 64 registers) would spill
 
   f32x2 zx[NZ], zy[NZ];
@@ -164,16 +171,16 @@ __global__ void __launch_bounds__(CF_WARPS * 32) k_colfft2(ColFftArgs a) {
 
   for (int j = j0; j < j1; ++j) {
     if constexpr (!PREFETCH) load_window(j);
-    if (hb) cf2_pass1<L1, NZ, 1>(zx, zy, sdst);
-    else cf2_pass1<L1, NZ, 0>(zx, zy, sdst);
+    if (hb) cf2_pass1<L1, NZ, 1, CP>(zx, zy, sdst);
+    else cf2_pass1<L1, NZ, 0, CP>(zx, zy, sdst);
     if constexpr (PREFETCH) load_window(j + 1);   // in flight during pass 2
     __syncthreads();
-    if (warp < L1 / 2) {
+    if (warp < L1 / G) {
       f32x2 X[16], Y[16];
 #pragma unroll
       for (int k = 0; k < 16; ++k) {
         f32x2 zx2, zy2, wx, wy;
-        cf2_lds(ssrc + (uint32_t)k * 256u, zx2, zy2);
+        cf2_lds(ssrc + (uint32_t)k * (16u * CP), zx2, zy2);
         cf2_lds(twbase + (((rho * (uint32_t)k) & ntm) << 4), wx, wy);
         // z * w = (zx wx - zy wy) + i (zx wy + zy wx)
         X[k] = fma2(zx2, wx, mul2(zy2, neg2(wy)));
@@ -194,12 +201,12 @@ __global__ void __launch_bounds__(CF_WARPS * 32) k_colfft2(ColFftArgs a) {
       if (lane == __ffs(tied) - 1) {
         const uint32_t s = 15u - (km & 15u);
         slots[warp] = make_key(__uint_as_float(km & 0xFFFFFFF0u),
-                               (rho + (uint32_t)L1 * s) * (uint32_t)a.nf + (uint32_t)(tile * 32 + 2 * cp) + (colb ? 1u : 0u));
+                               (rho + (uint32_t)L1 * s) * (uint32_t)a.nf + (uint32_t)(tile * 2 * CP + 2 * cp) + (colb ? 1u : 0u));
       }
     }
     __syncthreads();
     if (warp == 0) {
-      u64 k = lane < L1 / 2 ? slots[lane] : 0ull;
+      u64 k = lane < L1 / G && lane < NW ? slots[lane] : 0ull;
 #pragma unroll
       for (int o = 8; o >= 1; o >>= 1) {
         const u64 other = __shfl_xor_sync(0xffffffffu, k, o);

@@ -70,11 +70,16 @@ static cudaError_t colfft_one(const ColFftArgs &a, unsigned blocks, cudaStream_t
   if constexpr (L1 >= 16) {
     // Nt = 256 / 512: two columns per thread in split format (kernels_colfft2.cuh) unless VOLKS_CF2=0
     const bool cf2 = a.split2 != 0;
+    const size_t smem8 = (size_t)a.nt * sizeof(float4) + (size_t)L1 * 16 * 8 * sizeof(float4) + 16 * sizeof(u64);
     if (attr_only) {
-      const cudaError_t e = cudaFuncSetAttribute(k_colfft2<L1, NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      cudaError_t e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      if (e == cudaSuccess) e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem8);
       if (e != cudaSuccess) return e;
+    } else if (a.split2 == 2) {   // 16-column strips: twice the CTAs, 256 threads each
+      k_colfft2<L1, NZ, 8><<<blocks * 2, 256, smem8, st>>>(a);
+      return cudaSuccess;
     } else if (cf2) {
-      k_colfft2<L1, NZ><<<blocks, CF_WARPS * 32, smem, st>>>(a);
+      k_colfft2<L1, NZ, 16><<<blocks, CF_WARPS * 32, smem, st>>>(a);
       return cudaSuccess;
     }
   }
@@ -211,7 +216,7 @@ struct volks_plan {
   mutable cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
   mutable const float2 *d_cal = nullptr;   // volks_plan_set_cal: DEVICE cf32[nbl][nif][nchan] applied in the slab load
   int nslide = 0;                // widths on the sliding-sum path (k_fixup re-evaluates their outlier windows)
-  int cf_split2 = 1;             // VOLKS_CF2: k_colfft2 (two columns per thread, split format) for Nt = 256 / 512
+  int cf_split2 = 2;             // VOLKS_CF2: k_colfft2 (two columns per thread, split format) for Nt = 256 / 512
   int ai_psub = 1;               // f2 with nfa > 8192: nfa = ai_psub * row_nf (virtual sub-rows, kernels_generic.cuh)
   int row_nf = 0;                // size of the row transform (= sched.nf unless ai_psub > 1)
   size_t premod_off = 0;         // offset (float2) of the W_nfa table in d_tables
@@ -314,7 +319,7 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   size_t tw_total = (size_t)p->nf;
   const bool force_generic = env_is("VOLKS_PATH", "generic");
   const int seg_req = std::max(16, env_int("VOLKS_SLIDE_SEG", 256));
-  pl->cf_split2 = env_int("VOLKS_CF2", 1) != 0 ? 1 : 0;   // (k_colfft needs nf >= 32: Y rows are always pair-interleaved there)
+  pl->cf_split2 = env_int("VOLKS_CF2", 2);   // 2: 16-column strips (two 256-thread CTAs per SM), 1: 32-column strips, 0: k_colfft   // (k_colfft needs nf >= 32: Y rows are always pair-interleaved there)
   for (int q = 0; q < p->nwidths; ++q) {
     WidthPlan w;
     w.w = p->width[q]; w.s = p->stride[q]; w.nt = p->nt[q];
