@@ -131,8 +131,8 @@ __global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : 1) k_colfft
   constexpr int G = 32 / CP;                            // (t2 | rho) groups per warp
   constexpr int NW = CP;                                // warps per CTA
   extern __shared__ float4 cf_sm4[];
-  float4 *tw4s = cf_sm4;                                // [nt] rate twiddles (re, re, im, im)
-  float4 *S4 = cf_sm4 + a.nt;                           // [L1][16][CP] (X, Y) of a column pair
+  float4 *tw4s = cf_sm4;                                // [NW][16][G] pass-2 twiddles W_Nt^{rho k} (re, re, im, im), rho = G warp + hi
+  float4 *S4 = cf_sm4 + 512;                            // [L1][16][CP] (X, Y) of a column pair
   u64 *slots = (u64 *)(S4 + (size_t)L1 * 16 * CP);      // [NW] per-warp window keys
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int cp = lane & (CP - 1), hi = lane / CP;
@@ -144,11 +144,14 @@ __global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : 1) k_colfft
   const uint32_t rowb = (uint32_t)a.pitch * 8u;
   const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch) + (size_t)(tile * CP + cp) * 16u;
   u64 *keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
-  for (int i = threadIdx.x; i < a.nt; i += NW * 32) tw4s[i] = a.tw4[i];
+  // per-warp twiddle rows: the G values a warp reads for one k are adjacent (one conflict-free wavefront, no index arithmetic)
+  for (int i = threadIdx.x; i < 512; i += NW * 32) {
+    const uint32_t r = (uint32_t)(G * (i / (16 * G)) + i % G), k = (uint32_t)((i / G) & 15);
+    tw4s[i] = a.tw4[(r * k) & ((uint32_t)a.nt - 1u)];
+  }
   const int j0 = rg * a.wpc, j1 = min(a.nwin, j0 + a.wpc);
-  const uint32_t ntm = (uint32_t)a.nt - 1u;
   const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(S4);
-  const uint32_t twbase = (uint32_t)__cvta_generic_to_shared(tw4s);
+  const uint32_t twsrc = (uint32_t)__cvta_generic_to_shared(tw4s) + (uint32_t)(warp * 16 * G + hi) * 16u;
   // pass-1 role
   const int hb = warp & 1, t2 = (warp >> 1) + (16 / G) * hi;
   const uint32_t sdst = sbase + (uint32_t)(t2 * CP + cp) * 16u;
@@ -181,7 +184,8 @@ __global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : 1) k_colfft
       for (int k = 0; k < 16; ++k) {
         f32x2 zx2, zy2, wx, wy;
         cf2_lds(ssrc + (uint32_t)k * (16u * CP), zx2, zy2);
-        cf2_lds(twbase + (((rho * (uint32_t)k) & ntm) << 4), wx, wy);
+        if (k == 0) { X[0] = zx2; Y[0] = zy2; continue; }   // W^0 = 1
+        cf2_lds(twsrc + (uint32_t)k * (16u * G), wx, wy);
         // z * w = (zx wx - zy wy) + i (zx wy + zy wx)
         X[k] = fma2(zx2, wx, mul2(zy2, neg2(wy)));
         Y[k] = fma2(zx2, wy, mul2(zy2, wx));

@@ -70,16 +70,18 @@ static cudaError_t colfft_one(const ColFftArgs &a, unsigned blocks, cudaStream_t
   if constexpr (L1 >= 16) {
     // Nt = 256 / 512: two columns per thread in split format (kernels_colfft2.cuh) unless VOLKS_CF2=0
     const bool cf2 = a.split2 != 0;
-    const size_t smem8 = (size_t)a.nt * sizeof(float4) + (size_t)L1 * 16 * 8 * sizeof(float4) + 16 * sizeof(u64);
+    // k_colfft2: 512 twiddles + the strip S[L1][16][CP] + 16 slots
+    const size_t smem8 = 512 * sizeof(float4) + (size_t)L1 * 16 * 8 * sizeof(float4) + 16 * sizeof(u64);
+    const size_t smem16 = 512 * sizeof(float4) + (size_t)L1 * 16 * 16 * sizeof(float4) + 16 * sizeof(u64);
     if (attr_only) {
-      cudaError_t e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      cudaError_t e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem16);
       if (e == cudaSuccess) e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem8);
       if (e != cudaSuccess) return e;
     } else if (a.split2 == 2) {   // 16-column strips: twice the CTAs, 256 threads each
       k_colfft2<L1, NZ, 8><<<blocks * 2, 256, smem8, st>>>(a);
       return cudaSuccess;
     } else if (cf2) {
-      k_colfft2<L1, NZ, 16><<<blocks, CF_WARPS * 32, smem, st>>>(a);
+      k_colfft2<L1, NZ, 16><<<blocks, CF_WARPS * 32, smem16, st>>>(a);
       return cudaSuccess;
     }
   }
