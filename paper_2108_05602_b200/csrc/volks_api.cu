@@ -321,7 +321,7 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   size_t tw_total = (size_t)p->nf;
   const bool force_generic = env_is("VOLKS_PATH", "generic");
   const int seg_req = std::max(16, env_int("VOLKS_SLIDE_SEG", 256));
-  pl->cf_split2 = env_int("VOLKS_CF2", 2);   // 2: 16-column strips (two 256-thread CTAs per SM), 1: 32-column strips, 0: k_colfft   // (k_colfft needs nf >= 32: Y rows are always pair-interleaved there)
+  pl->cf_split2 = env_int("VOLKS_CF2", 2);   // 2: 16-column strips (two 256-thread CTAs per SM), 1: 32-column strips, 0: k_colfft (nf >= 32 there: Y rows are pair-interleaved)
   for (int q = 0; q < p->nwidths; ++q) {
     WidthPlan w;
     w.w = p->width[q]; w.s = p->stride[q]; w.nt = p->nt[q];

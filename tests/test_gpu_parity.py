@@ -127,6 +127,29 @@ def test_sliding_kernel_shapes(vb, oracle, shape):
     run_both(vb, oracle, vis, c, mode="fft")
 
 
+@pytest.mark.parametrize("cf2", ["2", "1", "0"])
+@pytest.mark.parametrize("shape", [
+    # Nt = 256 / 512 with stride != 1 or pad != 2: k_colfft2 (16- and 32-column strips) and k_colfft, every NZ
+    (1, 2, 300, 20, [1, 20, 40], [3, 7, 16], [256, 256, 512], 32),        # NZ = 1, 2, 4; one 32-column tile
+    (1, 1, 700, 50, [100, 200, 256], [25, 64, 100], [512, 256, 256], 64), # NZ = 8, 16, 16 (nt == w: no padding)
+    (2, 1, 600, 33, [300, 512], [50, 30], [512, 512], 128),               # NZ = 32 (nt == w), several strips
+])
+def test_colfft2_variants(vb, oracle, shape, cf2, monkeypatch):
+    """The two-columns-per-thread rate kernel (kernels_colfft2.cuh) in both strip widths, and the kernel it
+    replaced, against the oracle on the same inputs: every pruning depth NZ, windows of one CTA range,
+    a burst that gives a clear peak, and an all-zero span (tie-break -> index 0)."""
+    monkeypatch.setenv("VOLKS_CF2", cf2)
+    monkeypatch.setenv("VOLKS_CF_WPC", "8")                               # several window ranges per strip
+    nbl, nif, nap, nchan, widths, strides, nts, nf = shape
+    g = torch.Generator().manual_seed(nap * 13 + nchan)
+    vis = torch.view_as_complex(torch.randn((nbl, nif, nap, nchan, 2), generator=g) * 0.7071)
+    k = torch.arange(nchan)
+    vis[0, 0, nap // 3: nap // 3 + 30] += 0.8 * torch.exp(2j * np.pi * 3.0 * k / nf)   # delay bin 3
+    vis[0, 0, : 40] = 0                                                   # flagged span at the start
+    c = dict(widths=widths, strides=strides, nts=nts, nf=nf, snr_thresh=2.5)
+    run_both(vb, oracle, vis, c, mode="fft")
+
+
 def test_zero_windows_and_empty(vb):
     vis = torch.zeros((1, 1, 3, 8), dtype=torch.complex64)
     cands, n, peaks = vb.fringe_search(vis.cuda(), [4], [1], [8], 8, 6.0, want_peaks=True)
