@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : 1) k_colfft
   constexpr int G = 32 / CP;                            // (t2 | rho) groups per warp
   constexpr int NW = CP;                                // warps per CTA
   extern __shared__ float4 cf_sm4[];
-  float4 *tw4s = cf_sm4;                                // [NW][16][G] pass-2 twiddles W_Nt^{rho k} (re, re, im, im), rho = G warp + hi
+  float4 *tw4s = cf_sm4;                                // [NW][16][G] pass-2 twiddles W_Nt^{rho k} (re, re, im, im), rho = 2 (G (warp/2) + hi) + warp%2
   float4 *S4 = cf_sm4 + 512;                            // [L1][16][CP] (X, Y) of a column pair
   u64 *slots = (u64 *)(S4 + (size_t)L1 * 16 * CP);      // [NW] per-warp window keys
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -146,17 +146,23 @@ __global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : 1) k_colfft
   u64 *keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
   // per-warp twiddle rows: the G values a warp reads for one k are adjacent (one conflict-free wavefront, no index arithmetic)
   for (int i = threadIdx.x; i < 512; i += NW * 32) {
-    const uint32_t r = (uint32_t)(G * (i / (16 * G)) + i % G), k = (uint32_t)((i / G) & 15);
+    const int wi = i / (16 * G);
+    const uint32_t r = (uint32_t)(2 * (G * (wi >> 1) + i % G) + (wi & 1)), k = (uint32_t)((i / G) & 15);
     tw4s[i] = a.tw4[(r * k) & ((uint32_t)a.nt - 1u)];
   }
   const int j0 = rg * a.wpc, j1 = min(a.nwin, j0 + a.wpc);
+  __syncthreads();   // twiddle rows visible to both halves
   const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(S4);
   const uint32_t twsrc = (uint32_t)__cvta_generic_to_shared(tw4s) + (uint32_t)(warp * 16 * G + hi) * 16u;
   // pass-1 role
   const int hb = warp & 1, t2 = (warp >> 1) + (16 / G) * hi;
   const uint32_t sdst = sbase + (uint32_t)(t2 * CP + cp) * 16u;
   // pass-2 role
-  const uint32_t rho = (uint32_t)(G * warp + hi);
+  // the residues of a warp have the warp's parity hb: even and odd rho are two independent pipelines (pass 1 of
+  // parity hb feeds only pass 2 of parity hb), each the even / odd warps of the CTA behind its own named barrier
+  const uint32_t rho = (uint32_t)(2 * (G * (warp >> 1) + hi) + hb);
+  const bool p2_active = (warp >> 1) < L1 / (2 * G);
+  auto half_barrier = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(1 + hb), "r"(NW * 16) : "memory"); };
   const uint32_t ssrc = sbase + rho * (256u * CP) + (uint32_t)cp * 16u;
   constexpr bool PREFETCH = NZ <= 8;                    // NZ = 16 (+ pass 2's 64 registers) would spill
 
@@ -177,8 +183,8 @@ __global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : 1) k_colfft
     if (hb) cf2_pass1<L1, NZ, 1, CP>(zx, zy, sdst);
     else cf2_pass1<L1, NZ, 0, CP>(zx, zy, sdst);
     if constexpr (PREFETCH) load_window(j + 1);   // in flight during pass 2
-    __syncthreads();
-    if (warp < L1 / G) {
+    half_barrier();
+    if (p2_active) {
       f32x2 X[16], Y[16];
 #pragma unroll
       for (int k = 0; k < 16; ++k) {
@@ -208,9 +214,9 @@ __global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : 1) k_colfft
                                (rho + (uint32_t)L1 * s) * (uint32_t)a.nf + (uint32_t)(tile * 2 * CP + 2 * cp) + (colb ? 1u : 0u));
       }
     }
-    __syncthreads();
-    if (warp == 0) {
-      u64 k = lane < L1 / G && lane < NW ? slots[lane] : 0ull;
+    half_barrier();
+    if (warp == hb) {   // warps 0 and 1: the slots of their parity
+      u64 k = lane < L1 / (2 * G) && lane < NW / 2 ? slots[2 * lane + hb] : 0ull;
 #pragma unroll
       for (int o = 8; o >= 1; o >>= 1) {
         const u64 other = __shfl_xor_sync(0xffffffffu, k, o);
