@@ -98,6 +98,10 @@ __device__ __forceinline__ void cf2_sts(uint32_t addr, f32x2 a, f32x2 b) {
 }
 
 // pass 1 of one thread: parity HB of rho.  zx/zy: the NZ leading rows t2 + 16 t1 of the column pair.
+// bytes between consecutive rho in the strip S[rho][t2][pair]: 256 CP, plus 32 for CP = 4 so that the two groups of
+// a quarter warp (rho two apart, 64 B each) fall into different banks
+template <int CP> __host__ __device__ constexpr uint32_t cf2_rho_stride() { return 256u * CP + (CP == 4 ? 32u : 0u); }
+
 template <int L1, int NZ, int HB, int CP>
 __device__ __forceinline__ void cf2_pass1(const f32x2 (&zx)[NZ], const f32x2 (&zy)[NZ], uint32_t sdst) {
   constexpr int H = L1 / 2;
@@ -115,9 +119,9 @@ __device__ __forceinline__ void cf2_pass1(const f32x2 (&zx)[NZ], const f32x2 (&z
   }
   if constexpr (HB == 1) S2Twiddle<0, NZH, L1, H>::run(X, Y);
   FftDifS<H, NZH, 0, H>::run(X, Y);
-  // output i of the half transform is m = brev(i); rho = 2 m + HB; S[rho][t2][pair]: 256 CP bytes per rho
+  // output i of the half transform is m = brev(i); rho = 2 m + HB
 #pragma unroll
-  for (int i = 0; i < H; ++i) cf2_sts(sdst + (uint32_t)(2 * brev<H>(i) + HB) * (256u * CP), X[i], Y[i]);
+  for (int i = 0; i < H; ++i) cf2_sts(sdst + (uint32_t)(2 * brev<H>(i) + HB) * cf2_rho_stride<CP>(), X[i], Y[i]);
 }
 
 #ifndef CF2_MIN_CTAS8
@@ -125,15 +129,15 @@ __device__ __forceinline__ void cf2_pass1(const f32x2 (&zx)[NZ], const f32x2 (&z
 #endif
 // CP = column pairs per CTA (16: a 32-column strip, 512 threads; 8: a 16-column strip, 256 threads, several CTAs per SM)
 template <int L1, int NZ, int CP>
-__global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : 1) k_colfft2(ColFftArgs a) {
+__global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : CP == 4 ? 2 * CF2_MIN_CTAS8 : 1) k_colfft2(ColFftArgs a) {
   static_assert(L1 == 16 || L1 == 32, "Nt = 256 or 512");
-  static_assert(CP == 16 || CP == 8, "strip of 32 or 16 columns");
+  static_assert(CP == 16 || CP == 8 || CP == 4, "strip of 32, 16 or 8 columns");
   constexpr int G = 32 / CP;                            // (t2 | rho) groups per warp
   constexpr int NW = CP;                                // warps per CTA
   extern __shared__ float4 cf_sm4[];
   float4 *tw4s = cf_sm4;                                // [NW][16][G] pass-2 twiddles W_Nt^{rho k} (re, re, im, im), rho = 2 (G (warp/2) + hi) + warp%2
   float4 *S4 = cf_sm4 + 512;                            // [L1][16][CP] (X, Y) of a column pair
-  u64 *slots = (u64 *)(S4 + (size_t)L1 * 16 * CP);      // [NW] per-warp window keys
+  u64 *slots = (u64 *)((char *)S4 + (size_t)L1 * cf2_rho_stride<CP>());   // [NW] per-warp window keys
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int cp = lane & (CP - 1), hi = lane / CP;
   const int ntile = a.nf / (2 * CP);
@@ -155,7 +159,7 @@ __global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : 1) k_colfft
   const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(S4);
   const uint32_t twsrc = (uint32_t)__cvta_generic_to_shared(tw4s) + (uint32_t)(warp * 16 * G + hi) * 16u;
   // pass-1 role
-  const int hb = warp & 1, t2 = (warp >> 1) + (16 / G) * hi;
+  const int hb = warp & 1, t2 = G * (warp >> 1) + hi;   // the G rows of a warp are adjacent in S
   const uint32_t sdst = sbase + (uint32_t)(t2 * CP + cp) * 16u;
   // pass-2 role
   // the residues of a warp have the warp's parity hb: even and odd rho are two independent pipelines (pass 1 of
@@ -163,7 +167,7 @@ __global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : 1) k_colfft
   const uint32_t rho = (uint32_t)(2 * (G * (warp >> 1) + hi) + hb);
   const bool p2_active = (warp >> 1) < L1 / (2 * G);
   auto half_barrier = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(1 + hb), "r"(NW * 16) : "memory"); };
-  const uint32_t ssrc = sbase + rho * (256u * CP) + (uint32_t)cp * 16u;
+  const uint32_t ssrc = sbase + rho * cf2_rho_stride<CP>() + (uint32_t)cp * 16u;
   constexpr bool PREFETCH = NZ <= 8;                    // NZ = 16 (+ pass 2's 64 registers) would spill
 
   f32x2 zx[NZ], zy[NZ];

@@ -72,11 +72,16 @@ static cudaError_t colfft_one(const ColFftArgs &a, unsigned blocks, cudaStream_t
     const bool cf2 = a.split2 != 0;
     // k_colfft2: 512 twiddles + the strip S[L1][16][CP] + 16 slots
     const size_t smem8 = 512 * sizeof(float4) + (size_t)L1 * 16 * 8 * sizeof(float4) + 16 * sizeof(u64);
+    const size_t smem4 = 512 * sizeof(float4) + (size_t)L1 * (256 * 4 + 32) + 16 * sizeof(u64);
     const size_t smem16 = 512 * sizeof(float4) + (size_t)L1 * 16 * 16 * sizeof(float4) + 16 * sizeof(u64);
     if (attr_only) {
       cudaError_t e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem16);
       if (e == cudaSuccess) e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem8);
+      if (e == cudaSuccess) e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem4);
       if (e != cudaSuccess) return e;
+    } else if (a.split2 == 4) {   // 8-column strips: four times the CTAs, 128 threads each
+      k_colfft2<L1, NZ, 4><<<blocks * 4, 128, smem4, st>>>(a);
+      return cudaSuccess;
     } else if (a.split2 == 2) {   // 16-column strips: twice the CTAs, 256 threads each
       k_colfft2<L1, NZ, 8><<<blocks * 2, 256, smem8, st>>>(a);
       return cudaSuccess;

@@ -127,7 +127,7 @@ def test_sliding_kernel_shapes(vb, oracle, shape):
     run_both(vb, oracle, vis, c, mode="fft")
 
 
-@pytest.mark.parametrize("cf2", ["2", "1", "0"])
+@pytest.mark.parametrize("cf2", ["4", "2", "1", "0"])
 @pytest.mark.parametrize("shape", [
     # Nt = 256 / 512 with stride != 1 or pad != 2: k_colfft2 (16- and 32-column strips) and k_colfft, every NZ
     (1, 2, 300, 20, [1, 20, 40], [3, 7, 16], [256, 256, 512], 32),        # NZ = 1, 2, 4; one 32-column tile
