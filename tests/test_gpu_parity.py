@@ -148,6 +148,13 @@ def test_colfft2_variants(vb, oracle, shape, cf2, monkeypatch):
     vis[0, 0, : 40] = 0                                                   # flagged span at the start
     c = dict(widths=widths, strides=strides, nts=nts, nf=nf, snr_thresh=2.5)
     run_both(vb, oracle, vis, c, mode="fft")
+    # run to run bit-identical (the two parity pipelines of a CTA meet only in the ordered key maximum)
+    ref = None
+    for _ in range(3):
+        cands, n, peaks = vb.fringe_search(vis.cuda(), widths, strides, nts, nf, 2.5, want_peaks=True)
+        blob = (peaks.tobytes(), cands.tobytes())
+        assert ref is None or blob == ref
+        ref = blob
 
 
 def test_zero_windows_and_empty(vb):
