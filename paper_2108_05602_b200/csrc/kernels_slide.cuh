@@ -106,6 +106,7 @@ struct SlideState {
   // RING variant: shared-memory addresses of this lane's entry in the ring rows of the current block's
   // first leaving row (sm_out) and first entering row (sm_in); ring geometry in bytes
   uint32_t sm_out, sm_in, ring_lo, ring_hi, rrowb;
+  uint32_t twp, tw_lo, tw_hi;   // RING: this warp's twiddle row W_Nt^{rho t}, t = 0..Nt (shared memory), entry of the current block
 };
 
 // emit the window's contribution: per column the max of (power with its 4 low mantissa bits replaced
@@ -164,10 +165,12 @@ __device__ __forceinline__ void lds2(uint32_t addr, f32x2 &a, f32x2 &b) {
 
 // load the operands of the update t -> t+1 (rows t and t+w of both columns, warp-uniform twiddle).
 // BN = t - (first window of the current 16-step block), 0..16 (compile time; RING only).
-template <int L, bool MODD, bool RING, int BN>
+// RR: bytes per ring row when known at compile time (0: S.rrowb) - the row offsets become immediates
+template <int L, bool MODD, bool RING, int BN, int RR>
 __device__ __forceinline__ void slide_prefetch(SlideState<L> &S, uint32_t t) {
   if constexpr (RING) {
-    uint32_t ao = S.sm_out + BN * S.rrowb, ai = S.sm_in + BN * S.rrowb;
+    const uint32_t rrowb = RR ? (uint32_t)RR : S.rrowb;
+    uint32_t ao = S.sm_out + BN * rrowb, ai = S.sm_in + BN * rrowb;
     if constexpr (BN == 16) {   // first row of the next block: the ring may wrap here (and only here)
       ao = ao >= S.ring_hi ? ao - (S.ring_hi - S.ring_lo) : ao;
       ai = ai >= S.ring_hi ? ai - (S.ring_hi - S.ring_lo) : ai;
@@ -182,15 +185,16 @@ __device__ __forceinline__ void slide_prefetch(SlideState<L> &S, uint32_t t) {
     ldg2(S.pin + off, S.xin, S.yin);
     ldg2(S.pout + off, S.xout, S.yout);
   }
-  if constexpr (!MODD) ldg2(S.tw4 + (((S.rho * t) & S.ntmask) << 4), S.twx, S.twy);
+  if constexpr (RING) lds2(S.twp + BN * 16u, S.twx, S.twy);   // the warp's own row: consecutive entries, no index arithmetic
+  else if constexpr (!MODD) ldg2(S.tw4 + (((S.rho * t) & S.ntmask) << 4), S.twx, S.twy);
 }
 
 // advance window t0 -> t0+1;  B = t0 mod L (compile time).  Uses the operands prefetched one step
 // ago and prefetches those of t0+1.
-template <int L, int B, bool MODD, bool RING>
+template <int L, int B, bool MODD, bool RING, int RR>
 __device__ __forceinline__ void slide_update(SlideState<L> &S, uint32_t t0) {
   const f32x2 xin = S.xin, yin = S.yin, xout = S.xout, yout = S.yout, twx = S.twx, twy = S.twy;
-  slide_prefetch<L, MODD, RING, B + 1>(S, t0 + 1);
+  slide_prefetch<L, MODD, RING, B + 1, RR>(S, t0 + 1);
   if constexpr (MODD) {
     // M == 1, rho == 0: the thread holds every rate bin, both parities; W_Nt = W_L
     const SlideG Ge = slide_make_g(sub2(xin, xout), sub2(yin, yout));
@@ -207,15 +211,15 @@ __device__ __forceinline__ void slide_update(SlideState<L> &S, uint32_t t0) {
 }
 
 // L consecutive steps starting at t0 (t0 mod L == 0).  GUARD: only windows < tend exist.
-template <int L, int B, bool MODD, bool GUARD, bool RING>
+template <int L, int B, bool MODD, bool GUARD, bool RING, int RR>
 struct SlideSteps {
   static __device__ __forceinline__ void run(SlideState<L> &S, uint32_t t0, uint32_t tend, u64 *slot) {
     if constexpr (B < L) {
       if (!GUARD || t0 + B < tend) {
         slide_emit<L>(S, slot + B * SLIDE_WARPS);
-        if (!GUARD || t0 + B + 1 < tend) slide_update<L, B, MODD, RING>(S, t0 + B);
+        if (!GUARD || t0 + B + 1 < tend) slide_update<L, B, MODD, RING, RR>(S, t0 + B);
       }
-      SlideSteps<L, B + 1, MODD, GUARD, RING>::run(S, t0, tend, slot);
+      SlideSteps<L, B + 1, MODD, GUARD, RING, RR>::run(S, t0, tend, slot);
     }
   }
 };
@@ -272,7 +276,7 @@ __device__ __forceinline__ void slide_ring_fill(const SlideRing &G, uint32_t r0,
 }
 
 // L = min(16, Nt) bins per thread;  MODD <=> M == 1 (Nt <= 16);  RING (M >= 4 only): rows through shared memory.
-template <int L, bool MODD, bool RING>
+template <int L, bool MODD, bool RING, int RR = 0>
 __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(SlideArgs a) {
   // blockDim.x = 32 * min(SLIDE_WARPS, ndt * M): every warp of a CTA works on the same (pair, segment)
   __shared__ u64 slots[2][16 * SLIDE_WARPS];
@@ -319,11 +323,19 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
     S.ring_hi = S.ring_lo + G.R * G.rrowb;
     S.sm_out = S.ring_lo;                                             // rel 0
     S.sm_in = S.ring_lo + (uint32_t)a.w * G.rrowb;                    // rel w
+    // twiddle rows behind the ring: [warp][Nt + 1] float4, entry t = W_Nt^{rho t} pre-broadcast (entry Nt = entry 0)
+    S.tw_lo = G.base + G.R * G.rrowb + (uint32_t)warp * (uint32_t)(a.nt + 1) * 16u;
+    S.tw_hi = S.tw_lo + (uint32_t)a.nt * 16u;
+    S.twp = S.tw_lo;                                                  // T0 = 0 mod Nt
+    for (uint32_t i = lane; i <= (uint32_t)a.nt; i += 32u) {
+      const float4 v = __ldg(a.tw4 + ((S.rho * i) & S.ntmask));
+      asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(S.tw_lo + i * 16u), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+    }
     slide_ring_fill(G, 0u, (uint32_t)a.w + 17u);                      // rows of block 0 (and the start window)
     asm volatile("cp.async.wait_all;" ::: "memory");
     __syncthreads();
   }
-  slide_prefetch<L, MODD, RING, 0>(S, T0);
+  slide_prefetch<L, MODD, RING, 0, RR>(S, T0);
   {
     float2 Aa[L], Ab[L];
     slide_start_column<L, MODD>(Aa, S.pout, S.rowb, T0, (uint32_t)a.w, a.twt, S.rho, S.ntmask, 0);
@@ -336,14 +348,15 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   for (;; t0 += L, buf ^= 1u) {
     const bool full = t0 + L < tend;
     if constexpr (RING) slide_ring_fill(G, t0 - T0 + (uint32_t)a.w + 17u, 16u);   // the next block's new rows
-    if (full) SlideSteps<L, 0, MODD, false, RING>::run(S, t0, tend, &slots[buf][warp]);
-    else SlideSteps<L, 0, MODD, true, RING>::run(S, t0, tend, &slots[buf][warp]);
+    if (full) SlideSteps<L, 0, MODD, false, RING, RR>::run(S, t0, tend, &slots[buf][warp]);
+    else SlideSteps<L, 0, MODD, true, RING, RR>::run(S, t0, tend, &slots[buf][warp]);
     if constexpr (RING) asm volatile("cp.async.wait_all;" ::: "memory");
     slide_flush(S.keyp, slots[buf], t0, full ? (uint32_t)L : tend - t0, nwarps);
     if (!full) break;
     if constexpr (RING) {   // advance the block base by 16 rows (wraps only at a block boundary)
       S.sm_out += 16u * S.rrowb; S.sm_out = S.sm_out >= S.ring_hi ? S.sm_out - (S.ring_hi - S.ring_lo) : S.sm_out;
       S.sm_in += 16u * S.rrowb;  S.sm_in = S.sm_in >= S.ring_hi ? S.sm_in - (S.ring_hi - S.ring_lo) : S.sm_in;
+      S.twp += 16u * 16u;        S.twp = S.twp >= S.tw_hi ? S.twp - (S.tw_hi - S.tw_lo) : S.twp;
     }
   }
 }

@@ -201,8 +201,13 @@ static void launch_slide(const SlideArgs &a, cudaStream_t st) {
   if (a.nt >= 32) {
     // M >= 4: rows travel through a shared-memory ring of (w + 48) x 512 * (column groups) bytes
     const int dtc = std::max(1, wpb >> a.log2m);
-    const size_t ring = (size_t)(a.w + 48) * 512 * dtc;
-    if (a.log2m >= 2 && ring <= 100 * 1024) k_slide<16, false, true><<<blocks, thr, ring, st>>>(a);
+    // + the warps' twiddle rows ([wpb][Nt + 1] float4) behind the ring
+    const size_t ring = (size_t)(a.w + 48) * 512 * dtc + (size_t)wpb * (a.nt + 1) * 16;
+    if (a.log2m >= 2 && ring <= 100 * 1024) {
+      if (dtc == 1) k_slide<16, false, true, 512><<<blocks, thr, ring, st>>>(a);
+      else if (dtc == 2) k_slide<16, false, true, 1024><<<blocks, thr, ring, st>>>(a);
+      else k_slide<16, false, true><<<blocks, thr, ring, st>>>(a);
+    }
     else k_slide<16, false, false><<<blocks, thr, 0, st>>>(a);
   }
   else if (a.nt == 16) k_slide<16, true, false><<<blocks, thr, 0, st>>>(a);
@@ -451,6 +456,8 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
       ok = cuda_ok(launch_colfft(ca, w.cf_l1, w.cf_nz, 0, nullptr, true));
     }
   ok = ok && cuda_ok(cudaFuncSetAttribute(k_slide<16, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+  ok = ok && cuda_ok(cudaFuncSetAttribute(k_slide<16, false, true, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+  ok = ok && cuda_ok(cudaFuncSetAttribute(k_slide<16, false, true, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
   if (ok && (p->nf == 4096 || p->nf == 8192)) {
     RowArgs ra; memset(&ra, 0, sizeof ra);
     ra.paired = pl->paired; ra.nf = p->nf; ra.nchan = p->nchan; ra.nrows = 1;
