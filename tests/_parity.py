@@ -79,3 +79,54 @@ def check_candidates(gpu_cands, ora_cands, ora_peaks, keep, thresh, nf):
         assert abs(float(g["snr"]) - o["snr"]) <= RTOL * o["snr"]
         n += 1
     return n, nmarg_all
+
+
+def allif_plane_power(oracle, band, nw, widths, strides, nfa):
+    """Tie callback for the all-IF search: the ORACLE's power of delay bin `idx` of canonical window i,
+    from the rate-0 row of the oracle's own plane of that band window (oracle.allif_search's definition)."""
+    per = sum(nw)
+
+    def plane_power(i, idx):
+        b, r = divmod(i, per)
+        q = 0
+        while r >= nw[q]:
+            r -= nw[q]
+            q += 1
+        w, s = widths[q], strides[q]
+        nt = 1
+        while nt < w:
+            nt *= 2
+        _, plane = oracle.window(band[b, r * s: r * s + w], nt, nfa, mode="fft", want_plane=True)
+        z = plane[0, idx]
+        return float(z.real * z.real + z.imag * z.imag)
+    return plane_power
+
+
+def canonical_index(cands, nif, nw, bl0=0):
+    """Canonical window index c = (pair * per_pair + offc[q] + j) of candidate records, with pairs counted
+    from baseline `bl0` (a search over a slice of baselines)."""
+    nw = np.asarray(nw, dtype=np.int64)
+    offc = np.concatenate([[0], np.cumsum(nw)[:-1]])
+    pair = (cands["bl"].astype(np.int64) - bl0) * nif + cands["ifq"].astype(np.int64)
+    return pair * int(nw.sum()) + offc[cands["wid"]] + cands["win"].astype(np.int64)
+
+
+def check_candidates_whole(gpu_cands, gidx, ora_cands, ora_peaks, keep, thresh):
+    """check_candidates for lists of millions of records (vectorised; the same rule): `gidx` / `keep` are
+    the canonical window indices of the GPU / oracle candidates.  Ordered, duplicate-free; every firm oracle
+    candidate present; every extra marginal BY THE ORACLE'S snr; matched records agree in t0, power, snr.
+    Returns (#matched, #missing marginal, #extra marginal, #marginal windows in the slice)."""
+    assert np.all(np.diff(gidx) > 0), "GPU candidates not in canonical order / duplicated"
+    osnr = ora_peaks["snr"]
+    marginal = np.abs(osnr - thresh) <= RTOL * thresh
+    in_o = np.isin(gidx, keep, assume_unique=True)
+    missing = keep[~np.isin(keep, gidx, assume_unique=True)]
+    assert np.all(marginal[missing]), "missing candidates at windows %s (oracle snr %s)" % (missing[:5], osnr[missing[:5]])
+    extra = gidx[~in_o]
+    assert np.all(marginal[extra]), "unexpected candidates at windows %s (oracle snr %s)" % (extra[:5], osnr[extra[:5]])
+    pos = np.searchsorted(keep, gidx[in_o])
+    g, o = gpu_cands[in_o], ora_cands[pos]
+    assert np.array_equal(g["t0"], o["t0"]) and np.array_equal(g["wid"], o["wid"]) and np.array_equal(g["win"], o["win"])
+    assert np.all(np.abs(g["power"].astype(np.float64) - o["power"]) <= RTOL * o["power"])
+    assert np.all(np.abs(g["snr"].astype(np.float64) - o["snr"]) <= RTOL * o["snr"])
+    return int(in_o.sum()), int(missing.size), int(extra.size), int(marginal.sum())

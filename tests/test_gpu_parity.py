@@ -5,7 +5,7 @@ import pytest
 import torch
 
 import workloads
-from _parity import check_candidates, check_peaks, dense_index
+from _parity import allif_plane_power, check_candidates, check_peaks, dense_index
 
 pytestmark = pytest.mark.gpu
 
@@ -369,15 +369,7 @@ def test_allif_search_matches_oracle(vb, oracle, shape):
     assert np.all(pk["rate_idx"] == 0)
     band = oracle.allif_band(src)
 
-    def plane_power(i, idx):       # oracle power of one delay bin of canonical window i
-        per = sum(nw)
-        b, r = divmod(i, per)
-        q = 0
-        while r >= nw[q]:
-            r -= nw[q]; q += 1
-        a = np.fft.fft(band[b, r * strides[q]: r * strides[q] + widths[q]].astype(np.complex128).sum(axis=0), nfa)[idx]
-        return float(abs(a) ** 2)
-    check_peaks(pk, ora, nfa, plane_power)
+    check_peaks(pk, ora, nfa, allif_plane_power(oracle, band, nw, widths, strides, nfa))
     exp = np.nonzero(ora["snr"] > thresh)[0]
     marg = np.abs(ora["snr"] - thresh) <= 1e-4 * thresh
     assert abs(n - len(exp)) <= int(marg.sum()) and n >= 1
@@ -613,13 +605,37 @@ def test_random_allif_shapes(vb, oracle, seed):
     nw = [workloads.gen.nwin(nap, w, s) for w, s in zip(widths, strides)]
     band = oracle.allif_band(src)
 
-    def plane_power(i, idx):
-        b, r = divmod(i, sum(nw))
-        q = 0
-        while r >= nw[q]:
-            r -= nw[q]; q += 1
-        a = np.fft.fft(band[b, r * strides[q]: r * strides[q] + widths[q]].astype(np.complex128).sum(axis=0), nfa)[idx]
-        return float(abs(a) ** 2)
-    check_peaks(peaks[dense_index(nbl, 1, nw)], ora, nfa, plane_power)
+    check_peaks(peaks[dense_index(nbl, 1, nw)], ora, nfa, allif_plane_power(oracle, band, nw, widths, strides, nfa))
     marg = np.abs(ora["snr"] - 3.0) <= 1e-4 * 3.0
     assert abs(n - np.count_nonzero(ora["snr"] > 3.0)) <= int(marg.sum())
+
+
+def test_cufft_cross_check(vb, oracle):
+    """Pin P12 on the GPU side (north_star: "cuFFT only as a cross-check"; the transform is PAPER.md:83): a
+    handful of zero-padded planes formed by torch.fft.fft2 (cuFFT C2C, complex64) as a third opinion beside
+    the library's dense peaks and the oracle.  Test-only: nothing under paper_2108_05602_b200/ touches cuFFT."""
+    for cfg, over in [(1, {}), (2, dict(nbl=1, nif=2, nap=300, npulses=2)), (4, dict(nbl=1, nif=1, nap=300, npulses=1))]:
+        vis, c, _ = workloads.generate(cfg, **over)
+        nbl, nif, nap, nchan = vis.shape
+        dv = vis.cuda()
+        _, _, peaks = vb.fringe_search(dv, c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"], want_peaks=True)
+        nw = [workloads.gen.nwin(nap, w, s) for w, s in zip(c["widths"], c["strides"])]
+        rng = np.random.default_rng(40 + cfg)
+        for _ in range(6):
+            q = int(rng.integers(0, len(nw)))
+            pair, j = int(rng.integers(0, nbl * nif)), int(rng.integers(0, nw[q]))
+            w, s, nt, nf = c["widths"][q], c["strides"][q], c["nts"][q], c["nf"]
+            win = dv[pair // nif, pair % nif, j * s: j * s + w]
+            P = torch.fft.fft2(win, s=(nt, nf)).abs().square().double().cpu().numpy().reshape(-1)   # cuFFT
+            g = peaks[nbl * nif * sum(nw[:q]) + pair * nw[q] + j]
+            o, _ = oracle.window(win.cpu().numpy(), nt, nf, mode="fft")
+            gi = int(g["rate_idx"]) * nf + int(g["delay_idx"])
+            # cuFFT is itself fp32: the library's bin must carry cuFFT's maximum to within fp32 rounding, and
+            # where the oracle's argmax is unambiguous all three name the same bin
+            assert P[gi] >= P.max() * (1 - 1e-5)
+            assert abs(P.max() - o["p1"]) <= 1e-4 * o["p1"] and abs(float(g["power"]) - P.max()) <= 1e-4 * P.max()
+            if (o["p1"] - o["p2"]) / o["p1"] > 1e-4:
+                assert int(np.argmax(P)) == o["idx1"] == gi
+            assert abs(P.sum() / (nt * nf) - o["s1"] / (nt * nf)) <= 1e-4 * o["s1"] / (nt * nf)
+            noise = P.sum() / (nt * nf)
+            assert abs(float(g["snr"]) - np.sqrt(P.max() / noise)) <= 1e-4 * o["snr"]

@@ -313,6 +313,70 @@ def test_window_match_vs_python_graph_search(oracle):
     assert [(int(p["rep"]), int(p["nwidths_hit"]), int(p["t_begin"]), int(p["t_end"])) for p in got] == expect
 
 
+def test_baseline_match_constructions(oracle):
+    """f3 pins ON THE ORACLE (PAPER.md:198 "identified if it is detected with at least 5 baselines";
+    DESIGN.md A19): hand-built pulse lists whose answer is fixed by the rule itself."""
+    def run(rows, m):
+        bl, tb, te, snr = (np.array(x) for x in zip(*rows))
+        return oracle.baseline_match(bl, snr, tb, te, m)
+    # five baselines, pairwise overlapping extents -> one detection; extent = union; rep = max snr
+    five = [(b, 100 + b, 110 + b, 7.0 + b) for b in range(5)]
+    d = run(five, 5)
+    assert d == [dict(rep=4, nbaselines=5, t_begin=100, t_end=114)]
+    # four of them -> dropped at min_baselines 5, kept at 4
+    assert run(five[:4], 5) == []
+    assert run(five[:4], 4) == [dict(rep=3, nbaselines=4, t_begin=100, t_end=113)]
+    # the same baseline twice counts once
+    rep = [(0, 10, 20, 8.0), (0, 12, 22, 9.0), (1, 15, 25, 7.0)]
+    assert run(rep, 3) == []
+    assert run(rep, 2) == [dict(rep=1, nbaselines=2, t_begin=10, t_end=25)]
+    # chain: A and C do not overlap but both overlap B -> one cluster of 3 baselines; D is apart
+    chain = [(0, 0, 10, 6.5), (1, 9, 20, 6.6), (2, 19, 30, 6.4), (3, 40, 50, 9.0)]
+    assert run(chain, 3) == [dict(rep=1, nbaselines=3, t_begin=0, t_end=30)]
+    assert [x["rep"] for x in run(chain, 1)] == [1, 3]
+    # touching extents [0, 10) and [10, 20) do NOT link (half-open AP intervals)
+    touch = [(0, 0, 10, 7.0), (1, 10, 20, 7.0)]
+    assert run(touch, 2) == []
+    assert [x["nbaselines"] for x in run(touch, 1)] == [1, 1]
+    # ... one AP of overlap does
+    assert run([(0, 0, 11, 7.0), (1, 10, 20, 7.0)], 2) == [dict(rep=0, nbaselines=2, t_begin=0, t_end=20)]
+    # containment links; snr tie -> lowest index; output ordered by t_begin
+    two = [(0, 300, 400, 7.0), (1, 350, 360, 7.0), (2, 100, 120, 9.0), (3, 110, 130, 8.0)]
+    assert run(two, 2) == [dict(rep=2, nbaselines=2, t_begin=100, t_end=130), dict(rep=0, nbaselines=2, t_begin=300, t_end=400)]
+    # input order must not matter (components of a graph): permute the chain
+    perm = [chain[i] for i in (3, 2, 0, 1)]
+    d = run(perm, 3)
+    assert len(d) == 1 and (d[0]["nbaselines"], d[0]["t_begin"], d[0]["t_end"]) == (3, 0, 30) and perm[d[0]["rep"]][3] == 6.6
+    assert oracle.baseline_match(np.zeros(0, int), np.zeros(0), np.zeros(0, int), np.zeros(0, int), 1) == []
+
+
+def test_baseline_match_vs_sweep(oracle):
+    """Independent statement of the same rule: interval-overlap components on a line are the maximal
+    runs, in t_begin order, whose start lies before the running end (a sweep, no graph)."""
+    rng = np.random.default_rng(12)
+    for trial in range(30):
+        n = int(rng.integers(1, 70))
+        bl = rng.integers(0, 8, n)
+        tb = rng.integers(0, 500, n)
+        te = tb + rng.integers(1, 25, n)
+        snr = rng.integers(60, 90, n) / 10.0
+        got = oracle.baseline_match(bl, snr, tb, te, 3)
+        order = sorted(range(n), key=lambda i: (tb[i], i))
+        exp, i = [], 0
+        while i < n:
+            end, k, members = te[order[i]], i + 1, [order[i]]
+            while k < n and tb[order[k]] < end:
+                end = max(end, te[order[k]])
+                members.append(order[k])
+                k += 1
+            if len({int(bl[m]) for m in members}) >= 3:
+                best = max(sorted(members), key=lambda m: (snr[m], -m))
+                exp.append(dict(rep=best, nbaselines=len({int(bl[m]) for m in members}), t_begin=int(tb[order[i]]), t_end=int(end)))
+            i = k
+        exp.sort(key=lambda d: (d["t_begin"], d["rep"]))
+        assert got == exp
+
+
 def test_dedispersion_pins(oracle):
     """f1: per frequency point a time shift.  Pins: zero shift is the identity; a
     pulse dispersed by known shifts is restored sample for sample; samples shifted in from beyond the
