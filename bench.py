@@ -8,8 +8,11 @@ and windows of the config; candidates compacted).  Prints ONE JSON line on rank 
   value      windows/s with the visibility slab already resident in HBM (device-timed, CUDA events)
   e2e        the same metric through the public API with HOST buffers: pinned host -> device copy of
              the slab and device -> host read of the candidate list inside the timed region
-  roofline   dominant kernel: algorithmic flops per launch / live CUDA-event duration vs the FP32
-             FMA peak (bound "alu"; DESIGN.md derives the peak and the per-unit flops)
+  roofline   dominant kernel: EXECUTED flops per launch / live CUDA-event duration vs the FP32 FMA peak
+             measured in the same run (volks_measure_fp32_peak; bound "alu"; DESIGN.md section 6 states the
+             per-unit flops); the SURVEY 8(d) algorithmic count is printed beside it, labelled
+  other_configs  configs[3] and configs[4] timed the same way (default run only), so that north_star's
+             "configs[2-4]" are all driver-visible
   cpu_baseline  the float64 oracle, as it stands, on the host cores, on a bounded sample
 With --impl reference the oracle itself is the timed program (rank 0 only).
 """
@@ -44,6 +47,8 @@ def parse_args():
     ap.add_argument("--impl", default="volks", choices=["volks", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="default run only: skip the extra timing of configs[3] and configs[4]")
     ap.add_argument("--peaks", action="store_true", help="also write the dense per-window peak array")
     ap.add_argument("--allif", action="store_true",
                     help="time f2 instead: VOLKS2's all-IF one-delay search (Eq. 1) on the config's slab, band padded x2")
@@ -178,9 +183,19 @@ def run_reference(args):
     }))
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` captures (profiles/r01_ncu_rate_kernels.md); keyed by (config, kernel, width)
-NCU_TRAFFIC = {(2, "slide", 64): 3.97e9, (4, "colfft", 64): 3.97e9}
+def ncu_traffic_table():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the rate kernels, parsed from the committed
+    ncu summary profiles/dram_traffic.csv (columns: config,kernel,width,dram_bytes_per_launch,source; the
+    commands that made it are in profiles/dram_traffic.md).  Missing file or row -> traffic null."""
+    tab = {}
+    path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    if os.path.exists(path):
+        for line in open(path).read().splitlines()[1:]:
+            f = line.split(",")
+            if len(f) >= 4:
+                tab[(int(f[0]), f[1], int(f[2]))] = (float(f[3]), f[4] if len(f) > 4 else "")
+    return tab
+
 
 def max_over_ranks(dist, ms, device):
     """Replicas only: the one cross-rank step is the MAX of the device-timed
@@ -197,46 +212,68 @@ def aggregate_value(world, units_per_rank, ms_step):
     return world * units_per_rank / (ms_step * 1e-3)
 
 
-KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6: "slide", 7: "colfft", 8: "allif", 9: "fixup"}
+KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6: "slide", 7: "colfft", 8: "allif", 9: "fixup",
+              10: "winthr"}
 
 
-def run_volks(args):
-    import paper_2108_05602_b200 as vk
-    vk.lib()                                   # fails loudly if the CUDA library is missing
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
+def executed_flops_per_launch(c, kind, wid, nlaunch, npair, nap, alg_flops):
+    """Flops the kernel really executes per launch.  The sliding kernel does one complex
+    multiply-add (4 FMA = 8 flops) + |.|^2 (3 flops) per bin per window instead of an FFT: 11 per bin; the
+    FFT kernels execute the SURVEY 8(d) algorithmic count at most (pruned inputs: fewer), which is what is
+    charged to them.  profiles/ holds the ncu instruction counters these figures are checked against."""
+    if kind in (6, 11) and wid >= 0:
+        w_, nt_ = c["widths"][wid], c["nts"][wid]
+        return workloads.gen.nwin(nap, w_, 1) * npair * nt_ * c["nf"] * 11.0 / nlaunch
+    return alg_flops
 
-    # N independent replicas (DESIGN.md "Multi-GPU": the path needs no exchange; north_star fixes one
-    # GPU, so --gpus N runs N replicas, each the full config with its own seed)
-    vis, c, _ = workloads.generate(args.config, device=dev, seed=workloads.config(args.config)["seed"] + 17 * rank)
+
+def measure_fp32_peak(vk, local, stream):
+    """The FP32 FMA peak measured in this run (volks_measure_fp32_peak: dependent-free FFMA chains, CUDA
+    events, best of 5 launches of ~20 ms), with the SM clock sampled while it runs."""
+    smp = ClockSampler(local, period=0.02)
+    smp.start()
+    best, mean, ms = vk.measure_fp32_peak(5, stream)
+    smp.stop_flag = True
+    smp.join()
+    ck = smp.summary()
+    derived = SM_COUNT * FP32_LANES_PER_SM * 2 * (ck["sm_max_mhz"] or 1965) * 1e6 / 1e12
+    return {"tflops": best, "tflops_mean": mean, "launch_ms": ms, "sm_mhz": ck["sm_mhz"], "reasons": ck["reasons"],
+            "derived_tflops": derived,
+            "kind": "measured: volks_measure_fp32_peak (FFMA chains, 64 warps/SM, best of 5 launches; SM clock median "
+                    "%s MHz during the probe); derived 148 SM x 128 lanes x 2 x sm_max_mhz = %.2f" % (ck["sm_mhz"], derived)}
+
+
+def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traffic):
+    """Device-timed throughput + per-launch roofline of one config.  Returns a dict (tensors included, for
+    the e2e leg of the main config)."""
+    vis, c, _ = workloads.generate(cfg_id, device=dev, seed=workloads.config(cfg_id)["seed"] + 17 * rank)
     nbl, nif, nap, nchan = vis.shape
     if args.allif:
         # band padded x2, or x4 = the paper's padding factor (PAPER.md:83) for the EL060-shaped config 5
-        nfa = workloads.gen.next_pow2((4 if args.config == 5 else 2) * nif * nchan)
+        nfa = workloads.gen.next_pow2((4 if cfg_id == 5 else 2) * nif * nchan)
         plan = vk.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], None, nfa, c["snr_thresh"], allif=True)
     else:
         plan = vk.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"])
-    cap = 1 << 20
+    stream = torch.cuda.current_stream(dev)
     ws = torch.empty(plan.workspace_bytes, dtype=torch.uint8, device=dev)
-    cands = torch.empty(cap * vk.CAND_DTYPE.itemsize, dtype=torch.uint8, device=dev)
     ncand = torch.zeros(1, dtype=torch.int32, device=dev)
     peaks = torch.empty(plan.nwin_total * vk.PEAK_DTYPE.itemsize, dtype=torch.uint8, device=dev) if args.peaks else None
-    stream = torch.cuda.current_stream(dev)
-
     shift = None
     if args.dm:
         # IFs of 16 MHz above 1400 MHz (L band, like EL060: PAPER.md:172-173), referenced to the top frequency
         f = 1400.0 + 16.0 * np.arange(nif)[:, None] + (16.0 / nchan) * np.arange(nchan)[None, :]
         shift = torch.as_tensor(vk.dm_shifts(args.dm, f, f.max(), c["t_ap"]), device=dev)
+
+    # candidate capacity from the plan's own count: one sizing run (the count is the true total even when the
+    # list overflows), then a buffer that holds the whole list
+    cap = 1 << 16
+    cands = torch.empty(cap * vk.CAND_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+    plan.fringe_search(vis, ws, cands, ncand, peaks, stream, shift=shift)
+    torch.cuda.synchronize(dev)
+    n0 = int(ncand.item()) & 0xFFFFFFFF
+    if n0 > cap:
+        cap = (n0 + (1 << 16)) & ~((1 << 16) - 1)
+        cands = torch.empty(cap * vk.CAND_DTYPE.itemsize, dtype=torch.uint8, device=dev)
 
     def step():
         plan.fringe_search(vis, ws, cands, ncand, peaks, stream, shift=shift)
@@ -246,7 +283,7 @@ def run_volks(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(max(warmup, 3)):
         step()
     barrier()
     sampler = ClockSampler(local)
@@ -254,7 +291,7 @@ def run_volks(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record(stream)
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     e1.record(stream)
     barrier()
@@ -262,11 +299,12 @@ def run_volks(args):
     sampler.stop_flag = True
     sampler.join()
     ms_total = max_over_ranks(dist, ms_total, dev)
-    ms_step = ms_total / args.steps
+    ms_step = ms_total / steps
     nwin = plan.nwin_total
     nvis = nbl * nif * nap * nchan
+    world = int(os.environ.get("WORLD_SIZE", "1"))
     value = aggregate_value(world, nwin, ms_step)
-    n_found = int(ncand.item())
+    n_found = int(ncand.item()) & 0xFFFFFFFF
 
     # ---- roofline leg: per-launch CUDA-event durations on the launching stream ----
     plan.profile(True)
@@ -284,80 +322,81 @@ def run_volks(args):
     step_sum = sum(share.values())
     dom = max(share, key=share.get)
     dom_ms_avg = float(np.mean(per[dom]))
-    if dom[0] == 2:       # column kernel of width dom[1]: one launch per chunk of pairs
-        dom_flops = per_w_alg[dom[1]] / nlaunch[dom]
-    elif dom[0] in (6, 7):     # sliding-sum / column-FFT kernel of width dom[1]
-        dom_flops = (per_w_alg[dom[1]] if dom[1] >= 0 else sum(per_w_alg)) / nlaunch[dom]
-    elif dom[0] == 1:
-        dom_flops = row_alg / nlaunch[dom]
-    else:
-        dom_flops = 0.0
-    # flops the dominant kernel actually executes per launch: the sliding kernel does
-    # one complex multiply-add (4 FMA = 8 flops) + |.|^2 (3 flops) per bin per window instead of an FFT
-    if dom[0] == 6:
-        w_, nt_ = c["widths"][dom[1]], c["nts"][dom[1]]
-        exec_flops = workloads.gen.nwin(nap, w_, 1) * nbl * nif * nt_ * c["nf"] * 11.0 / nlaunch[dom]
-    else:
-        exec_flops = dom_flops
+    kname = "%s[w=%s]" % (KIND_NAMES.get(dom[0], str(dom[0])), c["widths"][dom[1]] if dom[1] >= 0 else "all")
+    kernel_ms = {"%s[%d]" % (KIND_NAMES.get(k[0], str(k[0])), k[1]): round(v, 4) for k, v in sorted(share.items())}
     clocks = sampler.summary()
+    base = dict(vk=vk, plan=plan, vis=vis, c=c, ws=ws, cands=cands, ncand=ncand, peaks=peaks, stream=stream, dev=dev,
+                rank=rank, world=world, dist=dist, ms_step=ms_step, value=value, nwin=nwin, nvis=nvis, n_found=n_found,
+                clocks=clocks, cap=cap, shift=shift)
     if args.allif:
         # f2 is bandwidth work: the row pass reads the slab once and writes the all-IF delay spectra, every
         # width's k_allif reads them once.  Roofline of the dominant kernel against measured HBM bandwidth.
         peaks_json = os.path.join(ROOT, "MEASURED_PEAKS.json")
         hbm = json.load(open(peaks_json))["hbm_gbs"] if os.path.exists(peaks_json) else 6650.0
-        ybytes = nbl * nap * (plan.nf + 16) * 8.0
+        pitch = plan.nf + 16 if plan.nf <= 8192 else plan.nf      # the plan's Y row pitch (sub-rows are contiguous)
+        ybytes = nbl * nap * pitch * 8.0
         dom_bytes = (ybytes + nvis * 8.0 if dom[0] == 1 else ybytes) / nlaunch[dom]
         gbs = dom_bytes / (dom_ms_avg * 1e-3) / 1e9
-        roofline = {"bound": "hbm", "kernel": "%s[w=%s]" % (KIND_NAMES[dom[0]], c["widths"][dom[1]] if dom[1] >= 0 else "all"),
-                    "achieved": gbs, "peak": hbm, "unit": "GB/s", "frac": gbs / hbm, "traffic": None,
-                    "launch_ms": dom_ms_avg, "share_of_step": share[dom] / step_sum,
-                    "peak_kind": "measured (MEASURED_PEAKS.json hbm_gbs)" if os.path.exists(peaks_json) else "fallback 6650 GB/s",
-                    "bytes_kind": "algorithmic: the chunk's all-IF delay spectra read once (row pass: + the slab read once)",
-                    "kernel_ms": {"%s[%d]" % (KIND_NAMES[k[0]], k[1]): round(v, 4) for k, v in sorted(share.items())}}
-        return dict(vk=vk, plan=plan, vis=vis, c=c, ws=ws, cands=cands, ncand=ncand, peaks=peaks, stream=stream,
-                    dev=dev, rank=rank, world=world, dist=dist, ms_step=ms_step, value=value, nwin=nwin, nvis=nvis,
-                    n_found=n_found, roofline=roofline, clocks=clocks, cap=cap, shift=shift)
-    peak_tf = SM_COUNT * FP32_LANES_PER_SM * 2 * (clocks["sm_max_mhz"] or 1965) * 1e6 / 1e12
-    achieved_tf = dom_flops / (dom_ms_avg * 1e-3) / 1e12
+        base["roofline"] = {
+            "bound": "hbm", "kernel": kname, "achieved": gbs, "peak": hbm, "unit": "GB/s", "frac": gbs / hbm,
+            "traffic": None, "launch_ms": dom_ms_avg, "share_of_step": share[dom] / step_sum,
+            "peak_kind": "measured (MEASURED_PEAKS.json hbm_gbs)" if os.path.exists(peaks_json) else "fallback 6650 GB/s",
+            "bytes_kind": "algorithmic: the chunk's all-IF delay spectra read once (row pass: + the slab read once)",
+            "kernel_ms": kernel_ms}
+        return base
+    if dom[0] == 1:
+        dom_alg = row_alg / nlaunch[dom]
+    elif dom[1] >= 0:
+        dom_alg = per_w_alg[dom[1]] / nlaunch[dom]
+    else:
+        dom_alg = 0.0
+    exec_flops = executed_flops_per_launch(c, dom[0], dom[1], nlaunch[dom], nbl * nif, nap, dom_alg)
+    peak_tf = peak["tflops"]
+    exec_tf = exec_flops / (dom_ms_avg * 1e-3) / 1e12
+    alg_tf = dom_alg / (dom_ms_avg * 1e-3) / 1e12
+    tr = traffic.get((c["id"], KIND_NAMES.get(dom[0], ""), c["widths"][dom[1]] if dom[1] >= 0 else -1))
     roofline = {
-        "bound": "alu", "kernel": "%s[w=%s]" % (KIND_NAMES[dom[0]], c["widths"][dom[1]] if dom[1] >= 0 else "all"),
-        "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
-        "traffic": NCU_TRAFFIC.get((c["id"], KIND_NAMES[dom[0]], c["widths"][dom[1]] if dom[1] >= 0 else -1)),
-        "launch_ms": dom_ms_avg,
-        "executed_tflops": exec_flops / (dom_ms_avg * 1e-3) / 1e12,
-        "executed_frac": exec_flops / (dom_ms_avg * 1e-3) / 1e12 / peak_tf, "share_of_step": share[dom] / step_sum,
-        "peak_kind": "derived: 148 SM x 128 FP32 lanes x 2 flop (FMA) x sm_max_mhz (DESIGN.md)",
-        "flops_kind": "algorithmic (SURVEY 8(d)): shared delay FFT per AP + 5 Nt log2 Nt per column + 5 per bin",
+        "bound": "alu", "kernel": kname, "achieved": exec_tf, "peak": peak_tf, "unit": "TFLOP/s",
+        "frac": exec_tf / peak_tf, "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None,
+        "launch_ms": dom_ms_avg, "share_of_step": share[dom] / step_sum,
+        "flops_kind": "executed: sliding kernels 11 flops per bin per window (complex multiply-add + |.|^2), FFT kernels "
+                      "the SURVEY 8(d) count (5 Nt log2 Nt per column + 5 per bin; 5 Nf log2 Nf per AP row)",
+        "peak_kind": peak["kind"], "peak_derived_tflops": peak["derived_tflops"],
+        "algorithmic_tflops": alg_tf, "algorithmic_frac": alg_tf / peak_tf,
+        "algorithmic_kind": "SURVEY 8(d) FFT-equivalent flops / time: exceeds 1 by construction for the sliding path "
+                            "(an algorithmic speed-up, not a fraction of the machine)",
         "whole_step_algorithmic_tflops": tot_alg / (ms_step * 1e-3) / 1e12,
         "whole_step_nominal_tflops": nominal_flops(c) / (ms_step * 1e-3) / 1e12,
         "hbm_gbs_algorithmic": nvis * 8 / (ms_step * 1e-3) / 1e9,
-        "kernel_ms": {"%s[%d]" % (KIND_NAMES[k[0]], k[1]): round(v, 4) for k, v in sorted(share.items())},
+        "kernel_ms": kernel_ms,
     }
-    return dict(vk=vk, plan=plan, vis=vis, c=c, ws=ws, cands=cands, ncand=ncand, peaks=peaks, stream=stream,
-                dev=dev, rank=rank, world=world, dist=dist, ms_step=ms_step, value=value, nwin=nwin, nvis=nvis,
-                n_found=n_found, roofline=roofline, clocks=clocks, cap=cap, shift=shift)
+    if roofline["frac"] > 1.0:
+        roofline["error"] = "executed flops above the measured peak: the per-bin accounting is wrong"
+    base["roofline"] = roofline
+    return base
 
 
 def run_e2e(R, steps):
     """Same metric through the public API with HOST buffers: every step copies the slab from pinned
-    host memory to the device, runs the search and reads the candidate list back."""
+    host memory to the device, runs the search and reads the WHOLE candidate list back."""
     vk, plan, dev, stream = R["vk"], R["plan"], R["dev"], R["stream"]
     h_vis = torch.empty(R["vis"].shape, dtype=torch.complex64, pin_memory=True)
     h_vis.copy_(R["vis"])
     h_n = torch.zeros(1, dtype=torch.int32, pin_memory=True)
     h_c = torch.empty(R["cap"] * vk.CAND_DTYPE.itemsize, dtype=torch.uint8, pin_memory=True)
-    d_vis = R["vis"]
-    d2h = 0
+    d2h, overflow = 0, False
 
     stage = torch.empty(2 * plan.stage_bytes, dtype=torch.uint8, device=dev)
 
     def step():
-        nonlocal d2h
+        nonlocal d2h, overflow
         # the public host-slab call: chunked pinned-host -> device copies overlapped with the kernels
         plan.search_host(h_vis, stage, R["ws"], R["cands"], R["ncand"], R["peaks"], stream, shift=R["shift"])
         h_n.copy_(R["ncand"], non_blocking=True)
         stream.synchronize()
-        n = min(int(h_n.item()), R["cap"]) * vk.CAND_DTYPE.itemsize
+        nf_ = int(h_n.item()) & 0xFFFFFFFF
+        overflow = overflow or nf_ > R["cap"]
+        n = min(nf_, R["cap"]) * vk.CAND_DTYPE.itemsize
         if n:
             h_c[:n].copy_(R["cands"][:n], non_blocking=True)
             stream.synchronize()
@@ -376,7 +415,18 @@ def run_e2e(R, steps):
     ms = e0.elapsed_time(e1)
     ms = max_over_ranks(R["dist"], ms, dev) / steps
     return {"value": R["world"] * R["nwin"] / (ms * 1e-3), "unit": "windows/s", "ms_per_step": ms,
-            "h2d_bytes_per_step": int(h_vis.numel() * 8), "d2h_bytes_per_step": int(d2h)}
+            "h2d_bytes_per_step": int(h_vis.numel() * 8), "d2h_bytes_per_step": int(d2h),
+            "candidates_read_back": int((d2h - 4) // vk.CAND_DTYPE.itemsize), "overflow": bool(overflow)}
+
+
+def brief(R):
+    """The part of a measurement that goes under other_configs."""
+    rf = R["roofline"]
+    return {"workload": workload_name(R["c"]), "ms_per_step": R["ms_step"], "windows_per_s": R["value"],
+            "visibilities_per_s": R["world"] * R["nvis"] / (R["ms_step"] * 1e-3), "windows": R["nwin"],
+            "candidates": R["n_found"], "clocks": R["clocks"],
+            "roofline": {k: rf[k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic", "launch_ms",
+                                            "share_of_step", "algorithmic_frac", "kernel_ms") if k in rf}}
 
 
 def main():
@@ -384,9 +434,41 @@ def main():
     if args.impl == "reference":
         run_reference(args)
         return
-    R = run_volks(args)
+    import paper_2108_05602_b200 as vk
+    vk.lib()                                   # fails loudly if the CUDA library is missing
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    traffic = ncu_traffic_table()
+    # N independent replicas (DESIGN.md "Multi-GPU": the path needs no exchange; north_star fixes one
+    # GPU, so --gpus N runs N replicas, each the full config with its own seed)
+    peak = measure_fp32_peak(vk, local, torch.cuda.current_stream(dev))
+    R = measure(vk, args, args.config, dev, local, rank, dist, args.steps, args.warmup, peak, traffic)
     c = R["c"]
     e2e = None if args.no_e2e else run_e2e(R, max(1, min(args.steps, 3)))
+    launches = R["plan"].launches * args.steps
+    plan_nf = R["plan"].nf
+    others = {}
+    if args.config == 2 and not args.allif and not args.dm and not args.no_other_configs:
+        main_line = {k: R[k] for k in ("value", "ms_step", "nwin", "nvis", "n_found", "clocks", "roofline", "world", "rank")}
+        R["plan"].close()
+        R = None
+        torch.cuda.empty_cache()
+        for other in (3, 4):
+            Ro = measure(vk, args, other, dev, local, rank, dist, max(1, min(args.steps, 3)), 3, peak, traffic)
+            others[str(other)] = brief(Ro)
+            Ro["plan"].close()
+            Ro = None
+            torch.cuda.empty_cache()
+        R = main_line
     cpu = None
     if R["rank"] == 0 and R["world"] == 1 and not args.no_cpu_baseline:
         from oracle import volks_oracle
@@ -406,15 +488,17 @@ def main():
                        "l2": "input slab (%.2f GB) larger than L2, no flush needed" % (R["nvis"] * 8 / 1e9)
                        if R["nvis"] * 8 > 126e6 else "input smaller than L2 (latency-bound config, report only)",
                        "replicas": R["world"], "dense_peaks": bool(args.peaks), "dm": args.dm,
-                       "search": "f2 all-IF one-delay search (Eq. 1), nfa %d" % R["plan"].nf if args.allif else "2-D per-IF fringe search"},
+                       "search": "f2 all-IF one-delay search (Eq. 1), nfa %d" % plan_nf if args.allif else "2-D per-IF fringe search"},
             "visibilities_per_s": R["world"] * R["nvis"] / (R["ms_step"] * 1e-3),
             "windows": R["nwin"], "candidates": R["n_found"],
-            "clocks": R["clocks"], "e2e": e2e, "gpu_launches": R["plan"].launches * args.steps,
-            "roofline": R["roofline"], "cpu_baseline": cpu,
+            "clocks": R["clocks"], "e2e": e2e, "gpu_launches": launches,
+            "roofline": R["roofline"], "cpu_baseline": cpu, "fp32_peak_probe": {k: peak[k] for k in ("tflops", "tflops_mean", "launch_ms", "sm_mhz", "reasons", "derived_tflops")},
         }
+        if others:
+            out["other_configs"] = others
         print(json.dumps(out))
-    if R["dist"] is not None:
-        R["dist"].destroy_process_group()
+    if dist is not None:
+        dist.destroy_process_group()
 
 
 if __name__ == "__main__":

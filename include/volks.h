@@ -58,7 +58,8 @@ typedef struct {
   const int32_t *width;         /* HOST [nwidths] w_q >= 1 APs                  */
   const int32_t *stride;        /* HOST [nwidths] s_q >= 1 APs; partial windows are dropped        */
   const int32_t *nt;            /* HOST [nwidths] padded time size: power of two, >= w_q           */
-  int32_t nf;                   /* padded frequency size: power of two, >= nchan     */
+  int32_t nf;                   /* padded frequency size: power of two, nchan <= nf <= 8192        */
+                                /* (PAPER.md:83); larger: VOLKS_EINVAL                             */
   float snr_thresh;             /* candidate iff snr > snr_thresh              */
 } volks_params;
 
@@ -82,12 +83,33 @@ typedef struct {
   int32_t t_begin, t_end; /* union AP extent [t_begin, t_end) of the cluster                       */
 } volks_pulse;
 
+/* Tuning and test options of a plan.  HOST memory; volks_options_init fills the defaults, then change what is
+ * needed and pass it to volks_plan_create_opt / volks_plan_create_allif_opt (NULL = the defaults).  The library
+ * reads no environment variables. */
+typedef struct {
+  int32_t struct_bytes;  /* sizeof(volks_options), set by volks_options_init; a mismatch is VOLKS_EINVAL            */
+  int32_t full_index;    /* 0 (default): a search WITHOUT d_peaks keeps the exact (rate, delay) index only for the   */
+                         /* windows that can be candidates (the stride-1 kernels then skip the per-bin index tags;   */
+                         /* candidates are bit-identical either way).  1: exact index for every window in every      */
+                         /* search - what volks_zscore_select needs from the search before it                        */
+  int32_t force_generic; /* 1: the generic kernels (k_row_fft, k_col) for every width (the parity suite runs both)   */
+  int32_t slide_seg;     /* windows per exactly restarted segment of the sliding kernel (default 256, >= 16)         */
+  int32_t y_pad;         /* padding elements of a row of delay spectra (default 16; even, 0..1024)                   */
+  int32_t chunk_mb;      /* MiB of delay spectra per chunk of (bl, ifq) pairs (default 4096; bounds the workspace)    */
+  int32_t cf_wpc;        /* windows per CTA of the column-FFT kernels (default 128)                                  */
+  int32_t cf2;           /* Nt = 256 / 512: 2 (default) 16-column strips, 1: 32-column, 4: 8-column, 0: k_colfft    */
+  int32_t ai_waves;      /* f2: waves of 296 CTAs the window segments of k_allif are sized for (default 2)           */
+  int32_t host_split;    /* volks_search_host copies 1/host_split of a plan chunk at a time (default 4)              */
+} volks_options;
+void volks_options_init(volks_options *o);
+
 typedef struct volks_plan volks_plan; /* opaque */
 
 /* Validate `p` (HOST), build the window schedule (per width: window count, kernel variant, grid
  * shape, canonical offsets) and upload the twiddle tables.  Uses the current CUDA device.
  * nap < w_q gives zero windows for that width, not an error.  *out receives the plan. */
 int volks_plan_create(const volks_params *p, volks_plan **out);
+int volks_plan_create_opt(const volks_params *p, const volks_options *opt, volks_plan **out);
 int volks_plan_destroy(volks_plan *plan);
 
 /* Sizes the caller needs.  All outputs HOST, each nullable.  nwin_per_width[q] counts windows of
@@ -136,6 +158,7 @@ int volks_fringe_search_dd(const volks_plan *plan, const void *d_vis, const int3
  * volks_zscore_select, volks_window_match (ifq = -1 groups a baseline) and volks_baseline_match apply
  * to its results unchanged. */
 int volks_plan_create_allif(const volks_params *p, volks_plan **out);
+int volks_plan_create_allif_opt(const volks_params *p, const volks_options *opt, volks_plan **out);
 int volks_allif_search(const volks_plan *plan, const void *d_vis, const int32_t *d_shift, void *d_workspace,
                        volks_peak *d_peaks, volks_cand *d_cands, uint32_t cand_capacity,
                        uint32_t *d_ncand, void *cuda_stream);
@@ -159,7 +182,9 @@ int volks_search_host(const volks_plan *plan, const void *h_vis, void *d_stage, 
  * left in `d_workspace` (same plan, workspace untouched since): per (bl, ifq, width) the window peak
  * powers P1_j are normalised across windows, z_j = (P1_j - mean)/std (population std; z = 0 if
  * std = 0); candidate iff z_j > z_thresh.  Outputs as volks_fringe_search, except that the `snr`
- * field of candidates (and of d_peaks, if given) carries z.  Asynchronous on `cuda_stream`. */
+ * field of candidates (and of d_peaks, if given) carries z.  Asynchronous on `cuda_stream`.
+ * The search before it must have kept every window's exact index: a plan created with volks_options.full_index
+ * = 1, or a search that wrote d_peaks; VOLKS_EINVAL otherwise. */
 int volks_zscore_select(const volks_plan *plan, void *d_workspace, float z_thresh, volks_peak *d_peaks,
                         volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand, void *cuda_stream);
 
@@ -213,7 +238,7 @@ int volks_baseline_match(const volks_pulse *pulses, uint32_t npulse, int32_t min
 int volks_bin_to_physical(int32_t nt, int32_t nf, int32_t rate_idx, int32_t delay_idx,
                           double ap_seconds, double chan_hz, double *rate_hz, double *delay_s);
 
-/* Number of kernels one volks_fringe_search enqueues (for launch accounting). */
+/* Number of kernels one volks_fringe_search (without d_peaks) enqueues (for launch accounting). */
 int volks_plan_launch_count(const volks_plan *plan);
 
 /* Optional per-launch timing for measurement (bench.py's roofline leg).  When enabled, every kernel
@@ -230,9 +255,19 @@ int volks_plan_launch_count(const volks_plan *plan);
 #define VOLKS_K_COLFFT 7   /* any stride, Nt 32..512: two-pass shared-memory column FFT + argmax    */
 #define VOLKS_K_ALLIF 8    /* f2: all-IF rate-0 window sums + argmax + noise                          */
 #define VOLKS_K_FIXUP 9    /* exact re-evaluation of the sliding widths' outlier windows               */
+#define VOLKS_K_WINTHR 10  /* per-window pre-thresholds of the candidates-only index mode              */
 int volks_plan_profile(volks_plan *plan, int enable);
 int volks_plan_profile_read(const volks_plan *plan, int32_t capacity, int32_t *kind, int32_t *wid,
                             float *ms, int32_t *n);
+
+/* Measurement helper (not on the search path): the FP32 FMA issue peak of the current device at the clocks it
+ * runs at - the denominator of bench.py's "alu" roofline (SURVEY 8(d) "the builder must
+ * measure it").  Launches `repeats` (1..1000) kernels of dependent-free FFMA chains (64 resident warps per SM,
+ * about 20 ms each on B200) on `cuda_stream`, times each with CUDA events and SYNCHRONISES; allocates and frees a
+ * small device buffer.  HOST outputs: *tflops_best = fastest launch, *tflops_mean, *ms_per_launch (the last two
+ * nullable).  Counts 2 flop per FMA per thread. */
+int volks_measure_fp32_peak(int32_t repeats, double *tflops_best, double *tflops_mean, double *ms_per_launch,
+                            void *cuda_stream);
 
 const char *volks_strerror(int code);
 int volks_version(void);

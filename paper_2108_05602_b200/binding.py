@@ -19,6 +19,7 @@ EXPORTS = (
     "volks_version", "volks_plan_profile", "volks_plan_profile_read", "volks_fringe_search_dd", "volks_dm_shifts",
     "volks_baseline_match", "volks_zscore_select", "volks_plan_create_allif", "volks_allif_search",
     "volks_plan_query_host", "volks_search_host", "volks_plan_set_cal", "volks_cal_phasors",
+    "volks_measure_fp32_peak", "volks_options_init", "volks_plan_create_opt", "volks_plan_create_allif_opt",
 )
 
 
@@ -28,6 +29,11 @@ class volks_params(ctypes.Structure):
                 ("width", ctypes.POINTER(ctypes.c_int32)), ("stride", ctypes.POINTER(ctypes.c_int32)),
                 ("nt", ctypes.POINTER(ctypes.c_int32)), ("nf", ctypes.c_int32),
                 ("snr_thresh", ctypes.c_float)]
+
+
+class volks_options(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in ("struct_bytes", "full_index", "force_generic", "slide_seg", "y_pad",
+                                              "chunk_mb", "cf_wpc", "cf2", "ai_waves", "host_split")]
 
 
 CAND_DTYPE = np.dtype([("bl", "<i4"), ("ifq", "<i4"), ("wid", "<i4"), ("win", "<i4"), ("t0", "<i4"),
@@ -54,12 +60,18 @@ def lib():
         L.volks_strerror.argtypes = [ctypes.c_int]
         L.volks_plan_create.argtypes = [ctypes.POINTER(volks_params), ctypes.POINTER(ctypes.c_void_p)]
         L.volks_plan_create_allif.argtypes = [ctypes.POINTER(volks_params), ctypes.POINTER(ctypes.c_void_p)]
+        L.volks_options_init.argtypes = [ctypes.POINTER(volks_options)]
+        L.volks_options_init.restype = None
+        L.volks_plan_create_opt.argtypes = [ctypes.POINTER(volks_params), ctypes.POINTER(volks_options), ctypes.POINTER(ctypes.c_void_p)]
+        L.volks_plan_create_allif_opt.argtypes = [ctypes.POINTER(volks_params), ctypes.POINTER(volks_options), ctypes.POINTER(ctypes.c_void_p)]
         L.volks_allif_search.argtypes = [ctypes.c_void_p] * 6 + [ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
         L.volks_plan_query_host.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_size_t)]
         L.volks_search_host.argtypes = [ctypes.c_void_p] * 7 + [ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
         L.volks_plan_set_cal.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
         L.volks_cal_phasors.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32,
                                         ctypes.c_double, ctypes.c_void_p]
+        L.volks_measure_fp32_peak.argtypes = [ctypes.c_int32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
+                                              ctypes.POINTER(ctypes.c_double), ctypes.c_void_p]
         L.volks_plan_destroy.argtypes = [ctypes.c_void_p]
         L.volks_plan_query.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_size_t),
                                        ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
@@ -96,28 +108,47 @@ def _check(rc):
         raise VolksError(rc)
 
 
-def plan_create_raw(nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh, allif=False):
-    """volks_plan_create[_allif]; returns (rc, handle) without raising (for error-path tests)."""
+def make_options(**kw):
+    """volks_options_init + keyword overrides (full_index, force_generic, slide_seg, y_pad, chunk_mb, cf_wpc, cf2,
+    ai_waves, host_split)."""
+    o = volks_options()
+    lib().volks_options_init(ctypes.byref(o))
+    for k, v in kw.items():
+        if k not in dict(volks_options._fields_) or k == "struct_bytes":
+            raise KeyError("unknown volks option %r" % k)
+        setattr(o, k, int(v))
+    return o
+
+
+def plan_create_raw(nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh, allif=False, options=None):
+    """volks_plan_create[_allif][_opt]; returns (rc, handle) without raising (for error-path tests).
+    options: None (defaults), a dict of overrides, or a volks_options."""
     n = len(widths)
     arr = lambda v: (ctypes.c_int32 * max(len(v), 1))(*[int(x) for x in v])
     w, s, t = arr(widths), arr(strides), arr(nts)
     p = volks_params(nbl, nif, nap, nchan, n, w, s, t, nf, float(snr_thresh))
     h = ctypes.c_void_p()
-    rc = (lib().volks_plan_create_allif if allif else lib().volks_plan_create)(ctypes.byref(p), ctypes.byref(h))
+    if options is None:
+        rc = (lib().volks_plan_create_allif if allif else lib().volks_plan_create)(ctypes.byref(p), ctypes.byref(h))
+    else:
+        o = make_options(**options) if isinstance(options, dict) else options
+        rc = (lib().volks_plan_create_allif_opt if allif else lib().volks_plan_create_opt)(
+            ctypes.byref(p), ctypes.byref(o), ctypes.byref(h))
     return rc, h
 
 
 class Plan:
     """volks_plan_* : validated parameters + window schedule + device tables."""
 
-    def __init__(self, nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh, allif=False):
-        """allif=True: the f2 plan (volks_plan_create_allif; `nts` ignored, nf = nfa)."""
+    def __init__(self, nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh, allif=False, options=None):
+        """allif=True: the f2 plan (volks_plan_create_allif; `nts` ignored, nf = nfa).
+        options: dict of volks_options overrides (e.g. dict(full_index=1)) or None."""
         self.allif = bool(allif)
         nts = [1] * len(widths) if allif else nts
         self.shape = (nbl, nif, nap, nchan)
         self.widths, self.strides, self.nts, self.nf = list(widths), list(strides), list(nts), nf
         self.snr_thresh = float(snr_thresh)
-        rc, self._h = plan_create_raw(nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh, allif)
+        rc, self._h = plan_create_raw(nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh, allif, options)
         _check(rc)
         ws, tot = ctypes.c_size_t(), ctypes.c_int64()
         per = (ctypes.c_int64 * len(widths))()
@@ -240,6 +271,14 @@ def baseline_match(pulses, min_baselines=5):
     return out[:n.value]
 
 
+def measure_fp32_peak(repeats=5, stream=None):
+    """volks_measure_fp32_peak -> (best TFLOP/s, mean TFLOP/s, ms per launch) on the current device."""
+    best, mean, ms = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    st = (stream or torch.cuda.current_stream()).cuda_stream
+    _check(lib().volks_measure_fp32_peak(int(repeats), ctypes.byref(best), ctypes.byref(mean), ctypes.byref(ms), st))
+    return best.value, mean.value, ms.value
+
+
 def bin_to_physical(nt, nf, rate_idx, delay_idx, ap_seconds, chan_hz):
     r, d = ctypes.c_double(), ctypes.c_double()
     _check(lib().volks_bin_to_physical(nt, nf, rate_idx, delay_idx, ap_seconds, chan_hz,
@@ -255,10 +294,11 @@ def dm_shifts(dm, f_chan_mhz, f_ref_mhz, ap_seconds):
     return out
 
 
-def allif_search(vis, widths, strides, nfa, snr_thresh, want_peaks=False, cand_capacity=1 << 20, shifts=None):
+def allif_search(vis, widths, strides, nfa, snr_thresh, want_peaks=False, cand_capacity=1 << 20, shifts=None,
+                 options=None):
     """One-shot f2 search (volks_plan_create_allif + volks_allif_search); returns like fringe_search."""
     nbl, nif, nap, nchan = vis.shape
-    plan = Plan(nbl, nif, nap, nchan, widths, strides, None, nfa, snr_thresh, allif=True)
+    plan = Plan(nbl, nif, nap, nchan, widths, strides, None, nfa, snr_thresh, allif=True, options=options)
     try:
         return fringe_search(vis, want_peaks=want_peaks, cand_capacity=cand_capacity, plan=plan, shifts=shifts)
     finally:
@@ -266,7 +306,7 @@ def allif_search(vis, widths, strides, nfa, snr_thresh, want_peaks=False, cand_c
 
 
 def fringe_search(vis, widths=None, strides=None, nts=None, nf=None, snr_thresh=None, want_peaks=False,
-                  cand_capacity=1 << 20, plan=None, shifts=None):
+                  cand_capacity=1 << 20, plan=None, shifts=None, options=None):
     """Convenience one-shot call: allocates workspace/outputs with torch, runs the search on the
     current stream, synchronises and returns (cands CAND_DTYPE[n], ncand_true, peaks|None)."""
     if not vis.is_cuda:
@@ -274,7 +314,7 @@ def fringe_search(vis, widths=None, strides=None, nts=None, nf=None, snr_thresh=
     own = plan is None
     if own:
         nbl, nif, nap, nchan = vis.shape
-        plan = Plan(nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh)
+        plan = Plan(nbl, nif, nap, nchan, widths, strides, nts, nf, snr_thresh, options=options)
     dev = vis.device
     ws = torch.empty(plan.workspace_bytes, dtype=torch.uint8, device=dev)
     cands = torch.empty(cand_capacity * CAND_DTYPE.itemsize, dtype=torch.uint8, device=dev)

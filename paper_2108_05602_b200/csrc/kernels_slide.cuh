@@ -54,6 +54,9 @@ struct SlideArgs {
   long long pair0;      // first pair of the chunk
   int nap, nf, w, nt, log2m, nwin, seg, nseg, pitch;
   uint32_t keymask;     // 0xFFFFFFF0, passed as data so that (p & mask) | id is ONE LOP3 (register mask)
+  // HY (candidates-only index mode): pre-threshold of every window of the chunk, as float bits, laid out like the
+  // keys but chunk-relative: thr[pl * per_pair + offc + t0] (k_winthr); unused by the fully tagged kernels
+  const uint32_t *thr;
 };
 
 // The per-step operand of one parity class, both columns: g = (GX, GY) and the (1 -+ i)/sqrt 2
@@ -130,6 +133,26 @@ __device__ __forceinline__ void slide_emit(const SlideState<L> &S, u64 *slot) {
     const uint32_t s = 15u - (km & 15u);
     *slot = make_key(__uint_as_float(km & 0xFFFFFFF0u), S.idx0 + s * S.idxs + (colb ? 1u : 0u));
   }
+}
+
+// HY emit: the window's maximum WITHOUT the bin tags (one 3-input max per bin instead of two LOP3 + the max), and
+// the tagged emit only when the warp's maximum exceeds the window's pre-threshold `thrbits` (k_winthr: 0.98 of the
+// power a candidate needs) - a warp-uniform branch that a noise window never takes.  Below it the slot carries the
+// (truncated) power alone: index word 0 = the lowest priority among equal powers, never reported, because a window
+// can only become a candidate through a warp that took the tagged path.  Powers are truncated like the tagged
+// keys (max then mask == mask then max), so both modes give bit-identical candidates.
+template <int L>
+__device__ __forceinline__ void slide_emit_hy(const SlideState<L> &S, u64 *slot, uint32_t thrbits) {
+  uint32_t ba = 0, bb = 0;
+#pragma unroll
+  for (int s = 0; s < L; ++s) {
+    const f32x2 pw = fma2(S.Y[s], S.Y[s], mul2(S.X[s], S.X[s]));
+    ba = max(ba, __float_as_uint(lo32(pw)));
+    bb = max(bb, __float_as_uint(hi32(pw)));
+  }
+  const uint32_t km = __reduce_max_sync(0xffffffffu, max(ba, bb));
+  if (km > thrbits) slide_emit<L>(S, slot);
+  else if (S.lane == 0) *slot = (u64)(km & 0xFFFFFFF0u) << 32;
 }
 
 // after a block of nsteps (<= 16) windows starting at t0: threads 0..nsteps-1 reduce the warps'
@@ -211,15 +234,22 @@ __device__ __forceinline__ void slide_update(SlideState<L> &S, uint32_t t0) {
 }
 
 // L consecutive steps starting at t0 (t0 mod L == 0).  GUARD: only windows < tend exist.
-template <int L, int B, bool MODD, bool GUARD, bool RING, int RR>
+// HY: thr_sm = shared address of the block's L pre-thresholds (float bits)
+template <int L, int B, bool MODD, bool GUARD, bool RING, int RR, bool HY>
 struct SlideSteps {
-  static __device__ __forceinline__ void run(SlideState<L> &S, uint32_t t0, uint32_t tend, u64 *slot) {
+  static __device__ __forceinline__ void run(SlideState<L> &S, uint32_t t0, uint32_t tend, u64 *slot, uint32_t thr_sm) {
     if constexpr (B < L) {
       if (!GUARD || t0 + B < tend) {
-        slide_emit<L>(S, slot + B * SLIDE_WARPS);
+        if constexpr (HY) {
+          uint32_t thrbits;
+          asm volatile("ld.shared.u32 %0, [%1];" : "=r"(thrbits) : "r"(thr_sm + 4u * B));   // pinned to its step
+          slide_emit_hy<L>(S, slot + B * SLIDE_WARPS, thrbits);
+        } else {
+          slide_emit<L>(S, slot + B * SLIDE_WARPS);
+        }
         if (!GUARD || t0 + B + 1 < tend) slide_update<L, B, MODD, RING, RR>(S, t0 + B);
       }
-      SlideSteps<L, B + 1, MODD, GUARD, RING, RR>::run(S, t0, tend, slot);
+      SlideSteps<L, B + 1, MODD, GUARD, RING, RR, HY>::run(S, t0, tend, slot, thr_sm);
     }
   }
 };
@@ -276,10 +306,12 @@ __device__ __forceinline__ void slide_ring_fill(const SlideRing &G, uint32_t r0,
 }
 
 // L = min(16, Nt) bins per thread;  MODD <=> M == 1 (Nt <= 16);  RING (M >= 4 only): rows through shared memory.
-template <int L, bool MODD, bool RING, int RR = 0>
+// HY: candidates-only index mode (slide_emit_hy).
+template <int L, bool MODD, bool RING, int RR = 0, bool HY = false>
 __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(SlideArgs a) {
   // blockDim.x = 32 * min(SLIDE_WARPS, ndt * M): every warp of a CTA works on the same (pair, segment)
   __shared__ u64 slots[2][16 * SLIDE_WARPS];
+  __shared__ uint32_t thrs[2][16];   // HY: pre-thresholds of the current / next block of L windows
   extern __shared__ float4 slide_ring[];
   const int nwarps = blockDim.x >> 5, warp = threadIdx.x >> 5;
   long long wt = (long long)blockIdx.x * nwarps + warp;
@@ -306,6 +338,13 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   S.keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
   const uint32_t T0 = (uint32_t)sg * (uint32_t)a.seg;                 // multiple of Nt and of L
   const uint32_t tend = min((uint32_t)a.nwin, T0 + (uint32_t)a.seg);  // windows [T0, tend)
+  const uint32_t *thrg = nullptr;
+  const uint32_t thr_sm = (uint32_t)__cvta_generic_to_shared(&thrs[0][0]);
+  if constexpr (HY) {
+    thrg = a.thr + (pl * a.per_pair + a.offc);
+    if (threadIdx.x < L) thrs[0][threadIdx.x] = T0 + threadIdx.x < tend ? __ldg(thrg + T0 + threadIdx.x) : 0xFFFFFFFFu;
+    if constexpr (!RING) __syncthreads();      // (RING: the barrier after the first ring fill orders it)
+  }
   SlideRing G;
   if constexpr (RING) {
     // the CTA's warps are (rho fastest, then dt): its first warp's dt is the first column group
@@ -348,8 +387,12 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   for (;; t0 += L, buf ^= 1u) {
     const bool full = t0 + L < tend;
     if constexpr (RING) slide_ring_fill(G, t0 - T0 + (uint32_t)a.w + 17u, 16u);   // the next block's new rows
-    if (full) SlideSteps<L, 0, MODD, false, RING, RR>::run(S, t0, tend, &slots[buf][warp]);
-    else SlideSteps<L, 0, MODD, true, RING, RR>::run(S, t0, tend, &slots[buf][warp]);
+    if constexpr (HY) {   // the next block's pre-thresholds (read after this block's flush barrier)
+      const uint32_t tn = t0 + L + threadIdx.x;
+      if (threadIdx.x < L) thrs[buf ^ 1u][threadIdx.x] = tn < tend ? __ldg(thrg + tn) : 0xFFFFFFFFu;
+    }
+    if (full) SlideSteps<L, 0, MODD, false, RING, RR, HY>::run(S, t0, tend, &slots[buf][warp], thr_sm + buf * 64u);
+    else SlideSteps<L, 0, MODD, true, RING, RR, HY>::run(S, t0, tend, &slots[buf][warp], thr_sm + buf * 64u);
     if constexpr (RING) asm volatile("cp.async.wait_all;" ::: "memory");
     slide_flush(S.keyp, slots[buf], t0, full ? (uint32_t)L : tend - t0, nwarps);
     if (!full) break;
@@ -359,6 +402,38 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
       S.twp += 16u * 16u;        S.twp = S.twp >= S.tw_hi ? S.twp - (S.tw_hi - S.tw_lo) : S.twp;
     }
   }
+}
+
+// Pre-thresholds of the HY mode: one thread per (pair of the chunk, sliding width, window):
+//   thr = SLIDE_PRE * snr_thresh^2 * sum_{t<w} E[t0 + t]   (the window energy = the noise of a7, summed in the
+// order k_finalize uses), stored as float bits.  A window is a candidate iff P1 > snr_thresh^2 * energy, so every
+// candidate's winning warp sees its maximum above thr and takes the tagged path.
+#ifndef SLIDE_PRE
+#define SLIDE_PRE 0.98f
+#endif
+struct WinThrArgs {
+  const float *E;        // [npair][nap] per-AP energies
+  uint32_t *thr;         // [pairs of the chunk][per_pair]
+  long long per_pair, pair0, total;   // total = pairs of the chunk * windows of the sliding widths per pair
+  float thr2;            // snr_thresh^2
+  int nap, nq;
+  int w[16], nwin[16];
+  long long offc[16], cum[17];        // cum: prefix sums of nwin over the listed widths
+};
+
+__global__ void __launch_bounds__(256) k_winthr(WinThrArgs a) {
+  const long long gid = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (gid >= a.total) return;
+  const long long per = a.cum[a.nq];
+  const long long pl = gid / per;
+  long long r = gid - pl * per;
+  int i = 0;
+  while (r >= a.cum[i + 1]) ++i;
+  const int j = (int)(r - a.cum[i]);
+  const float *e = a.E + (a.pair0 + pl) * a.nap + j;
+  float es = 0.f;
+  for (int t = 0; t < a.w[i]; ++t) es += e[t];
+  a.thr[pl * a.per_pair + a.offc[i] + j] = __float_as_uint(SLIDE_PRE * a.thr2 * es);
 }
 
 }  // namespace volks

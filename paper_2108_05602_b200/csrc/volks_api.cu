@@ -15,6 +15,7 @@
 #include "kernels_colfft.cuh"
 #include "kernels_allif.cuh"
 #include "kernels_fixup.cuh"
+#include "kernels_probe.cuh"
 
 using namespace volks;
 
@@ -42,19 +43,8 @@ struct WidthPlan {
   bool colfft;          // two-pass shared-memory column FFT (kernels_colfft.cuh): Nt = 32..512, nf % 32 == 0
   int cf_l1, cf_nz, cf_wpc, cf_nrange;
   int seg, nseg;        // sliding path: windows per exactly restarted segment, segments per pair
+  bool hy;              // sliding path: eligible for the candidates-only index mode (k_slide HY)
 };
-
-// Tuning / test switches read once per plan (documented in DESIGN.md "Kernel selection"):
-//   VOLKS_PATH=generic   force the generic multi-pass kernels for every width
-//   VOLKS_SLIDE_SEG=n    windows per restarted segment of the sliding kernel (default 256)
-int env_int(const char *name, int dflt) {
-  const char *v = getenv(name);
-  return v && *v ? atoi(v) : dflt;
-}
-bool env_is(const char *name, const char *val) {
-  const char *v = getenv(name);
-  return v && strcmp(v, val) == 0;
-}
 
 template <int L>
 static void launch_col(const ColArgs &a, cudaStream_t st) {
@@ -192,7 +182,8 @@ static bool launch_row2(const RowArgs &a, cudaStream_t st) {
   return row2_nz<8, 8>(a, nza, blocks, st);
 }
 
-static void launch_slide(const SlideArgs &a, cudaStream_t st) {
+// hy: candidates-only index mode (kernels_slide.cuh slide_emit_hy; widths with Nt >= 32 only)
+static void launch_slide(const SlideArgs &a, bool hy, cudaStream_t st) {
   // every warp of a CTA must share its (pair, segment): warps per CTA = min(SLIDE_WARPS, ndt * M)
   const long long per_seg = (long long)(a.nf / 64) << a.log2m;
   const int wpb = (int)std::min<long long>(SLIDE_WARPS, per_seg);
@@ -204,15 +195,33 @@ static void launch_slide(const SlideArgs &a, cudaStream_t st) {
     // + the warps' twiddle rows ([wpb][Nt + 1] float4) behind the ring
     const size_t ring = (size_t)(a.w + 48) * 512 * dtc + (size_t)wpb * (a.nt + 1) * 16;
     if (a.log2m >= 2 && ring <= 100 * 1024) {
-      if (dtc == 1) k_slide<16, false, true, 512><<<blocks, thr, ring, st>>>(a);
-      else if (dtc == 2) k_slide<16, false, true, 1024><<<blocks, thr, ring, st>>>(a);
-      else k_slide<16, false, true><<<blocks, thr, ring, st>>>(a);
+      if (hy) {
+        if (dtc == 1) k_slide<16, false, true, 512, true><<<blocks, thr, ring, st>>>(a);
+        else if (dtc == 2) k_slide<16, false, true, 1024, true><<<blocks, thr, ring, st>>>(a);
+        else k_slide<16, false, true, 0, true><<<blocks, thr, ring, st>>>(a);
+      } else {
+        if (dtc == 1) k_slide<16, false, true, 512><<<blocks, thr, ring, st>>>(a);
+        else if (dtc == 2) k_slide<16, false, true, 1024><<<blocks, thr, ring, st>>>(a);
+        else k_slide<16, false, true><<<blocks, thr, ring, st>>>(a);
+      }
     }
+    else if (hy) k_slide<16, false, false, 0, true><<<blocks, thr, 0, st>>>(a);
     else k_slide<16, false, false><<<blocks, thr, 0, st>>>(a);
   }
   else if (a.nt == 16) k_slide<16, true, false><<<blocks, thr, 0, st>>>(a);
   else if (a.nt == 8) k_slide<8, true, false><<<blocks, thr, 0, st>>>(a);
   else k_slide<4, true, false><<<blocks, thr, 0, st>>>(a);
+}
+
+// the ring kernels' dynamic shared memory limit (per device, process-wide: set before every plan's first use)
+static bool slide_attrs() {
+  const int lim = 100 * 1024;
+  return cudaFuncSetAttribute(k_slide<16, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
+         cudaFuncSetAttribute(k_slide<16, false, true, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
+         cudaFuncSetAttribute(k_slide<16, false, true, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
+         cudaFuncSetAttribute(k_slide<16, false, true, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
+         cudaFuncSetAttribute(k_slide<16, false, true, 512, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
+         cudaFuncSetAttribute(k_slide<16, false, true, 1024, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess;
 }
 
 }  // namespace
@@ -228,7 +237,12 @@ struct volks_plan {
   mutable cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
   mutable const float2 *d_cal = nullptr;   // volks_plan_set_cal: DEVICE cf32[nbl][nif][nchan] applied in the slab load
   int nslide = 0;                // widths on the sliding-sum path (k_fixup re-evaluates their outlier windows)
-  int cf_split2 = 2;             // VOLKS_CF2: k_colfft2 (two columns per thread, split format) for Nt = 256 / 512
+  volks_options opt;             // the options the plan was created with (defaults: volks_options_init)
+  int nhy = 0;                   // sliding widths eligible for the candidates-only index mode
+  size_t off_thr = 0;            // their windows' pre-thresholds (k_winthr), chunk-relative
+  mutable bool last_full_index = true;   // the most recent search left exact indices for EVERY window (volks_zscore_select)
+  int device = 0;                // the CUDA device the plan was created on
+  int cf_split2 = 2;             // opt.cf2: k_colfft2 (two columns per thread, split format) for Nt = 256 / 512
   int ai_psub = 1;               // f2 with nfa > 8192: nfa = ai_psub * row_nf (virtual sub-rows, kernels_generic.cuh)
   int row_nf = 0;                // size of the row transform (= sched.nf unless ai_psub > 1)
   size_t premod_off = 0;         // offset (float2) of the W_nfa table in d_tables
@@ -282,11 +296,20 @@ const char *volks_strerror(int code) {
   }
 }
 
-static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif, int ai_nchan, int psub = 1);
+static int plan_create_impl(const volks_params *p, const volks_options *o, volks_plan **out, int ai_nif, int ai_nchan, int psub = 1);
 
-int volks_plan_create(const volks_params *p, volks_plan **out) { return plan_create_impl(p, out, 0, 0); }
+void volks_options_init(volks_options *o) {
+  if (!o) return;
+  memset(o, 0, sizeof *o);
+  o->struct_bytes = (int32_t)sizeof(volks_options);
+  o->slide_seg = 256; o->y_pad = 16; o->chunk_mb = 4096; o->cf_wpc = 128; o->cf2 = 2; o->ai_waves = 2; o->host_split = 4;
+}
 
-int volks_plan_create_allif(const volks_params *p, volks_plan **out) {
+int volks_plan_create(const volks_params *p, volks_plan **out) { return plan_create_impl(p, nullptr, out, 0, 0); }
+int volks_plan_create_opt(const volks_params *p, const volks_options *o, volks_plan **out) { return plan_create_impl(p, o, out, 0, 0); }
+int volks_plan_create_allif(const volks_params *p, volks_plan **out) { return volks_plan_create_allif_opt(p, nullptr, out); }
+
+int volks_plan_create_allif_opt(const volks_params *p, const volks_options *o, volks_plan **out) {
   if (!p || !out) return VOLKS_EINVAL;
   *out = nullptr;
   if (p->nbl < 1 || p->nif < 1 || p->nchan < 1 || p->nwidths < 1 || p->nwidths > VOLKS_MAX_WIDTHS) return VOLKS_EINVAL;
@@ -299,16 +322,25 @@ int volks_plan_create_allif(const volks_params *p, volks_plan **out) {
   // nfa > 8192 (EL060: 8 IF x 1024 x pad 4 = 32768): psub interleaved 8192-point transforms per AP
   const int psub = p->nf > 8192 ? p->nf / 8192 : 1;
   b.nf = p->nf / psub;
-  return plan_create_impl(&b, out, p->nif, p->nchan, psub);
+  return plan_create_impl(&b, o, out, p->nif, p->nchan, psub);
 }
 
-static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif, int ai_nchan, int psub) {
+static int plan_create_impl(const volks_params *p, const volks_options *o, volks_plan **out, int ai_nif, int ai_nchan, int psub) {
   if (!p || !out) return VOLKS_EINVAL;
   *out = nullptr;
+  volks_options opt;
+  volks_options_init(&opt);
+  if (o) {
+    if (o->struct_bytes != (int32_t)sizeof(volks_options)) return VOLKS_EINVAL;   // built against another header
+    opt = *o;
+    if (opt.slide_seg < 16 || opt.y_pad < 0 || opt.y_pad > 1024 || (opt.y_pad & 1) || opt.chunk_mb < 1 || opt.cf_wpc < 1 ||
+        (opt.cf2 != 0 && opt.cf2 != 1 && opt.cf2 != 2 && opt.cf2 != 4) || opt.ai_waves < 1 || opt.host_split < 1)
+      return VOLKS_EINVAL;
+  }
   const bool allif = ai_nif > 0;
   if (p->nbl < 1 || p->nif < 1 || p->nap < 0 || p->nchan < 1) return VOLKS_EINVAL;
   if (p->nwidths < 1 || p->nwidths > VOLKS_MAX_WIDTHS || !p->width || !p->stride || !p->nt) return VOLKS_EINVAL;
-  if (!is_pow2(p->nf) || p->nf < p->nchan || p->nf > (1 << 14)) return VOLKS_EINVAL;
+  if (!is_pow2(p->nf) || p->nf < p->nchan || p->nf > 8192) return VOLKS_EINVAL;   // row transforms up to 8192 points
   if (!(p->snr_thresh == p->snr_thresh)) return VOLKS_EINVAL;
   for (int q = 0; q < p->nwidths; ++q) {
     if (p->width[q] < 1 || p->stride[q] < 1 || !is_pow2(p->nt[q]) || (!allif && p->nt[q] < p->width[q])) return VOLKS_EINVAL;
@@ -329,9 +361,11 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   s.ngs = allif ? psub : 1;
   long long per_pair = 0;
   size_t tw_total = (size_t)p->nf;
-  const bool force_generic = env_is("VOLKS_PATH", "generic");
-  const int seg_req = std::max(16, env_int("VOLKS_SLIDE_SEG", 256));
-  pl->cf_split2 = env_int("VOLKS_CF2", 2);   // 2: 16-column strips (two 256-thread CTAs per SM), 1: 32-column strips, 0: k_colfft (nf >= 32 there: Y rows are pair-interleaved)
+  pl->opt = opt;
+  if (!cuda_ok(cudaGetDevice(&pl->device))) { delete pl; return VOLKS_ECUDA; }
+  const bool force_generic = opt.force_generic != 0;
+  const int seg_req = std::max(16, opt.slide_seg);
+  pl->cf_split2 = opt.cf2;   // 2: 16-column strips (two 256-thread CTAs per SM), 1: 32-column strips, 0: k_colfft (nf >= 32 there: Y rows are pair-interleaved)
   for (int q = 0; q < p->nwidths; ++q) {
     WidthPlan w;
     w.w = p->width[q]; w.s = p->stride[q]; w.nt = p->nt[q];
@@ -342,12 +376,16 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
     w.slide = !force_generic && w.s == 1 && w.w >= 2 && w.nt == 2 * w.w && p->nf >= 64 &&
               ((long long)p->nap + SLIDE_PF + 2) * (p->nf + 64) * 8 < (1LL << 32);
     if (allif) w.slide = false;
+    // candidates-only index mode: the tag-free maximum pays when a noise window stays below the pre-threshold, i.e.
+    // when snr_thresh^2 is well above the expected noise maximum ln(Nt Nf) + 0.58 of the plane (else: tagged kernel)
+    w.hy = w.slide && w.nt >= 32 && !opt.full_index && p->snr_thresh > 0.f &&
+           (double)p->snr_thresh * p->snr_thresh >= log((double)w.nt * p->nf) + 4.0;
     w.colfft = !allif && !force_generic && !w.slide && w.nt >= 32 && w.nt <= 512 && p->nf >= 32 && w.nwin > 0;
     w.cf_l1 = w.nt / 16;
     w.cf_nz = 1;
     while (w.cf_nz * 16 < w.w) w.cf_nz *= 2;
     // windows per CTA: up to 128 (L1 reuse of overlapping windows), fewer when the grid would not fill 148 SMs x 4
-    w.cf_wpc = (int)std::min<long long>(env_int("VOLKS_CF_WPC", 128),
+    w.cf_wpc = (int)std::min<long long>(opt.cf_wpc,
                                         std::max<long long>(8, (long long)p->nbl * p->nif * (p->nf / 32) * w.nwin / 592));
     w.cf_nrange = (int)((w.nwin + w.cf_wpc - 1) / w.cf_wpc);
     w.seg = std::max((seg_req / w.nt) * w.nt, w.nt);
@@ -379,23 +417,23 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   // chunking of the delay-spectrum intermediate Y over (bl, ifq) pairs: <= 4 GiB per chunk
   // Y row pitch: nf + 16 elements (one 128-byte line) when rows would otherwise sit a power of two
   // apart and fall into the same few L1 sets (kernels_slide.cuh reads w+1 rows of a column tile)
-  pl->pitch = (p->nf >= 32 && psub == 1) ? p->nf + env_int("VOLKS_Y_PAD", 16) : p->nf;   // sub-rows are contiguous
+  pl->pitch = (p->nf >= 32 && psub == 1) ? p->nf + opt.y_pad : p->nf;   // sub-rows are contiguous
   pl->paired = p->nf >= 2 ? 1 : 0;
   pl->row_generic = force_generic;
   const size_t y_pair = (size_t)p->nap * psub * pl->pitch * sizeof(float2);
   // VOLKS_CHUNK_MB: bytes of delay spectra per chunk of pairs (default 4 GiB; tests use small chunks)
-  const size_t budget = (size_t)std::max(1, env_int("VOLKS_CHUNK_MB", 4096)) << 20;
+  const size_t budget = (size_t)opt.chunk_mb << 20;
   long long ppc = y_pair ? (long long)std::max<size_t>(1, budget / std::max<size_t>(y_pair, 1)) : pl->npair;
   ppc = std::min(ppc, pl->npair);
   pl->nchunks = (pl->npair + ppc - 1) / ppc;
   pl->pairs_per_chunk = (pl->npair + pl->nchunks - 1) / pl->nchunks;
   pl->nchunks = (pl->npair + pl->pairs_per_chunk - 1) / pl->pairs_per_chunk;
-  pl->host_split = std::max(1, env_int("VOLKS_HOST_SPLIT", 4));
+  pl->host_split = opt.host_split;
   if (allif) {
     // k_allif launches pairs_per_chunk x psub x nseg CTAs of up to 1024 threads (two per SM): size the
     // segments of windows for about VOLKS_AI_WAVES (default 2) waves of 296 CTAs (restart cost per segment: w rows;
     // measured at the paper's size: 1 wave 41.5 ms per trial, 2 waves 38.1, 4 waves 38.7, 8 waves 39.7)
-    const long long waves = std::max(1, env_int("VOLKS_AI_WAVES", 2));
+    const long long waves = opt.ai_waves;
     for (auto &w : pl->wp) {
       if (w.nwin <= 0) continue;
       const long long want = std::max<long long>(1, (296 * waves + pl->pairs_per_chunk * psub - 1) / (pl->pairs_per_chunk * psub));
@@ -407,6 +445,21 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   }
 
   pl->nfin_blocks = (s.nwin_total + FIN_THREADS * FIN_TILES - 1) / (FIN_THREADS * FIN_TILES);
+  {
+    // every grid of a search must fit the 2^31 - 1 limit of gridDim.x (the launches cast to unsigned)
+    const long long GMAX = (1LL << 31) - 1, ppc_ = pl->pairs_per_chunk;
+    bool fits = pl->nfin_blocks <= GMAX && ppc_ * p->nap * psub <= GMAX;
+    for (auto &w : pl->wp) {
+      if (w.nwin == 0) continue;
+      const long double col_blocks = ((long double)ppc_ * w.nwin * (1 << w.log2m) * p->nf * psub + 255) / 256;
+      const long double slide_blocks = (long double)ppc_ * w.nseg * std::max(1, p->nf / 64) * (1 << w.log2m);
+      const long double cf_blocks = (long double)ppc_ * std::max(1, p->nf / 32) * w.cf_nrange * 4;
+      const long double ai_blocks = (long double)ppc_ * w.nseg * psub;
+      if ((!w.slide && !w.colfft && !allif && col_blocks > GMAX) || (w.slide && slide_blocks > GMAX) ||
+          (w.colfft && cf_blocks > GMAX) || (allif && ai_blocks > GMAX)) fits = false;
+    }
+    if (!fits) { delete pl; return VOLKS_EINVAL; }
+  }
   size_t off = 0;
   pl->off_keys = off; off = align_up(off + (size_t)std::max<long long>(s.nwin_total, 1) * sizeof(u64), 256);
   pl->off_E = off;    off = align_up(off + (size_t)std::max<long long>(pl->npair * p->nap, 1) * sizeof(float), 256);
@@ -414,6 +467,8 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   // + padding rows: the sliding kernel loads one row, and prefetches SLIDE_PF + 1 rows, past the last sample
   pl->off_noise = off; off = align_up(off + (allif ? (size_t)std::max<long long>(s.nwin_total, 1) * s.ngs * sizeof(float) : 0), 256);
   pl->off_zst = off;  off = align_up(off + (size_t)std::max<long long>(pl->npair * p->nwidths, 1) * sizeof(double2), 256);
+  for (auto &w : pl->wp) pl->nhy += (w.hy && w.nwin > 0) ? 1 : 0;
+  pl->off_thr = off;  off = align_up(off + (pl->nhy ? (size_t)pl->pairs_per_chunk * per_pair * sizeof(uint32_t) : 0), 256);
   pl->off_Y = off;    off = align_up(off + (size_t)pl->pairs_per_chunk * std::max<size_t>(y_pair, 8) + (size_t)(SLIDE_PF + 2) * pl->pitch * sizeof(float2), 256);
   pl->ws_bytes = off;
 
@@ -424,7 +479,8 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
       if (pl->wp[q].w == 1 && pl->wp[q].nwin > 0) pl->wid1 = q;
   for (int q = 0; q < p->nwidths; ++q) active += (pl->wp[q].nwin > 0 && q != pl->wid1) ? 1 : 0;
   // kernels of this library per search (the key memset is a driver memset, not counted)
-  pl->launches = s.nwin_total > 0 ? (int)(pl->nchunks * (1 + active + (pl->nslide > 0 ? 1 : 0)) + 3) : 0;
+  // (a search without dense peaks; with them the candidates-only index mode and its k_winthr launch are off)
+  pl->launches = s.nwin_total > 0 ? (int)(pl->nchunks * (1 + active + (pl->nslide > 0 ? 1 : 0) + (pl->nhy > 0 ? 1 : 0)) + 3) : 0;
 
   // tables, computed in double precision on the host
   if (psub > 1) { pl->premod_off = tw_total; tw_total += (size_t)s.nf; }
@@ -448,20 +504,20 @@ static int plan_create_impl(const volks_params *p, volks_plan **out, int ai_nif,
   bool ok = cuda_ok(cudaMalloc(&pl->d_tables, tw_total * sizeof(float2))) &&
             cuda_ok(cudaMalloc(&pl->d_sched, sizeof(Sched))) &&
             cuda_ok(cudaMemcpy(pl->d_tables, tab.data(), tw_total * sizeof(float2), cudaMemcpyHostToDevice)) &&
-            cuda_ok(cudaMemcpy(pl->d_sched, &s, sizeof(Sched), cudaMemcpyHostToDevice)) &&
-            cuda_ok(cudaFuncSetAttribute(k_row_fft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->row_smem));
+            cuda_ok(cudaMemcpy(pl->d_sched, &s, sizeof(Sched), cudaMemcpyHostToDevice));
+  // kernel attributes are process-wide per device: every kernel gets the MAXIMUM it can ever need (never a
+  // plan-dependent value, so that a later plan cannot lower an earlier one's limit)
+  ok = ok && cuda_ok(cudaFuncSetAttribute(k_row_fft, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
   for (auto &w : pl->wp)
     if (ok && w.colfft) {
       ColFftArgs ca; memset(&ca, 0, sizeof ca); ca.nt = w.nt;
       ok = cuda_ok(launch_colfft(ca, w.cf_l1, w.cf_nz, 0, nullptr, true));
     }
-  ok = ok && cuda_ok(cudaFuncSetAttribute(k_slide<16, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-  ok = ok && cuda_ok(cudaFuncSetAttribute(k_slide<16, false, true, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-  ok = ok && cuda_ok(cudaFuncSetAttribute(k_slide<16, false, true, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+  if (ok && !slide_attrs()) ok = cuda_ok(cudaGetLastError()) && false;
   if (ok && (p->nf == 4096 || p->nf == 8192)) {
     RowArgs ra; memset(&ra, 0, sizeof ra);
     ra.paired = pl->paired; ra.nf = p->nf; ra.nchan = p->nchan; ra.nrows = 1;
-    launch_rowbig(ra, nullptr, true);
+    if (!launch_rowbig(ra, nullptr, true)) { cuda_ok(cudaGetLastError()); snprintf(g_cuda_msg, sizeof g_cuda_msg, "k_rowbig: shared memory attribute refused"); ok = false; }
   }
   if (!ok) { volks_plan_destroy(pl); return VOLKS_ECUDA; }
   *out = pl;
@@ -563,9 +619,18 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
       }
     }
   }
+  {
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev))) return VOLKS_ECUDA;
+    if (dev != pl->device) return VOLKS_EINVAL;        // the plan's tables live on the device it was created on
+  }
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const Sched &s = pl->sched;
   char *ws = (char *)d_workspace;
+  // candidates-only index mode for the eligible sliding widths unless the dense peak array (every window's exact
+  // index) is wanted or the plan was created with full_index
+  const bool hy = pl->nhy > 0 && d_peaks == nullptr;
+  pl->last_full_index = !hy;
   u64 *keys = (u64 *)(ws + pl->off_keys);
   float *E = (float *)(ws + pl->off_E);
   uint32_t *cnt = (uint32_t *)(ws + pl->off_cnt);
@@ -615,6 +680,20 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         k_row_fft<<<(unsigned)rblocks, ra.tpr * ra.rows_per_cta, pl->row_smem, st>>>(ra);
       if (d_stage && !cuda_ok(cudaEventRecord(pl->ev_free[ch & 1], st))) return VOLKS_ECUDA;
     }
+    if (hy) {
+      WinThrArgs ta;
+      ta.E = E; ta.thr = (uint32_t *)(ws + pl->off_thr); ta.per_pair = s.per_pair; ta.pair0 = pair0;
+      ta.thr2 = s.snr_thresh * s.snr_thresh; ta.nap = s.nap; ta.nq = 0; ta.cum[0] = 0;
+      for (int q = 0; q < s.nwidths; ++q) {
+        const WidthPlan &w = pl->wp[q];
+        if (!w.hy || w.nwin == 0) continue;
+        const int i = ta.nq++;
+        ta.w[i] = w.w; ta.nwin[i] = (int)w.nwin; ta.offc[i] = s.offc[q]; ta.cum[i + 1] = ta.cum[i] + w.nwin;
+      }
+      ta.total = np * ta.cum[ta.nq];
+      ProfScope ps(pl, st, VOLKS_K_WINTHR, -1);
+      k_winthr<<<(unsigned)((ta.total + 255) / 256), 256, 0, st>>>(ta);
+    }
     for (int q = 0; q < s.nwidths; ++q) {
       const WidthPlan &w = pl->wp[q];
       if (w.nwin == 0 || q == pl->wid1) continue;
@@ -648,8 +727,9 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         sa.nap = s.nap; sa.nf = s.nf; sa.w = w.w; sa.nt = w.nt; sa.log2m = w.log2m; sa.nwin = (int)w.nwin;
         sa.seg = w.seg; sa.nseg = w.nseg; sa.keymask = 0xFFFFFFF0u; sa.pitch = pl->pitch;
         sa.ntasks = ((np * w.nseg * (long long)(s.nf / 64)) << w.log2m);
+        sa.thr = (const uint32_t *)(ws + pl->off_thr);
         ProfScope ps(pl, st, VOLKS_K_SLIDE, q);
-        launch_slide(sa, st);
+        launch_slide(sa, hy && w.hy, st);
         continue;
       }
       if (w.colfft) {
@@ -707,6 +787,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
 int volks_zscore_select(const volks_plan *pl, void *d_workspace, float z_thresh, volks_peak *d_peaks,
                         volks_cand *d_cands, uint32_t cand_capacity, uint32_t *d_ncand, void *cuda_stream) {
   if (!pl || !d_workspace || !d_ncand || (!d_cands && cand_capacity > 0) || !(z_thresh == z_thresh)) return VOLKS_EINVAL;
+  if (!pl->last_full_index) return VOLKS_EINVAL;   // the last search kept exact indices for its candidates only
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const Sched &s = pl->sched;
   if (s.nwin_total == 0) return cuda_ok(cudaMemsetAsync(d_ncand, 0, sizeof(uint32_t), st)) ? VOLKS_OK : VOLKS_ECUDA;
@@ -828,6 +909,39 @@ int volks_baseline_match(const volks_pulse *pulses, uint32_t npulse, int32_t min
   }
   *nout = found;
   return found > capacity ? VOLKS_EOVERFLOW : VOLKS_OK;
+}
+
+int volks_measure_fp32_peak(int32_t repeats, double *tflops_best, double *tflops_mean, double *ms_per_launch,
+                            void *cuda_stream) {
+  if (repeats < 1 || repeats > 1000 || !tflops_best) return VOLKS_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = 0, sms = 0;
+  if (!cuda_ok(cudaGetDevice(&dev)) || !cuda_ok(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)))
+    return VOLKS_ECUDA;
+  const int ctas = sms * 8, thr = 256, iters = 65536;     // ~20 ms per launch on B200
+  float *buf = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (!cuda_ok(cudaMalloc(&buf, (size_t)ctas * thr * sizeof(float)))) return VOLKS_ECUDA;
+  bool ok = cuda_ok(cudaEventCreate(&e0)) && cuda_ok(cudaEventCreate(&e1));
+  const double flops = (double)ctas * thr * iters * 32.0 * 2.0;
+  double best = 0.0, sum = 0.0, ms_sum = 0.0;
+  if (ok) k_fp32_probe<<<ctas, thr, 0, st>>>(buf, iters / 8, 0.999f, 1e-3f);   // warm-up (clocks, code load)
+  for (int r = 0; ok && r < repeats; ++r) {
+    ok = cuda_ok(cudaEventRecord(e0, st));
+    k_fp32_probe<<<ctas, thr, 0, st>>>(buf, iters, 0.999f, 1e-3f);
+    ok = ok && cuda_ok(cudaEventRecord(e1, st)) && cuda_ok(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    ok = ok && cuda_ok(cudaEventElapsedTime(&ms, e0, e1)) && ms > 0.f;
+    if (ok) { const double tf = flops / (ms * 1e-3) / 1e12; best = std::max(best, tf); sum += tf; ms_sum += ms; }
+  }
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
+  cudaFree(buf);
+  if (!ok) return VOLKS_ECUDA;
+  *tflops_best = best;
+  if (tflops_mean) *tflops_mean = sum / repeats;
+  if (ms_per_launch) *ms_per_launch = ms_sum / repeats;
+  return VOLKS_OK;
 }
 
 int volks_dm_shifts(double dm, const double *f_chan_mhz, int32_t n, double f_ref_mhz, double ap_seconds,

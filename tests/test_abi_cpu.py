@@ -21,7 +21,7 @@ def vb():
 def test_exports_every_declared_symbol(vb):
     hdr = open(os.path.join(ROOT, "include", "volks.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(volks_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(volks_[a-z0-9_]+)\s*\(", hdr))
     assert {"volks_plan_create", "volks_fringe_search", "volks_window_match"} <= declared
     L = vb.lib()
     for name in declared:
@@ -43,6 +43,29 @@ def test_plan_create_rejects_bad_params_before_cuda(vb, kw):
     a.update(kw)
     rc, h = vb.plan_create_raw(**a)
     assert rc == -1 and not h
+
+
+def test_options_defaults_and_validation_before_cuda(vb):
+    """volks_options: defaults from volks_options_init; bad values and a mismatched struct size are rejected
+    before any CUDA call; nf above the row kernels' 8192 points is an explicit VOLKS_EINVAL."""
+    o = vb.make_options()
+    assert (o.struct_bytes, o.full_index, o.force_generic, o.slide_seg, o.y_pad, o.chunk_mb, o.cf_wpc, o.cf2, o.ai_waves,
+            o.host_split) == (40, 0, 0, 256, 16, 4096, 128, 2, 2, 4)
+    a = dict(nbl=1, nif=1, nap=512, nchan=32, widths=[8], strides=[1], nts=[16], nf=64, snr_thresh=6.0)
+    for bad in (dict(slide_seg=8), dict(y_pad=3), dict(y_pad=-2), dict(chunk_mb=0), dict(cf2=3), dict(ai_waves=0),
+                dict(host_split=0), dict(cf_wpc=0)):
+        rc, h = vb.plan_create_raw(options=bad, **a)
+        assert rc == -1 and not h, bad
+    o = vb.make_options()
+    o.struct_bytes = 36
+    rc, h = vb.plan_create_raw(options=o, **a)
+    assert rc == -1 and not h
+    with pytest.raises(KeyError):
+        vb.make_options(no_such_option=1)
+    rc, h = vb.plan_create_raw(**dict(a, nf=16384))
+    assert rc == -1 and not h
+    src = open(os.path.join(ROOT, "paper_2108_05602_b200", "csrc", "volks_api.cu")).read()
+    assert "getenv" not in src          # the library reads no environment variables
 
 
 def test_strerror_and_version(vb):

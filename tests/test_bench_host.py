@@ -52,3 +52,16 @@ def test_single_process_path_and_flop_accounting():
     assert per_w[5] == (120000 - 64 + 1) * npair * (256 * 5.0 * 128 * 7 + 5.0 * 128 * 256)
     assert abs(tot - 2.21e13) < 0.02e13                     # 2.21e13 algorithmic flops
     assert abs(bench.nominal_flops(c) - 4.36e13) < 0.03e13  # ... and 4.36e13 nominal
+
+
+def test_traffic_table_and_executed_flops():
+    import bench
+    import workloads
+    tab = bench.ncu_traffic_table()
+    assert (2, "slide", 64) in tab and tab[(2, "slide", 64)][0] > 1e9 and "profiles/" in tab[(2, "slide", 64)][1]
+    c = workloads.config(2)
+    # sliding kernel, w = 64 (Nt 128, Nf 256): 11 flops per bin per window, 5 launches
+    ex = bench.executed_flops_per_launch(c, 6, 5, 5, 80, c["nap"], 1.0)
+    assert ex == (120000 - 64 + 1) * 80 * 128 * 256 * 11.0 / 5
+    # FFT kernels are charged the algorithmic count
+    assert bench.executed_flops_per_launch(workloads.config(4), 7, 0, 7, 84, 20000, 123.0) == 123.0

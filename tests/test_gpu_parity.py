@@ -33,11 +33,15 @@ def make_plane_power(oracle, vis_np, c):
     return plane_power
 
 
-def run_both(vb, oracle, vis, c, thresh=None, mode="cached"):
+def run_both(vb, oracle, vis, c, thresh=None, mode="cached", options=None):
     thresh = c["snr_thresh"] if thresh is None else thresh
     nbl, nif, nap, nchan = vis.shape
     cands, n, peaks = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], thresh,
-                                       want_peaks=True)
+                                       want_peaks=True, options=options)
+    # the same search without the dense peak array: the stride-1 kernels may run in the candidates-only index
+    # mode (volks_options.full_index = 0); the candidate list must be the same, bit for bit
+    cands2, n2, _ = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], thresh, options=options)
+    assert n2 == n and cands2.tobytes() == cands.tobytes()
     ora, _ = oracle.search(vis.cpu().numpy(), c["widths"], c["strides"], c["nts"], c["nf"], mode=mode)
     nw = [workloads.gen.nwin(nap, w, s) for w, s in zip(c["widths"], c["strides"])]
     di = dense_index(nbl, nif, nw)
@@ -78,17 +82,14 @@ def test_reduced_configs(vb, oracle, cfg, over):
     (2, dict(nbl=1, nif=2, nap=700, npulses=3)),
     (3, dict(nbl=2, nif=2, nap=900, npulses=4)),
 ])
-def test_generic_and_sliding_paths_agree_with_oracle(vb, oracle, cfg, over, monkeypatch):
-    """The same stride-1 inputs through the generic kernels (VOLKS_PATH=generic) and through the
+def test_generic_and_sliding_paths_agree_with_oracle(vb, oracle, cfg, over):
+    """The same stride-1 inputs through the generic kernels (volks_options.force_generic) and through the
     sliding-sum kernels with a short restart interval (several segments + a ragged tail)."""
     vis, c, _ = workloads.generate(cfg, **over)
-    monkeypatch.setenv("VOLKS_PATH", "generic")
-    run_both(vb, oracle, vis, c)
-    monkeypatch.delenv("VOLKS_PATH")
-    monkeypatch.setenv("VOLKS_SLIDE_SEG", "128")
-    run_both(vb, oracle, vis, c, thresh=3.0)
-    monkeypatch.setenv("VOLKS_SLIDE_SEG", "1024")
-    run_both(vb, oracle, vis, c)
+    run_both(vb, oracle, vis, c, options=dict(force_generic=1))
+    run_both(vb, oracle, vis, c, thresh=3.0, options=dict(slide_seg=128))
+    run_both(vb, oracle, vis, c, options=dict(slide_seg=1024))
+    run_both(vb, oracle, vis, c, options=dict(full_index=1))
 
 
 @pytest.mark.parametrize("shape", [
@@ -134,12 +135,11 @@ def test_sliding_kernel_shapes(vb, oracle, shape):
     (1, 1, 700, 50, [100, 200, 256], [25, 64, 100], [512, 256, 256], 64), # NZ = 8, 16, 16 (nt == w: no padding)
     (2, 1, 600, 33, [300, 512], [50, 30], [512, 512], 128),               # NZ = 32 (nt == w), several strips
 ])
-def test_colfft2_variants(vb, oracle, shape, cf2, monkeypatch):
+def test_colfft2_variants(vb, oracle, shape, cf2):
     """The two-columns-per-thread rate kernel (kernels_colfft2.cuh) in both strip widths, and the kernel it
     replaced, against the oracle on the same inputs: every pruning depth NZ, windows of one CTA range,
     a burst that gives a clear peak, and an all-zero span (tie-break -> index 0)."""
-    monkeypatch.setenv("VOLKS_CF2", cf2)
-    monkeypatch.setenv("VOLKS_CF_WPC", "8")                               # several window ranges per strip
+    opts = dict(cf2=int(cf2), cf_wpc=8)                                   # several window ranges per strip
     nbl, nif, nap, nchan, widths, strides, nts, nf = shape
     g = torch.Generator().manual_seed(nap * 13 + nchan)
     vis = torch.view_as_complex(torch.randn((nbl, nif, nap, nchan, 2), generator=g) * 0.7071)
@@ -147,11 +147,11 @@ def test_colfft2_variants(vb, oracle, shape, cf2, monkeypatch):
     vis[0, 0, nap // 3: nap // 3 + 30] += 0.8 * torch.exp(2j * np.pi * 3.0 * k / nf)   # delay bin 3
     vis[0, 0, : 40] = 0                                                   # flagged span at the start
     c = dict(widths=widths, strides=strides, nts=nts, nf=nf, snr_thresh=2.5)
-    run_both(vb, oracle, vis, c, mode="fft")
+    run_both(vb, oracle, vis, c, mode="fft", options=opts)
     # run to run bit-identical (the two parity pipelines of a CTA meet only in the ordered key maximum)
     ref = None
     for _ in range(3):
-        cands, n, peaks = vb.fringe_search(vis.cuda(), widths, strides, nts, nf, 2.5, want_peaks=True)
+        cands, n, peaks = vb.fringe_search(vis.cuda(), widths, strides, nts, nf, 2.5, want_peaks=True, options=opts)
         blob = (peaks.tobytes(), cands.tobytes())
         assert ref is None or blob == ref
         ref = blob
@@ -302,7 +302,9 @@ def test_zscore_selection_matches_oracle(vb, oracle, cfg, over):
     windows whose oracle z lies within that margin of the threshold)."""
     vis, c, _ = workloads.generate(cfg, **over)
     nbl, nif, nap, nchan = vis.shape
-    plan = vb.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"])
+    # the z-score pass needs every window's exact index from the search before it: volks_options.full_index
+    plan = vb.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"],
+                   options=dict(full_index=1))
     dev = torch.device("cuda")
     ws = torch.empty(plan.workspace_bytes, dtype=torch.uint8, device=dev)
     cap = 1 << 16
@@ -383,17 +385,17 @@ def test_allif_search_matches_oracle(vb, oracle, shape):
 
 @pytest.mark.parametrize("chunk_mb", ["1", "8"])   # 8 MB: several pairs per plan chunk, the host path takes a quarter at a time
 @pytest.mark.parametrize("allif", [False, True])
-def test_host_slab_search_is_identical(vb, allif, chunk_mb, monkeypatch):
+def test_host_slab_search_is_identical(vb, allif, chunk_mb):
     """volks_search_host (slab in pinned host memory, chunked copies overlapped with the kernels) must
     give bit-identical candidates and peaks to the device-slab call; small chunks force several
     copy/compute rounds through both stage halves, twice in a row (stage reuse across calls)."""
-    monkeypatch.setenv("VOLKS_CHUNK_MB", chunk_mb)
+    opts = dict(chunk_mb=int(chunk_mb))
     vis, c, _ = workloads.generate(2, nbl=3, nif=3, nap=600, npulses=3)
     nbl, nif, nap, nchan = vis.shape
     if allif:
-        plan = vb.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], None, 1024, 4.0, allif=True)
+        plan = vb.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], None, 1024, 4.0, allif=True, options=opts)
     else:
-        plan = vb.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], c["nts"], c["nf"], 4.0)
+        plan = vb.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], c["nts"], c["nf"], 4.0, options=opts)
     dev = torch.device("cuda")
     ws = torch.empty(plan.workspace_bytes, dtype=torch.uint8, device=dev)
     cap = 1 << 16
