@@ -88,10 +88,10 @@ typedef struct {
  * reads no environment variables. */
 typedef struct {
   int32_t struct_bytes;  /* sizeof(volks_options), set by volks_options_init; a mismatch is VOLKS_EINVAL            */
-  int32_t full_index;    /* 0 (default): a search WITHOUT d_peaks keeps the exact (rate, delay) index only for the   */
-                         /* windows that can be candidates (the stride-1 kernels then skip the per-bin index tags;   */
-                         /* candidates are bit-identical either way).  1: exact index for every window in every      */
-                         /* search - what volks_zscore_select needs from the search before it                        */
+  int32_t full_index;    /* 0 (default): a search WITHOUT d_peaks finds the exact (rate, delay) bin only of the      */
+                         /* windows that can be candidates (and may skip segments of narrow windows that cannot hold  */
+                         /* one, see no_prune); candidates are bit-identical either way.  1: every window's peak in   */
+                         /* every search - what volks_zscore_select needs from the search before it                  */
   int32_t force_generic; /* 1: the generic kernels (k_row_fft, k_col) for every width (the parity suite runs both)   */
   int32_t slide_seg;     /* windows per exactly restarted segment of the sliding kernel (default 256, >= 16)         */
   int32_t y_pad;         /* padding elements of a row of delay spectra (default 16; even, 0..1024)                   */
@@ -100,6 +100,10 @@ typedef struct {
   int32_t cf2;           /* Nt = 256 / 512: 2 (default) 16-column strips, 1: 32-column, 4: 8-column, 0: k_colfft    */
   int32_t ai_waves;      /* f2: waves of 296 CTAs the window segments of k_allif are sized for (default 2)           */
   int32_t host_split;    /* volks_search_host copies 1/host_split of a plan chunk at a time (default 4)              */
+  int32_t no_prune;      /* 1: switch off the exact pruning of the narrow stride-1 widths (full_index = 0 only): by   */
+                         /* default a segment of windows whose amplitude-sum bound stays below the threshold in every */
+                         /* delay column is not transformed at all (it cannot hold a candidate)                       */
+  int32_t prune_seg;     /* windows per pruned segment (default 64; power of two, 16..4096)                          */
 } volks_options;
 void volks_options_init(volks_options *o);
 
@@ -256,6 +260,8 @@ int volks_plan_launch_count(const volks_plan *plan);
 #define VOLKS_K_ALLIF 8    /* f2: all-IF rate-0 window sums + argmax + noise                          */
 #define VOLKS_K_FIXUP 9    /* exact re-evaluation of the sliding widths' outlier windows               */
 #define VOLKS_K_WINTHR 10  /* per-window pre-thresholds of the candidates-only index mode              */
+#define VOLKS_K_BOUND 11   /* amplitude-sum bound: which segments of the narrow widths can hold candidates */
+#define VOLKS_K_RECOVER 12 /* peak bin of the stride-1 windows (w >= 16) by exact re-evaluation of one tile */
 int volks_plan_profile(volks_plan *plan, int enable);
 int volks_plan_profile_read(const volks_plan *plan, int32_t capacity, int32_t *kind, int32_t *wid,
                             float *ms, int32_t *n);

@@ -28,6 +28,10 @@ struct FixArgs {
   int q[16], w[16], nt[16], seg[16], nseg[16], nwin[16];
   long long offc[16], tw_off[16];
   int unit0[17];         // prefix sums of nseg over the sliding widths (units per pair = unit0[nq])
+  // pruned widths (kernels_prune.cuh): segments whose flag is 0 were not evaluated (all keys zero): nothing to fix
+  const unsigned char *flags;   // [pairs of the chunk][flag_nq][flag_nseg] or nullptr
+  int flag_q[16];               // index of sliding width i among the pruned widths, or -1
+  int flag_nq, flag_nseg;
 };
 
 // peak key of rate residue rho, column d of the window starting at row0 (already includes pair and t0)
@@ -65,6 +69,7 @@ __global__ void __launch_bounds__(256) k_fixup(FixArgs a) {
   int u = (int)(blockIdx.x % upp), i = 0;
   while (u >= a.unit0[i + 1]) ++i;
   const int sg = u - a.unit0[i];
+  if (a.flags && a.flag_q[i] >= 0 && !a.flags[(pl * a.flag_nq + a.flag_q[i]) * a.flag_nseg + sg]) return;
   const int w = a.w[i], nt = a.nt[i], seg = a.seg[i];
   const int j0 = sg * seg, n = min(seg, a.nwin[i] - j0);          // windows j0 .. j0+n-1 (seg <= 256? see below)
   u64 *keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc[i]);

@@ -54,9 +54,10 @@ struct SlideArgs {
   long long pair0;      // first pair of the chunk
   int nap, nf, w, nt, log2m, nwin, seg, nseg, pitch;
   uint32_t keymask;     // 0xFFFFFFF0, passed as data so that (p & mask) | id is ONE LOP3 (register mask)
-  // HY (candidates-only index mode): pre-threshold of every window of the chunk, as float bits, laid out like the
-  // keys but chunk-relative: thr[pl * per_pair + offc + t0] (k_winthr); unused by the fully tagged kernels
-  const uint32_t *thr;
+  // pruned widths (kernels_prune.cuh): flags[pl * flag_stride + segment] == 0 means no window of the segment can be
+  // a candidate - the CTA returns at once; nullptr = every segment is evaluated
+  const unsigned char *flags;
+  int flag_stride;
 };
 
 // The per-step operand of one parity class, both columns: g = (GX, GY) and the (1 -+ i)/sqrt 2
@@ -106,6 +107,7 @@ struct SlideState {
   u64 *keyp;                    // canonical key of window t0 = keyp[t0]
   uint32_t rowb;                // bytes per Y row
   uint32_t ntmask, rho, idx0, idxs, keymask, lane;   // plane index of bin s, column a: idx0 + s * idxs
+  uint32_t tilekey;             // 0xFFFFFFFF - (2^31 | idx0), slide_emit_u
   // RING variant: shared-memory addresses of this lane's entry in the ring rows of the current block's
   // first leaving row (sm_out) and first entering row (sm_in); ring geometry in bytes
   uint32_t sm_out, sm_in, ring_lo, ring_hi, rrowb;
@@ -135,14 +137,13 @@ __device__ __forceinline__ void slide_emit(const SlideState<L> &S, u64 *slot) {
   }
 }
 
-// HY emit: the window's maximum WITHOUT the bin tags (one 3-input max per bin instead of two LOP3 + the max), and
-// the tagged emit only when the warp's maximum exceeds the window's pre-threshold `thrbits` (k_winthr: 0.98 of the
-// power a candidate needs) - a warp-uniform branch that a noise window never takes.  Below it the slot carries the
-// (truncated) power alone: index word 0 = the lowest priority among equal powers, never reported, because a window
-// can only become a candidate through a warp that took the tagged path.  Powers are truncated like the tagged
-// keys (max then mask == mask then max), so both modes give bit-identical candidates.
+// Untagged emit (the kernels with M >= 2, i.e. w >= 16): the maximum power and the delay COLUMN it sits in - one
+// 3-input max per bin instead of two LOP3 + the max.  The slot carries (exact power bits, 2^31 | plane index of the
+// column's first bin rho * nf + d): which of the column's 16 rate bins r = rho + M s holds the maximum is found
+// afterwards, for the windows that need it, by k_recover (an exact re-evaluation of that one column: 16 bins from
+// w samples); DESIGN.md section 6.  Ties between columns: the lower one.
 template <int L>
-__device__ __forceinline__ void slide_emit_hy(const SlideState<L> &S, u64 *slot, uint32_t thrbits) {
+__device__ __forceinline__ void slide_emit_u(const SlideState<L> &S, u64 *slot) {
   uint32_t ba = 0, bb = 0;
 #pragma unroll
   for (int s = 0; s < L; ++s) {
@@ -150,9 +151,11 @@ __device__ __forceinline__ void slide_emit_hy(const SlideState<L> &S, u64 *slot,
     ba = max(ba, __float_as_uint(lo32(pw)));
     bb = max(bb, __float_as_uint(hi32(pw)));
   }
-  const uint32_t km = __reduce_max_sync(0xffffffffu, max(ba, bb));
-  if (km > thrbits) slide_emit<L>(S, slot);
-  else if (S.lane == 0) *slot = (u64)(km & 0xFFFFFFF0u) << 32;
+  const uint32_t best = max(ba, bb);
+  const uint32_t km = __reduce_max_sync(0xffffffffu, best);
+  const uint32_t tied = __ballot_sync(0xffffffffu, best == km);
+  if (S.lane == (uint32_t)__ffs(tied) - 1u)
+    *slot = ((u64)km << 32) | (u64)(S.tilekey - (bb > ba ? 1u : 0u));
 }
 
 // after a block of nsteps (<= 16) windows starting at t0: threads 0..nsteps-1 reduce the warps'
@@ -234,22 +237,17 @@ __device__ __forceinline__ void slide_update(SlideState<L> &S, uint32_t t0) {
 }
 
 // L consecutive steps starting at t0 (t0 mod L == 0).  GUARD: only windows < tend exist.
-// HY: thr_sm = shared address of the block's L pre-thresholds (float bits)
-template <int L, int B, bool MODD, bool GUARD, bool RING, int RR, bool HY>
+template <int L, int B, bool MODD, bool GUARD, bool RING, int RR>
 struct SlideSteps {
-  static __device__ __forceinline__ void run(SlideState<L> &S, uint32_t t0, uint32_t tend, u64 *slot, uint32_t thr_sm) {
+  static __device__ __forceinline__ void run(SlideState<L> &S, uint32_t t0, uint32_t tend, u64 *slot) {
     if constexpr (B < L) {
       if (!GUARD || t0 + B < tend) {
-        if constexpr (HY) {
-          uint32_t thrbits;
-          asm volatile("ld.shared.u32 %0, [%1];" : "=r"(thrbits) : "r"(thr_sm + 4u * B));   // pinned to its step
-          slide_emit_hy<L>(S, slot + B * SLIDE_WARPS, thrbits);
-        } else {
-          slide_emit<L>(S, slot + B * SLIDE_WARPS);
-        }
+        // M == 1 (w <= 8): tagged keys, exact index at once; M >= 2: power + tile id, index by k_recover
+        if constexpr (MODD) slide_emit<L>(S, slot + B * SLIDE_WARPS);
+        else slide_emit_u<L>(S, slot + B * SLIDE_WARPS);
         if (!GUARD || t0 + B + 1 < tend) slide_update<L, B, MODD, RING, RR>(S, t0 + B);
       }
-      SlideSteps<L, B + 1, MODD, GUARD, RING, RR, HY>::run(S, t0, tend, slot, thr_sm);
+      SlideSteps<L, B + 1, MODD, GUARD, RING, RR>::run(S, t0, tend, slot);
     }
   }
 };
@@ -306,12 +304,10 @@ __device__ __forceinline__ void slide_ring_fill(const SlideRing &G, uint32_t r0,
 }
 
 // L = min(16, Nt) bins per thread;  MODD <=> M == 1 (Nt <= 16);  RING (M >= 4 only): rows through shared memory.
-// HY: candidates-only index mode (slide_emit_hy).
-template <int L, bool MODD, bool RING, int RR = 0, bool HY = false>
+template <int L, bool MODD, bool RING, int RR = 0>
 __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(SlideArgs a) {
   // blockDim.x = 32 * min(SLIDE_WARPS, ndt * M): every warp of a CTA works on the same (pair, segment)
   __shared__ u64 slots[2][16 * SLIDE_WARPS];
-  __shared__ uint32_t thrs[2][16];   // HY: pre-thresholds of the current / next block of L windows
   extern __shared__ float4 slide_ring[];
   const int nwarps = blockDim.x >> 5, warp = threadIdx.x >> 5;
   long long wt = (long long)blockIdx.x * nwarps + warp;
@@ -324,10 +320,12 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   const int dt = (int)(wt % ndt); wt /= ndt;
   const int sg = (int)(wt % a.nseg);
   const long long pl = wt / a.nseg;
+  if (a.flags && !a.flags[pl * a.flag_stride + sg]) return;   // the whole CTA shares (pair, segment)
   const uint32_t c = (uint32_t)(dt * 32) + lane;  // column pair (2c, 2c+1)
   S.ntmask = (uint32_t)(a.nt - 1);
   S.idx0 = S.rho * (uint32_t)a.nf + 2u * c;       // plane index r * nf + d of bin s: r = rho + M s
   S.idxs = (uint32_t)a.nf << a.log2m;
+  S.tilekey = 0xFFFFFFFFu - (0x80000000u | S.idx0);   // bit 31: a column (its bin s = 0), not yet a bin
   const float sg1 = (S.rho & 1u) ? -1.f : 1.f;
   S.sgn2 = pk(sg1, sg1);
   S.keymask = a.keymask;
@@ -338,13 +336,6 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   S.keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
   const uint32_t T0 = (uint32_t)sg * (uint32_t)a.seg;                 // multiple of Nt and of L
   const uint32_t tend = min((uint32_t)a.nwin, T0 + (uint32_t)a.seg);  // windows [T0, tend)
-  const uint32_t *thrg = nullptr;
-  const uint32_t thr_sm = (uint32_t)__cvta_generic_to_shared(&thrs[0][0]);
-  if constexpr (HY) {
-    thrg = a.thr + (pl * a.per_pair + a.offc);
-    if (threadIdx.x < L) thrs[0][threadIdx.x] = T0 + threadIdx.x < tend ? __ldg(thrg + T0 + threadIdx.x) : 0xFFFFFFFFu;
-    if constexpr (!RING) __syncthreads();      // (RING: the barrier after the first ring fill orders it)
-  }
   SlideRing G;
   if constexpr (RING) {
     // the CTA's warps are (rho fastest, then dt): its first warp's dt is the first column group
@@ -387,12 +378,8 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   for (;; t0 += L, buf ^= 1u) {
     const bool full = t0 + L < tend;
     if constexpr (RING) slide_ring_fill(G, t0 - T0 + (uint32_t)a.w + 17u, 16u);   // the next block's new rows
-    if constexpr (HY) {   // the next block's pre-thresholds (read after this block's flush barrier)
-      const uint32_t tn = t0 + L + threadIdx.x;
-      if (threadIdx.x < L) thrs[buf ^ 1u][threadIdx.x] = tn < tend ? __ldg(thrg + tn) : 0xFFFFFFFFu;
-    }
-    if (full) SlideSteps<L, 0, MODD, false, RING, RR, HY>::run(S, t0, tend, &slots[buf][warp], thr_sm + buf * 64u);
-    else SlideSteps<L, 0, MODD, true, RING, RR, HY>::run(S, t0, tend, &slots[buf][warp], thr_sm + buf * 64u);
+    if (full) SlideSteps<L, 0, MODD, false, RING, RR>::run(S, t0, tend, &slots[buf][warp]);
+    else SlideSteps<L, 0, MODD, true, RING, RR>::run(S, t0, tend, &slots[buf][warp]);
     if constexpr (RING) asm volatile("cp.async.wait_all;" ::: "memory");
     slide_flush(S.keyp, slots[buf], t0, full ? (uint32_t)L : tend - t0, nwarps);
     if (!full) break;
@@ -404,10 +391,10 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   }
 }
 
-// Pre-thresholds of the HY mode: one thread per (pair of the chunk, sliding width, window):
+// Pre-thresholds of the candidates-only mode: one thread per (pair of the chunk, sliding width, window):
 //   thr = SLIDE_PRE * snr_thresh^2 * sum_{t<w} E[t0 + t]   (the window energy = the noise of a7, summed in the
 // order k_finalize uses), stored as float bits.  A window is a candidate iff P1 > snr_thresh^2 * energy, so every
-// candidate's winning warp sees its maximum above thr and takes the tagged path.
+// candidate lies above thr: k_recover finds the index of exactly those windows, k_bound keeps their segments.
 #ifndef SLIDE_PRE
 #define SLIDE_PRE 0.98f
 #endif

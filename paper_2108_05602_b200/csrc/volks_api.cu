@@ -16,6 +16,8 @@
 #include "kernels_allif.cuh"
 #include "kernels_fixup.cuh"
 #include "kernels_probe.cuh"
+#include "kernels_prune.cuh"
+#include "kernels_recover.cuh"
 
 using namespace volks;
 
@@ -43,7 +45,8 @@ struct WidthPlan {
   bool colfft;          // two-pass shared-memory column FFT (kernels_colfft.cuh): Nt = 32..512, nf % 32 == 0
   int cf_l1, cf_nz, cf_wpc, cf_nrange;
   int seg, nseg;        // sliding path: windows per exactly restarted segment, segments per pair
-  bool hy;              // sliding path: eligible for the candidates-only index mode (k_slide HY)
+  bool untag;           // sliding path with M >= 2 (Nt >= 32): untagged kernel, peak bin by k_recover
+  int prune;            // sliding path: index among the plan's pruned widths (kernels_prune.cuh), or -1
 };
 
 template <int L>
@@ -182,8 +185,7 @@ static bool launch_row2(const RowArgs &a, cudaStream_t st) {
   return row2_nz<8, 8>(a, nza, blocks, st);
 }
 
-// hy: candidates-only index mode (kernels_slide.cuh slide_emit_hy; widths with Nt >= 32 only)
-static void launch_slide(const SlideArgs &a, bool hy, cudaStream_t st) {
+static void launch_slide(const SlideArgs &a, cudaStream_t st) {
   // every warp of a CTA must share its (pair, segment): warps per CTA = min(SLIDE_WARPS, ndt * M)
   const long long per_seg = (long long)(a.nf / 64) << a.log2m;
   const int wpb = (int)std::min<long long>(SLIDE_WARPS, per_seg);
@@ -195,17 +197,10 @@ static void launch_slide(const SlideArgs &a, bool hy, cudaStream_t st) {
     // + the warps' twiddle rows ([wpb][Nt + 1] float4) behind the ring
     const size_t ring = (size_t)(a.w + 48) * 512 * dtc + (size_t)wpb * (a.nt + 1) * 16;
     if (a.log2m >= 2 && ring <= 100 * 1024) {
-      if (hy) {
-        if (dtc == 1) k_slide<16, false, true, 512, true><<<blocks, thr, ring, st>>>(a);
-        else if (dtc == 2) k_slide<16, false, true, 1024, true><<<blocks, thr, ring, st>>>(a);
-        else k_slide<16, false, true, 0, true><<<blocks, thr, ring, st>>>(a);
-      } else {
-        if (dtc == 1) k_slide<16, false, true, 512><<<blocks, thr, ring, st>>>(a);
-        else if (dtc == 2) k_slide<16, false, true, 1024><<<blocks, thr, ring, st>>>(a);
-        else k_slide<16, false, true><<<blocks, thr, ring, st>>>(a);
-      }
+      if (dtc == 1) k_slide<16, false, true, 512><<<blocks, thr, ring, st>>>(a);
+      else if (dtc == 2) k_slide<16, false, true, 1024><<<blocks, thr, ring, st>>>(a);
+      else k_slide<16, false, true><<<blocks, thr, ring, st>>>(a);
     }
-    else if (hy) k_slide<16, false, false, 0, true><<<blocks, thr, 0, st>>>(a);
     else k_slide<16, false, false><<<blocks, thr, 0, st>>>(a);
   }
   else if (a.nt == 16) k_slide<16, true, false><<<blocks, thr, 0, st>>>(a);
@@ -213,15 +208,12 @@ static void launch_slide(const SlideArgs &a, bool hy, cudaStream_t st) {
   else k_slide<4, true, false><<<blocks, thr, 0, st>>>(a);
 }
 
-// the ring kernels' dynamic shared memory limit (per device, process-wide: set before every plan's first use)
+// the ring kernels' dynamic shared memory limit (per device, process-wide: always the maximum they can need)
 static bool slide_attrs() {
   const int lim = 100 * 1024;
   return cudaFuncSetAttribute(k_slide<16, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
          cudaFuncSetAttribute(k_slide<16, false, true, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
-         cudaFuncSetAttribute(k_slide<16, false, true, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
-         cudaFuncSetAttribute(k_slide<16, false, true, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
-         cudaFuncSetAttribute(k_slide<16, false, true, 512, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
-         cudaFuncSetAttribute(k_slide<16, false, true, 1024, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess;
+         cudaFuncSetAttribute(k_slide<16, false, true, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess;
 }
 
 }  // namespace
@@ -238,7 +230,10 @@ struct volks_plan {
   mutable const float2 *d_cal = nullptr;   // volks_plan_set_cal: DEVICE cf32[nbl][nif][nchan] applied in the slab load
   int nslide = 0;                // widths on the sliding-sum path (k_fixup re-evaluates their outlier windows)
   volks_options opt;             // the options the plan was created with (defaults: volks_options_init)
-  int nhy = 0;                   // sliding widths eligible for the candidates-only index mode
+  int nuntag = 0;                // sliding widths with untagged kernels (their peak bins come from k_recover)
+  bool cand_only = false;        // searches without d_peaks recover indices / evaluate segments for possible candidates only
+  int nprune = 0, prune_nseg = 0, prune_seg = 0, prune_wmax = 0;   // pruned widths (k_bound): count, common segmentation
+  size_t off_flags = 0;          // their segment flags [pairs_per_chunk][nprune][prune_nseg]
   size_t off_thr = 0;            // their windows' pre-thresholds (k_winthr), chunk-relative
   mutable bool last_full_index = true;   // the most recent search left exact indices for EVERY window (volks_zscore_select)
   int device = 0;                // the CUDA device the plan was created on
@@ -303,6 +298,7 @@ void volks_options_init(volks_options *o) {
   memset(o, 0, sizeof *o);
   o->struct_bytes = (int32_t)sizeof(volks_options);
   o->slide_seg = 256; o->y_pad = 16; o->chunk_mb = 4096; o->cf_wpc = 128; o->cf2 = 2; o->ai_waves = 2; o->host_split = 4;
+  o->prune_seg = 64;
 }
 
 int volks_plan_create(const volks_params *p, volks_plan **out) { return plan_create_impl(p, nullptr, out, 0, 0); }
@@ -334,7 +330,8 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
     if (o->struct_bytes != (int32_t)sizeof(volks_options)) return VOLKS_EINVAL;   // built against another header
     opt = *o;
     if (opt.slide_seg < 16 || opt.y_pad < 0 || opt.y_pad > 1024 || (opt.y_pad & 1) || opt.chunk_mb < 1 || opt.cf_wpc < 1 ||
-        (opt.cf2 != 0 && opt.cf2 != 1 && opt.cf2 != 2 && opt.cf2 != 4) || opt.ai_waves < 1 || opt.host_split < 1)
+        (opt.cf2 != 0 && opt.cf2 != 1 && opt.cf2 != 2 && opt.cf2 != 4) || opt.ai_waves < 1 || opt.host_split < 1 ||
+        opt.prune_seg < 16 || opt.prune_seg > 4096 || !is_pow2(opt.prune_seg))
       return VOLKS_EINVAL;
   }
   const bool allif = ai_nif > 0;
@@ -376,11 +373,14 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
     w.slide = !force_generic && w.s == 1 && w.w >= 2 && w.nt == 2 * w.w && p->nf >= 64 &&
               ((long long)p->nap + SLIDE_PF + 2) * (p->nf + 64) * 8 < (1LL << 32);
     if (allif) w.slide = false;
-    // candidates-only index mode: the tag-free maximum pays when a noise window stays below the pre-threshold, i.e.
-    // when snr_thresh^2 is well above the expected noise maximum ln(Nt Nf) + 0.58 of the plane (else: tagged kernel)
-    w.hy = w.slide && w.nt >= 32 && !opt.full_index && p->snr_thresh > 0.f &&
-           (double)p->snr_thresh * p->snr_thresh >= log((double)w.nt * p->nf) + 4.0;
+    w.untag = w.slide && w.nt >= 32;
     w.colfft = !allif && !force_generic && !w.slide && w.nt >= 32 && w.nt <= 512 && p->nf >= 32 && w.nwin > 0;
+    // exact pruning by the amplitude-sum bound (kernels_prune.cuh): narrow widths whose noise-only bound stays
+    // >= 4.5 deviations below the threshold, (0.99 snr_thresh - 0.886 sqrt(w)) / 0.4637 (Rayleigh amplitudes)
+    w.prune = -1;
+    if (w.slide && !opt.full_index && !opt.no_prune && p->snr_thresh > 0.f && w.w <= PRUNE_RING && pl->nprune < PRUNE_MAXQ &&
+        p->nap >= w.w && (0.99 * p->snr_thresh - 0.886 * sqrt((double)w.w)) / 0.4637 >= 4.5 && w.nt <= opt.prune_seg)
+      w.prune = pl->nprune++;
     w.cf_l1 = w.nt / 16;
     w.cf_nz = 1;
     while (w.cf_nz * 16 < w.w) w.cf_nz *= 2;
@@ -389,6 +389,7 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
                                         std::max<long long>(8, (long long)p->nbl * p->nif * (p->nf / 32) * w.nwin / 592));
     w.cf_nrange = (int)((w.nwin + w.cf_wpc - 1) / w.cf_wpc);
     w.seg = std::max((seg_req / w.nt) * w.nt, w.nt);
+    if (w.prune >= 0) w.seg = opt.prune_seg;      // one segmentation for every pruned width (a multiple of its Nt)
     // f2: one CTA per (baseline, segment): segments short enough to fill 148 SMs x 2, at most seg_req windows
     if (allif) w.seg = (int)std::max<long long>(16, std::min<long long>((seg_req / 16) * 16, (w.nwin * p->nbl / 296 + 15) / 16 * 16));
     w.nseg = w.nwin > 0 ? (int)((w.nwin + w.seg - 1) / w.seg) : 0;
@@ -458,6 +459,9 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
       if ((!w.slide && !w.colfft && !allif && col_blocks > GMAX) || (w.slide && slide_blocks > GMAX) ||
           (w.colfft && cf_blocks > GMAX) || (allif && ai_blocks > GMAX)) fits = false;
     }
+    long long rec_warps = 0;
+    for (auto &w : pl->wp) rec_warps += (w.slide && w.nt >= 32) ? w.nwin : 0;
+    if ((long double)ppc_ * rec_warps / 128 > GMAX) fits = false;    // k_recover: one thread per window
     if (!fits) { delete pl; return VOLKS_EINVAL; }
   }
   size_t off = 0;
@@ -467,8 +471,16 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
   // + padding rows: the sliding kernel loads one row, and prefetches SLIDE_PF + 1 rows, past the last sample
   pl->off_noise = off; off = align_up(off + (allif ? (size_t)std::max<long long>(s.nwin_total, 1) * s.ngs * sizeof(float) : 0), 256);
   pl->off_zst = off;  off = align_up(off + (size_t)std::max<long long>(pl->npair * p->nwidths, 1) * sizeof(double2), 256);
-  for (auto &w : pl->wp) pl->nhy += (w.hy && w.nwin > 0) ? 1 : 0;
-  pl->off_thr = off;  off = align_up(off + (pl->nhy ? (size_t)pl->pairs_per_chunk * per_pair * sizeof(uint32_t) : 0), 256);
+  // candidates-only mode (volks_options.full_index = 0, a positive threshold): a search without d_peaks finds the
+  // peak bin only of windows above their pre-threshold and prunes the narrow widths (kernels_prune.cuh)
+  pl->cand_only = !opt.full_index && p->snr_thresh > 0.f;
+  for (auto &w : pl->wp) {
+    pl->nuntag += (w.untag && w.nwin > 0) ? 1 : 0;
+    if (w.prune >= 0) { pl->prune_nseg = std::max(pl->prune_nseg, w.nseg); pl->prune_wmax = std::max(pl->prune_wmax, w.w); }
+  }
+  pl->prune_seg = opt.prune_seg;
+  pl->off_thr = off;  off = align_up(off + ((pl->cand_only && (pl->nuntag || pl->nprune)) ? (size_t)pl->pairs_per_chunk * per_pair * sizeof(uint32_t) : 0), 256);
+  pl->off_flags = off; off = align_up(off + (size_t)pl->pairs_per_chunk * pl->nprune * pl->prune_nseg, 256);
   pl->off_Y = off;    off = align_up(off + (size_t)pl->pairs_per_chunk * std::max<size_t>(y_pair, 8) + (size_t)(SLIDE_PF + 2) * pl->pitch * sizeof(float2), 256);
   pl->ws_bytes = off;
 
@@ -480,7 +492,7 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
   for (int q = 0; q < p->nwidths; ++q) active += (pl->wp[q].nwin > 0 && q != pl->wid1) ? 1 : 0;
   // kernels of this library per search (the key memset is a driver memset, not counted)
   // (a search without dense peaks; with them the candidates-only index mode and its k_winthr launch are off)
-  pl->launches = s.nwin_total > 0 ? (int)(pl->nchunks * (1 + active + (pl->nslide > 0 ? 1 : 0) + (pl->nhy > 0 ? 1 : 0)) + 3) : 0;
+  pl->launches = s.nwin_total > 0 ? (int)(pl->nchunks * (1 + active + (pl->nslide > 0 ? 1 : 0) + ((pl->cand_only && (pl->nuntag || pl->nprune)) ? 1 : 0) + (pl->nprune ? 1 : 0) + (pl->nuntag ? 1 : 0)) + 3) : 0;
 
   // tables, computed in double precision on the host
   if (psub > 1) { pl->premod_off = tw_total; tw_total += (size_t)s.nf; }
@@ -629,7 +641,8 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
   char *ws = (char *)d_workspace;
   // candidates-only index mode for the eligible sliding widths unless the dense peak array (every window's exact
   // index) is wanted or the plan was created with full_index
-  const bool hy = pl->nhy > 0 && d_peaks == nullptr;
+  const bool hy = pl->cand_only && (pl->nuntag > 0 || pl->nprune > 0) && d_peaks == nullptr;
+  const unsigned char *flags = hy && pl->nprune ? (const unsigned char *)(ws + pl->off_flags) : nullptr;
   pl->last_full_index = !hy;
   u64 *keys = (u64 *)(ws + pl->off_keys);
   float *E = (float *)(ws + pl->off_E);
@@ -686,13 +699,32 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
       ta.thr2 = s.snr_thresh * s.snr_thresh; ta.nap = s.nap; ta.nq = 0; ta.cum[0] = 0;
       for (int q = 0; q < s.nwidths; ++q) {
         const WidthPlan &w = pl->wp[q];
-        if (!w.hy || w.nwin == 0) continue;
+        if ((!w.untag && w.prune < 0) || w.nwin == 0) continue;
         const int i = ta.nq++;
         ta.w[i] = w.w; ta.nwin[i] = (int)w.nwin; ta.offc[i] = s.offc[q]; ta.cum[i + 1] = ta.cum[i] + w.nwin;
       }
       ta.total = np * ta.cum[ta.nq];
-      ProfScope ps(pl, st, VOLKS_K_WINTHR, -1);
-      k_winthr<<<(unsigned)((ta.total + 255) / 256), 256, 0, st>>>(ta);
+      {
+        ProfScope ps(pl, st, VOLKS_K_WINTHR, -1);
+        k_winthr<<<(unsigned)((ta.total + 255) / 256), 256, 0, st>>>(ta);
+      }
+      if (flags) {
+        PruneArgs pa;
+        pa.Y = Y; pa.thr = ta.thr; pa.flags = (unsigned char *)(ws + pl->off_flags); pa.per_pair = s.per_pair;
+        pa.nap = s.nap; pa.nf = s.nf; pa.pitch = pl->pitch; pa.nq = pl->nprune; pa.seg = pl->prune_seg;
+        pa.nseg = pl->prune_nseg; pa.wmax = pl->prune_wmax;
+        for (int q = 0; q < s.nwidths; ++q) {
+          const WidthPlan &w = pl->wp[q];
+          if (w.prune < 0) continue;
+          pa.w[w.prune] = w.w; pa.nwin[w.prune] = (int)w.nwin; pa.offc[w.prune] = s.offc[q];
+        }
+        const int T = 2 * pa.seg, thr = std::min(PRUNE_THREADS, s.nf / 2);
+        pa.ring = pa.wmax <= 16 ? 16 : 32;                 // rows of amplitude history (a power of two >= wmax)
+        const size_t smem = (size_t)((pa.nq * T + 3) & ~3) * sizeof(float) + (size_t)pa.ring * thr * sizeof(f32x2);
+        const unsigned blocks = (unsigned)(np * ((pa.nseg + 1) / 2));
+        ProfScope ps(pl, st, VOLKS_K_BOUND, -1);
+        k_bound<<<blocks, thr, smem, st>>>(pa);
+      }
     }
     for (int q = 0; q < s.nwidths; ++q) {
       const WidthPlan &w = pl->wp[q];
@@ -727,9 +759,10 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         sa.nap = s.nap; sa.nf = s.nf; sa.w = w.w; sa.nt = w.nt; sa.log2m = w.log2m; sa.nwin = (int)w.nwin;
         sa.seg = w.seg; sa.nseg = w.nseg; sa.keymask = 0xFFFFFFF0u; sa.pitch = pl->pitch;
         sa.ntasks = ((np * w.nseg * (long long)(s.nf / 64)) << w.log2m);
-        sa.thr = (const uint32_t *)(ws + pl->off_thr);
+        sa.flags = flags && w.prune >= 0 ? flags + (size_t)w.prune * pl->prune_nseg : nullptr;
+        sa.flag_stride = pl->nprune * pl->prune_nseg;
         ProfScope ps(pl, st, VOLKS_K_SLIDE, q);
-        launch_slide(sa, hy && w.hy, st);
+        launch_slide(sa, st);
         continue;
       }
       if (w.colfft) {
@@ -757,16 +790,34 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
       fa.Y = Y; fa.keys = keys; fa.tables = pl->d_tables; fa.per_pair = s.per_pair; fa.pair0 = pair0;
       fa.nap = s.nap; fa.nf = s.nf; fa.log2nf = s.log2nf; fa.pitch = pl->pitch; fa.paired = pl->paired;
       fa.nq = 0; fa.unit0[0] = 0;
+      fa.flags = flags; fa.flag_nq = pl->nprune; fa.flag_nseg = pl->prune_nseg;
       for (int q = 0; q < s.nwidths; ++q) {
         const WidthPlan &w = pl->wp[q];
         if (!w.slide || w.nwin == 0) continue;
         const int i = fa.nq++;
         fa.q[i] = q; fa.w[i] = w.w; fa.nt[i] = w.nt; fa.seg[i] = w.seg; fa.nseg[i] = w.nseg; fa.nwin[i] = (int)w.nwin;
-        fa.offc[i] = s.offc[q]; fa.tw_off[i] = (long long)w.tw_off;
+        fa.offc[i] = s.offc[q]; fa.tw_off[i] = (long long)w.tw_off; fa.flag_q[i] = w.prune;
         fa.unit0[i + 1] = fa.unit0[i] + w.nseg;
       }
       ProfScope ps(pl, st, VOLKS_K_FIXUP, -1);
       k_fixup<<<(unsigned)(np * fa.unit0[fa.nq]), 256, 0, st>>>(fa);
+    }
+    // the peak bins of the untagged sliding widths: every window (full index) or the possible candidates
+    if (pl->nuntag > 0) {
+      RecoverArgs ra2;
+      ra2.Y = Y; ra2.keys = keys; ra2.thr = hy ? (const uint32_t *)(ws + pl->off_thr) : nullptr; ra2.tables = pl->d_tables;
+      ra2.per_pair = s.per_pair; ra2.pair0 = pair0; ra2.nap = s.nap; ra2.nf = s.nf; ra2.log2nf = s.log2nf; ra2.pitch = pl->pitch;
+      ra2.nq = 0; ra2.cum[0] = 0;
+      for (int q = 0; q < s.nwidths; ++q) {
+        const WidthPlan &w = pl->wp[q];
+        if (!w.untag || w.nwin == 0) continue;
+        const int i = ra2.nq++;
+        ra2.w[i] = w.w; ra2.nt[i] = w.nt; ra2.log2m[i] = w.log2m; ra2.nwin[i] = (int)w.nwin; ra2.offc[i] = s.offc[q];
+        ra2.tw_off[i] = (long long)w.tw_off; ra2.cum[i + 1] = ra2.cum[i] + w.nwin;
+      }
+      ra2.total = np * ra2.cum[ra2.nq];
+      ProfScope ps(pl, st, VOLKS_K_RECOVER, -1);
+      k_recover<<<(unsigned)((ra2.total + 127) / 128), 128, 0, st>>>(ra2);
     }
   }
   {

@@ -50,10 +50,10 @@ def test_options_defaults_and_validation_before_cuda(vb):
     before any CUDA call; nf above the row kernels' 8192 points is an explicit VOLKS_EINVAL."""
     o = vb.make_options()
     assert (o.struct_bytes, o.full_index, o.force_generic, o.slide_seg, o.y_pad, o.chunk_mb, o.cf_wpc, o.cf2, o.ai_waves,
-            o.host_split) == (40, 0, 0, 256, 16, 4096, 128, 2, 2, 4)
+            o.host_split, o.no_prune, o.prune_seg) == (48, 0, 0, 256, 16, 4096, 128, 2, 2, 4, 0, 64)
     a = dict(nbl=1, nif=1, nap=512, nchan=32, widths=[8], strides=[1], nts=[16], nf=64, snr_thresh=6.0)
     for bad in (dict(slide_seg=8), dict(y_pad=3), dict(y_pad=-2), dict(chunk_mb=0), dict(cf2=3), dict(ai_waves=0),
-                dict(host_split=0), dict(cf_wpc=0)):
+                dict(host_split=0), dict(cf_wpc=0), dict(prune_seg=48), dict(prune_seg=8)):
         rc, h = vb.plan_create_raw(options=bad, **a)
         assert rc == -1 and not h, bad
     o = vb.make_options()
