@@ -243,7 +243,7 @@ def measure_fp32_peak(vk, local, stream):
                     "%s MHz during the probe); derived 148 SM x 128 lanes x 2 x sm_max_mhz = %.2f" % (ck["sm_mhz"], derived)}
 
 
-def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traffic):
+def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traffic, also_full_index=False):
     """Device-timed throughput + per-launch roofline of one config.  Returns a dict (tensors included, for
     the e2e leg of the main config)."""
     vis, c, _ = workloads.generate(cfg_id, device=dev, seed=workloads.config(cfg_id)["seed"] + 17 * rank)
@@ -306,6 +306,22 @@ def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traff
     value = aggregate_value(world, nwin, ms_step)
     n_found = int(ncand.item()) & 0xFFFFFFFF
 
+    # ---- the other index mode: every window's peak written (dense peak array), nothing pruned ----
+    full_ms = None
+    if also_full_index and peaks is None and not args.allif:
+        pk_all = torch.empty(plan.nwin_total * vk.PEAK_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+        for _ in range(2):
+            plan.fringe_search(vis, ws, cands, ncand, pk_all, stream, shift=shift)
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        f0.record(stream)
+        for _ in range(3):
+            plan.fringe_search(vis, ws, cands, ncand, pk_all, stream, shift=shift)
+        f1.record(stream)
+        torch.cuda.synchronize(dev)
+        full_ms = max_over_ranks(dist, f0.elapsed_time(f1), dev) / 3
+        del pk_all
+
     # ---- roofline leg: per-launch CUDA-event durations on the launching stream ----
     plan.profile(True)
     per = {}
@@ -327,7 +343,7 @@ def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traff
     clocks = sampler.summary()
     base = dict(vk=vk, plan=plan, vis=vis, c=c, ws=ws, cands=cands, ncand=ncand, peaks=peaks, stream=stream, dev=dev,
                 rank=rank, world=world, dist=dist, ms_step=ms_step, value=value, nwin=nwin, nvis=nvis, n_found=n_found,
-                clocks=clocks, cap=cap, shift=shift)
+                clocks=clocks, cap=cap, shift=shift, full_ms=full_ms)
     if args.allif:
         # f2 is bandwidth work: the row pass reads the slab once and writes the all-IF delay spectra, every
         # width's k_allif reads them once.  Roofline of the dominant kernel against measured HBM bandwidth.
@@ -344,9 +360,26 @@ def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traff
             "bytes_kind": "algorithmic: the chunk's all-IF delay spectra read once (row pass: + the slab read once)",
             "kernel_ms": kernel_ms}
         return base
-    if dom[0] == 1:
-        dom_alg = row_alg / nlaunch[dom]
-    elif dom[1] >= 0:
+    if dom[0] in (1, 11):
+        # the row pass (slab read once, delay spectra written once) and the pruning pass (delay spectra read once)
+        # are bandwidth work: roofline against the measured HBM copy bandwidth
+        peaks_json = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        hbm = json.load(open(peaks_json))["hbm_gbs"] if os.path.exists(peaks_json) else 6650.0
+        pitch = c["nf"] + 16 if c["nf"] >= 32 else c["nf"]                # the plan's Y row pitch (default y_pad)
+        ybytes = nbl * nif * nap * pitch * 8.0
+        dom_bytes = (ybytes + nvis * 8.0 + nbl * nif * nap * 4.0 if dom[0] == 1 else ybytes) / nlaunch[dom]
+        gbs = dom_bytes / (dom_ms_avg * 1e-3) / 1e9
+        tr = traffic.get((c["id"], KIND_NAMES.get(dom[0], ""), -1))
+        base["roofline"] = {
+            "bound": "hbm", "kernel": kname, "achieved": gbs, "peak": hbm, "unit": "GB/s", "frac": gbs / hbm,
+            "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None,
+            "launch_ms": dom_ms_avg, "share_of_step": share[dom] / step_sum,
+            "peak_kind": "measured (MEASURED_PEAKS.json hbm_gbs)" if os.path.exists(peaks_json) else "fallback 6650 GB/s",
+            "bytes_kind": "algorithmic: the chunk's delay spectra %s" % ("written once + the slab read once + per-AP energies"
+                                                                          if dom[0] == 1 else "read once"),
+            "hbm_gbs_algorithmic": nvis * 8 / (ms_step * 1e-3) / 1e9, "kernel_ms": kernel_ms}
+        return base
+    if dom[1] >= 0:
         dom_alg = per_w_alg[dom[1]] / nlaunch[dom]
     else:
         dom_alg = 0.0
@@ -426,7 +459,7 @@ def brief(R):
             "visibilities_per_s": R["world"] * R["nvis"] / (R["ms_step"] * 1e-3), "windows": R["nwin"],
             "candidates": R["n_found"], "clocks": R["clocks"],
             "roofline": {k: rf[k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic", "launch_ms",
-                                            "share_of_step", "algorithmic_frac", "kernel_ms") if k in rf}}
+                                            "share_of_step", "algorithmic_frac", "bytes_kind", "kernel_ms") if k in rf}}
 
 
 def main():
@@ -451,14 +484,14 @@ def main():
     # N independent replicas (the path needs no exchange; north_star fixes one
     # GPU, so --gpus N runs N replicas, each the full config with its own seed)
     peak = measure_fp32_peak(vk, local, torch.cuda.current_stream(dev))
-    R = measure(vk, args, args.config, dev, local, rank, dist, args.steps, args.warmup, peak, traffic)
+    R = measure(vk, args, args.config, dev, local, rank, dist, args.steps, args.warmup, peak, traffic, also_full_index=True)
     c = R["c"]
     e2e = None if args.no_e2e else run_e2e(R, max(1, min(args.steps, 3)))
     launches = R["plan"].launches * args.steps
     plan_nf = R["plan"].nf
     others = {}
     if args.config == 2 and not args.allif and not args.dm and not args.no_other_configs:
-        main_line = {k: R[k] for k in ("value", "ms_step", "nwin", "nvis", "n_found", "clocks", "roofline", "world", "rank")}
+        main_line = {k: R[k] for k in ("value", "ms_step", "nwin", "nvis", "n_found", "clocks", "roofline", "world", "rank", "full_ms")}
         R["plan"].close()
         R = None
         torch.cuda.empty_cache()
@@ -488,10 +521,17 @@ def main():
                        "l2": "input slab (%.2f GB) larger than L2, no flush needed" % (R["nvis"] * 8 / 1e9)
                        if R["nvis"] * 8 > 126e6 else "input smaller than L2 (latency-bound config, report only)",
                        "replicas": R["world"], "dense_peaks": bool(args.peaks), "dm": args.dm,
+                       "index_mode": "full (dense peak array: every window's peak bin)" if args.peaks else
+                                     "candidates-only (default volks_options): candidates complete and bit-identical to the full "
+                                     "mode; peak bins found for possible candidates only, segments of narrow windows whose "
+                                     "amplitude-sum bound excludes a candidate are not transformed",
                        "search": "f2 all-IF one-delay search (Eq. 1), nfa %d" % plan_nf if args.allif else "2-D per-IF fringe search"},
             "visibilities_per_s": R["world"] * R["nvis"] / (R["ms_step"] * 1e-3),
             "windows": R["nwin"], "candidates": R["n_found"],
             "clocks": R["clocks"], "e2e": e2e, "gpu_launches": launches,
+            "full_index": None if R.get("full_ms") is None else
+                          {"ms_per_step": R["full_ms"], "windows_per_s": R["world"] * R["nwin"] / (R["full_ms"] * 1e-3),
+                           "what": "the same search with the dense per-window peak array (every window transformed and indexed)"},
             "roofline": R["roofline"], "cpu_baseline": cpu, "fp32_peak_probe": {k: peak[k] for k in ("tflops", "tflops_mean", "launch_ms", "sm_mhz", "reasons", "derived_tflops")},
         }
         if others:

@@ -59,6 +59,8 @@ __device__ __forceinline__ u64 fix_task(const FixArgs &a, const float2 *twt, siz
   return make_key(best, (uint32_t)(rho + (bs << log2m)) * (uint32_t)a.nf + (uint32_t)d);
 }
 
+constexpr int FIX_GROUP = 16;   // segments per CTA (a unit): most are skipped at once, a CTA per segment was launch-bound
+
 __global__ void __launch_bounds__(256) k_fixup(FixArgs a) {
   __shared__ float pmax[256];
   __shared__ u64 red[8];
@@ -68,8 +70,9 @@ __global__ void __launch_bounds__(256) k_fixup(FixArgs a) {
   const long long pl = blockIdx.x / upp;
   int u = (int)(blockIdx.x % upp), i = 0;
   while (u >= a.unit0[i + 1]) ++i;
-  const int sg = u - a.unit0[i];
-  if (a.flags && a.flag_q[i] >= 0 && !a.flags[(pl * a.flag_nq + a.flag_q[i]) * a.flag_nseg + sg]) return;
+  const int sg_lo = (u - a.unit0[i]) * FIX_GROUP, sg_hi = min(a.nseg[i], sg_lo + FIX_GROUP);
+  for (int sg = sg_lo; sg < sg_hi; ++sg) {
+  if (a.flags && a.flag_q[i] >= 0 && !a.flags[(pl * a.flag_nq + a.flag_q[i]) * a.flag_nseg + sg]) continue;
   const int w = a.w[i], nt = a.nt[i], seg = a.seg[i];
   const int j0 = sg * seg, n = min(seg, a.nwin[i] - j0);          // windows j0 .. j0+n-1 (seg <= 256? see below)
   u64 *keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc[i]);
@@ -122,6 +125,7 @@ __global__ void __launch_bounds__(256) k_fixup(FixArgs a) {
     }
     if (threadIdx.x == 0) carry = pmax[255];
     __syncthreads();
+  }
   }
 }
 

@@ -11,8 +11,8 @@
 // the peak search of a whole segment of windows are needed only where some window of it comes near the threshold
 // in some column: around pulses and interference.
 //   k_bound   one pass over the chunk's delay spectra: CTA = (pair, tile of 2 segments of window starts),
-//             thread = column pair, the last 32 amplitudes of its columns in a shared-memory ring, one running
-//             sum per pruned width; flags[pair][width][segment] = 1 iff some (window, column) of the segment has
+//             thread = column pair, the running amplitude sums of its columns in a shared-memory ring (a window's
+//             bound is the difference of two of them); flags[pair][width][segment] = 1 iff some (window, column) of the segment has
 //             bound^2 > pre-threshold of that window (k_winthr: 0.98 snr_thresh^2 noise - the 2 % cover every
 //             rounding on both sides).  The sliding kernels return at once for a segment whose flag is 0; its
 //             windows keep the zero key (power 0, snr 0: not candidates - which is all the mode promises).
@@ -37,37 +37,51 @@ struct PruneArgs {
   long long offc[PRUNE_MAXQ];
 };
 
+template <int NQ>
 __global__ void __launch_bounds__(PRUNE_THREADS) k_bound(PruneArgs a) {
   extern __shared__ float prune_sm[];
-  // shared: thr[nq][2 seg] floats, then the ring [a.ring][blockDim.x] of packed amplitude pairs
-  const int T = 2 * a.seg;
+  // shared: thr[NQ][TP] floats (TP = 2 seg + 64: 32 entries of +inf before and after the tile's windows, so that
+  // window starts outside the tile need no branch), then the ring [a.ring][blockDim.x] of packed running sums
+  const int T = 2 * a.seg, TP = T + 64;
   float *thr_sm = prune_sm;
-  f32x2 *ring = (f32x2 *)(prune_sm + ((a.nq * T + 3) & ~3));
   __shared__ int any[PRUNE_MAXQ][2];
   const int ntile = (a.nseg + 1) / 2;
   const long long pl = blockIdx.x / ntile;
   const int tile = (int)(blockIdx.x % ntile);
   const int R0 = tile * T;                                   // first window start (= first row) of the tile
-  const int nthr = blockDim.x, rmask = a.ring - 1;
-  for (int i = threadIdx.x; i < a.nq * T; i += nthr) {
-    const int q = i / T, j = i - q * T;
-    thr_sm[i] = R0 + j < a.nwin[q] ? __uint_as_float(__ldg(a.thr + pl * a.per_pair + a.offc[q] + R0 + j)) : 3.0e38f;
+  const int nthr = blockDim.x;                               // a power of two (nf / 2 or 128)
+  for (int i = threadIdx.x; i < NQ * TP; i += nthr) {
+    const int q = i / TP, j = i - q * TP - 32;
+    thr_sm[i] = (j >= 0 && j < T && R0 + j < a.nwin[q]) ? __uint_as_float(__ldg(a.thr + pl * a.per_pair + a.offc[q] + R0 + j)) : 3.0e38f;
   }
   if (threadIdx.x < PRUNE_MAXQ * 2) any[threadIdx.x >> 1][threadIdx.x & 1] = 0;
-  __syncthreads();
   const int nrows = min(T + a.wmax - 1, a.nap - R0);         // rows R0 .. R0 + nrows - 1 exist
   const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch);
   const size_t rowb = (size_t)a.pitch * 8u;
-  f32x2 *myring = ring + threadIdx.x;
+  // ring of running sums C[r] = sum_{r' <= r} |Y[r']| of the thread's two columns: the bound of the window of width w
+  // ending at row r is C[r] - C[r - w] (C = 0 before the tile: the ring starts zeroed).  Byte offsets wrap with one AND.
+  char *ring = (char *)(prune_sm + ((NQ * TP + 3) & ~3)) + threadIdx.x * 8u;
+  const uint32_t rstride = (uint32_t)nthr * 8u, rmask = (uint32_t)a.ring * rstride - 1u;
+  // per width: byte offset of the leaving sum relative to the entering one, the threshold row, the first row of the
+  // tile's second segment, the two flag bits
+  uint32_t back[NQ], rhalf[NQ];
+  const float *thq[NQ];
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) {
+    back[q] = (uint32_t)a.w[q] * rstride;
+    thq[q] = thr_sm + q * TP + 33 - a.w[q];                  // thq[q][r] = pre-threshold of the window ending at row r
+    rhalf[q] = (uint32_t)(a.seg + a.w[q] - 1);
+  }
+  __syncthreads();
   unsigned hit = 0;                                          // bit 2 q + half
   for (int c = threadIdx.x; c < (a.nf >> 1); c += nthr) {
-    f32x2 S[PRUNE_MAXQ];
-#pragma unroll
-    for (int q = 0; q < PRUNE_MAXQ; ++q) S[q] = pk(0.f, 0.f);
+    for (int k = 0; k < a.ring; ++k) *(f32x2 *)(ring + (uint32_t)k * rstride) = pk(0.f, 0.f);
     const char *p = ybase + (size_t)R0 * rowb + (size_t)c * 16u;
     f32x2 bx[4], by[4];                                      // four rows in flight
 #pragma unroll
     for (int u = 0; u < 4; ++u) { bx[u] = by[u] = pk(0.f, 0.f); if (u < nrows) ldg2(p + (size_t)u * rowb, bx[u], by[u]); }
+    f32x2 C = pk(0.f, 0.f);
+    uint32_t roff = 0;
     for (int r0 = 0; r0 < nrows; r0 += 4) {
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
@@ -79,39 +93,35 @@ __global__ void __launch_bounds__(PRUNE_THREADS) k_bound(PruneArgs a) {
           float aa, ab;
           asm("sqrt.approx.f32 %0, %1;" : "=f"(aa) : "f"(lo32(e)));
           asm("sqrt.approx.f32 %0, %1;" : "=f"(ab) : "f"(hi32(e)));
-          const f32x2 amp = pk(aa, ab);
-          // (the leaving amplitudes are read BEFORE the new one is stored: for w == ring they share a slot)
+          C = add2(C, pk(aa, ab));
+          f32x2 old[NQ];
+          float th[NQ];
 #pragma unroll
-          for (int q = 0; q < PRUNE_MAXQ; ++q) {
-            if (q < a.nq) {                                  // uniform
-              const int wq = a.w[q];
-              S[q] = add2(S[q], amp);
-              if (r >= wq) S[q] = sub2(S[q], myring[((r - wq) & rmask) * nthr]);
-            }
+          for (int q = 0; q < NQ; ++q) {                     // (read before this row's store: for w == ring they share a slot)
+            old[q] = *(const f32x2 *)(ring + ((roff - back[q]) & rmask));
+            th[q] = thq[q][r];
           }
-          myring[(r & rmask) * nthr] = amp;
 #pragma unroll
-          for (int q = 0; q < PRUNE_MAXQ; ++q) {
-            if (q < a.nq) {
-              const int j = r - a.w[q] + 1;                  // window start relative to the tile
-              if (j >= 0 && j < T) {
-                const float th = thr_sm[q * T + j];
-                const float sa = lo32(S[q]), sb = hi32(S[q]);
-                if (sa * sa > th || sb * sb > th) hit |= 1u << (2 * q + (j >= a.seg ? 1 : 0));
-              }
-            }
+          for (int q = 0; q < NQ; ++q) {
+            const f32x2 S = sub2(C, old[q]);
+            const float m = fmaxf(lo32(S), hi32(S));
+            if (m * m > th[q]) hit |= (uint32_t)r >= rhalf[q] ? 2u << (2 * q) : 1u << (2 * q);
           }
+          *(f32x2 *)(ring + (roff & rmask)) = C;
+          roff += rstride;
         }
       }
     }
   }
-  for (int q = 0; q < a.nq; ++q)
+#pragma unroll
+  for (int q = 0; q < NQ; ++q)
+#pragma unroll
     for (int h = 0; h < 2; ++h)
       if (__ballot_sync(0xffffffffu, (hit >> (2 * q + h)) & 1u) && (threadIdx.x & 31) == 0) any[q][h] = 1;
   __syncthreads();
-  if (threadIdx.x < a.nq * 2) {
+  if (threadIdx.x < NQ * 2) {
     const int q = threadIdx.x >> 1, h = threadIdx.x & 1, sg = 2 * tile + h;
-    if (sg < a.nseg) a.flags[(pl * a.nq + q) * a.nseg + sg] = (unsigned char)any[q][h];
+    if (sg < a.nseg) a.flags[(pl * NQ + q) * a.nseg + sg] = (unsigned char)any[q][h];
   }
 }
 

@@ -720,10 +720,19 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         }
         const int T = 2 * pa.seg, thr = std::min(PRUNE_THREADS, s.nf / 2);
         pa.ring = pa.wmax <= 16 ? 16 : 32;                 // rows of amplitude history (a power of two >= wmax)
-        const size_t smem = (size_t)((pa.nq * T + 3) & ~3) * sizeof(float) + (size_t)pa.ring * thr * sizeof(f32x2);
+        const size_t smem = (size_t)((pa.nq * (T + 64) + 3) & ~3) * sizeof(float) + (size_t)pa.ring * thr * sizeof(f32x2);
         const unsigned blocks = (unsigned)(np * ((pa.nseg + 1) / 2));
         ProfScope ps(pl, st, VOLKS_K_BOUND, -1);
-        k_bound<<<blocks, thr, smem, st>>>(pa);
+        switch (pa.nq) {
+          case 1: k_bound<1><<<blocks, thr, smem, st>>>(pa); break;
+          case 2: k_bound<2><<<blocks, thr, smem, st>>>(pa); break;
+          case 3: k_bound<3><<<blocks, thr, smem, st>>>(pa); break;
+          case 4: k_bound<4><<<blocks, thr, smem, st>>>(pa); break;
+          case 5: k_bound<5><<<blocks, thr, smem, st>>>(pa); break;
+          case 6: k_bound<6><<<blocks, thr, smem, st>>>(pa); break;
+          case 7: k_bound<7><<<blocks, thr, smem, st>>>(pa); break;
+          default: k_bound<8><<<blocks, thr, smem, st>>>(pa); break;
+        }
       }
     }
     for (int q = 0; q < s.nwidths; ++q) {
@@ -797,7 +806,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         const int i = fa.nq++;
         fa.q[i] = q; fa.w[i] = w.w; fa.nt[i] = w.nt; fa.seg[i] = w.seg; fa.nseg[i] = w.nseg; fa.nwin[i] = (int)w.nwin;
         fa.offc[i] = s.offc[q]; fa.tw_off[i] = (long long)w.tw_off; fa.flag_q[i] = w.prune;
-        fa.unit0[i + 1] = fa.unit0[i] + w.nseg;
+        fa.unit0[i + 1] = fa.unit0[i] + (w.nseg + FIX_GROUP - 1) / FIX_GROUP;
       }
       ProfScope ps(pl, st, VOLKS_K_FIXUP, -1);
       k_fixup<<<(unsigned)(np * fa.unit0[fa.nq]), 256, 0, st>>>(fa);
