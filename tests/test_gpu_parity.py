@@ -641,3 +641,65 @@ def test_cufft_cross_check(vb, oracle):
             assert abs(P.sum() / (nt * nf) - o["s1"] / (nt * nf)) <= 1e-4 * o["s1"] / (nt * nf)
             noise = P.sum() / (nt * nf)
             assert abs(float(g["snr"]) - np.sqrt(P.max() / noise)) <= 1e-4 * o["snr"]
+
+
+def test_sliding_sum_adversarial(vb, oracle):
+    """The worst case the sliding kernels can meet without the fix-up stepping in (the 1e-4 bound of the
+    sliding sum is statistical): one delay column driven by a coherent burst whose power stays just UNDER the fix-up
+    ratio (1000x) of the windows that follow, and after it the same weak noiseless tone in every AP, so that every
+    window of the rest of the segment has the same small peak and any residue of the burst shows directly.  Every
+    window of every sliding width must stay within 1e-4 of the oracle, in both index modes."""
+    nchan, nap, nf = 64, 900, 128
+    widths, strides, nts = [2, 4, 8, 16, 32, 64], [1] * 6, [4, 8, 16, 32, 64, 128]
+    k = torch.arange(nchan, dtype=torch.float64)
+    tone = torch.polar(torch.full((nchan,), 0.01, dtype=torch.float64), 2 * np.pi * 9.0 * k / nf)   # on delay bin 9
+    vis = tone.to(torch.complex64).repeat(nap, 1).reshape(1, 1, nap, nchan).clone()
+    # the peak power of a tone window is (a w nchan)^2; with 4 burst APs at 480 a inside, a w = 64 window peaks at
+    # ((60 + 4 * 480) a nchan)^2 = 957 x the later windows: just under the fix-up ratio for the width with the longest
+    # memory, far above it for the narrow ones (their windows after the burst are re-evaluated, which is tested too)
+    vis[0, 0, 130:134] = (tone * 480.0).to(torch.complex64)
+    g = torch.Generator().manual_seed(5)
+    vis += (torch.view_as_complex(torch.randn((1, 1, nap, nchan, 2), generator=g)) * 1e-6)   # breaks exact ties only
+    c = dict(widths=widths, strides=strides, nts=nts, nf=nf, snr_thresh=6.0)
+    (nties, perr, serr), ncand, cands, ora = run_both(vb, oracle, vis, c, mode="fft")
+    assert perr <= 1e-4 and serr <= 1e-4 and ncand > 1000          # (nearly every window is a candidate: a pure tone)
+    run_both(vb, oracle, vis, c, mode="fft", options=dict(slide_seg=1024))   # the longest segment the option allows here
+
+
+@pytest.mark.parametrize("prune_seg", [16, 64, 256])
+def test_pruning_keeps_every_candidate(vb, oracle, prune_seg):
+    """Candidates-only mode (volks_options defaults) against the full-index mode and the oracle on data where the
+    amplitude-sum bound prunes most segments: weak and strong pulses at segment seams, a pulse in the last windows, an
+    RFI burst, a flagged (zero) span.  Within one plan the two index modes must agree bit for bit (run_both asserts it);
+    across segment lengths / pruning off / full_index the arithmetic of the sliding sum differs in the last bits, so
+    there the lists must hold the same windows and bins with powers equal to 1e-5."""
+    vis, c, _ = workloads.generate(3, nbl=2, nif=2, nap=2100, npulses=0)
+    nbl, nif, nap, nchan = vis.shape
+    k = torch.arange(nchan, dtype=torch.float64)
+    def pulse(bl, ifq, t0, w, a, tau):
+        ph = torch.polar(torch.full((nchan,), a, dtype=torch.float64), 2 * np.pi * tau * k / nchan)
+        vis[bl, ifq, t0:t0 + w] += ph.to(torch.complex64)
+    pulse(0, 0, 60, 8, 1.2, 3.0)          # inside one segment of 64
+    pulse(0, 1, 63, 2, 2.5, -5.0)         # straddles a seam at 64
+    pulse(1, 0, 255, 16, 0.9, 1.0)        # straddles a seam at 256
+    pulse(1, 1, nap - 5, 5, 3.0, 7.0)     # the last windows of the slab
+    pulse(0, 0, 1000, 1, 6.0, 0.0)        # a single-AP burst
+    pulse(1, 0, 1500, 4, 0.45, 2.0)       # weak: near the threshold for some widths
+    vis[1, 1, 700:900] = 0                # flagged span
+    ref = None
+    for opts in (dict(prune_seg=prune_seg), dict(no_prune=1), dict(full_index=1)):
+        stats, ncand, cands, ora = run_both(vb, oracle, vis, c, options=opts)
+        assert ncand >= 20
+        if ref is not None:
+            for f in ("bl", "ifq", "wid", "win", "t0", "rate_idx", "delay_idx"):
+                assert np.array_equal(cands[f], ref[f]), f
+            assert np.all(np.abs(cands["power"] - ref["power"]) <= 1e-5 * ref["power"])
+        ref = cands
+    plan = vb.Plan(nbl, nif, nap, nchan, c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"])
+    ws = torch.empty(plan.workspace_bytes, dtype=torch.uint8, device="cuda")
+    cbuf = torch.empty(1 << 16, dtype=torch.uint8, device="cuda")
+    nc = torch.zeros(1, dtype=torch.int32, device="cuda")
+    plan.fringe_search(vis.cuda(), ws, cbuf, nc)
+    with pytest.raises(vb.VolksError):                 # the candidates-only search left no exact index for every window
+        plan.zscore_select(ws, 3.0, cbuf, nc)
+    plan.close()
