@@ -95,6 +95,16 @@ static inline void scan_bin(vo_peak *pk, double p, int64_t i) {
   if (p > pk->p1) { pk->p2 = pk->p1; pk->idx2 = pk->idx1; pk->p1 = p; pk->idx1 = i; }
   else if (p > pk->p2) { pk->p2 = p; pk->idx2 = i; }
 }
+/* Restricted delay search range ("the delay search range and the related FFT size is configured for
+ * projected baselines shorter than 3000 km"; reading A14): the maximum is looked for only in the delay
+ * bins dlo, dlo+1, ..., dhi of the padded axis, wrapping through nf-1 -> 0 when dlo > dhi (delays around zero are
+ * {nf-m .. nf-1, 0 .. m}); the noise statistic S1 stays the sum over the WHOLE plane.  dlo < 0: whole axis. */
+static inline int delay_in_range(int d, int dlo, int dhi) {
+  if (dlo < 0) return 1;
+  return dlo <= dhi ? (d >= dlo && d <= dhi) : (d >= dlo || d <= dhi);
+}
+/* a bin outside the range still counts for S1 */
+static inline void scan_bin_out(vo_peak *pk, double p) { pk->s1 += p; }
 static void scan_end(vo_peak *pk, int nt, int nf) {
   double noise = pk->s1 / ((double)nt * (double)nf);
   pk->snr = noise > 0.0 ? sqrt(pk->p1 / noise) : 0.0;
@@ -103,7 +113,7 @@ static void scan_end(vo_peak *pk, int nt, int nf) {
 /* mode 0: the definition.  win = float32 [w][nchan][2] with row stride `ld` complex samples.
  * If plane != NULL it receives F as [nt][nf] complex128. */
 static void window_direct(const float *win, int64_t ld, int w, int nchan, int nt, int nf,
-                          cplx *plane, vo_peak *pk) {
+                          cplx *plane, vo_peak *pk, int dlo, int dhi) {
   scan_begin(pk);
   for (int r = 0; r < nt; ++r)
     for (int d = 0; d < nf; ++d) {
@@ -117,7 +127,8 @@ static void window_direct(const float *win, int64_t ld, int w, int nchan, int nt
           acc += v * (cos(ph) + I * sin(ph));
         }
       if (plane) plane[(int64_t)r * nf + d] = acc;
-      scan_bin(pk, creal(acc) * creal(acc) + cimag(acc) * cimag(acc), (int64_t)r * nf + d);
+      if (delay_in_range(d, dlo, dhi)) scan_bin(pk, creal(acc) * creal(acc) + cimag(acc) * cimag(acc), (int64_t)r * nf + d);
+      else scan_bin_out(pk, creal(acc) * creal(acc) + cimag(acc) * cimag(acc));
     }
   scan_end(pk, nt, nf);
 }
@@ -149,11 +160,12 @@ static void plane_fft(const float *win, int64_t ld, int w, int nchan, int nt, in
   free(rowin); free(rowout);
 }
 
-static void scan_plane(const cplx *plane, int nt, int nf, vo_peak *pk) {
+static void scan_plane(const cplx *plane, int nt, int nf, vo_peak *pk, int dlo, int dhi) {
   scan_begin(pk);
   for (int64_t i = 0; i < (int64_t)nt * nf; ++i) {
     double re = creal(plane[i]), im = cimag(plane[i]);
-    scan_bin(pk, re * re + im * im, i);
+    if (delay_in_range((int)(i % nf), dlo, dhi)) scan_bin(pk, re * re + im * im, i);
+    else scan_bin_out(pk, re * re + im * im);
   }
   scan_end(pk, nt, nf);
 }
@@ -164,17 +176,18 @@ static void scan_plane(const cplx *plane, int nt, int nf, vo_peak *pk) {
  * samples of which the first nchan per row are used.  mode 0 = direct sum, 1 = FFT.
  * plane (nullable) receives F as [nt][nf] complex128.  Returns 0, or -1 on bad arguments. */
 int vo_window(int mode, const float *win, int64_t ld, int w, int nchan, int nt, int nf,
-              double *plane_out, vo_peak *pk) {
+              double *plane_out, vo_peak *pk, int dlo, int dhi) {
   if (!win || !pk || w < 1 || nchan < 1 || nt < w || nf < nchan) return -1;
+  if (dlo >= nf || dhi >= nf || (dlo >= 0 && dhi < 0)) return -1;
   if (mode == 0) {
-    window_direct(win, ld, w, nchan, nt, nf, (cplx *)plane_out, pk);
+    window_direct(win, ld, w, nchan, nt, nf, (cplx *)plane_out, pk, dlo, dhi);
     return 0;
   }
   if (!is_pow2(nt) || !is_pow2(nf)) return -1;
   cplx *twf = make_twiddles(nf), *twt = make_twiddles(nt);
   cplx *plane = plane_out ? (cplx *)plane_out : (cplx *)malloc(sizeof(cplx) * (size_t)nt * nf);
   plane_fft(win, ld, w, nchan, nt, nf, plane, twf, twt);
-  scan_plane(plane, nt, nf, pk);
+  scan_plane(plane, nt, nf, pk, dlo, dhi);
   if (!plane_out) free(plane);
   free(twf); free(twt);
   return 0;
@@ -194,8 +207,9 @@ static int64_t nwin_of(int nap, int w, int s) { return nap < w ? 0 : (int64_t)(n
 
 int vo_search(const float *vis, int nbl, int nif, int nap, int nchan, int nwidths,
               const int32_t *width, const int32_t *stride, const int32_t *nt, int nf, int mode,
-              const int64_t *sel, int64_t nsel, vo_peak *out, int nthreads) {
+              const int64_t *sel, int64_t nsel, vo_peak *out, int nthreads, int dlo, int dhi) {
   if (!vis || !out || nbl < 1 || nif < 1 || nap < 0 || nchan < 1 || nwidths < 1) return -1;
+  if (dlo >= nf || dhi >= nf || (dlo >= 0 && dhi < 0)) return -1;
   if (nf < nchan || (mode != 0 && !is_pow2(nf))) return -1;
   int ntmax = 1;
   int64_t per_pair = 0;
@@ -261,7 +275,10 @@ int vo_search(const float *vis, int nbl, int nif, int nap, int nchan, int nwidth
             }
             vo_peak pk;
             scan_begin(&pk);
-            for (int64_t i = 0; i < (int64_t)ntq * nf; ++i) scan_bin(&pk, P[i], i);
+            for (int64_t i = 0; i < (int64_t)ntq * nf; ++i) {
+              if (delay_in_range((int)(i % nf), dlo, dhi)) scan_bin(&pk, P[i], i);
+              else scan_bin_out(&pk, P[i]);
+            }
             scan_end(&pk, ntq, nf);
             out[pair * per_pair + off + j] = pk;
           }
@@ -299,11 +316,11 @@ int vo_search(const float *vis, int nbl, int nif, int nap, int nchan, int nwidth
       int64_t t0 = rem * stride[q];
       const float *win = vis + 2 * ((pair * nap + t0) * (int64_t)nchan);
       if (wmode == 0) {
-        window_direct(win, nchan, width[q], nchan, nt[q], nf, NULL, &out[i]);
+        window_direct(win, nchan, width[q], nchan, nt[q], nf, NULL, &out[i], dlo, dhi);
       } else {
         cplx *twt = make_twiddles(nt[q]);
         plane_fft(win, nchan, width[q], nchan, nt[q], nf, plane, twf, twt);
-        scan_plane(plane, nt[q], nf, &out[i]);
+        scan_plane(plane, nt[q], nf, &out[i], dlo, dhi);
         free(twt);
       }
     }

@@ -14,7 +14,9 @@ DESIGN.md) except `window_match`, which is pinned only by hand-built constructio
 brute-force statement of the same rule (the paper gives no worked example) - see DESIGN.md.
 `dedisperse` / `dm_shifts` (step 4) are pinned by test_dedispersion_pins and
 test_dedispersed_pulse_closed_form; `allif_search` (Eq. 1) by test_allif_search_pins; `zscore_candidates`
-by test_zscore_selection_pins; `baseline_match` by constructions only (parity unpinned beyond those).
+by test_zscore_selection_pins; `baseline_match` by direct constructions and an independent sweep statement
+(test_baseline_match_constructions, test_baseline_match_vs_sweep); the restricted delay range (`delay_range`,
+PAPER.md:208) by test_delay_range_pins (closed form off the allowed columns, numpy.fft2 masked, Parseval unchanged).
 """
 import ctypes
 import os
@@ -77,7 +79,18 @@ def nwin(nap, w, s):
     return 0 if nap < w else (nap - w) // s + 1
 
 
-def window(win, nt, nf, mode="fft", want_plane=False):
+def _range(delay_range):
+    """(dlo, dhi) of a restricted delay search range, or (-1, -1) for the whole axis (A14):
+    the maximum is looked for in the padded delay bins dlo..dhi, wrapping through nf-1 -> 0 when dlo > dhi; the noise
+    statistic stays the whole plane's."""
+    if delay_range is None:
+        return -1, -1
+    lo, hi = int(delay_range[0]), int(delay_range[1])
+    assert lo >= 0 and hi >= 0
+    return lo, hi
+
+
+def window(win, nt, nf, mode="fft", want_plane=False, delay_range=None):
     """Fringe-search one window.  win: complex [w][nchan].  Returns (peak record, plane|None)."""
     lib = _load()
     win, wf = _as_f32_pairs(win)
@@ -88,13 +101,13 @@ def window(win, nt, nf, mode="fft", want_plane=False):
         ctypes.c_int(MODES[mode]), wf.ctypes.data_as(ctypes.c_void_p), ctypes.c_int64(nchan),
         ctypes.c_int(w), ctypes.c_int(nchan), ctypes.c_int(nt), ctypes.c_int(nf),
         plane.ctypes.data_as(ctypes.c_void_p) if want_plane else None,
-        pk.ctypes.data_as(ctypes.c_void_p))
+        pk.ctypes.data_as(ctypes.c_void_p), ctypes.c_int(_range(delay_range)[0]), ctypes.c_int(_range(delay_range)[1]))
     if rc != 0:
         raise ValueError("vo_window: bad arguments")
     return pk[0], plane
 
 
-def search(vis, widths, strides, nts, nf, mode="cached", select=None, nthreads=0):
+def search(vis, widths, strides, nts, nf, mode="cached", select=None, nthreads=0, delay_range=None):
     """Peak record of every window (or of the canonical indices in `select`).
 
     vis: complex64 [nbl][nif][nap][nchan].  Output order: canonical (bl, ifq, q, j).
@@ -116,7 +129,8 @@ def search(vis, widths, strides, nts, nf, mode="cached", select=None, nthreads=0
         ctypes.c_int(nap), ctypes.c_int(nchan), ctypes.c_int(len(widths)),
         widths.ctypes.data_as(ctypes.c_void_p), strides.ctypes.data_as(ctypes.c_void_p),
         nts.ctypes.data_as(ctypes.c_void_p), ctypes.c_int(nf), ctypes.c_int(MODES[mode]),
-        selp, ctypes.c_int64(nsel), out.ctypes.data_as(ctypes.c_void_p), ctypes.c_int(nthreads))
+        selp, ctypes.c_int64(nsel), out.ctypes.data_as(ctypes.c_void_p), ctypes.c_int(nthreads),
+        ctypes.c_int(_range(delay_range)[0]), ctypes.c_int(_range(delay_range)[1]))
     if used < 0:
         raise ValueError("vo_search: bad arguments")
     return out, used

@@ -313,6 +313,58 @@ def test_window_match_vs_python_graph_search(oracle):
     assert [(int(p["rep"]), int(p["nwidths_hit"]), int(p["t_begin"]), int(p["t_end"])) for p in got] == expect
 
 
+def test_delay_range_pins(oracle):
+    """Restricted delay search range ("the delay search range and the related FFT size is configured for
+    projected baselines shorter than 3000 km"; A14): the argmax runs over the allowed delay bins only (a range
+    that wraps through zero when lo > hi), the noise statistic stays the whole plane's."""
+    w, nchan, nt, nf, a = 8, 32, 16, 64, 0.7
+    tau, rho = 5.0, 2.0                              # on-bin fringe: peak at padded (r*, d*) = (4, 10)
+    t, k = np.arange(w)[:, None], np.arange(nchan)[None, :]
+    win = (a * np.exp(2j * np.pi * (tau * k / nchan + rho * t / w))).astype(np.complex64)
+    full, _ = oracle.window(win, nt, nf)
+    assert full["idx1"] == 4 * nf + 10
+    for rg in [(0, nf - 1), (10, 10), (3, 20), (60, 12)]:         # ranges that contain d* = 10: nothing changes
+        r, _ = oracle.window(win, nt, nf, delay_range=rg)
+        assert (r["idx1"], r["p1"], r["s1"], r["snr"]) == (full["idx1"], full["p1"], full["s1"], full["snr"])
+    # ranges that exclude d*: closed form |F[r][d]| = a |D_w(r/Nt - rho/w)| |D_nchan(d/Nf - tau/nchan)|, D_M(x) =
+    # sin(pi M x)/sin(pi x); the rate factor peaks at r = 4 (value w), the delay factor decides among the allowed d
+    def dirichlet(m, x):
+        x = np.asarray(x, dtype=np.float64)
+        den = np.sin(np.pi * x)
+        return np.where(np.abs(den) < 1e-12, float(m), np.sin(np.pi * m * x) / np.where(np.abs(den) < 1e-12, 1.0, den))
+    for rg in [(12, 30), (40, 8), (11, 11), (0, 9)]:
+        lo, hi = rg
+        cols = [d for d in range(nf) if (lo <= d <= hi if lo <= hi else (d >= lo or d <= hi))]
+        amp = a * w * np.abs(dirichlet(nchan, np.array(cols) / nf - tau / nchan))
+        best = int(np.argmax(amp))                   # first maximum = lowest d (cols ascend)
+        r, _ = oracle.window(win, nt, nf, delay_range=rg)
+        assert r["idx1"] == 4 * nf + cols[best], (rg, r["idx1"], cols[best])
+        assert abs(r["p1"] - amp[best] ** 2) <= 1e-6 * max(amp[best] ** 2, 1.0)     # inputs are float32
+        assert abs(r["s1"] - full["s1"]) <= 1e-9 * full["s1"]                       # Parseval: the noise is unchanged
+        assert abs(r["snr"] - np.sqrt(r["p1"] / (full["s1"] / (nt * nf)))) <= 1e-12 * max(r["snr"], 1.0)
+    # library special case on noise: numpy.fft2's plane, masked, in all three modes of a search
+    rng = np.random.default_rng(21)
+    vis = (rng.normal(size=(1, 2, 40, 12)) + 1j * rng.normal(size=(1, 2, 40, 12))).astype(np.complex64)
+    widths, strides, nts, nf2 = [3, 8], [2, 5], [4, 16], 16
+    for rg in [(2, 6), (13, 1), (7, 7)]:
+        lo, hi = rg
+        allowed = np.array([(lo <= d <= hi if lo <= hi else (d >= lo or d <= hi)) for d in range(nf2)])
+        res = {m: oracle.search(vis, widths, strides, nts, nf2, mode=m, delay_range=rg)[0] for m in ("direct", "fft", "cached")}
+        i = 0
+        for pair in range(2):
+            for wq, sq, ntq in zip(widths, strides, nts):
+                for j in range(oracle.nwin(40, wq, sq)):
+                    P = np.abs(np.fft.fft2(vis[0, pair, j * sq: j * sq + wq].astype(np.complex128), s=(ntq, nf2))) ** 2
+                    Pm = np.where(allowed[None, :], P, -1.0)
+                    for m in res:
+                        r = res[m][i]
+                        assert r["idx1"] == int(np.argmax(Pm)) and abs(r["p1"] - Pm.max()) <= 1e-9 * Pm.max()
+                        assert abs(r["s1"] - P.sum()) <= 1e-9 * P.sum()
+                    i += 1
+    with pytest.raises(ValueError):
+        oracle.window(win, nt, nf, delay_range=(0, nf))
+
+
 def test_baseline_match_constructions(oracle):
     """f3 pins ON THE ORACLE (PAPER.md:198 "identified if it is detected with at least 5 baselines";
     DESIGN.md A19): hand-built pulse lists whose answer is fixed by the rule itself."""
