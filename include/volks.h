@@ -104,6 +104,11 @@ typedef struct {
                          /* default a segment of windows whose amplitude-sum bound stays below the threshold in every */
                          /* delay column is not transformed at all (it cannot hold a candidate)                       */
   int32_t prune_seg;     /* windows per pruned segment (default 64; power of two, 16..4096)                          */
+  int32_t delay_lo;      /* restricted delay search range ("the delay search range and the related FFT   */
+  int32_t delay_hi;      /* size is configured for projected baselines shorter than 3000 km"): the peak is looked for */
+                         /* in the bins delay_lo .. delay_hi of the padded delay axis only, wrapping through nf-1 -> 0 */
+                         /* when delay_lo > delay_hi (delays around zero: {nf-m .. nf-1, 0 .. m}); the noise statistic */
+                         /* stays the whole plane's.  Default 0, -1: the whole axis.  For an all-IF plan: bins of nfa.  */
 } volks_options;
 void volks_options_init(volks_options *o);
 

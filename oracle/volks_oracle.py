@@ -283,7 +283,7 @@ def allif_band(vis):
     return np.ascontiguousarray(vis.transpose(0, 2, 1, 3)).reshape(nbl, nap, nif * nchan)
 
 
-def allif_search(vis, widths, strides, nfa):
+def allif_search(vis, widths, strides, nfa, delay_range=None):
     """f2 - VOLKS2's own fringe search, Eq. 1: ONE delay across all IFs,
         G(dtau) = sum_n sum_j S(n, j) e^{-i Phi},  Phi = 2 pi f_j^n dtau,
     evaluated with one zero-padded FFT over the whole band per AP ("32768 sized FFT"),
@@ -292,7 +292,12 @@ def allif_search(vis, widths, strides, nfa):
     (P1, idx1) first argmax, (P2, idx2) runner-up, S1 = sum_d P, snr = sqrt(P1/(S1/nfa)) (A3's statistic
     on the delay axis).  Evaluated as the rate-0 row of this oracle's own 2-D plane of the band window
     (pin P4 / PAPER.md:133, 143: summing per-AP spectra == spectrum of the sum).
+    delay_range = (lo, hi): the maximum is looked for in the delay bins lo..hi of the nfa axis only (wrapping when
+    lo > hi), the noise S1 stays the sum over the whole axis.
     Output order: canonical (bl, q, j); PEAK_DTYPE records."""
+    lo, hi = _range(delay_range)
+    dd = np.arange(nfa)
+    allowed = np.ones(nfa, bool) if lo < 0 else ((dd >= lo) & (dd <= hi) if lo <= hi else (dd >= lo) | (dd <= hi))
     band = allif_band(vis)
     nbl, nap, nm = band.shape
     out = []
@@ -304,14 +309,15 @@ def allif_search(vis, widths, strides, nfa):
             for j in range(nwin(nap, int(w), int(s))):
                 _, plane = window(band[b, j * s: j * s + w], nt, nfa, mode="fft", want_plane=True)
                 a = plane[0]
-                p = a.real * a.real + a.imag * a.imag
+                pall = a.real * a.real + a.imag * a.imag
+                p = np.where(allowed, pall, -1.0)        # bins outside the searched range cannot be the peak
                 i1 = int(np.argmax(p))
                 q = p.copy()
                 q[i1] = -1.0
                 i2 = int(np.argmax(q)) if nfa > 1 else i1
-                s1 = float(p.sum())
+                s1 = float(pall.sum())
                 noise = s1 / nfa
-                out.append((p[i1], q[i2] if nfa > 1 else 0.0, s1, np.sqrt(p[i1] / noise) if noise > 0 else 0.0, i1, i2))
+                out.append((p[i1], max(q[i2], 0.0) if nfa > 1 else 0.0, s1, np.sqrt(p[i1] / noise) if noise > 0 else 0.0, i1, i2))
     return np.array(out, dtype=PEAK_DTYPE) if out else np.zeros(0, dtype=PEAK_DTYPE)
 
 

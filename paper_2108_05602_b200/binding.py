@@ -33,7 +33,8 @@ class volks_params(ctypes.Structure):
 
 class volks_options(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in ("struct_bytes", "full_index", "force_generic", "slide_seg", "y_pad",
-                                              "chunk_mb", "cf_wpc", "cf2", "ai_waves", "host_split", "no_prune", "prune_seg")]
+                                              "chunk_mb", "cf_wpc", "cf2", "ai_waves", "host_split", "no_prune", "prune_seg",
+                                              "delay_lo", "delay_hi")]
 
 
 CAND_DTYPE = np.dtype([("bl", "<i4"), ("ifq", "<i4"), ("wid", "<i4"), ("win", "<i4"), ("t0", "<i4"),
@@ -110,7 +111,7 @@ def _check(rc):
 
 def make_options(**kw):
     """volks_options_init + keyword overrides (full_index, force_generic, slide_seg, y_pad, chunk_mb, cf_wpc, cf2,
-    ai_waves, host_split, no_prune, prune_seg)."""
+    ai_waves, host_split, no_prune, prune_seg, delay_lo, delay_hi)."""
     o = volks_options()
     lib().volks_options_init(ctypes.byref(o))
     for k, v in kw.items():

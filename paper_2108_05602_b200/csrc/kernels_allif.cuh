@@ -31,6 +31,8 @@ struct AllifArgs {
   const float *E;       // per-AP band energies [npairs_total][nap] (row kernel): detects energy collapse
   long long per_pair, offc, pair0;
   int nap, nf, w, stride, nwin, seg, nseg, pitch;
+  int dlo, dhi;         // restricted delay search range (true bins, wrapping when dlo > dhi; dlo < 0: whole axis): the
+                        // argmax looks at these bins only, the noise sum S1 runs over the whole axis
   int gsplit;           // nfa > 8192: nf = gsplit * 8192, column c of a row is sub-row rho = c / 8192, d' = c % 8192,
                         // delay d = gsplit d' + rho; one CTA per (baseline, segment, sub-row) (CP = 4);
                         // keys combine by atomicMax, the noise as gsplit partial sums added in order by the finalize
@@ -95,15 +97,18 @@ __global__ void __launch_bounds__(1024) k_allif(AllifArgs a) {
         const uint32_t dp = 2u * (uint32_t)(threadIdx.x + i * blockDim.x);
         const uint32_t d0 = SPLIT ? dp * (uint32_t)gs + (uint32_t)gpart : dp, d1 = d0 + (uint32_t)gs;
         const uint32_t p0 = __float_as_uint(lo32(pw)), p1 = __float_as_uint(hi32(pw));
-        if (p0 > pb || (p0 == pb && d0 < db)) { pb = p0; db = d0; }
-        if (p1 > pb || (p1 == pb && d1 < db)) { pb = p1; db = d1; }
+        const bool in0 = a.dlo < 0 || (a.dlo <= a.dhi ? ((int)d0 >= a.dlo && (int)d0 <= a.dhi) : ((int)d0 >= a.dlo || (int)d0 <= a.dhi));
+        const bool in1 = a.dlo < 0 || (a.dlo <= a.dhi ? ((int)d1 >= a.dlo && (int)d1 <= a.dhi) : ((int)d1 >= a.dlo || (int)d1 <= a.dhi));
+        if (in0 && (p0 > pb || (p0 == pb && d0 < db))) { pb = p0; db = d0; }
+        if (in1 && (p1 > pb || (p1 == pb && d1 < db))) { pb = p1; db = d1; }
         ps += lo32(pw) + hi32(pw);
       }
       const uint32_t km = __reduce_max_sync(0xffffffffu, pb);
       const uint32_t dm = __reduce_min_sync(0xffffffffu, pb == km ? db : 0xFFFFFFFFu);
 #pragma unroll
       for (int o = 16; o >= 1; o >>= 1) ps += __shfl_xor_sync(0xffffffffu, ps, o);
-      if (lane == 0) { kslot[b][warp] = make_key(__uint_as_float(km), dm); sslot[b][warp] = ps; }
+      // (a warp none of whose columns lies in the range: dm = 2^32 - 1, the lowest key there is: it never wins)
+      if (lane == 0) { kslot[b][warp] = dm == 0xFFFFFFFFu ? 0ull : make_key(__uint_as_float(km), dm); sslot[b][warp] = ps; }
       // next window
       if (slide && j + 1 < j1) {
         const int t0 = j * a.stride;

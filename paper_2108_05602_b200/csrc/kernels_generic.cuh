@@ -48,7 +48,16 @@ struct RowArgs {
   // cal[pair * nchan + k] (all-IF mode: pair = bl, k = n * nchan_src + j - the same memory layout
   // cf32[nbl][nif][nchan]); nullptr = none
   const float2 *cal;
+  // restricted delay search range (volks_options.delay_lo / delay_hi): the delay spectra of the bins
+  // outside dlo..dhi (wrapping when dlo > dhi) are written as ZERO, so that no rate kernel can find a peak there, while
+  // the noise statistic (the per-AP energies, from the input side) is untouched.  dlo < 0: the whole axis.
+  int dlo, dhi;
 };
+
+// delay bin d inside the searched range?
+__device__ __forceinline__ bool delay_ok(int d, int dlo, int dhi) {
+  return dlo < 0 || (dlo <= dhi ? (d >= dlo && d <= dhi) : (d >= dlo || d <= dhi));
+}
 
 // index of a row's per-AP energy: every row when psub == 1, else only the rho == 0 sub-row (-1 = none)
 __device__ __forceinline__ long long e_index(const RowArgs &a, long long row) {
@@ -246,7 +255,9 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
     float2 *dst = a.Y + rrel * (long long)a.pitch;
     if (a.paired) {
       for (int c = lane; c < (nf >> 1); c += tpr) {
-        const float2 v0 = in[2 * c], v1 = in[2 * c + 1];
+        float2 v0 = in[2 * c], v1 = in[2 * c + 1];
+        if (!delay_ok(2 * c, a.dlo, a.dhi)) v0 = make_float2(0.f, 0.f);
+        if (!delay_ok(2 * c + 1, a.dlo, a.dhi)) v1 = make_float2(0.f, 0.f);
         ((float4 *)dst)[c] = make_float4(v0.x, v1.x, v0.y, v1.y);
         const u64 k0 = make_key(cnorm(v0), (uint32_t)(2 * c)), k1 = make_key(cnorm(v1), (uint32_t)(2 * c + 1));
         key = k0 > key ? k0 : key;
@@ -254,7 +265,7 @@ __global__ void __launch_bounds__(512) k_row_fft(RowArgs a) {
       }
     } else {
       for (int k = lane; k < nf; k += tpr) {
-        const float2 v = in[k];
+        const float2 v = delay_ok(k, a.dlo, a.dhi) ? in[k] : make_float2(0.f, 0.f);
         dst[k] = v;
         const u64 kk = make_key(cnorm(v), (uint32_t)k);
         key = kk > key ? kk : key;
@@ -340,7 +351,8 @@ __global__ void __launch_bounds__(256) k_row2(RowArgs a) {
 #pragma unroll
   for (int i = 0; i < N1; ++i) {
     const int col = N2 * brev<N1>(i) + l;
-    const float re = lo32(v[i]), im = hi32(v[i]);
+    const bool inr = delay_ok(col, a.dlo, a.dhi);
+    const float re = inr ? lo32(v[i]) : 0.f, im = inr ? hi32(v[i]) : 0.f;
     const float got = __shfl_xor_sync(0xffffffffu, (l & 1) ? re : im, 1);
     if (live) {
       float *p = dst + ((col >> 1) << 2) + ((l & 1) << 1);
@@ -464,7 +476,9 @@ __global__ void __launch_bounds__(256) k_row3(RowArgs a) {
   u64 key = 0;
   float4 *dst = (float4 *)(a.Y + rrel * (long long)a.pitch);
   for (int c = tid; c < NF / 2; c += 256) {
-    const float4 q = ((const float4 *)img)[c ^ ((c >> 3) & 7)];
+    float4 q = ((const float4 *)img)[c ^ ((c >> 3) & 7)];
+    if (!delay_ok(2 * c, a.dlo, a.dhi)) { q.x = 0.f; q.z = 0.f; }
+    if (!delay_ok(2 * c + 1, a.dlo, a.dhi)) { q.y = 0.f; q.w = 0.f; }
     dst[c] = q;
     const u64 k0 = make_key(fmaf(q.x, q.x, q.z * q.z), (uint32_t)(2 * c)), k1 = make_key(fmaf(q.y, q.y, q.w * q.w), (uint32_t)(2 * c + 1));
     key = k0 > key ? k0 : key;
@@ -563,8 +577,11 @@ __global__ void __launch_bounds__(NF / 16, 2) k_rowbig(RowArgs a) {
   // ---- store: pair-interleaved float4 rows, the w = 1 peak
   u64 key = 0;
   float4 *dst = (float4 *)(a.Y + rrel * (long long)a.pitch);
-  auto emit = [&](int c, f32x2 z0, f32x2 z1) {   // columns 2c, 2c + 1
-    const float4 q = make_float4(lo32(z0), lo32(z1), hi32(z0), hi32(z1));
+  const int psub = a.psub, srho = src.rho;
+  auto emit = [&](int c, f32x2 z0, f32x2 z1) {   // columns 2c, 2c + 1 (true delay bin of column d': psub d' + rho)
+    float4 q = make_float4(lo32(z0), lo32(z1), hi32(z0), hi32(z1));
+    if (!delay_ok(2 * c * psub + srho, a.dlo, a.dhi)) { q.x = 0.f; q.z = 0.f; }
+    if (!delay_ok((2 * c + 1) * psub + srho, a.dlo, a.dhi)) { q.y = 0.f; q.w = 0.f; }
     dst[c] = q;
     if (a.keys1) {   // uniform
       const u64 k0 = make_key(fmaf(q.x, q.x, q.z * q.z), (uint32_t)(2 * c)), k1 = make_key(fmaf(q.y, q.y, q.w * q.w), (uint32_t)(2 * c + 1));
@@ -689,6 +706,7 @@ struct Sched {   // the window schedule (device copy lives in the plan)
   int allif;              // f2: one delay across all IFs (pairs = baselines; records carry ifq = -1)
   int ngs;                // f2: partial noise sums per window (k_allif's gsplit), 1 otherwise
   float snr_thresh;
+  int dlo, dhi, dfirst;   // restricted delay range (dlo < 0: none); dfirst = the lowest searched delay bin
   long long per_pair, nwin_total;
   int width[16], stride[16], nt[16];
   long long nwin[16];     // windows per pair
@@ -728,7 +746,9 @@ __device__ __forceinline__ WinStat window_stat(const Sched &s, const u64 *keys, 
   // an all-zero window (flagged data, the zero fill of dedispersion) has an identically zero plane:
   // P1 = 0 at (0, 0) by the tie rule.  The sliding sum would leave rounding residue of earlier samples
   // here, so the exact statement is made from the energy (es == 0 iff every sample is zero).
-  if (es == 0.f) { o.power = 0.f; o.rate_idx = 0; o.delay_idx = 0; }
+  // (with a restricted delay range the first searched bin is (0, dfirst); a plane whose searched bins are all zero
+  //  reports it too)
+  if (es == 0.f || o.power == 0.f) { o.power = 0.f; o.rate_idx = 0; o.delay_idx = s.dfirst; }
   if (zst) {
     const double2 ms = zst[o.pair * s.nwidths + q];
     o.snr = (float)(((double)o.power - ms.x) * ms.y);

@@ -299,6 +299,7 @@ void volks_options_init(volks_options *o) {
   o->struct_bytes = (int32_t)sizeof(volks_options);
   o->slide_seg = 256; o->y_pad = 16; o->chunk_mb = 4096; o->cf_wpc = 128; o->cf2 = 2; o->ai_waves = 2; o->host_split = 4;
   o->prune_seg = 64;
+  o->delay_lo = 0; o->delay_hi = -1;      // the whole delay axis
 }
 
 int volks_plan_create(const volks_params *p, volks_plan **out) { return plan_create_impl(p, nullptr, out, 0, 0); }
@@ -333,6 +334,9 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
         (opt.cf2 != 0 && opt.cf2 != 1 && opt.cf2 != 2 && opt.cf2 != 4) || opt.ai_waves < 1 || opt.host_split < 1 ||
         opt.prune_seg < 16 || opt.prune_seg > 4096 || !is_pow2(opt.prune_seg))
       return VOLKS_EINVAL;
+    // a restricted delay range is given in bins of the padded delay axis the caller asked for (nf, or nfa for f2)
+    if (opt.delay_hi >= 0 && (opt.delay_lo < 0 || opt.delay_lo >= p->nf * psub || opt.delay_hi >= p->nf * psub)) return VOLKS_EINVAL;
+    if (opt.delay_hi < -1) return VOLKS_EINVAL;
   }
   const bool allif = ai_nif > 0;
   if (p->nbl < 1 || p->nif < 1 || p->nap < 0 || p->nchan < 1) return VOLKS_EINVAL;
@@ -349,6 +353,10 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
   memset(&s, 0, sizeof s);
   s.nwidths = p->nwidths; s.nbl = p->nbl; s.nif = p->nif; s.nap = p->nap; s.nf = p->nf * psub;
   s.log2nf = ilog2(s.nf); s.snr_thresh = p->snr_thresh;
+  if (opt.delay_hi >= 0 && !(opt.delay_lo == 0 && opt.delay_hi == s.nf - 1)) {
+    s.dlo = opt.delay_lo; s.dhi = opt.delay_hi;
+    s.dfirst = s.dlo <= s.dhi ? s.dlo : 0;       // a wrapping range contains bin 0
+  } else { s.dlo = -1; s.dhi = -1; s.dfirst = 0; }
   pl->ai_psub = psub; pl->row_nf = p->nf;
   pl->nchan = p->nchan;
   pl->npair = (long long)p->nbl * p->nif;
@@ -683,6 +691,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
     ra.psub = pl->ai_psub; ra.premod = pl->ai_psub > 1 ? pl->d_tables + pl->premod_off : nullptr;
     ra.nchan = pl->nchan; ra.nf = pl->row_nf; ra.tpr = pl->row_tpr; ra.rows_per_cta = pl->row_rows_per_cta; ra.pitch = pl->pitch; ra.paired = pl->paired;
     ra.cal = pl->d_cal;
+    ra.dlo = pl->ai_nif ? -1 : s.dlo; ra.dhi = pl->ai_nif ? -1 : s.dhi;   // (f2: k_allif masks its argmax; its noise needs every column)
     ra.shift = d_shift; ra.nif = s.nif; ra.allif_nif = pl->ai_nif; ra.allif_nchan = pl->ai_nchan;
     ra.keys1 = nullptr; ra.per_pair = s.per_pair; ra.nap = s.nap; ra.stride1 = 1; ra.nwin1 = 0;
     if (pl->wid1 >= 0) { ra.keys1 = keys + s.offc[pl->wid1]; ra.stride1 = s.stride[pl->wid1]; ra.nwin1 = (int)s.nwin[pl->wid1]; }
@@ -750,7 +759,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         aa.per_pair = s.per_pair; aa.offc = s.offc[q]; aa.pair0 = pair0;
         aa.nap = s.nap; aa.nf = s.nf; aa.w = w.w; aa.stride = w.s; aa.nwin = (int)w.nwin; aa.seg = w.seg;
         aa.nseg = w.nseg; aa.pitch = pl->pitch * pl->ai_psub;
-        aa.gsplit = s.ngs;
+        aa.gsplit = s.ngs; aa.dlo = s.dlo; aa.dhi = s.dhi;
         const int cols = s.nf / s.ngs;                               // columns per CTA
         const int thr = std::min(1024, cols / 2), cp = cols / 2 / thr;
         const unsigned blocks = (unsigned)(np * w.nseg * s.ngs);

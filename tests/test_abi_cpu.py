@@ -50,14 +50,15 @@ def test_options_defaults_and_validation_before_cuda(vb):
     before any CUDA call; nf above the row kernels' 8192 points is an explicit VOLKS_EINVAL."""
     o = vb.make_options()
     assert (o.struct_bytes, o.full_index, o.force_generic, o.slide_seg, o.y_pad, o.chunk_mb, o.cf_wpc, o.cf2, o.ai_waves,
-            o.host_split, o.no_prune, o.prune_seg) == (48, 0, 0, 256, 16, 4096, 128, 2, 2, 4, 0, 64)
+            o.host_split, o.no_prune, o.prune_seg, o.delay_lo, o.delay_hi) == (56, 0, 0, 256, 16, 4096, 128, 2, 2, 4, 0, 64, 0, -1)
     a = dict(nbl=1, nif=1, nap=512, nchan=32, widths=[8], strides=[1], nts=[16], nf=64, snr_thresh=6.0)
     for bad in (dict(slide_seg=8), dict(y_pad=3), dict(y_pad=-2), dict(chunk_mb=0), dict(cf2=3), dict(ai_waves=0),
-                dict(host_split=0), dict(cf_wpc=0), dict(prune_seg=48), dict(prune_seg=8)):
+                dict(host_split=0), dict(cf_wpc=0), dict(prune_seg=48), dict(prune_seg=8),
+                dict(delay_lo=0, delay_hi=64), dict(delay_lo=-1, delay_hi=3), dict(delay_lo=64, delay_hi=3), dict(delay_hi=-2)):
         rc, h = vb.plan_create_raw(options=bad, **a)
         assert rc == -1 and not h, bad
     o = vb.make_options()
-    o.struct_bytes = 36
+    o.struct_bytes = 48
     rc, h = vb.plan_create_raw(options=o, **a)
     assert rc == -1 and not h
     with pytest.raises(KeyError):

@@ -33,16 +33,18 @@ def make_plane_power(oracle, vis_np, c):
     return plane_power
 
 
-def run_both(vb, oracle, vis, c, thresh=None, mode="cached", options=None):
+def run_both(vb, oracle, vis, c, thresh=None, mode="cached", options=None, delay_range=None):
     thresh = c["snr_thresh"] if thresh is None else thresh
     nbl, nif, nap, nchan = vis.shape
+    if delay_range is not None:
+        options = dict(options or {}, delay_lo=delay_range[0], delay_hi=delay_range[1])
     cands, n, peaks = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], thresh,
                                        want_peaks=True, options=options)
     # the same search without the dense peak array: the stride-1 kernels may run in the candidates-only index
     # mode (volks_options.full_index = 0); the candidate list must be the same, bit for bit
     cands2, n2, _ = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], thresh, options=options)
     assert n2 == n and cands2.tobytes() == cands.tobytes()
-    ora, _ = oracle.search(vis.cpu().numpy(), c["widths"], c["strides"], c["nts"], c["nf"], mode=mode)
+    ora, _ = oracle.search(vis.cpu().numpy(), c["widths"], c["strides"], c["nts"], c["nf"], mode=mode, delay_range=delay_range)
     nw = [workloads.gen.nwin(nap, w, s) for w, s in zip(c["widths"], c["strides"])]
     di = dense_index(nbl, nif, nw)
     assert len(ora) == len(peaks) == len(di)
@@ -703,3 +705,47 @@ def test_pruning_keeps_every_candidate(vb, oracle, prune_seg):
     with pytest.raises(vb.VolksError):                 # the candidates-only search left no exact index for every window
         plan.zscore_select(ws, 3.0, cbuf, nc)
     plan.close()
+
+
+@pytest.mark.parametrize("cfg,over,ranges", [
+    (2, dict(nbl=1, nif=2, nap=500, npulses=3), [(250, 5), (3, 40), (100, 100), (64, 127), (1, 255)]),   # nf 256: sliding kernels, all widths
+    (3, dict(nbl=2, nif=1, nap=700, npulses=3), [(120, 7), (0, 63), (9, 9)]),                            # nf 128, incl. w = 1 (row kernel peaks)
+    (4, dict(nbl=1, nif=1, nap=400, npulses=1), [(2040, 7), (100, 1500)]),                               # nf 2048: k_row3 + k_colfft2
+    (1, dict(nap=500), [(120, 8), (5, 70)]),                                                             # stride > 1: k_colfft / k_col
+])
+def test_delay_range_restriction(vb, oracle, cfg, over, ranges):
+    """volks_options.delay_lo / delay_hi ("the delay search range ... is configured for projected baselines
+    shorter than 3000 km"): the peak is searched in the allowed delay bins only (wrapping ranges around zero delay, a
+    single bin, whole 64-column groups in and out), the noise statistic is the whole plane's; every window and the
+    candidate lists of both index modes against the oracle's restricted scan."""
+    vis, c, _ = workloads.generate(cfg, **over)
+    full = run_both(vb, oracle, vis, c)
+    for rg in ranges:
+        stats, ncand, cands, ora = run_both(vb, oracle, vis, c, delay_range=rg)
+        lo, hi = rg
+        d = cands["delay_idx"]
+        assert np.all((d >= lo) & (d <= hi) if lo <= hi else (d >= lo) | (d <= hi))
+        run_both(vb, oracle, vis, c, thresh=3.0, delay_range=rg)
+    # the whole axis given explicitly is the unrestricted search
+    same = run_both(vb, oracle, vis, c, delay_range=(0, c["nf"] - 1))
+    assert same[2].tobytes() == full[2].tobytes()
+
+
+def test_delay_range_allif(vb, oracle):
+    """The same restriction on f2 (the paper's own all-IF search): bins of the nfa axis, incl. nfa > 8192 (interleaved
+    sub-rows); the noise is still the mean over the whole delay axis."""
+    for (nbl, nif, nap, nchan, nfa, rg) in [(2, 4, 120, 64, 512, (500, 11)), (1, 8, 40, 1024, 32768, (32000, 700)), (1, 2, 90, 32, 128, (17, 17))]:
+        g = torch.Generator().manual_seed(nfa)
+        vis = torch.view_as_complex(torch.randn((nbl, nif, nap, nchan, 2), generator=g) * 0.7071)
+        widths, strides = [1, 4, 8], [1, 1, 3]
+        cands, n, peaks = vb.allif_search(vis.cuda(), widths, strides, nfa, 2.0, want_peaks=True,
+                                          options=dict(delay_lo=rg[0], delay_hi=rg[1]))
+        ora = oracle.allif_search(vis.numpy(), widths, strides, nfa, delay_range=rg)
+        nw = [workloads.gen.nwin(nap, w, s) for w, s in zip(widths, strides)]
+        pk = peaks[dense_index(nbl, 1, nw)]
+        lo, hi = rg
+        d = pk["delay_idx"]
+        assert np.all((d >= lo) | (d <= hi) if lo > hi else (d >= lo) & (d <= hi))
+        band = oracle.allif_band(vis.numpy())
+        check_peaks(pk, ora, nfa, allif_plane_power(oracle, band, nw, widths, strides, nfa))
+        assert n == np.count_nonzero(ora["snr"] > 2.0) or np.any(np.abs(ora["snr"] - 2.0) <= 2e-4)

@@ -363,6 +363,21 @@ def test_delay_range_pins(oracle):
                     i += 1
     with pytest.raises(ValueError):
         oracle.window(win, nt, nf, delay_range=(0, nf))
+    # f2 (all-IF): the same masked argmax on the nfa axis against numpy.fft of the summed band, noise unchanged
+    v2 = (rng.normal(size=(1, 3, 20, 8)) + 1j * rng.normal(size=(1, 3, 20, 8))).astype(np.complex64)
+    band = v2.transpose(0, 2, 1, 3).reshape(1, 20, 24)
+    for rg in [(60, 3), (5, 30)]:
+        res = oracle.allif_search(v2, [1, 4], [1, 2], 64, delay_range=rg)
+        allowed = np.array([(d >= rg[0] or d <= rg[1]) if rg[0] > rg[1] else rg[0] <= d <= rg[1] for d in range(64)])
+        i = 0
+        for wq, sq in zip([1, 4], [1, 2]):
+            for j in range(oracle.nwin(20, wq, sq)):
+                P = np.abs(np.fft.fft(band[0, j * sq: j * sq + wq].astype(np.complex128).sum(axis=0), 64)) ** 2
+                Pm = np.where(allowed, P, -1.0)
+                assert res[i]["idx1"] == int(np.argmax(Pm)) and abs(res[i]["p1"] - Pm.max()) <= 1e-9 * Pm.max()
+                assert abs(res[i]["s1"] - P.sum()) <= 1e-9 * P.sum()
+                i += 1
+    assert np.array_equal(oracle.allif_search(v2, [4], [2], 64, delay_range=(0, 63)), oracle.allif_search(v2, [4], [2], 64))
 
 
 def test_baseline_match_constructions(oracle):
