@@ -33,6 +33,7 @@ struct PruneArgs {
   unsigned char *flags;   // [pairs of the chunk][nq][nseg]
   long long per_pair;
   int nap, nf, pitch, nq, seg, nseg, wmax, ring;
+  int ncp, cp_na, cp_a0, cp_b0;   // column pairs to look at (restricted delay range): pair i < cp_na is cp_a0 + i, else cp_b0 + i - cp_na
   int w[PRUNE_MAXQ], nwin[PRUNE_MAXQ];
   long long offc[PRUNE_MAXQ];
 };
@@ -74,7 +75,8 @@ __global__ void __launch_bounds__(PRUNE_THREADS) k_bound(PruneArgs a) {
   }
   __syncthreads();
   unsigned hit = 0;                                          // bit 2 q + half
-  for (int c = threadIdx.x; c < (a.nf >> 1); c += nthr) {
+  for (int ci = threadIdx.x; ci < a.ncp; ci += nthr) {
+    const int c = ci < a.cp_na ? a.cp_a0 + ci : a.cp_b0 + (ci - a.cp_na);
     for (int k = 0; k < a.ring; ++k) *(f32x2 *)(ring + (uint32_t)k * rstride) = pk(0.f, 0.f);
     const char *p = ybase + (size_t)R0 * rowb + (size_t)c * 16u;
     f32x2 bx[4], by[4];                                      // four rows in flight

@@ -54,6 +54,9 @@ struct SlideArgs {
   long long pair0;      // first pair of the chunk
   int nap, nf, w, nt, log2m, nwin, seg, nseg, pitch;
   uint32_t keymask;     // 0xFFFFFFF0, passed as data so that (p & mask) | id is ONE LOP3 (register mask)
+  // restricted delay range: only the 64-column groups that hold searched bins are worked on.  ndt groups in two
+  // pieces: group i < dt_na is column group dt_a0 + i, the others dt_b0 + (i - dt_na) (whole axis: ndt = nf / 64)
+  int ndt, dt_na, dt_a0, dt_b0;
   // pruned widths (kernels_prune.cuh): flags[pl * flag_stride + segment] == 0 means no window of the segment can be
   // a candidate - the CTA returns at once; nullptr = every segment is evaluated
   const unsigned char *flags;
@@ -313,11 +316,12 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   long long wt = (long long)blockIdx.x * nwarps + warp;
   const uint32_t lane = threadIdx.x & 31u;
   const int M = 1 << a.log2m;
-  const int ndt = a.nf >> 6;                      // 64 columns per warp
+  const int ndt = a.ndt;                          // 64 columns per warp; the groups with searched delay bins
   SlideState<L> S;
   S.lane = lane;
   S.rho = (uint32_t)(wt & (M - 1)); wt >>= a.log2m;
-  const int dt = (int)(wt % ndt); wt /= ndt;
+  const int dti = (int)(wt % ndt); wt /= ndt;
+  const int dt = dti < a.dt_na ? a.dt_a0 + dti : a.dt_b0 + (dti - a.dt_na);
   const int sg = (int)(wt % a.nseg);
   const long long pl = wt / a.nseg;
   if (a.flags && !a.flags[pl * a.flag_stride + sg]) return;   // the whole CTA shares (pair, segment)
@@ -340,7 +344,8 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   if constexpr (RING) {
     // the CTA's warps are (rho fastest, then dt): its first warp's dt is the first column group
     const long long wt0 = ((long long)blockIdx.x * nwarps) >> a.log2m;
-    const int dt0 = (int)(wt0 % ndt);
+    const int dti0 = (int)(wt0 % ndt);              // (the pieces are multiples of the CTA's groups: contiguous columns)
+    const int dt0 = dti0 < a.dt_na ? a.dt_a0 + dti0 : a.dt_b0 + (dti0 - a.dt_na);
     const int dtc = nwarps >> a.log2m > 0 ? nwarps >> a.log2m : 1;    // column groups per CTA
     G.base = (uint32_t)__cvta_generic_to_shared(slide_ring);
     G.rrowb = 512u * (uint32_t)dtc;

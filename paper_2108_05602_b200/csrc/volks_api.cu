@@ -187,8 +187,9 @@ static bool launch_row2(const RowArgs &a, cudaStream_t st) {
 
 static void launch_slide(const SlideArgs &a, cudaStream_t st) {
   // every warp of a CTA must share its (pair, segment): warps per CTA = min(SLIDE_WARPS, ndt * M)
-  const long long per_seg = (long long)(a.nf / 64) << a.log2m;
-  const int wpb = (int)std::min<long long>(SLIDE_WARPS, per_seg);
+  const long long per_seg = (long long)a.ndt << a.log2m;
+  int wpb = SLIDE_WARPS;                         // the largest power of two <= 8 that divides the warps of a segment
+  while (per_seg % wpb) wpb >>= 1;
   const unsigned blocks = (unsigned)(a.ntasks / wpb);
   const int thr = wpb * 32;
   if (a.nt >= 32) {
@@ -233,6 +234,7 @@ struct volks_plan {
   int nuntag = 0;                // sliding widths with untagged kernels (their peak bins come from k_recover)
   bool cand_only = false;        // searches without d_peaks recover indices / evaluate segments for possible candidates only
   int nprune = 0, prune_nseg = 0, prune_seg = 0, prune_wmax = 0;   // pruned widths (k_bound): count, common segmentation
+  int dt_n = 0, dt_na = 0, dt_a0 = 0, dt_b0 = 0;   // 64-column groups the sliding kernels / k_bound work on (restricted delay range)
   size_t off_flags = 0;          // their segment flags [pairs_per_chunk][nprune][prune_nseg]
   size_t off_thr = 0;            // their windows' pre-thresholds (k_winthr), chunk-relative
   mutable bool last_full_index = true;   // the most recent search left exact indices for EVERY window (volks_zscore_select)
@@ -357,6 +359,22 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
     s.dlo = opt.delay_lo; s.dhi = opt.delay_hi;
     s.dfirst = s.dlo <= s.dhi ? s.dlo : 0;       // a wrapping range contains bin 0
   } else { s.dlo = -1; s.dhi = -1; s.dfirst = 0; }
+  {
+    // 64-column groups that hold searched bins, as at most two pieces (a wrapping range: the low bins, then the high
+    // ones), each widened to an even group boundary so that the two-group CTAs of k_slide read contiguous columns
+    const int ng = std::max(1, s.nf / 64);
+    pl->dt_n = ng; pl->dt_na = ng; pl->dt_a0 = 0; pl->dt_b0 = 0;
+    if (s.dlo >= 0 && ng >= 2 && !allif) {
+      auto lo2 = [](int g) { return g & ~1; };
+      auto hi2 = [&](int g) { return std::min(ng, (g + 2) & ~1); };     // exclusive, even
+      if (s.dlo <= s.dhi) { pl->dt_a0 = lo2(s.dlo / 64); pl->dt_na = hi2(s.dhi / 64) - pl->dt_a0; pl->dt_n = pl->dt_na; }
+      else {
+        const int a1 = hi2(s.dhi / 64), b0 = lo2(s.dlo / 64);            // [0, a1) and [b0, ng)
+        if (a1 >= b0) { pl->dt_a0 = 0; pl->dt_na = ng; pl->dt_n = ng; }
+        else { pl->dt_a0 = 0; pl->dt_na = a1; pl->dt_b0 = b0; pl->dt_n = a1 + (ng - b0); }
+      }
+    }
+  }
   pl->ai_psub = psub; pl->row_nf = p->nf;
   pl->nchan = p->nchan;
   pl->npair = (long long)p->nbl * p->nif;
@@ -722,12 +740,13 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         pa.Y = Y; pa.thr = ta.thr; pa.flags = (unsigned char *)(ws + pl->off_flags); pa.per_pair = s.per_pair;
         pa.nap = s.nap; pa.nf = s.nf; pa.pitch = pl->pitch; pa.nq = pl->nprune; pa.seg = pl->prune_seg;
         pa.nseg = pl->prune_nseg; pa.wmax = pl->prune_wmax;
+        pa.ncp = pl->dt_n * 32; pa.cp_na = pl->dt_na * 32; pa.cp_a0 = pl->dt_a0 * 32; pa.cp_b0 = pl->dt_b0 * 32;
         for (int q = 0; q < s.nwidths; ++q) {
           const WidthPlan &w = pl->wp[q];
           if (w.prune < 0) continue;
           pa.w[w.prune] = w.w; pa.nwin[w.prune] = (int)w.nwin; pa.offc[w.prune] = s.offc[q];
         }
-        const int T = 2 * pa.seg, thr = std::min(PRUNE_THREADS, s.nf / 2);
+        const int T = 2 * pa.seg, thr = std::min(PRUNE_THREADS, s.nf / 2);   // (nf >= 64: a power of two >= 32)
         pa.ring = pa.wmax <= 16 ? 16 : 32;                 // rows of amplitude history (a power of two >= wmax)
         const size_t smem = (size_t)((pa.nq * (T + 64) + 3) & ~3) * sizeof(float) + (size_t)pa.ring * thr * sizeof(f32x2);
         const unsigned blocks = (unsigned)(np * ((pa.nseg + 1) / 2));
@@ -776,7 +795,8 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         sa.per_pair = s.per_pair; sa.offc = s.offc[q]; sa.pair0 = pair0;
         sa.nap = s.nap; sa.nf = s.nf; sa.w = w.w; sa.nt = w.nt; sa.log2m = w.log2m; sa.nwin = (int)w.nwin;
         sa.seg = w.seg; sa.nseg = w.nseg; sa.keymask = 0xFFFFFFF0u; sa.pitch = pl->pitch;
-        sa.ntasks = ((np * w.nseg * (long long)(s.nf / 64)) << w.log2m);
+        sa.ndt = pl->dt_n; sa.dt_na = pl->dt_na; sa.dt_a0 = pl->dt_a0; sa.dt_b0 = pl->dt_b0;
+        sa.ntasks = ((np * w.nseg * (long long)pl->dt_n) << w.log2m);
         sa.flags = flags && w.prune >= 0 ? flags + (size_t)w.prune * pl->prune_nseg : nullptr;
         sa.flag_stride = pl->nprune * pl->prune_nseg;
         ProfScope ps(pl, st, VOLKS_K_SLIDE, q);
