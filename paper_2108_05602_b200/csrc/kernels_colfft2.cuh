@@ -201,22 +201,22 @@ __global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : CP == 4 ? 2
         Y[k] = fma2(zx2, wy, mul2(zy2, wx));
       }
       FftDifS<16, 16, 0, 16>::run(X, Y);
+      // untagged maximum (as k_slide for w >= 16): power and the delay column; the rate bin among the 16 of (rho, column)
+      // is k_recover's exact re-evaluation (key = power bits, 2^31 | plane index of the column's bin s = 0)
       uint32_t ba = 0, bb = 0;
 #pragma unroll
       for (int i = 0; i < 16; ++i) {
         const f32x2 pw = fma2(Y[i], Y[i], mul2(X[i], X[i]));
-        ba = max(ba, (__float_as_uint(lo32(pw)) & a.keymask) | (uint32_t)(15 - brev<16>(i)));
-        bb = max(bb, (__float_as_uint(hi32(pw)) & a.keymask) | (uint32_t)(15 - brev<16>(i)));
+        ba = max(ba, __float_as_uint(lo32(pw)));
+        bb = max(bb, __float_as_uint(hi32(pw)));
       }
       const bool colb = bb > ba;
       const uint32_t best = colb ? bb : ba;
       const uint32_t km = __reduce_max_sync(0xffffffffu, best);
       const uint32_t tied = __ballot_sync(0xffffffffu, best == km);
-      if (lane == __ffs(tied) - 1) {
-        const uint32_t s = 15u - (km & 15u);
-        slots[warp] = make_key(__uint_as_float(km & 0xFFFFFFF0u),
-                               (rho + (uint32_t)L1 * s) * (uint32_t)a.nf + (uint32_t)(tile * 2 * CP + 2 * cp) + (colb ? 1u : 0u));
-      }
+      if (lane == __ffs(tied) - 1)
+        slots[warp] = ((u64)km << 32) |
+                      (u64)(0xFFFFFFFFu - (0x80000000u | (rho * (uint32_t)a.nf + (uint32_t)(tile * 2 * CP + 2 * cp) + (colb ? 1u : 0u))));
     }
     half_barrier();
     if (warp == hb) {   // warps 0 and 1: the slots of their parity

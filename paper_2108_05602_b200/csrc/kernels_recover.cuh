@@ -1,6 +1,6 @@
 // kernels_recover.cuh - the peak bin of the stride-1 windows whose sliding kernel ran without bin tags.
 //
-// k_slide (w >= 16) leaves per window the maximum power and the COLUMN it came from: one rate residue rho and one
+// k_slide (w >= 16) and k_colfft2 (Nt = 256, 512) leave per window the maximum power and the COLUMN it came from: one rate residue rho and one
 // delay column d, i.e. the 16 rate bins r = rho + M s of that column.  Which of them is the peak is decided here:
 //   k_recover   one thread per (pair, width, window).  The thread leaves at once unless the window needs its index:
 //               every window in the full-index mode (dense peaks, volks_zscore_select), otherwise the windows whose
@@ -27,7 +27,7 @@ struct RecoverArgs {
   const float2 *tables;   // plan tables; rate twiddles of width i at tables + tw_off[i]
   long long per_pair, pair0, total;   // total = pairs of the chunk * cum[nq]
   int nap, nf, log2nf, pitch, nq;
-  int w[16], nt[16], log2m[16], nwin[16];
+  int w[16], stride[16], nt[16], log2m[16], nwin[16];
   long long offc[16], tw_off[16], cum[17];   // cum: prefix sums of nwin (windows per pair of the listed widths)
 };
 
@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(128) k_recover(RecoverArgs a) {
   const int w = a.w[i], ntm = a.nt[i] - 1;
   const float2 *twt = a.tables + a.tw_off[i];
   // element d of a pair-interleaved row: float index 4 (d / 2) + (d & 1), imaginary part 2 floats on
-  const float *p = (const float *)(a.Y + ((size_t)pl * a.nap + (size_t)j) * a.pitch) + ((d >> 1) << 2) + (d & 1);   // stride 1: t0 = j
+  const float *p = (const float *)(a.Y + ((size_t)pl * a.nap + (size_t)j * a.stride[i]) * a.pitch) + ((d >> 1) << 2) + (d & 1);   // t0 = j * stride
   const size_t rowf = (size_t)a.pitch * 2u;
   float2 f[16];
 #pragma unroll

@@ -409,7 +409,7 @@ struct WinThrArgs {
   long long per_pair, pair0, total;   // total = pairs of the chunk * windows of the sliding widths per pair
   float thr2;            // snr_thresh^2
   int nap, nq;
-  int w[16], nwin[16];
+  int w[16], stride[16], nwin[16];
   long long offc[16], cum[17];        // cum: prefix sums of nwin over the listed widths
 };
 
@@ -422,7 +422,7 @@ __global__ void __launch_bounds__(256) k_winthr(WinThrArgs a) {
   int i = 0;
   while (r >= a.cum[i + 1]) ++i;
   const int j = (int)(r - a.cum[i]);
-  const float *e = a.E + (a.pair0 + pl) * a.nap + j;
+  const float *e = a.E + (a.pair0 + pl) * a.nap + (long long)j * a.stride[i];   // t0 = j * stride
   float es = 0.f;
   for (int t = 0; t < a.w[i]; ++t) es += e[t];
   a.thr[pl * a.per_pair + a.offc[i] + j] = __float_as_uint(SLIDE_PRE * a.thr2 * es);

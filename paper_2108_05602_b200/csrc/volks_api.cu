@@ -399,7 +399,7 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
     w.slide = !force_generic && w.s == 1 && w.w >= 2 && w.nt == 2 * w.w && p->nf >= 64 &&
               ((long long)p->nap + SLIDE_PF + 2) * (p->nf + 64) * 8 < (1LL << 32);
     if (allif) w.slide = false;
-    w.untag = w.slide && w.nt >= 32;
+    w.untag = w.slide && w.nt >= 32;     // (+ the k_colfft2 widths, set below once colfft is known)
     w.colfft = !allif && !force_generic && !w.slide && w.nt >= 32 && w.nt <= 512 && p->nf >= 32 && w.nwin > 0;
     // exact pruning by the amplitude-sum bound (kernels_prune.cuh): narrow widths whose noise-only bound stays
     // >= 4.5 deviations below the threshold, (0.99 snr_thresh - 0.886 sqrt(w)) / 0.4637 (Rayleigh amplitudes)
@@ -408,6 +408,7 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
         p->nap >= w.w && (0.99 * p->snr_thresh - 0.886 * sqrt((double)w.w)) / 0.4637 >= 4.5 && w.nt <= opt.prune_seg)
       w.prune = pl->nprune++;
     w.cf_l1 = w.nt / 16;
+    if (w.colfft && w.nt >= 256 && opt.cf2 != 0) w.untag = true;   // k_colfft2 keeps no bin tags either
     w.cf_nz = 1;
     while (w.cf_nz * 16 < w.w) w.cf_nz *= 2;
     // windows per CTA: up to 128 (L1 reuse of overlapping windows), fewer when the grid would not fill 148 SMs x 4
@@ -486,7 +487,7 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
           (w.colfft && cf_blocks > GMAX) || (allif && ai_blocks > GMAX)) fits = false;
     }
     long long rec_warps = 0;
-    for (auto &w : pl->wp) rec_warps += (w.slide && w.nt >= 32) ? w.nwin : 0;
+    for (auto &w : pl->wp) rec_warps += w.untag ? w.nwin : 0;
     if ((long double)ppc_ * rec_warps / 128 > GMAX) fits = false;    // k_recover: one thread per window
     if (!fits) { delete pl; return VOLKS_EINVAL; }
   }
@@ -728,7 +729,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         const WidthPlan &w = pl->wp[q];
         if ((!w.untag && w.prune < 0) || w.nwin == 0) continue;
         const int i = ta.nq++;
-        ta.w[i] = w.w; ta.nwin[i] = (int)w.nwin; ta.offc[i] = s.offc[q]; ta.cum[i + 1] = ta.cum[i] + w.nwin;
+        ta.w[i] = w.w; ta.stride[i] = w.s; ta.nwin[i] = (int)w.nwin; ta.offc[i] = s.offc[q]; ta.cum[i + 1] = ta.cum[i] + w.nwin;
       }
       ta.total = np * ta.cum[ta.nq];
       {
@@ -850,7 +851,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         const WidthPlan &w = pl->wp[q];
         if (!w.untag || w.nwin == 0) continue;
         const int i = ra2.nq++;
-        ra2.w[i] = w.w; ra2.nt[i] = w.nt; ra2.log2m[i] = w.log2m; ra2.nwin[i] = (int)w.nwin; ra2.offc[i] = s.offc[q];
+        ra2.w[i] = w.w; ra2.stride[i] = w.s; ra2.nt[i] = w.nt; ra2.log2m[i] = w.log2m; ra2.nwin[i] = (int)w.nwin; ra2.offc[i] = s.offc[q];
         ra2.tw_off[i] = (long long)w.tw_off; ra2.cum[i + 1] = ra2.cum[i] + w.nwin;
       }
       ra2.total = np * ra2.cum[ra2.nq];
