@@ -32,6 +32,10 @@ struct FixArgs {
   const unsigned char *flags;   // [pairs of the chunk][flag_nq][flag_nseg] or nullptr
   int flag_q[16];               // index of sliding width i among the pruned widths, or -1
   int flag_nq, flag_nseg;
+  // the column-level width (kernels_coleval.cuh) in the candidates-only mode: its sliding kernel ran only on the tiles
+  // k_bound marked dense: cwdense[pl * cw_ntile + segment] (its segments are those tiles); cw_i = its index here or -1
+  const unsigned char *cwdense;
+  int cw_i, cw_ntile;
 };
 
 // peak key of rate residue rho, column d of the window starting at row0 (already includes pair and t0)
@@ -73,6 +77,7 @@ __global__ void __launch_bounds__(256) k_fixup(FixArgs a) {
   const int sg_lo = (u - a.unit0[i]) * FIX_GROUP, sg_hi = min(a.nseg[i], sg_lo + FIX_GROUP);
   for (int sg = sg_lo; sg < sg_hi; ++sg) {
   if (a.flags && a.flag_q[i] >= 0 && !a.flags[(pl * a.flag_nq + a.flag_q[i]) * a.flag_nseg + sg]) continue;
+  if (a.cwdense && i == a.cw_i && !a.cwdense[pl * a.cw_ntile + sg]) continue;
   const int w = a.w[i], nt = a.nt[i], seg = a.seg[i];
   const int j0 = sg * seg, n = min(seg, a.nwin[i] - j0);          // windows j0 .. j0+n-1 (seg <= 256? see below)
   u64 *keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc[i]);

@@ -36,9 +36,16 @@ struct PruneArgs {
   int ncp, cp_na, cp_a0, cp_b0;   // column pairs to look at (restricted delay range): pair i < cp_na is cp_a0 + i, else cp_b0 + i - cp_na
   int w[PRUNE_MAXQ], nwin[PRUNE_MAXQ];
   long long offc[PRUNE_MAXQ];
+  // column-level width (NCW = 1: the LAST listed width): besides its segment flags, one bit per (window, delay column):
+  // cwmask[(pl * cw_nwords + window / 32) * nf + column], zeroed before the launch (k_coleval, kernels_coleval.cuh)
+  uint32_t *cwmask;
+  int cw_nwords;
+  // ... and one byte per (pair, tile): 1 = more than 1/8 of the tile's (window, column) bits are set (interference,
+  // a strong source): the sliding kernel evaluates that tile (it is cheaper there), k_coleval skips it
+  unsigned char *cwdense;
 };
 
-template <int NQ>
+template <int NQ, int NCW>
 __global__ void __launch_bounds__(PRUNE_THREADS) k_bound(PruneArgs a) {
   extern __shared__ float prune_sm[];
   // shared: thr[NQ][TP] floats (TP = 2 seg + 64: 32 entries of +inf before and after the tile's windows, so that
@@ -46,6 +53,7 @@ __global__ void __launch_bounds__(PRUNE_THREADS) k_bound(PruneArgs a) {
   const int T = 2 * a.seg, TP = T + 64;
   float *thr_sm = prune_sm;
   __shared__ int any[PRUNE_MAXQ][2];
+  __shared__ int cwtotal;
   const int ntile = (a.nseg + 1) / 2;
   const long long pl = blockIdx.x / ntile;
   const int tile = (int)(blockIdx.x % ntile);
@@ -56,6 +64,8 @@ __global__ void __launch_bounds__(PRUNE_THREADS) k_bound(PruneArgs a) {
     thr_sm[i] = (j >= 0 && j < T && R0 + j < a.nwin[q]) ? __uint_as_float(__ldg(a.thr + pl * a.per_pair + a.offc[q] + R0 + j)) : 3.0e38f;
   }
   if (threadIdx.x < PRUNE_MAXQ * 2) any[threadIdx.x >> 1][threadIdx.x & 1] = 0;
+  if (threadIdx.x == 0) cwtotal = 0;
+  int cwcount = 0;
   const int nrows = min(T + a.wmax - 1, a.nap - R0);         // rows R0 .. R0 + nrows - 1 exist
   const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch);
   const size_t rowb = (size_t)a.pitch * 8u;
@@ -83,7 +93,7 @@ __global__ void __launch_bounds__(PRUNE_THREADS) k_bound(PruneArgs a) {
 #pragma unroll
     for (int u = 0; u < 4; ++u) { bx[u] = by[u] = pk(0.f, 0.f); if (u < nrows) ldg2(p + (size_t)u * rowb, bx[u], by[u]); }
     f32x2 C = pk(0.f, 0.f);
-    uint32_t roff = 0;
+    uint32_t roff = 0, cwa = 0, cwb = 0;
     for (int r0 = 0; r0 < nrows; r0 += 4) {
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
@@ -107,7 +117,23 @@ __global__ void __launch_bounds__(PRUNE_THREADS) k_bound(PruneArgs a) {
           for (int q = 0; q < NQ; ++q) {
             const f32x2 S = sub2(C, old[q]);
             const float m = fmaxf(lo32(S), hi32(S));
-            if (m * m > th[q]) hit |= (uint32_t)r >= rhalf[q] ? 2u << (2 * q) : 1u << (2 * q);
+            const bool h = m * m > th[q];
+            if (h) hit |= (uint32_t)r >= rhalf[q] ? 2u << (2 * q) : 1u << (2 * q);
+            if constexpr (NCW == 1) {
+              if (q == NQ - 1) {                             // the column-level width: a bit per (window, column pair)
+                const int j = r - a.w[q] + 1;
+                if (j >= 0 && j < T) {
+                  cwa |= (lo32(S) * lo32(S) > th[q] ? 1u : 0u) << (j & 31);
+                  cwb |= (hi32(S) * hi32(S) > th[q] ? 1u : 0u) << (j & 31);
+                  if ((j & 31) == 31 || r == nrows - 1) {
+                    cwcount += __popc(cwa) + __popc(cwb);
+                    if (cwa | cwb)
+                      *(uint2 *)(a.cwmask + ((size_t)pl * a.cw_nwords + ((R0 + j) >> 5)) * (size_t)a.nf + 2 * c) = make_uint2(cwa, cwb);
+                    cwa = 0; cwb = 0;
+                  }
+                }
+              }
+            }
           }
           *(f32x2 *)(ring + (roff & rmask)) = C;
           roff += rstride;
@@ -120,7 +146,14 @@ __global__ void __launch_bounds__(PRUNE_THREADS) k_bound(PruneArgs a) {
 #pragma unroll
     for (int h = 0; h < 2; ++h)
       if (__ballot_sync(0xffffffffu, (hit >> (2 * q + h)) & 1u) && (threadIdx.x & 31) == 0) any[q][h] = 1;
+  if constexpr (NCW == 1) {
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) cwcount += __shfl_xor_sync(0xffffffffu, cwcount, o);
+    if ((threadIdx.x & 31) == 0 && cwcount) atomicAdd(&cwtotal, cwcount);
+  }
   __syncthreads();
+  if (NCW == 1 && threadIdx.x == 0)
+    a.cwdense[pl * ntile + tile] = (unsigned char)((long long)cwtotal * 8 > (long long)T * 2 * a.ncp ? 1 : 0);
   if (threadIdx.x < NQ * 2) {
     const int q = threadIdx.x >> 1, h = threadIdx.x & 1, sg = 2 * tile + h;
     if (sg < a.nseg) a.flags[(pl * NQ + q) * a.nseg + sg] = (unsigned char)any[q][h];

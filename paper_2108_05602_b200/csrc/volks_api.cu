@@ -18,6 +18,7 @@
 #include "kernels_probe.cuh"
 #include "kernels_prune.cuh"
 #include "kernels_recover.cuh"
+#include "kernels_coleval.cuh"
 
 using namespace volks;
 
@@ -47,6 +48,7 @@ struct WidthPlan {
   int seg, nseg;        // sliding path: windows per exactly restarted segment, segments per pair
   bool untag;           // sliding path with M >= 2 (Nt >= 32): untagged kernel, peak bin by k_recover
   int prune;            // sliding path: index among the plan's pruned widths (kernels_prune.cuh), or -1
+  bool cw;              // sliding path: the plan's column-level width (kernels_coleval.cuh)
 };
 
 template <int L>
@@ -234,6 +236,8 @@ struct volks_plan {
   int nuntag = 0;                // sliding widths with untagged kernels (their peak bins come from k_recover)
   bool cand_only = false;        // searches without d_peaks recover indices / evaluate segments for possible candidates only
   int nprune = 0, prune_nseg = 0, prune_seg = 0, prune_wmax = 0;   // pruned widths (k_bound): count, common segmentation
+  int cwq = -1, cw_nwords = 0;   // the column-level width (index into wp) and the 32-window words of its bit mask per pair
+  size_t off_cwmask = 0, off_cwdense = 0;
   int dt_n = 0, dt_na = 0, dt_a0 = 0, dt_b0 = 0;   // 64-column groups the sliding kernels / k_bound work on (restricted delay range)
   size_t off_flags = 0;          // their segment flags [pairs_per_chunk][nprune][prune_nseg]
   size_t off_thr = 0;            // their windows' pre-thresholds (k_winthr), chunk-relative
@@ -404,9 +408,16 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
     // exact pruning by the amplitude-sum bound (kernels_prune.cuh): narrow widths whose noise-only bound stays
     // >= 4.5 deviations below the threshold, (0.99 snr_thresh - 0.886 sqrt(w)) / 0.4637 (Rayleigh amplitudes)
     w.prune = -1;
-    if (w.slide && !opt.full_index && !opt.no_prune && p->snr_thresh > 0.f && w.w <= PRUNE_RING && pl->nprune < PRUNE_MAXQ &&
+    if (w.slide && !opt.full_index && !opt.no_prune && p->snr_thresh > 0.f && w.w <= PRUNE_RING &&
+        pl->nprune + (pl->cwq >= 0 ? 1 : 0) < PRUNE_MAXQ &&
         p->nap >= w.w && (0.99 * p->snr_thresh - 0.886 * sqrt((double)w.w)) / 0.4637 >= 4.5 && w.nt <= opt.prune_seg)
       w.prune = pl->nprune++;
+    // column-level pruning (kernels_coleval.cuh) for ONE width whose bound is too weak for whole segments but leaves
+    // few delay columns per window: >= 1.5 deviations (<= 7 % of the columns pass on noise); w = 32 at snr_thresh 6
+    w.cw = false;
+    if (w.prune < 0 && pl->cwq < 0 && w.slide && w.nt >= 32 && !opt.full_index && !opt.no_prune && p->snr_thresh > 0.f &&
+        w.w <= PRUNE_RING && pl->nprune < PRUNE_MAXQ && p->nap >= w.w && w.nt <= 2 * PRUNE_RING && opt.prune_seg == 64 &&
+        (0.99 * p->snr_thresh - 0.886 * sqrt((double)w.w)) / 0.4637 >= 1.5) { w.cw = true; pl->cwq = q; }
     w.cf_l1 = w.nt / 16;
     if (w.colfft && w.nt >= 256 && opt.cf2 != 0) w.untag = true;   // k_colfft2 keeps no bin tags either
     w.cf_nz = 1;
@@ -417,6 +428,7 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
     w.cf_nrange = (int)((w.nwin + w.cf_wpc - 1) / w.cf_wpc);
     w.seg = std::max((seg_req / w.nt) * w.nt, w.nt);
     if (w.prune >= 0) w.seg = opt.prune_seg;      // one segmentation for every pruned width (a multiple of its Nt)
+    if (w.cw) w.seg = CE_TILE;                    // the column-level width: segments = k_coleval's / k_bound's tiles of 128
     // f2: one CTA per (baseline, segment): segments short enough to fill 148 SMs x 2, at most seg_req windows
     if (allif) w.seg = (int)std::max<long long>(16, std::min<long long>((seg_req / 16) * 16, (w.nwin * p->nbl / 296 + 15) / 16 * 16));
     w.nseg = w.nwin > 0 ? (int)((w.nwin + w.seg - 1) / w.seg) : 0;
@@ -503,11 +515,18 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
   pl->cand_only = !opt.full_index && p->snr_thresh > 0.f;
   for (auto &w : pl->wp) {
     pl->nuntag += (w.untag && w.nwin > 0) ? 1 : 0;
-    if (w.prune >= 0) { pl->prune_nseg = std::max(pl->prune_nseg, w.nseg); pl->prune_wmax = std::max(pl->prune_wmax, w.w); }
+    if (w.prune >= 0 || w.cw) {
+      pl->prune_nseg = std::max(pl->prune_nseg, (int)((w.nwin + opt.prune_seg - 1) / opt.prune_seg));
+      pl->prune_wmax = std::max(pl->prune_wmax, w.w);
+    }
   }
   pl->prune_seg = opt.prune_seg;
   pl->off_thr = off;  off = align_up(off + ((pl->cand_only && (pl->nuntag || pl->nprune)) ? (size_t)pl->pairs_per_chunk * per_pair * sizeof(uint32_t) : 0), 256);
-  pl->off_flags = off; off = align_up(off + (size_t)pl->pairs_per_chunk * pl->nprune * pl->prune_nseg, 256);
+  pl->off_flags = off; off = align_up(off + (size_t)pl->pairs_per_chunk * (pl->nprune + 1) * pl->prune_nseg, 256);
+  // the column-level width's bits: k_bound's tiles are 2 prune_seg windows, a multiple of 32
+  pl->cw_nwords = pl->cwq >= 0 ? (int)(((pl->prune_nseg + 1) / 2) * (2 * opt.prune_seg / 32)) : 0;
+  pl->off_cwdense = off; off = align_up(off + (size_t)pl->pairs_per_chunk * ((pl->prune_nseg + 1) / 2) + 1, 256);
+  pl->off_cwmask = off; off = align_up(off + (size_t)pl->pairs_per_chunk * pl->cw_nwords * p->nf * sizeof(uint32_t), 256);
   pl->off_Y = off;    off = align_up(off + (size_t)pl->pairs_per_chunk * std::max<size_t>(y_pair, 8) + (size_t)(SLIDE_PF + 2) * pl->pitch * sizeof(float2), 256);
   pl->ws_bytes = off;
 
@@ -721,7 +740,8 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         k_row_fft<<<(unsigned)rblocks, ra.tpr * ra.rows_per_cta, pl->row_smem, st>>>(ra);
       if (d_stage && !cuda_ok(cudaEventRecord(pl->ev_free[ch & 1], st))) return VOLKS_ECUDA;
     }
-    if (hy) {
+    const bool use_cw = pl->cwq >= 0 && pl->wp[pl->cwq].nwin > 0;   // (needs the pre-thresholds and k_bound in both index modes)
+    if (hy || use_cw) {
       WinThrArgs ta;
       ta.E = E; ta.thr = (uint32_t *)(ws + pl->off_thr); ta.per_pair = s.per_pair; ta.pair0 = pair0;
       ta.thr2 = s.snr_thresh * s.snr_thresh; ta.nap = s.nap; ta.nq = 0; ta.cum[0] = 0;
@@ -736,32 +756,40 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         ProfScope ps(pl, st, VOLKS_K_WINTHR, -1);
         k_winthr<<<(unsigned)((ta.total + 255) / 256), 256, 0, st>>>(ta);
       }
-      if (flags) {
+      if (flags || use_cw) {
         PruneArgs pa;
         pa.Y = Y; pa.thr = ta.thr; pa.flags = (unsigned char *)(ws + pl->off_flags); pa.per_pair = s.per_pair;
-        pa.nap = s.nap; pa.nf = s.nf; pa.pitch = pl->pitch; pa.nq = pl->nprune; pa.seg = pl->prune_seg;
-        pa.nseg = pl->prune_nseg; pa.wmax = pl->prune_wmax;
+        pa.nap = s.nap; pa.nf = s.nf; pa.pitch = pl->pitch; pa.seg = pl->prune_seg;
+        pa.nseg = pl->prune_nseg;
         pa.ncp = pl->dt_n * 32; pa.cp_na = pl->dt_na * 32; pa.cp_a0 = pl->dt_a0 * 32; pa.cp_b0 = pl->dt_b0 * 32;
-        for (int q = 0; q < s.nwidths; ++q) {
+        // the pruned widths (candidates-only mode), then the column-level width as the last entry
+        pa.nq = 0; pa.wmax = 1;
+        for (int q = 0; q < s.nwidths && flags; ++q) {
           const WidthPlan &w = pl->wp[q];
           if (w.prune < 0) continue;
           pa.w[w.prune] = w.w; pa.nwin[w.prune] = (int)w.nwin; pa.offc[w.prune] = s.offc[q];
+          pa.nq = std::max(pa.nq, w.prune + 1); pa.wmax = std::max(pa.wmax, w.w);
+        }
+        pa.cwmask = nullptr; pa.cw_nwords = pl->cw_nwords; pa.cwdense = (unsigned char *)(ws + pl->off_cwdense);
+        if (use_cw) {
+          const WidthPlan &w = pl->wp[pl->cwq];
+          const int i = pa.nq++;
+          pa.w[i] = w.w; pa.nwin[i] = (int)w.nwin; pa.offc[i] = s.offc[pl->cwq]; pa.wmax = std::max(pa.wmax, w.w);
+          pa.cwmask = (uint32_t *)(ws + pl->off_cwmask);
+          if (!cuda_ok(cudaMemsetAsync(pa.cwmask, 0, (size_t)np * pl->cw_nwords * s.nf * sizeof(uint32_t), st))) return VOLKS_ECUDA;
         }
         const int T = 2 * pa.seg, thr = std::min(PRUNE_THREADS, s.nf / 2);   // (nf >= 64: a power of two >= 32)
         pa.ring = pa.wmax <= 16 ? 16 : 32;                 // rows of amplitude history (a power of two >= wmax)
         const size_t smem = (size_t)((pa.nq * (T + 64) + 3) & ~3) * sizeof(float) + (size_t)pa.ring * thr * sizeof(f32x2);
         const unsigned blocks = (unsigned)(np * ((pa.nseg + 1) / 2));
         ProfScope ps(pl, st, VOLKS_K_BOUND, -1);
-        switch (pa.nq) {
-          case 1: k_bound<1><<<blocks, thr, smem, st>>>(pa); break;
-          case 2: k_bound<2><<<blocks, thr, smem, st>>>(pa); break;
-          case 3: k_bound<3><<<blocks, thr, smem, st>>>(pa); break;
-          case 4: k_bound<4><<<blocks, thr, smem, st>>>(pa); break;
-          case 5: k_bound<5><<<blocks, thr, smem, st>>>(pa); break;
-          case 6: k_bound<6><<<blocks, thr, smem, st>>>(pa); break;
-          case 7: k_bound<7><<<blocks, thr, smem, st>>>(pa); break;
-          default: k_bound<8><<<blocks, thr, smem, st>>>(pa); break;
-        }
+#define VOLKS_BOUND(NQ_)                                                                   \
+  case NQ_:                                                                                \
+    if (use_cw) k_bound<NQ_, 1><<<blocks, thr, smem, st>>>(pa);                            \
+    else k_bound<NQ_, 0><<<blocks, thr, smem, st>>>(pa);                                   \
+    break;
+        switch (pa.nq) { VOLKS_BOUND(1) VOLKS_BOUND(2) VOLKS_BOUND(3) VOLKS_BOUND(4) VOLKS_BOUND(5) VOLKS_BOUND(6) VOLKS_BOUND(7) VOLKS_BOUND(8) }
+#undef VOLKS_BOUND
       }
     }
     for (int q = 0; q < s.nwidths; ++q) {
@@ -799,7 +827,8 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         sa.ndt = pl->dt_n; sa.dt_na = pl->dt_na; sa.dt_a0 = pl->dt_a0; sa.dt_b0 = pl->dt_b0;
         sa.ntasks = ((np * w.nseg * (long long)pl->dt_n) << w.log2m);
         sa.flags = flags && w.prune >= 0 ? flags + (size_t)w.prune * pl->prune_nseg : nullptr;
-        sa.flag_stride = pl->nprune * pl->prune_nseg;
+        sa.flag_stride = (pl->nprune + (use_cw ? 1 : 0)) * pl->prune_nseg;
+        if (hy && w.cw) { sa.flags = (const unsigned char *)(ws + pl->off_cwdense); sa.flag_stride = (pl->prune_nseg + 1) / 2; }   // dense tiles only
         ProfScope ps(pl, st, VOLKS_K_SLIDE, q);
         launch_slide(sa, st);
         continue;
@@ -829,17 +858,19 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
       fa.Y = Y; fa.keys = keys; fa.tables = pl->d_tables; fa.per_pair = s.per_pair; fa.pair0 = pair0;
       fa.nap = s.nap; fa.nf = s.nf; fa.log2nf = s.log2nf; fa.pitch = pl->pitch; fa.paired = pl->paired;
       fa.nq = 0; fa.unit0[0] = 0;
-      fa.flags = flags; fa.flag_nq = pl->nprune; fa.flag_nseg = pl->prune_nseg;
+      fa.cwdense = hy && use_cw ? (const unsigned char *)(ws + pl->off_cwdense) : nullptr; fa.cw_i = -1; fa.cw_ntile = (pl->prune_nseg + 1) / 2;
+      fa.flags = flags; fa.flag_nq = pl->nprune + (use_cw ? 1 : 0); fa.flag_nseg = pl->prune_nseg;
       for (int q = 0; q < s.nwidths; ++q) {
         const WidthPlan &w = pl->wp[q];
         if (!w.slide || w.nwin == 0) continue;
         const int i = fa.nq++;
+        if (hy && w.cw) fa.cw_i = i;
         fa.q[i] = q; fa.w[i] = w.w; fa.nt[i] = w.nt; fa.seg[i] = w.seg; fa.nseg[i] = w.nseg; fa.nwin[i] = (int)w.nwin;
         fa.offc[i] = s.offc[q]; fa.tw_off[i] = (long long)w.tw_off; fa.flag_q[i] = w.prune;
         fa.unit0[i + 1] = fa.unit0[i] + (w.nseg + FIX_GROUP - 1) / FIX_GROUP;
       }
       ProfScope ps(pl, st, VOLKS_K_FIXUP, -1);
-      k_fixup<<<(unsigned)(np * fa.unit0[fa.nq]), 256, 0, st>>>(fa);
+      if (fa.unit0[fa.nq] > 0) k_fixup<<<(unsigned)(np * fa.unit0[fa.nq]), 256, 0, st>>>(fa);
     }
     // the peak bins of the untagged sliding widths: every window (full index) or the possible candidates
     if (pl->nuntag > 0) {
@@ -857,6 +888,19 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
       ra2.total = np * ra2.cum[ra2.nq];
       ProfScope ps(pl, st, VOLKS_K_RECOVER, -1);
       k_recover<<<(unsigned)((ra2.total + 127) / 128), 128, 0, st>>>(ra2);
+    }
+    // the column-level width: every listed (window, column pair) by the definition; replaces the keys of those windows
+    if (use_cw) {
+      const WidthPlan &w = pl->wp[pl->cwq];
+      ColEvalArgs ea;
+      ea.Y = Y; ea.keys = keys; ea.mask = (const uint32_t *)(ws + pl->off_cwmask);
+      ea.twt = pl->d_tables + w.tw_off; ea.thr = (const uint32_t *)(ws + pl->off_thr);
+      ea.per_pair = s.per_pair; ea.offc = s.offc[pl->cwq]; ea.pair0 = pair0;
+      ea.nap = s.nap; ea.nf = s.nf; ea.pitch = pl->pitch; ea.w = w.w; ea.nt = w.nt; ea.log2m = w.log2m;
+      ea.nwin = (int)w.nwin; ea.nwords = pl->cw_nwords; ea.dense = (const unsigned char *)(ws + pl->off_cwdense);
+      ea.dstride = (pl->prune_nseg + 1) / 2; ea.only_above = hy ? 0 : 1;
+      ProfScope ps(pl, st, VOLKS_K_COLEVAL, pl->cwq);
+      k_coleval<<<(unsigned)(np * ((w.nwin + CE_TILE - 1) / CE_TILE)), CE_THREADS, 0, st>>>(ea);
     }
   }
   {
