@@ -348,20 +348,29 @@ __global__ void __launch_bounds__(256) k_row2(RowArgs a) {
   FftDif2<N1, N1, 0, N1>::run(v);
   u64 key = 0;
   float *dst = (float *)(a.Y + rrel * (long long)a.pitch);
+  if (a.dlo >= 0) {   // uniform: restricted delay range - the spectra outside it are written as zero
+#pragma unroll
+    for (int i = 0; i < N1; ++i)
+      if (!delay_ok(N2 * brev<N1>(i) + l, a.dlo, a.dhi)) v[i] = pk(0.f, 0.f);
+  }
+  // column 2c keeps (re, re') and column 2c + 1 keeps (im, im') of the pair's float4: one 64-bit store per lane
+  float *dstl = dst + ((l >> 1) << 2) + ((l & 1) << 1);
 #pragma unroll
   for (int i = 0; i < N1; ++i) {
-    const int col = N2 * brev<N1>(i) + l;
-    const bool inr = delay_ok(col, a.dlo, a.dhi);
-    const float re = inr ? lo32(v[i]) : 0.f, im = inr ? hi32(v[i]) : 0.f;
+    const float re = lo32(v[i]), im = hi32(v[i]);
     const float got = __shfl_xor_sync(0xffffffffu, (l & 1) ? re : im, 1);
-    if (live) {
-      float *p = dst + ((col >> 1) << 2) + ((l & 1) << 1);
-      *(float2 *)p = (l & 1) ? make_float2(got, im) : make_float2(re, got);
-    }
-    const u64 kk = make_key(fmaf(re, re, im * im), (uint32_t)col);
-    key = kk > key ? kk : key;
+    if (live) *(float2 *)(dstl + 2 * N2 * brev<N1>(i)) = (l & 1) ? make_float2(got, im) : make_float2(re, got);
   }
-  if (a.keys1) {   // uniform branch
+  if (a.keys1) {   // uniform branch: the w = 1 peaks (power, lowest column) of this row
+    float bp = -1.f;
+    int bc = 0;
+#pragma unroll
+    for (int i = 0; i < N1; ++i) {
+      const int col = N2 * brev<N1>(i) + l;
+      const float pw = fmaf(lo32(v[i]), lo32(v[i]), hi32(v[i]) * hi32(v[i]));
+      if (pw > bp || (pw == bp && col < bc)) { bp = pw; bc = col; }
+    }
+    key = make_key(bp, (uint32_t)bc);
 #pragma unroll
     for (int o = G >> 1; o >= 1; o >>= 1) {
       const u64 other = __shfl_xor_sync(0xffffffffu, key, o);
@@ -480,9 +489,11 @@ __global__ void __launch_bounds__(256) k_row3(RowArgs a) {
     if (!delay_ok(2 * c, a.dlo, a.dhi)) { q.x = 0.f; q.z = 0.f; }
     if (!delay_ok(2 * c + 1, a.dlo, a.dhi)) { q.y = 0.f; q.w = 0.f; }
     dst[c] = q;
-    const u64 k0 = make_key(fmaf(q.x, q.x, q.z * q.z), (uint32_t)(2 * c)), k1 = make_key(fmaf(q.y, q.y, q.w * q.w), (uint32_t)(2 * c + 1));
-    key = k0 > key ? k0 : key;
-    key = k1 > key ? k1 : key;
+    if (a.keys1) {   // uniform: the w = 1 peaks
+      const u64 k0 = make_key(fmaf(q.x, q.x, q.z * q.z), (uint32_t)(2 * c)), k1 = make_key(fmaf(q.y, q.y, q.w * q.w), (uint32_t)(2 * c + 1));
+      key = k0 > key ? k0 : key;
+      key = k1 > key ? k1 : key;
+    }
   }
   if (a.keys1) {   // uniform branch
 #pragma unroll
