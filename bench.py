@@ -216,14 +216,30 @@ KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6:
               10: "winthr", 11: "bound", 12: "recover", 13: "coleval"}
 
 
+# Executed flops per unit, pinned by ncu (profiles/r02_counters.md: sm__sass_thread_inst_executed_op_fp32_pred_on counts a
+# packed FFMA2 / FMUL2 / FADD2 once per thread; the FFMA2 : (FMUL2 + FADD2) mix comes from the kernel's SASS):
+#   k_slide, w >= 16: 4.96e11 flops per w = 64 launch of config 2 / 6.29e10 bin-steps = 7.9 flops per bin per window (a complex
+#     multiply-add is 8 flops only for the non-trivial half of the twiddles; the others are two adds; + 3 for |.|^2)
+#   k_colfft2, Nt = 512: 1088 / 1326 / 1532 flops per thread and window for w <= 64 / 128 / 256 (pass 1 pruned to the non-zero
+#     inputs), 16 threads per delay column: 17408 / 21216 / 24512 per (window, column) against the SURVEY count 25600
+SLIDE_FLOPS_PER_BIN = 7.9
+COLFFT2_FLOPS_PER_COLUMN = {4: 17408.0, 8: 21216.0, 16: 24512.0}
+
+
 def executed_flops_per_launch(c, kind, wid, nlaunch, npair, nap, alg_flops):
-    """Flops the kernel really executes per launch.  The sliding kernel does one complex
-    multiply-add (4 FMA = 8 flops) + |.|^2 (3 flops) per bin per window instead of an FFT: 11 per bin; the
-    FFT kernels execute the SURVEY 8(d) algorithmic count at most (pruned inputs: fewer), which is what is
-    charged to them.  profiles/ holds the ncu instruction counters these figures are checked against."""
-    if kind in (6, 11) and wid >= 0:
-        w_, nt_ = c["widths"][wid], c["nts"][wid]
-        return workloads.gen.nwin(nap, w_, 1) * npair * nt_ * c["nf"] * 11.0 / nlaunch
+    """Flops the kernel really executes per launch, counter-pinned where a capture exists; a
+    kernel without one is charged the SURVEY 8(d) algorithmic count (an upper bound: pruned inputs execute fewer)."""
+    if wid < 0:
+        return alg_flops
+    w_, s_, nt_ = c["widths"][wid], c["strides"][wid], c["nts"][wid]
+    nwin = workloads.gen.nwin(nap, w_, s_) * npair
+    if kind == 6:
+        return nwin * nt_ * c["nf"] * SLIDE_FLOPS_PER_BIN / nlaunch
+    nz = 1
+    while nz * 16 < w_:
+        nz *= 2
+    if kind == 7 and nt_ == 512 and nz in COLFFT2_FLOPS_PER_COLUMN:
+        return nwin * c["nf"] * COLFFT2_FLOPS_PER_COLUMN[nz] / nlaunch
     return alg_flops
 
 
@@ -392,8 +408,11 @@ def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traff
         "bound": "alu", "kernel": kname, "achieved": exec_tf, "peak": peak_tf, "unit": "TFLOP/s",
         "frac": exec_tf / peak_tf, "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None,
         "launch_ms": dom_ms_avg, "share_of_step": share[dom] / step_sum,
-        "flops_kind": "executed: sliding kernels 11 flops per bin per window (complex multiply-add + |.|^2), FFT kernels "
-                      "the SURVEY 8(d) count (5 Nt log2 Nt per column + 5 per bin; 5 Nf log2 Nf per AP row)",
+        "flops_kind": "executed, pinned by ncu's instruction counters (profiles/r02_counters.md): k_slide 7.9 flops per bin "
+                      "per window, k_colfft2 (Nt 512) 17408 / 21216 / 24512 flops per (window, column) for w <= 64 / 128 / 256; "
+                      "other kernels the SURVEY 8(d) count",
+        "fma_pipe_note": "packed FP32 adds and multiplies occupy the FMA pipe like FMAs but count half the flops, so the "
+                         "flop fraction understates the pipe: ncu reads the FMA pipe 68 % busy for k_slide w = 64 (profiles/)",
         "peak_kind": peak["kind"], "peak_derived_tflops": peak["derived_tflops"],
         "algorithmic_tflops": alg_tf, "algorithmic_frac": alg_tf / peak_tf,
         "algorithmic_kind": "SURVEY 8(d) FFT-equivalent flops / time: exceeds 1 by construction for the sliding path "

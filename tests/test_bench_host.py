@@ -60,8 +60,10 @@ def test_traffic_table_and_executed_flops():
     tab = bench.ncu_traffic_table()
     assert (2, "slide", 64) in tab and tab[(2, "slide", 64)][0] > 1e9 and "profiles/" in tab[(2, "slide", 64)][1]
     c = workloads.config(2)
-    # sliding kernel, w = 64 (Nt 128, Nf 256): 11 flops per bin per window, 5 launches
+    # sliding kernel, w = 64 (Nt 128, Nf 256): 7.9 flops per bin per window (ncu-pinned), 5 launches
     ex = bench.executed_flops_per_launch(c, 6, 5, 5, 80, c["nap"], 1.0)
-    assert ex == (120000 - 64 + 1) * 80 * 128 * 256 * 11.0 / 5
-    # FFT kernels are charged the algorithmic count
-    assert bench.executed_flops_per_launch(workloads.config(4), 7, 0, 7, 84, 20000, 123.0) == 123.0
+    assert ex == (120000 - 64 + 1) * 80 * 128 * 256 * 7.9 / 5
+    # k_colfft2 at Nt = 512: the counter-pinned flops per (window, column); kernels without a capture: the algorithmic count
+    c4 = workloads.config(4)
+    assert bench.executed_flops_per_launch(c4, 7, 0, 7, 84, 20000, 123.0) == 1247 * 84 * 2048 * 17408.0 / 7
+    assert bench.executed_flops_per_launch(c4, 1, -1, 7, 84, 20000, 123.0) == 123.0
