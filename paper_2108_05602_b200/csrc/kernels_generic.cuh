@@ -743,6 +743,13 @@ __device__ __forceinline__ WinStat window_stat(const Sched &s, const u64 *keys, 
   o.q = q; o.j = (int)rem; o.t0 = o.j * s.stride[q];
   const u64 k = keys[c];
   o.power = key_power(k);
+  if (o.power == 0.f) {
+    // a zero key: an all-zero window, or one the candidates-only mode did not evaluate (pruned, skipped): power 0 at
+    // the first searched bin, snr 0 - the window energy is not needed (most windows of a pruned search end here)
+    o.rate_idx = 0; o.delay_idx = s.dfirst; o.snr = 0.f;
+    if (zst) { const double2 ms = zst[o.pair * s.nwidths + q]; o.snr = (float)((0.0 - ms.x) * ms.y); }
+    return o;
+  }
   const uint32_t idx = key_index(k);
   o.rate_idx = (int)(idx >> s.log2nf);
   o.delay_idx = (int)(idx & (uint32_t)(s.nf - 1));
