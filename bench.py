@@ -220,10 +220,10 @@ KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6:
 # packed FFMA2 / FMUL2 / FADD2 once per thread; the FFMA2 : (FMUL2 + FADD2) mix comes from the kernel's SASS):
 #   k_slide, w >= 16: 4.96e11 flops per w = 64 launch of config 2 / 6.29e10 bin-steps = 7.9 flops per bin per window (a complex
 #     multiply-add is 8 flops only for the non-trivial half of the twiddles; the others are two adds; + 3 for |.|^2)
-#   k_colfft2, Nt = 512: 1088 / 1326 / 1532 flops per thread and window for w <= 64 / 128 / 256 (pass 1 pruned to the non-zero
-#     inputs), 16 threads per delay column: 17408 / 21216 / 24512 per (window, column) against the SURVEY count 25600
+#   k_colfft2, Nt = 512: 5553 / 6359 / 7089 packed instructions per (window, delay column) for w <= 64 / 128 / 256 (pass 1
+#     pruned to the non-zero inputs) at 2.47 / 2.45 / 2.42 flops each: 13700 / 15600 / 17200 against the SURVEY count 25600
 SLIDE_FLOPS_PER_BIN = 7.9
-COLFFT2_FLOPS_PER_COLUMN = {4: 17408.0, 8: 21216.0, 16: 24512.0}
+COLFFT2_FLOPS_PER_COLUMN = {4: 13700.0, 8: 15600.0, 16: 17200.0}
 
 
 def executed_flops_per_launch(c, kind, wid, nlaunch, npair, nap, alg_flops):
@@ -409,10 +409,10 @@ def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traff
         "frac": exec_tf / peak_tf, "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None,
         "launch_ms": dom_ms_avg, "share_of_step": share[dom] / step_sum,
         "flops_kind": "executed, pinned by ncu's instruction counters (profiles/r02_counters.md): k_slide 7.9 flops per bin "
-                      "per window, k_colfft2 (Nt 512) 17408 / 21216 / 24512 flops per (window, column) for w <= 64 / 128 / 256; "
+                      "per window, k_colfft2 (Nt 512) 13700 / 15600 / 17200 flops per (window, column) for w <= 64 / 128 / 256; "
                       "other kernels the SURVEY 8(d) count",
         "fma_pipe_note": "packed FP32 adds and multiplies occupy the FMA pipe like FMAs but count half the flops, so the "
-                         "flop fraction understates the pipe: ncu reads the FMA pipe 68 % busy for k_slide w = 64 (profiles/)",
+                         "flop fraction understates the pipe: ncu reads the FMA pipe 68 % busy for k_slide w = 64 and k_colfft2 w = 64 (profiles/r02_counters.md)",
         "peak_kind": peak["kind"], "peak_derived_tflops": peak["derived_tflops"],
         "algorithmic_tflops": alg_tf, "algorithmic_frac": alg_tf / peak_tf,
         "algorithmic_kind": "SURVEY 8(d) FFT-equivalent flops / time: exceeds 1 by construction for the sliding path "
