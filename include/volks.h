@@ -48,6 +48,7 @@ extern "C" {
 #define VOLKS_ECUDA (-2)     /* CUDA allocation / launch failure (sticky error text: strerror)   */
 #define VOLKS_ENOMEM (-3)    /* host allocation failure                                           */
 #define VOLKS_EOVERFLOW (-4) /* returned by volks_window_match when capacity < number of pulses   */
+#define VOLKS_ELIMIT (-5)    /* volks_search_noalloc: the problem needs more than its static scratch */
 
 #define VOLKS_MAX_WIDTHS 16
 
@@ -280,6 +281,31 @@ int volks_plan_profile_read(const volks_plan *plan, int32_t capacity, int32_t *k
  * nullable).  Counts 2 flop per FMA per thread. */
 int volks_measure_fp32_peak(int32_t repeats, double *tflops_best, double *tflops_mean, double *ms_per_launch,
                             void *cuda_stream);
+
+/* The search for callers that CANNOT ALLOCATE (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): one call, no plan, no workspace.  It computes what volks_fringe_search computes (the
+ * definition at the top of this file: every window's peak, snr, the ordered candidate list) with the general
+ * kernels (k_row_fft, k_col, finalize / scan / scatter), and keeps EVERY intermediate - window schedule, twiddle
+ * tables, per-window keys, per-AP energies, block counts, the delay spectra - in one file-scope device array of
+ * VOLKS_NOALLOC_SCRATCH_BYTES (32 MiB) that every GPU loading the library holds until exit.  The call makes no
+ * cudaMalloc / cudaFree and no allocating library call; it only enqueues a memset and kernels on `cuda_stream`
+ * (asynchronous: results are valid after the stream is synchronised) - the first call on a device also looks up the
+ * array's device address (cudaGetSymbolAddress) and raises one kernel's shared-memory limit.
+ *   p            HOST search parameters, as for volks_plan_create (nf <= 8192; read during the call only)
+ *   d_vis        DEVICE cf32[nbl][nif][nap][nchan], read-only
+ *   d_peaks      DEVICE volks_peak[nwin_total] in the dense layout of volks_fringe_search, or NULL
+ *   d_cands      DEVICE volks_cand[cand_capacity], canonical order; d_ncand DEVICE uint32, the TRUE total
+ * Size limit: 1 KiB + 8 (nf + sum_q nt_q) + 8 nwin_total + 4 nbl nif nap + 8 nbl nif nap pitch (pitch = nf + 16 for
+ * nf >= 32, else nf) + small change must fit the 32 MiB; larger problems return VOLKS_ELIMIT before anything is
+ * enqueued (BASELINE.json configs 0 and 1 fit; use a plan for the large ones).  It always searches the whole delay
+ * axis and every window's exact peak (no options).
+ * SHARED STATE: every call on a device uses the same array, which keeps the last call's contents (the call clears
+ * what must start at zero).  Two calls that overlap on the GPU - different streams, or different host threads
+ * without a common stream order - RACE on it; calls on one stream are ordered and safe.
+ * Returns VOLKS_OK, VOLKS_EINVAL (bad parameters / null pointers), VOLKS_ELIMIT, or VOLKS_ECUDA. */
+#define VOLKS_NOALLOC_SCRATCH_BYTES (32u << 20)
+int volks_search_noalloc(const volks_params *p, const void *d_vis, volks_peak *d_peaks, volks_cand *d_cands,
+                         uint32_t cand_capacity, uint32_t *d_ncand, void *cuda_stream);
 
 const char *volks_strerror(int code);
 int volks_version(void);

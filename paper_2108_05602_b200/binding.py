@@ -11,7 +11,8 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libvolks_b200.so")
 
-VOLKS_OK, VOLKS_EINVAL, VOLKS_ECUDA, VOLKS_ENOMEM, VOLKS_EOVERFLOW = 0, -1, -2, -3, -4
+VOLKS_OK, VOLKS_EINVAL, VOLKS_ECUDA, VOLKS_ENOMEM, VOLKS_EOVERFLOW, VOLKS_ELIMIT = 0, -1, -2, -3, -4, -5
+NOALLOC_SCRATCH_BYTES = 32 << 20      # VOLKS_NOALLOC_SCRATCH_BYTES
 
 EXPORTS = (
     "volks_plan_create", "volks_plan_destroy", "volks_plan_query", "volks_fringe_search",
@@ -20,6 +21,7 @@ EXPORTS = (
     "volks_baseline_match", "volks_zscore_select", "volks_plan_create_allif", "volks_allif_search",
     "volks_plan_query_host", "volks_search_host", "volks_plan_set_cal", "volks_cal_phasors",
     "volks_measure_fp32_peak", "volks_options_init", "volks_plan_create_opt", "volks_plan_create_allif_opt",
+    "volks_search_noalloc",
 )
 
 
@@ -73,6 +75,8 @@ def lib():
                                         ctypes.c_double, ctypes.c_void_p]
         L.volks_measure_fp32_peak.argtypes = [ctypes.c_int32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
                                               ctypes.POINTER(ctypes.c_double), ctypes.c_void_p]
+        L.volks_search_noalloc.argtypes = [ctypes.POINTER(volks_params), ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+                                           ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p]
         L.volks_plan_destroy.argtypes = [ctypes.c_void_p]
         L.volks_plan_query.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_size_t),
                                        ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
@@ -270,6 +274,23 @@ def baseline_match(pulses, min_baselines=5):
     _check(lib().volks_baseline_match(pulses.ctypes.data, len(pulses), min_baselines, out.ctypes.data, len(out),
                                       ctypes.byref(n)))
     return out[:n.value]
+
+
+def search_noalloc(vis, widths, strides, nts, nf, snr_thresh, cands, ncand, peaks=None, stream=None):
+    """volks_search_noalloc: the search without plan or workspace (every intermediate in the library's static 32 MiB
+    device array; no allocation inside the call).  All buffers are the caller's torch CUDA tensors: vis complex64
+    [nbl][nif][nap][nchan]; cands uint8 [capacity*36]; ncand int32 [1]; peaks uint8 [nwin_total*16] or None.
+    Asynchronous on `stream`.  Returns the library's code (VOLKS_OK / VOLKS_ELIMIT ...) without raising."""
+    assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous()
+    nbl, nif, nap, nchan = vis.shape
+    n = len(widths)
+    arr = lambda v: (ctypes.c_int32 * max(len(v), 1))(*[int(x) for x in v])
+    w, s, t = arr(widths), arr(strides), arr(nts)
+    p = volks_params(nbl, nif, nap, nchan, n, w, s, t, int(nf), float(snr_thresh))
+    cap = cands.numel() * cands.element_size() // CAND_DTYPE.itemsize
+    st = (stream or torch.cuda.current_stream(vis.device)).cuda_stream
+    return lib().volks_search_noalloc(ctypes.byref(p), vis.data_ptr(), peaks.data_ptr() if peaks is not None else None,
+                                      cands.data_ptr() if cap else None, cap, ncand.data_ptr(), st)
 
 
 def measure_fp32_peak(repeats=5, stream=None):

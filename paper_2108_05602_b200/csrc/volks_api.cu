@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -293,6 +294,7 @@ const char *volks_strerror(int code) {
     case VOLKS_ECUDA: return g_cuda_msg[0] ? g_cuda_msg : "CUDA error";
     case VOLKS_ENOMEM: return "out of host memory";
     case VOLKS_EOVERFLOW: return "output capacity exceeded";
+    case VOLKS_ELIMIT: return "problem larger than the static scratch of volks_search_noalloc (VOLKS_NOALLOC_SCRATCH_BYTES)";
     default: return "unknown error";
   }
 }
@@ -1103,3 +1105,153 @@ int volks_bin_to_physical(int32_t nt, int32_t nf, int32_t rate_idx, int32_t dela
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// volks_search_noalloc: the same search for callers that cannot allocate (include/volks.h).
+// Every intermediate - the window schedule, the twiddle tables, the per-window keys, the per-AP energies, the
+// block counts and the delay spectra - lives in ONE file-scope device array that every GPU loading this library
+// holds until exit.  g_noalloc_scratch is a HOST-SIDE STAND-IN in host code, not a device address: the address is
+// taken once per device with cudaGetSymbolAddress (that device current) and only that pointer goes to kernels.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_noalloc_scratch[VOLKS_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+unsigned char *g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {nullptr};   // per device, filled on first use
+std::mutex g_noalloc_mutex;
+
+struct NoAllocTables { int nf, nq; int nt[VOLKS_MAX_WIDTHS]; long long off[VOLKS_MAX_WIDTHS]; };
+
+// writes the schedule and the twiddle tables into the scratch (double-precision sincospi, rounded once to float)
+__global__ void __launch_bounds__(256) k_noalloc_setup(Sched s, NoAllocTables t, Sched *d_sched, float2 *tab) {
+  const long long gid = (long long)blockIdx.x * 256 + threadIdx.x, nthr = (long long)gridDim.x * 256;
+  if (gid == 0) *d_sched = s;
+  for (long long k = gid; k < t.nf; k += nthr) {
+    double sn, cs;
+    sincospi(-2.0 * (double)k / (double)t.nf, &sn, &cs);
+    tab[k] = make_float2((float)cs, (float)sn);
+  }
+  for (int q = 0; q < t.nq; ++q)
+    for (long long k = gid; k < t.nt[q]; k += nthr) {
+      double sn, cs;
+      sincospi(-2.0 * (double)k / (double)t.nt[q], &sn, &cs);
+      tab[t.off[q] + k] = make_float2((float)cs, (float)sn);
+    }
+}
+
+// device address of the scratch on the CURRENT device (nullptr + g_cuda_msg on failure); once per device
+unsigned char *noalloc_scratch_ptr() {
+  int dev = -1;
+  if (!cuda_ok(cudaGetDevice(&dev))) return nullptr;
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) { snprintf(g_cuda_msg, sizeof g_cuda_msg, "device ordinal %d not supported", dev); return nullptr; }
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_ptr[dev]) {
+    void *p = nullptr;
+    if (!cuda_ok(cudaGetSymbolAddress(&p, g_noalloc_scratch)) || !p) return nullptr;
+    // the generic row kernel's dynamic shared memory limit: the same maximum volks_plan_create sets (per device)
+    if (!cuda_ok(cudaFuncSetAttribute(k_row_fft, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024))) return nullptr;
+    g_noalloc_ptr[dev] = (unsigned char *)p;
+  }
+  return g_noalloc_ptr[dev];
+}
+
+}  // namespace
+
+extern "C" int volks_search_noalloc(const volks_params *p, const void *d_vis, volks_peak *d_peaks, volks_cand *d_cands,
+                                    uint32_t cand_capacity, uint32_t *d_ncand, void *cuda_stream) {
+  if (!p || !d_vis || !d_ncand || (!d_cands && cand_capacity > 0)) return VOLKS_EINVAL;
+  if (p->nbl < 1 || p->nif < 1 || p->nap < 0 || p->nchan < 1) return VOLKS_EINVAL;
+  if (p->nwidths < 1 || p->nwidths > VOLKS_MAX_WIDTHS || !p->width || !p->stride || !p->nt) return VOLKS_EINVAL;
+  if (!is_pow2(p->nf) || p->nf < p->nchan || p->nf > 8192) return VOLKS_EINVAL;
+  if (!(p->snr_thresh == p->snr_thresh)) return VOLKS_EINVAL;
+  const long long npair = (long long)p->nbl * p->nif;
+  Sched s;
+  memset(&s, 0, sizeof s);
+  s.nwidths = p->nwidths; s.nbl = p->nbl; s.nif = p->nif; s.nap = p->nap; s.nf = p->nf; s.log2nf = ilog2(p->nf);
+  s.allif = 0; s.ngs = 1; s.snr_thresh = p->snr_thresh; s.dlo = -1; s.dhi = -1; s.dfirst = 0;
+  NoAllocTables t;
+  memset(&t, 0, sizeof t);
+  t.nf = p->nf; t.nq = p->nwidths;
+  long long per_pair = 0, tab_elems = p->nf;
+  for (int q = 0; q < p->nwidths; ++q) {
+    if (p->width[q] < 1 || p->stride[q] < 1 || !is_pow2(p->nt[q]) || p->nt[q] < p->width[q]) return VOLKS_EINVAL;
+    if ((long long)p->nt[q] * p->nf > (1LL << 31)) return VOLKS_EINVAL;
+    s.width[q] = p->width[q]; s.stride[q] = p->stride[q]; s.nt[q] = p->nt[q];
+    s.nwin[q] = p->nap < p->width[q] ? 0 : (long long)(p->nap - p->width[q]) / p->stride[q] + 1;
+    s.offc[q] = per_pair; s.offd[q] = npair * per_pair;
+    per_pair += s.nwin[q];
+    t.nt[q] = p->nt[q]; t.off[q] = tab_elems; tab_elems += p->nt[q];
+    // k_col's grid (one thread per (window, rate residue, delay column)) must fit gridDim.x: checked before any launch
+    const long double col_threads = (long double)npair * s.nwin[q] * (p->nt[q] / std::min(16, p->nt[q])) * p->nf;
+    if (col_threads / 256 > 2147483000.0L) return VOLKS_ELIMIT;
+  }
+  s.per_pair = per_pair; s.nwin_total = per_pair * npair;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (s.nwin_total == 0) return cuda_ok(cudaMemsetAsync(d_ncand, 0, sizeof(uint32_t), st)) ? VOLKS_OK : VOLKS_ECUDA;
+
+  // layout inside the static scratch (256-byte aligned pieces); everything beyond its stated size is refused
+  const int pitch = p->nf >= 32 ? p->nf + 16 : p->nf, paired = p->nf >= 2 ? 1 : 0;
+  const long long nfin = (s.nwin_total + FIN_THREADS * FIN_TILES - 1) / (FIN_THREADS * FIN_TILES);
+  const long double need_ld = 1024.0L + 8.0L * tab_elems + 8.0L * s.nwin_total + 4.0L * npair * p->nap + 4.0L * nfin +
+                              8.0L * npair * (long double)p->nap * pitch + 6 * 256.0L;
+  if (need_ld > (long double)VOLKS_NOALLOC_SCRATCH_BYTES) return VOLKS_ELIMIT;
+  size_t off = 0;
+  const size_t off_sched = off; off = align_up(off + sizeof(Sched), 256);
+  const size_t off_tab = off;   off = align_up(off + (size_t)tab_elems * sizeof(float2), 256);
+  const size_t off_keys = off;  off = align_up(off + (size_t)s.nwin_total * sizeof(u64), 256);
+  const size_t off_E = off;     off = align_up(off + (size_t)npair * p->nap * sizeof(float), 256);
+  const size_t off_cnt = off;   off = align_up(off + (size_t)nfin * sizeof(uint32_t), 256);
+  const size_t off_Y = off;     off = align_up(off + (size_t)npair * p->nap * pitch * sizeof(float2), 256);
+  if (off > (size_t)VOLKS_NOALLOC_SCRATCH_BYTES) return VOLKS_ELIMIT;
+  const long long GMAX = (1LL << 31) - 1;
+  if (npair * p->nap > GMAX || nfin > GMAX) return VOLKS_ELIMIT;
+
+  unsigned char *base = noalloc_scratch_ptr();      // the DEVICE address of g_noalloc_scratch on the current device
+  if (!base) return VOLKS_ECUDA;
+  Sched *d_sched = (Sched *)(base + off_sched);
+  float2 *tab = (float2 *)(base + off_tab);
+  u64 *keys = (u64 *)(base + off_keys);
+  float *E = (float *)(base + off_E);
+  uint32_t *cnt = (uint32_t *)(base + off_cnt);
+  float2 *Y = (float2 *)(base + off_Y);
+
+  // the scratch keeps the last call's contents: the keys meet in an atomicMax and must start at zero; the schedule,
+  // tables, energies, counts and spectra are written in full before they are read
+  if (!cuda_ok(cudaMemsetAsync(keys, 0, (size_t)s.nwin_total * sizeof(u64), st))) return VOLKS_ECUDA;
+  k_noalloc_setup<<<(unsigned)std::min<long long>(64, (tab_elems + 255) / 256), 256, 0, st>>>(s, t, d_sched, tab);
+
+  RowArgs ra;
+  memset(&ra, 0, sizeof ra);
+  ra.vis = (const float2 *)d_vis; ra.Y = Y; ra.E = E; ra.twf = tab; ra.row0 = 0; ra.nrows = npair * p->nap;
+  ra.nchan = p->nchan; ra.nf = p->nf;
+  ra.tpr = p->nf <= 512 ? std::max(1, std::min(32, p->nf / 4)) : std::min(512, p->nf / 4);
+  ra.rows_per_cta = std::max(1, 256 / ra.tpr);
+  ra.pitch = pitch; ra.paired = paired; ra.keys1 = nullptr; ra.per_pair = per_pair; ra.nap = p->nap; ra.stride1 = 1; ra.nwin1 = 0;
+  ra.shift = nullptr; ra.nif = p->nif; ra.allif_nif = 0; ra.allif_nchan = 0; ra.psub = 1; ra.premod = nullptr; ra.cal = nullptr;
+  ra.dlo = -1; ra.dhi = -1;
+  const size_t row_smem = (size_t)2 * ra.rows_per_cta * p->nf * sizeof(float2) + (size_t)ra.rows_per_cta * 16 * sizeof(u64);
+  const long long rblocks = (ra.nrows + ra.rows_per_cta - 1) / ra.rows_per_cta;
+  if (ra.nrows > 0) k_row_fft<<<(unsigned)rblocks, ra.tpr * ra.rows_per_cta, row_smem, st>>>(ra);
+
+  for (int q = 0; q < p->nwidths; ++q) {
+    if (s.nwin[q] == 0) continue;
+    ColArgs ca;
+    const int L = std::min(16, p->nt[q]);
+    ca.Y = Y; ca.keys = keys; ca.twt = tab + t.off[q]; ca.per_pair = per_pair; ca.offc = s.offc[q]; ca.pair0 = 0;
+    ca.nap = p->nap; ca.nf = p->nf; ca.log2nf = s.log2nf; ca.w = p->width[q]; ca.stride = p->stride[q]; ca.nt = p->nt[q];
+    ca.log2m = ilog2(p->nt[q] / L); ca.nwin = (int)s.nwin[q]; ca.pitch = pitch; ca.paired = paired;
+    ca.total = ((npair * s.nwin[q]) << ca.log2m) * p->nf;
+    switch (L) {
+      case 1: launch_col<1>(ca, st); break;
+      case 2: launch_col<2>(ca, st); break;
+      case 4: launch_col<4>(ca, st); break;
+      case 8: launch_col<8>(ca, st); break;
+      default: launch_col<16>(ca, st); break;
+    }
+  }
+  k_finalize<<<(unsigned)nfin, FIN_THREADS, 0, st>>>(d_sched, keys, E, (float4 *)d_peaks, cnt, nullptr, 0.f, nullptr);
+  k_scan<<<1, 1024, 0, st>>>(cnt, nfin, d_ncand);
+  k_scatter<<<(unsigned)nfin, FIN_THREADS, 0, st>>>(d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity, nullptr, 0.f, nullptr);
+  return cuda_ok(cudaGetLastError()) ? VOLKS_OK : VOLKS_ECUDA;
+}
