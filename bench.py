@@ -223,6 +223,12 @@ KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6:
 #   k_colfft2, Nt = 512: 5553 / 6359 / 7089 packed instructions per (window, delay column) for w <= 64 / 128 / 256 (pass 1
 #     pruned to the non-zero inputs) at 2.47 / 2.45 / 2.42 flops each: 13700 / 15600 / 17200 against the SURVEY count 25600
 SLIDE_FLOPS_PER_BIN = 7.9
+# ... and the same counters as FP32 lane-OPERATIONS (an add, a multiply and an FMA each count once per lane; a packed
+# instruction is two lanes): k_slide 1.625e11 thread-instructions x 2 / 6.288e10 bin-steps = 5.17 per bin per window;
+# k_colfft2 2 x (5553 / 6359 / 7089) per (window, column).  Against the peak OPERATION rate (measured FMA peak / 2 flops per
+# FMA) this is the share of the FP32 pipe's issue slots the kernel fills - what ncu reports as FMA-pipe cycles active.
+SLIDE_OPS_PER_BIN = 5.17
+COLFFT2_OPS_PER_COLUMN = {4: 11106.0, 8: 12718.0, 16: 14178.0}
 COLFFT2_FLOPS_PER_COLUMN = {4: 13700.0, 8: 15600.0, 16: 17200.0}
 
 
@@ -241,6 +247,22 @@ def executed_flops_per_launch(c, kind, wid, nlaunch, npair, nap, alg_flops):
     if kind == 7 and nt_ == 512 and nz in COLFFT2_FLOPS_PER_COLUMN:
         return nwin * c["nf"] * COLFFT2_FLOPS_PER_COLUMN[nz] / nlaunch
     return alg_flops
+
+
+def executed_ops_per_launch(c, kind, wid, nlaunch, npair, nap):
+    """FP32 lane-operations per launch (see SLIDE_OPS_PER_BIN), or None for kernels without a counter capture."""
+    if wid < 0:
+        return None
+    w_, s_, nt_ = c["widths"][wid], c["strides"][wid], c["nts"][wid]
+    nwin = workloads.gen.nwin(nap, w_, s_) * npair
+    if kind == 6:
+        return nwin * nt_ * c["nf"] * SLIDE_OPS_PER_BIN / nlaunch
+    nz = 1
+    while nz * 16 < w_:
+        nz *= 2
+    if kind == 7 and nt_ == 512 and nz in COLFFT2_OPS_PER_COLUMN:
+        return nwin * c["nf"] * COLFFT2_OPS_PER_COLUMN[nz] / nlaunch
+    return None
 
 
 def measure_fp32_peak(vk, local, stream):
@@ -404,6 +426,7 @@ def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traff
     exec_tf = exec_flops / (dom_ms_avg * 1e-3) / 1e12
     alg_tf = dom_alg / (dom_ms_avg * 1e-3) / 1e12
     tr = traffic.get((c["id"], KIND_NAMES.get(dom[0], ""), c["widths"][dom[1]] if dom[1] >= 0 else -1))
+    ops = executed_ops_per_launch(c, dom[0], dom[1], nlaunch[dom], nbl * nif, nap)
     roofline = {
         "bound": "alu", "kernel": kname, "achieved": exec_tf, "peak": peak_tf, "unit": "TFLOP/s",
         "frac": exec_tf / peak_tf, "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None,
@@ -414,6 +437,9 @@ def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traff
         "fma_pipe_note": "packed FP32 adds and multiplies occupy the FMA pipe like FMAs but count half the flops, so the "
                          "flop fraction understates the pipe: ncu reads the FMA pipe 68 % busy for k_slide w = 64 and k_colfft2 w = 64 (profiles/r02_counters.md)",
         "peak_kind": peak["kind"], "peak_derived_tflops": peak["derived_tflops"],
+        "fp32_op_frac": None if ops is None else ops / (dom_ms_avg * 1e-3) / (peak_tf * 1e12 / 2.0),
+        "fp32_op_kind": "executed FP32 lane-operations (add, multiply and FMA each one; ncu-pinned) / time / peak operation rate "
+                        "(measured FMA peak / 2): the share of FP32 issue slots filled; `frac` counts flops, which halves every add",
         "algorithmic_tflops": alg_tf, "algorithmic_frac": alg_tf / peak_tf,
         "algorithmic_kind": "SURVEY 8(d) FFT-equivalent flops / time: exceeds 1 by construction for the sliding path "
                             "(an algorithmic speed-up, not a fraction of the machine)",
@@ -478,7 +504,7 @@ def brief(R):
             "visibilities_per_s": R["world"] * R["nvis"] / (R["ms_step"] * 1e-3), "windows": R["nwin"],
             "candidates": R["n_found"], "clocks": R["clocks"],
             "roofline": {k: rf[k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic", "launch_ms",
-                                            "share_of_step", "algorithmic_frac", "bytes_kind", "kernel_ms") if k in rf}}
+                                            "share_of_step", "fp32_op_frac", "algorithmic_frac", "bytes_kind", "kernel_ms") if k in rf}}
 
 
 def main():

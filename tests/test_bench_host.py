@@ -67,3 +67,7 @@ def test_traffic_table_and_executed_flops():
     c4 = workloads.config(4)
     assert bench.executed_flops_per_launch(c4, 7, 0, 7, 84, 20000, 123.0) == 1247 * 84 * 2048 * 13700.0 / 7
     assert bench.executed_flops_per_launch(c4, 1, -1, 7, 84, 20000, 123.0) == 123.0
+    # the same launches as FP32 lane-operations (the pipe-level view); kernels without a capture give None
+    assert bench.executed_ops_per_launch(c, 6, 5, 5, 80, c["nap"]) == (120000 - 64 + 1) * 80 * 128 * 256 * 5.17 / 5
+    assert bench.executed_ops_per_launch(c4, 7, 2, 7, 84, 20000) == 309 * 84 * 2048 * 14178.0 / 7
+    assert bench.executed_ops_per_launch(c4, 1, -1, 7, 84, 20000) is None
