@@ -229,10 +229,14 @@ SLIDE_FLOPS_PER_BIN = 7.9
 # FMA) this is the share of the FP32 pipe's issue slots the kernel fills - what ncu reports as FMA-pipe cycles active.
 SLIDE_OPS_PER_BIN = 5.17
 COLFFT2_OPS_PER_COLUMN = {4: 11106.0, 8: 12718.0, 16: 14178.0}
+# k_colfft2 SKIP (the default candidates-only mode: pass 2 only where a candidate is possible; profiles/r02_counters.md,
+# configs[4]'s data): 2071 / 2884 / 3617 packed instructions per (window, column): pass 1 + the 32 FFMA2 of the bound
+COLFFT2_SKIP_FLOPS_PER_COLUMN = {4: 5900.0, 8: 7850.0, 16: 9560.0}
+COLFFT2_SKIP_OPS_PER_COLUMN = {4: 4142.0, 8: 5768.0, 16: 7234.0}
 COLFFT2_FLOPS_PER_COLUMN = {4: 13700.0, 8: 15600.0, 16: 17200.0}
 
 
-def executed_flops_per_launch(c, kind, wid, nlaunch, npair, nap, alg_flops):
+def executed_flops_per_launch(c, kind, wid, nlaunch, npair, nap, alg_flops, cand_only=False):
     """Flops the kernel really executes per launch, counter-pinned where a capture exists; a
     kernel without one is charged the SURVEY 8(d) algorithmic count (an upper bound: pruned inputs execute fewer)."""
     if wid < 0:
@@ -245,11 +249,11 @@ def executed_flops_per_launch(c, kind, wid, nlaunch, npair, nap, alg_flops):
     while nz * 16 < w_:
         nz *= 2
     if kind == 7 and nt_ == 512 and nz in COLFFT2_FLOPS_PER_COLUMN:
-        return nwin * c["nf"] * COLFFT2_FLOPS_PER_COLUMN[nz] / nlaunch
+        return nwin * c["nf"] * (COLFFT2_SKIP_FLOPS_PER_COLUMN if cand_only else COLFFT2_FLOPS_PER_COLUMN)[nz] / nlaunch
     return alg_flops
 
 
-def executed_ops_per_launch(c, kind, wid, nlaunch, npair, nap):
+def executed_ops_per_launch(c, kind, wid, nlaunch, npair, nap, cand_only=False):
     """FP32 lane-operations per launch (see SLIDE_OPS_PER_BIN), or None for kernels without a counter capture."""
     if wid < 0:
         return None
@@ -261,7 +265,7 @@ def executed_ops_per_launch(c, kind, wid, nlaunch, npair, nap):
     while nz * 16 < w_:
         nz *= 2
     if kind == 7 and nt_ == 512 and nz in COLFFT2_OPS_PER_COLUMN:
-        return nwin * c["nf"] * COLFFT2_OPS_PER_COLUMN[nz] / nlaunch
+        return nwin * c["nf"] * (COLFFT2_SKIP_OPS_PER_COLUMN if cand_only else COLFFT2_OPS_PER_COLUMN)[nz] / nlaunch
     return None
 
 
@@ -421,12 +425,13 @@ def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traff
         dom_alg = per_w_alg[dom[1]] / nlaunch[dom]
     else:
         dom_alg = 0.0
-    exec_flops = executed_flops_per_launch(c, dom[0], dom[1], nlaunch[dom], nbl * nif, nap, dom_alg)
+    cand_only = peaks is None              # default options: no dense peak array = the candidates-only index mode
+    exec_flops = executed_flops_per_launch(c, dom[0], dom[1], nlaunch[dom], nbl * nif, nap, dom_alg, cand_only)
     peak_tf = peak["tflops"]
     exec_tf = exec_flops / (dom_ms_avg * 1e-3) / 1e12
     alg_tf = dom_alg / (dom_ms_avg * 1e-3) / 1e12
     tr = traffic.get((c["id"], KIND_NAMES.get(dom[0], ""), c["widths"][dom[1]] if dom[1] >= 0 else -1))
-    ops = executed_ops_per_launch(c, dom[0], dom[1], nlaunch[dom], nbl * nif, nap)
+    ops = executed_ops_per_launch(c, dom[0], dom[1], nlaunch[dom], nbl * nif, nap, cand_only)
     roofline = {
         "bound": "alu", "kernel": kname, "achieved": exec_tf, "peak": peak_tf, "unit": "TFLOP/s",
         "frac": exec_tf / peak_tf, "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None,

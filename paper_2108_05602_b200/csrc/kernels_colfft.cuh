@@ -32,6 +32,9 @@ struct ColFftArgs {
   int wpc;              // windows per CTA (consecutive)
   int nrange;           // ceil(nwin / wpc)
   uint32_t keymask;     // 0xFFFFFFF0 (register operand of the single-LOP3 key tag)
+  // k_colfft2 SKIP (candidates-only mode): pre-threshold of every window of the chunk as float bits (k_winthr),
+  // thr[pl * per_pair + offc + j]; nullptr = every (rate residue, column) is transformed
+  const uint32_t *thr;
 };
 
 // L1 = Nt/16 (2..32), NZ = leading non-zero inputs of the L1-point transform (power of two <= L1).

@@ -128,7 +128,15 @@ __device__ __forceinline__ void cf2_pass1(const f32x2 (&zx)[NZ], const f32x2 (&z
 #define CF2_MIN_CTAS8 2   // CTAs per SM the CP = 8 variant is compiled for (register cap 128)
 #endif
 // CP = column pairs per CTA (16: a 32-column strip, 512 threads; 8: a 16-column strip, 256 threads, several CTAs per SM)
-template <int L1, int NZ, int CP>
+// SKIP (candidates-only mode): pass 2 of a (rate residue rho, column) is left out when none of its 16 bins can reach the
+// window's pre-threshold.  The bins are F[rho + L1 s] = sum_{t2 < 16} W_16^{s t2} W_Nt^{rho t2} S[rho][t2]: unit-modulus
+// multiples of the 16 pass-1 sums the thread has just loaded, so by the triangle and Cauchy-Schwarz inequalities
+//   |F[rho + L1 s]|^2 <= (sum_t2 |S[rho][t2]|)^2 <= 16 sum_t2 |S[rho][t2]|^2      for every s.
+// For noise the right-hand side lies about 4.8 deviations below the pre-threshold (0.98 of the power a candidate needs)
+// whatever the width, so nearly every warp skips the twiddles, the 16-point transform and the powers; a window none of
+// whose (rho, column) is evaluated keeps the zero key (not a candidate - all the mode promises).  A candidate's peak
+// exceeds the pre-threshold, hence its (rho, column) passes the test and is evaluated exactly as without SKIP.
+template <int L1, int NZ, int CP, bool SKIP = false>
 __global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : CP == 4 ? 2 * CF2_MIN_CTAS8 : 1) k_colfft2(ColFftArgs a) {
   static_assert(L1 == 16 || L1 == 32, "Nt = 256 or 512");
   static_assert(CP == 16 || CP == 8 || CP == 4, "strip of 32, 16 or 8 columns");
@@ -190,16 +198,42 @@ __global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : CP == 4 ? 2
     half_barrier();
     if (p2_active) {
       f32x2 X[16], Y[16];
+      bool go = true;
+      if constexpr (SKIP) {
+        const float thrj = __uint_as_float(__ldg(a.thr + pl * a.per_pair + a.offc + j));
+        f32x2 e = pk(0.f, 0.f);
 #pragma unroll
-      for (int k = 0; k < 16; ++k) {
-        f32x2 zx2, zy2, wx, wy;
-        cf2_lds(ssrc + (uint32_t)k * (16u * CP), zx2, zy2);
-        if (k == 0) { X[0] = zx2; Y[0] = zy2; continue; }   // W^0 = 1
-        cf2_lds(twsrc + (uint32_t)k * (16u * G), wx, wy);
-        // z * w = (zx wx - zy wy) + i (zx wy + zy wx)
-        X[k] = fma2(zx2, wx, mul2(zy2, neg2(wy)));
-        Y[k] = fma2(zx2, wy, mul2(zy2, wx));
+        for (int k = 0; k < 16; ++k) {
+          cf2_lds(ssrc + (uint32_t)k * (16u * CP), X[k], Y[k]);
+          e = fma2(X[k], X[k], e);
+          e = fma2(Y[k], Y[k], e);
+        }
+        go = __any_sync(0xffffffffu, 16.0016f * fmaxf(lo32(e), hi32(e)) > thrj);   // warp-uniform
+        if (go) {
+#pragma unroll
+          for (int k = 1; k < 16; ++k) {
+            f32x2 wx, wy;
+            cf2_lds(twsrc + (uint32_t)k * (16u * G), wx, wy);
+            const f32x2 zx2 = X[k], zy2 = Y[k];
+            X[k] = fma2(zx2, wx, mul2(zy2, neg2(wy)));
+            Y[k] = fma2(zx2, wy, mul2(zy2, wx));
+          }
+        } else if (lane == 0) {
+          slots[warp] = 0ull;
+        }
+      } else {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+          f32x2 zx2, zy2, wx, wy;
+          cf2_lds(ssrc + (uint32_t)k * (16u * CP), zx2, zy2);
+          if (k == 0) { X[0] = zx2; Y[0] = zy2; continue; }   // W^0 = 1
+          cf2_lds(twsrc + (uint32_t)k * (16u * G), wx, wy);
+          // z * w = (zx wx - zy wy) + i (zx wy + zy wx)
+          X[k] = fma2(zx2, wx, mul2(zy2, neg2(wy)));
+          Y[k] = fma2(zx2, wy, mul2(zy2, wx));
+        }
       }
+      if (go) {
       FftDifS<16, 16, 0, 16>::run(X, Y);
       // untagged maximum (as k_slide for w >= 16): power and the delay column; the rate bin among the 16 of (rho, column)
       // is k_recover's exact re-evaluation (key = power bits, 2^31 | plane index of the column's bin s = 0)
@@ -217,6 +251,7 @@ __global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : CP == 4 ? 2
       if (lane == __ffs(tied) - 1)
         slots[warp] = ((u64)km << 32) |
                       (u64)(0xFFFFFFFFu - (0x80000000u | (rho * (uint32_t)a.nf + (uint32_t)(tile * 2 * CP + 2 * cp) + (colb ? 1u : 0u))));
+      }
     }
     half_barrier();
     if (warp == hb) {   // warps 0 and 1: the slots of their parity

@@ -73,13 +73,15 @@ static cudaError_t colfft_one(const ColFftArgs &a, unsigned blocks, cudaStream_t
     if (attr_only) {
       cudaError_t e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem16);
       if (e == cudaSuccess) e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem8);
+      if (e == cudaSuccess) e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem8);
       if (e == cudaSuccess) e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem4);
       if (e != cudaSuccess) return e;
     } else if (a.split2 == 4) {   // 8-column strips: four times the CTAs, 128 threads each
       k_colfft2<L1, NZ, 4><<<blocks * 4, 128, smem4, st>>>(a);
       return cudaSuccess;
     } else if (a.split2 == 2) {   // 16-column strips: twice the CTAs, 256 threads each
-      k_colfft2<L1, NZ, 8><<<blocks * 2, 256, smem8, st>>>(a);
+      if (a.thr) k_colfft2<L1, NZ, 8, true><<<blocks * 2, 256, smem8, st>>>(a);   // candidates-only mode: pass 2 only where needed
+      else k_colfft2<L1, NZ, 8><<<blocks * 2, 256, smem8, st>>>(a);
       return cudaSuccess;
     } else if (cf2) {
       k_colfft2<L1, NZ, 16><<<blocks, CF_WARPS * 32, smem16, st>>>(a);
@@ -841,6 +843,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         fa.per_pair = s.per_pair; fa.offc = s.offc[q]; fa.pair0 = pair0;
         fa.nap = s.nap; fa.nf = s.nf; fa.w = w.w; fa.stride = w.s; fa.nt = w.nt; fa.nwin = (int)w.nwin;
         fa.pitch = pl->pitch; fa.paired = pl->paired; fa.split2 = pl->cf_split2; fa.wpc = w.cf_wpc; fa.nrange = w.cf_nrange; fa.keymask = 0xFFFFFFF0u;
+        fa.thr = hy && w.untag ? (const uint32_t *)(ws + pl->off_thr) : nullptr;
         ProfScope ps(pl, st, VOLKS_K_COLFFT, q);
         if (!cuda_ok(launch_colfft(fa, w.cf_l1, w.cf_nz, np * (s.nf / 32) * w.cf_nrange, st, false))) return VOLKS_ECUDA;
         continue;
