@@ -213,7 +213,7 @@ def aggregate_value(world, units_per_rank, ms_step):
 
 
 KIND_NAMES = {1: "row_fft", 2: "col", 3: "finalize", 4: "scan", 5: "scatter", 6: "slide", 7: "colfft", 8: "allif", 9: "fixup",
-              10: "winthr", 11: "bound", 12: "recover", 13: "coleval"}
+              10: "winthr", 11: "bound", 12: "recover", 13: "coleval", 14: "sfold", 15: "sfold_eval"}
 
 
 # Executed flops per unit, pinned by ncu (profiles/r02_counters.md: sm__sass_thread_inst_executed_op_fp32_pred_on counts a

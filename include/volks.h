@@ -267,6 +267,8 @@ int volks_plan_launch_count(const volks_plan *plan);
 #define VOLKS_K_FIXUP 9    /* exact re-evaluation of the sliding widths' outlier windows               */
 #define VOLKS_K_WINTHR 10  /* per-window pre-thresholds of the candidates-only index mode              */
 #define VOLKS_K_BOUND 11   /* amplitude-sum bound: which segments of the narrow widths can hold candidates */
+#define VOLKS_K_SFOLD 14   /* candidates-only mode, wide stride-1 widths: folded sliding sum -> hit masks            */
+#define VOLKS_K_SFOLD_EVAL 15 /* ... exact transform of the flagged (window, rate residue, 64-column tile)s        */
 #define VOLKS_K_COLEVAL 13 /* one width by the definition in the (window, column) pairs the bound leaves          */
 #define VOLKS_K_RECOVER 12 /* peak bin of the stride-1 windows (w >= 16) by exact re-evaluation of one tile */
 int volks_plan_profile(volks_plan *plan, int enable);

@@ -36,6 +36,9 @@ struct FixArgs {
   // k_bound marked dense: cwdense[pl * cw_ntile + segment] (its segments are those tiles); cw_i = its index here or -1
   const unsigned char *cwdense;
   int cw_i, cw_ntile;
+  // a folded-sum width (kernels_sfold.cuh) in the candidates-only mode: sfdense[i][pl * nseg[i] + segment] = 1 for the
+  // segments the sliding kernel evaluated; nullptr = every segment
+  const unsigned char *sfdense[16];
 };
 
 // peak key of rate residue rho, column d of the window starting at row0 (already includes pair and t0)
@@ -78,6 +81,7 @@ __global__ void __launch_bounds__(256) k_fixup(FixArgs a) {
   for (int sg = sg_lo; sg < sg_hi; ++sg) {
   if (a.flags && a.flag_q[i] >= 0 && !a.flags[(pl * a.flag_nq + a.flag_q[i]) * a.flag_nseg + sg]) continue;
   if (a.cwdense && i == a.cw_i && !a.cwdense[pl * a.cw_ntile + sg]) continue;
+  if (a.sfdense[i] && !a.sfdense[i][pl * a.nseg[i] + sg]) continue;
   const int w = a.w[i], nt = a.nt[i], seg = a.seg[i];
   const int j0 = sg * seg, n = min(seg, a.nwin[i] - j0);          // windows j0 .. j0+n-1 (seg <= 256? see below)
   u64 *keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc[i]);

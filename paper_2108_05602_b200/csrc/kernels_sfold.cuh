@@ -1,0 +1,160 @@
+// kernels_sfold.cuh - the stride-1 rate transform in the candidates-only mode for the wide widths (Nt >= 64):
+// the sliding sum kept in FOLDED form, the transform done only where a candidate is possible.
+//
+// With the absolute-phase sum of kernels_slide.cuh, A[rho + M s] = sum_{t in window} y[t] W_Nt^{rho t} W_16^{s (t mod 16)}
+// (M = Nt / 16), the 16 rate bins of one (rate residue rho, delay column) are the 16-point DFT of the folded sums
+//   f[k] = sum_{t in window, t = k mod 16} y[t] W_Nt^{rho t},      A[rho + M s] = sum_{k < 16} W_16^{s k} f[k].
+// The window width is a multiple of 16, so sliding the window by one AP removes a sample from and adds a sample to the
+// SAME class k = t0 mod 16: ONE complex multiply-add per step,  f[k] += W_Nt^{rho t0} ((-1)^rho y[t0 + w] - y[t0]),
+// instead of the sixteen of k_slide.  The bins themselves are needed only where one of them can reach the window's
+// pre-threshold (k_winthr: 0.98 of the power a candidate needs), and every bin obeys the triangle inequality
+//   |A[rho + M s]| <= sum_k |f[k]| <= sum_k ( max(|x_k|, |y_k|) + (sqrt 2 - 1) min(|x_k|, |y_k|) ) =: e      (f[k] = x_k + i y_k),
+// the second step being an upper bound of |z| without a square root (the chord of sqrt(1 + r^2) on [0, 1]; within 8 %).
+// For noise e is a sum of 16 near-Rayleigh terms: mean 29.6, deviation 3.8 in units of sqrt(nchan) sigma sqrt(w / 64) x ...;
+// at snr_thresh 6 the amplitude pre-threshold (47.5 in the same units) lies 4.7 deviations above the mean at any width
+// with a near-Gaussian tail: about 1e-6 per column, 1e-4 of the (window, rho, 64-column tile) triples pass on noise.
+// (The Cauchy-Schwarz form 16 sum |f|^2 - a Gamma(16) tail - let 0.7 % pass and was measured at 3.5 % on configs[2].)
+//   k_slide<.., FOLD>  (kernels_slide.cuh) the fold is a MODE of the sliding kernel and inherits its operand path (the
+//                 cp.async shared-memory ring, twiddle rows at immediate offsets, loads one step ahead): warp = (pair,
+//                 segment, rho, 64-column tile), lane = column pair, state f[16] of both columns (packed FP32) and e.
+//                 Per step: k_slide's operand g, one packed complex add into f[t0 mod 16], e updated by the change of
+//                 that term (summed afresh every 16 steps), and ONE BIT: does e of either column of any lane exceed
+//                 the window's amplitude pre-threshold.  No branch, no key: per 16 windows the warp stores a 16-bit hit mask.
+//   k_sfold_density   per (pair, segment): more than 1/8 of the segment's hit bits set (interference: a tone raises |Y| in
+//                 every delay column) -> `dense`: the ordinary sliding kernel evaluates that segment (it costs 141 warp
+//                 instructions per 1024 bins of a window; an evaluation from the samples several times that).
+//   k_sfold_eval  the other segments: a warp reads 32 masks, ballots the non-zero ones and takes them in turn: the first
+//                 flagged window of the (rho, tile) is folded from its w samples, the following ones by sliding; at every
+//                 flagged window the 16-point transform of a copy, |.|^2, the first maximum in plane order: exact keys
+//                 (power, plane index), atomicMax per window.
+// A candidate has a bin above the pre-threshold, so its (rho, tile) is flagged and evaluated exactly; a window without a
+// flagged tile keeps the zero key (not a candidate - all the candidates-only mode promises, R6).
+#pragma once
+#include "common.cuh"
+#include "kernels_colfft2.cuh"   // FftDifS: split-format 16-point DIF
+
+namespace volks {
+
+struct SfoldArgs {
+  const float2 *Y;       // [pairs of the chunk][nap][pitch] pair-interleaved delay spectra
+  const float4 *tw4;     // [nt] rate twiddles exp(-2 pi i k/nt), pre-broadcast (re, re, im, im)
+  const unsigned short *hits;   // [pairs of the chunk][nblk][ndt][M] hit masks of k_slide<FOLD>: bit B = window 16 blk + B
+  unsigned char *dense;  // [pairs of the chunk][nseg]
+  u64 *keys;             // canonical window keys
+  long long ntasks;      // k_sfold_eval: warps = pairs * nblk * ndt * M;  k_sfold_density: CTAs = pairs * nseg
+  long long per_pair, offc, pair0;
+  int nap, nf, w, nt, log2m, nwin, seg, nseg, pitch, nblk;
+  int ndt, dt_na, dt_a0, dt_b0;   // the 64-column groups worked on (restricted delay range), as in SlideArgs
+};
+
+__global__ void __launch_bounds__(128) k_sfold_density(SfoldArgs a) {
+  __shared__ int part[4];
+  const long long pl = blockIdx.x / a.nseg;
+  const int sg = (int)(blockIdx.x % a.nseg);
+  const int wps = (a.ndt << a.log2m);                       // words per block of 16 windows
+  const int blk0 = sg * (a.seg >> 4), blk1 = min(a.nblk, blk0 + (a.seg >> 4));
+  const unsigned short *h = a.hits + ((size_t)pl * a.nblk + blk0) * wps;
+  const int nwords = (blk1 - blk0) * wps;
+  int n = 0;
+  for (int i = threadIdx.x; i < nwords; i += 128) n += __popc((unsigned)h[i]);
+#pragma unroll
+  for (int o = 16; o >= 1; o >>= 1) n += __shfl_xor_sync(0xffffffffu, n, o);
+  if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = n;
+  __syncthreads();
+  if (threadIdx.x == 0) a.dense[pl * a.nseg + sg] = (unsigned char)((part[0] + part[1] + part[2] + part[3]) * 8 > nwords * 16 ? 1 : 0);
+}
+
+// ONE warp per CTA (a CTA's registers are released only when all its warps are done, and nearly every warp is done at
+// once).  The warp reads 32 consecutive hit words in one coalesced load, ballots the non-zero ones of segments the
+// sliding kernel does not have, and works through those one after the other (each needs the whole warp).
+__global__ void __launch_bounds__(32) k_sfold_eval(SfoldArgs a) {
+  const uint32_t lane = threadIdx.x & 31u;
+  const long long w0 = (long long)blockIdx.x * 32 + lane;              // this lane's hit word (pair, block, tile, rho)
+  const int M = 1 << a.log2m;
+  uint32_t mymask = 0;
+  if (w0 < a.ntasks) {
+    mymask = a.hits[w0];
+    if (mymask) {
+      const long long q = (w0 >> a.log2m) / a.ndt;                     // pair * nblk + block
+      if (a.dense[(q / a.nblk) * a.nseg + (int)((q % a.nblk) / (a.seg >> 4))]) mymask = 0;   // the sliding kernel has this segment
+    }
+  }
+  uint32_t todo = __ballot_sync(0xffffffffu, mymask != 0);
+  for (; todo; todo &= todo - 1) {
+  const int src = __ffs(todo) - 1;
+  uint32_t mask = __shfl_sync(0xffffffffu, mymask, src);
+  long long wt = (long long)blockIdx.x * 32 + src;
+  const uint32_t rho = (uint32_t)(wt & (M - 1)); wt >>= a.log2m;
+  const int dti = (int)(wt % a.ndt); wt /= a.ndt;
+  const int dt = dti < a.dt_na ? a.dt_a0 + dti : a.dt_b0 + (dti - a.dt_na);
+  const uint32_t blk = (uint32_t)(wt % a.nblk);
+  const long long pl = wt / a.nblk;
+  const uint32_t c = (uint32_t)dt * 32u + lane;                        // column pair (2c, 2c + 1): one 128-bit load per row
+  const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch) + (size_t)c * 16u;
+  const size_t rowb = (size_t)a.pitch * 8u;
+  const char *tw4 = (const char *)a.tw4;
+  u64 *keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
+  const uint32_t ntm = (uint32_t)(a.nt - 1);
+  // from the first to the last flagged window of the word: fold the first from its samples (absolute phase: f[k] is the
+  // class (t + k) mod 16 of window t), then slide window by window - ONE sum changes per step, kept at index 0 by rotating
+  // f; a rotation multiplies every bin of the 16-point transform by a unit phase, so the powers do not notice it
+  const int first = __ffs(mask) - 1, last = 31 - __clz(mask);
+  const float sg1 = (rho & 1u) ? -1.f : 1.f;
+  const f32x2 sgn2 = pk(sg1, sg1);
+  f32x2 X[16], Yv[16];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) { X[k] = pk(0.f, 0.f); Yv[k] = pk(0.f, 0.f); }
+  {
+    const uint32_t t0 = blk * 16u + (uint32_t)first;
+    for (uint32_t tb = 0; tb < (uint32_t)a.w; tb += 16) {
+#pragma unroll
+      for (int k = 0; k < 16; ++k) {
+        f32x2 yx, yy, twx, twy;
+        ldg2(ybase + (size_t)(t0 + tb + k) * rowb, yx, yy);
+        ldg2(tw4 + (((rho * (t0 + tb + k)) & ntm) << 4), twx, twy);
+        X[k] = fma2(yx, twx, fma2(yy, neg2(twy), X[k]));
+        Yv[k] = fma2(yx, twy, fma2(yy, twx, Yv[k]));
+      }
+    }
+  }
+  for (int b = first;; ++b) {
+    const uint32_t t = blk * 16u + (uint32_t)b;
+    if ((mask >> b) & 1u) {
+      f32x2 GX[16], GY[16];
+#pragma unroll
+      for (int k = 0; k < 16; ++k) { GX[k] = X[k]; GY[k] = Yv[k]; }
+      FftDifS<16, 16, 0, 16>::run(GX, GY);
+      u64 key = 0;
+#pragma unroll
+      for (int s = 0; s < 16; ++s) {                                   // plane order: bins r = rho + M s, then the column
+        const int o = brev<16>(s);                                     // output o holds bin s
+        const f32x2 pw = fma2(GY[o], GY[o], mul2(GX[o], GX[o]));
+        const uint32_t idx = (rho + ((uint32_t)s << a.log2m)) * (uint32_t)a.nf + 2u * c;
+        const u64 ka = make_key(lo32(pw), idx), kb = make_key(hi32(pw), idx + 1u);
+        key = ka > key ? ka : key;
+        key = kb > key ? kb : key;
+      }
+#pragma unroll
+      for (int o = 16; o >= 1; o >>= 1) {
+        const u64 other = __shfl_xor_sync(0xffffffffu, key, o);
+        key = other > key ? other : key;
+      }
+      if (lane == 0) atomicMax(keyp + t, key);
+    }
+    if (b == last) break;
+    // window t -> t + 1: sample t leaves, sample t + w enters, both of the class now at index 0
+    f32x2 xin, yin, xout, yout, twx, twy;
+    ldg2(ybase + (size_t)(t + a.w) * rowb, xin, yin);
+    ldg2(ybase + (size_t)t * rowb, xout, yout);
+    ldg2(tw4 + (((rho * t) & ntm) << 4), twx, twy);
+    const f32x2 dx = fma2(xin, sgn2, neg2(xout)), dy = fma2(yin, sgn2, neg2(yout));
+    const f32x2 nx = add2(X[0], fma2(dx, twx, mul2(dy, neg2(twy))));
+    const f32x2 ny = add2(Yv[0], fma2(dx, twy, mul2(dy, twx)));
+#pragma unroll
+    for (int k = 0; k < 15; ++k) { X[k] = X[k + 1]; Yv[k] = Yv[k + 1]; }
+    X[15] = nx; Yv[15] = ny;
+  }
+  }
+}
+
+}  // namespace volks

@@ -57,6 +57,11 @@ struct SlideArgs {
   // restricted delay range: only the 64-column groups that hold searched bins are worked on.  ndt groups in two
   // pieces: group i < dt_na is column group dt_a0 + i, the others dt_b0 + (i - dt_na) (whole axis: ndt = nf / 64)
   int ndt, dt_na, dt_a0, dt_b0;
+  // FOLD mode (kernels_sfold.cuh): pre-thresholds (float bits), chunk-relative thr[pl * per_pair + offc + t0], and
+  // the hit masks [pairs of the chunk][nblk][ndt][M] it writes (bit B of a word = window 16 blk + B)
+  const uint32_t *thr;
+  unsigned short *hits;
+  int nblk;
   // pruned widths (kernels_prune.cuh): flags[pl * flag_stride + segment] == 0 means no window of the segment can be
   // a candidate - the CTA returns at once; nullptr = every segment is evaluated
   const unsigned char *flags;
@@ -97,6 +102,13 @@ __device__ __forceinline__ void cmac2_w16(f32x2 &X, f32x2 &Y, const SlideG &G) {
   }
 }
 
+// FOLD mode: an upper bound of |z| for both columns of a packed complex value without a square root:
+//   |z| <= max(|x|, |y|) + (sqrt 2 - 1) min(|x|, |y|)   (the chord of the convex sqrt(1 + r^2) on r in [0, 1]; within 8 %)
+__device__ __forceinline__ f32x2 fold_oct(f32x2 X, f32x2 Y) {
+  const float xa = fabsf(lo32(X)), ya = fabsf(lo32(Y)), xb = fabsf(hi32(X)), yb = fabsf(hi32(Y));
+  return pk(fmaf(0.41421357f, fminf(xa, ya), fmaxf(xa, ya)), fmaf(0.41421357f, fminf(xb, yb), fmaxf(xb, yb)));
+}
+
 // One warp's state while it walks a segment of consecutive windows.
 template <int L>
 struct SlideState {
@@ -115,6 +127,12 @@ struct SlideState {
   // first leaving row (sm_out) and first entering row (sm_in); ring geometry in bytes
   uint32_t sm_out, sm_in, ring_lo, ring_hi, rrowb;
   uint32_t twp, tw_lo, tw_hi;   // RING: this warp's twiddle row W_Nt^{rho t}, t = 0..Nt (shared memory), entry of the current block
+  // FOLD mode: X / Y hold the folded sums f[k] (k = t mod 16) instead of the bins; e = sum_k fold_oct(f[k]) >= sum_k |f[k]|
+  // of both columns, mask = this block's hit bits, mythr = lane B's copy of the AMPLITUDE pre-threshold of window (block
+  // start + B), lowered by 1e-3 for the rounding of e
+  f32x2 e;
+  uint32_t mask;
+  float mythr;
 };
 
 // emit the window's contribution: per column the max of (power with its 4 low mantissa bits replaced
@@ -220,7 +238,7 @@ __device__ __forceinline__ void slide_prefetch(SlideState<L> &S, uint32_t t) {
 
 // advance window t0 -> t0+1;  B = t0 mod L (compile time).  Uses the operands prefetched one step
 // ago and prefetches those of t0+1.
-template <int L, int B, bool MODD, bool RING, int RR>
+template <int L, int B, bool MODD, bool RING, int RR, bool FOLD = false>
 __device__ __forceinline__ void slide_update(SlideState<L> &S, uint32_t t0) {
   const f32x2 xin = S.xin, yin = S.yin, xout = S.xout, yout = S.yout, twx = S.twx, twy = S.twy;
   slide_prefetch<L, MODD, RING, B + 1, RR>(S, t0 + 1);
@@ -234,23 +252,35 @@ __device__ __forceinline__ void slide_update(SlideState<L> &S, uint32_t t0) {
     const f32x2 dx = fma2(xin, S.sgn2, neg2(xout)), dy = fma2(yin, S.sgn2, neg2(yout));
     const f32x2 gx = fma2(dx, twx, mul2(dy, neg2(twy)));
     const f32x2 gy = fma2(dx, twy, mul2(dy, twx));
-    const SlideG G = slide_make_g(gx, gy);
-    SlideBins<L, B, 0>::run(S, G, G);
+    if constexpr (FOLD) {
+      // the leaving and the entering sample share the class B = t0 mod 16 (w is a multiple of 16): ONE sum changes
+      const f32x2 eo = fold_oct(S.X[B], S.Y[B]);
+      S.X[B] = add2(S.X[B], gx); S.Y[B] = add2(S.Y[B], gy);
+      S.e = add2(sub2(S.e, eo), fold_oct(S.X[B], S.Y[B]));
+    } else {
+      const SlideG G = slide_make_g(gx, gy);
+      SlideBins<L, B, 0>::run(S, G, G);
+    }
   }
 }
 
 // L consecutive steps starting at t0 (t0 mod L == 0).  GUARD: only windows < tend exist.
-template <int L, int B, bool MODD, bool GUARD, bool RING, int RR>
+template <int L, int B, bool MODD, bool GUARD, bool RING, int RR, bool FOLD = false>
 struct SlideSteps {
   static __device__ __forceinline__ void run(SlideState<L> &S, uint32_t t0, uint32_t tend, u64 *slot) {
     if constexpr (B < L) {
       if (!GUARD || t0 + B < tend) {
+        if constexpr (FOLD) {
+          // every bin of (rho, column) obeys |A| <= sum_k |f[k]| <= e (kernels_sfold.cuh): one bit per window, no branch
+          const float thrB = __shfl_sync(0xffffffffu, S.mythr, B);
+          if (__any_sync(0xffffffffu, fmaxf(lo32(S.e), hi32(S.e)) > thrB)) S.mask |= 1u << B;
+        }
         // M == 1 (w <= 8): tagged keys, exact index at once; M >= 2: power + tile id, index by k_recover
-        if constexpr (MODD) slide_emit<L>(S, slot + B * SLIDE_WARPS);
+        else if constexpr (MODD) slide_emit<L>(S, slot + B * SLIDE_WARPS);
         else slide_emit_u<L>(S, slot + B * SLIDE_WARPS);
-        if (!GUARD || t0 + B + 1 < tend) slide_update<L, B, MODD, RING, RR>(S, t0 + B);
+        if (!GUARD || t0 + B + 1 < tend) slide_update<L, B, MODD, RING, RR, FOLD>(S, t0 + B);
       }
-      SlideSteps<L, B + 1, MODD, GUARD, RING, RR>::run(S, t0, tend, slot);
+      SlideSteps<L, B + 1, MODD, GUARD, RING, RR, FOLD>::run(S, t0, tend, slot);
     }
   }
 };
@@ -258,7 +288,7 @@ struct SlideSteps {
 // exact transform of window T0 for ONE column (col = 0/1 of the pair):
 //   A[rho + M s] = sum_{t2<L} W_L^{s t2} f[t2],  f[t2] = sum_{t1} y[T0+t2+L t1] W_Nt^{rho (t2+L t1)}
 // (T0 = 0 mod Nt, so absolute and window-relative phases coincide).  Result in natural s order.
-template <int L, bool MODD>
+template <int L, bool MODD, bool FOLD = false>
 __device__ __forceinline__ void slide_start_column(float2 (&A)[L], const char *pout, uint32_t rowb, uint32_t T0,
                                                    uint32_t w, const float2 *twt, uint32_t rho, uint32_t ntmask, int col) {
   float2 f[L];
@@ -275,6 +305,11 @@ __device__ __forceinline__ void slide_start_column(float2 (&A)[L], const char *p
         else cmac(f[t2], y, __ldg(twt + ((rho * t) & ntmask)));
       }
     }
+  }
+  if constexpr (FOLD) {      // the folded sums themselves (class t2 = t mod L)
+#pragma unroll
+    for (int s = 0; s < L; ++s) A[s] = f[s];
+    return;
   }
   FftDif<L, 0, L>::run(f);
 #pragma unroll
@@ -307,7 +342,8 @@ __device__ __forceinline__ void slide_ring_fill(const SlideRing &G, uint32_t r0,
 }
 
 // L = min(16, Nt) bins per thread;  MODD <=> M == 1 (Nt <= 16);  RING (M >= 4 only): rows through shared memory.
-template <int L, bool MODD, bool RING, int RR = 0>
+// FOLD (M >= 4, candidates-only mode): the folded-sum form of kernels_sfold.cuh - no bins, no keys, one hit bit per window
+template <int L, bool MODD, bool RING, int RR = 0, bool FOLD = false>
 __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(SlideArgs a) {
   // blockDim.x = 32 * min(SLIDE_WARPS, ndt * M): every warp of a CTA works on the same (pair, segment)
   __shared__ u64 slots[2][16 * SLIDE_WARPS];
@@ -373,20 +409,40 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   slide_prefetch<L, MODD, RING, 0, RR>(S, T0);
   {
     float2 Aa[L], Ab[L];
-    slide_start_column<L, MODD>(Aa, S.pout, S.rowb, T0, (uint32_t)a.w, a.twt, S.rho, S.ntmask, 0);
-    slide_start_column<L, MODD>(Ab, S.pout, S.rowb, T0, (uint32_t)a.w, a.twt, S.rho, S.ntmask, 1);
+    slide_start_column<L, MODD, FOLD>(Aa, S.pout, S.rowb, T0, (uint32_t)a.w, a.twt, S.rho, S.ntmask, 0);
+    slide_start_column<L, MODD, FOLD>(Ab, S.pout, S.rowb, T0, (uint32_t)a.w, a.twt, S.rho, S.ntmask, 1);
 #pragma unroll
     for (int s = 0; s < L; ++s) { S.X[s] = pk(Aa[s].x, Ab[s].x); S.Y[s] = pk(Aa[s].y, Ab[s].y); }
   }
 
+  [[maybe_unused]] const uint32_t *thrp = nullptr;
+  [[maybe_unused]] unsigned short *hp = nullptr;
+  if constexpr (FOLD) {
+    thrp = a.thr + (pl * a.per_pair + a.offc);
+    hp = a.hits + (((size_t)pl * a.nblk) * ndt + dti) * M + S.rho;      // + blk * ndt * M
+  }
   uint32_t t0 = T0, buf = 0;
   for (;; t0 += L, buf ^= 1u) {
     const bool full = t0 + L < tend;
     if constexpr (RING) slide_ring_fill(G, t0 - T0 + (uint32_t)a.w + 17u, 16u);   // the next block's new rows
-    if (full) SlideSteps<L, 0, MODD, false, RING, RR>::run(S, t0, tend, &slots[buf][warp]);
-    else SlideSteps<L, 0, MODD, true, RING, RR>::run(S, t0, tend, &slots[buf][warp]);
+    if constexpr (FOLD) {
+      S.mythr = (lane < (uint32_t)L && t0 + lane < tend) ? 0.999f * sqrtf(__uint_as_float(__ldg(thrp + t0 + lane))) : 3.0e38f;
+      if ((((t0 - T0) >> 4) & 3u) == 0u) {       // summed afresh every 64 steps (the updates in between drift by ~1e-5)
+        S.e = pk(0.f, 0.f);
+#pragma unroll
+        for (int k = 0; k < L; ++k) S.e = add2(S.e, fold_oct(S.X[k], S.Y[k]));
+      }
+      S.mask = 0;
+    }
+    if (full) SlideSteps<L, 0, MODD, false, RING, RR, FOLD>::run(S, t0, tend, &slots[buf][warp]);
+    else SlideSteps<L, 0, MODD, true, RING, RR, FOLD>::run(S, t0, tend, &slots[buf][warp]);
     if constexpr (RING) asm volatile("cp.async.wait_all;" ::: "memory");
-    slide_flush(S.keyp, slots[buf], t0, full ? (uint32_t)L : tend - t0, nwarps);
+    if constexpr (FOLD) {
+      if (lane == 0) hp[(size_t)(t0 >> 4) * (size_t)(ndt * M)] = (unsigned short)S.mask;
+      if constexpr (RING) __syncthreads();       // the ring rows of the next block are complete and visible
+    } else {
+      slide_flush(S.keyp, slots[buf], t0, full ? (uint32_t)L : tend - t0, nwarps);
+    }
     if (!full) break;
     if constexpr (RING) {   // advance the block base by 16 rows (wraps only at a block boundary)
       S.sm_out += 16u * S.rrowb; S.sm_out = S.sm_out >= S.ring_hi ? S.sm_out - (S.ring_hi - S.ring_lo) : S.sm_out;

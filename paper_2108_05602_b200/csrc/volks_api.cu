@@ -20,6 +20,7 @@
 #include "kernels_prune.cuh"
 #include "kernels_recover.cuh"
 #include "kernels_coleval.cuh"
+#include "kernels_sfold.cuh"
 
 using namespace volks;
 
@@ -50,6 +51,10 @@ struct WidthPlan {
   bool untag;           // sliding path with M >= 2 (Nt >= 32): untagged kernel, peak bin by k_recover
   int prune;            // sliding path: index among the plan's pruned widths (kernels_prune.cuh), or -1
   bool cw;              // sliding path: the plan's column-level width (kernels_coleval.cuh)
+  bool sf;              // sliding path, candidates-only mode: folded sliding sum + evaluation of the flagged tiles (kernels_sfold.cuh)
+  size_t off_hits;      // ... its hit masks in the workspace
+  size_t off_sfdense;   // ... its per-segment density flags
+  int nblk;             // ... blocks of 16 windows per pair
 };
 
 template <int L>
@@ -190,7 +195,8 @@ static bool launch_row2(const RowArgs &a, cudaStream_t st) {
   return row2_nz<8, 8>(a, nza, blocks, st);
 }
 
-static void launch_slide(const SlideArgs &a, cudaStream_t st) {
+// fold: the FOLD mode of the kernel (kernels_sfold.cuh; Nt >= 64 only: M >= 4)
+static void launch_slide(const SlideArgs &a, cudaStream_t st, bool fold = false) {
   // every warp of a CTA must share its (pair, segment): warps per CTA = min(SLIDE_WARPS, ndt * M)
   const long long per_seg = (long long)a.ndt << a.log2m;
   int wpb = SLIDE_WARPS;                         // the largest power of two <= 8 that divides the warps of a segment
@@ -203,10 +209,17 @@ static void launch_slide(const SlideArgs &a, cudaStream_t st) {
     // + the warps' twiddle rows ([wpb][Nt + 1] float4) behind the ring
     const size_t ring = (size_t)(a.w + 48) * 512 * dtc + (size_t)wpb * (a.nt + 1) * 16;
     if (a.log2m >= 2 && ring <= 100 * 1024) {
-      if (dtc == 1) k_slide<16, false, true, 512><<<blocks, thr, ring, st>>>(a);
-      else if (dtc == 2) k_slide<16, false, true, 1024><<<blocks, thr, ring, st>>>(a);
-      else k_slide<16, false, true><<<blocks, thr, ring, st>>>(a);
+      if (fold) {
+        if (dtc == 1) k_slide<16, false, true, 512, true><<<blocks, thr, ring, st>>>(a);
+        else if (dtc == 2) k_slide<16, false, true, 1024, true><<<blocks, thr, ring, st>>>(a);
+        else k_slide<16, false, true, 0, true><<<blocks, thr, ring, st>>>(a);
+      } else {
+        if (dtc == 1) k_slide<16, false, true, 512><<<blocks, thr, ring, st>>>(a);
+        else if (dtc == 2) k_slide<16, false, true, 1024><<<blocks, thr, ring, st>>>(a);
+        else k_slide<16, false, true><<<blocks, thr, ring, st>>>(a);
+      }
     }
+    else if (fold) k_slide<16, false, false, 0, true><<<blocks, thr, 0, st>>>(a);
     else k_slide<16, false, false><<<blocks, thr, 0, st>>>(a);
   }
   else if (a.nt == 16) k_slide<16, true, false><<<blocks, thr, 0, st>>>(a);
@@ -219,7 +232,10 @@ static bool slide_attrs() {
   const int lim = 100 * 1024;
   return cudaFuncSetAttribute(k_slide<16, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
          cudaFuncSetAttribute(k_slide<16, false, true, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
-         cudaFuncSetAttribute(k_slide<16, false, true, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess;
+         cudaFuncSetAttribute(k_slide<16, false, true, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
+         cudaFuncSetAttribute(k_slide<16, false, true, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
+         cudaFuncSetAttribute(k_slide<16, false, true, 512, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess &&
+         cudaFuncSetAttribute(k_slide<16, false, true, 1024, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess;
 }
 
 }  // namespace
@@ -239,6 +255,7 @@ struct volks_plan {
   int nuntag = 0;                // sliding widths with untagged kernels (their peak bins come from k_recover)
   bool cand_only = false;        // searches without d_peaks recover indices / evaluate segments for possible candidates only
   int nprune = 0, prune_nseg = 0, prune_seg = 0, prune_wmax = 0;   // pruned widths (k_bound): count, common segmentation
+  int nsf = 0;                   // widths on the folded-sum path in the candidates-only mode (kernels_sfold.cuh)
   int cwq = -1, cw_nwords = 0;   // the column-level width (index into wp) and the 32-window words of its bit mask per pair
   size_t off_cwmask = 0, off_cwdense = 0;
   int dt_n = 0, dt_na = 0, dt_a0 = 0, dt_b0 = 0;   // 64-column groups the sliding kernels / k_bound work on (restricted delay range)
@@ -422,6 +439,11 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
     if (w.prune < 0 && pl->cwq < 0 && w.slide && w.nt >= 32 && !opt.full_index && !opt.no_prune && p->snr_thresh > 0.f &&
         w.w <= PRUNE_RING && pl->nprune < PRUNE_MAXQ && p->nap >= w.w && w.nt <= 2 * PRUNE_RING && opt.prune_seg == 64 &&
         (0.99 * p->snr_thresh - 0.886 * sqrt((double)w.w)) / 0.4637 >= 1.5) { w.cw = true; pl->cwq = q; }
+    // folded sliding sum (kernels_sfold.cuh) for the wide stride-1 widths in the candidates-only mode: pays when noise
+    // stays below the Cauchy-Schwarz bound's test, 16 x Gamma(16): (0.98 snr_thresh^2 / 16 - 1) / 0.25 >= 4 deviations
+    w.sf = w.slide && w.nt >= 64 && w.prune < 0 && !w.cw && !opt.full_index && !opt.no_prune && p->snr_thresh > 0.f &&
+           (0.98 * p->snr_thresh * p->snr_thresh / 16.0 - 1.0) / 0.25 >= 4.0;
+    w.off_hits = 0; w.nblk = (int)((w.nwin + 15) / 16);
     w.cf_l1 = w.nt / 16;
     if (w.colfft && w.nt >= 256 && opt.cf2 != 0) w.untag = true;   // k_colfft2 keeps no bin tags either
     w.cf_nz = 1;
@@ -502,6 +524,8 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
       if ((!w.slide && !w.colfft && !allif && col_blocks > GMAX) || (w.slide && slide_blocks > GMAX) ||
           (w.colfft && cf_blocks > GMAX) || (allif && ai_blocks > GMAX)) fits = false;
     }
+    for (auto &w : pl->wp)     // k_sfold_eval: one warp per (block of 16 windows, 64-column group, rate residue)
+      if (w.sf && (long double)ppc_ * w.nblk * std::max(1, p->nf / 64) * (1 << w.log2m) > GMAX) fits = false;
     long long rec_warps = 0;
     for (auto &w : pl->wp) rec_warps += w.untag ? w.nwin : 0;
     if ((long double)ppc_ * rec_warps / 128 > GMAX) fits = false;    // k_recover: one thread per window
@@ -531,6 +555,14 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
   pl->cw_nwords = pl->cwq >= 0 ? (int)(((pl->prune_nseg + 1) / 2) * (2 * opt.prune_seg / 32)) : 0;
   pl->off_cwdense = off; off = align_up(off + (size_t)pl->pairs_per_chunk * ((pl->prune_nseg + 1) / 2) + 1, 256);
   pl->off_cwmask = off; off = align_up(off + (size_t)pl->pairs_per_chunk * pl->cw_nwords * p->nf * sizeof(uint32_t), 256);
+  for (auto &w : pl->wp) {      // hit masks of the folded-sum widths: [pairs of the chunk][nblk][64-column groups][M] u16
+    if (!w.sf || w.nwin == 0) { w.sf = false; continue; }
+    pl->nsf += 1;
+    w.off_hits = off;
+    off = align_up(off + (size_t)pl->pairs_per_chunk * w.nblk * pl->dt_n * (1 << w.log2m) * sizeof(unsigned short), 256);
+    w.off_sfdense = off;
+    off = align_up(off + (size_t)pl->pairs_per_chunk * w.nseg, 256);
+  }
   pl->off_Y = off;    off = align_up(off + (size_t)pl->pairs_per_chunk * std::max<size_t>(y_pair, 8) + (size_t)(SLIDE_PF + 2) * pl->pitch * sizeof(float2), 256);
   pl->ws_bytes = off;
 
@@ -542,7 +574,7 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
   for (int q = 0; q < p->nwidths; ++q) active += (pl->wp[q].nwin > 0 && q != pl->wid1) ? 1 : 0;
   // kernels of this library per search (the key memset is a driver memset, not counted)
   // (a search without dense peaks; with them the candidates-only index mode and its k_winthr launch are off)
-  pl->launches = s.nwin_total > 0 ? (int)(pl->nchunks * (1 + active + (pl->nslide > 0 ? 1 : 0) + ((pl->cand_only && (pl->nuntag || pl->nprune)) ? 1 : 0) + (pl->nprune ? 1 : 0) + (pl->nuntag ? 1 : 0)) + 3) : 0;
+  pl->launches = s.nwin_total > 0 ? (int)(pl->nchunks * (1 + active + (pl->nslide > 0 ? 1 : 0) + ((pl->cand_only && (pl->nuntag || pl->nprune)) ? 1 : 0) + ((pl->nprune || pl->cwq >= 0) ? 1 : 0) + (pl->nuntag ? 1 : 0) + (pl->cwq >= 0 ? 1 : 0) + 3 * pl->nsf) + 3) : 0;
 
   // tables, computed in double precision on the host
   if (psub > 1) { pl->premod_off = tw_total; tw_total += (size_t)s.nf; }
@@ -822,6 +854,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         else k_allif<4, false><<<blocks, thr, 0, st>>>(aa);
         continue;
       }
+      const bool fold = w.slide && w.sf && hy;   // candidates-only mode, wide stride-1 width (kernels_sfold.cuh)
       if (w.slide) {
         SlideArgs sa;
         sa.Y = Y; sa.keys = keys; sa.twt = pl->d_tables + w.tw_off; sa.tw4 = (const float4 *)(pl->d_tables + w.tw4_off);
@@ -833,6 +866,31 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         sa.flags = flags && w.prune >= 0 ? flags + (size_t)w.prune * pl->prune_nseg : nullptr;
         sa.flag_stride = (pl->nprune + (use_cw ? 1 : 0)) * pl->prune_nseg;
         if (hy && w.cw) { sa.flags = (const unsigned char *)(ws + pl->off_cwdense); sa.flag_stride = (pl->prune_nseg + 1) / 2; }   // dense tiles only
+        sa.thr = (const uint32_t *)(ws + pl->off_thr); sa.hits = nullptr; sa.nblk = w.nblk;
+        if (fold) {
+          // 1. the folded sliding sum: one hit bit per (window, rate residue, 64-column tile)
+          sa.hits = (unsigned short *)(ws + w.off_hits);
+          {
+            ProfScope ps(pl, st, VOLKS_K_SFOLD, q);
+            launch_slide(sa, st, true);
+          }
+          // 2. segments with more than 1/8 of their bits set (interference) go to the ordinary sliding kernel
+          SfoldArgs ea;
+          ea.Y = Y; ea.tw4 = (const float4 *)(pl->d_tables + w.tw4_off); ea.hits = sa.hits; ea.dense = (unsigned char *)(ws + w.off_sfdense); ea.keys = keys;
+          ea.per_pair = s.per_pair; ea.offc = s.offc[q]; ea.pair0 = pair0;
+          ea.nap = s.nap; ea.nf = s.nf; ea.w = w.w; ea.nt = w.nt; ea.log2m = w.log2m; ea.nwin = (int)w.nwin;
+          ea.seg = w.seg; ea.nseg = w.nseg; ea.pitch = pl->pitch; ea.nblk = w.nblk;
+          ea.ndt = pl->dt_n; ea.dt_na = pl->dt_na; ea.dt_a0 = pl->dt_a0; ea.dt_b0 = pl->dt_b0;
+          ea.ntasks = np * w.nseg;
+          {
+            ProfScope ps(pl, st, VOLKS_K_SFOLD_EVAL, q);
+            k_sfold_density<<<(unsigned)ea.ntasks, 128, 0, st>>>(ea);
+            // 3. every other flagged (window, rho, tile) exactly, from its samples
+            ea.ntasks = ((np * w.nblk * (long long)pl->dt_n) << w.log2m);
+            k_sfold_eval<<<(unsigned)((ea.ntasks + 31) / 32), 32, 0, st>>>(ea);
+          }
+          sa.hits = nullptr; sa.flags = ea.dense; sa.flag_stride = w.nseg;     // 4. the dense segments, below
+        }
         ProfScope ps(pl, st, VOLKS_K_SLIDE, q);
         launch_slide(sa, st);
         continue;
@@ -870,6 +928,8 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         if (!w.slide || w.nwin == 0) continue;
         const int i = fa.nq++;
         if (hy && w.cw) fa.cw_i = i;
+        // a folded-sum width: only its dense segments went through the sliding kernel (the others hold exact keys)
+        fa.sfdense[i] = hy && w.sf ? (const unsigned char *)(ws + w.off_sfdense) : nullptr;
         fa.q[i] = q; fa.w[i] = w.w; fa.nt[i] = w.nt; fa.seg[i] = w.seg; fa.nseg[i] = w.nseg; fa.nwin[i] = (int)w.nwin;
         fa.offc[i] = s.offc[q]; fa.tw_off[i] = (long long)w.tw_off; fa.flag_q[i] = w.prune;
         fa.unit0[i + 1] = fa.unit0[i] + (w.nseg + FIX_GROUP - 1) / FIX_GROUP;

@@ -130,3 +130,13 @@ def check_candidates_whole(gpu_cands, gidx, ora_cands, ora_peaks, keep, thresh):
     assert np.all(np.abs(g["power"].astype(np.float64) - o["power"]) <= RTOL * o["power"])
     assert np.all(np.abs(g["snr"].astype(np.float64) - o["snr"]) <= RTOL * o["snr"])
     return int(in_o.sum()), int(missing.size), int(extra.size), int(marginal.sum())
+
+
+def check_candidate_bins(gpu_cands, cidx, ora_peaks, nf, plane_power=None):
+    """The (rate, delay) bin, power and snr of candidate records against the oracle's peaks of the same windows
+    (`cidx` = canonical window index of every record), by the rules of check_peaks."""
+    gp = np.zeros(len(gpu_cands), dtype=[("power", "<f4"), ("snr", "<f4"), ("rate_idx", "<i4"), ("delay_idx", "<i4")])
+    for f in ("power", "snr", "rate_idx", "delay_idx"):
+        gp[f] = gpu_cands[f]
+    pp = None if plane_power is None else (lambda i, idx: plane_power(int(cidx[i]), idx))
+    return check_peaks(gp, ora_peaks[cidx], nf, pp)
