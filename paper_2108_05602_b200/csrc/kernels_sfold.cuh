@@ -35,6 +35,10 @@
 
 namespace volks {
 
+#ifndef SFOLD_SEGMUL
+#define SFOLD_SEGMUL 4            // segment of k_slide<FOLD> = this many segments of the sliding kernel
+#endif
+
 struct SfoldArgs {
   const float2 *Y;       // [pairs of the chunk][nap][pitch] pair-interleaved delay spectra
   const float4 *tw4;     // [nt] rate twiddles exp(-2 pi i k/nt), pre-broadcast (re, re, im, im)

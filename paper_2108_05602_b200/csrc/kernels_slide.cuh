@@ -128,11 +128,11 @@ struct SlideState {
   uint32_t sm_out, sm_in, ring_lo, ring_hi, rrowb;
   uint32_t twp, tw_lo, tw_hi;   // RING: this warp's twiddle row W_Nt^{rho t}, t = 0..Nt (shared memory), entry of the current block
   // FOLD mode: X / Y hold the folded sums f[k] (k = t mod 16) instead of the bins; e = sum_k fold_oct(f[k]) >= sum_k |f[k]|
-  // of both columns, mask = this block's hit bits, mythr = lane B's copy of the AMPLITUDE pre-threshold of window (block
-  // start + B), lowered by 1e-3 for the rounding of e
+  // of both columns; the AMPLITUDE pre-thresholds of the block's 16 windows (lowered by 1e-3 for the rounding of e) sit in
+  // shared memory - every warp of the CTA works on the same windows
   f32x2 e;
-  uint32_t mask;
-  float mythr;
+  uint32_t mask;                // this LANE's hit bits (OR-reduced over the warp at the end of the block)
+  uint32_t thrs;                // shared address of the current block's 16 amplitude thresholds (CTA-wide: one segment)
 };
 
 // emit the window's contribution: per column the max of (power with its 4 low mantissa bits replaced
@@ -271,9 +271,10 @@ struct SlideSteps {
     if constexpr (B < L) {
       if (!GUARD || t0 + B < tend) {
         if constexpr (FOLD) {
-          // every bin of (rho, column) obeys |A| <= sum_k |f[k]| <= e (kernels_sfold.cuh): one bit per window, no branch
-          const float thrB = __shfl_sync(0xffffffffu, S.mythr, B);
-          if (__any_sync(0xffffffffu, fmaxf(lo32(S.e), hi32(S.e)) > thrB)) S.mask |= 1u << B;
+          // every bin of (rho, column) obeys |A| <= sum_k |f[k]| <= e (kernels_sfold.cuh): one bit per window and lane, no branch
+          float thrB;                               // a broadcast shared-memory load: no warp collective in the steps
+          asm volatile("ld.shared.f32 %0, [%1];" : "=f"(thrB) : "r"(S.thrs + 4u * B));
+          if (fmaxf(lo32(S.e), hi32(S.e)) > thrB) S.mask |= 1u << B;
         }
         // M == 1 (w <= 8): tagged keys, exact index at once; M >= 2: power + tile id, index by k_recover
         else if constexpr (MODD) slide_emit<L>(S, slot + B * SLIDE_WARPS);
@@ -341,12 +342,29 @@ __device__ __forceinline__ void slide_ring_fill(const SlideRing &G, uint32_t r0,
   }
 }
 
+// the same for the 16 new rows of a block, rel in [r0, r0 + 16), whose first row sits in ring slot `slot` (kept by the
+// caller: no modulo); RR = bytes per ring row at compile time (a power of two: shifts for the row / chunk split), or 0
+template <int RR>
+__device__ __forceinline__ void slide_ring_fill_block(const SlideRing &G, uint32_t r0, uint32_t slot) {
+  const uint32_t cpr = RR ? (uint32_t)RR >> 4 : G.rrowb >> 4;
+  for (uint32_t i = threadIdx.x; i < 16u * cpr; i += blockDim.x) {
+    const uint32_t r = i / cpr, c = i - r * cpr;
+    uint32_t sl = slot + r;
+    sl = sl >= G.R ? sl - G.R : sl;
+    const uint32_t grow = min(G.T0 + r0 + r, G.nap);
+    const uint32_t dst = G.base + sl * (RR ? (uint32_t)RR : G.rrowb) + (c << 4);
+    const char *src = G.gsrc + (size_t)grow * G.rowb + (c << 4);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src));
+  }
+}
+
 // L = min(16, Nt) bins per thread;  MODD <=> M == 1 (Nt <= 16);  RING (M >= 4 only): rows through shared memory.
 // FOLD (M >= 4, candidates-only mode): the folded-sum form of kernels_sfold.cuh - no bins, no keys, one hit bit per window
 template <int L, bool MODD, bool RING, int RR = 0, bool FOLD = false>
 __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(SlideArgs a) {
   // blockDim.x = 32 * min(SLIDE_WARPS, ndt * M): every warp of a CTA works on the same (pair, segment)
   __shared__ u64 slots[2][16 * SLIDE_WARPS];
+  [[maybe_unused]] __shared__ float fthr[2][16];   // FOLD: amplitude pre-thresholds of the current / the next block
   extern __shared__ float4 slide_ring[];
   const int nwarps = blockDim.x >> 5, warp = threadIdx.x >> 5;
   long long wt = (long long)blockIdx.x * nwarps + warp;
@@ -376,6 +394,17 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
   S.keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
   const uint32_t T0 = (uint32_t)sg * (uint32_t)a.seg;                 // multiple of Nt and of L
   const uint32_t tend = min((uint32_t)a.nwin, T0 + (uint32_t)a.seg);  // windows [T0, tend)
+  [[maybe_unused]] const uint32_t *thrp = nullptr;
+  [[maybe_unused]] unsigned short *hp = nullptr;
+  [[maybe_unused]] uint32_t thr_next = 0x7f000000u;   // float bits: 1.7e38
+  if constexpr (FOLD) {
+    thrp = a.thr + (pl * a.per_pair + a.offc);
+    hp = a.hits + (((size_t)pl * a.nblk) * ndt + dti) * M + S.rho;      // + blk * ndt * M
+    if (threadIdx.x < 16) {   // threads 0..15 keep the thresholds two blocks ahead: raw in a register, converted a block later
+      fthr[0][threadIdx.x] = T0 + threadIdx.x < tend ? 0.999f * sqrtf(__uint_as_float(__ldg(thrp + T0 + threadIdx.x))) : 3.0e38f;
+      thr_next = T0 + 16u + threadIdx.x < tend ? __ldg(thrp + T0 + 16u + threadIdx.x) : 0x7f000000u;
+    }
+  }
   SlideRing G;
   if constexpr (RING) {
     // the CTA's warps are (rho fastest, then dt): its first warp's dt is the first column group
@@ -406,8 +435,24 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
     asm volatile("cp.async.wait_all;" ::: "memory");
     __syncthreads();
   }
+  if constexpr (FOLD && !RING) __syncthreads();                         // fthr[0]
   slide_prefetch<L, MODD, RING, 0, RR>(S, T0);
-  {
+  if constexpr (FOLD && RING) {
+    // the first window's samples are rows 0 .. w - 1 of the ring, their twiddles W_Nt^{rho t} entries 0 .. w - 1 of the
+    // warp's row (T0 = 0 mod Nt): both columns at once, packed
+#pragma unroll
+    for (int k = 0; k < L; ++k) { S.X[k] = pk(0.f, 0.f); S.Y[k] = pk(0.f, 0.f); }
+    for (uint32_t tb = 0; tb < (uint32_t)a.w; tb += L) {
+#pragma unroll
+      for (int k = 0; k < L; ++k) {
+        f32x2 yx, yy, twx, twy;
+        lds2(S.ring_lo + (tb + k) * S.rrowb, yx, yy);
+        lds2(S.tw_lo + (tb + k) * 16u, twx, twy);
+        S.X[k] = fma2(yx, twx, fma2(yy, neg2(twy), S.X[k]));
+        S.Y[k] = fma2(yx, twy, fma2(yy, twx, S.Y[k]));
+      }
+    }
+  } else {
     float2 Aa[L], Ab[L];
     slide_start_column<L, MODD, FOLD>(Aa, S.pout, S.rowb, T0, (uint32_t)a.w, a.twt, S.rho, S.ntmask, 0);
     slide_start_column<L, MODD, FOLD>(Ab, S.pout, S.rowb, T0, (uint32_t)a.w, a.twt, S.rho, S.ntmask, 1);
@@ -415,18 +460,20 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
     for (int s = 0; s < L; ++s) { S.X[s] = pk(Aa[s].x, Ab[s].x); S.Y[s] = pk(Aa[s].y, Ab[s].y); }
   }
 
-  [[maybe_unused]] const uint32_t *thrp = nullptr;
-  [[maybe_unused]] unsigned short *hp = nullptr;
-  if constexpr (FOLD) {
-    thrp = a.thr + (pl * a.per_pair + a.offc);
-    hp = a.hits + (((size_t)pl * a.nblk) * ndt + dti) * M + S.rho;      // + blk * ndt * M
-  }
+  [[maybe_unused]] uint32_t fslot = (uint32_t)a.w + 17u;   // RING: slot of the next row to fill (R = w + 48 > w + 17)
   uint32_t t0 = T0, buf = 0;
   for (;; t0 += L, buf ^= 1u) {
     const bool full = t0 + L < tend;
-    if constexpr (RING) slide_ring_fill(G, t0 - T0 + (uint32_t)a.w + 17u, 16u);   // the next block's new rows
+    if constexpr (RING) {                        // the next block's new rows
+      slide_ring_fill_block<RR>(G, t0 - T0 + (uint32_t)a.w + 17u, fslot);
+      fslot += 16u; fslot = fslot >= G.R ? fslot - G.R : fslot;
+    }
     if constexpr (FOLD) {
-      S.mythr = (lane < (uint32_t)L && t0 + lane < tend) ? 0.999f * sqrtf(__uint_as_float(__ldg(thrp + t0 + lane))) : 3.0e38f;
+      if (full && threadIdx.x < 16) {            // the next block's thresholds; visible after this block's barrier
+        fthr[buf ^ 1u][threadIdx.x] = 0.999f * sqrtf(__uint_as_float(thr_next));
+        thr_next = t0 + 32u + threadIdx.x < tend ? __ldg(thrp + t0 + 32u + threadIdx.x) : 0x7f000000u;
+      }
+      S.thrs = (uint32_t)__cvta_generic_to_shared(&fthr[buf][0]);
       if ((((t0 - T0) >> 4) & 3u) == 0u) {       // summed afresh every 64 steps (the updates in between drift by ~1e-5)
         S.e = pk(0.f, 0.f);
 #pragma unroll
@@ -438,8 +485,9 @@ __global__ void __launch_bounds__(SLIDE_WARPS * 32, SLIDE_MIN_CTAS) k_slide(Slid
     else SlideSteps<L, 0, MODD, true, RING, RR, FOLD>::run(S, t0, tend, &slots[buf][warp]);
     if constexpr (RING) asm volatile("cp.async.wait_all;" ::: "memory");
     if constexpr (FOLD) {
-      if (lane == 0) hp[(size_t)(t0 >> 4) * (size_t)(ndt * M)] = (unsigned short)S.mask;
-      if constexpr (RING) __syncthreads();       // the ring rows of the next block are complete and visible
+      const uint32_t hit = __reduce_or_sync(0xffffffffu, S.mask);
+      if (lane == 0) hp[(size_t)(t0 >> 4) * (size_t)(ndt * M)] = (unsigned short)hit;
+      __syncthreads();                           // the next block's thresholds (and ring rows) are complete and visible
     } else {
       slide_flush(S.keyp, slots[buf], t0, full ? (uint32_t)L : tend - t0, nwarps);
     }

@@ -869,11 +869,17 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         sa.thr = (const uint32_t *)(ws + pl->off_thr); sa.hits = nullptr; sa.nblk = w.nblk;
         if (fold) {
           // 1. the folded sliding sum: one hit bit per (window, rate residue, 64-column tile)
+          // (longer segments than the sliding kernel's: a step costs a fifth, so the start of a segment - its first window
+          // folded from w samples - weighs five times as much)
           sa.hits = (unsigned short *)(ws + w.off_hits);
+          sa.seg = w.seg * SFOLD_SEGMUL; sa.nseg = (int)((w.nwin + sa.seg - 1) / sa.seg);
+          sa.ntasks = ((np * sa.nseg * (long long)pl->dt_n) << w.log2m);
           {
             ProfScope ps(pl, st, VOLKS_K_SFOLD, q);
             launch_slide(sa, st, true);
           }
+          sa.seg = w.seg; sa.nseg = w.nseg;
+          sa.ntasks = ((np * w.nseg * (long long)pl->dt_n) << w.log2m);
           // 2. segments with more than 1/8 of their bits set (interference) go to the ordinary sliding kernel
           SfoldArgs ea;
           ea.Y = Y; ea.tw4 = (const float4 *)(pl->d_tables + w.tw4_off); ea.hits = sa.hits; ea.dense = (unsigned char *)(ws + w.off_sfdense); ea.keys = keys;
