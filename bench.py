@@ -234,6 +234,17 @@ COLFFT2_OPS_PER_COLUMN = {4: 11106.0, 8: 12718.0, 16: 14178.0}
 COLFFT2_SKIP_FLOPS_PER_COLUMN = {4: 5900.0, 8: 7850.0, 16: 9560.0}
 COLFFT2_SKIP_OPS_PER_COLUMN = {4: 4142.0, 8: 5768.0, 16: 7234.0}
 COLFFT2_FLOPS_PER_COLUMN = {4: 13700.0, 8: 15600.0, 16: 17200.0}
+# k_slide<FOLD> (kind 14, the folded sliding sum of the candidates-only mode; profiles/r02_counters.md, configs[2] w = 64):
+# 5.111e10 FP32 thread-instructions per launch, 8.87e9 of them scalar (the FFMAs of the octagonal bound); the rest is half
+# packed arithmetic (per step 4 FFMA2 : 2 FMUL2 : 4 FADD2 = 2.8 flops each) and half FMNMX / FSETP (comparisons: no flops)
+# = 7.69e10 flops per launch / 6.288e10 bin-steps = 1.22 flops per bin per window (the 16 bins of a (residue, column) share
+# ONE complex update); lane-operations 2 x 2.11e10 + 8.87e9 = 5.11e10 -> 0.81 per bin per window
+SFOLD_FLOPS_PER_BIN = 1.22
+SFOLD_OPS_PER_BIN = 0.81
+# warp instructions per bin per window (smsp__inst_executed.sum / bin-steps): against the issue rate of 148 SMs x 4
+# schedulers x the SM clock this is the share of issue slots filled
+WARP_INST_PER_BIN = {6: 8.715e9 / 6.288e10, 14: 2.828e9 / 6.288e10}
+SM_COUNT_ISSUE = 148 * 4
 
 
 def executed_flops_per_launch(c, kind, wid, nlaunch, npair, nap, alg_flops, cand_only=False):
@@ -245,6 +256,8 @@ def executed_flops_per_launch(c, kind, wid, nlaunch, npair, nap, alg_flops, cand
     nwin = workloads.gen.nwin(nap, w_, s_) * npair
     if kind == 6:
         return nwin * nt_ * c["nf"] * SLIDE_FLOPS_PER_BIN / nlaunch
+    if kind == 14:
+        return nwin * nt_ * c["nf"] * SFOLD_FLOPS_PER_BIN / nlaunch
     nz = 1
     while nz * 16 < w_:
         nz *= 2
@@ -261,12 +274,22 @@ def executed_ops_per_launch(c, kind, wid, nlaunch, npair, nap, cand_only=False):
     nwin = workloads.gen.nwin(nap, w_, s_) * npair
     if kind == 6:
         return nwin * nt_ * c["nf"] * SLIDE_OPS_PER_BIN / nlaunch
+    if kind == 14:
+        return nwin * nt_ * c["nf"] * SFOLD_OPS_PER_BIN / nlaunch
     nz = 1
     while nz * 16 < w_:
         nz *= 2
     if kind == 7 and nt_ == 512 and nz in COLFFT2_OPS_PER_COLUMN:
         return nwin * c["nf"] * (COLFFT2_SKIP_OPS_PER_COLUMN if cand_only else COLFFT2_OPS_PER_COLUMN)[nz] / nlaunch
     return None
+
+
+def executed_warp_inst_per_launch(c, kind, wid, nlaunch, npair, nap):
+    """Warp instructions per launch of the sliding kernels (ncu-pinned), or None."""
+    if wid < 0 or kind not in WARP_INST_PER_BIN or c["nts"][wid] < 32:
+        return None
+    nwin = workloads.gen.nwin(nap, c["widths"][wid], c["strides"][wid]) * npair
+    return nwin * c["nts"][wid] * c["nf"] * WARP_INST_PER_BIN[kind] / nlaunch
 
 
 def measure_fp32_peak(vk, local, stream):
@@ -432,12 +455,13 @@ def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traff
     alg_tf = dom_alg / (dom_ms_avg * 1e-3) / 1e12
     tr = traffic.get((c["id"], KIND_NAMES.get(dom[0], ""), c["widths"][dom[1]] if dom[1] >= 0 else -1))
     ops = executed_ops_per_launch(c, dom[0], dom[1], nlaunch[dom], nbl * nif, nap, cand_only)
+    winst = executed_warp_inst_per_launch(c, dom[0], dom[1], nlaunch[dom], nbl * nif, nap)
     roofline = {
         "bound": "alu", "kernel": kname, "achieved": exec_tf, "peak": peak_tf, "unit": "TFLOP/s",
         "frac": exec_tf / peak_tf, "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None,
         "launch_ms": dom_ms_avg, "share_of_step": share[dom] / step_sum,
         "flops_kind": "executed, pinned by ncu's instruction counters (profiles/r02_counters.md): k_slide 7.9 flops per bin "
-                      "per window, k_colfft2 (Nt 512) 13700 / 15600 / 17200 flops per (window, column) for w <= 64 / 128 / 256; "
+                      "per window (its folded form, sfold, 1.22: one complex update serves the 16 bins of a (residue, column)), k_colfft2 (Nt 512) 13700 / 15600 / 17200 flops per (window, column) for w <= 64 / 128 / 256; "
                       "other kernels the SURVEY 8(d) count",
         "fma_pipe_note": "packed FP32 adds and multiplies occupy the FMA pipe like FMAs but count half the flops, so the "
                          "flop fraction understates the pipe: ncu reads the FMA pipe 68 % busy for k_slide w = 64 and k_colfft2 w = 64 (profiles/r02_counters.md)",
@@ -445,6 +469,11 @@ def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traff
         "fp32_op_frac": None if ops is None else ops / (dom_ms_avg * 1e-3) / (peak_tf * 1e12 / 2.0),
         "fp32_op_kind": "executed FP32 lane-operations (add, multiply and FMA each one; ncu-pinned) / time / peak operation rate "
                         "(measured FMA peak / 2): the share of FP32 issue slots filled; `frac` counts flops, which halves every add",
+        "issue_frac": None if winst is None or not clocks.get("sm_mhz") else
+                      winst / (dom_ms_avg * 1e-3) / (SM_COUNT_ISSUE * clocks["sm_mhz"] * 1e6),
+        "issue_kind": "executed warp instructions (ncu-pinned per bin per window) / time / (148 SMs x 4 schedulers x the median "
+                      "SM clock of this run): the kernel mixes FMA-pipe, ALU-pipe (min / max / compare) and shared-memory "
+                      "instructions, so the issue rate bounds it before any one pipe does",
         "algorithmic_tflops": alg_tf, "algorithmic_frac": alg_tf / peak_tf,
         "algorithmic_kind": "SURVEY 8(d) FFT-equivalent flops / time: exceeds 1 by construction for the sliding path "
                             "(an algorithmic speed-up, not a fraction of the machine)",
@@ -509,7 +538,7 @@ def brief(R):
             "visibilities_per_s": R["world"] * R["nvis"] / (R["ms_step"] * 1e-3), "windows": R["nwin"],
             "candidates": R["n_found"], "clocks": R["clocks"],
             "roofline": {k: rf[k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic", "launch_ms",
-                                            "share_of_step", "fp32_op_frac", "algorithmic_frac", "bytes_kind", "kernel_ms") if k in rf}}
+                                            "share_of_step", "fp32_op_frac", "issue_frac", "algorithmic_frac", "bytes_kind", "kernel_ms") if k in rf}}
 
 
 def main():

@@ -8,7 +8,9 @@
 //               columns at a time, a fixed order); every thread takes entries in turn: it loads the window's w <= 32
 //               samples of the column ONCE into registers and, for every rate residue rho < M, folds them with
 //               W_Nt^{rho t} into 16 sums and runs the 16-point transform - all Nt rate bins of the column, exactly
-//               (the code of k_recover, for every residue) - keeping the first maximum in plane order.  The window's
+//               (the code of k_recover, for every residue) - keeping the first maximum in plane order.  A residue
+//               whose folded sums cannot reach the window's pre-threshold (sum_k |f[k]| bounds its 16 bins) skips the
+//               transform: nearly all of them, the amplitude-sum bound of k_bound being much the weaker one.  The window's
 //               key becomes the maximum over its entries (a shared-memory atomicMax per tile) and REPLACES what the
 //               window held, if it exceeds the window's pre-threshold.
 // A candidate has P1 > snr_thresh^2 noise > pre-threshold and P1 <= bound^2 of its column, so its column is listed and
@@ -48,6 +50,7 @@ __global__ void __launch_bounds__(CE_THREADS, 2) k_coleval(ColEvalArgs a) {
   __shared__ float2 tws[2 * CE_WMAX];                   // the width's Nt <= 64 twiddles
   __shared__ int wcount[CE_THREADS / 32 + 1];
   __shared__ unsigned char need[CE_TILE];
+  __shared__ float wthr[CE_TILE];                       // the windows' pre-thresholds (powers), lowered for the bound below
   __shared__ int total_sm;
   const int ntile = (a.nwin + CE_TILE - 1) / CE_TILE;
   const long long pl = blockIdx.x / ntile;
@@ -64,6 +67,7 @@ __global__ void __launch_bounds__(CE_THREADS, 2) k_coleval(ColEvalArgs a) {
       nd = (uint32_t)(a.keys[a.pair0 * a.per_pair + rel] >> 32) > __ldg(a.thr + rel);
     }
     need[threadIdx.x] = nd ? 1 : 0;
+    wthr[threadIdx.x] = J0 + threadIdx.x < a.nwin ? 0.998f * __uint_as_float(__ldg(a.thr + pl * a.per_pair + a.offc + J0 + threadIdx.x)) : 3.0e38f;
   }
   if (threadIdx.x < a.nt) tws[threadIdx.x] = __ldg(a.twt + threadIdx.x);
   const float *ybase = (const float *)(a.Y + (size_t)pl * a.nap * a.pitch);
@@ -113,6 +117,7 @@ __global__ void __launch_bounds__(CE_THREADS, 2) k_coleval(ColEvalArgs a) {
       }
       float best = -1.f;
       uint32_t bidx = 0;
+      const float thrw = wthr[j];
       for (int rho = 0; rho < M; ++rho) {
         float2 f[16];
 #pragma unroll
@@ -120,6 +125,16 @@ __global__ void __launch_bounds__(CE_THREADS, 2) k_coleval(ColEvalArgs a) {
           f[t2] = cmul(y[t2], tws[(rho * t2) & ntm]);
           cmac(f[t2], y[t2 + 16], tws[(rho * (t2 + 16)) & ntm]);
         }
+        // the 16 bins of this residue obey |A| <= sum_k |f[k]| <= e (the octagonal bound of kernels_sfold.cuh, 4.7 noise
+        // deviations below the pre-threshold at snr_thresh 6): a residue that cannot reach the window's pre-threshold
+        // cannot change the outcome (the key is replaced only by a power above it) and skips its transform
+        float e = 0.f;
+#pragma unroll
+        for (int t2 = 0; t2 < 16; ++t2) {
+          const float ax = fabsf(f[t2].x), ay = fabsf(f[t2].y);
+          e += fmaxf(ax, ay) + 0.41421357f * fminf(ax, ay);
+        }
+        if (e * e <= thrw) continue;
         FftDif<16, 0, 16>::run(f);
 #pragma unroll
         for (int s = 0; s < 16; ++s) {                    // plane order within the column: rho + M s ascending in s
@@ -128,7 +143,7 @@ __global__ void __launch_bounds__(CE_THREADS, 2) k_coleval(ColEvalArgs a) {
           if (pw > best || (pw == best && idx < bidx)) { best = pw; bidx = idx; }
         }
       }
-      atomicMax(&wkey[j], make_key(best, bidx));
+      if (best >= 0.f) atomicMax(&wkey[j], make_key(best, bidx));
     }
   }
   __syncthreads();

@@ -71,3 +71,10 @@ def test_traffic_table_and_executed_flops():
     assert bench.executed_ops_per_launch(c, 6, 5, 5, 80, c["nap"]) == (120000 - 64 + 1) * 80 * 128 * 256 * 5.17 / 5
     assert bench.executed_ops_per_launch(c4, 7, 2, 7, 84, 20000) == 309 * 84 * 2048 * 14178.0 / 7
     assert bench.executed_ops_per_launch(c4, 1, -1, 7, 84, 20000) is None
+    # the folded sliding sum (kind 14): 1.22 flops, 0.81 lane-operations and 0.045 warp instructions per bin per window
+    bins = (120000 - 64 + 1) * 80 * 128 * 256
+    assert bench.executed_flops_per_launch(c, 14, 5, 5, 80, c["nap"], 1.0) == bins * 1.22 / 5
+    assert bench.executed_ops_per_launch(c, 14, 5, 5, 80, c["nap"]) == bins * 0.81 / 5
+    assert abs(bench.executed_warp_inst_per_launch(c, 14, 5, 5, 80, c["nap"]) - bins * 0.04497 / 5) < 1e-3 * bins * 0.045 / 5
+    assert bench.executed_warp_inst_per_launch(c, 6, 0, 5, 80, c["nap"]) is None     # the narrow widths: no capture
+    assert bench.executed_warp_inst_per_launch(c, 1, -1, 5, 80, c["nap"]) is None
