@@ -45,22 +45,41 @@ struct PruneArgs {
   unsigned char *cwdense;
 };
 
-template <int NQ, int NCW>
-__global__ void __launch_bounds__(PRUNE_THREADS) k_bound(PruneArgs a) {
-  extern __shared__ float prune_sm[];
-  // shared: thr[NQ][TP] floats (TP = 2 seg + 64: 32 entries of +inf before and after the tile's windows, so that
-  // window starts outside the tile need no branch), then the ring [a.ring][blockDim.x] of packed running sums
+constexpr int PRUNE_MIRROR = 4;    // ring rows 0..3 are stored a second time behind the last: 4 consecutive rows never wrap
+
+// dynamic shared memory of k_bound<NQ, NCW, NTHR>: thresholds + the ring of running sums (8 B per thread and row);
+// NTHR = 64 or 128 threads (the ring's row stride is a compile-time constant)
+__host__ __device__ inline size_t prune_smem_bytes(int nq, int seg, int ring, int nthr) {
+  return (size_t)((nq * (2 * seg + 64) + 3) & ~3) * sizeof(float) + (size_t)(ring + PRUNE_MIRROR) * nthr * 8;
+}
+
+// Per row and thread: one 128-bit load issued EIGHT rows ahead (with four ncu read long-scoreboard 2.1 - 3.6 of 4 warps and
+// half the DRAM bandwidth), the two amplitudes, one running sum; per width ONE shared-memory load (the running sum w rows
+// back), a subtract, the larger column, d = bound^2 - pre-threshold, and a running maximum of d - no compare, no branch.
+// The sign of the maximum is looked at three times per tile: the rows are split where the windows' segment changes (rows
+// below rA belong to the tile's first segment for every width, rows from rB on to the second; the few rows in between
+// flag both - a flag too many costs an evaluation, never a candidate).
+// What bounds it (ncu, profiles/r02_ncu_kernels.md): the shared-memory data path (one 64-bit ring load per width and row,
+// the ring store) and DRAM at 60 - 70 % of its peak; staging the rows through shared memory with cp.async 12 rows ahead
+// removed the long-scoreboard stalls but added 8 wavefronts per warp-row to that path and came out even.
+template <int NQ, int NCW, int NTHR>
+__global__ void __launch_bounds__(NTHR) k_bound(PruneArgs a) {
+  constexpr int PRUNE_RSTRIDE = NTHR * 8;    // bytes per ring row
+  extern __shared__ float4 prune_sm4[];
+  // shared: thr[NQ][TP] floats (TP = 2 seg + 64), indexed by the window's LAST row relative to the tile: entry r of width q
+  // = pre-threshold of the window starting at row r - w[q] + 1 (+inf where the tile has no such window: no branch), then
+  // the ring [a.ring + 4][NTHR] of packed running sums
   const int T = 2 * a.seg, TP = T + 64;
-  float *thr_sm = prune_sm;
+  float *thr_sm = (float *)prune_sm4;
   __shared__ int any[PRUNE_MAXQ][2];
   __shared__ int cwtotal;
   const int ntile = (a.nseg + 1) / 2;
   const long long pl = blockIdx.x / ntile;
   const int tile = (int)(blockIdx.x % ntile);
   const int R0 = tile * T;                                   // first window start (= first row) of the tile
-  const int nthr = blockDim.x;                               // a power of two (nf / 2 or 128)
+  const int nthr = blockDim.x;                               // a power of two <= NTHR (nf / 2 or 128)
   for (int i = threadIdx.x; i < NQ * TP; i += nthr) {
-    const int q = i / TP, j = i - q * TP - 32;
+    const int q = i / TP, j = i - q * TP - a.w[q] + 1;
     thr_sm[i] = (j >= 0 && j < T && R0 + j < a.nwin[q]) ? __uint_as_float(__ldg(a.thr + pl * a.per_pair + a.offc[q] + R0 + j)) : 3.0e38f;
   }
   if (threadIdx.x < PRUNE_MAXQ * 2) any[threadIdx.x >> 1][threadIdx.x & 1] = 0;
@@ -70,74 +89,97 @@ __global__ void __launch_bounds__(PRUNE_THREADS) k_bound(PruneArgs a) {
   const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch);
   const size_t rowb = (size_t)a.pitch * 8u;
   // ring of running sums C[r] = sum_{r' <= r} |Y[r']| of the thread's two columns: the bound of the window of width w
-  // ending at row r is C[r] - C[r - w] (C = 0 before the tile: the ring starts zeroed).  Byte offsets wrap with one AND.
-  char *ring = (char *)(prune_sm + ((NQ * TP + 3) & ~3)) + threadIdx.x * 8u;
-  const uint32_t rstride = (uint32_t)nthr * 8u, rmask = (uint32_t)a.ring * rstride - 1u;
-  // per width: byte offset of the leaving sum relative to the entering one, the threshold row, the first row of the
-  // tile's second segment, the two flag bits
-  uint32_t back[NQ], rhalf[NQ];
-  const float *thq[NQ];
+  // ending at row r is C[r] - C[r - w] (C = 0 before the tile: the ring starts zeroed)
+  char *ring = (char *)(thr_sm + ((NQ * TP + 3) & ~3)) + threadIdx.x * 8u;
+  const uint32_t rmask = (uint32_t)a.ring * PRUNE_RSTRIDE - 1u;
+  uint32_t back[NQ];
+  int wmin = a.w[0];
 #pragma unroll
-  for (int q = 0; q < NQ; ++q) {
-    back[q] = (uint32_t)a.w[q] * rstride;
-    thq[q] = thr_sm + q * TP + 33 - a.w[q];                  // thq[q][r] = pre-threshold of the window ending at row r
-    rhalf[q] = (uint32_t)(a.seg + a.w[q] - 1);
-  }
+  for (int q = 0; q < NQ; ++q) { back[q] = (uint32_t)a.w[q] * PRUNE_RSTRIDE; wmin = min(wmin, a.w[q]); }
+  const int rA = (a.seg + wmin - 1) & ~3, rB = (a.seg + a.wmax - 1 + 3) & ~3;   // (multiples of 4: looked at per 4 rows)
+  [[maybe_unused]] const int wcw = a.w[NQ - 1];
   __syncthreads();
   unsigned hit = 0;                                          // bit 2 q + half
   for (int ci = threadIdx.x; ci < a.ncp; ci += nthr) {
     const int c = ci < a.cp_na ? a.cp_a0 + ci : a.cp_b0 + (ci - a.cp_na);
-    for (int k = 0; k < a.ring; ++k) *(f32x2 *)(ring + (uint32_t)k * rstride) = pk(0.f, 0.f);
+    for (int k = 0; k < a.ring + PRUNE_MIRROR; ++k) *(f32x2 *)(ring + (uint32_t)k * PRUNE_RSTRIDE) = pk(0.f, 0.f);
     const char *p = ybase + (size_t)R0 * rowb + (size_t)c * 16u;
-    f32x2 bx[4], by[4];                                      // four rows in flight
+    f32x2 bx[8], by[8];                                      // eight rows in flight
 #pragma unroll
-    for (int u = 0; u < 4; ++u) { bx[u] = by[u] = pk(0.f, 0.f); if (u < nrows) ldg2(p + (size_t)u * rowb, bx[u], by[u]); }
+    for (int u = 0; u < 8; ++u) { bx[u] = by[u] = pk(0.f, 0.f); if (u < nrows) ldg2(p + (size_t)u * rowb, bx[u], by[u]); }
     f32x2 C = pk(0.f, 0.f);
-    uint32_t roff = 0, cwa = 0, cwb = 0;
-    for (int r0 = 0; r0 < nrows; r0 += 4) {
+    float mx[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) mx[q] = -3.0e38f;
+    uint32_t roff = 0, cwa = 0, cwb = 0, halves = 1u;        // halves: the segments (bit 0 / 1) the current rows can belong to
+    // the column-level width: rows until its next word of 32 windows is complete; the word's address
+    [[maybe_unused]] int cwn = wcw + 31;
+    [[maybe_unused]] uint32_t *cwp = NCW == 1 ? a.cwmask + ((size_t)pl * a.cw_nwords + (R0 >> 5)) * (size_t)a.nf + 2 * c : nullptr;
+    for (int r8 = 0; r8 < nrows; r8 += 8) {
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int r0 = r8 + 4 * h;
+      if (r0 >= nrows) break;
+      if (r0 == rA || r0 == rB) {                            // (uniform) the rows' segment changes: note the sign, start afresh
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) { if (mx[q] > 0.f) hit |= halves << (2 * q); mx[q] = -3.0e38f; }
+        halves = r0 == rB ? 2u : 3u;
+      }
+      const char *ob[NQ];                                    // ring slot of row r0 - w[q]: this and the next 3 slots never wrap
+      float4 th4[NQ];
+#pragma unroll
+      for (int q = 0; q < NQ; ++q) {
+        ob[q] = ring + ((roff - back[q]) & rmask);
+        th4[q] = *(const float4 *)(thr_sm + q * TP + r0);
+      }
+      const bool mir = roff == 0;
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
         const int r = r0 + u;
-        const f32x2 x = bx[u], y = by[u];
-        if (r + 4 < nrows) ldg2(p + (size_t)(r + 4) * rowb, bx[u], by[u]);
+        const f32x2 x = bx[4 * h + u], y = by[4 * h + u];
+        if (r + 8 < nrows) ldg2(p + (size_t)(r + 8) * rowb, bx[4 * h + u], by[4 * h + u]);
         if (r < nrows) {
           const f32x2 e = fma2(y, y, mul2(x, x));
           float aa, ab;
-          asm("sqrt.approx.f32 %0, %1;" : "=f"(aa) : "f"(lo32(e)));
-          asm("sqrt.approx.f32 %0, %1;" : "=f"(ab) : "f"(hi32(e)));
+          asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(aa) : "f"(lo32(e)));
+          asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(ab) : "f"(hi32(e)));
           C = add2(C, pk(aa, ab));
-          f32x2 old[NQ];
-          float th[NQ];
 #pragma unroll
           for (int q = 0; q < NQ; ++q) {                     // (read before this row's store: for w == ring they share a slot)
-            old[q] = *(const f32x2 *)(ring + ((roff - back[q]) & rmask));
-            th[q] = thq[q][r];
-          }
-#pragma unroll
-          for (int q = 0; q < NQ; ++q) {
-            const f32x2 S = sub2(C, old[q]);
+            const f32x2 S = sub2(C, *(const f32x2 *)(ob[q] + u * PRUNE_RSTRIDE));
+            const float th = u == 0 ? th4[q].x : u == 1 ? th4[q].y : u == 2 ? th4[q].z : th4[q].w;
             const float m = fmaxf(lo32(S), hi32(S));
-            const bool h = m * m > th[q];
-            if (h) hit |= (uint32_t)r >= rhalf[q] ? 2u << (2 * q) : 1u << (2 * q);
+            mx[q] = fmaxf(mx[q], fmaf(m, m, -th));
             if constexpr (NCW == 1) {
-              if (q == NQ - 1) {                             // the column-level width: a bit per (window, column pair)
-                const int j = r - a.w[q] + 1;
-                if (j >= 0 && j < T) {
-                  cwa |= (lo32(S) * lo32(S) > th[q] ? 1u : 0u) << (j & 31);
-                  cwb |= (hi32(S) * hi32(S) > th[q] ? 1u : 0u) << (j & 31);
-                  if ((j & 31) == 31 || r == nrows - 1) {
-                    cwcount += __popc(cwa) + __popc(cwb);
-                    if (cwa | cwb)
-                      *(uint2 *)(a.cwmask + ((size_t)pl * a.cw_nwords + ((R0 + j) >> 5)) * (size_t)a.nf + 2 * c) = make_uint2(cwa, cwb);
-                    cwa = 0; cwb = 0;
-                  }
+              if (q == NQ - 1) {                             // the column-level width: a bit per (window, column)
+                // th - S^2 is negative iff the column's bound exceeds the pre-threshold: its sign bit enters a shift
+                // register (the latest window in bit 0: reversed when the word of 32 windows is complete)
+                cwa = __funnelshift_l(__float_as_uint(fmaf(-lo32(S), lo32(S), th)), cwa, 1);
+                cwb = __funnelshift_l(__float_as_uint(fmaf(-hi32(S), hi32(S), th)), cwb, 1);
+                if (--cwn == 0) {                            // the window starting at this row - wcw + 1 completes a word
+                  const uint32_t wa = __brev(cwa), wb = __brev(cwb);
+                  cwcount += __popc(wa) + __popc(wb);
+                  if (wa | wb) *(uint2 *)cwp = make_uint2(wa, wb);
+                  cwp += a.nf;
+                  cwn = 32;
                 }
               }
             }
           }
-          *(f32x2 *)(ring + (roff & rmask)) = C;
-          roff += rstride;
+          *(f32x2 *)(ring + roff + u * PRUNE_RSTRIDE) = C;
+          if (mir) *(f32x2 *)(ring + (a.ring + u) * PRUNE_RSTRIDE) = C;
         }
+      }
+      roff = (roff + 4u * PRUNE_RSTRIDE) & rmask;
+    }
+    }
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) if (mx[q] > 0.f) hit |= halves << (2 * q);
+    if constexpr (NCW == 1) {
+      if (cwn < 32) {                                        // the last, incomplete word: 32 - cwn windows, the first in bit 0
+        const uint32_t wa = __brev(cwa) >> cwn, wb = __brev(cwb) >> cwn;
+        cwcount += __popc(wa) + __popc(wb);
+        if (wa | wb) *(uint2 *)cwp = make_uint2(wa, wb);
       }
     }
   }

@@ -238,6 +238,20 @@ static bool slide_attrs() {
          cudaFuncSetAttribute(k_slide<16, false, true, 1024, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) == cudaSuccess;
 }
 
+// k_bound's dynamic shared memory limit (per device, process-wide)
+constexpr size_t PRUNE_SMEM_LIMIT = 96 * 1024;
+template <int NQ>
+static bool bound_attr() {
+  return cudaFuncSetAttribute(k_bound<NQ, 0, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PRUNE_SMEM_LIMIT) == cudaSuccess &&
+         cudaFuncSetAttribute(k_bound<NQ, 1, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PRUNE_SMEM_LIMIT) == cudaSuccess &&
+         cudaFuncSetAttribute(k_bound<NQ, 0, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PRUNE_SMEM_LIMIT) == cudaSuccess &&
+         cudaFuncSetAttribute(k_bound<NQ, 1, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PRUNE_SMEM_LIMIT) == cudaSuccess;
+}
+static bool bound_attrs() {
+  return bound_attr<1>() && bound_attr<2>() && bound_attr<3>() && bound_attr<4>() && bound_attr<5>() && bound_attr<6>() &&
+         bound_attr<7>() && bound_attr<8>();
+}
+
 }  // namespace
 
 struct volks_plan {
@@ -549,6 +563,11 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
     }
   }
   pl->prune_seg = opt.prune_seg;
+  // k_bound's shared memory (thresholds of a tile of 2 prune_seg windows per width + the ring + the staged rows)
+  if ((pl->nprune || pl->cwq >= 0) && prune_smem_bytes(pl->nprune + 1, opt.prune_seg, PRUNE_RING, PRUNE_THREADS) > PRUNE_SMEM_LIMIT) {
+    delete pl;
+    return VOLKS_EINVAL;
+  }
   pl->off_thr = off;  off = align_up(off + ((pl->cand_only && (pl->nuntag || pl->nprune)) ? (size_t)pl->pairs_per_chunk * per_pair * sizeof(uint32_t) : 0), 256);
   pl->off_flags = off; off = align_up(off + (size_t)pl->pairs_per_chunk * (pl->nprune + 1) * pl->prune_nseg, 256);
   // the column-level width's bits: k_bound's tiles are 2 prune_seg windows, a multiple of 32
@@ -608,6 +627,7 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
       ok = cuda_ok(launch_colfft(ca, w.cf_l1, w.cf_nz, 0, nullptr, true));
     }
   if (ok && !slide_attrs()) ok = cuda_ok(cudaGetLastError()) && false;
+  if (ok && !bound_attrs()) ok = cuda_ok(cudaGetLastError()) && false;
   if (ok && (p->nf == 4096 || p->nf == 8192)) {
     RowArgs ra; memset(&ra, 0, sizeof ra);
     ra.paired = pl->paired; ra.nf = p->nf; ra.nchan = p->nchan; ra.nrows = 1;
@@ -814,15 +834,16 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
           pa.cwmask = (uint32_t *)(ws + pl->off_cwmask);
           if (!cuda_ok(cudaMemsetAsync(pa.cwmask, 0, (size_t)np * pl->cw_nwords * s.nf * sizeof(uint32_t), st))) return VOLKS_ECUDA;
         }
-        const int T = 2 * pa.seg, thr = std::min(PRUNE_THREADS, s.nf / 2);   // (nf >= 64: a power of two >= 32)
+        const int thr = std::min(PRUNE_THREADS, s.nf / 2);   // (nf >= 64: a power of two >= 32)
         pa.ring = pa.wmax <= 16 ? 16 : 32;                 // rows of amplitude history (a power of two >= wmax)
-        const size_t smem = (size_t)((pa.nq * (T + 64) + 3) & ~3) * sizeof(float) + (size_t)pa.ring * thr * sizeof(f32x2);
+        const int nthr_t = thr > 64 ? 128 : 64;            // the kernel's compile-time thread count (row strides)
+        const size_t smem = prune_smem_bytes(pa.nq, pa.seg, pa.ring, nthr_t);
         const unsigned blocks = (unsigned)(np * ((pa.nseg + 1) / 2));
         ProfScope ps(pl, st, VOLKS_K_BOUND, -1);
 #define VOLKS_BOUND(NQ_)                                                                   \
   case NQ_:                                                                                \
-    if (use_cw) k_bound<NQ_, 1><<<blocks, thr, smem, st>>>(pa);                            \
-    else k_bound<NQ_, 0><<<blocks, thr, smem, st>>>(pa);                                   \
+    if (use_cw) { if (nthr_t == 128) k_bound<NQ_, 1, 128><<<blocks, thr, smem, st>>>(pa); else k_bound<NQ_, 1, 64><<<blocks, thr, smem, st>>>(pa); } \
+    else { if (nthr_t == 128) k_bound<NQ_, 0, 128><<<blocks, thr, smem, st>>>(pa); else k_bound<NQ_, 0, 64><<<blocks, thr, smem, st>>>(pa); } \
     break;
         switch (pa.nq) { VOLKS_BOUND(1) VOLKS_BOUND(2) VOLKS_BOUND(3) VOLKS_BOUND(4) VOLKS_BOUND(5) VOLKS_BOUND(6) VOLKS_BOUND(7) VOLKS_BOUND(8) }
 #undef VOLKS_BOUND
