@@ -202,4 +202,137 @@ __global__ void __launch_bounds__(NTHR) k_bound(PruneArgs a) {
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// k_pairfold - the column bits of the column-level width when it is w = 32 at Nt = 64 (M = 4 rate residues): the folded
+// bound of kernels_sfold.cuh instead of the amplitude sum, in one streaming pass.
+// The 16 bins r = rho + 4 s of residue rho are the 16-point DFT of f_rho[k] = y[t0 + k] W_64^{rho k} + y[t0 + k + 16]
+// W_64^{rho (k + 16)}, and |f_rho[k]| = |y[t0 + k] + (-i)^rho y[t0 + k + 16]| =: A_rho[t0 + k] - no multiply, and a function of
+// the ABSOLUTE row t = t0 + k alone.  So  max_s |F[rho + 4 s][d]| <= e_rho(t0) = sum_{t0 <= t < t0 + 16} A_rho[t]:  four sliding
+// sums of width 16 per column.  For noise e_rho has mean 3.55 sqrt(P0), deviation 0.46 sqrt(P0) against the amplitude
+// pre-threshold 5.94 sqrt(P0) (P0 = the mean bin power): 5.2 deviations, where the plain amplitude sum of k_bound has 2.0 and
+// lets 2 - 3 % of the (window, column) pairs through to k_coleval.  A candidate's bin exceeds the pre-threshold, so its
+// column's bit is set (exactness as for k_bound); the bits and the per-tile density bytes have k_bound's format.
+//   CTA = (pair, 256 window starts), thread = column pair; per row: one 128-bit load (eight rows in flight), the row 16
+//   back from a shared-memory ring, four packed complex add/subtracts, four packed |.|^2, eight square roots, the four
+//   amplitudes 16 rows back from a second ring, e_rho += A_new - A_old, the largest e per column, its square against the
+//   window's pre-threshold by a sign-bit shift register (as in k_bound).
+constexpr int PF_T = 256;          // window starts per CTA (two tiles of k_coleval)
+constexpr int PF_W = 32;           // the width this kernel is for (Nt = 64)
+constexpr int PF_THREADS = 128;
+
+struct PairFoldArgs {
+  const float2 *Y;        // [pairs of the chunk][nap][pitch] pair-interleaved delay spectra
+  const uint32_t *thr;    // pre-thresholds (float bits): thr[pl * per_pair + offc + t0]
+  uint32_t *cwmask;       // [(pl * cw_nwords + window / 32) * nf + column], zeroed before the launch
+  unsigned char *cwdense; // [pl * ntile128 + tile of 128 windows]
+  long long per_pair, offc;
+  int nap, nf, pitch, nwin, cw_nwords, ntile128;
+  int ncp, cp_na, cp_a0, cp_b0;   // column pairs to look at (restricted delay range), as in PruneArgs
+};
+
+__host__ __device__ inline size_t pairfold_smem_bytes() {
+  return (size_t)(PF_T + 64) * sizeof(float) + (size_t)16 * PF_THREADS * 16 + (size_t)4 * 16 * PF_THREADS * 8;
+}
+
+__global__ void __launch_bounds__(PF_THREADS) k_pairfold(PairFoldArgs a) {
+  extern __shared__ float4 pf_sm4[];
+  float *thr_sm = (float *)pf_sm4;                             // [PF_T + 64]: entry r = pre-threshold of the window ENDING at row r
+  __shared__ int cwtotal[2];
+  const int ntile = (a.nwin + PF_T - 1) / PF_T;
+  const long long pl = blockIdx.x / ntile;
+  const int tile = (int)(blockIdx.x % ntile);
+  const int R0 = tile * PF_T;
+  for (int i = threadIdx.x; i < PF_T + 64; i += PF_THREADS) {
+    const int j = i - PF_W + 1;
+    thr_sm[i] = (j >= 0 && j < PF_T && R0 + j < a.nwin) ? __uint_as_float(__ldg(a.thr + pl * a.per_pair + a.offc + R0 + j)) : 3.0e38f;
+  }
+  if (threadIdx.x < 2) cwtotal[threadIdx.x] = 0;
+  const int nrows = min(PF_T + PF_W - 1, a.nap - R0);
+  const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch);
+  const size_t rowb = (size_t)a.pitch * 8u;
+  // rings (slot = row & 15): the raw rows [16][PF_THREADS] float4, the amplitudes [4][16][PF_THREADS] f32x2
+  const uint32_t raw = (uint32_t)__cvta_generic_to_shared(thr_sm + PF_T + 64) + threadIdx.x * 16u;
+  char *amp = (char *)(thr_sm + PF_T + 64) + 16 * PF_THREADS * 16 + threadIdx.x * 8u;
+  constexpr uint32_t RAWROW = PF_THREADS * 16, AMPROW = PF_THREADS * 8, AMPRHO = 16 * AMPROW;
+  __syncthreads();
+  int cnt0 = 0, cnt1 = 0;                                      // set bits of the two 128-window halves
+  for (int ci = threadIdx.x; ci < a.ncp; ci += PF_THREADS) {
+    const int c = ci < a.cp_na ? a.cp_a0 + ci : a.cp_b0 + (ci - a.cp_na);
+    for (int k = 0; k < 64; ++k) *(f32x2 *)(amp + (uint32_t)k * AMPROW) = pk(0.f, 0.f);
+    const char *p = ybase + (size_t)R0 * rowb + (size_t)c * 16u;
+    f32x2 bx[16], by[16];                                      // sixteen rows in flight (two CTAs per SM: registers to spare)
+#pragma unroll
+    for (int u = 0; u < 16; ++u) { bx[u] = by[u] = pk(0.f, 0.f); if (u < nrows) ldg2(p + (size_t)u * rowb, bx[u], by[u]); }
+    f32x2 e0 = pk(0.f, 0.f), e1 = e0, e2 = e0, e3 = e0;
+    uint32_t cwa = 0, cwb = 0;
+    int cwn = PF_W + 31;                                       // rows until the next word of 32 windows is complete
+    uint32_t *cwp = a.cwmask + ((size_t)pl * a.cw_nwords + (R0 >> 5)) * (size_t)a.nf + 2 * c;
+    int nword = 0;
+    for (int r16 = 0; r16 < nrows; r16 += 16) {
+#pragma unroll
+      for (int u = 0; u < 16; ++u) {
+        const int r = r16 + u;
+        const f32x2 x = bx[u], y = by[u];
+        if (r + 16 < nrows) ldg2(p + (size_t)(r + 16) * rowb, bx[u], by[u]);
+        if (r < nrows) {
+          const uint32_t slot = (uint32_t)u;                   // = r & 15: after unrolling the ring offsets are immediates
+          if (r16 > 0) {
+            f32x2 xo, yo;                                      // the row 16 back: the class's first sample
+            lds2(raw + slot * RAWROW, xo, yo);
+            // f_rho = y[t] + (-i)^rho y[t + 16]:  rho 0: (xo + x, yo + y), 1: (xo + y, yo - x), 2: (xo - x, yo - y), 3: (xo - y, yo + x)
+            const f32x2 ax0 = add2(xo, x), ay0 = add2(yo, y), ax2 = sub2(xo, x), ay2 = sub2(yo, y);
+            const f32x2 ax1 = add2(xo, y), ay1 = sub2(yo, x), ax3 = sub2(xo, y), ay3 = add2(yo, x);
+            const f32x2 p0 = fma2(ay0, ay0, mul2(ax0, ax0)), p1 = fma2(ay1, ay1, mul2(ax1, ax1));
+            const f32x2 p2 = fma2(ay2, ay2, mul2(ax2, ax2)), p3 = fma2(ay3, ay3, mul2(ax3, ax3));
+            float s0a, s0b, s1a, s1b, s2a, s2b, s3a, s3b;
+            asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s0a) : "f"(lo32(p0)));
+            asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s0b) : "f"(hi32(p0)));
+            asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s1a) : "f"(lo32(p1)));
+            asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s1b) : "f"(hi32(p1)));
+            asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s2a) : "f"(lo32(p2)));
+            asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s2b) : "f"(hi32(p2)));
+            asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s3a) : "f"(lo32(p3)));
+            asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s3b) : "f"(hi32(p3)));
+            const f32x2 A0 = pk(s0a, s0b), A1 = pk(s1a, s1b), A2 = pk(s2a, s2b), A3 = pk(s3a, s3b);
+            char *as = amp + slot * AMPROW;                    // the amplitudes of row t - 16 leave, those of t = r - 16 enter
+            e0 = add2(e0, sub2(A0, *(const f32x2 *)(as)));
+            e1 = add2(e1, sub2(A1, *(const f32x2 *)(as + AMPRHO)));
+            e2 = add2(e2, sub2(A2, *(const f32x2 *)(as + 2 * AMPRHO)));
+            e3 = add2(e3, sub2(A3, *(const f32x2 *)(as + 3 * AMPRHO)));
+            *(f32x2 *)(as) = A0; *(f32x2 *)(as + AMPRHO) = A1; *(f32x2 *)(as + 2 * AMPRHO) = A2; *(f32x2 *)(as + 3 * AMPRHO) = A3;
+          }
+          asm volatile("st.shared.v2.b64 [%0], {%1, %2};" ::"r"(raw + slot * RAWROW), "l"(x), "l"(y) : "memory");
+          // the window ending at this row (start r - 31): the largest of the four bounds per column, squared, against its
+          // pre-threshold; the sign bit of thr - e^2 enters the shift register (latest window in bit 0)
+          const float ma = fmaxf(fmaxf(lo32(e0), lo32(e1)), fmaxf(lo32(e2), lo32(e3)));
+          const float mb = fmaxf(fmaxf(hi32(e0), hi32(e1)), fmaxf(hi32(e2), hi32(e3)));
+          const float th = thr_sm[r];
+          cwa = __funnelshift_l(__float_as_uint(fmaf(-ma, ma, th)), cwa, 1);
+          cwb = __funnelshift_l(__float_as_uint(fmaf(-mb, mb, th)), cwb, 1);
+          if (--cwn == 0) {
+            const uint32_t wa = __brev(cwa), wb = __brev(cwb);
+            const int n = __popc(wa) + __popc(wb);
+            if (nword < 4) cnt0 += n; else cnt1 += n;
+            if (wa | wb) *(uint2 *)cwp = make_uint2(wa, wb);
+            cwp += a.nf; ++nword;
+            cwn = 32;
+          }
+        }
+      }
+    }
+    if (cwn < 32) {                                            // the last, incomplete word
+      const uint32_t wa = __brev(cwa) >> cwn, wb = __brev(cwb) >> cwn;
+      const int n = __popc(wa) + __popc(wb);
+      if (nword < 4) cnt0 += n; else cnt1 += n;
+      if (wa | wb) *(uint2 *)cwp = make_uint2(wa, wb);
+    }
+  }
+#pragma unroll
+  for (int o = 16; o >= 1; o >>= 1) { cnt0 += __shfl_xor_sync(0xffffffffu, cnt0, o); cnt1 += __shfl_xor_sync(0xffffffffu, cnt1, o); }
+  if ((threadIdx.x & 31) == 0) { if (cnt0) atomicAdd(&cwtotal[0], cnt0); if (cnt1) atomicAdd(&cwtotal[1], cnt1); }
+  __syncthreads();
+  if (threadIdx.x < 2 && 2 * tile + (int)threadIdx.x < a.ntile128)   // dense: more than 1/8 of the 128 x columns bits (k_bound's rule)
+    a.cwdense[pl * a.ntile128 + 2 * tile + threadIdx.x] = (unsigned char)((long long)cwtotal[threadIdx.x] * 8 > 128LL * 2 * a.ncp ? 1 : 0);
+}
+
 }  // namespace volks

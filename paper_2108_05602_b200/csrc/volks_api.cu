@@ -248,7 +248,8 @@ static bool bound_attr() {
          cudaFuncSetAttribute(k_bound<NQ, 1, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PRUNE_SMEM_LIMIT) == cudaSuccess;
 }
 static bool bound_attrs() {
-  return bound_attr<1>() && bound_attr<2>() && bound_attr<3>() && bound_attr<4>() && bound_attr<5>() && bound_attr<6>() &&
+  return cudaFuncSetAttribute(k_pairfold, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pairfold_smem_bytes()) == cudaSuccess &&
+         bound_attr<1>() && bound_attr<2>() && bound_attr<3>() && bound_attr<4>() && bound_attr<5>() && bound_attr<6>() &&
          bound_attr<7>() && bound_attr<8>();
 }
 
@@ -270,6 +271,7 @@ struct volks_plan {
   bool cand_only = false;        // searches without d_peaks recover indices / evaluate segments for possible candidates only
   int nprune = 0, prune_nseg = 0, prune_seg = 0, prune_wmax = 0;   // pruned widths (k_bound): count, common segmentation
   int nsf = 0;                   // widths on the folded-sum path in the candidates-only mode (kernels_sfold.cuh)
+  bool cw_pf = false;            // the column-level width is w = 32 at Nt = 64: its bits come from k_pairfold (folded bound), not k_bound
   int cwq = -1, cw_nwords = 0;   // the column-level width (index into wp) and the 32-window words of its bit mask per pair
   size_t off_cwmask = 0, off_cwdense = 0;
   int dt_n = 0, dt_na = 0, dt_a0 = 0, dt_b0 = 0;   // 64-column groups the sliding kernels / k_bound work on (restricted delay range)
@@ -571,6 +573,7 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
   pl->off_thr = off;  off = align_up(off + ((pl->cand_only && (pl->nuntag || pl->nprune)) ? (size_t)pl->pairs_per_chunk * per_pair * sizeof(uint32_t) : 0), 256);
   pl->off_flags = off; off = align_up(off + (size_t)pl->pairs_per_chunk * (pl->nprune + 1) * pl->prune_nseg, 256);
   // the column-level width's bits: k_bound's tiles are 2 prune_seg windows, a multiple of 32
+  pl->cw_pf = pl->cwq >= 0 && pl->wp[pl->cwq].w == PF_W && pl->wp[pl->cwq].nt == 2 * PF_W && opt.prune_seg == 64;
   pl->cw_nwords = pl->cwq >= 0 ? (int)(((pl->prune_nseg + 1) / 2) * (2 * opt.prune_seg / 32)) : 0;
   pl->off_cwdense = off; off = align_up(off + (size_t)pl->pairs_per_chunk * ((pl->prune_nseg + 1) / 2) + 1, 256);
   pl->off_cwmask = off; off = align_up(off + (size_t)pl->pairs_per_chunk * pl->cw_nwords * p->nf * sizeof(uint32_t), 256);
@@ -593,7 +596,7 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
   for (int q = 0; q < p->nwidths; ++q) active += (pl->wp[q].nwin > 0 && q != pl->wid1) ? 1 : 0;
   // kernels of this library per search (the key memset is a driver memset, not counted)
   // (a search without dense peaks; with them the candidates-only index mode and its k_winthr launch are off)
-  pl->launches = s.nwin_total > 0 ? (int)(pl->nchunks * (1 + active + (pl->nslide > 0 ? 1 : 0) + ((pl->cand_only && (pl->nuntag || pl->nprune)) ? 1 : 0) + ((pl->nprune || pl->cwq >= 0) ? 1 : 0) + (pl->nuntag ? 1 : 0) + (pl->cwq >= 0 ? 1 : 0) + 3 * pl->nsf) + 3) : 0;
+  pl->launches = s.nwin_total > 0 ? (int)(pl->nchunks * (1 + active + (pl->nslide > 0 ? 1 : 0) + ((pl->cand_only && (pl->nuntag || pl->nprune)) ? 1 : 0) + ((pl->nprune || (pl->cwq >= 0 && !pl->cw_pf)) ? 1 : 0) + (pl->cw_pf ? 1 : 0) + (pl->nuntag ? 1 : 0) + (pl->cwq >= 0 ? 1 : 0) + 3 * pl->nsf) + 3) : 0;
 
   // tables, computed in double precision on the host
   if (psub > 1) { pl->premod_off = tw_total; tw_total += (size_t)s.nf; }
@@ -797,6 +800,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
       if (d_stage && !cuda_ok(cudaEventRecord(pl->ev_free[ch & 1], st))) return VOLKS_ECUDA;
     }
     const bool use_cw = pl->cwq >= 0 && pl->wp[pl->cwq].nwin > 0;   // (needs the pre-thresholds and k_bound in both index modes)
+    const int cw_in_bound = use_cw && !pl->cw_pf ? 1 : 0;           // the column-level width is one of k_bound's widths
     if (hy || use_cw) {
       WinThrArgs ta;
       ta.E = E; ta.thr = (uint32_t *)(ws + pl->off_thr); ta.per_pair = s.per_pair; ta.pair0 = pair0;
@@ -828,11 +832,13 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         }
         pa.cwmask = nullptr; pa.cw_nwords = pl->cw_nwords; pa.cwdense = (unsigned char *)(ws + pl->off_cwdense);
         if (use_cw) {
+          pa.cwmask = (uint32_t *)(ws + pl->off_cwmask);
+          if (!cuda_ok(cudaMemsetAsync(pa.cwmask, 0, (size_t)np * pl->cw_nwords * s.nf * sizeof(uint32_t), st))) return VOLKS_ECUDA;
+        }
+        if (cw_in_bound) {
           const WidthPlan &w = pl->wp[pl->cwq];
           const int i = pa.nq++;
           pa.w[i] = w.w; pa.nwin[i] = (int)w.nwin; pa.offc[i] = s.offc[pl->cwq]; pa.wmax = std::max(pa.wmax, w.w);
-          pa.cwmask = (uint32_t *)(ws + pl->off_cwmask);
-          if (!cuda_ok(cudaMemsetAsync(pa.cwmask, 0, (size_t)np * pl->cw_nwords * s.nf * sizeof(uint32_t), st))) return VOLKS_ECUDA;
         }
         const int thr = std::min(PRUNE_THREADS, s.nf / 2);   // (nf >= 64: a power of two >= 32)
         pa.ring = pa.wmax <= 16 ? 16 : 32;                 // rows of amplitude history (a power of two >= wmax)
@@ -842,11 +848,21 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         ProfScope ps(pl, st, VOLKS_K_BOUND, -1);
 #define VOLKS_BOUND(NQ_)                                                                   \
   case NQ_:                                                                                \
-    if (use_cw) { if (nthr_t == 128) k_bound<NQ_, 1, 128><<<blocks, thr, smem, st>>>(pa); else k_bound<NQ_, 1, 64><<<blocks, thr, smem, st>>>(pa); } \
+    if (cw_in_bound) { if (nthr_t == 128) k_bound<NQ_, 1, 128><<<blocks, thr, smem, st>>>(pa); else k_bound<NQ_, 1, 64><<<blocks, thr, smem, st>>>(pa); } \
     else { if (nthr_t == 128) k_bound<NQ_, 0, 128><<<blocks, thr, smem, st>>>(pa); else k_bound<NQ_, 0, 64><<<blocks, thr, smem, st>>>(pa); } \
     break;
         switch (pa.nq) { VOLKS_BOUND(1) VOLKS_BOUND(2) VOLKS_BOUND(3) VOLKS_BOUND(4) VOLKS_BOUND(5) VOLKS_BOUND(6) VOLKS_BOUND(7) VOLKS_BOUND(8) }
 #undef VOLKS_BOUND
+        if (use_cw && pl->cw_pf) {     // the column-level width's bits by the folded bound (same stream, same profile slot)
+          const WidthPlan &w = pl->wp[pl->cwq];
+          PairFoldArgs fa;
+          fa.Y = Y; fa.thr = ta.thr; fa.cwmask = pa.cwmask; fa.cwdense = pa.cwdense;
+          fa.per_pair = s.per_pair; fa.offc = s.offc[pl->cwq];
+          fa.nap = s.nap; fa.nf = s.nf; fa.pitch = pl->pitch; fa.nwin = (int)w.nwin; fa.cw_nwords = pl->cw_nwords;
+          fa.ntile128 = (pl->prune_nseg + 1) / 2;
+          fa.ncp = pa.ncp; fa.cp_na = pa.cp_na; fa.cp_a0 = pa.cp_a0; fa.cp_b0 = pa.cp_b0;
+          k_pairfold<<<(unsigned)(np * ((w.nwin + PF_T - 1) / PF_T)), PF_THREADS, pairfold_smem_bytes(), st>>>(fa);
+        }
       }
     }
     for (int q = 0; q < s.nwidths; ++q) {
@@ -885,7 +901,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         sa.ndt = pl->dt_n; sa.dt_na = pl->dt_na; sa.dt_a0 = pl->dt_a0; sa.dt_b0 = pl->dt_b0;
         sa.ntasks = ((np * w.nseg * (long long)pl->dt_n) << w.log2m);
         sa.flags = flags && w.prune >= 0 ? flags + (size_t)w.prune * pl->prune_nseg : nullptr;
-        sa.flag_stride = (pl->nprune + (use_cw ? 1 : 0)) * pl->prune_nseg;
+        sa.flag_stride = (pl->nprune + cw_in_bound) * pl->prune_nseg;
         if (hy && w.cw) { sa.flags = (const unsigned char *)(ws + pl->off_cwdense); sa.flag_stride = (pl->prune_nseg + 1) / 2; }   // dense tiles only
         sa.thr = (const uint32_t *)(ws + pl->off_thr); sa.hits = nullptr; sa.nblk = w.nblk;
         if (fold) {
@@ -949,7 +965,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
       fa.nap = s.nap; fa.nf = s.nf; fa.log2nf = s.log2nf; fa.pitch = pl->pitch; fa.paired = pl->paired;
       fa.nq = 0; fa.unit0[0] = 0;
       fa.cwdense = hy && use_cw ? (const unsigned char *)(ws + pl->off_cwdense) : nullptr; fa.cw_i = -1; fa.cw_ntile = (pl->prune_nseg + 1) / 2;
-      fa.flags = flags; fa.flag_nq = pl->nprune + (use_cw ? 1 : 0); fa.flag_nseg = pl->prune_nseg;
+      fa.flags = flags; fa.flag_nq = pl->nprune + cw_in_bound; fa.flag_nseg = pl->prune_nseg;
       for (int q = 0; q < s.nwidths; ++q) {
         const WidthPlan &w = pl->wp[q];
         if (!w.slide || w.nwin == 0) continue;
