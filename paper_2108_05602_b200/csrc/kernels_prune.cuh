@@ -213,8 +213,8 @@ __global__ void __launch_bounds__(NTHR) k_bound(PruneArgs a) {
 // lets 2 - 3 % of the (window, column) pairs through to k_coleval.  A candidate's bin exceeds the pre-threshold, so its
 // column's bit is set (exactness as for k_bound); the bits and the per-tile density bytes have k_bound's format.
 //   CTA = (pair, 256 window starts), thread = column pair; per row: one 128-bit load (eight rows in flight), the row 16
-//   back from a shared-memory ring, four packed complex add/subtracts, four packed |.|^2, eight square roots, the four
-//   amplitudes 16 rows back from a second ring, e_rho += A_new - A_old, the largest e per column, its square against the
+//   back from registers (the loop is unrolled 16 times), four packed complex add/subtracts, four packed |.|^2, eight square roots, the four
+//   amplitudes 16 rows back from a shared-memory ring, e_rho += A_new - A_old, the largest e per column, its square against the
 //   window's pre-threshold by a sign-bit shift register (as in k_bound).
 constexpr int PF_T = 256;          // window starts per CTA (two tiles of k_coleval)
 constexpr int PF_W = 32;           // the width this kernel is for (Nt = 64)
@@ -231,7 +231,7 @@ struct PairFoldArgs {
 };
 
 __host__ __device__ inline size_t pairfold_smem_bytes() {
-  return (size_t)(PF_T + 64) * sizeof(float) + (size_t)16 * PF_THREADS * 16 + (size_t)4 * 16 * PF_THREADS * 8;
+  return (size_t)(PF_T + 64) * sizeof(float) + (size_t)4 * 16 * PF_THREADS * 8;
 }
 
 __global__ void __launch_bounds__(PF_THREADS) k_pairfold(PairFoldArgs a) {
@@ -250,19 +250,21 @@ __global__ void __launch_bounds__(PF_THREADS) k_pairfold(PairFoldArgs a) {
   const int nrows = min(PF_T + PF_W - 1, a.nap - R0);
   const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch);
   const size_t rowb = (size_t)a.pitch * 8u;
-  // rings (slot = row & 15): the raw rows [16][PF_THREADS] float4, the amplitudes [4][16][PF_THREADS] f32x2
-  const uint32_t raw = (uint32_t)__cvta_generic_to_shared(thr_sm + PF_T + 64) + threadIdx.x * 16u;
-  char *amp = (char *)(thr_sm + PF_T + 64) + 16 * PF_THREADS * 16 + threadIdx.x * 8u;
-  constexpr uint32_t RAWROW = PF_THREADS * 16, AMPROW = PF_THREADS * 8, AMPRHO = 16 * AMPROW;
+  // ring (slot = row & 15) of the amplitudes [4][16][PF_THREADS] f32x2
+  char *amp = (char *)(thr_sm + PF_T + 64) + threadIdx.x * 8u;
+  constexpr uint32_t AMPROW = PF_THREADS * 8, AMPRHO = 16 * AMPROW;
   __syncthreads();
   int cnt0 = 0, cnt1 = 0;                                      // set bits of the two 128-window halves
   for (int ci = threadIdx.x; ci < a.ncp; ci += PF_THREADS) {
     const int c = ci < a.cp_na ? a.cp_a0 + ci : a.cp_b0 + (ci - a.cp_na);
     for (int k = 0; k < 64; ++k) *(f32x2 *)(amp + (uint32_t)k * AMPROW) = pk(0.f, 0.f);
     const char *p = ybase + (size_t)R0 * rowb + (size_t)c * 16u;
-    f32x2 bx[16], by[16];                                      // sixteen rows in flight (two CTAs per SM: registers to spare)
+    f32x2 bx[8], by[8];                                        // eight rows in flight
+    f32x2 px[16], py[16];                                      // the sixteen rows before the current one (registers, not a ring)
 #pragma unroll
-    for (int u = 0; u < 16; ++u) { bx[u] = by[u] = pk(0.f, 0.f); if (u < nrows) ldg2(p + (size_t)u * rowb, bx[u], by[u]); }
+    for (int u = 0; u < 8; ++u) { bx[u] = by[u] = pk(0.f, 0.f); if (u < nrows) ldg2(p + (size_t)u * rowb, bx[u], by[u]); }
+#pragma unroll
+    for (int u = 0; u < 16; ++u) px[u] = py[u] = pk(0.f, 0.f);
     f32x2 e0 = pk(0.f, 0.f), e1 = e0, e2 = e0, e3 = e0;
     uint32_t cwa = 0, cwb = 0;
     int cwn = PF_W + 31;                                       // rows until the next word of 32 windows is complete
@@ -272,13 +274,13 @@ __global__ void __launch_bounds__(PF_THREADS) k_pairfold(PairFoldArgs a) {
 #pragma unroll
       for (int u = 0; u < 16; ++u) {
         const int r = r16 + u;
-        const f32x2 x = bx[u], y = by[u];
-        if (r + 16 < nrows) ldg2(p + (size_t)(r + 16) * rowb, bx[u], by[u]);
+        const f32x2 x = bx[u & 7], y = by[u & 7];
+        if (r + 8 < nrows) ldg2(p + (size_t)(r + 8) * rowb, bx[u & 7], by[u & 7]);
         if (r < nrows) {
           const uint32_t slot = (uint32_t)u;                   // = r & 15: after unrolling the ring offsets are immediates
+          const f32x2 xo = px[u], yo = py[u];                  // the row 16 back: the class's first sample
+          px[u] = x; py[u] = y;
           if (r16 > 0) {
-            f32x2 xo, yo;                                      // the row 16 back: the class's first sample
-            lds2(raw + slot * RAWROW, xo, yo);
             // f_rho = y[t] + (-i)^rho y[t + 16]:  rho 0: (xo + x, yo + y), 1: (xo + y, yo - x), 2: (xo - x, yo - y), 3: (xo - y, yo + x)
             const f32x2 ax0 = add2(xo, x), ay0 = add2(yo, y), ax2 = sub2(xo, x), ay2 = sub2(yo, y);
             const f32x2 ax1 = add2(xo, y), ay1 = sub2(yo, x), ax3 = sub2(xo, y), ay3 = add2(yo, x);
@@ -301,7 +303,6 @@ __global__ void __launch_bounds__(PF_THREADS) k_pairfold(PairFoldArgs a) {
             e3 = add2(e3, sub2(A3, *(const f32x2 *)(as + 3 * AMPRHO)));
             *(f32x2 *)(as) = A0; *(f32x2 *)(as + AMPRHO) = A1; *(f32x2 *)(as + 2 * AMPRHO) = A2; *(f32x2 *)(as + 3 * AMPRHO) = A3;
           }
-          asm volatile("st.shared.v2.b64 [%0], {%1, %2};" ::"r"(raw + slot * RAWROW), "l"(x), "l"(y) : "memory");
           // the window ending at this row (start r - 31): the largest of the four bounds per column, squared, against its
           // pre-threshold; the sign bit of thr - e^2 enters the shift register (latest window in bit 0)
           const float ma = fmaxf(fmaxf(lo32(e0), lo32(e1)), fmaxf(lo32(e2), lo32(e3)));

@@ -721,6 +721,42 @@ def test_pruning_keeps_every_candidate(vb, oracle, prune_seg):
     plan.close()
 
 
+@pytest.mark.gpu
+def test_folded_column_bound_every_residue(vb, oracle):
+    """The column bits of the w = 32 width come from k_pairfold's folded bound, four sliding sums of
+    |y[t] + (-i)^rho y[t + 16]| (rho = rate bin mod 4).  Pulses barely above the threshold whose rate falls into each of
+    the four residues - a wrong sign in one of the four combinations would lose exactly one of them - placed at the
+    kernel's tile seam (window 256), at the first and the last windows, plus two tones (the dense rule) on one pair.  Candidates-only and full-index lists are checked against the oracle by run_both."""
+    vis, c, _ = workloads.generate(2, nbl=2, nif=2, nap=900, npulses=0)
+    nbl, nif, nap, nchan = vis.shape
+    k = torch.arange(nchan, dtype=torch.float64)
+    t = torch.arange(nap, dtype=torch.float64)
+    def pulse(bl, ifq, t0, w, a, tau, r, nt=64):
+        # delay tau (channels -> columns) and rate bin r of an Nt-point transform: + signs (workloads/gen.py)
+        ph = 2 * np.pi * tau * k[None, :] / nchan + 2 * np.pi * r * t[t0:t0 + w, None] / nt
+        vis[bl, ifq, t0:t0 + w] += torch.polar(torch.full(ph.shape, a, dtype=torch.float64), ph).to(torch.complex64)
+    a32 = 7.5 / np.sqrt(32 * nchan)             # amplitude of a 32-AP pulse at S/N 7.5 in the w = 32 plane (noise power 1 per sample)
+    # (baseline 0 carries configs[2]'s own interference - a dense pair; the pulses go on baseline 1)
+    pulse(1, 0, 100, 32, a32, 3.0, 0)
+    pulse(1, 0, 240, 32, a32, -7.0, 1)          # straddles window 256
+    pulse(1, 1, 400, 32, a32, 11.0, 2)
+    pulse(1, 1, 520, 32, a32, 0.5, 3)
+    pulse(1, 0, 0, 32, a32, 20.0, 5)            # the first windows, residue 1
+    pulse(1, 0, nap - 32, 32, a32, -15.0, 62)   # the last window, residue 2
+    pulse(1, 1, 640, 32, a32, 2.0, 31)          # residue 3
+    # two tones (one alone never reaches S/N 6 at w = 32: its own energy raises the noise estimate to S/N -> sqrt(32));
+    # where they add coherently - 40 % of the delay columns - every window's bit is set: the dense rule
+    for ch in (7, 50):
+        vis[0, 1, :, ch] += (30.0 * torch.exp(2j * np.pi * 0.003 * t)).to(torch.complex64)
+    cc = dict(c, widths=[32, 64], strides=[1, 1], nts=[64, 128])
+    for opts in (None, dict(full_index=1)):
+        stats, ncand, cands, ora = run_both(vb, oracle, vis, cc, options=opts)
+        got = {(int(x["bl"]), int(x["ifq"]), int(x["wid"])) for x in cands}
+        assert {(0, 1, 0), (1, 0, 0), (1, 1, 0)} <= got                 # the tones' pair and both pulse pairs have w = 32 candidates
+        w32 = cands[(cands["wid"] == 0) & (cands["bl"] == 1)]
+        assert {int(r) % 4 for r in w32["rate_idx"]} == {0, 1, 2, 3}
+
+
 @pytest.mark.parametrize("cfg,over,ranges", [
     (2, dict(nbl=1, nif=2, nap=500, npulses=3), [(250, 5), (3, 40), (100, 100), (64, 127), (1, 255)]),   # nf 256: sliding kernels, all widths
     (3, dict(nbl=2, nif=1, nap=700, npulses=3), [(120, 7), (0, 63), (9, 9)]),                            # nf 128, incl. w = 1 (row kernel peaks)
