@@ -23,10 +23,10 @@
 //   k_sfold_density   per (pair, segment): more than 1/8 of the segment's hit bits set (interference: a tone raises |Y| in
 //                 every delay column) -> `dense`: the ordinary sliding kernel evaluates that segment (it costs 141 warp
 //                 instructions per 1024 bins of a window; an evaluation from the samples several times that).
-//   k_sfold_eval  the other segments: a warp reads 32 masks, ballots the non-zero ones and takes them in turn: the first
-//                 flagged window of the (rho, tile) is folded from its w samples, the following ones by sliding; at every
-//                 flagged window the 16-point transform of a copy, |.|^2, the first maximum in plane order: exact keys
-//                 (power, plane index), atomicMax per window.
+//   k_sfold_compact, k_sfold_eval  the other segments: their non-zero mask words go into a list; a fixed grid of warps
+//                 takes one word at a time: the first flagged window of the (rho, tile) is folded from its w samples, the
+//                 following ones by sliding; at every flagged window the 16-point transform of a copy, |.|^2, the first
+//                 maximum in plane order: exact keys (power, plane index), atomicMax per window.
 // A candidate has a bin above the pre-threshold, so its (rho, tile) is flagged and evaluated exactly; a window without a
 // flagged tile keeps the zero key (not a candidate - all the candidates-only mode promises, R6).
 #pragma once
@@ -39,11 +39,14 @@ namespace volks {
 #define SFOLD_SEGMUL 4            // segment of k_slide<FOLD> = this many segments of the sliding kernel
 #endif
 
+constexpr int SFOLD_EVAL_WARPS = 148 * 8;   // k_sfold_eval's grid: one-warp CTAs, 8 resident per SM at 248 registers
+
 struct SfoldArgs {
   const float2 *Y;       // [pairs of the chunk][nap][pitch] pair-interleaved delay spectra
   const float4 *tw4;     // [nt] rate twiddles exp(-2 pi i k/nt), pre-broadcast (re, re, im, im)
   const unsigned short *hits;   // [pairs of the chunk][nblk][ndt][M] hit masks of k_slide<FOLD>: bit B = window 16 blk + B
   unsigned char *dense;  // [pairs of the chunk][nseg]
+  uint32_t *list;        // [0] = number of entries, then the indices of the non-zero mask words of the sparse segments
   u64 *keys;             // canonical window keys
   long long ntasks;      // k_sfold_eval: warps = pairs * nblk * ndt * M;  k_sfold_density: CTAs = pairs * nseg
   long long per_pair, offc, pair0;
@@ -66,28 +69,38 @@ __global__ void __launch_bounds__(128) k_sfold_density(SfoldArgs a) {
   if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = n;
   __syncthreads();
   if (threadIdx.x == 0) a.dense[pl * a.nseg + sg] = (unsigned char)((part[0] + part[1] + part[2] + part[3]) * 8 > nwords * 16 ? 1 : 0);
+  if (blockIdx.x == 0 && threadIdx.x == 0) a.list[0] = 0;   // (k_sfold_compact follows on the same stream)
 }
 
-// ONE warp per CTA (a CTA's registers are released only when all its warps are done, and nearly every warp is done at
-// once).  The warp reads 32 consecutive hit words in one coalesced load, ballots the non-zero ones of segments the
-// sliding kernel does not have, and works through those one after the other (each needs the whole warp).
+// the non-zero mask words of the segments the sliding kernel does not take, as a list (order: whatever the atomics give -
+// the evaluation ends in atomicMax over a total order, so the result does not depend on it).  The flagged words cluster
+// around the pulses: with one warp per 32 consecutive words the busy warps decided the kernel's length (61 % of the SMs'
+// cycles active); from the list every warp takes one word at a time.
+__global__ void __launch_bounds__(256) k_sfold_compact(SfoldArgs a) {
+  const long long w0 = (long long)blockIdx.x * 256 + threadIdx.x;      // hit word (pair, block, tile, rho)
+  bool take = false;
+  if (w0 < a.ntasks && a.hits[w0] != 0) {
+    const long long q = (w0 >> a.log2m) / a.ndt;                       // pair * nblk + block
+    take = !a.dense[(q / a.nblk) * a.nseg + (int)((q % a.nblk) / (a.seg >> 4))];
+  }
+  const uint32_t m = __ballot_sync(0xffffffffu, take);
+  if (m == 0) return;
+  const uint32_t lane = threadIdx.x & 31u;
+  uint32_t base = 0;
+  if (lane == (uint32_t)(__ffs(m) - 1)) base = atomicAdd(a.list, (uint32_t)__popc(m));
+  base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
+  if (take) a.list[1 + base + __popc(m & ((1u << lane) - 1u))] = (uint32_t)w0;
+}
+
+// ONE warp per CTA (a CTA's registers are released only when all its warps are done); a fixed grid of warps walks the
+// list of k_sfold_compact, one mask word (16 windows of one (pair, rate residue, 64-column tile)) at a time.
 __global__ void __launch_bounds__(32) k_sfold_eval(SfoldArgs a) {
   const uint32_t lane = threadIdx.x & 31u;
-  const long long w0 = (long long)blockIdx.x * 32 + lane;              // this lane's hit word (pair, block, tile, rho)
   const int M = 1 << a.log2m;
-  uint32_t mymask = 0;
-  if (w0 < a.ntasks) {
-    mymask = a.hits[w0];
-    if (mymask) {
-      const long long q = (w0 >> a.log2m) / a.ndt;                     // pair * nblk + block
-      if (a.dense[(q / a.nblk) * a.nseg + (int)((q % a.nblk) / (a.seg >> 4))]) mymask = 0;   // the sliding kernel has this segment
-    }
-  }
-  uint32_t todo = __ballot_sync(0xffffffffu, mymask != 0);
-  for (; todo; todo &= todo - 1) {
-  const int src = __ffs(todo) - 1;
-  uint32_t mask = __shfl_sync(0xffffffffu, mymask, src);
-  long long wt = (long long)blockIdx.x * 32 + src;
+  const uint32_t nlist = a.list[0];
+  for (uint32_t li = blockIdx.x; li < nlist; li += gridDim.x) {
+  long long wt = (long long)a.list[1 + li];
+  const uint32_t mask = a.hits[wt];
   const uint32_t rho = (uint32_t)(wt & (M - 1)); wt >>= a.log2m;
   const int dti = (int)(wt % a.ndt); wt /= a.ndt;
   const int dt = dti < a.dt_na ? a.dt_a0 + dti : a.dt_b0 + (dti - a.dt_na);
