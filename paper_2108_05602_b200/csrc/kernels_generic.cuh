@@ -387,6 +387,114 @@ __global__ void __launch_bounds__(256) k_row2(RowArgs a) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// Row (delay) FFT for nf = 128 as 16 x 8 (n = n1 + 16 n2, k = 8 k1 + k2): a row is a group of EIGHT lanes, every lane
+// busy in both steps (k_row2<8, 16, .> leaves half of its 16 lanes idle in step A), four rows per warp, and a CTA walks
+// ROW128_RB batches of 32 rows so that a thread's twiddles W_128^{n1 k2} (n1 = l, l + 8) are formed once, not per row.
+// ncu on configs[3] (nchan 32): k_row2<8, 16, 4> issued 275 warp instructions per row at 61 % of the HBM bandwidth.
+//   step A, lane l: for n1 = l and l + 8 the 8-point packed DIF FFT over n2 pruned to the NZA non-zero inputs (nchan <= 16 NZA),
+//           times W_128^{n1 k2}, into shared memory E[n1][k2];  step C, lane k2 = l: 16-point FFT over n1, paired store,
+//           per-AP energy, the w = 1 peak - as in k_row2.
+// ------------------------------------------------------------------------------------------------
+constexpr int ROW128_RB = 4;      // batches of 32 rows per CTA
+
+__device__ __forceinline__ void c2_powers8(const float2 *tab, int ts, f32x2 (&w)[8]) {
+  w[0] = pk(1.f, 0.f);
+  w[1] = c2_from(__ldg(tab + ts)); w[4] = c2_from(__ldg(tab + 4 * ts));
+  w[2] = c2_mul(w[1], w[1]); w[3] = c2_mul(w[2], w[1]);
+  w[5] = c2_mul(w[4], w[1]); w[6] = c2_mul(w[4], w[2]); w[7] = c2_mul(w[4], w[3]);
+}
+
+template <int NZA>
+__global__ void __launch_bounds__(256) k_row128(RowArgs a) {
+  constexpr int N1 = 16, N2 = 8, G = 8, RPC = 256 / G, EP = N2 + 1;
+  constexpr int GS = N1 * EP + 8;                         // f32x2 per row group: 16 banks between neighbours (no conflicts)
+  __shared__ f32x2 ex[RPC * GS];
+  const int g = threadIdx.x / G, l = threadIdx.x % G;
+  f32x2 *E = ex + g * GS;
+  f32x2 wA[8], wB[8];                                     // W_128^{n1 k2} for n1 = l and l + 8
+  c2_powers8(a.twf, l, wA);
+  c2_powers8(a.twf, l + 8, wB);
+  float *dst0 = (float *)a.Y;
+  for (int rb = 0; rb < ROW128_RB; ++rb) {
+    const long long rfirst = ((long long)blockIdx.x * ROW128_RB + rb) * RPC;
+    if (rfirst >= a.nrows) break;                         // (uniform)
+    const long long rrel = rfirst + g;
+    const bool live = rrel < a.nrows;
+    float e = 0.f;
+    const RowSrc src(a, live ? a.row0 + rrel : a.row0);
+#pragma unroll
+    for (int ia = 0; ia < 2; ++ia) {
+      const int n1 = l + 8 * ia;
+      f32x2 z[N2];
+      float2 v[NZA];
+      if (!src.gather) {
+#pragma unroll
+        for (int n2 = 0; n2 < NZA; ++n2) {
+          const int n = n1 + N1 * n2;
+          v[n2] = (live && n < a.nchan) ? __ldg(src.base + n) : make_float2(0.f, 0.f);
+        }
+      } else {
+        src.template load_strided<NZA>(n1, N1, live ? a.nchan : 0, v);
+      }
+#pragma unroll
+      for (int n2 = 0; n2 < NZA; ++n2) { e += cnorm(v[n2]); z[n2] = c2_from(v[n2]); }
+      FftDif2<N2, NZA, 0, N2>::run(z);
+#pragma unroll
+      for (int i = 0; i < N2; ++i) {
+        const int k2 = brev<N2>(i);
+        E[n1 * EP + k2] = k2 ? c2_mul(z[i], ia ? wB[k2] : wA[k2]) : z[i];
+      }
+    }
+#pragma unroll
+    for (int o = G >> 1; o >= 1; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+    if (live && l == 0) { const long long ei = e_index(a, a.row0 + rrel); if (ei >= 0) a.E[ei] = e; }
+    __syncwarp();
+    f32x2 v[N1];
+#pragma unroll
+    for (int n1 = 0; n1 < N1; ++n1) v[n1] = E[n1 * EP + l];
+    __syncwarp();                                         // E is rewritten by the next batch
+    FftDif2<N1, N1, 0, N1>::run(v);
+    float *dst = dst0 + rrel * (long long)a.pitch * 2;
+    if (a.dlo >= 0) {   // uniform: restricted delay range - the spectra outside it are written as zero
+#pragma unroll
+      for (int i = 0; i < N1; ++i)
+        if (!delay_ok(N2 * brev<N1>(i) + l, a.dlo, a.dhi)) v[i] = pk(0.f, 0.f);
+    }
+    // column 2c keeps (re, re') and column 2c + 1 keeps (im, im') of the pair's float4: one 64-bit store per lane
+    float *dstl = dst + ((l >> 1) << 2) + ((l & 1) << 1);
+#pragma unroll
+    for (int i = 0; i < N1; ++i) {
+      const float re = lo32(v[i]), im = hi32(v[i]);
+      const float got = __shfl_xor_sync(0xffffffffu, (l & 1) ? re : im, 1);
+      if (live) *(float2 *)(dstl + 2 * N2 * brev<N1>(i)) = (l & 1) ? make_float2(got, im) : make_float2(re, got);
+    }
+    if (a.keys1) {   // uniform branch: the w = 1 peaks (power, lowest column) of this row
+      float bp = -1.f;
+      int bc = 0;
+#pragma unroll
+      for (int i = 0; i < N1; ++i) {
+        const int col = N2 * brev<N1>(i) + l;
+        const float pw = fmaf(lo32(v[i]), lo32(v[i]), hi32(v[i]) * hi32(v[i]));
+        if (pw > bp || (pw == bp && col < bc)) { bp = pw; bc = col; }
+      }
+      u64 key = make_key(bp, (uint32_t)bc);
+#pragma unroll
+      for (int o = G >> 1; o >= 1; o >>= 1) {
+        const u64 other = __shfl_xor_sync(0xffffffffu, key, o);
+        key = other > key ? other : key;
+      }
+      if (live && l == 0) {
+        const long long row = a.row0 + rrel;
+        const long long pair = row / a.nap;
+        const int t = (int)(row - pair * a.nap);
+        const int j = t / a.stride1;
+        if (j * a.stride1 == t && j < a.nwin1) a.keys1[pair * a.per_pair + j] = key;
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Row (delay) FFT, register form, for nf = 256 * N3 (N3 = 2, 4, 8: nf = 512, 1024, 2048 = config 4).
 // One row per CTA of 256 threads.  n = n' + 256 n3 (n' < 256), k = N3 k' + k3:
 //   X[N3 k' + k3] = sum_{n'} W_256^{n' k'} [ W_nf^{n' k3} sum_{n3} x[n' + 256 n3] W_N3^{n3 k3} ]

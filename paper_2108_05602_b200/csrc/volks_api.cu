@@ -186,6 +186,18 @@ static bool launch_row2(const RowArgs &a, cudaStream_t st) {
     }
     return false;
   }
+  if (a.nf == 128) {           // 16 x 8 with eight lanes per row (k_row128)
+    int nza = 1;
+    while (nza * 16 < a.nchan) nza *= 2;
+    const unsigned blocks = (unsigned)((a.nrows + 32 * ROW128_RB - 1) / (32 * ROW128_RB));
+    switch (nza) {
+      case 1: k_row128<1><<<blocks, 256, 0, st>>>(a); return true;
+      case 2: k_row128<2><<<blocks, 256, 0, st>>>(a); return true;
+      case 4: k_row128<4><<<blocks, 256, 0, st>>>(a); return true;
+      case 8: k_row128<8><<<blocks, 256, 0, st>>>(a); return true;
+    }
+    return false;
+  }
   int n1, n2;
   if (a.nf == 256) { n1 = 16; n2 = 16; } else if (a.nf == 128) { n1 = 8; n2 = 16; } else if (a.nf == 64) { n1 = 8; n2 = 8; } else return false;
   int nza = 1;
