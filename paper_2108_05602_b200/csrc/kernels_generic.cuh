@@ -835,6 +835,13 @@ struct Sched {   // the window schedule (device copy lives in the plan)
 
 struct WinStat { float power, snr; int rate_idx, delay_idx, q, j, t0; long long pair; };
 
+// the CTA's shared copy of the schedule, word by word by all threads (one thread copying 640 bytes was a quarter of
+// k_finalize on a candidates-only search, where the rest of the kernel is a scan of the keys); caller synchronises
+__device__ __forceinline__ void sched_load(Sched &dst, const Sched *src) {
+  static_assert(sizeof(Sched) % 4 == 0, "copied as 32-bit words");
+  for (int i = threadIdx.x; i < (int)(sizeof(Sched) / 4); i += blockDim.x) ((uint32_t *)&dst)[i] = ((const uint32_t *)src)[i];
+}
+
 // Selection statistic: the in-plane amplitude snr (a7), or - when `zst` is given (f4, the other reading
 // of PAPER.md:196) - the peak power normalised ACROSS the windows of its (pair, width) series:
 // z = (P1 - mean) * inv_std with zst[pair * nwidths + q] = (mean, 1/std) (inv_std = 0 when std = 0).
@@ -921,13 +928,18 @@ __global__ void __launch_bounds__(FIN_THREADS) k_finalize(const Sched *sp, const
                                                           const double2 *zst, float zth, const float *noise) {
   __shared__ Sched s;
   __shared__ uint32_t wsum[FIN_THREADS / 32];
-  if (threadIdx.x == 0) s = *sp;
+  sched_load(s, sp);
   __syncthreads();
   uint32_t mine = 0;
   const long long base = (long long)blockIdx.x * (FIN_THREADS * FIN_TILES);
+  // a zero key is a window with power 0 and snr 0 (window_stat): with a non-negative threshold and neither dense peaks nor
+  // the z-score asked for it is no candidate and nothing is written - no index arithmetic for it (a candidates-only search
+  // leaves most keys zero: the pass is then a scan of the key array)
+  const bool skip_zero = !peaks && !zst && s.snr_thresh >= 0.f;
   for (int tile = 0; tile < FIN_TILES; ++tile) {
     const long long c = base + tile * FIN_THREADS + threadIdx.x;
     if (c < s.nwin_total) {
+      if (skip_zero && (keys[c] >> 32) == 0ull) continue;
       const WinStat o = window_stat(s, keys, E, c, zst, noise);
       if (peaks) {
         const long long di = s.offd[o.q] + o.pair * s.nwin[o.q] + o.j;
@@ -969,19 +981,24 @@ struct CandOut { int bl, ifq, wid, win, t0, rate_idx, delay_idx; float power, sn
 
 __global__ void __launch_bounds__(FIN_THREADS) k_scatter(const Sched *sp, const u64 *keys, const float *E,
                                                          const uint32_t *blockoff, CandOut *cands,
-                                                         uint32_t capacity, const double2 *zst, float zth, const float *noise) {
+                                                         uint32_t capacity, const double2 *zst, float zth, const float *noise,
+                                                         const uint32_t *total) {
   __shared__ Sched s;
   __shared__ uint32_t wsum[FIN_THREADS / 32];
   __shared__ uint32_t running;
-  if (threadIdx.x == 0) { s = *sp; running = blockoff[blockIdx.x]; }
+  // a block without candidates (k_finalize counted them; `total` is k_scan's sum) has nothing to write
+  if ((blockIdx.x + 1 < gridDim.x ? blockoff[blockIdx.x + 1] : *total) == blockoff[blockIdx.x]) return;
+  sched_load(s, sp);
+  if (threadIdx.x == 0) running = blockoff[blockIdx.x];
   __syncthreads();
+  const bool skip_zero = !zst && s.snr_thresh >= 0.f;
   const long long base = (long long)blockIdx.x * (FIN_THREADS * FIN_TILES);
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   for (int tile = 0; tile < FIN_TILES; ++tile) {
     const long long c = base + tile * FIN_THREADS + threadIdx.x;
     WinStat o;
     bool flag = false;
-    if (c < s.nwin_total) {
+    if (c < s.nwin_total && !(skip_zero && (keys[c] >> 32) == 0ull)) {
       o = window_stat(s, keys, E, c, zst, noise);
       flag = o.snr > (zst ? zth : s.snr_thresh);
     }

@@ -1037,7 +1037,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
   }
   {
     ProfScope ps(pl, st, VOLKS_K_SCATTER, -1);
-    k_scatter<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity, nullptr, 0.f, noise);
+    k_scatter<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity, nullptr, 0.f, noise, d_ncand);
   }
   return cuda_ok(cudaGetLastError()) ? VOLKS_OK : VOLKS_ECUDA;
 }
@@ -1058,7 +1058,7 @@ int volks_zscore_select(const volks_plan *pl, void *d_workspace, float z_thresh,
   k_zstat<<<(unsigned)(pl->npair * s.nwidths), 256, 0, st>>>(pl->d_sched, keys, E, zst, noise);
   k_finalize<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, (float4 *)d_peaks, cnt, zst, z_thresh, noise);
   k_scan<<<1, 1024, 0, st>>>(cnt, pl->nfin_blocks, d_ncand);
-  k_scatter<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity, zst, z_thresh, noise);
+  k_scatter<<<(unsigned)pl->nfin_blocks, FIN_THREADS, 0, st>>>(pl->d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity, zst, z_thresh, noise, d_ncand);
   return cuda_ok(cudaGetLastError()) ? VOLKS_OK : VOLKS_ECUDA;
 }
 
@@ -1374,6 +1374,6 @@ extern "C" int volks_search_noalloc(const volks_params *p, const void *d_vis, vo
   }
   k_finalize<<<(unsigned)nfin, FIN_THREADS, 0, st>>>(d_sched, keys, E, (float4 *)d_peaks, cnt, nullptr, 0.f, nullptr);
   k_scan<<<1, 1024, 0, st>>>(cnt, nfin, d_ncand);
-  k_scatter<<<(unsigned)nfin, FIN_THREADS, 0, st>>>(d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity, nullptr, 0.f, nullptr);
+  k_scatter<<<(unsigned)nfin, FIN_THREADS, 0, st>>>(d_sched, keys, E, cnt, (CandOut *)d_cands, cand_capacity, nullptr, 0.f, nullptr, d_ncand);
   return cuda_ok(cudaGetLastError()) ? VOLKS_OK : VOLKS_ECUDA;
 }
