@@ -414,8 +414,7 @@ def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traff
         # width's k_allif reads them once.  Roofline of the dominant kernel against measured HBM bandwidth.
         peaks_json = os.path.join(ROOT, "MEASURED_PEAKS.json")
         hbm = json.load(open(peaks_json))["hbm_gbs"] if os.path.exists(peaks_json) else 6650.0
-        pitch = plan.nf + 16 if plan.nf <= 8192 else plan.nf      # the plan's Y row pitch (sub-rows are contiguous)
-        ybytes = nbl * nap * pitch * 8.0
+        ybytes = nbl * nap * plan.nf * 8.0                        # the band's delay spectra (row padding is never touched)
         dom_bytes = (ybytes + nvis * 8.0 if dom[0] == 1 else ybytes) / nlaunch[dom]
         gbs = dom_bytes / (dom_ms_avg * 1e-3) / 1e9
         base["roofline"] = {
@@ -430,8 +429,7 @@ def measure(vk, args, cfg_id, dev, local, rank, dist, steps, warmup, peak, traff
         # are bandwidth work: roofline against the measured HBM copy bandwidth
         peaks_json = os.path.join(ROOT, "MEASURED_PEAKS.json")
         hbm = json.load(open(peaks_json))["hbm_gbs"] if os.path.exists(peaks_json) else 6650.0
-        pitch = c["nf"] + 16 if c["nf"] >= 32 else c["nf"]                # the plan's Y row pitch (default y_pad)
-        ybytes = nbl * nif * nap * pitch * 8.0
+        ybytes = nbl * nif * nap * c["nf"] * 8.0                          # the Nf columns of a row (its padding is never touched)
         dom_bytes = (ybytes + nvis * 8.0 + nbl * nif * nap * 4.0 if dom[0] == 1 else ybytes) / nlaunch[dom]
         gbs = dom_bytes / (dom_ms_avg * 1e-3) / 1e9
         tr = traffic.get((c["id"], KIND_NAMES.get(dom[0], ""), -1))
