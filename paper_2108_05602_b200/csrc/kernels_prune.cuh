@@ -212,11 +212,11 @@ __global__ void __launch_bounds__(NTHR) k_bound(PruneArgs a) {
 // pre-threshold 5.94 sqrt(P0) (P0 = the mean bin power): 5.2 deviations, where the plain amplitude sum of k_bound has 2.0 and
 // lets 2 - 3 % of the (window, column) pairs through to k_coleval.  A candidate's bin exceeds the pre-threshold, so its
 // column's bit is set (exactness as for k_bound); the bits and the per-tile density bytes have k_bound's format.
-//   CTA = (pair, 256 window starts), thread = column pair; per row: one 128-bit load (eight rows in flight), the row 16
+//   CTA = (pair, 512 window starts), thread = column pair; per row: one 128-bit load (eight rows in flight), the row 16
 //   back from registers (the loop is unrolled 16 times), four packed complex add/subtracts, four packed |.|^2, eight square roots, the four
 //   amplitudes 16 rows back from a shared-memory ring, e_rho += A_new - A_old, the largest e per column, its square against the
 //   window's pre-threshold by a sign-bit shift register (as in k_bound).
-constexpr int PF_T = 256;          // window starts per CTA (two tiles of k_coleval)
+constexpr int PF_T = 512;          // window starts per CTA (four tiles of k_coleval: 31 halo rows per 512)
 constexpr int PF_W = 32;           // the width this kernel is for (Nt = 64)
 constexpr int PF_THREADS = 128;
 
@@ -237,7 +237,8 @@ __host__ __device__ inline size_t pairfold_smem_bytes() {
 __global__ void __launch_bounds__(PF_THREADS) k_pairfold(PairFoldArgs a) {
   extern __shared__ float4 pf_sm4[];
   float *thr_sm = (float *)pf_sm4;                             // [PF_T + 64]: entry r = pre-threshold of the window ENDING at row r
-  __shared__ int cwtotal[2];
+  constexpr int NT128 = PF_T / 128;                            // k_coleval tiles per CTA
+  __shared__ int cwtotal[NT128];
   const int ntile = (a.nwin + PF_T - 1) / PF_T;
   const long long pl = blockIdx.x / ntile;
   const int tile = (int)(blockIdx.x % ntile);
@@ -246,7 +247,7 @@ __global__ void __launch_bounds__(PF_THREADS) k_pairfold(PairFoldArgs a) {
     const int j = i - PF_W + 1;
     thr_sm[i] = (j >= 0 && j < PF_T && R0 + j < a.nwin) ? __uint_as_float(__ldg(a.thr + pl * a.per_pair + a.offc + R0 + j)) : 3.0e38f;
   }
-  if (threadIdx.x < 2) cwtotal[threadIdx.x] = 0;
+  if (threadIdx.x < NT128) cwtotal[threadIdx.x] = 0;
   const int nrows = min(PF_T + PF_W - 1, a.nap - R0);
   const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch);
   const size_t rowb = (size_t)a.pitch * 8u;
@@ -254,7 +255,9 @@ __global__ void __launch_bounds__(PF_THREADS) k_pairfold(PairFoldArgs a) {
   char *amp = (char *)(thr_sm + PF_T + 64) + threadIdx.x * 8u;
   constexpr uint32_t AMPROW = PF_THREADS * 8, AMPRHO = 16 * AMPROW;
   __syncthreads();
-  int cnt0 = 0, cnt1 = 0;                                      // set bits of the two 128-window halves
+  int cnt[NT128];                                              // set bits per tile of 128 windows
+#pragma unroll
+  for (int i = 0; i < NT128; ++i) cnt[i] = 0;
   for (int ci = threadIdx.x; ci < a.ncp; ci += PF_THREADS) {
     const int c = ci < a.cp_na ? a.cp_a0 + ci : a.cp_b0 + (ci - a.cp_na);
     for (int k = 0; k < 64; ++k) *(f32x2 *)(amp + (uint32_t)k * AMPROW) = pk(0.f, 0.f);
@@ -313,7 +316,8 @@ __global__ void __launch_bounds__(PF_THREADS) k_pairfold(PairFoldArgs a) {
           if (--cwn == 0) {
             const uint32_t wa = __brev(cwa), wb = __brev(cwb);
             const int n = __popc(wa) + __popc(wb);
-            if (nword < 4) cnt0 += n; else cnt1 += n;
+#pragma unroll
+            for (int i = 0; i < NT128; ++i) cnt[i] += (nword >> 2) == i ? n : 0;
             if (wa | wb) *(uint2 *)cwp = make_uint2(wa, wb);
             cwp += a.nf; ++nword;
             cwn = 32;
@@ -324,16 +328,20 @@ __global__ void __launch_bounds__(PF_THREADS) k_pairfold(PairFoldArgs a) {
     if (cwn < 32) {                                            // the last, incomplete word
       const uint32_t wa = __brev(cwa) >> cwn, wb = __brev(cwb) >> cwn;
       const int n = __popc(wa) + __popc(wb);
-      if (nword < 4) cnt0 += n; else cnt1 += n;
+#pragma unroll
+      for (int i = 0; i < NT128; ++i) cnt[i] += (nword >> 2) == i ? n : 0;
       if (wa | wb) *(uint2 *)cwp = make_uint2(wa, wb);
     }
   }
 #pragma unroll
-  for (int o = 16; o >= 1; o >>= 1) { cnt0 += __shfl_xor_sync(0xffffffffu, cnt0, o); cnt1 += __shfl_xor_sync(0xffffffffu, cnt1, o); }
-  if ((threadIdx.x & 31) == 0) { if (cnt0) atomicAdd(&cwtotal[0], cnt0); if (cnt1) atomicAdd(&cwtotal[1], cnt1); }
+  for (int i = 0; i < NT128; ++i) {
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) cnt[i] += __shfl_xor_sync(0xffffffffu, cnt[i], o);
+    if ((threadIdx.x & 31) == 0 && cnt[i]) atomicAdd(&cwtotal[i], cnt[i]);
+  }
   __syncthreads();
-  if (threadIdx.x < 2 && 2 * tile + (int)threadIdx.x < a.ntile128)   // dense: more than 1/8 of the 128 x columns bits (k_bound's rule)
-    a.cwdense[pl * a.ntile128 + 2 * tile + threadIdx.x] = (unsigned char)((long long)cwtotal[threadIdx.x] * 8 > 128LL * 2 * a.ncp ? 1 : 0);
+  if (threadIdx.x < NT128 && NT128 * tile + (int)threadIdx.x < a.ntile128)   // dense: more than 1/8 of the 128 x columns bits (k_bound's rule)
+    a.cwdense[pl * a.ntile128 + NT128 * tile + threadIdx.x] = (unsigned char)((long long)cwtotal[threadIdx.x] * 8 > 128LL * 2 * a.ncp ? 1 : 0);
 }
 
 }  // namespace volks
