@@ -749,7 +749,8 @@ def test_folded_column_bound_every_residue(vb, oracle):
     for ch in (7, 50):
         vis[0, 1, :, ch] += (30.0 * torch.exp(2j * np.pi * 0.003 * t)).to(torch.complex64)
     cc = dict(c, widths=[32, 64], strides=[1, 1], nts=[64, 128])
-    for opts in (None, dict(full_index=1)):
+    # (prune_seg = 128 switches the column-level rule off: w = 32 then runs on the folded sliding sum with M = 4 residues)
+    for opts in (None, dict(full_index=1), dict(prune_seg=128)):
         stats, ncand, cands, ora = run_both(vb, oracle, vis, cc, options=opts)
         got = {(int(x["bl"]), int(x["ifq"]), int(x["wid"])) for x in cands}
         assert {(0, 1, 0), (1, 0, 0), (1, 1, 0)} <= got                 # the tones' pair and both pulse pairs have w = 32 candidates
