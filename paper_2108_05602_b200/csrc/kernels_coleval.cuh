@@ -37,6 +37,7 @@ struct ColEvalArgs {
   const uint32_t *mask;   // k_bound's bits: mask[(pl * nwords + window / 32) * nf + column]
   const uint32_t *thr;    // pre-thresholds (float bits), chunk-relative: thr[pl * per_pair + offc + t0]
   const unsigned char *dense;   // k_bound: dense[pl * dstride + tile] = 1: the sliding kernel evaluates this tile, not this kernel
+  const unsigned char *empty;   // ... empty[pl * dstride + tile] = 1: no bit of the tile is set (nothing to list: most tiles)
   const float2 *twt;      // [nt] rate twiddles exp(-2 pi i k/nt)
   long long per_pair, offc, pair0;
   int nap, nf, pitch, w, nt, log2m, nwin, nwords, dstride;   // dstride: tiles per pair in `dense` (k_bound's count)
@@ -55,7 +56,7 @@ __global__ void __launch_bounds__(CE_THREADS, 2) k_coleval(ColEvalArgs a) {
   const int ntile = (a.nwin + CE_TILE - 1) / CE_TILE;
   const long long pl = blockIdx.x / ntile;
   const int tile = (int)(blockIdx.x % ntile);
-  if (a.dense[pl * a.dstride + tile]) return;
+  if (a.dense[pl * a.dstride + tile] || a.empty[pl * a.dstride + tile]) return;
   const int J0 = tile * CE_TILE;
   const int M = 1 << a.log2m, ntm = a.nt - 1;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;

@@ -43,6 +43,7 @@ struct PruneArgs {
   // ... and one byte per (pair, tile): 1 = more than 1/8 of the tile's (window, column) bits are set (interference,
   // a strong source): the sliding kernel evaluates that tile (it is cheaper there), k_coleval skips it
   unsigned char *cwdense;
+  unsigned char *cwempty; // ... and 1 = no bit of the tile is set: k_coleval has nothing to list there
 };
 
 constexpr int PRUNE_MIRROR = 4;    // ring rows 0..3 are stored a second time behind the last: 4 consecutive rows never wrap
@@ -194,8 +195,10 @@ __global__ void __launch_bounds__(NTHR) k_bound(PruneArgs a) {
     if ((threadIdx.x & 31) == 0 && cwcount) atomicAdd(&cwtotal, cwcount);
   }
   __syncthreads();
-  if (NCW == 1 && threadIdx.x == 0)
+  if (NCW == 1 && threadIdx.x == 0) {
     a.cwdense[pl * ntile + tile] = (unsigned char)((long long)cwtotal * 8 > (long long)T * 2 * a.ncp ? 1 : 0);
+    a.cwempty[pl * ntile + tile] = (unsigned char)(cwtotal == 0 ? 1 : 0);
+  }
   if (threadIdx.x < NQ * 2) {
     const int q = threadIdx.x >> 1, h = threadIdx.x & 1, sg = 2 * tile + h;
     if (sg < a.nseg) a.flags[(pl * NQ + q) * a.nseg + sg] = (unsigned char)any[q][h];
@@ -225,6 +228,7 @@ struct PairFoldArgs {
   const uint32_t *thr;    // pre-thresholds (float bits): thr[pl * per_pair + offc + t0]
   uint32_t *cwmask;       // [(pl * cw_nwords + window / 32) * nf + column], zeroed before the launch
   unsigned char *cwdense; // [pl * ntile128 + tile of 128 windows]
+  unsigned char *cwempty; // same index: 1 = no bit of the tile is set
   long long per_pair, offc;
   int nap, nf, pitch, nwin, cw_nwords, ntile128;
   int ncp, cp_na, cp_a0, cp_b0;   // column pairs to look at (restricted delay range), as in PruneArgs
@@ -340,8 +344,10 @@ __global__ void __launch_bounds__(PF_THREADS) k_pairfold(PairFoldArgs a) {
     if ((threadIdx.x & 31) == 0 && cnt[i]) atomicAdd(&cwtotal[i], cnt[i]);
   }
   __syncthreads();
-  if (threadIdx.x < NT128 && NT128 * tile + (int)threadIdx.x < a.ntile128)   // dense: more than 1/8 of the 128 x columns bits (k_bound's rule)
+  if (threadIdx.x < NT128 && NT128 * tile + (int)threadIdx.x < a.ntile128) {   // dense: more than 1/8 of the 128 x columns bits (k_bound's rule)
     a.cwdense[pl * a.ntile128 + NT128 * tile + threadIdx.x] = (unsigned char)((long long)cwtotal[threadIdx.x] * 8 > 128LL * 2 * a.ncp ? 1 : 0);
+    a.cwempty[pl * a.ntile128 + NT128 * tile + threadIdx.x] = (unsigned char)(cwtotal[threadIdx.x] == 0 ? 1 : 0);
+  }
 }
 
 }  // namespace volks

@@ -588,7 +588,8 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
   // the column-level width's bits: k_bound's tiles are 2 prune_seg windows, a multiple of 32
   pl->cw_pf = pl->cwq >= 0 && pl->wp[pl->cwq].w == PF_W && pl->wp[pl->cwq].nt == 2 * PF_W && opt.prune_seg == 64;
   pl->cw_nwords = pl->cwq >= 0 ? (int)(((pl->prune_nseg + 1) / 2) * (2 * opt.prune_seg / 32)) : 0;
-  pl->off_cwdense = off; off = align_up(off + (size_t)pl->pairs_per_chunk * ((pl->prune_nseg + 1) / 2) + 1, 256);
+  // (twice: the density bytes, then one byte per tile "no bit set" for k_coleval)
+  pl->off_cwdense = off; off = align_up(off + 2 * (size_t)pl->pairs_per_chunk * ((pl->prune_nseg + 1) / 2) + 1, 256);
   pl->off_cwmask = off; off = align_up(off + (size_t)pl->pairs_per_chunk * pl->cw_nwords * p->nf * sizeof(uint32_t), 256);
   for (auto &w : pl->wp) {      // hit masks of the folded-sum widths: [pairs of the chunk][nblk][64-column groups][M] u16
     if (!w.sf || w.nwin == 0) { w.sf = false; continue; }
@@ -846,6 +847,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
           pa.nq = std::max(pa.nq, w.prune + 1); pa.wmax = std::max(pa.wmax, w.w);
         }
         pa.cwmask = nullptr; pa.cw_nwords = pl->cw_nwords; pa.cwdense = (unsigned char *)(ws + pl->off_cwdense);
+        pa.cwempty = pa.cwdense + (size_t)pl->pairs_per_chunk * ((pl->prune_nseg + 1) / 2);
         if (use_cw) {
           pa.cwmask = (uint32_t *)(ws + pl->off_cwmask);
           if (!cuda_ok(cudaMemsetAsync(pa.cwmask, 0, (size_t)np * pl->cw_nwords * s.nf * sizeof(uint32_t), st))) return VOLKS_ECUDA;
@@ -871,7 +873,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         if (use_cw && pl->cw_pf) {     // the column-level width's bits by the folded bound (same stream, same profile slot)
           const WidthPlan &w = pl->wp[pl->cwq];
           PairFoldArgs fa;
-          fa.Y = Y; fa.thr = ta.thr; fa.cwmask = pa.cwmask; fa.cwdense = pa.cwdense;
+          fa.Y = Y; fa.thr = ta.thr; fa.cwmask = pa.cwmask; fa.cwdense = pa.cwdense; fa.cwempty = pa.cwempty;
           fa.per_pair = s.per_pair; fa.offc = s.offc[pl->cwq];
           fa.nap = s.nap; fa.nf = s.nf; fa.pitch = pl->pitch; fa.nwin = (int)w.nwin; fa.cw_nwords = pl->cw_nwords;
           fa.ntile128 = (pl->prune_nseg + 1) / 2;
@@ -1022,6 +1024,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
       ea.per_pair = s.per_pair; ea.offc = s.offc[pl->cwq]; ea.pair0 = pair0;
       ea.nap = s.nap; ea.nf = s.nf; ea.pitch = pl->pitch; ea.w = w.w; ea.nt = w.nt; ea.log2m = w.log2m;
       ea.nwin = (int)w.nwin; ea.nwords = pl->cw_nwords; ea.dense = (const unsigned char *)(ws + pl->off_cwdense);
+      ea.empty = ea.dense + (size_t)pl->pairs_per_chunk * ((pl->prune_nseg + 1) / 2);
       ea.dstride = (pl->prune_nseg + 1) / 2; ea.only_above = hy ? 0 : 1;
       ProfScope ps(pl, st, VOLKS_K_COLEVAL, pl->cwq);
       k_coleval<<<(unsigned)(np * ((w.nwin + CE_TILE - 1) / CE_TILE)), CE_THREADS, 0, st>>>(ea);
