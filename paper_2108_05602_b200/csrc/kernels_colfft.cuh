@@ -35,6 +35,7 @@ struct ColFftArgs {
   // k_colfft2 SKIP (candidates-only mode): pre-threshold of every window of the chunk as float bits (k_winthr),
   // thr[pl * per_pair + offc + j]; nullptr = every (rate residue, column) is transformed
   const uint32_t *thr;
+  int energy_first;     // host side only: with thr, launch k_colfft2e (the energies before the sums) instead of k_colfft2<SKIP>
 };
 
 // L1 = Nt/16 (2..32), NZ = leading non-zero inputs of the L1-point transform (power of two <= L1).

@@ -266,4 +266,167 @@ __global__ void __launch_bounds__(CP * 32, CP == 8 ? CF2_MIN_CTAS8 : CP == 4 ? 2
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// k_colfft2e - the SKIP kernel with the energies first (candidates-only mode, 16-column strips).
+// ncu on configs[4] had k_colfft2<.., SKIP> bound by the shared-memory data path (75 % busy): every pass-1 sum S[rho][t2]
+// of a (window, strip) was written (16 B per column pair) and read back although the bound test only needs |S|^2.  Here a
+// pass-1 thread keeps its 16 sums in registers and stores their ENERGIES (8 B per column pair: half the traffic each way);
+// the pass-2 threads add the 16 energies of their (rho, column pair), test 16 sum |S|^2 against the window's
+// pre-threshold (the Cauchy-Schwarz bound of k_colfft2) and raise a flag for their parity half of the CTA.  Only if the
+// flag is up - a window that can hold a candidate in this strip: about one (window, strip) in a hundred - the sums
+// themselves are stored, a third barrier is taken and the flagged warps run pass 2 exactly as k_colfft2 does.
+#ifndef CF2_ENERGY_FIRST
+#define CF2_ENERGY_FIRST 1
+#endif
+constexpr uint32_t CF2E_RHO = 1024u + 32u;   // bytes between consecutive rho in E[rho][t2][pair]: the two residue groups a
+                                             // half warp reads (two rho apart) fall into different banks
+
+template <int L1, int NZ, int HB>
+__device__ __forceinline__ void cf2_pass1_keep(const f32x2 (&zx)[NZ], const f32x2 (&zy)[NZ], f32x2 (&X)[L1 / 2], f32x2 (&Y)[L1 / 2]) {
+  constexpr int H = L1 / 2;
+  constexpr int NZH = NZ < H ? NZ : H;
+  if constexpr (NZ <= H) {
+#pragma unroll
+    for (int k = 0; k < NZ; ++k) { X[k] = zx[k]; Y[k] = zy[k]; }
+  } else {
+#pragma unroll
+    for (int k = 0; k < H; ++k) {
+      X[k] = HB ? sub2(zx[k], zx[k + H]) : add2(zx[k], zx[k + H]);
+      Y[k] = HB ? sub2(zy[k], zy[k + H]) : add2(zy[k], zy[k + H]);
+    }
+  }
+  if constexpr (HB == 1) S2Twiddle<0, NZH, L1, H>::run(X, Y);
+  FftDifS<H, NZH, 0, H>::run(X, Y);          // output i is m = brev(i): rho = 2 m + HB
+}
+
+template <int L1, int NZ>
+__global__ void __launch_bounds__(256, CF2_MIN_CTAS8) k_colfft2e(ColFftArgs a) {
+  static_assert(L1 == 16 || L1 == 32, "Nt = 256 or 512");
+  constexpr int CP = 8, G = 32 / CP, NW = CP, H = L1 / 2;
+  extern __shared__ float4 cf_sm4[];
+  float4 *tw4s = cf_sm4;                                // as in k_colfft2
+  float4 *S4 = cf_sm4 + 512;                            // [L1][16][CP] (X, Y) of a column pair
+  u64 *slots = (u64 *)((char *)S4 + (size_t)L1 * cf2_rho_stride<CP>());
+  // the energy strip E[rho][t2][pair] behind the slots (not inside S: the two parity halves run windows apart, one may
+  // store sums while the other still reads energies)
+  const uint32_t ebase = (uint32_t)__cvta_generic_to_shared(slots + 16);
+  __shared__ int flag_sm[2][2];                         // [parity half][window parity]: some warp of the half passed the test
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int cp = lane & (CP - 1), hi = lane / CP;
+  const int ntile = a.nf / (2 * CP);
+  long long u = blockIdx.x;
+  const int rg = (int)(u % a.nrange); u /= a.nrange;
+  const int tile = (int)(u % ntile);
+  const long long pl = u / ntile;
+  const uint32_t rowb = (uint32_t)a.pitch * 8u;
+  const char *ybase = (const char *)(a.Y + (size_t)pl * a.nap * a.pitch) + (size_t)(tile * CP + cp) * 16u;
+  u64 *keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc);
+  for (int i = threadIdx.x; i < 512; i += NW * 32) {
+    const int wi = i / (16 * G);
+    const uint32_t r = (uint32_t)(2 * (G * (wi >> 1) + i % G) + (wi & 1)), k = (uint32_t)((i / G) & 15);
+    tw4s[i] = a.tw4[(r * k) & ((uint32_t)a.nt - 1u)];
+  }
+  if (threadIdx.x < 4) ((int *)flag_sm)[threadIdx.x] = 0;
+  const int j0 = rg * a.wpc, j1 = min(a.nwin, j0 + a.wpc);
+  __syncthreads();
+  const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(S4);
+  const uint32_t twsrc = (uint32_t)__cvta_generic_to_shared(tw4s) + (uint32_t)(warp * 16 * G + hi) * 16u;
+  const int hb = warp & 1, t2 = G * (warp >> 1) + hi;
+  const uint32_t sdst = sbase + (uint32_t)(t2 * CP + cp) * 16u;
+  const uint32_t edst = ebase + (uint32_t)(t2 * CP + cp) * 8u;
+  const uint32_t rho = (uint32_t)(2 * (G * (warp >> 1) + hi) + hb);
+  const bool p2_active = (warp >> 1) < L1 / (2 * G);
+  auto half_barrier = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(1 + hb), "r"(NW * 16) : "memory"); };
+  const uint32_t ssrc = sbase + rho * cf2_rho_stride<CP>() + (uint32_t)cp * 16u;
+  const uint32_t esrc = ebase + rho * CF2E_RHO + (uint32_t)cp * 8u;
+  constexpr bool PREFETCH = NZ <= 8;                    // (as k_colfft2: NZ = 16 would spill)
+
+  f32x2 zx[NZ], zy[NZ];
+  auto load_window = [&](int j) {
+    const size_t t0 = (size_t)j * a.stride;
+#pragma unroll
+    for (int t1 = 0; t1 < NZ; ++t1) {
+      const int t = t2 + 16 * t1;
+      if (j < j1 && t < a.w) ldg2(ybase + (t0 + t) * rowb, zx[t1], zy[t1]);
+      else { zx[t1] = pk(0.f, 0.f); zy[t1] = pk(0.f, 0.f); }
+    }
+  };
+  if constexpr (PREFETCH) load_window(j0);
+
+  for (int j = j0; j < j1; ++j) {
+    if constexpr (!PREFETCH) load_window(j);
+    f32x2 SX[H], SY[H];                                 // this thread's pass-1 sums: rho = 2 brev(i) + hb, its t2, its column pair
+    if (hb) cf2_pass1_keep<L1, NZ, 1>(zx, zy, SX, SY);
+    else cf2_pass1_keep<L1, NZ, 0>(zx, zy, SX, SY);
+#pragma unroll
+    for (int i = 0; i < H; ++i) {
+      const f32x2 en = fma2(SY[i], SY[i], mul2(SX[i], SX[i]));
+      asm volatile("st.shared.b64 [%0], %1;" ::"r"(edst + (uint32_t)(2 * brev<H>(i) + hb) * CF2E_RHO), "l"(en) : "memory");
+    }
+    if constexpr (PREFETCH) load_window(j + 1);         // in flight during the test
+    half_barrier();
+    bool go = false;
+    if (p2_active) {
+      const float thrj = __uint_as_float(__ldg(a.thr + pl * a.per_pair + a.offc + j));
+      f32x2 e = pk(0.f, 0.f);
+#pragma unroll
+      for (int k = 0; k < 16; ++k) {
+        f32x2 en;
+        asm volatile("ld.shared.b64 %0, [%1];" : "=l"(en) : "r"(esrc + (uint32_t)k * (8u * CP)));
+        e = add2(e, en);
+      }
+      go = __any_sync(0xffffffffu, 16.0016f * fmaxf(lo32(e), hi32(e)) > thrj);   // warp-uniform
+      if (go && lane == 0) flag_sm[hb][j & 1] = 1;
+    }
+    half_barrier();
+    const bool any = flag_sm[hb][j & 1] != 0;           // uniform in the half
+    if (warp == hb && lane == 0) flag_sm[hb][(j + 1) & 1] = 0;   // (last read before this window's first barrier)
+    if (!any) continue;                                 // no candidate possible in this strip: the window keeps its key
+#pragma unroll
+    for (int i = 0; i < H; ++i) cf2_sts(sdst + (uint32_t)(2 * brev<H>(i) + hb) * cf2_rho_stride<CP>(), SX[i], SY[i]);
+    half_barrier();
+    if (p2_active) {
+      if (go) {
+        f32x2 X[16], Y[16];
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+          f32x2 zx2, zy2, wx, wy;
+          cf2_lds(ssrc + (uint32_t)k * (16u * CP), zx2, zy2);
+          if (k == 0) { X[0] = zx2; Y[0] = zy2; continue; }   // W^0 = 1
+          cf2_lds(twsrc + (uint32_t)k * (16u * G), wx, wy);
+          X[k] = fma2(zx2, wx, mul2(zy2, neg2(wy)));
+          Y[k] = fma2(zx2, wy, mul2(zy2, wx));
+        }
+        FftDifS<16, 16, 0, 16>::run(X, Y);
+        uint32_t ba = 0, bb = 0;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          const f32x2 pw = fma2(Y[i], Y[i], mul2(X[i], X[i]));
+          ba = max(ba, __float_as_uint(lo32(pw)));
+          bb = max(bb, __float_as_uint(hi32(pw)));
+        }
+        const bool colb = bb > ba;
+        const uint32_t best = colb ? bb : ba;
+        const uint32_t km = __reduce_max_sync(0xffffffffu, best);
+        const uint32_t tied = __ballot_sync(0xffffffffu, best == km);
+        if (lane == __ffs(tied) - 1)
+          slots[warp] = ((u64)km << 32) |
+                        (u64)(0xFFFFFFFFu - (0x80000000u | (rho * (uint32_t)a.nf + (uint32_t)(tile * 2 * CP + 2 * cp) + (colb ? 1u : 0u))));
+      } else if (lane == 0) {
+        slots[warp] = 0ull;
+      }
+    }
+    half_barrier();
+    if (warp == hb) {   // warps 0 and 1: the slots of their parity
+      u64 k = lane < L1 / (2 * G) && lane < NW / 2 ? slots[2 * lane + hb] : 0ull;
+#pragma unroll
+      for (int o = 8; o >= 1; o >>= 1) {
+        const u64 other = __shfl_xor_sync(0xffffffffu, k, o);
+        k = other > k ? other : k;
+      }
+      if (lane == 0) atomicMax(keyp + j, k);
+    }
+  }
+}
+
 }  // namespace volks

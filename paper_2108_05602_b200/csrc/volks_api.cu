@@ -74,19 +74,24 @@ static cudaError_t colfft_one(const ColFftArgs &a, unsigned blocks, cudaStream_t
     const bool cf2 = a.split2 != 0;
     // k_colfft2: 512 twiddles + the strip S[L1][16][CP] + 16 slots
     const size_t smem8 = 512 * sizeof(float4) + (size_t)L1 * 16 * 8 * sizeof(float4) + 16 * sizeof(u64);
+    const size_t smem8e = smem8 + (size_t)L1 * CF2E_RHO;   // k_colfft2e: + the energy strip
     const size_t smem4 = 512 * sizeof(float4) + (size_t)L1 * (256 * 4 + 32) + 16 * sizeof(u64);
     const size_t smem16 = 512 * sizeof(float4) + (size_t)L1 * 16 * 16 * sizeof(float4) + 16 * sizeof(u64);
     if (attr_only) {
       cudaError_t e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem16);
       if (e == cudaSuccess) e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem8);
       if (e == cudaSuccess) e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem8);
+      if (e == cudaSuccess) e = cudaFuncSetAttribute(k_colfft2e<L1, NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem8e);
       if (e == cudaSuccess) e = cudaFuncSetAttribute(k_colfft2<L1, NZ, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem4);
       if (e != cudaSuccess) return e;
     } else if (a.split2 == 4) {   // 8-column strips: four times the CTAs, 128 threads each
       k_colfft2<L1, NZ, 4><<<blocks * 4, 128, smem4, st>>>(a);
       return cudaSuccess;
     } else if (a.split2 == 2) {   // 16-column strips: twice the CTAs, 256 threads each
-      if (a.thr) k_colfft2<L1, NZ, 8, true><<<blocks * 2, 256, smem8, st>>>(a);   // candidates-only mode: pass 2 only where needed
+      // candidates-only mode: energies first (measured on configs[4]: w = 64 / 128 / 256 take 52.7 / 41.9 / 33.9 ms per step
+      // with it, 66.4 / 42.4 / 30.4 ms with k_colfft2<SKIP>: the widest windows keep the older kernel)
+      if (a.thr && a.energy_first && NZ <= 8) k_colfft2e<L1, NZ><<<blocks * 2, 256, smem8e, st>>>(a);
+      else if (a.thr) k_colfft2<L1, NZ, 8, true><<<blocks * 2, 256, smem8, st>>>(a);   // ... pass 2 only where needed
       else k_colfft2<L1, NZ, 8><<<blocks * 2, 256, smem8, st>>>(a);
       return cudaSuccess;
     } else if (cf2) {
@@ -963,6 +968,7 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
         fa.nap = s.nap; fa.nf = s.nf; fa.w = w.w; fa.stride = w.s; fa.nt = w.nt; fa.nwin = (int)w.nwin;
         fa.pitch = pl->pitch; fa.paired = pl->paired; fa.split2 = pl->cf_split2; fa.wpc = w.cf_wpc; fa.nrange = w.cf_nrange; fa.keymask = 0xFFFFFFF0u;
         fa.thr = hy && w.untag ? (const uint32_t *)(ws + pl->off_thr) : nullptr;
+        fa.energy_first = CF2_ENERGY_FIRST;
         ProfScope ps(pl, st, VOLKS_K_COLFFT, q);
         if (!cuda_ok(launch_colfft(fa, w.cf_l1, w.cf_nz, np * (s.nf / 32) * w.cf_nrange, st, false))) return VOLKS_ECUDA;
         continue;
