@@ -231,8 +231,10 @@ SLIDE_OPS_PER_BIN = 5.17
 COLFFT2_OPS_PER_COLUMN = {4: 11106.0, 8: 12718.0, 16: 14178.0}
 # k_colfft2 SKIP (the default candidates-only mode: pass 2 only where a candidate is possible; profiles/r02_counters.md,
 # configs[4]'s data): 2071 / 2884 / 3617 packed instructions per (window, column): pass 1 + the 32 FFMA2 of the bound
-COLFFT2_SKIP_FLOPS_PER_COLUMN = {4: 5900.0, 8: 7850.0, 16: 9560.0}
-COLFFT2_SKIP_OPS_PER_COLUMN = {4: 4142.0, 8: 5768.0, 16: 7234.0}
+# (w <= 64 / 128 now run k_colfft2e, which adds the energies of the pass-1 sums: 2328 / 3140 packed instructions per (window,
+# column), 257 / 256 of them the FMUL2 + FFMA2 of |S|^2 at 3 flops on average)
+COLFFT2_SKIP_FLOPS_PER_COLUMN = {4: 6670.0, 8: 8620.0, 16: 9560.0}
+COLFFT2_SKIP_OPS_PER_COLUMN = {4: 4656.0, 8: 6280.0, 16: 7234.0}
 COLFFT2_FLOPS_PER_COLUMN = {4: 13700.0, 8: 15600.0, 16: 17200.0}
 # k_slide<FOLD> (kind 14, the folded sliding sum of the candidates-only mode; profiles/r02_counters.md, configs[2] w = 64):
 # 5.111e10 FP32 thread-instructions per launch, 8.87e9 of them scalar (the FFMAs of the octagonal bound); the rest is half
