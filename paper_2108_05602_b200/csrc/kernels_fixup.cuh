@@ -78,10 +78,20 @@ __global__ void __launch_bounds__(256) k_fixup(FixArgs a) {
   int u = (int)(blockIdx.x % upp), i = 0;
   while (u >= a.unit0[i + 1]) ++i;
   const int sg_lo = (u - a.unit0[i]) * FIX_GROUP, sg_hi = min(a.nseg[i], sg_lo + FIX_GROUP);
+  // which of the unit's segments were evaluated at all: the 16 flag bytes in ONE round trip (thread per segment) - read
+  // one after the other by the whole CTA they were most of this kernel's time on a pruned search
+  __shared__ unsigned char todo[FIX_GROUP];
+  if (threadIdx.x < FIX_GROUP) {
+    const int sg = sg_lo + (int)threadIdx.x;
+    bool run = sg < sg_hi;
+    if (run && a.flags && a.flag_q[i] >= 0 && !a.flags[(pl * a.flag_nq + a.flag_q[i]) * a.flag_nseg + sg]) run = false;
+    if (run && a.cwdense && i == a.cw_i && !a.cwdense[pl * a.cw_ntile + sg]) run = false;
+    if (run && a.sfdense[i] && !a.sfdense[i][pl * a.nseg[i] + sg]) run = false;
+    todo[threadIdx.x] = run ? 1 : 0;
+  }
+  __syncthreads();
   for (int sg = sg_lo; sg < sg_hi; ++sg) {
-  if (a.flags && a.flag_q[i] >= 0 && !a.flags[(pl * a.flag_nq + a.flag_q[i]) * a.flag_nseg + sg]) continue;
-  if (a.cwdense && i == a.cw_i && !a.cwdense[pl * a.cw_ntile + sg]) continue;
-  if (a.sfdense[i] && !a.sfdense[i][pl * a.nseg[i] + sg]) continue;
+  if (!todo[sg - sg_lo]) continue;
   const int w = a.w[i], nt = a.nt[i], seg = a.seg[i];
   const int j0 = sg * seg, n = min(seg, a.nwin[i] - j0);          // windows j0 .. j0+n-1 (seg <= 256? see below)
   u64 *keyp = a.keys + ((a.pair0 + pl) * a.per_pair + a.offc[i]);
