@@ -215,6 +215,26 @@ def test_capacity_overflow_and_determinism(vb):
     assert nz == na and len(z) == 0
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg,over", [
+    (2, dict(nbl=2, nif=2, nap=3000, npulses=6)),    # pruned widths, k_pairfold + k_coleval, the folded sliding sum + its list
+    (3, dict(nbl=2, nif=2, nap=4000, npulses=6)),    # k_row128, all widths pruned
+    (4, dict(nbl=1, nif=2, nap=2500, npulses=3)),    # k_colfft2e (flags between the parity halves), k_colfft2<SKIP>
+])
+def test_candidates_only_mode_is_deterministic(vb, cfg, over):
+    """The candidates-only search (atomics into lists and flags, independently running CTA halves) must give the same
+    bytes run after run: five searches of one plan and a fresh plan, threshold 6 (every bound active)."""
+    vis, c, _ = workloads.generate(cfg, **over)
+    v = vis.cuda()
+    ref = None
+    for _ in range(6):
+        a, na, _ = vb.fringe_search(v, c["widths"], c["strides"], c["nts"], c["nf"], c["snr_thresh"])
+        assert na == len(a) and na > 0
+        if ref is None:
+            ref = a.tobytes()
+        assert a.tobytes() == ref
+
+
 def test_peaks_optional_same_candidates(vb):
     vis, c, _ = workloads.generate(0)
     a, na, _ = vb.fringe_search(vis.cuda(), c["widths"], c["strides"], c["nts"], c["nf"], 6.0, want_peaks=False)
