@@ -39,14 +39,28 @@ namespace volks {
 #define SFOLD_SEGMUL 4            // segment of k_slide<FOLD> = this many segments of the sliding kernel
 #endif
 
+// Dynamic range.  The fold kernel's running sums keep about 2^-23 x 2 x 64 steps of relative rounding of the LARGEST value
+// they held; when a row of overwhelming energy leaves the window, that residue stays behind at its absolute size and can
+// exceed the 1e-3 margin of the amplitude threshold.  nf * E[t] bounds |Y[t][d]|^2 of every column of row t: where it
+// exceeds FOLD_BIG x the power pre-threshold of the window starting there (amplitude ratio 64), k_sfold_guard flags every
+// window from that block to the end of the fold segment (evaluated exactly from their samples by k_sfold_eval, which for
+// its part re-folds after such a row instead of sliding across it).
+#ifndef FOLD_BIG
+#define FOLD_BIG 4096.0f
+#endif
+
 constexpr int SFOLD_EVAL_WARPS = 148 * 8;   // k_sfold_eval's grid: one-warp CTAs, 8 resident per SM at 248 registers
 
 struct SfoldArgs {
   const float2 *Y;       // [pairs of the chunk][nap][pitch] pair-interleaved delay spectra
   const float4 *tw4;     // [nt] rate twiddles exp(-2 pi i k/nt), pre-broadcast (re, re, im, im)
   const unsigned short *hits;   // [pairs of the chunk][nblk][ndt][M] hit masks of k_slide<FOLD>: bit B = window 16 blk + B
+  unsigned short *hits_rw;      // the same array for k_sfold_guard
+  unsigned short *big16;        // [pairs of the chunk][nblk]: bit i = row 16 blk + i has overwhelming energy (k_sfold_guard)
   unsigned char *dense;  // [pairs of the chunk][nseg]
   uint32_t *list;        // [0] = number of entries, then the indices of the non-zero mask words of the sparse segments
+  const uint32_t *thr;   // pre-thresholds (float bits), chunk-relative: thr[pl * per_pair + offc + t0]
+  const float *E;        // per-AP energies of the chunk's pairs: E[pl * nap + t] (FOLD_BIG, kernels_slide.cuh)
   u64 *keys;             // canonical window keys
   long long ntasks;      // k_sfold_eval: warps = pairs * nblk * ndt * M;  k_sfold_density: CTAs = pairs * nseg
   long long per_pair, offc, pair0;
@@ -70,6 +84,40 @@ __global__ void __launch_bounds__(128) k_sfold_density(SfoldArgs a) {
   __syncthreads();
   if (threadIdx.x == 0) a.dense[pl * a.nseg + sg] = (unsigned char)((part[0] + part[1] + part[2] + part[3]) * 8 > nwords * 16 ? 1 : 0);
   if (blockIdx.x == 0 && threadIdx.x == 0) a.list[0] = 0;   // (k_sfold_compact follows on the same stream)
+}
+
+// one CTA per (pair, fold segment of `fseg` windows): the first block of 16 windows in which a row of overwhelming energy
+// leaves; from there to the end of the segment every mask word becomes "all windows" (rare: most CTAs only read)
+__global__ void __launch_bounds__(128) k_sfold_guard(SfoldArgs a, int fseg) {
+  __shared__ int firstblk;
+  const int nfseg = (a.nwin + fseg - 1) / fseg;
+  const long long pl = blockIdx.x / nfseg;
+  const int fs = (int)(blockIdx.x % nfseg);
+  const int t0 = fs * fseg, t1 = min(a.nwin, t0 + fseg);
+  if (threadIdx.x == 0) firstblk = 0x7fffffff;
+  __syncthreads();
+  const uint32_t *thrp = a.thr + (pl * a.per_pair + a.offc);
+  const float *ep = a.E + pl * a.nap;
+  int mine = 0x7fffffff;
+  for (int tb = t0; tb < t1; tb += 128) {                   // (t0 is a multiple of 16: a warp covers two blocks of 16 rows)
+    const int t = tb + (int)threadIdx.x;
+    const bool big = t < t1 && (float)a.nf * __ldg(ep + t) > FOLD_BIG * __uint_as_float(__ldg(thrp + t));
+    if (big) mine = min(mine, t >> 4);
+    const uint32_t m = __ballot_sync(0xffffffffu, big);     // one 16-bit word per block for k_sfold_eval: bit i = row 16 blk + i
+    if ((threadIdx.x & 15) == 0 && t < t1) a.big16[(size_t)pl * a.nblk + (t >> 4)] = (unsigned short)((m >> (threadIdx.x & 16)) & 0xFFFFu);
+  }
+  if (mine != 0x7fffffff) atomicMin(&firstblk, mine);
+  __syncthreads();
+  const int fb = firstblk;
+  if (fb == 0x7fffffff) return;
+  const int wps = a.ndt << a.log2m;                         // words per block of 16 windows
+  const int b1 = (t1 + 15) >> 4;
+  unsigned short *h = a.hits_rw + ((size_t)pl * a.nblk) * wps;
+  for (int i = threadIdx.x; i < (b1 - fb) * wps; i += 128) {
+    const int blk = fb + i / wps;
+    const int nvalid = min(16, a.nwin - blk * 16);
+    h[(size_t)blk * wps + i % wps] = (unsigned short)((1u << nvalid) - 1u);
+  }
 }
 
 // the non-zero mask words of the segments the sliding kernel does not take, as a list (order: whatever the atomics give -
@@ -101,6 +149,7 @@ __global__ void __launch_bounds__(32) k_sfold_eval(SfoldArgs a) {
   for (uint32_t li = blockIdx.x; li < nlist; li += gridDim.x) {
   long long wt = (long long)a.list[1 + li];
   const uint32_t mask = a.hits[wt];
+  const uint32_t bigmask = a.big16[((wt >> a.log2m) / a.ndt)];         // (pair * nblk + block): rows of overwhelming energy
   const uint32_t rho = (uint32_t)(wt & (M - 1)); wt >>= a.log2m;
   const int dti = (int)(wt % a.ndt); wt /= a.ndt;
   const int dt = dti < a.dt_na ? a.dt_a0 + dti : a.dt_b0 + (dti - a.dt_na);
@@ -119,10 +168,9 @@ __global__ void __launch_bounds__(32) k_sfold_eval(SfoldArgs a) {
   const float sg1 = (rho & 1u) ? -1.f : 1.f;
   const f32x2 sgn2 = pk(sg1, sg1);
   f32x2 X[16], Yv[16];
+  auto fold_at = [&](uint32_t t0) {                                    // the folded sums of window t0 from its w samples
 #pragma unroll
-  for (int k = 0; k < 16; ++k) { X[k] = pk(0.f, 0.f); Yv[k] = pk(0.f, 0.f); }
-  {
-    const uint32_t t0 = blk * 16u + (uint32_t)first;
+    for (int k = 0; k < 16; ++k) { X[k] = pk(0.f, 0.f); Yv[k] = pk(0.f, 0.f); }
     for (uint32_t tb = 0; tb < (uint32_t)a.w; tb += 16) {
 #pragma unroll
       for (int k = 0; k < 16; ++k) {
@@ -133,10 +181,13 @@ __global__ void __launch_bounds__(32) k_sfold_eval(SfoldArgs a) {
         Yv[k] = fma2(yx, twy, fma2(yy, twx, Yv[k]));
       }
     }
-  }
+  };
+  fold_at(blk * 16u + (uint32_t)first);
+  bool stale = false;                                                  // a row of overwhelming energy has left since the last fold
   for (int b = first;; ++b) {
     const uint32_t t = blk * 16u + (uint32_t)b;
     if ((mask >> b) & 1u) {
+      if (stale) { fold_at(t); stale = false; }                        // (its rounding residue would sit in the slid sums)
       f32x2 GX[16], GY[16];
 #pragma unroll
       for (int k = 0; k < 16; ++k) { GX[k] = X[k]; GY[k] = Yv[k]; }
@@ -160,6 +211,7 @@ __global__ void __launch_bounds__(32) k_sfold_eval(SfoldArgs a) {
     }
     if (b == last) break;
     // window t -> t + 1: sample t leaves, sample t + w enters, both of the class now at index 0
+    stale = stale || ((bigmask >> b) & 1u);                            // (warp-uniform)
     f32x2 xin, yin, xout, yout, twx, twy;
     ldg2(ybase + (size_t)(t + a.w) * rowb, xin, yin);
     ldg2(ybase + (size_t)t * rowb, xout, yout);

@@ -55,6 +55,7 @@ struct WidthPlan {
   size_t off_hits;      // ... its hit masks in the workspace
   size_t off_sfdense;   // ... its per-segment density flags
   size_t off_sflist;    // ... the list of non-zero mask words (count first)
+  size_t off_sfbig;     // ... one 16-bit word per block of 16 rows: rows of overwhelming energy (k_sfold_guard)
   int nblk;             // ... blocks of 16 windows per pair
 };
 
@@ -603,6 +604,8 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
     off = align_up(off + (size_t)pl->pairs_per_chunk * w.nblk * pl->dt_n * (1 << w.log2m) * sizeof(unsigned short), 256);
     w.off_sfdense = off;
     off = align_up(off + (size_t)pl->pairs_per_chunk * w.nseg, 256);
+    w.off_sfbig = off;
+    off = align_up(off + (size_t)pl->pairs_per_chunk * w.nblk * sizeof(unsigned short), 256);
     w.off_sflist = off;
     off = align_up(off + (1 + (size_t)pl->pairs_per_chunk * w.nblk * pl->dt_n * (1 << w.log2m)) * sizeof(uint32_t), 256);
   }
@@ -617,7 +620,7 @@ static int plan_create_impl(const volks_params *p, const volks_options *o, volks
   for (int q = 0; q < p->nwidths; ++q) active += (pl->wp[q].nwin > 0 && q != pl->wid1) ? 1 : 0;
   // kernels of this library per search (the key memset is a driver memset, not counted)
   // (a search without dense peaks; with them the candidates-only index mode and its k_winthr launch are off)
-  pl->launches = s.nwin_total > 0 ? (int)(pl->nchunks * (1 + active + (pl->nslide > 0 ? 1 : 0) + ((pl->cand_only && (pl->nuntag || pl->nprune)) ? 1 : 0) + ((pl->nprune || (pl->cwq >= 0 && !pl->cw_pf)) ? 1 : 0) + (pl->cw_pf ? 1 : 0) + (pl->nuntag ? 1 : 0) + (pl->cwq >= 0 ? 1 : 0) + 4 * pl->nsf) + 3) : 0;
+  pl->launches = s.nwin_total > 0 ? (int)(pl->nchunks * (1 + active + (pl->nslide > 0 ? 1 : 0) + ((pl->cand_only && (pl->nuntag || pl->nprune)) ? 1 : 0) + ((pl->nprune || (pl->cwq >= 0 && !pl->cw_pf)) ? 1 : 0) + (pl->cw_pf ? 1 : 0) + (pl->nuntag ? 1 : 0) + (pl->cwq >= 0 ? 1 : 0) + 5 * pl->nsf) + 3) : 0;
 
   // tables, computed in double precision on the host
   if (psub > 1) { pl->premod_off = tw_total; tw_total += (size_t)s.nf; }
@@ -942,6 +945,8 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
           // 2. segments with more than 1/8 of their bits set (interference) go to the ordinary sliding kernel
           SfoldArgs ea;
           ea.Y = Y; ea.tw4 = (const float4 *)(pl->d_tables + w.tw4_off); ea.hits = sa.hits; ea.dense = (unsigned char *)(ws + w.off_sfdense); ea.list = (uint32_t *)(ws + w.off_sflist); ea.keys = keys;
+          ea.thr = sa.thr; ea.E = E + pair0 * (long long)s.nap; ea.hits_rw = (unsigned short *)(ws + w.off_hits);
+          ea.big16 = (unsigned short *)(ws + w.off_sfbig);
           ea.per_pair = s.per_pair; ea.offc = s.offc[q]; ea.pair0 = pair0;
           ea.nap = s.nap; ea.nf = s.nf; ea.w = w.w; ea.nt = w.nt; ea.log2m = w.log2m; ea.nwin = (int)w.nwin;
           ea.seg = w.seg; ea.nseg = w.nseg; ea.pitch = pl->pitch; ea.nblk = w.nblk;
@@ -949,6 +954,10 @@ static int run_search(const volks_plan *pl, const void *d_vis, void *d_stage, co
           ea.ntasks = np * w.nseg;
           {
             ProfScope ps(pl, st, VOLKS_K_SFOLD_EVAL, q);
+            {   // dynamic-range guard: windows behind a row of overwhelming energy are flagged wholesale
+              const int fseg = w.seg * SFOLD_SEGMUL;
+              k_sfold_guard<<<(unsigned)(np * ((w.nwin + fseg - 1) / fseg)), 128, 0, st>>>(ea, fseg);
+            }
             k_sfold_density<<<(unsigned)ea.ntasks, 128, 0, st>>>(ea);
             // 3. every other flagged (window, rho, tile) exactly, from its samples
             ea.ntasks = ((np * w.nblk * (long long)pl->dt_n) << w.log2m);

@@ -537,7 +537,15 @@ def test_dynamic_range_after_strong_samples(vb, oracle):
     vis[0, :, 100:104] *= 3000.0
     vis[0, 0, 300:500] = 0
     vis[0, 0, 400, 7] = 0.3 + 0.1j
-    run_both(vb, oracle, vis, c)
+    # a threshold-level 64-AP pulse whose windows start right after the burst has left them (window 104 on): the folded
+    # sliding sum (candidates-only mode) must not test them with sums that still carry the burst's rounding residue
+    nchan = vis.shape[3]
+    k = torch.arange(nchan, dtype=torch.float64)
+    ph = torch.polar(torch.full((nchan,), 7.5 / np.sqrt(64 * nchan), dtype=torch.float64), 2 * np.pi * 5.0 * k / nchan)
+    vis[0, 1, 106:170] += ph.to(torch.complex64)
+    stats, ncand, cands, ora = run_both(vb, oracle, vis, c)
+    w64 = cands[(cands["wid"] == len(c["widths"]) - 1) & (cands["ifq"] == 1)]
+    assert np.any((w64["t0"] >= 104) & (w64["t0"] <= 112))       # the pulse is found in the windows just behind the burst
     cands, n, peaks = vb.allif_search(vis.cuda(), c["widths"], c["strides"], 512, 4.0, want_peaks=True)
     ora = oracle.allif_search(vis.numpy(), c["widths"], c["strides"], 512)
     nw = [workloads.gen.nwin(vis.shape[2], w, s) for w, s in zip(c["widths"], c["strides"])]
