@@ -182,12 +182,13 @@ __global__ void __launch_bounds__(32) k_sfold_eval(SfoldArgs a) {
       }
     }
   };
-  fold_at(blk * 16u + (uint32_t)first);
-  bool stale = false;                                                  // a row of overwhelming energy has left since the last fold
+  // (ONE fold site: the first flagged window, and again at the next flagged window behind a row of overwhelming energy,
+  // whose rounding residue would sit in the slid sums)
+  bool stale = true;
   for (int b = first;; ++b) {
     const uint32_t t = blk * 16u + (uint32_t)b;
     if ((mask >> b) & 1u) {
-      if (stale) { fold_at(t); stale = false; }                        // (its rounding residue would sit in the slid sums)
+      if (stale) { fold_at(t); stale = false; }
       f32x2 GX[16], GY[16];
 #pragma unroll
       for (int k = 0; k < 16; ++k) { GX[k] = X[k]; GY[k] = Yv[k]; }
@@ -212,6 +213,7 @@ __global__ void __launch_bounds__(32) k_sfold_eval(SfoldArgs a) {
     if (b == last) break;
     // window t -> t + 1: sample t leaves, sample t + w enters, both of the class now at index 0
     stale = stale || ((bigmask >> b) & 1u);                            // (warp-uniform)
+    if (stale) continue;                                               // nothing worth sliding
     f32x2 xin, yin, xout, yout, twx, twy;
     ldg2(ybase + (size_t)(t + a.w) * rowb, xin, yin);
     ldg2(ybase + (size_t)t * rowb, xout, yout);
